@@ -1,0 +1,111 @@
+/*
+ * dp.h -- C ABI of the B200-native Deep Potential (smooth edition, se_a) evaluator.
+ *
+ * One call, dp_compute, evaluates energy, per-atom energy, forces and virial of a periodic system:
+ * the per-step "key function" of DeePMD-kit (section IV: "the calculation of atomic
+ * energies and forces predicted by the DP model") with the model structure of PAPER.md:51 (section
+ * III-B, Fig. 1), the neighbour-list layout of PAPER.md:109-119 (section V-B1/2), the Environment /
+ * ProdForce / ProdViral operators of PAPER.md:121 and the precision schemes of PAPER.md:125.
+ * Every formula the paper leaves to its references is the reading listed in DESIGN.md ("Readings").
+ *
+ * Conventions
+ *   - extern "C", plain pointers and sizes only.  "_dev" pointers are CUDA device pointers (caller
+ *     owned, e.g. torch tensors' data_ptr()); "_host" / unmarked struct members are host pointers.
+ *   - All functions return DP_OK (0) or a negative dp_error; nothing throws or aborts across the ABI.
+ *   - dp_compute only ENQUEUES work on the caller's CUDA stream: no host synchronisation, no allocation
+ *     (the paper's "trunk of GPU memory allocated at the initialisation stage", is the
+ *     caller-owned workspace).  Outputs are valid after the stream is synchronised.
+ *   - Units: Angstrom, eV, eV/Angstrom; virial in eV.  Outputs are fp64 in every precision mode
+ *     ("outputs of the fitting net ... converted back to double precision").
+ *   - There is no CPU fallback: without a CUDA device every compute entry point returns DP_ECUDA.
+ */
+#ifndef DP_B200_H
+#define DP_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dp_model dp_model; /* opaque; owns device copies of the (re-laid-out, converted) weights */
+
+/* PAPER.md:125.  DP_FP64: everything double.  DP_MIX32: nets in fp32, coordinates / environment matrix /
+ * force and virial accumulation in fp64.  DP_MIX16: embedding net and fitting layers 1-2 with fp16 operands
+ * on tensor cores and fp32 accumulation, tanh and the last fitting layer in fp32, fp64 accumulation of
+ * forces and virial. */
+typedef enum { DP_FP64 = 0, DP_MIX32 = 1, DP_MIX16 = 2 } dp_precision;
+
+typedef enum {
+    DP_OK = 0,
+    DP_EINVAL = -1,   /* null pointer, natoms <= 0, rc_smth >= rc, rc*rc >= 128, sel <= 0, unsupported widths */
+    DP_EBOX = -2,     /* box not orthorhombic, or a box length < 2*rc                                        */
+    DP_ENOMEM = -3,   /* workspace_bytes < dp_workspace_bytes(model, natoms)                                  */
+    DP_ETYPE = -4,    /* an atom type outside type_map (detected on device, reported by dp_status)            */
+    DP_ECUDA = -5,    /* CUDA runtime error or no device                                                      */
+    DP_ENEIGH = -6,   /* an atom has more candidates inside rc than the sort buffer holds (dp_status)         */
+    DP_EUNSUPPORTED = -7 /* precision mode / shape not built                                                 */
+} dp_error;
+
+/* Host-side description of one model; read only during dp_create (weights are copied and converted once,
+ * round-to-nearest-even: "trained in double precision, and cast").
+ * Dense layers are y = x W + b with W row-major [in][out].
+ * Layer rule (Fig. 1(e),(f)): out == 2*in -> y = (x,x) + tanh(xW+b); out == in -> y = x + tanh(xW+b);
+ * otherwise y = tanh(xW+b).  The last fitting layer is linear. */
+typedef struct {
+    int ntypes;              /* T, 1..4                                                                    */
+    int embed_widths[3];     /* (m0, m1, m2); this build supports (25, 50, 100) only                       */
+    int axis;                /* M2 (16): D = A^T A[:, :M2]                                                   */
+    int fit_widths[3];       /* (240, 240, 240)                                                             */
+    const double *embed;     /* T*T nets, index a*T+b (a centre type, b neighbour type):
+                                W1[1*m0] b1[m0] W2[m0*m1] b2[m1] W3[m1*m2] b3[m2]                           */
+    const double *fit;       /* T nets: V1[(m2*axis)*f0] c1[f0] V2[f0*f1] c2[f1] V3[f1*f2] c3[f2] v4[f2] c4[1] */
+    const double *ebias;     /* [T] per-type energy bias added to E_i                                       */
+    const double *avg;       /* [T][4] per CENTRE type: R^ = (R~ - avg) / std                               */
+    const double *std;       /* [T][4]                                                                      */
+} dp_weights;
+
+/* Create a model.  type_map[user_type] -> model type in [0,T) or -1 (unmapped -> DP_ETYPE at compute time);
+ * n_type_map entries.  sel[b] = neighbour capacity of type b ("cut-off number of neighbors").
+ * rc_smth < rc, rc*rc < 128 (distance field of the 64-bit sort key).  *out is set on DP_OK. */
+int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_type_map, double rc,
+              double rc_smth, const int *sel, dp_precision prec);
+
+/* Bytes of device workspace dp_compute needs for up to natoms atoms (0 on invalid arguments). */
+size_t dp_workspace_bytes(const dp_model *m, long natoms);
+
+/* One evaluation.  coords_dev [natoms][3] fp64 (may lie outside the box; wrapped canonically),
+ * types_dev [natoms] int32 USER types, box_host[9] row-major rows a,b,c (orthorhombic, lengths >= 2 rc),
+ * workspace_dev: >= dp_workspace_bytes, 256-byte aligned, contents undefined on entry and exit,
+ * cuda_stream: a cudaStream_t (NULL = default stream).
+ * Outputs (device, fp64): energy_dev[1]; atom_energy_dev[natoms] or NULL; forces_dev[natoms][3];
+ * virial_dev[9] row-major, Xi_ab = -sum d_a (dE/dd_b) = -dE/d(strain_ab), or NULL.
+ * A neighbour block that exceeds its capacity keeps the nearest sel[b]; this is counted,
+ * not an error. */
+int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *types_dev,
+               const double *box_host, void *workspace_dev, size_t workspace_bytes, void *cuda_stream,
+               double *energy_dev, double *atom_energy_dev, double *forces_dev, double *virial_dev);
+
+/* The formatted neighbour list of the LAST dp_compute on this model (workspace must still be alive):
+ * nlist_dev [natoms][Nm] int32, user indices, rows in user order, type-blocked, each block sorted by
+ * (quantised r^2, j), -1 padded.  Enqueued on cuda_stream. */
+int dp_get_nlist(dp_model *m, int *nlist_dev, void *cuda_stream);
+
+/* Synchronises the stream of the last dp_compute and reports device-detected conditions:
+ * returns DP_OK, DP_ETYPE or DP_ENEIGH; *n_truncated_atoms (may be NULL) = atoms with an over-full block. */
+int dp_status(dp_model *m, long *n_truncated_atoms);
+
+/* Number of kernels dp_compute enqueues for this model (for launch accounting in benchmarks). */
+int dp_launches_per_compute(const dp_model *m);
+
+/* Neighbour rows actually pushed through the embedding net by the last dp_compute (after dp_status):
+ * forward and backward counts; padded rows of a block collapse to one representative row. */
+int dp_last_row_counts(dp_model *m, long *rows_forward, long *rows_backward);
+
+void dp_destroy(dp_model *m);
+const char *dp_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DP_B200_H */

@@ -1,0 +1,314 @@
+// C-ABI entry points (include/dp.h): model creation (weight conversion + re-layout into MMA fragment order),
+// workspace carve-up (the caller-owned "trunk"), kernel sequencing on the caller's stream.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "dp_internal.h"
+
+namespace {
+
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+long ncell_max_for(long N) { return N < 512 ? 512 : N; }
+
+WsLayout ws_layout(const dp_model *m, long N) {
+    WsLayout L{};
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t r = o; o = align256(o + bytes); return r; };
+    const size_t nbins = (size_t)m->T * (size_t)ncell_max_for(N);
+    L.status = take(64);
+    L.bin_count = take(sizeof(int) * (nbins + 1));
+    L.bin_start = take(sizeof(int) * (nbins + 1));
+    L.bin_cursor = take(sizeof(int) * nbins);
+    L.atom_bin = take(sizeof(int) * (size_t)N);
+    L.tmp_order = take(sizeof(int) * (size_t)N);
+    L.perm = take(sizeof(int) * (size_t)N);
+    L.inv = take(sizeof(int) * (size_t)N);
+    L.xs = take(sizeof(double) * 3 * (size_t)N);
+    L.xw = take(sizeof(double) * 3 * (size_t)N);
+    L.nlist = take(sizeof(int) * (size_t)N * m->Nm);
+    L.nreal = take(sizeof(int) * (size_t)N * m->T);
+    L.A = take(sizeof(double) * (size_t)N * 4 * M2E);
+    L.gAf = take(sizeof(double) * (size_t)N * 3 * NT3 * 32);
+    L.fit_act = take(sizeof(double) * (size_t)N * 240 * 7);
+    L.gD = take(sizeof(double) * (size_t)N * M2E * 16);
+    L.eatom = take(sizeof(double) * (size_t)N);
+    L.fsorted = take(sizeof(double) * 3 * (size_t)N);
+    L.virial = take(sizeof(double) * 16);
+    L.total = o;
+    return L;
+}
+
+bool make_grid(const dp_model *m, long N, const double *box, Grid3 *g) {
+    if (box[1] != 0 || box[2] != 0 || box[3] != 0 || box[5] != 0 || box[6] != 0 || box[7] != 0) return false;
+    const double Ls[3] = {box[0], box[4], box[8]};
+    for (int a = 0; a < 3; ++a) {
+        if (!(Ls[a] >= 2.0 * m->rc)) return false;
+        g->L[a] = Ls[a];
+        int nc = (int)std::floor(Ls[a] / (m->rc * (1.0 + 1e-9)));
+        g->nc[a] = nc < 1 ? 1 : nc;
+    }
+    const long cap = ncell_max_for(N);
+    while ((long)g->nc[0] * g->nc[1] * g->nc[2] > cap) {
+        int big = 0;
+        for (int a = 1; a < 3; ++a) if (g->nc[a] > g->nc[big]) big = a;
+        g->nc[big] -= 1;
+    }
+    for (int a = 0; a < 3; ++a) g->inv_cw[a] = (double)g->nc[a] / Ls[a];
+    g->ncell = g->nc[0] * g->nc[1] * g->nc[2];
+    return true;
+}
+
+// logical feature maps of the register-chained embedding net (dp_internal.h)
+inline int f2map(int nt, int r, int j) { int e = 4 * nt + r; return e < M0 ? e + M0 * j : -1; }
+inline int f3map(int nt3, int r, int j3) { int f = f2map(nt3 >> 1, r, nt3 & 1); return f < 0 ? -1 : f + M1 * j3; }
+
+template <typename TW>
+void build_embed_frag(const double *net, EmbedNetFrag<TW> *out) {
+    const double *W1 = net, *b1 = W1 + M0, *W2 = b1 + M0, *b2 = W2 + M0 * M1, *W3 = b2 + M1, *b3 = W3 + M1 * M2E;
+    std::memset(out, 0, sizeof(*out));
+    for (int kc = 0; kc < KC1; ++kc)
+        for (int r = 0; r < 4; ++r) {
+            int e = 4 * kc + r;
+            if (e < M0) { out->w1[4 * kc + r] = (TW)W1[e]; out->b1[4 * kc + r] = (TW)b1[e]; }
+        }
+    for (int nt = 0; nt < NT2; ++nt)
+        for (int r = 0; r < 4; ++r)
+            for (int j = 0; j < 2; ++j) { int f = f2map(nt, r, j); if (f >= 0) out->b2[nt * 8 + 2 * r + j] = (TW)b2[f]; }
+    for (int nt = 0; nt < NT3; ++nt)
+        for (int r = 0; r < 4; ++r)
+            for (int j = 0; j < 2; ++j) { int f = f3map(nt, r, j); if (f >= 0) out->b3[nt * 8 + 2 * r + j] = (TW)b3[f]; }
+    for (int kc = 0; kc < KC1; ++kc)
+        for (int nt = 0; nt < NT2; ++nt)
+            for (int l = 0; l < 32; ++l) {
+                int ein = 4 * kc + (l & 3), n = l >> 2, fo = f2map(nt, n >> 1, n & 1);
+                if (ein < M0 && fo >= 0) out->W2f[(kc * NT2 + nt) * 32 + l] = (TW)W2[ein * M1 + fo];
+            }
+    for (int kc = 0; kc < 2 * NT2; ++kc)
+        for (int nt3 = 0; nt3 < NT3; ++nt3)
+            for (int l = 0; l < 32; ++l) {
+                int fin = f2map(kc >> 1, l & 3, kc & 1), n = l >> 2, fo = f3map(nt3, n >> 1, n & 1);
+                if (fin >= 0 && fo >= 0) out->W3f[(kc * NT3 + nt3) * 32 + l] = (TW)W3[fin * M2E + fo];
+            }
+    for (int kc = 0; kc < 2 * NT3; ++kc)
+        for (int nt2 = 0; nt2 < NT2; ++nt2)
+            for (int l = 0; l < 32; ++l) {
+                int fo = f3map(kc >> 1, l & 3, kc & 1), n = l >> 2, fin = f2map(nt2, n >> 1, n & 1);
+                if (fin >= 0 && fo >= 0) out->W3Tf[(kc * NT2 + nt2) * 32 + l] = (TW)W3[fin * M2E + fo];
+            }
+    for (int kc = 0; kc < 2 * NT2; ++kc)
+        for (int nt1 = 0; nt1 < 4; ++nt1)
+            for (int l = 0; l < 32; ++l) {
+                int fo = f2map(kc >> 1, l & 3, kc & 1), n = l >> 2;
+                int kc1 = 2 * nt1 + (n & 1), e = 4 * kc1 + (n >> 1);
+                if (kc1 < KC1 && e < M0 && fo >= 0) out->W2Tf[(kc * 4 + nt1) * 32 + l] = (TW)W2[e * M1 + fo];
+            }
+}
+
+template <typename Tp>
+cudaError_t upload(const std::vector<Tp> &h, void **dev) {
+    cudaError_t e = cudaMalloc(dev, h.size() * sizeof(Tp));
+    if (e != cudaSuccess) return e;
+    return cudaMemcpy(*dev, h.data(), h.size() * sizeof(Tp), cudaMemcpyHostToDevice);
+}
+
+__global__ void k_finalize(long N, const int *__restrict__ perm, const double *__restrict__ fsorted,
+                           const double *__restrict__ eatom, const double *__restrict__ vir_ws,
+                           double *__restrict__ energy, double *__restrict__ eatom_out, double *__restrict__ forces,
+                           double *__restrict__ virial) {
+    __shared__ double red[8];
+    const long s = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    double e = 0.0;
+    if (s < N) {
+        const int u = perm[s];
+        e = eatom[s];
+        if (eatom_out) eatom_out[u] = e;
+        forces[3L * u] = fsorted[3 * s];
+        forces[3L * u + 1] = fsorted[3 * s + 1];
+        forces[3L * u + 2] = fsorted[3 * s + 2];
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = e;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += red[w];
+        atomicAdd(energy, t);
+    }
+    if (virial && blockIdx.x == 0 && threadIdx.x < 9) virial[threadIdx.x] = vir_ws[threadIdx.x];
+}
+
+}  // namespace
+
+cudaError_t launch_finalize(const dp_model *m, long N, char *ws, const WsLayout &L, double *energy, double *eatom,
+                            double *forces, double *virial, cudaStream_t st) {
+    (void)m;
+    k_finalize<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(N, (int *)(ws + L.perm), (double *)(ws + L.fsorted),
+                                                           (double *)(ws + L.eatom), (double *)(ws + L.virial), energy,
+                                                           eatom, forces, virial);
+    return cudaGetLastError();
+}
+
+extern "C" {
+
+const char *dp_strerror(int code) {
+    switch (code) {
+        case DP_OK: return "ok";
+        case DP_EINVAL: return "invalid argument";
+        case DP_EBOX: return "box must be orthorhombic with every length >= 2*rc";
+        case DP_ENOMEM: return "workspace too small";
+        case DP_ETYPE: return "atom type outside type_map";
+        case DP_ECUDA: return "CUDA error or no device";
+        case DP_ENEIGH: return "too many neighbour candidates for the sort buffer";
+        case DP_EUNSUPPORTED: return "precision mode or shape not supported by this build";
+        default: return "unknown error";
+    }
+}
+
+int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_type_map, double rc, double rc_smth,
+              const int *sel, dp_precision prec) {
+    if (!out || !w || !type_map || !sel || n_type_map <= 0) return DP_EINVAL;
+    if (!w->embed || !w->fit || !w->ebias || !w->avg || !w->std) return DP_EINVAL;
+    const int T = w->ntypes;
+    if (T < 1 || T > DP_MAX_TYPES) return DP_EINVAL;
+    if (!(rc > 0) || !(rc_smth >= 0) || !(rc_smth < rc) || !(rc * rc < 128.0)) return DP_EINVAL;
+    if (w->embed_widths[0] != M0 || w->embed_widths[1] != M1 || w->embed_widths[2] != M2E || w->axis != 16 ||
+        w->fit_widths[0] != 240 || w->fit_widths[1] != 240 || w->fit_widths[2] != 240)
+        return DP_EUNSUPPORTED;
+    if (prec != DP_FP64) return DP_EUNSUPPORTED;
+    int maxsel = 0, Nm = 0;
+    for (int b = 0; b < T; ++b) { if (sel[b] <= 0) return DP_EINVAL; Nm += sel[b]; if (sel[b] > maxsel) maxsel = sel[b]; }
+    for (int k = 0; k < n_type_map; ++k) if (type_map[k] >= T) return DP_EINVAL;
+    for (int a = 0; a < T; ++a) for (int c = 0; c < 4; ++c) if (!(w->std[4 * a + c] > 0)) return DP_EINVAL;
+    int dev = 0, ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return DP_ECUDA;
+    if (cudaGetDevice(&dev) != cudaSuccess) return DP_ECUDA;
+    dp_model *m = new (std::nothrow) dp_model();
+    if (!m) return DP_EINVAL;
+    std::memset(m, 0, sizeof(*m));
+    m->T = T; m->Nm = Nm; m->axis = 16; m->F = 240; m->rc = rc; m->rc_smth = rc_smth; m->prec = prec;
+    m->n_type_map = n_type_map;
+    for (int b = 0; b < T; ++b) { m->sel[b] = sel[b]; m->off[b + 1] = m->off[b] + sel[b]; }
+    int cap = 256;
+    while (cap < 2 * maxsel) cap <<= 1;
+    if (cap > 4096) cap = 4096;
+    if (cap < maxsel) { delete m; return DP_EINVAL; }
+    m->sort_cap = cap;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) { delete m; return DP_ECUDA; }
+    m->num_sms = prop.multiProcessorCount;
+
+    cudaError_t e = cudaSuccess;
+    auto ok = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
+    std::vector<int> tm(type_map, type_map + n_type_map);
+    ok(upload(tm, (void **)&m->type_map_dev));
+    const size_t ensz = (size_t)M0 + M0 + M0 * M1 + M1 + M1 * M2E + M2E;
+    {
+        std::vector<EmbedNetFrag<double>> frags((size_t)T * T);
+        for (int ab = 0; ab < T * T; ++ab) build_embed_frag<double>(w->embed + ab * ensz, &frags[ab]);
+        ok(upload(frags, &m->embed_frag_dev));
+    }
+    const int ND = M2E * 16, F = 240;
+    const size_t fnsz = (size_t)ND * F + F + (size_t)F * F + F + (size_t)F * F + F + F + 1;
+    std::vector<double> V1((size_t)T * ND * F), V2((size_t)T * F * F), V3((size_t)T * F * F), c1(T * F), c2(T * F),
+        c3(T * F), v4(T * F), c4(T);
+    for (int a = 0; a < T; ++a) {
+        const double *p = w->fit + a * fnsz;
+        std::memcpy(&V1[(size_t)a * ND * F], p, sizeof(double) * ND * F); p += (size_t)ND * F;
+        std::memcpy(&c1[a * F], p, sizeof(double) * F); p += F;
+        std::memcpy(&V2[(size_t)a * F * F], p, sizeof(double) * F * F); p += (size_t)F * F;
+        std::memcpy(&c2[a * F], p, sizeof(double) * F); p += F;
+        std::memcpy(&V3[(size_t)a * F * F], p, sizeof(double) * F * F); p += (size_t)F * F;
+        std::memcpy(&c3[a * F], p, sizeof(double) * F); p += F;
+        std::memcpy(&v4[a * F], p, sizeof(double) * F); p += F;
+        c4[a] = p[0];
+    }
+    ok(upload(V1, &m->fitV1_dev)); ok(upload(V2, &m->fitV2_dev)); ok(upload(V3, &m->fitV3_dev));
+    ok(upload(c1, &m->fitc1_dev)); ok(upload(c2, &m->fitc2_dev)); ok(upload(c3, &m->fitc3_dev));
+    ok(upload(v4, &m->fitv4_dev)); ok(upload(c4, &m->fitc4_dev));
+    std::vector<double> avg(w->avg, w->avg + 4 * T), sd(w->std, w->std + 4 * T), eb(w->ebias, w->ebias + T);
+    ok(upload(avg, (void **)&m->avg_dev)); ok(upload(sd, (void **)&m->std_dev)); ok(upload(eb, (void **)&m->ebias_dev));
+    if (e != cudaSuccess) { dp_destroy(m); return DP_ECUDA; }
+    *out = m;
+    return DP_OK;
+}
+
+void dp_destroy(dp_model *m) {
+    if (!m) return;
+    void *ptrs[] = {m->type_map_dev, m->embed_frag_dev, m->avg_dev, m->std_dev, m->ebias_dev, m->fitV1_dev, m->fitV2_dev,
+                    m->fitV3_dev, m->fitc1_dev, m->fitc2_dev, m->fitc3_dev, m->fitv4_dev, m->fitc4_dev};
+    for (void *p : ptrs) if (p) cudaFree(p);
+    delete m;
+}
+
+size_t dp_workspace_bytes(const dp_model *m, long natoms) {
+    if (!m || natoms <= 0 || natoms > 16777216) return 0;
+    return ws_layout(m, natoms).total;
+}
+
+int dp_launches_per_compute(const dp_model *m) { return m ? 17 : 0; }
+
+int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *types_dev, const double *box_host,
+               void *workspace_dev, size_t workspace_bytes, void *cuda_stream, double *energy_dev,
+               double *atom_energy_dev, double *forces_dev, double *virial_dev) {
+    if (!m || natoms <= 0 || natoms > 16777216 || !coords_dev || !types_dev || !box_host || !workspace_dev ||
+        !energy_dev || !forces_dev)
+        return DP_EINVAL;
+    if (((uintptr_t)workspace_dev & 255) != 0) return DP_EINVAL;
+    Grid3 g;
+    if (!make_grid(m, natoms, box_host, &g)) return DP_EBOX;
+    const WsLayout L = ws_layout(m, natoms);
+    if (workspace_bytes < L.total) return DP_ENOMEM;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    char *ws = (char *)workspace_dev;
+    cudaError_t e = cudaSuccess;
+    auto ok = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
+    ok(cudaMemsetAsync(ws + L.status, 0, 64, st));
+    ok(cudaMemsetAsync(ws + L.fsorted, 0, sizeof(double) * 3 * (size_t)natoms, st));
+    ok(cudaMemsetAsync(ws + L.virial, 0, sizeof(double) * 16, st));
+    ok(cudaMemsetAsync(energy_dev, 0, sizeof(double), st));
+    ok(launch_build_cells(m, natoms, coords_dev, types_dev, g, ws, L, st));
+    ok(launch_nlist(m, natoms, g, ws, L, st));
+    ok(launch_embed_fwd_f64(m, natoms, g, ws, L, st));
+    ok(launch_fit_f64(m, natoms, g, ws, L, st));
+    ok(launch_embed_bwd_f64(m, natoms, g, ws, L, st));
+    ok(launch_finalize(m, natoms, ws, L, energy_dev, atom_energy_dev, forces_dev, virial_dev, st));
+    m->last_natoms = natoms; m->last_ws = workspace_dev; m->last_stream = st;
+    return e == cudaSuccess ? DP_OK : DP_ECUDA;
+}
+
+int dp_get_nlist(dp_model *m, int *nlist_dev, void *cuda_stream) {
+    if (!m || !nlist_dev || !m->last_ws) return DP_EINVAL;
+    const WsLayout L = ws_layout(m, m->last_natoms);
+    cudaError_t e = launch_get_nlist(m, m->last_natoms, (char *)m->last_ws, L, nlist_dev, (cudaStream_t)cuda_stream);
+    return e == cudaSuccess ? DP_OK : DP_ECUDA;
+}
+
+int dp_status(dp_model *m, long *n_truncated_atoms) {
+    if (!m || !m->last_ws) return DP_EINVAL;
+    if (cudaStreamSynchronize(m->last_stream) != cudaSuccess) return DP_ECUDA;
+    int st[2] = {0, 0};
+    const WsLayout L = ws_layout(m, m->last_natoms);
+    if (cudaMemcpy(st, (char *)m->last_ws + L.status, sizeof(st), cudaMemcpyDeviceToHost) != cudaSuccess) return DP_ECUDA;
+    if (n_truncated_atoms) *n_truncated_atoms = st[1];
+    if (st[0] & 1) return DP_ETYPE;
+    if (st[0] & 2) return DP_ENEIGH;
+    return DP_OK;
+}
+
+int dp_last_row_counts(dp_model *m, long *rows_forward, long *rows_backward) {
+    if (!m || !m->last_ws) return DP_EINVAL;
+    if (cudaStreamSynchronize(m->last_stream) != cudaSuccess) return DP_ECUDA;
+    unsigned long long c[2] = {0, 0};
+    const WsLayout L = ws_layout(m, m->last_natoms);
+    if (cudaMemcpy(c, (char *)m->last_ws + L.status + 8, sizeof(c), cudaMemcpyDeviceToHost) != cudaSuccess) return DP_ECUDA;
+    if (rows_forward) *rows_forward = (long)c[0];
+    if (rows_backward) *rows_backward = (long)c[1];
+    return DP_OK;
+}
+
+}  // extern "C"

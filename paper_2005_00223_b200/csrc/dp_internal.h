@@ -1,0 +1,104 @@
+// Internal declarations of the CUDA path (never included by oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/dp.h"
+
+#define DP_MAX_TYPES 4
+#define DP_WARPS_PER_CTA 8
+
+// ---------------------------------------------------------------- shapes fixed by this build (dp.h: widths (25,50,100))
+constexpr int M0 = 25, M1 = 50, M2E = 100;   // embedding widths
+constexpr int KC1 = 7;                       // ceil(M0/4) k-chunks of layer-1 output
+constexpr int NT2 = 7;                       // 8-wide tiles of layer-2 output (56 positions, 50 real)
+constexpr int NT3 = 14;                      // 8-wide tiles of layer-3 output (112 positions, 100 real)
+constexpr int M2P = NT3 * 8;                 // padded G width
+constexpr int ROWCHUNK = 64;                 // neighbour rows staged per pre-pass / post-pass
+
+// Fragment-ordered embedding net (one per (centre type, neighbour type)), element type TW.
+// Logical feature <-> internal position maps:
+//   layer-1 slot (kc,r)        : e  = 4*kc + r                       (valid if < 25)
+//   layer-2 position (nt,r,j)  : f2 = (4*nt + r) + 25*j              (valid if 4*nt+r < 25)
+//   layer-3 position (nt3,r,j3): f3 = f2(nt3/2, r, nt3%2) + 50*j3    (valid if f2 valid)
+template <typename TW>
+struct EmbedNetFrag {
+    TW w1[KC1 * 4];                 // by slot
+    TW b1[KC1 * 4];
+    TW b2[NT2 * 8];                 // by position nt*8 + 2r + j
+    TW b3[NT3 * 8];
+    TW W2f[KC1 * NT2 * 32];         // forward B fragments  [kc][nt][lane]
+    TW W3f[NT3 * NT3 * 32];         // forward B fragments  [kc'=2nt2+j2][nt3][lane]
+    TW W3Tf[2 * NT3 * NT2 * 32];    // backward B fragments [kc=2nt3+j3][nt2][lane]
+    TW W2Tf[NT3 * 4 * 32];          // backward B fragments [kc=2nt2+j2][nt1][lane]
+};
+
+struct dp_model {
+    int T;
+    int sel[DP_MAX_TYPES];
+    int off[DP_MAX_TYPES + 1];
+    int Nm;
+    int axis;                       // 16
+    int F;                          // fitting width 240
+    double rc, rc_smth;
+    dp_precision prec;
+    int n_type_map;
+    int *type_map_dev;
+    // device weights
+    void *embed_frag_dev;           // T*T EmbedNetFrag<TW>
+    double *avg_dev, *std_dev;      // [T][4]
+    double *ebias_dev;              // [T]
+    // fitting nets (per type): V1 [1600][240], V2, V3 [240][240] row-major in x out, biases, v4, c4
+    void *fitV1_dev, *fitV2_dev, *fitV3_dev;   // TW
+    void *fitc1_dev, *fitc2_dev, *fitc3_dev, *fitv4_dev, *fitc4_dev;  // TW / float
+    int num_sms;
+    // state of the last compute
+    long last_natoms;
+    void *last_ws;
+    cudaStream_t last_stream;
+    int sort_cap;
+};
+
+// Workspace carve-up (all offsets 256-byte aligned), filled by dp_ws_layout().
+struct WsLayout {
+    size_t total;
+    size_t status;      // int[8]: [0] error flags, [1] n_truncated, [2] rows_fwd(lo) ... as unsigned long long at [2],[4]
+    size_t bin_count;   // int[nbins+1]
+    size_t bin_start;   // int[nbins+1]
+    size_t bin_cursor;  // int[nbins]
+    size_t atom_bin;    // int[N]
+    size_t tmp_order;   // int[N]
+    size_t perm;        // int[N]  sorted -> user
+    size_t inv;         // int[N]  user -> sorted
+    size_t xs;          // double[N][3] wrapped coords, sorted order
+    size_t xw;          // double[N][3] wrapped coords, user order
+    size_t nlist;       // int[N][Nm] sorted-space indices
+    size_t nreal;       // int[N][T]
+    size_t A;           // double[N][4][100]   (float for mixed modes)
+    size_t gAf;         // gA fragments [N][42][32]
+    size_t fit_act;     // 7 activation buffers [N][240]
+    size_t gD;          // [N][1600]
+    size_t eatom;       // double[N] sorted order
+    size_t fsorted;     // double[N][3] sorted order
+    size_t virial;      // double[9] + energy accumulators
+};
+
+struct Grid3 {
+    int nc[3];          // cells per axis
+    double L[3];
+    double inv_cw[3];   // nc / L
+    int ncell;
+};
+
+// launchers (each returns cudaGetLastError())
+cudaError_t launch_build_cells(const dp_model *m, long N, const double *coords, const int *types, const Grid3 &g,
+                               char *ws, const WsLayout &L, cudaStream_t st);
+cudaError_t launch_nlist(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+cudaError_t launch_get_nlist(const dp_model *m, long N, char *ws, const WsLayout &L, int *out, cudaStream_t st);
+cudaError_t launch_embed_fwd_f64(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+cudaError_t launch_embed_bwd_f64(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+cudaError_t launch_fit_f64(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+cudaError_t launch_finalize(const dp_model *m, long N, char *ws, const WsLayout &L, double *energy, double *eatom,
+                            double *forces, double *virial, cudaStream_t st);
+int embed_smem_bytes_fwd_f64();
+int embed_smem_bytes_bwd_f64();

@@ -1,0 +1,288 @@
+// S5 (descriptor) + S6 (fitting net forward and backward) of SURVEY.md section 8(a), FP64 mode.
+//
+// D_i = A_i^T A_i[:, :M2] ("the descriptor is the product of terms involving R~ and G"), fitting net
+// 1600 -> 240 -> 240 -> 240 -> 1 with identity skips (Fig. 1(d),(f), 151), backward by hand with
+// tanh' = 1 - tanh^2 fused into the GEMM epilogues.  The GEMMs are batched over the atoms of one
+// centre type and run on the FP64 tensor pipe (DMMA m8n8k4); bias, tanh, skip and tanh' live in the epilogue
+// (PAPER.md:133-134 merged them into cuBLAS GEMM calls; here they never reach memory as separate passes).
+#include "dp_internal.h"
+
+namespace {
+
+constexpr int BM = 64, BN = 80, BK = 16;
+constexpr int AS_STRIDE = BK + 4;      // doubles; conflict-free A-fragment loads
+constexpr int BS_STRIDE = BN + 4;      // doubles; conflict-free B-fragment loads (B stored [k][n])
+constexpr int BT_STRIDE = BK + 4;      // B stored [n][k] for the transposed products
+constexpr int AS_TILE = BM * AS_STRIDE;
+constexpr int B_TILE = (BK * BS_STRIDE > BN * BT_STRIDE) ? BK * BS_STRIDE : BN * BT_STRIDE;
+
+__device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b) {
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+        : "+d"(c0), "+d"(c1)
+        : "d"(a), "d"(b));
+}
+
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc, bool valid) {
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+    int sz = valid ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(s), "l"(gsrc), "r"(sz));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N)); }
+
+struct FitArgs {
+    int ncell;
+    const int *bin_start;
+    int K, N;                 // GEMM inner and output widths
+    const double *A; int lda;             // [rows][K]
+    const double *B; long b_type_stride; int ldb;   // weights of type a at B + a*b_type_stride
+    const double *bias; int bias_type_stride;       // epilogue vector (c1/c2/c3 or v4)
+    const double *v4; int v4_type_stride;
+    const double *aux0; const double *aux1;         // epilogue inputs [rows][240]
+    double *out0; double *out1; int ldo;
+};
+
+// MODE: 0 L1 fwd, 1 L2 fwd, 2 L3 fwd, 3 L3 bwd, 4 L2 bwd, 5 L1 bwd (see file header of DESIGN.md section "fitting")
+template <int MODE>
+__global__ void __launch_bounds__(256) k_fit_gemm(FitArgs p) {
+    constexpr bool BT = MODE >= 3;
+    __shared__ __align__(16) double sm[2 * (AS_TILE + B_TILE)];
+    const int a = blockIdx.z;
+    const int ts0 = p.bin_start[a * p.ncell], ts1 = p.bin_start[(a + 1) * p.ncell];
+    const int row0 = ts0 + blockIdx.x * BM;
+    if (row0 >= ts1) return;
+    const int n0 = blockIdx.y * BN;
+    const double *Bw = p.B + a * p.b_type_stride;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int wm = wid >> 1, wn = wid & 1;         // 4 x 2 warps, warp tile 16 x 40
+    const int q4 = lane >> 2, r = lane & 3;
+
+    auto load_tiles = [&](int stage, int k0) {
+        double *As = sm + stage * (AS_TILE + B_TILE);
+        double *Bs = As + AS_TILE;
+#pragma unroll
+        for (int c = tid; c < BM * (BK / 2); c += 256) {
+            const int row = c >> 3, c8 = c & 7;
+            const bool ok = row0 + row < ts1;
+            const double *src = p.A + (long)(ok ? row0 + row : ts0) * p.lda + k0 + 2 * c8;
+            cp_async16(As + row * AS_STRIDE + 2 * c8, src, ok);
+        }
+        if (!BT) {
+            for (int c = tid; c < BK * (BN / 2); c += 256) {
+                const int k = c / (BN / 2), cc = c % (BN / 2);
+                cp_async16(Bs + k * BS_STRIDE + 2 * cc, Bw + (long)(k0 + k) * p.ldb + n0 + 2 * cc, true);
+            }
+        } else {
+            for (int c = tid; c < BN * (BK / 2); c += 256) {
+                const int n = c >> 3, c8 = c & 7;
+                cp_async16(Bs + n * BT_STRIDE + 2 * c8, Bw + (long)(n0 + n) * p.ldb + k0 + 2 * c8, true);
+            }
+        }
+        cp_async_commit();
+    };
+
+    double acc[2][5][2];
+#pragma unroll
+    for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+        for (int nt = 0; nt < 5; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
+
+    const int nk = p.K / BK;
+    load_tiles(0, 0);
+    for (int ks = 0; ks < nk; ++ks) {
+        if (ks + 1 < nk) { load_tiles((ks + 1) & 1, (ks + 1) * BK); cp_async_wait<1>(); }
+        else cp_async_wait<0>();
+        __syncthreads();
+        const double *As = sm + (ks & 1) * (AS_TILE + B_TILE);
+        const double *Bs = As + AS_TILE;
+#pragma unroll
+        for (int kc = 0; kc < BK / 4; ++kc) {
+            double af[2], bf[5];
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt) af[mt] = As[(wm * 16 + mt * 8 + q4) * AS_STRIDE + kc * 4 + r];
+#pragma unroll
+            for (int nt = 0; nt < 5; ++nt)
+                bf[nt] = BT ? Bs[(wn * 40 + nt * 8 + q4) * BT_STRIDE + kc * 4 + r]
+                            : Bs[(kc * 4 + r) * BS_STRIDE + wn * 40 + nt * 8 + q4];
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+                for (int nt = 0; nt < 5; ++nt) dmma(acc[mt][nt][0], acc[mt][nt][1], af[mt], bf[nt]);
+        }
+        __syncthreads();
+    }
+
+    // epilogue: thread holds (row = wm*16 + mt*8 + q4, cols n0 + wn*40 + nt*8 + 2r + {0,1})
+#pragma unroll
+    for (int mt = 0; mt < 2; ++mt) {
+        const int row = row0 + wm * 16 + mt * 8 + q4;
+        if (row >= ts1) continue;
+#pragma unroll
+        for (int nt = 0; nt < 5; ++nt) {
+            const int col = n0 + wn * 40 + nt * 8 + 2 * r;
+            const long o = (long)row * p.ldo + col;
+            double v0 = acc[mt][nt][0], v1 = acc[mt][nt][1];
+            if (MODE == 0) {
+                const double *b = p.bias + a * p.bias_type_stride + col;
+                *reinterpret_cast<double2 *>(p.out0 + o) = make_double2(tanh(v0 + b[0]), tanh(v1 + b[1]));
+            } else if (MODE == 1) {
+                const double *b = p.bias + a * p.bias_type_stride + col;
+                const double2 h = *reinterpret_cast<const double2 *>(p.aux0 + o);
+                const double t0 = tanh(v0 + b[0]), t1 = tanh(v1 + b[1]);
+                *reinterpret_cast<double2 *>(p.out0 + o) = make_double2(t0, t1);
+                *reinterpret_cast<double2 *>(p.out1 + o) = make_double2(h.x + t0, h.y + t1);
+            } else if (MODE == 2) {
+                const double *b = p.bias + a * p.bias_type_stride + col;
+                const double *v4 = p.v4 + a * p.v4_type_stride + col;
+                const double2 h = *reinterpret_cast<const double2 *>(p.aux0 + o);
+                const double t0 = tanh(v0 + b[0]), t1 = tanh(v1 + b[1]);
+                *reinterpret_cast<double2 *>(p.out0 + o) = make_double2(v4[0] * (1.0 - t0 * t0), v4[1] * (1.0 - t1 * t1));
+                *reinterpret_cast<double2 *>(p.out1 + o) = make_double2(h.x + t0, h.y + t1);
+            } else if (MODE == 3) {
+                const double *v4 = p.v4 + a * p.v4_type_stride + col;
+                const double2 t = *reinterpret_cast<const double2 *>(p.aux0 + o);     // t2
+                const double g0 = v4[0] + v0, g1 = v4[1] + v1;
+                *reinterpret_cast<double2 *>(p.out0 + o) = make_double2(g0, g1);
+                *reinterpret_cast<double2 *>(p.out1 + o) = make_double2(g0 * (1.0 - t.x * t.x), g1 * (1.0 - t.y * t.y));
+            } else if (MODE == 4) {
+                const double2 g = *reinterpret_cast<const double2 *>(p.aux0 + o);     // g2
+                const double2 h = *reinterpret_cast<const double2 *>(p.aux1 + o);     // h1
+                const double g0 = g.x + v0, g1 = g.y + v1;
+                *reinterpret_cast<double2 *>(p.out0 + o) = make_double2(g0 * (1.0 - h.x * h.x), g1 * (1.0 - h.y * h.y));
+            } else {
+                *reinterpret_cast<double2 *>(p.out0 + o) = make_double2(v0, v1);
+            }
+        }
+    }
+}
+
+// D[i][m*16 + a] = sum_c A[i][c][m] A[i][c][a]    (N6, Q6, Q7); one warp per atom
+__global__ void __launch_bounds__(256) k_descr(long N, const double *__restrict__ Amat, double *__restrict__ D) {
+    __shared__ double sA[8][4 * M2E];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const long i = blockIdx.x * 8L + wid;
+    if (i >= N) return;
+    for (int k = lane; k < 4 * M2E; k += 32) sA[wid][k] = Amat[i * 4 * M2E + k];
+    __syncwarp();
+    for (int idx = lane; idx < M2E * 16; idx += 32) {
+        const int m = idx >> 4, ax = idx & 15;
+        double acc = 0.0;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) acc += sA[wid][c * M2E + m] * sA[wid][c * M2E + ax];
+        D[i * (M2E * 16) + idx] = acc;
+    }
+}
+
+__device__ __forceinline__ int type_of_sorted(int i, int T, int ncell, const int *bin_start) {
+    int a = 0;
+    for (int t = 1; t < T; ++t) a += i >= bin_start[t * ncell];
+    return a;
+}
+
+// E_i = h3 . v4 + c4 + ebias[type]   (N7, Q10); one warp per atom
+__global__ void __launch_bounds__(256) k_energy(long N, int T, int ncell, const int *__restrict__ bin_start,
+                                                const double *__restrict__ h3, const double *__restrict__ v4,
+                                                const double *__restrict__ c4, const double *__restrict__ ebias,
+                                                double *__restrict__ eatom) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const long i = blockIdx.x * 8L + wid;
+    if (i >= N) return;
+    const int a = type_of_sorted((int)i, T, ncell, bin_start);
+    double acc = 0.0;
+    for (int n = lane; n < 240; n += 32) acc += h3[i * 240 + n] * v4[a * 240 + n];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) eatom[i] = acc + c4[a] + ebias[a];
+}
+
+__device__ __forceinline__ int feature3(int nt3, int r, int j3) {
+    const int e = 4 * (nt3 >> 1) + r;
+    return e < M0 ? e + M0 * (nt3 & 1) + M1 * j3 : -1;
+}
+
+// gA[c][m] = sum_a gD[m][a] A[c][a] + [m < 16] sum_m' gD[m'][m] A[c][m']   (N8), written as the MMA fragments the
+// embedding backward consumes (layout in embed_f64.cu), pre-scaled by 1/Nm.  One warp per atom.
+__global__ void __launch_bounds__(128) k_gA(long N, double inv_nm, const double *__restrict__ Amat,
+                                            const double *__restrict__ gD, double *__restrict__ gAf) {
+    extern __shared__ double smg[];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const long i = blockIdx.x * 4L + wid;
+    if (i >= N) return;
+    double *sA = smg + wid * (4 * M2E + M2E * 16 + 4 * M2E);
+    double *sG = sA + 4 * M2E;
+    double *sO = sG + M2E * 16;
+    for (int k = lane; k < 4 * M2E; k += 32) sA[k] = Amat[i * 4 * M2E + k];
+    for (int k = lane; k < M2E * 16; k += 32) sG[k] = gD[i * (M2E * 16) + k];
+    __syncwarp();
+    for (int idx = lane; idx < 4 * M2E; idx += 32) {
+        const int c = idx / M2E, m = idx % M2E;
+        double acc = 0.0;
+#pragma unroll
+        for (int ax = 0; ax < 16; ++ax) acc += sG[m * 16 + ax] * sA[c * M2E + ax];
+        if (m < 16)
+            for (int mp = 0; mp < M2E; ++mp) acc += sG[mp * 16 + m] * sA[c * M2E + mp];
+        sO[idx] = acc * inv_nm;
+    }
+    __syncwarp();
+    double *out = gAf + i * (3 * NT3 * 32);
+    const int q4 = lane >> 2, r = lane & 3;
+    for (int nt3 = 0; nt3 < NT3; ++nt3) {
+        const int f = feature3(nt3, q4 >> 1, q4 & 1);
+        out[nt3 * 32 + lane] = f >= 0 ? sO[r * M2E + f] : 0.0;
+    }
+    for (int kc = 0; kc < 2 * NT3; ++kc) {
+        const int f = feature3(kc >> 1, r, kc & 1);
+        out[(NT3 + kc) * 32 + lane] = (f >= 0 && q4 < 4) ? sO[q4 * M2E + f] : 0.0;
+    }
+}
+
+}  // namespace
+
+cudaError_t launch_fit_f64(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    const int F = 240, ND = M2E * 16;
+    const int T = m->T;
+    double *Amat = (double *)(ws + L.A);
+    double *D = (double *)(ws + L.gD);          // D and gD share one [N][1600] buffer (D is dead after layer 1)
+    double *act = (double *)(ws + L.fit_act);
+    const size_t S = (size_t)N * F;
+    double *h1 = act, *t2 = act + S, *h2 = act + 2 * S, *gz3 = act + 3 * S, *h3 = act + 4 * S, *g2 = act + 5 * S,
+           *gz2 = act + 6 * S, *gz1 = h2;      // h2 is dead after the layer-3 forward
+    const int *bin_start = (const int *)(ws + L.bin_start);
+    const double *V1 = (const double *)m->fitV1_dev, *V2 = (const double *)m->fitV2_dev, *V3 = (const double *)m->fitV3_dev;
+    const double *c1 = (const double *)m->fitc1_dev, *c2 = (const double *)m->fitc2_dev, *c3 = (const double *)m->fitc3_dev;
+    const double *v4 = (const double *)m->fitv4_dev, *c4 = (const double *)m->fitc4_dev;
+    const unsigned gx = (unsigned)((N + BM - 1) / BM);
+    const unsigned nb8 = (unsigned)((N + 7) / 8);
+
+    k_descr<<<nb8, 256, 0, st>>>(N, Amat, D);
+
+    FitArgs p{};
+    p.ncell = g.ncell; p.bin_start = bin_start; p.v4 = v4; p.v4_type_stride = F; p.bias_type_stride = F;
+    // layer 1 forward: h1 = tanh(D V1 + c1)
+    p.K = ND; p.N = F; p.A = D; p.lda = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.ldb = F; p.bias = c1;
+    p.out0 = h1; p.ldo = F;
+    k_fit_gemm<0><<<dim3(gx, F / BN, T), 256, 0, st>>>(p);
+    // layer 2 forward: t2 = tanh(h1 V2 + c2), h2 = h1 + t2
+    p.K = F; p.A = h1; p.lda = F; p.B = V2; p.b_type_stride = (long)F * F; p.bias = c2; p.aux0 = h1; p.out0 = t2; p.out1 = h2;
+    k_fit_gemm<1><<<dim3(gx, F / BN, T), 256, 0, st>>>(p);
+    // layer 3 forward: t3 = tanh(h2 V3 + c3), h3 = h2 + t3, gz3 = v4 (1 - t3^2)
+    p.A = h2; p.B = V3; p.bias = c3; p.aux0 = h2; p.out0 = gz3; p.out1 = h3;
+    k_fit_gemm<2><<<dim3(gx, F / BN, T), 256, 0, st>>>(p);
+    k_energy<<<nb8, 256, 0, st>>>(N, T, g.ncell, bin_start, h3, v4, c4, m->ebias_dev, (double *)(ws + L.eatom));
+    // layer 3 backward: g2 = v4 + gz3 V3^T, gz2 = g2 (1 - t2^2)
+    p.A = gz3; p.B = V3; p.aux0 = t2; p.out0 = g2; p.out1 = gz2;
+    k_fit_gemm<3><<<dim3(gx, F / BN, T), 256, 0, st>>>(p);
+    // layer 2 backward: g1 = g2 + gz2 V2^T, gz1 = g1 (1 - h1^2)
+    p.A = gz2; p.B = V2; p.aux0 = g2; p.aux1 = h1; p.out0 = gz1; p.out1 = nullptr;
+    k_fit_gemm<4><<<dim3(gx, F / BN, T), 256, 0, st>>>(p);
+    // layer 1 backward: gD = gz1 V1^T
+    p.A = gz1; p.N = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.out0 = D; p.ldo = ND;
+    k_fit_gemm<5><<<dim3(gx, ND / BN, T), 256, 0, st>>>(p);
+    // gD, A -> gA fragments for the embedding backward
+    static bool attr = false;
+    const int smem = 4 * (4 * M2E + M2E * 16 + 4 * M2E) * 8;
+    if (!attr) { cudaFuncSetAttribute(k_gA, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr = true; }
+    k_gA<<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, 1.0 / (double)m->Nm, Amat, D, (double *)(ws + L.gAf));
+    return cudaGetLastError();
+}

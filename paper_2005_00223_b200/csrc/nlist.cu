@@ -1,0 +1,245 @@
+// S1 + S2 of SURVEY.md section 8(a): canonical wrap, (type, cell) binning, and the formatted neighbour list
+// "sorted by type, then by distance, padded to the cut-off number, nearest N_max kept" with one
+// 64-bit key per element (binary restatement, reading Q11).  Bit-exact against the
+// oracle: the arithmetic that decides list membership and order uses explicit round-to-nearest intrinsics so
+// that nvcc cannot contract it differently from the reading N2 of DESIGN.md.
+#include "dp_internal.h"
+
+namespace {
+
+__device__ __forceinline__ double wrap_coord(double x, double L) {
+    double t = __ddiv_rn(x, L);
+    double f = floor(t);
+    double xw = __fma_rn(-f, L, x);
+    if (xw >= L) xw = __dsub_rn(xw, L);
+    if (xw < 0.0) xw = __dadd_rn(xw, L);
+    return xw;
+}
+
+__device__ __forceinline__ int cell_of(double xw, double inv_cw, int nc) {
+    int c = (int)(xw * inv_cw);
+    return c < 0 ? 0 : (c >= nc ? nc - 1 : c);
+}
+
+__global__ void k_wrap_bin(long N, const double *__restrict__ coords, const int *__restrict__ types,
+                           const int *__restrict__ type_map, int n_type_map, Grid3 g, double *__restrict__ xw,
+                           int *__restrict__ atom_bin, int *__restrict__ bin_count, int *__restrict__ status) {
+    long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int c[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        double w = wrap_coord(coords[3 * i + a], g.L[a]);
+        xw[3 * i + a] = w;
+        c[a] = cell_of(w, g.inv_cw[a], g.nc[a]);
+    }
+    int ut = types[i];
+    int mt = (ut >= 0 && ut < n_type_map) ? type_map[ut] : -1;
+    if (mt < 0) { atomicOr(&status[0], 1); mt = 0; }
+    int bin = mt * g.ncell + (c[0] * g.nc[1] + c[1]) * g.nc[2] + c[2];
+    atom_bin[i] = bin;
+    atomicAdd(&bin_count[bin], 1);
+}
+
+// exclusive scan of bin_count[0..n) -> bin_start[0..n]; one block.
+__global__ void k_scan(int n, const int *__restrict__ cnt, int *__restrict__ start) {
+    __shared__ int warp_sums[32];
+    __shared__ int carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    for (int base = 0; base < n; base += blockDim.x) {
+        int i = base + threadIdx.x;
+        int v = i < n ? cnt[i] : 0;
+        int x = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        if (lane == 31) warp_sums[wid] = x;
+        __syncthreads();
+        if (wid == 0) {
+            int s = lane < nw ? warp_sums[lane] : 0;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                int y = __shfl_up_sync(0xffffffffu, s, o);
+                if (lane >= o) s += y;
+            }
+            warp_sums[lane] = s;
+        }
+        __syncthreads();
+        int prefix = carry + (wid ? warp_sums[wid - 1] : 0) + x - v;
+        if (i < n) start[i] = prefix;
+        __syncthreads();
+        if (threadIdx.x == blockDim.x - 1) carry = prefix + v;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) start[n] = carry;
+}
+
+__global__ void k_scatter(long N, const int *__restrict__ atom_bin, const int *__restrict__ bin_start,
+                          int *__restrict__ cursor, int *__restrict__ tmp_order) {
+    long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int bin = atom_bin[i];
+    int slot = bin_start[bin] + atomicAdd(&cursor[bin], 1);
+    tmp_order[slot] = (int)i;
+}
+
+// order every bin by user index (makes the internal order, hence every later summation order, reproducible)
+__global__ void k_bin_sort(long N, const int *__restrict__ atom_bin, const int *__restrict__ bin_start,
+                           const int *__restrict__ tmp_order, const double *__restrict__ xw, int *__restrict__ perm,
+                           int *__restrict__ inv, double *__restrict__ xs) {
+    long s = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    int u = tmp_order[s];
+    int bin = atom_bin[u];
+    int b0 = bin_start[bin], b1 = bin_start[bin + 1];
+    int rank = 0;
+    for (int t = b0; t < b1; ++t) rank += tmp_order[t] < u;
+    int dst = b0 + rank;
+    perm[dst] = u;
+    inv[u] = dst;
+    xs[3 * (long)dst + 0] = xw[3 * (long)u + 0];
+    xs[3 * (long)dst + 1] = xw[3 * (long)u + 1];
+    xs[3 * (long)dst + 2] = xw[3 * (long)u + 2];
+}
+
+__device__ __forceinline__ double min_image(double t, double L, double halfL) {
+    double s = t > halfL ? -1.0 : (t < -halfL ? 1.0 : 0.0);
+    return __dadd_rn(t, __dmul_rn(s, L));
+}
+
+// One warp per (sorted) atom.  keys live in shared memory, cap entries per warp.
+__global__ void __launch_bounds__(128)
+k_nlist(long N, int T, Grid3 g, double rc2, int cap, const int *__restrict__ bin_start,
+        const double *__restrict__ xs, const int *__restrict__ perm, const int *__restrict__ inv,
+        int Nm, int4 sel4, int *__restrict__ nlist, int *__restrict__ nreal, int *__restrict__ status) {
+    extern __shared__ unsigned long long keys_all[];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const long i = blockIdx.x * 4L + wid;
+    if (i >= N) return;
+    unsigned long long *keys = keys_all + (size_t)wid * cap;
+    const int sel[4] = {sel4.x, sel4.y, sel4.z, sel4.w};
+    const double xi = xs[3 * i], yi = xs[3 * i + 1], zi = xs[3 * i + 2];
+    const int cx = cell_of(xi, g.inv_cw[0], g.nc[0]), cy = cell_of(yi, g.inv_cw[1], g.nc[1]),
+              cz = cell_of(zi, g.inv_cw[2], g.nc[2]);
+    const int lo0 = g.nc[0] >= 3 ? -1 : 0, hi0 = g.nc[0] >= 2 ? 1 : 0;
+    const int lo1 = g.nc[1] >= 3 ? -1 : 0, hi1 = g.nc[1] >= 2 ? 1 : 0;
+    const int lo2 = g.nc[2] >= 3 ? -1 : 0, hi2 = g.nc[2] >= 2 ? 1 : 0;
+    const double hx = 0.5 * g.L[0], hy = 0.5 * g.L[1], hz = 0.5 * g.L[2];
+    bool truncated = false;
+    int off = 0;
+    for (int b = 0; b < T; ++b) {
+        int n = 0;
+        for (int ox = lo0; ox <= hi0; ++ox) {
+            int ax = cx + ox; ax += ax < 0 ? g.nc[0] : 0; ax -= ax >= g.nc[0] ? g.nc[0] : 0;
+            for (int oy = lo1; oy <= hi1; ++oy) {
+                int ay = cy + oy; ay += ay < 0 ? g.nc[1] : 0; ay -= ay >= g.nc[1] ? g.nc[1] : 0;
+                for (int oz = lo2; oz <= hi2; ++oz) {
+                    int az = cz + oz; az += az < 0 ? g.nc[2] : 0; az -= az >= g.nc[2] ? g.nc[2] : 0;
+                    const int bin = b * g.ncell + (ax * g.nc[1] + ay) * g.nc[2] + az;
+                    const int s0 = bin_start[bin], s1 = bin_start[bin + 1];
+                    for (int base = s0; base < s1; base += 32) {
+                        const int s = base + lane;
+                        bool ok = false;
+                        unsigned long long key = 0;
+                        if (s < s1 && s != i) {
+                            double dx = min_image(__dsub_rn(xs[3 * (long)s], xi), g.L[0], hx);
+                            double dy = min_image(__dsub_rn(xs[3 * (long)s + 1], yi), g.L[1], hy);
+                            double dz = min_image(__dsub_rn(xs[3 * (long)s + 2], zi), g.L[2], hz);
+                            double r2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
+                            if (r2 < rc2) {
+                                ok = true;
+                                key = (__double2ull_rd(r2 * 536870912.0) << 24) | (unsigned long long)perm[s];
+                            }
+                        }
+                        const unsigned mask = __ballot_sync(0xffffffffu, ok);
+                        const int pos = n + __popc(mask & ((1u << lane) - 1u));
+                        if (ok && pos < cap) keys[pos] = key;
+                        n += __popc(mask);
+                    }
+                }
+            }
+        }
+        if (n > cap) { if (lane == 0) atomicOr(&status[0], 2); n = cap; }
+        int P = 32;
+        while (P < n) P <<= 1;
+        for (int k = n + lane; k < P; k += 32) keys[k] = ~0ull;
+        __syncwarp();
+        for (int k = 2; k <= P; k <<= 1) {
+            for (int j = k >> 1; j > 0; j >>= 1) {
+                for (int idx = lane; idx < P; idx += 32) {
+                    const int ixj = idx ^ j;
+                    if (ixj > idx) {
+                        const unsigned long long a = keys[idx], c = keys[ixj];
+                        const bool asc = (idx & k) == 0;
+                        if ((a > c) == asc) { keys[idx] = c; keys[ixj] = a; }
+                    }
+                }
+                __syncwarp();
+            }
+        }
+        const int nkeep = n < sel[b] ? n : sel[b];
+        for (int k = lane; k < sel[b]; k += 32)
+            nlist[i * Nm + off + k] = k < nkeep ? inv[(int)(keys[k] & 0xFFFFFFull)] : -1;
+        if (lane == 0) nreal[i * T + b] = nkeep;
+        truncated |= n > sel[b];
+        off += sel[b];
+        __syncwarp();
+    }
+    if (truncated && lane == 0) atomicAdd(&status[1], 1);
+}
+
+__global__ void k_get_nlist(long N, int Nm, const int *__restrict__ nlist, const int *__restrict__ perm,
+                            int *__restrict__ out) {
+    long t = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (t >= N * Nm) return;
+    long i = t / Nm;
+    int k = (int)(t - i * Nm);
+    int v = nlist[t];
+    out[(long)perm[i] * Nm + k] = v >= 0 ? perm[v] : -1;
+}
+
+}  // namespace
+
+cudaError_t launch_build_cells(const dp_model *m, long N, const double *coords, const int *types, const Grid3 &g,
+                               char *ws, const WsLayout &L, cudaStream_t st) {
+    const int nbins = m->T * g.ncell;
+    int *status = (int *)(ws + L.status);
+    int *cnt = (int *)(ws + L.bin_count), *start = (int *)(ws + L.bin_start), *cursor = (int *)(ws + L.bin_cursor);
+    cudaMemsetAsync(cnt, 0, sizeof(int) * (size_t)(nbins + 1), st);
+    cudaMemsetAsync(cursor, 0, sizeof(int) * (size_t)nbins, st);
+    const int nb = (int)((N + 255) / 256);
+    k_wrap_bin<<<nb, 256, 0, st>>>(N, coords, types, m->type_map_dev, m->n_type_map, g, (double *)(ws + L.xw),
+                                   (int *)(ws + L.atom_bin), cnt, status);
+    k_scan<<<1, 1024, 0, st>>>(nbins, cnt, start);
+    k_scatter<<<nb, 256, 0, st>>>(N, (int *)(ws + L.atom_bin), start, cursor, (int *)(ws + L.tmp_order));
+    k_bin_sort<<<nb, 256, 0, st>>>(N, (int *)(ws + L.atom_bin), start, (int *)(ws + L.tmp_order),
+                                   (double *)(ws + L.xw), (int *)(ws + L.perm), (int *)(ws + L.inv),
+                                   (double *)(ws + L.xs));
+    return cudaGetLastError();
+}
+
+cudaError_t launch_nlist(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    const int cap = m->sort_cap;
+    const size_t smem = (size_t)4 * cap * sizeof(unsigned long long);
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(k_nlist, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 4096 * 8);
+        attr_set = true;
+    }
+    int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
+    k_nlist<<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, m->T, g, m->rc * m->rc, cap, (int *)(ws + L.bin_start),
+                                                       (double *)(ws + L.xs), (int *)(ws + L.perm),
+                                                       (int *)(ws + L.inv), m->Nm, sel4, (int *)(ws + L.nlist),
+                                                       (int *)(ws + L.nreal), (int *)(ws + L.status));
+    return cudaGetLastError();
+}
+
+cudaError_t launch_get_nlist(const dp_model *m, long N, char *ws, const WsLayout &L, int *out, cudaStream_t st) {
+    long tot = N * m->Nm;
+    k_get_nlist<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(N, m->Nm, (int *)(ws + L.nlist), (int *)(ws + L.perm), out);
+    return cudaGetLastError();
+}
