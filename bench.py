@@ -1,0 +1,267 @@
+#!/usr/bin/env python
+"""Benchmark of the DP energy/force/virial hot path (BASELINE.json metric: atom-steps/s on one B200).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..4] [--impl ours|reference]
+
+One "step" = one dp_compute (all of SURVEY.md section 8(a): cell list, formatted neighbour list, environment
+matrix, embedding net + contraction, fitting net forward/backward, embedding backward, ProdForce, ProdViral)
+on one seeded synthetic configuration.  The path does not shard (BASELINE north_star: one GPU, no
+collectives): with --gpus N every rank runs an independent replica ("replicas only") and the
+value is the aggregate, scaling "weak".  Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+# algorithmic flops (FMA = 2, tanh not counted, no credit for padding or recomputation)
+FLOP_ROW_FWD = 12550 + 800          # embedding GEMMs forward + contraction forward, per neighbour row
+FLOP_ROW_BWD = 12550 + 1600         # embedding GEMMs backward + contraction backward, per neighbour row
+FLOP_ATOM_FIT = 2036160             # fitting fwd + bwd + descriptor fwd/bwd, per atom
+FP64_OVER_BF16_NOMINAL = 45.0 / 2250.0   # guide's nominal dense ratio: B200 FP64 tensor 45 TF vs bf16 2250 TF
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm=d["hbm_gbs"], bf16=d["bf16_tflops"], bf16_sus=d.get("bf16_tflops_sustained", d["bf16_tflops"]),
+                    src="measured (MEASURED_PEAKS.json)")
+    return dict(hbm=6650.0, bf16=1590.0, bf16_sus=1400.0, src="fallback (B200_PROFILING.md)")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows = []
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([t.strip() for t in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(s, ncen):
+    """Time the oracle, as it stands, on ncen evenly spaced centres of the workload (host cores)."""
+    from oracle import oracle
+    cen = np.unique(np.linspace(0, s.natoms - 1, ncen).astype(np.int64))
+    t0 = time.perf_counter()
+    oracle.evaluate(s.coords, s.types, s.box, s.model, centers=cen)
+    dt = time.perf_counter() - t0
+    return len(cen), dt, oracle.num_threads()
+
+
+def run_reference(args, s):
+    """--impl reference: the CPU oracle on a bounded sample per step (a deliberately slow program)."""
+    ncen = 256 if s.natoms > 2000 else min(s.natoms, 256)
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample(s, ncen)
+    tot = 0.0
+    n = 0
+    cores = 1
+    for _ in range(args.steps):
+        n, dt, cores = oracle_sample(s, ncen)
+        tot += dt
+    val = n * args.steps / tot
+    line = {"impl": "reference", "metric": "atom_steps_per_s", "value": val, "unit": "atom-steps/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": s.name, "natoms": s.natoms, "precision": "fp64 oracle"},
+            "cpu_baseline": {"value": val, "unit": "atom-steps/s", "cores": cores, "kind": "oracle",
+                             "sample": f"{n} evenly spaced centre atoms of {s.name} per step (brute-force list + full E_i and slot gradients)"},
+            "e2e": {"value": val, "unit": "atom-steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default: c2, copper 13,500 fp64)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    from paper_2005_00223_b200 import synth
+    if args.impl == "reference":
+        if rank == 0:
+            run_reference(args, synth.config(args.config))
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2005_00223_b200 import binding
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    s = synth.config(args.config)
+    N = s.natoms
+    model = binding.DPModel(s.model, s.precision)
+    coords_h = torch.from_numpy(s.coords).pin_memory()
+    types_h = torch.from_numpy(s.types).pin_memory()
+    coords = coords_h.to(dev)
+    types = types_h.to(dev)
+    out = model.compute(coords, types, s.box)
+    rc, ntr = model.status()
+    if rc != 0:
+        raise SystemExit(f"dp_status = {rc}")
+    nl = model.get_nlist()
+    real_rows = int((nl >= 0).sum().item())
+    rows_f, rows_b = model.last_row_counts()
+    del nl
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > L2 (126 MB)
+    st = torch.cuda.current_stream(dev)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+
+    for _ in range(args.warmup):
+        model.compute(coords, types, s.box, out=out)
+    model.profile_enable(True)
+    K = args.steps
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    phases = np.zeros(5)
+    sampler = ClockSampler(local_rank)
+    barrier()
+    sampler.start()
+    for k in range(K):
+        flush.fill_(k & 0xFF)                      # L2 flush, outside the timed events
+        ev[k][0].record(st)
+        model.compute(coords, types, s.box, out=out)
+        ev[k][1].record(st)
+        phases += model.profile_read()             # synchronises; the gap is outside the timed events
+    barrier()
+    clocks = sampler.stop()
+    model.profile_enable(False)
+    t_ms = sum(a.elapsed_time(b) for a, b in ev)
+    phases /= K
+
+    # end to end through the public API with HOST buffers: H2D of inputs, compute, D2H of results, every step
+    res_h = dict(energy=torch.empty(1, dtype=torch.float64).pin_memory(),
+                 forces=torch.empty((N, 3), dtype=torch.float64).pin_memory(),
+                 virial=torch.empty(9, dtype=torch.float64).pin_memory(),
+                 atom_energy=torch.empty(N, dtype=torch.float64).pin_memory())
+    cdev = torch.empty_like(coords)
+    tdev = torch.empty_like(types)
+
+    def e2e_step():
+        cdev.copy_(coords_h, non_blocking=True)
+        tdev.copy_(types_h, non_blocking=True)
+        model.compute(cdev, tdev, s.box, out=out)
+        for k_, v in res_h.items():
+            v.copy_(out[k_], non_blocking=True)
+
+    e2e_step()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(st)
+    for k in range(K):
+        e2e_step()
+    e1.record(st)
+    barrier()
+    e2e_ms = e0.elapsed_time(e1)
+    h2d = N * 24 + N * 4
+    d2h = 8 + N * 24 + 72 + N * 8
+
+    tt = torch.tensor([t_ms, e2e_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    t_ms, e2e_ms = float(tt[0]), float(tt[1])
+
+    if rank == 0:
+        pk = peaks()
+        ms_step = t_ms / K
+        value = world * N * K / (t_ms * 1e-3)
+        fp64_peak = pk["bf16_sus"] * FP64_OVER_BF16_NOMINAL
+        dom_flops = real_rows * FLOP_ROW_BWD
+        ach = dom_flops / (phases[3] * 1e-3) / 1e12
+        kern = {"nlist_ms": phases[0], "embed_fwd_ms": phases[1], "fit_ms": phases[2], "embed_bwd_ms": phases[3],
+                "finalize_ms": phases[4],
+                "embed_fwd_tflops": real_rows * FLOP_ROW_FWD / (phases[1] * 1e-3) / 1e12,
+                "fit_tflops": N * FLOP_ATOM_FIT / (phases[2] * 1e-3) / 1e12,
+                "embed_bwd_tflops": ach,
+                "step_tflops": (real_rows * (FLOP_ROW_FWD + FLOP_ROW_BWD) + N * FLOP_ATOM_FIT) / (ms_step * 1e-3) / 1e12}
+        line = {"metric": "atom_steps_per_s", "value": value, "unit": "atom-steps/s", "n_gpus": world, "steps": K,
+                "warmup": args.warmup, "ms_per_step": ms_step, "s_per_step_per_atom": ms_step * 1e-3 / N,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": {"fp64": "f64", "mix32": "f32", "mix16": "f16"}[s.precision], "data": "synthetic",
+                "config": {"workload": s.name, "natoms": N, "precision": s.precision, "nm": s.model.nm,
+                           "real_neighbour_rows": real_rows, "rows_through_embedding_fwd": rows_f,
+                           "rows_through_embedding_bwd": rows_b, "n_truncated_atoms": ntr,
+                           "parallelism": "replicas only" if world > 1 else "single GPU",
+                           "l2": "256 MB flush between timed steps, per-step CUDA events"},
+                "clocks": clocks,
+                "e2e": {"value": world * N * K / (e2e_ms * 1e-3), "unit": "atom-steps/s", "h2d_bytes_per_step": h2d,
+                        "d2h_bytes_per_step": d2h},
+                "gpu_launches": model.launches_per_compute() * K,
+                "roofline": {"kernel": "k_embed_bwd_f64", "bound": "tensor", "achieved": ach, "peak": fp64_peak,
+                             "unit": "TFLOP/s", "frac": ach / fp64_peak, "traffic": None,
+                             "peak_source": f"{pk['src']}: bf16 sustained {pk['bf16_sus']} TF/s x nominal fp64/bf16 ratio 45/2250",
+                             "flops_per_launch": dom_flops,
+                             "note": "algorithmic backward flops (14,150 per real neighbour row); the in-kernel forward recompute is not credited"},
+                "kernels": kern}
+        if world == 1 and not args.no_cpu_baseline:
+            ncen = min(N, 4096)
+            n, dt, cores = oracle_sample(s, ncen)
+            line["cpu_baseline"] = {"value": n / dt, "unit": "atom-steps/s", "cores": cores, "kind": "oracle",
+                                    "sample": f"{n} evenly spaced centre atoms of {s.name}, one evaluation ({dt:.1f} s)"}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

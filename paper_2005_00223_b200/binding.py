@@ -17,7 +17,8 @@ _lib = None
 DP_FP64, DP_MIX32, DP_MIX16 = 0, 1, 2
 PRECISIONS = {"fp64": DP_FP64, "mix32": DP_MIX32, "mix16": DP_MIX16}
 EXPORTS = ["dp_create", "dp_workspace_bytes", "dp_compute", "dp_get_nlist", "dp_status",
-           "dp_launches_per_compute", "dp_last_row_counts", "dp_destroy", "dp_strerror"]
+           "dp_launches_per_compute", "dp_last_row_counts", "dp_profile_enable", "dp_profile_read", "dp_destroy",
+           "dp_strerror"]
 
 
 class DPError(RuntimeError):
@@ -59,6 +60,10 @@ def lib():
         L.dp_launches_per_compute.argtypes = [vp]
         L.dp_last_row_counts.restype = C.c_int
         L.dp_last_row_counts.argtypes = [vp, C.POINTER(C.c_long), C.POINTER(C.c_long)]
+        L.dp_profile_enable.restype = C.c_int
+        L.dp_profile_enable.argtypes = [vp, C.c_int]
+        L.dp_profile_read.restype = C.c_int
+        L.dp_profile_read.argtypes = [vp, dp]
         L.dp_destroy.restype = None
         L.dp_destroy.argtypes = [vp]
         _lib = L
@@ -156,6 +161,19 @@ class DPModel:
         if rc != 0:
             raise DPError(rc, "dp_last_row_counts")
         return int(a.value), int(b.value)
+
+    def profile_enable(self, on=True):
+        rc = lib().dp_profile_enable(self._h, 1 if on else 0)
+        if rc != 0:
+            raise DPError(rc, "dp_profile_enable")
+
+    def profile_read(self):
+        """Per-phase milliseconds of the last compute: nlist, embed_fwd, fit, embed_bwd, finalize."""
+        ms = np.zeros(5)
+        rc = lib().dp_profile_read(self._h, _dptr(ms))
+        if rc != 0:
+            raise DPError(rc, "dp_profile_read")
+        return ms
 
     def close(self):
         if self._h:

@@ -242,6 +242,7 @@ void dp_destroy(dp_model *m) {
     void *ptrs[] = {m->type_map_dev, m->embed_frag_dev, m->avg_dev, m->std_dev, m->ebias_dev, m->fitV1_dev, m->fitV2_dev,
                     m->fitV3_dev, m->fitc1_dev, m->fitc2_dev, m->fitc3_dev, m->fitv4_dev, m->fitc4_dev};
     for (void *p : ptrs) if (p) cudaFree(p);
+    if (m->ev[0]) for (int k = 0; k <= DP_NPHASES; ++k) cudaEventDestroy(m->ev[k]);
     delete m;
 }
 
@@ -271,14 +272,42 @@ int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *ty
     ok(cudaMemsetAsync(ws + L.fsorted, 0, sizeof(double) * 3 * (size_t)natoms, st));
     ok(cudaMemsetAsync(ws + L.virial, 0, sizeof(double) * 16, st));
     ok(cudaMemsetAsync(energy_dev, 0, sizeof(double), st));
+    auto mark = [&](int k) { if (m->profile) ok(cudaEventRecord(m->ev[k], st)); };
+    mark(0);
     ok(launch_build_cells(m, natoms, coords_dev, types_dev, g, ws, L, st));
     ok(launch_nlist(m, natoms, g, ws, L, st));
+    mark(1);
     ok(launch_embed_fwd_f64(m, natoms, g, ws, L, st));
+    mark(2);
     ok(launch_fit_f64(m, natoms, g, ws, L, st));
+    mark(3);
     ok(launch_embed_bwd_f64(m, natoms, g, ws, L, st));
+    mark(4);
     ok(launch_finalize(m, natoms, ws, L, energy_dev, atom_energy_dev, forces_dev, virial_dev, st));
+    mark(5);
     m->last_natoms = natoms; m->last_ws = workspace_dev; m->last_stream = st;
     return e == cudaSuccess ? DP_OK : DP_ECUDA;
+}
+
+int dp_profile_enable(dp_model *m, int on) {
+    if (!m) return DP_EINVAL;
+    if (on && !m->ev[0]) {
+        for (int k = 0; k <= DP_NPHASES; ++k)
+            if (cudaEventCreate(&m->ev[k]) != cudaSuccess) return DP_ECUDA;
+    }
+    m->profile = on ? 1 : 0;
+    return DP_OK;
+}
+
+int dp_profile_read(dp_model *m, double *ms_host) {
+    if (!m || !ms_host || !m->profile || !m->last_ws) return DP_EINVAL;
+    if (cudaEventSynchronize(m->ev[DP_NPHASES]) != cudaSuccess) return DP_ECUDA;
+    for (int k = 0; k < DP_NPHASES; ++k) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, m->ev[k], m->ev[k + 1]) != cudaSuccess) return DP_ECUDA;
+        ms_host[k] = ms;
+    }
+    return DP_OK;
 }
 
 int dp_get_nlist(dp_model *m, int *nlist_dev, void *cuda_stream) {

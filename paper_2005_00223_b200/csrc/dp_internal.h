@@ -57,6 +57,8 @@ struct dp_model {
     void *last_ws;
     cudaStream_t last_stream;
     int sort_cap;
+    int profile;
+    cudaEvent_t ev[DP_NPHASES + 1];
 };
 
 // Workspace carve-up (all offsets 256-byte aligned), filled by dp_ws_layout().
