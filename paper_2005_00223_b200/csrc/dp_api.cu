@@ -2,11 +2,12 @@
 // workspace carve-up (the caller-owned "trunk"), kernel sequencing on the caller's stream.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
 
-#include "dp_internal.h"
+#include "embed_mix.cuh"
 
 namespace {
 
@@ -31,10 +32,13 @@ WsLayout ws_layout(const dp_model *m, long N) {
     L.xw = take(sizeof(double) * 3 * (size_t)N);
     L.nlist = take(sizeof(int) * (size_t)N * m->Nm);
     L.nreal = take(sizeof(int) * (size_t)N * m->T);
-    L.A = take(sizeof(double) * (size_t)N * 4 * M2E);
-    L.gAf = take(sizeof(double) * (size_t)N * 3 * NT3 * 32);
-    L.fit_act = take(sizeof(double) * (size_t)N * 240 * 7);
-    L.gD = take(sizeof(double) * (size_t)N * M2E * 16);
+    const size_t esz = m->prec == DP_FP64 ? sizeof(double) : sizeof(float);
+    L.A = take(esz * (size_t)N * 4 * M2E);
+    if (m->prec == DP_FP64) L.gAf = take(sizeof(double) * (size_t)N * 3 * NT3 * 32);
+    else L.gAf = take(sizeof(uint32_t) * (size_t)N * 2 * 28 * 32);
+    L.gscale = take(sizeof(float) * (size_t)N);
+    L.fit_act = take(esz * (size_t)N * 240 * 7);
+    L.gD = take(esz * (size_t)N * M2E * 16);
     L.eatom = take(sizeof(double) * (size_t)N);
     L.fsorted = take(sizeof(double) * 3 * (size_t)N);
     L.virial = take(sizeof(double) * 16);
@@ -108,6 +112,67 @@ void build_embed_frag(const double *net, EmbedNetFrag<TW> *out) {
             }
 }
 
+inline uint32_t hbits2(float x, float y) {
+    return (uint32_t)__half_as_ushort(__float2half_rn(x)) | ((uint32_t)__half_as_ushort(__float2half_rn(y)) << 16);
+}
+// part 0: fp16(x); part 1: fp16(x - fp16(x))
+inline float hpart(double x, int part) {
+    float xf = (float)x;
+    float hi = __half2float(__float2half_rn(xf));
+    return part == 0 ? hi : xf - hi;
+}
+
+template <int NSW>
+void build_embed_frag_h(const double *net, EmbedNetFragH<NSW> *out) {
+    const double *W1 = net, *b1 = W1 + M0, *W2 = b1 + M0, *b2 = W2 + M0 * M1, *W3 = b2 + M1, *b3 = W3 + M1 * M2E;
+    std::memset(out, 0, sizeof(*out));
+    for (int e = 0; e < M0; ++e) { out->w1[e] = (float)W1[e]; out->b1[e] = (float)b1[e]; }
+    for (int nt = 0; nt < HNT2; ++nt)
+        for (int r = 0; r < 4; ++r)
+            for (int j = 0; j < 2; ++j) { int f = h_f2(nt, r, j); if (f >= 0) out->b2[nt * 8 + 2 * r + j] = (float)b2[f]; }
+    for (int nt = 0; nt < HNT3; ++nt)
+        for (int r = 0; r < 4; ++r)
+            for (int j = 0; j < 2; ++j) { int f = h_f3(nt, r, j); if (f >= 0) out->b3[nt * 8 + 2 * r + j] = (float)b3[f]; }
+    auto w2 = [&](int e, int f) { return (e >= 0 && e < M0 && f >= 0) ? W2[e * M1 + f] : 0.0; };
+    auto w3 = [&](int fi, int fo) { return (fi >= 0 && fo >= 0) ? W3[fi * M2E + fo] : 0.0; };
+    for (int p = 0; p < NSW; ++p)
+        for (int l = 0; l < 32; ++l) {
+            const int r = l & 3, g = l >> 2;
+            // layer 2 forward: K natural e = 16 s + 8 h + 2r + {0,1}; N position (nt, g/2, g%2)
+            for (int s = 0; s < 2; ++s)
+                for (int nt = 0; nt < HNT2; ++nt)
+                    for (int h = 0; h < 2; ++h) {
+                        int e0 = 16 * s + 8 * h + 2 * r, fo = h_f2(nt, g >> 1, g & 1);
+                        out->W2f[p][s][nt][l][h] = hbits2(hpart(w2(e0, fo), p), hpart(w2(e0 + 1, fo), p));
+                    }
+            // layer 3 forward: K positions of y2 (tile 2s + h, r, j); N position (nt3, g/2, g%2)
+            for (int s = 0; s < 4; ++s)
+                for (int nt3 = 0; nt3 < HNT3; ++nt3)
+                    for (int h = 0; h < 2; ++h) {
+                        int t = 2 * s + h;
+                        if (t >= HNT2) continue;
+                        int fo = h_f3(nt3, g >> 1, g & 1);
+                        out->W3f[p][s][nt3][l][h] = hbits2(hpart(w3(h_f2(t, r, 0), fo), p), hpart(w3(h_f2(t, r, 1), fo), p));
+                    }
+            // layer 3 backward: K positions of G (tile 2s + h, r, j3); N position of y2 (nt2, g/2, g%2)
+            for (int s = 0; s < 7; ++s)
+                for (int nt2 = 0; nt2 < HNT2; ++nt2)
+                    for (int h = 0; h < 2; ++h) {
+                        int t = 2 * s + h, fi = h_f2(nt2, g >> 1, g & 1);
+                        out->W3Tf[p][s][nt2][l][h] = hbits2(hpart(w3(fi, h_f3(t, r, 0)), p), hpart(w3(fi, h_f3(t, r, 1)), p));
+                    }
+            // layer 2 backward: K positions of y2 (tile 2s + h, r, j2); N natural e = 8 t1 + g
+            for (int s = 0; s < 4; ++s)
+                for (int t1 = 0; t1 < 4; ++t1)
+                    for (int h = 0; h < 2; ++h) {
+                        int t = 2 * s + h;
+                        if (t >= HNT2) continue;
+                        int e = 8 * t1 + g;
+                        out->W2Tf[p][s][t1][l][h] = hbits2(hpart(w2(e, h_f2(t, r, 0)), p), hpart(w2(e, h_f2(t, r, 1)), p));
+                    }
+        }
+}
+
 template <typename Tp>
 cudaError_t upload(const std::vector<Tp> &h, void **dev) {
     cudaError_t e = cudaMalloc(dev, h.size() * sizeof(Tp));
@@ -179,7 +244,7 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
     if (w->embed_widths[0] != M0 || w->embed_widths[1] != M1 || w->embed_widths[2] != M2E || w->axis != 16 ||
         w->fit_widths[0] != 240 || w->fit_widths[1] != 240 || w->fit_widths[2] != 240)
         return DP_EUNSUPPORTED;
-    if (prec != DP_FP64) return DP_EUNSUPPORTED;
+    if (prec != DP_FP64 && prec != DP_MIX32 && prec != DP_MIX16) return DP_EINVAL;
     int maxsel = 0, Nm = 0;
     for (int b = 0; b < T; ++b) { if (sel[b] <= 0) return DP_EINVAL; Nm += sel[b]; if (sel[b] > maxsel) maxsel = sel[b]; }
     for (int k = 0; k < n_type_map; ++k) if (type_map[k] >= T) return DP_EINVAL;
@@ -192,6 +257,16 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
     std::memset(m, 0, sizeof(*m));
     m->T = T; m->Nm = Nm; m->axis = 16; m->F = 240; m->rc = rc; m->rc_smth = rc_smth; m->prec = prec;
     m->n_type_map = n_type_map;
+    if (prec == DP_MIX32) { m->mix_ns = 3; m->mix_nsc = 3; m->mix_tanh_approx = 0; m->mix_fit_ns = 3; m->mix_fit3_ns = 3; }
+    if (prec == DP_MIX16) {
+        // defaults from the precision study in DESIGN.md: fp16 weights, activations carried as hi + lo fp16 pairs
+        m->mix_ns = 2; m->mix_nsc = 3; m->mix_tanh_approx = 1; m->mix_fit_ns = 2; m->mix_fit3_ns = 2;
+        if (const char *e = std::getenv("DP_MIX16_NS")) { int v = std::atoi(e); if (v >= 1 && v <= 4) m->mix_ns = v; }
+        if (const char *e = std::getenv("DP_MIX16_NSC")) m->mix_nsc = std::atoi(e) == 3 ? 3 : 1;
+        if (const char *e = std::getenv("DP_MIX16_TANH_APPROX")) m->mix_tanh_approx = std::atoi(e) ? 1 : 0;
+        if (const char *e = std::getenv("DP_MIX16_FIT_NS")) { int v = std::atoi(e); if (v >= 1 && v <= 3) m->mix_fit_ns = v; }
+        if (const char *e = std::getenv("DP_MIX16_FIT3_NS")) { int v = std::atoi(e); if (v >= 1 && v <= 3) m->mix_fit3_ns = v; }
+    }
     for (int b = 0; b < T; ++b) { m->sel[b] = sel[b]; m->off[b + 1] = m->off[b] + sel[b]; }
     int cap = 256;
     while (cap < 2 * maxsel) cap <<= 1;
@@ -207,9 +282,21 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
     std::vector<int> tm(type_map, type_map + n_type_map);
     ok(upload(tm, (void **)&m->type_map_dev));
     const size_t ensz = (size_t)M0 + M0 + M0 * M1 + M1 + M1 * M2E + M2E;
-    {
+    if (prec == DP_FP64) {
         std::vector<EmbedNetFrag<double>> frags((size_t)T * T);
         for (int ab = 0; ab < T * T; ++ab) build_embed_frag<double>(w->embed + ab * ensz, &frags[ab]);
+        ok(upload(frags, &m->embed_frag_dev));
+    } else if (prec == DP_MIX32) {
+        std::vector<EmbedNetFragH<2>> frags((size_t)T * T);
+        for (int ab = 0; ab < T * T; ++ab) build_embed_frag_h<2>(w->embed + ab * ensz, &frags[ab]);
+        ok(upload(frags, &m->embed_frag_dev));
+    } else if (ns_wparts(m->mix_ns) == 2) {
+        std::vector<EmbedNetFragH<2>> frags((size_t)T * T);
+        for (int ab = 0; ab < T * T; ++ab) build_embed_frag_h<2>(w->embed + ab * ensz, &frags[ab]);
+        ok(upload(frags, &m->embed_frag_dev));
+    } else {
+        std::vector<EmbedNetFragH<1>> frags((size_t)T * T);
+        for (int ab = 0; ab < T * T; ++ab) build_embed_frag_h<1>(w->embed + ab * ensz, &frags[ab]);
         ok(upload(frags, &m->embed_frag_dev));
     }
     const int ND = M2E * 16, F = 240;
@@ -227,9 +314,16 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
         std::memcpy(&v4[a * F], p, sizeof(double) * F); p += F;
         c4[a] = p[0];
     }
-    ok(upload(V1, &m->fitV1_dev)); ok(upload(V2, &m->fitV2_dev)); ok(upload(V3, &m->fitV3_dev));
-    ok(upload(c1, &m->fitc1_dev)); ok(upload(c2, &m->fitc2_dev)); ok(upload(c3, &m->fitc3_dev));
-    ok(upload(v4, &m->fitv4_dev)); ok(upload(c4, &m->fitc4_dev));
+    if (prec == DP_FP64) {
+        ok(upload(V1, &m->fitV1_dev)); ok(upload(V2, &m->fitV2_dev)); ok(upload(V3, &m->fitV3_dev));
+        ok(upload(c1, &m->fitc1_dev)); ok(upload(c2, &m->fitc2_dev)); ok(upload(c3, &m->fitc3_dev));
+        ok(upload(v4, &m->fitv4_dev)); ok(upload(c4, &m->fitc4_dev));
+    } else {   // "trained in double precision, and cast": fp32 copies, fp16 rounding happens per MMA operand
+        auto f32 = [](const std::vector<double> &v) { return std::vector<float>(v.begin(), v.end()); };
+        ok(upload(f32(V1), &m->fitV1_dev)); ok(upload(f32(V2), &m->fitV2_dev)); ok(upload(f32(V3), &m->fitV3_dev));
+        ok(upload(f32(c1), &m->fitc1_dev)); ok(upload(f32(c2), &m->fitc2_dev)); ok(upload(f32(c3), &m->fitc3_dev));
+        ok(upload(f32(v4), &m->fitv4_dev)); ok(upload(f32(c4), &m->fitc4_dev));
+    }
     std::vector<double> avg(w->avg, w->avg + 4 * T), sd(w->std, w->std + 4 * T), eb(w->ebias, w->ebias + T);
     ok(upload(avg, (void **)&m->avg_dev)); ok(upload(sd, (void **)&m->std_dev)); ok(upload(eb, (void **)&m->ebias_dev));
     if (e != cudaSuccess) { dp_destroy(m); return DP_ECUDA; }
@@ -277,11 +371,12 @@ int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *ty
     ok(launch_build_cells(m, natoms, coords_dev, types_dev, g, ws, L, st));
     ok(launch_nlist(m, natoms, g, ws, L, st));
     mark(1);
-    ok(launch_embed_fwd_f64(m, natoms, g, ws, L, st));
+    const bool f64 = m->prec == DP_FP64;
+    ok(f64 ? launch_embed_fwd_f64(m, natoms, g, ws, L, st) : launch_embed_fwd_mix(m, natoms, g, ws, L, st));
     mark(2);
-    ok(launch_fit_f64(m, natoms, g, ws, L, st));
+    ok(f64 ? launch_fit_f64(m, natoms, g, ws, L, st) : launch_fit_mix(m, natoms, g, ws, L, st));
     mark(3);
-    ok(launch_embed_bwd_f64(m, natoms, g, ws, L, st));
+    ok(f64 ? launch_embed_bwd_f64(m, natoms, g, ws, L, st) : launch_embed_bwd_mix(m, natoms, g, ws, L, st));
     mark(4);
     ok(launch_finalize(m, natoms, ws, L, energy_dev, atom_energy_dev, forces_dev, virial_dev, st));
     mark(5);

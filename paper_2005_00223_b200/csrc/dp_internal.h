@@ -57,6 +57,9 @@ struct dp_model {
     void *last_ws;
     cudaStream_t last_stream;
     int sort_cap;
+    // mixed-mode variant knobs: operand parts of the net MMAs (1 = fp16, 3 = split), of the contraction-type MMAs,
+    // tanh.approx vs tanhf, and operand parts of fitting layers 1-2
+    int mix_ns, mix_nsc, mix_tanh_approx, mix_fit_ns, mix_fit3_ns;
     int profile;
     cudaEvent_t ev[DP_NPHASES + 1];
 };
@@ -77,7 +80,8 @@ struct WsLayout {
     size_t nlist;       // int[N][Nm] sorted-space indices
     size_t nreal;       // int[N][T]
     size_t A;           // double[N][4][100]   (float for mixed modes)
-    size_t gAf;         // gA fragments [N][42][32]
+    size_t gAf;         // gA fragments [N][42][32] doubles (fp64) / [N][NSW][28][32] words (mixed)
+    size_t gscale;      // float[N] power-of-two scale of the mixed gA fragments
     size_t fit_act;     // 7 activation buffers [N][240]
     size_t gD;          // [N][1600]
     size_t eatom;       // double[N] sorted order
@@ -102,5 +106,8 @@ cudaError_t launch_embed_bwd_f64(const dp_model *m, long N, const Grid3 &g, char
 cudaError_t launch_fit_f64(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_finalize(const dp_model *m, long N, char *ws, const WsLayout &L, double *energy, double *eatom,
                             double *forces, double *virial, cudaStream_t st);
+cudaError_t launch_embed_fwd_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+cudaError_t launch_embed_bwd_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 int embed_smem_bytes_fwd_f64();
 int embed_smem_bytes_bwd_f64();

@@ -1,0 +1,338 @@
+// S5 (descriptor) + S6 (fitting net forward and backward) in the mixed-precision modes.
+// GEMMs batched over the atoms of one centre type on fp16 tensor-core MMAs (m16n8k16) with fp32 accumulation;
+// NS = 1 rounds the operands to fp16, NS = 3 splits them (hi + lo) for single-precision products.
+// MIX-16: layers 1 and 2 (and their backward products) NS = 1, the third 240x240 layer NS = 3 and the output layer in
+// fp32 ("in the last layer of the fitting net, both data storage and arithmetic operations are kept in single
+// precision", reading Q16).  MIX-32: NS = 3 everywhere.  Activations are stored in fp32.
+#include "embed_mix.cuh"
+
+namespace {
+
+constexpr int BM = 128, BN = 80, BK = 16;      // K = 240 and 1600 are multiples of 16, not of 32
+constexpr int AS_STRIDE = BK + 8;       // floats: conflict-free float2 fragment loads
+constexpr int BS_STRIDE = BN + 4;       // B stored [k][n]
+constexpr int BT_STRIDE = BK + 8;       // B stored [n][k]
+constexpr int AS_TILE = BM * AS_STRIDE;
+constexpr int B_TILE = (BK * BS_STRIDE > BN * BT_STRIDE) ? BK * BS_STRIDE : BN * BT_STRIDE;
+constexpr int FIT_SMEM_BYTES = 2 * (AS_TILE + B_TILE) * 4;
+
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc, bool valid) {
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+    int sz = valid ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(s), "l"(gsrc), "r"(sz));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N)); }
+
+struct FitArgsF {
+    int ncell;
+    const int *bin_start;
+    int K, N;
+    const float *A; int lda;
+    const float *B; long b_type_stride; int ldb;
+    const float *bias; int bias_type_stride;
+    const float *v4; int v4_type_stride;
+    const float *aux0; const float *aux1;
+    float *out0; float *out1; int ldo;
+};
+
+template <bool SPLIT>
+__device__ __forceinline__ void cvt_pair(float x, float y, uint32_t &hi, uint32_t &lo) {
+    if (!SPLIT) { hi = pack_h2(x, y); lo = 0; }
+    else split_h2(x, y, hi, lo);
+}
+
+template <int MODE, int NS, bool APPROX>
+__global__ void __launch_bounds__(256) k_fitm_gemm(FitArgsF p) {
+    constexpr bool BT = MODE >= 3;
+    extern __shared__ __align__(16) float smf[];
+    const int a = blockIdx.z;
+    const int ts0 = p.bin_start[a * p.ncell], ts1 = p.bin_start[(a + 1) * p.ncell];
+    const int row0 = ts0 + blockIdx.y * BM;
+    if (row0 >= ts1) return;
+    const int n0 = blockIdx.x * BN;
+    const float *Bw = p.B + a * p.b_type_stride;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int wm = wid >> 1, wn = wid & 1;          // 4 x 2 warps, warp tile 32 x 40
+    const int g = lane >> 2, r = lane & 3;
+
+    auto load_tiles = [&](int stage, int k0) {
+        float *As = smf + stage * (AS_TILE + B_TILE);
+        float *Bs = As + AS_TILE;
+        for (int c = tid; c < BM * (BK / 4); c += 256) {
+            const int row = c / (BK / 4), c4 = c % (BK / 4);
+            const bool ok = row0 + row < ts1;
+            cp_async16(As + row * AS_STRIDE + 4 * c4, p.A + (long)(ok ? row0 + row : ts0) * p.lda + k0 + 4 * c4, ok);
+        }
+        if (!BT) {
+            for (int c = tid; c < BK * (BN / 4); c += 256) {
+                const int k = c / (BN / 4), cc = c % (BN / 4);
+                cp_async16(Bs + k * BS_STRIDE + 4 * cc, Bw + (long)(k0 + k) * p.ldb + n0 + 4 * cc, true);
+            }
+        } else {
+            for (int c = tid; c < BN * (BK / 4); c += 256) {
+                const int n = c / (BK / 4), c4 = c % (BK / 4);
+                cp_async16(Bs + n * BT_STRIDE + 4 * c4, Bw + (long)(n0 + n) * p.ldb + k0 + 4 * c4, true);
+            }
+        }
+        cp_async_commit();
+    };
+
+    float acc[2][5][4];
+#pragma unroll
+    for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+        for (int nt = 0; nt < 5; ++nt)
+#pragma unroll
+            for (int k = 0; k < 4; ++k) acc[mt][nt][k] = 0.f;
+
+    const int nk = p.K / BK;
+    load_tiles(0, 0);
+    for (int ks = 0; ks < nk; ++ks) {
+        if (ks + 1 < nk) { load_tiles((ks + 1) & 1, (ks + 1) * BK); cp_async_wait<1>(); }
+        else cp_async_wait<0>();
+        __syncthreads();
+        const float *As = smf + (ks & 1) * (AS_TILE + B_TILE);
+        const float *Bs = As + AS_TILE;
+#pragma unroll
+        for (int kk = 0; kk < BK / 16; ++kk) {
+            uint32_t ah[2][4], al[2][4], bh[5][2], bl[5][2];
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt) {
+                const float *ap = As + (wm * 32 + mt * 16 + g) * AS_STRIDE + kk * 16 + 2 * r;
+                const float2 x0 = *reinterpret_cast<const float2 *>(ap);
+                const float2 x1 = *reinterpret_cast<const float2 *>(ap + 8 * AS_STRIDE);
+                const float2 x2 = *reinterpret_cast<const float2 *>(ap + 8);
+                const float2 x3 = *reinterpret_cast<const float2 *>(ap + 8 * AS_STRIDE + 8);
+                cvt_pair<ns_asplit(NS)>(x0.x, x0.y, ah[mt][0], al[mt][0]); cvt_pair<ns_asplit(NS)>(x1.x, x1.y, ah[mt][1], al[mt][1]);
+                cvt_pair<ns_asplit(NS)>(x2.x, x2.y, ah[mt][2], al[mt][2]); cvt_pair<ns_asplit(NS)>(x3.x, x3.y, ah[mt][3], al[mt][3]);
+            }
+#pragma unroll
+            for (int nt = 0; nt < 5; ++nt) {
+                const int n = wn * 40 + nt * 8 + g;
+                if (BT) {
+                    const float *bp = Bs + n * BT_STRIDE + kk * 16 + 2 * r;
+                    const float2 y0 = *reinterpret_cast<const float2 *>(bp);
+                    const float2 y1 = *reinterpret_cast<const float2 *>(bp + 8);
+                    cvt_pair<ns_wsplit(NS)>(y0.x, y0.y, bh[nt][0], bl[nt][0]); cvt_pair<ns_wsplit(NS)>(y1.x, y1.y, bh[nt][1], bl[nt][1]);
+                } else {
+                    const float *bp = Bs + (kk * 16 + 2 * r) * BS_STRIDE + n;
+                    cvt_pair<ns_wsplit(NS)>(bp[0], bp[BS_STRIDE], bh[nt][0], bl[nt][0]);
+                    cvt_pair<ns_wsplit(NS)>(bp[8 * BS_STRIDE], bp[9 * BS_STRIDE], bh[nt][1], bl[nt][1]);
+                }
+            }
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+                for (int nt = 0; nt < 5; ++nt) {
+                    mma16816(acc[mt][nt], ah[mt][0], ah[mt][1], ah[mt][2], ah[mt][3], bh[nt][0], bh[nt][1]);
+                    if (ns_wsplit(NS)) mma16816(acc[mt][nt], ah[mt][0], ah[mt][1], ah[mt][2], ah[mt][3], bl[nt][0], bl[nt][1]);
+                    if (ns_asplit(NS)) mma16816(acc[mt][nt], al[mt][0], al[mt][1], al[mt][2], al[mt][3], bh[nt][0], bh[nt][1]);
+                }
+        }
+        __syncthreads();
+    }
+
+#pragma unroll
+    for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+        for (int hrow = 0; hrow < 2; ++hrow) {
+            const int row = row0 + wm * 32 + mt * 16 + g + 8 * hrow;
+            if (row >= ts1) continue;
+#pragma unroll
+            for (int nt = 0; nt < 5; ++nt) {
+                const int col = n0 + wn * 40 + nt * 8 + 2 * r;
+                const long o = (long)row * p.ldo + col;
+                const float v0 = acc[mt][nt][2 * hrow], v1 = acc[mt][nt][2 * hrow + 1];
+                if (MODE == 0) {
+                    const float *b = p.bias + a * p.bias_type_stride + col;
+                    *reinterpret_cast<float2 *>(p.out0 + o) = make_float2(act_tanh<APPROX>(v0 + b[0]), act_tanh<APPROX>(v1 + b[1]));
+                } else if (MODE == 1) {
+                    const float *b = p.bias + a * p.bias_type_stride + col;
+                    const float2 h = *reinterpret_cast<const float2 *>(p.aux0 + o);
+                    const float t0 = act_tanh<APPROX>(v0 + b[0]), t1 = act_tanh<APPROX>(v1 + b[1]);
+                    *reinterpret_cast<float2 *>(p.out0 + o) = make_float2(t0, t1);
+                    *reinterpret_cast<float2 *>(p.out1 + o) = make_float2(h.x + t0, h.y + t1);
+                } else if (MODE == 2) {
+                    const float *b = p.bias + a * p.bias_type_stride + col;
+                    const float *v4 = p.v4 + a * p.v4_type_stride + col;
+                    const float2 h = *reinterpret_cast<const float2 *>(p.aux0 + o);
+                    const float t0 = tanhf(v0 + b[0]), t1 = tanhf(v1 + b[1]);
+                    *reinterpret_cast<float2 *>(p.out0 + o) = make_float2(v4[0] * (1.f - t0 * t0), v4[1] * (1.f - t1 * t1));
+                    *reinterpret_cast<float2 *>(p.out1 + o) = make_float2(h.x + t0, h.y + t1);
+                } else if (MODE == 3) {
+                    const float *v4 = p.v4 + a * p.v4_type_stride + col;
+                    const float2 t = *reinterpret_cast<const float2 *>(p.aux0 + o);
+                    const float g0 = v4[0] + v0, g1 = v4[1] + v1;
+                    *reinterpret_cast<float2 *>(p.out0 + o) = make_float2(g0, g1);
+                    *reinterpret_cast<float2 *>(p.out1 + o) = make_float2(g0 * (1.f - t.x * t.x), g1 * (1.f - t.y * t.y));
+                } else if (MODE == 4) {
+                    const float2 gg = *reinterpret_cast<const float2 *>(p.aux0 + o);
+                    const float2 h = *reinterpret_cast<const float2 *>(p.aux1 + o);
+                    const float g0 = gg.x + v0, g1 = gg.y + v1;
+                    *reinterpret_cast<float2 *>(p.out0 + o) = make_float2(g0 * (1.f - h.x * h.x), g1 * (1.f - h.y * h.y));
+                } else {
+                    *reinterpret_cast<float2 *>(p.out0 + o) = make_float2(v0, v1);
+                }
+            }
+        }
+}
+
+__global__ void __launch_bounds__(256) k_descr_f(long N, const float *__restrict__ Amat, float *__restrict__ D) {
+    __shared__ float sA[8][4 * M2E];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const long i = blockIdx.x * 8L + wid;
+    if (i >= N) return;
+    for (int k = lane; k < 4 * M2E; k += 32) sA[wid][k] = Amat[i * 4 * M2E + k];
+    __syncwarp();
+    for (int idx = lane; idx < M2E * 16; idx += 32) {
+        const int m = idx >> 4, ax = idx & 15;
+        float acc = 0.f;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) acc = fmaf(sA[wid][c * M2E + m], sA[wid][c * M2E + ax], acc);
+        D[i * (M2E * 16) + idx] = acc;
+    }
+}
+
+__device__ __forceinline__ int type_of_sorted(int i, int T, int ncell, const int *bin_start) {
+    int a = 0;
+    for (int t = 1; t < T; ++t) a += i >= bin_start[t * ncell];
+    return a;
+}
+
+// E_i: last layer in fp32, result converted to fp64 and the fp64 energy bias added
+__global__ void __launch_bounds__(256) k_energy_f(long N, int T, int ncell, const int *__restrict__ bin_start,
+                                                  const float *__restrict__ h3, const float *__restrict__ v4,
+                                                  const float *__restrict__ c4, const double *__restrict__ ebias,
+                                                  double *__restrict__ eatom) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const long i = blockIdx.x * 8L + wid;
+    if (i >= N) return;
+    const int a = type_of_sorted((int)i, T, ncell, bin_start);
+    float acc = 0.f;
+    for (int n = lane; n < 240; n += 32) acc = fmaf(h3[i * 240 + n], v4[a * 240 + n], acc);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) eatom[i] = (double)(acc + c4[a]) + ebias[a];
+}
+
+// gA (fp32) -> scaled fp16 MMA fragments for the embedding backward (layout in embed_mix.cu)
+template <int NSW>
+__global__ void __launch_bounds__(128) k_gA_f(long N, const float *__restrict__ Amat, const float *__restrict__ gD,
+                                              uint32_t *__restrict__ gAf, float *__restrict__ gscale) {
+    extern __shared__ float smg[];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const long i = blockIdx.x * 4L + wid;
+    if (i >= N) return;
+    float *sA = smg + wid * (4 * M2E + M2E * 16 + 4 * M2E);
+    float *sG = sA + 4 * M2E;
+    float *sO = sG + M2E * 16;
+    for (int k = lane; k < 4 * M2E; k += 32) sA[k] = Amat[i * 4 * M2E + k];
+    for (int k = lane; k < M2E * 16; k += 32) sG[k] = gD[i * (M2E * 16) + k];
+    __syncwarp();
+    float mx = 0.f;
+    for (int idx = lane; idx < 4 * M2E; idx += 32) {
+        const int c = idx / M2E, m = idx % M2E;
+        float acc = 0.f;
+#pragma unroll
+        for (int ax = 0; ax < 16; ++ax) acc = fmaf(sG[m * 16 + ax], sA[c * M2E + ax], acc);
+        if (m < 16)
+            for (int mp = 0; mp < M2E; ++mp) acc = fmaf(sG[mp * 16 + m], sA[c * M2E + mp], acc);
+        sO[idx] = acc;
+        mx = fmaxf(mx, fabsf(acc));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    // power-of-two scale bringing max|gA| into [0.5, 1)
+    int ex = 0;
+    if (mx > 0.f) frexpf(mx, &ex);
+    const float sc = ldexpf(1.f, -ex);
+    if (lane == 0) gscale[i] = sc;
+    __syncwarp();
+    uint32_t *out = gAf + i * (2 * 28 * 32);
+    const int g = lane >> 2, r = lane & 3;
+    for (int nt3 = 0; nt3 < HNT3; ++nt3) {
+        const int f = h_f3(nt3, g >> 1, g & 1);
+        float x = 0.f, y = 0.f;
+        if (f >= 0 && r < 2) { x = sO[(2 * r) * M2E + f] * sc; y = sO[(2 * r + 1) * M2E + f] * sc; }
+        uint32_t hi, lo;
+        split_h2(x, y, hi, lo);
+        out[nt3 * 32 + lane] = hi;
+        if (NSW == 2) out[(28 + nt3) * 32 + lane] = lo;
+    }
+    for (int t = 0; t < HNT3; ++t) {
+        const int f0 = h_f3(t, r, 0), f1 = h_f3(t, r, 1);
+        float x = 0.f, y = 0.f;
+        if (f0 >= 0 && g < 4) { x = sO[g * M2E + f0] * sc; y = sO[g * M2E + f1] * sc; }
+        uint32_t hi, lo;
+        split_h2(x, y, hi, lo);
+        out[(14 + t) * 32 + lane] = hi;
+        if (NSW == 2) out[(28 + 14 + t) * 32 + lane] = lo;
+    }
+}
+
+template <int MODE, int NS, bool APPROX>
+void launch_gemm_t(const FitArgsF &p, dim3 grid, cudaStream_t st) {
+    static bool attr = false;
+    if (!attr) { cudaFuncSetAttribute(k_fitm_gemm<MODE, NS, APPROX>, cudaFuncAttributeMaxDynamicSharedMemorySize, FIT_SMEM_BYTES); attr = true; }
+    k_fitm_gemm<MODE, NS, APPROX><<<grid, 256, FIT_SMEM_BYTES, st>>>(p);
+}
+// ns: 1 fp16 operands, 2 activations split, 3 activations and weights split; apx: tanh.approx in the epilogue (modes 0, 1)
+template <int MODE>
+void launch_gemm(int ns, bool apx, const FitArgsF &p, dim3 grid, cudaStream_t st) {
+    constexpr bool HAS_TANH = MODE <= 1;
+    if (HAS_TANH && apx) {
+        if (ns == 1) launch_gemm_t<MODE, 1, HAS_TANH>(p, grid, st);
+        else if (ns == 2) launch_gemm_t<MODE, 2, HAS_TANH>(p, grid, st);
+        else launch_gemm_t<MODE, 3, HAS_TANH>(p, grid, st);
+    } else {
+        if (ns == 1) launch_gemm_t<MODE, 1, false>(p, grid, st);
+        else if (ns == 2) launch_gemm_t<MODE, 2, false>(p, grid, st);
+        else launch_gemm_t<MODE, 3, false>(p, grid, st);
+    }
+}
+
+}  // namespace
+
+cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    const int F = 240, ND = M2E * 16;
+    const int T = m->T;
+    const int ns12 = m->mix_fit_ns, ns3 = m->mix_fit3_ns;   // operand parts of layers 1-2 and of the third 240x240 layer
+    const bool apx = m->mix_tanh_approx != 0;
+    float *Amat = (float *)(ws + L.A);
+    float *D = (float *)(ws + L.gD);
+    float *act = (float *)(ws + L.fit_act);
+    const size_t S = (size_t)N * F;
+    float *h1 = act, *t2 = act + S, *h2 = act + 2 * S, *gz3 = act + 3 * S, *h3 = act + 4 * S, *g2 = act + 5 * S,
+          *gz2 = act + 6 * S, *gz1 = h2;
+    const int *bin_start = (const int *)(ws + L.bin_start);
+    const float *V1 = (const float *)m->fitV1_dev, *V2 = (const float *)m->fitV2_dev, *V3 = (const float *)m->fitV3_dev;
+    const float *c1 = (const float *)m->fitc1_dev, *c2 = (const float *)m->fitc2_dev, *c3 = (const float *)m->fitc3_dev;
+    const float *v4 = (const float *)m->fitv4_dev, *c4 = (const float *)m->fitc4_dev;
+    const unsigned gy = (unsigned)((N + BM - 1) / BM);
+    const unsigned nb8 = (unsigned)((N + 7) / 8);
+
+    k_descr_f<<<nb8, 256, 0, st>>>(N, Amat, D);
+    FitArgsF p{};
+    p.ncell = g.ncell; p.bin_start = bin_start; p.v4 = v4; p.v4_type_stride = F; p.bias_type_stride = F;
+    p.K = ND; p.N = F; p.A = D; p.lda = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.ldb = F; p.bias = c1;
+    p.out0 = h1; p.ldo = F;
+    const dim3 g240(F / BN, gy, T), g1600(ND / BN, gy, T);
+    launch_gemm<0>(ns12, apx, p, g240, st);
+    p.K = F; p.A = h1; p.lda = F; p.B = V2; p.b_type_stride = (long)F * F; p.bias = c2; p.aux0 = h1; p.out0 = t2; p.out1 = h2;
+    launch_gemm<1>(ns12, apx, p, g240, st);
+    p.A = h2; p.B = V3; p.bias = c3; p.aux0 = h2; p.out0 = gz3; p.out1 = h3;
+    launch_gemm<2>(ns3, false, p, g240, st);
+    k_energy_f<<<nb8, 256, 0, st>>>(N, T, g.ncell, bin_start, h3, v4, c4, m->ebias_dev, (double *)(ws + L.eatom));
+    p.A = gz3; p.B = V3; p.aux0 = t2; p.out0 = g2; p.out1 = gz2;
+    launch_gemm<3>(ns3, false, p, g240, st);
+    p.A = gz2; p.B = V2; p.aux0 = g2; p.aux1 = h1; p.out0 = gz1; p.out1 = nullptr;
+    launch_gemm<4>(ns12, false, p, g240, st);
+    p.A = gz1; p.N = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.out0 = D; p.ldo = ND;
+    launch_gemm<5>(ns12, false, p, g1600, st);
+    const int smem = 4 * (4 * M2E + M2E * 16 + 4 * M2E) * 4;
+    if (m->mix_nsc == 1) k_gA_f<1><<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, Amat, D, (uint32_t *)(ws + L.gAf), (float *)(ws + L.gscale));
+    else k_gA_f<2><<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, Amat, D, (uint32_t *)(ws + L.gAf), (float *)(ws + L.gscale));
+    return cudaGetLastError();
+}

@@ -75,3 +75,75 @@ def test_ragged_small_and_padded_blocks():
     o = oracle.evaluate(s.coords, s.types, s.box, s.model)
     g = _gpu_eval(s)
     _check_fp64(g, o)
+
+
+# ------------------------------------------------------------------ mixed precision, BASELINE tolerances
+def _check_forces(g, o, tol):
+    rms = np.sqrt((o["forces"] ** 2).mean())
+    err = np.abs(g["forces"] - o["forces"]).max()
+    assert err <= tol * rms, (err / rms, tol)
+
+
+def test_water_mix32_and_mix16_full_parity():
+    """config 1 geometry in both mixed modes: list bit-exact, MIX-32 1e-4 RMS(F), MIX-16 5e-3 RMS(F)."""
+    s = synth.config(1)
+    o = oracle.evaluate(s.coords, s.types, s.box, s.model)
+    for prec, tol, tolE in (("mix32", 1e-4, 2e-5), ("mix16", 5e-3, 1e-3)):
+        g = _gpu_eval(s, prec)
+        assert np.array_equal(g["nlist"], o["nlist"])
+        _check_forces(g, o, tol)
+        assert abs(g["energy"][0] - o["energy"]) / s.natoms <= tolE          # eV per atom
+        vmax = np.abs(o["virial"]).max()
+        assert np.abs(g["virial"] - o["virial"]).max() <= tol * vmax
+
+
+def test_copper_mix16_parity_config0_geometry():
+    s = synth.config(0)
+    o = oracle.evaluate(s.coords, s.types, s.box, s.model)
+    g = _gpu_eval(s, "mix16")
+    assert np.array_equal(g["nlist"], o["nlist"])
+    _check_forces(g, o, 5e-3)
+
+
+def _sampled_check(idx, nsample, tol, tolEi):
+    from sampling import sampled_oracle
+    import torch
+    from paper_2005_00223_b200 import binding
+    s = synth.config(idx)
+    so = sampled_oracle(s, nsample=nsample, seed=idx)
+    m = binding.DPModel(s.model, s.precision)
+    out = m.compute(torch.from_numpy(s.coords).cuda(), torch.from_numpy(s.types).cuda(), s.box)
+    rc, ntr = m.status()
+    assert rc == 0
+    nl = m.get_nlist()[torch.from_numpy(so["centers"]).cuda()].cpu().numpy()
+    F = out["forces"].cpu().numpy()
+    ea = out["atom_energy"].cpu().numpy()
+    E = float(out["energy"].item())
+    m.close()
+    assert np.array_equal(nl, so["nlist"])                                  # bit-exact rows of every evaluated centre
+    assert np.abs(ea[so["centers"]] - so["atom_energy"]).max() <= tolEi
+    err = np.abs(F[so["sample"]] - so["forces"]).max()
+    assert err <= tol * so["rms_f"], (err / so["rms_f"], tol)
+    # properties that hold at any size: total energy = sum of atomic energies, no net force
+    assert abs(E - ea.sum()) <= 1e-9 * abs(E)
+    assert np.abs(F.sum(0)).max() <= 1e-6 * np.abs(F).sum(0).max()
+    return ntr
+
+
+def test_config2_fp64_full_size():
+    """copper 13,500 atoms, FP64 with DMMA: full oracle (seconds)."""
+    s = synth.config(2)
+    o = oracle.evaluate(s.coords, s.types, s.box, s.model)
+    g = _gpu_eval(s)
+    _check_fp64(g, o)
+
+
+def test_config3_mix32_full_size_sampled():
+    """water 110,592 atoms, MIX-32, in the launch configuration bench.py times; sampled oracle centres."""
+    ntr = _sampled_check(3, nsample=64, tol=1e-4, tolEi=2e-5)
+    assert ntr > 0            # the 97.4 A box over-fills a few blocks (DESIGN.md reading Q23)
+
+
+def test_config4_mix16_full_size_sampled():
+    """copper 1,048,576 atoms, MIX-16, shuffled atom order; sampled oracle centres."""
+    _sampled_check(4, nsample=48, tol=5e-3, tolEi=1e-3)
