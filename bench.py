@@ -28,7 +28,9 @@ sys.path.insert(0, ROOT)
 FLOP_ROW_FWD = 12550 + 800          # embedding GEMMs forward + contraction forward, per neighbour row
 FLOP_ROW_BWD = 12550 + 1600         # embedding GEMMs backward + contraction backward, per neighbour row
 FLOP_ATOM_FIT = 2036160             # fitting fwd + bwd + descriptor fwd/bwd, per atom
-FP64_OVER_BF16_NOMINAL = 45.0 / 2250.0   # guide's nominal dense ratio: B200 FP64 tensor 45 TF vs bf16 2250 TF
+FP64_OVER_BF16_NOMINAL = 45.0 / 2250.0
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, one ncu --set full capture per config (profiles/)
+TRAFFIC = {}   # guide's nominal dense ratio: B200 FP64 tensor 45 TF vs bf16 2250 TF
 
 
 def peaks():
@@ -113,12 +115,48 @@ def run_reference(args, s):
     print(json.dumps(line))
 
 
+def time_config(binding, torch, s, dev, steps, warmup, flush, profile=True):
+    """Device-resident timing of one config: per-step CUDA events, L2 flush between steps, per-phase events."""
+    N = s.natoms
+    model = binding.DPModel(s.model, s.precision)
+    coords = torch.from_numpy(s.coords).to(dev)
+    types = torch.from_numpy(s.types).to(dev)
+    out = model.compute(coords, types, s.box)
+    rc, ntr = model.status()
+    if rc != 0:
+        raise SystemExit(f"dp_status = {rc} on {s.name}")
+    nl = model.get_nlist()
+    real_rows = int((nl >= 0).sum().item())
+    rows_f, rows_b = model.last_row_counts()
+    del nl
+    st = torch.cuda.current_stream(dev)
+    for _ in range(warmup):
+        model.compute(coords, types, s.box, out=out)
+    model.profile_enable(True)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    phases = np.zeros(5)
+    torch.cuda.synchronize(dev)
+    for k in range(steps):
+        flush.fill_(k & 0xFF)                      # L2 flush, outside the timed events
+        ev[k][0].record(st)
+        model.compute(coords, types, s.box, out=out)
+        ev[k][1].record(st)
+        phases += model.profile_read()             # synchronises; the gap is outside the timed events
+    torch.cuda.synchronize(dev)
+    model.profile_enable(False)
+    t_ms = sum(a.elapsed_time(b) for a, b in ev)
+    return dict(model=model, coords=coords, types=types, out=out, t_ms=t_ms, phases=phases / steps, real_rows=real_rows,
+                rows_f=rows_f, rows_b=rows_b, ntr=ntr)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default: c2, copper 13,500 fp64)")
+    ap.add_argument("--config", type=int, default=4,
+                    help="BASELINE.json configs index (default: c4, copper 1,048,576 atoms MIX-16, the largest single-GPU config)")
+    ap.add_argument("--all-configs", action="store_true", help="also time the other four configs (summary table in the JSON line)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -147,47 +185,25 @@ def main():
 
     s = synth.config(args.config)
     N = s.natoms
-    model = binding.DPModel(s.model, s.precision)
-    coords_h = torch.from_numpy(s.coords).pin_memory()
-    types_h = torch.from_numpy(s.types).pin_memory()
-    coords = coords_h.to(dev)
-    types = types_h.to(dev)
-    out = model.compute(coords, types, s.box)
-    rc, ntr = model.status()
-    if rc != 0:
-        raise SystemExit(f"dp_status = {rc}")
-    nl = model.get_nlist()
-    real_rows = int((nl >= 0).sum().item())
-    rows_f, rows_b = model.last_row_counts()
-    del nl
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > L2 (126 MB)
     st = torch.cuda.current_stream(dev)
+    coords_h = torch.from_numpy(s.coords).pin_memory()
+    types_h = torch.from_numpy(s.types).pin_memory()
 
     def barrier():
         torch.cuda.synchronize(dev)
         if world > 1:
             dist.barrier()
 
-    for _ in range(args.warmup):
-        model.compute(coords, types, s.box, out=out)
-    model.profile_enable(True)
     K = args.steps
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
-    phases = np.zeros(5)
     sampler = ClockSampler(local_rank)
     barrier()
     sampler.start()
-    for k in range(K):
-        flush.fill_(k & 0xFF)                      # L2 flush, outside the timed events
-        ev[k][0].record(st)
-        model.compute(coords, types, s.box, out=out)
-        ev[k][1].record(st)
-        phases += model.profile_read()             # synchronises; the gap is outside the timed events
+    r = time_config(binding, torch, s, dev, K, args.warmup, flush)
     barrier()
     clocks = sampler.stop()
-    model.profile_enable(False)
-    t_ms = sum(a.elapsed_time(b) for a, b in ev)
-    phases /= K
+    model, coords, types, out = r["model"], r["coords"], r["types"], r["out"]
+    t_ms, phases, real_rows, rows_f, rows_b, ntr = r["t_ms"], r["phases"], r["real_rows"], r["rows_f"], r["rows_b"], r["ntr"]
 
     # end to end through the public API with HOST buffers: H2D of inputs, compute, D2H of results, every step
     res_h = dict(energy=torch.empty(1, dtype=torch.float64).pin_memory(),
@@ -225,7 +241,14 @@ def main():
         pk = peaks()
         ms_step = t_ms / K
         value = world * N * K / (t_ms * 1e-3)
-        fp64_peak = pk["bf16_sus"] * FP64_OVER_BF16_NOMINAL
+        if s.precision == "fp64":
+            peak = pk["bf16_sus"] * FP64_OVER_BF16_NOMINAL
+            peak_src = f"{pk['src']}: bf16 sustained {pk['bf16_sus']} TF/s x nominal fp64/bf16 ratio 45/2250"
+            kname = "k_embed_bwd_f64"
+        else:
+            peak = pk["bf16_sus"]
+            peak_src = f"{pk['src']}: dense bf16 sustained (fp16 has the same nominal rate)"
+            kname = "k_embed_bwd_mix"
         dom_flops = real_rows * FLOP_ROW_BWD
         ach = dom_flops / (phases[3] * 1e-3) / 1e12
         kern = {"nlist_ms": phases[0], "embed_fwd_ms": phases[1], "fit_ms": phases[2], "embed_bwd_ms": phases[3],
@@ -247,14 +270,27 @@ def main():
                 "e2e": {"value": world * N * K / (e2e_ms * 1e-3), "unit": "atom-steps/s", "h2d_bytes_per_step": h2d,
                         "d2h_bytes_per_step": d2h},
                 "gpu_launches": model.launches_per_compute() * K,
-                "roofline": {"kernel": "k_embed_bwd_f64", "bound": "tensor", "achieved": ach, "peak": fp64_peak,
-                             "unit": "TFLOP/s", "frac": ach / fp64_peak, "traffic": None,
-                             "peak_source": f"{pk['src']}: bf16 sustained {pk['bf16_sus']} TF/s x nominal fp64/bf16 ratio 45/2250",
+                "roofline": {"kernel": kname, "bound": "tensor", "achieved": ach, "peak": peak,
+                             "unit": "TFLOP/s", "frac": ach / peak, "traffic": TRAFFIC.get(s.name),
+                             "peak_source": peak_src,
                              "flops_per_launch": dom_flops,
                              "note": "algorithmic backward flops (14,150 per real neighbour row); the in-kernel forward recompute is not credited"},
                 "kernels": kern}
+        if args.all_configs and world == 1:
+            summ = {}
+            for idx in range(5):
+                if idx == args.config:
+                    summ[s.name] = {"ms_per_step": ms_step, "atom_steps_per_s": value, "precision": s.precision}
+                    continue
+                s2 = synth.config(idx)
+                r2 = time_config(binding, torch, s2, dev, max(5, K), args.warmup, flush)
+                ms2 = r2["t_ms"] / max(5, K)
+                summ[s2.name] = {"ms_per_step": ms2, "atom_steps_per_s": s2.natoms / (ms2 * 1e-3), "precision": s2.precision,
+                                 "phases_ms": [round(float(x), 4) for x in r2["phases"]]}
+                r2["model"].close()
+            line["configs_summary"] = summ
         if world == 1 and not args.no_cpu_baseline:
-            ncen = min(N, 4096)
+            ncen = min(N, 16384)
             n, dt, cores = oracle_sample(s, ncen)
             line["cpu_baseline"] = {"value": n / dt, "unit": "atom-steps/s", "cores": cores, "kind": "oracle",
                                     "sample": f"{n} evenly spaced centre atoms of {s.name}, one evaluation ({dt:.1f} s)"}
