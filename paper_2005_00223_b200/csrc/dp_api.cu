@@ -8,6 +8,7 @@
 #include <vector>
 
 #include "embed_mix.cuh"
+#include "embed_tc.cuh"
 
 namespace {
 
@@ -32,6 +33,12 @@ WsLayout ws_layout(const dp_model *m, long N) {
     L.xw = take(sizeof(double) * 3 * (size_t)N);
     L.nlist = take(sizeof(int) * (size_t)N * m->Nm);
     L.nreal = take(sizeof(int) * (size_t)N * m->T);
+    if (m->prec != DP_FP64) {
+        L.rowcnt = take(sizeof(int) * (size_t)N * m->T);
+        L.rowstart = take(sizeof(int) * ((size_t)N + 1) * m->T);
+        L.rows_rh = take(sizeof(float) * 4 * (size_t)N * m->Nm);     // block b starts at row offset N*off[b]
+        L.rows_id = take(sizeof(int) * 2 * (size_t)N * m->Nm);
+    }
     const size_t esz = m->prec == DP_FP64 ? sizeof(double) : sizeof(float);
     L.A = take(esz * (size_t)N * 4 * M2E);
     if (m->prec == DP_FP64) L.gAf = take(sizeof(double) * (size_t)N * 3 * NT3 * 32);
@@ -173,6 +180,23 @@ void build_embed_frag_h(const double *net, EmbedNetFragH<NSW> *out) {
         }
 }
 
+template <int NSW>
+void build_embed_tc(const double *net, EmbedNetTC<NSW> *out) {
+    const double *W1 = net, *b1 = W1 + M0, *W2 = b1 + M0, *b2 = W2 + M0 * M1, *W3 = b2 + M1, *b3 = W3 + M1 * M2E;
+    std::memset(out, 0, sizeof(*out));
+    for (int p1 = 0; p1 < TC_K1; ++p1) { int e = tc_e_of_p1(p1); if (e >= 0) { out->w1[p1] = (float)W1[e]; out->b1[p1] = (float)b1[e]; } }
+    for (int n = 0; n < TC_N2; ++n) { int f = tc_f_of_n(n); if (f >= 0) out->b2[n] = (float)b2[f]; }
+    for (int c = 0; c < TC_N3; ++c) { int m = tc_m_of_c3(c); if (m >= 0) out->b3[c] = (float)b3[m]; }
+    auto w2 = [&](int p1, int n) { int e = tc_e_of_p1(p1), f = tc_f_of_n(n); return (e >= 0 && f >= 0) ? W2[e * M1 + f] : 0.0; };
+    auto w3 = [&](int n, int c) { int f = tc_f_of_n(n), m = tc_m_of_c3(c); return (f >= 0 && m >= 0) ? W3[f * M2E + m] : 0.0; };
+    for (int p = 0; p < NSW; ++p) {
+        for (int k = 0; k < TC_K1; ++k) for (int n = 0; n < TC_N2; ++n) out->W2[p][k >> 3][n][k & 7] = __float2half_rn(hpart(w2(k, n), p));
+        for (int k = 0; k < TC_N2; ++k) for (int c = 0; c < TC_N3; ++c) out->W3[p][k >> 3][c][k & 7] = __float2half_rn(hpart(w3(k, c), p));
+        for (int k = 0; k < TC_N3; ++k) for (int n = 0; n < TC_N2; ++n) out->W3T[p][k >> 3][n][k & 7] = __float2half_rn(hpart(w3(n, k), p));
+        for (int k = 0; k < TC_N2; ++k) for (int q = 0; q < TC_K1; ++q) out->W2T[p][k >> 3][q][k & 7] = __float2half_rn(hpart(w2(q, k), p));
+    }
+}
+
 template <typename Tp>
 cudaError_t upload(const std::vector<Tp> &h, void **dev) {
     cudaError_t e = cudaMalloc(dev, h.size() * sizeof(Tp));
@@ -260,8 +284,9 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
     if (prec == DP_MIX32) { m->mix_ns = 3; m->mix_nsc = 3; m->mix_tanh_approx = 0; m->mix_fit_ns = 3; m->mix_fit3_ns = 3; }
     if (prec == DP_MIX16) {
         // defaults from the precision study in DESIGN.md: fp16 weights, activations carried as hi + lo fp16 pairs
-        m->mix_ns = 2; m->mix_nsc = 3; m->mix_tanh_approx = 1; m->mix_fit_ns = 2; m->mix_fit3_ns = 2;
-        if (const char *e = std::getenv("DP_MIX16_NS")) { int v = std::atoi(e); if (v >= 1 && v <= 4) m->mix_ns = v; }
+        m->mix_ns = 2; m->mix_nsc = 3; m->mix_tanh_approx = 1; m->mix_fit_ns = 2; m->mix_fit3_ns = 2; m->mix_ns_bwd = 1;
+        if (const char *e = std::getenv("DP_MIX16_NS_BWD")) m->mix_ns_bwd = std::atoi(e) == 1 ? 1 : 2;
+        if (const char *e = std::getenv("DP_MIX16_NS")) { int v = std::atoi(e); if (v >= 1 && v <= 2) m->mix_ns = v; }
         if (const char *e = std::getenv("DP_MIX16_NSC")) m->mix_nsc = std::atoi(e) == 3 ? 3 : 1;
         if (const char *e = std::getenv("DP_MIX16_TANH_APPROX")) m->mix_tanh_approx = std::atoi(e) ? 1 : 0;
         if (const char *e = std::getenv("DP_MIX16_FIT_NS")) { int v = std::atoi(e); if (v >= 1 && v <= 3) m->mix_fit_ns = v; }
@@ -290,15 +315,22 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
         std::vector<EmbedNetFragH<2>> frags((size_t)T * T);
         for (int ab = 0; ab < T * T; ++ab) build_embed_frag_h<2>(w->embed + ab * ensz, &frags[ab]);
         ok(upload(frags, &m->embed_frag_dev));
-    } else if (ns_wparts(m->mix_ns) == 2) {
-        std::vector<EmbedNetFragH<2>> frags((size_t)T * T);
-        for (int ab = 0; ab < T * T; ++ab) build_embed_frag_h<2>(w->embed + ab * ensz, &frags[ab]);
-        ok(upload(frags, &m->embed_frag_dev));
     } else {
         std::vector<EmbedNetFragH<1>> frags((size_t)T * T);
         for (int ab = 0; ab < T * T; ++ab) build_embed_frag_h<1>(w->embed + ab * ensz, &frags[ab]);
         ok(upload(frags, &m->embed_frag_dev));
     }
+    if (prec == DP_MIX32) {
+        std::vector<EmbedNetTC<2>> nets((size_t)T * T);
+        for (int ab = 0; ab < T * T; ++ab) build_embed_tc<2>(w->embed + ab * ensz, &nets[ab]);
+        ok(upload(nets, &m->embed_tc_dev));
+    } else if (prec == DP_MIX16) {
+        std::vector<EmbedNetTC<1>> nets((size_t)T * T);
+        for (int ab = 0; ab < T * T; ++ab) build_embed_tc<1>(w->embed + ab * ensz, &nets[ab]);
+        ok(upload(nets, &m->embed_tc_dev));
+    }
+    m->use_tc = 1;
+    if (const char *e = std::getenv("DP_EMBED_TC")) m->use_tc = std::atoi(e) ? 1 : 0;
     const int ND = M2E * 16, F = 240;
     const size_t fnsz = (size_t)ND * F + F + (size_t)F * F + F + (size_t)F * F + F + F + 1;
     std::vector<double> V1((size_t)T * ND * F), V2((size_t)T * F * F), V3((size_t)T * F * F), c1(T * F), c2(T * F),
@@ -333,7 +365,7 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
 
 void dp_destroy(dp_model *m) {
     if (!m) return;
-    void *ptrs[] = {m->type_map_dev, m->embed_frag_dev, m->avg_dev, m->std_dev, m->ebias_dev, m->fitV1_dev, m->fitV2_dev,
+    void *ptrs[] = {m->type_map_dev, m->embed_frag_dev, m->embed_tc_dev, m->avg_dev, m->std_dev, m->ebias_dev, m->fitV1_dev, m->fitV2_dev,
                     m->fitV3_dev, m->fitc1_dev, m->fitc2_dev, m->fitc3_dev, m->fitv4_dev, m->fitc4_dev};
     for (void *p : ptrs) if (p) cudaFree(p);
     if (m->ev[0]) for (int k = 0; k <= DP_NPHASES; ++k) cudaEventDestroy(m->ev[k]);
@@ -372,7 +404,8 @@ int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *ty
     ok(launch_nlist(m, natoms, g, ws, L, st));
     mark(1);
     const bool f64 = m->prec == DP_FP64;
-    ok(f64 ? launch_embed_fwd_f64(m, natoms, g, ws, L, st) : launch_embed_fwd_mix(m, natoms, g, ws, L, st));
+    ok(f64 ? launch_embed_fwd_f64(m, natoms, g, ws, L, st)
+           : (m->use_tc ? launch_embed_fwd_tc(m, natoms, g, ws, L, st) : launch_embed_fwd_mix(m, natoms, g, ws, L, st)));
     mark(2);
     ok(f64 ? launch_fit_f64(m, natoms, g, ws, L, st) : launch_fit_mix(m, natoms, g, ws, L, st));
     mark(3);

@@ -46,6 +46,8 @@ struct dp_model {
     int *type_map_dev;
     // device weights
     void *embed_frag_dev;           // T*T EmbedNetFrag<TW>
+    void *embed_tc_dev;             // T*T EmbedNetTC<NSW> (mixed modes, tcgen05 path)
+    int use_tc;                     // mixed modes: embedding forward on tcgen05
     double *avg_dev, *std_dev;      // [T][4]
     double *ebias_dev;              // [T]
     // fitting nets (per type): V1 [1600][240], V2, V3 [240][240] row-major in x out, biases, v4, c4
@@ -59,7 +61,7 @@ struct dp_model {
     int sort_cap;
     // mixed-mode variant knobs: operand parts of the net MMAs (1 = fp16, 3 = split), of the contraction-type MMAs,
     // tanh.approx vs tanhf, and operand parts of fitting layers 1-2
-    int mix_ns, mix_nsc, mix_tanh_approx, mix_fit_ns, mix_fit3_ns;
+    int mix_ns, mix_nsc, mix_tanh_approx, mix_fit_ns, mix_fit3_ns, mix_ns_bwd;
     int profile;
     cudaEvent_t ev[DP_NPHASES + 1];
 };
@@ -79,6 +81,10 @@ struct WsLayout {
     size_t xw;          // double[N][3] wrapped coords, user order
     size_t nlist;       // int[N][Nm] sorted-space indices
     size_t nreal;       // int[N][T]
+    size_t rowcnt;      // int[T][N]   rows per (neighbour type, atom): real + one padded-row representative (mixed modes)
+    size_t rowstart;    // int[T][N+1] exclusive prefix of rowcnt over the sorted atoms
+    size_t rows_rh;     // float4[T][N*sel_b...] compact env rows R^ (mixed modes, tcgen05 path)
+    size_t rows_id;     // int2 {atom, k | padflag<<30}
     size_t A;           // double[N][4][100]   (float for mixed modes)
     size_t gAf;         // gA fragments [N][42][32] doubles (fp64) / [N][NSW][28][32] words (mixed)
     size_t gscale;      // float[N] power-of-two scale of the mixed gA fragments
@@ -108,6 +114,7 @@ cudaError_t launch_finalize(const dp_model *m, long N, char *ws, const WsLayout 
                             double *forces, double *virial, cudaStream_t st);
 cudaError_t launch_embed_fwd_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_embed_bwd_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+cudaError_t launch_embed_fwd_tc(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 int embed_smem_bytes_fwd_f64();
 int embed_smem_bytes_bwd_f64();

@@ -281,7 +281,7 @@ k_embed_fwd_mix(int T, int ncell, int Nm, int4 sel4, EnvParams ep, const EmbedNe
 //   [p][0..14)[lane]     dG  MMA (k8) B fragment of tile nt3:  (r < 2) ? half2(gA[2r][f], gA[2r+1][f]) : 0, f = f3(nt3, g/2, g%2)
 //   [p][14 + 2s + h][lane] dR^ MMA (k16 step s) B registers h = 0,1: (g < 4) ? half2(gA[g][f3(2s+h, r, 0)], gA[g][f3(2s+h, r, 1)]) : 0
 // all scaled by gscale[i] (a power of two that brings max|gA| near 1); results are multiplied by 1/(Nm*gscale).
-template <int NS, int NSC, bool APPROX>
+template <int NS, int NSC, bool APPROX, int NSB>
 __global__ void __launch_bounds__(DP_WARPS_PER_CTA * 32, 1)
 k_embed_bwd_mix(int T, int ncell, int Nm, int4 sel4, EnvParams ep, const EmbedNetFragH<ns_wparts(NS)> *__restrict__ nets,
                 const double *__restrict__ avg, const double *__restrict__ stdv, const int *__restrict__ bin_start,
@@ -382,12 +382,12 @@ k_embed_bwd_mix(int T, int ncell, int Nm, int4 sel4, EnvParams ep, const EmbedNe
                         // dy2 += dz3 W3^T   (K = 14 tiles = 7 k16 steps, N = 7 tiles)
 #pragma unroll
                         for (int s = 0; s < HNT3 / 2; ++s) {
-                            AFrag<NS> a_;
-                            make_afrag<NS>(a_, t3c[2 * s][0], t3c[2 * s][1], t3c[2 * s][2], t3c[2 * s][3], t3c[2 * s + 1][0],
+                            AFrag<NSB> a_;
+                            make_afrag<NSB>(a_, t3c[2 * s][0], t3c[2 * s][1], t3c[2 * s][2], t3c[2 * s][3], t3c[2 * s + 1][0],
                                            t3c[2 * s + 1][1], t3c[2 * s + 1][2], t3c[2 * s + 1][3]);
 #pragma unroll
                             for (int nt2 = 0; nt2 < HNT2; ++nt2)
-                                mma_k16<NS>(dy2[nt2], a_, net->W3Tf[0][s][nt2][lane], net->W3Tf[NSW - 1][s][nt2][lane]);
+                                mma_k16<NSB>(dy2[nt2], a_, net->W3Tf[0][s][nt2][lane], net->W3Tf[NSW - 1][s][nt2][lane]);
                         }
                         // residual dy1 (slot q = 2t + j1 <- dy2 tile q, both j2) ; dz2 = dy2 (1 - t2^2)
                         float dy1[4][4];
@@ -403,18 +403,18 @@ k_embed_bwd_mix(int T, int ncell, int Nm, int4 sel4, EnvParams ep, const EmbedNe
                         // dy1 += dz2 W2^T   (K = 7 tiles = 3 k16 + 1 k8, N = 4 tiles of y1 slots)
 #pragma unroll
                         for (int s = 0; s < 4; ++s) {
-                            AFrag<NS> a_;
+                            AFrag<NSB> a_;
                             if (s < 3) {
-                                make_afrag<NS>(a_, dy2[2 * s][0], dy2[2 * s][1], dy2[2 * s][2], dy2[2 * s][3], dy2[2 * s + 1][0],
+                                make_afrag<NSB>(a_, dy2[2 * s][0], dy2[2 * s][1], dy2[2 * s][2], dy2[2 * s][3], dy2[2 * s + 1][0],
                                                dy2[2 * s + 1][1], dy2[2 * s + 1][2], dy2[2 * s + 1][3]);
 #pragma unroll
                                 for (int t1 = 0; t1 < 4; ++t1)
-                                    mma_k16<NS>(dy1[t1], a_, net->W2Tf[0][s][t1][lane], net->W2Tf[NSW - 1][s][t1][lane]);
+                                    mma_k16<NSB>(dy1[t1], a_, net->W2Tf[0][s][t1][lane], net->W2Tf[NSW - 1][s][t1][lane]);
                             } else {
-                                make_afrag8<NS>(a_, dy2[6][0], dy2[6][1], dy2[6][2], dy2[6][3]);
+                                make_afrag8<NSB>(a_, dy2[6][0], dy2[6][1], dy2[6][2], dy2[6][3]);
 #pragma unroll
                                 for (int t1 = 0; t1 < 4; ++t1)
-                                    mma_k8<NS>(dy1[t1], a_, net->W2Tf[0][s][t1][lane], net->W2Tf[NSW - 1][s][t1][lane]);
+                                    mma_k8<NSB>(dy1[t1], a_, net->W2Tf[0][s][t1][lane], net->W2Tf[NSW - 1][s][t1][lane]);
                             }
                         }
                         // layer 1: ds[row] = sum_e dy1 (1 - y1^2) W1[e]
@@ -519,12 +519,12 @@ cudaError_t launch_fwd(const dp_model *m, long N, const Grid3 &g, char *ws, cons
     return cudaGetLastError();
 }
 
-template <int NS, int NSC, bool APPROX>
+template <int NS, int NSC, bool APPROX, int NSB>
 cudaError_t launch_bwd(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
     static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(k_embed_bwd_mix<NS, NSC, APPROX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<NS>()); attr = true; }
+    if (!attr) { cudaFuncSetAttribute(k_embed_bwd_mix<NS, NSC, APPROX, NSB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<NS>()); attr = true; }
     int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
-    k_embed_bwd_mix<NS, NSC, APPROX><<<embed_grid(m, N), DP_WARPS_PER_CTA * 32, smem_bytes<NS>(), st>>>(
+    k_embed_bwd_mix<NS, NSC, APPROX, NSB><<<embed_grid(m, N), DP_WARPS_PER_CTA * 32, smem_bytes<NS>(), st>>>(
         m->T, g.ncell, m->Nm, sel4, make_env(m, g), (const EmbedNetFragH<ns_wparts(NS)> *)m->embed_frag_dev, m->avg_dev,
         m->std_dev, (int *)(ws + L.bin_start), (double *)(ws + L.xs), (int *)(ws + L.nlist), (int *)(ws + L.nreal),
         (const uint32_t *)(ws + L.gAf), (const float *)(ws + L.gscale), (double *)(ws + L.fsorted),
@@ -534,20 +534,14 @@ cudaError_t launch_bwd(const dp_model *m, long N, const Grid3 &g, char *ws, cons
 
 }  // namespace
 
-#define DISPATCH1(FN, NS_)                                                                                     \
-    return m->mix_nsc == 3 ? FN<NS_, 3, true>(m, N, g, ws, L, st) : FN<NS_, 1, true>(m, N, g, ws, L, st);
-#define DISPATCH(FN)                                                                                           \
-    if (m->prec == DP_MIX32) return FN<3, 3, false>(m, N, g, ws, L, st);                                       \
-    switch (m->mix_ns) {                                                                                       \
-        case 2: DISPATCH1(FN, 2)                                                                               \
-        case 3: DISPATCH1(FN, 3)                                                                               \
-        case 4: DISPATCH1(FN, 4)                                                                               \
-        default: DISPATCH1(FN, 1)                                                                              \
-    }
-
 cudaError_t launch_embed_fwd_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    DISPATCH(launch_fwd)
+    if (m->prec == DP_MIX32) return launch_fwd<3, 3, false>(m, N, g, ws, L, st);
+    if (m->mix_ns == 1) return m->mix_nsc == 3 ? launch_fwd<1, 3, true>(m, N, g, ws, L, st) : launch_fwd<1, 1, true>(m, N, g, ws, L, st);
+    return m->mix_nsc == 3 ? launch_fwd<2, 3, true>(m, N, g, ws, L, st) : launch_fwd<2, 1, true>(m, N, g, ws, L, st);
 }
 cudaError_t launch_embed_bwd_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    DISPATCH(launch_bwd)
+    if (m->prec == DP_MIX32) return launch_bwd<3, 3, false, 3>(m, N, g, ws, L, st);
+    if (m->mix_ns == 1) return m->mix_nsc == 3 ? launch_bwd<1, 3, true, 1>(m, N, g, ws, L, st) : launch_bwd<1, 1, true, 1>(m, N, g, ws, L, st);
+    if (m->mix_ns_bwd == 1) return m->mix_nsc == 3 ? launch_bwd<2, 3, true, 1>(m, N, g, ws, L, st) : launch_bwd<2, 1, true, 1>(m, N, g, ws, L, st);
+    return m->mix_nsc == 3 ? launch_bwd<2, 3, true, 2>(m, N, g, ws, L, st) : launch_bwd<2, 1, true, 2>(m, N, g, ws, L, st);
 }

@@ -56,12 +56,12 @@ __device__ __forceinline__ uint32_t pack_h2(float x, float y) {
     return *reinterpret_cast<uint32_t *>(&h);
 }
 // x = hi + lo with hi = fp16(x), lo = fp16(x - hi)
+// hi is x truncated to 11 significant bits (exactly representable in fp16 for normal-range values), so the
+// fp32 -> fp16 conversion of hi is exact and no conversion back is needed to form the remainder.
 __device__ __forceinline__ void split_h2(float x, float y, uint32_t &hi, uint32_t &lo) {
-    __half2 h = __floats2half2_rn(x, y);
-    float2 hf = __half22float2(h);
-    __half2 l = __floats2half2_rn(x - hf.x, y - hf.y);
-    hi = *reinterpret_cast<uint32_t *>(&h);
-    lo = *reinterpret_cast<uint32_t *>(&l);
+    const float xh = __int_as_float(__float_as_int(x) & 0xFFFFE000), yh = __int_as_float(__float_as_int(y) & 0xFFFFE000);
+    hi = pack_h2(xh, yh);
+    lo = pack_h2(x - xh, y - yh);
 }
 __device__ __forceinline__ uint32_t movmatrix_trans(uint32_t x) {
     uint32_t y;

@@ -41,17 +41,20 @@ __global__ void k_wrap_bin(long N, const double *__restrict__ coords, const int 
     atomicAdd(&bin_count[bin], 1);
 }
 
-// exclusive scan of bin_count[0..n) -> bin_start[0..n]; one block.
+// exclusive scan of cnt[0..n) -> start[0..n]; one block, 4 elements per thread per pass.
 __global__ void k_scan(int n, const int *__restrict__ cnt, int *__restrict__ start) {
     __shared__ int warp_sums[32];
     __shared__ int carry;
     if (threadIdx.x == 0) carry = 0;
     __syncthreads();
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    for (int base = 0; base < n; base += blockDim.x) {
-        int i = base + threadIdx.x;
-        int v = i < n ? cnt[i] : 0;
-        int x = v;
+    for (int base = 0; base < n; base += 4 * blockDim.x) {
+        const int i0 = base + 4 * threadIdx.x;
+        int v[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) v[k] = i0 + k < n ? cnt[i0 + k] : 0;
+        const int tsum = v[0] + v[1] + v[2] + v[3];
+        int x = tsum;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             int y = __shfl_up_sync(0xffffffffu, x, o);
@@ -69,10 +72,14 @@ __global__ void k_scan(int n, const int *__restrict__ cnt, int *__restrict__ sta
             warp_sums[lane] = s;
         }
         __syncthreads();
-        int prefix = carry + (wid ? warp_sums[wid - 1] : 0) + x - v;
-        if (i < n) start[i] = prefix;
+        int prefix = carry + (wid ? warp_sums[wid - 1] : 0) + x - tsum;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            if (i0 + k < n) start[i0 + k] = prefix;
+            prefix += v[k];
+        }
         __syncthreads();
-        if (threadIdx.x == blockDim.x - 1) carry = prefix + v;
+        if (threadIdx.x == blockDim.x - 1) carry = prefix;
         __syncthreads();
     }
     if (threadIdx.x == 0) start[n] = carry;
@@ -115,7 +122,8 @@ __device__ __forceinline__ double min_image(double t, double L, double halfL) {
 __global__ void __launch_bounds__(128)
 k_nlist(long N, int T, Grid3 g, double rc2, int cap, const int *__restrict__ bin_start,
         const double *__restrict__ xs, const int *__restrict__ perm, const int *__restrict__ inv,
-        int Nm, int4 sel4, int *__restrict__ nlist, int *__restrict__ nreal, int *__restrict__ status) {
+        int Nm, int4 sel4, int *__restrict__ nlist, int *__restrict__ nreal, int *__restrict__ rowcnt,
+        int *__restrict__ status) {
     extern __shared__ unsigned long long keys_all[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const long i = blockIdx.x * 4L + wid;
@@ -184,7 +192,10 @@ k_nlist(long N, int T, Grid3 g, double rc2, int cap, const int *__restrict__ bin
         const int nkeep = n < sel[b] ? n : sel[b];
         for (int k = lane; k < sel[b]; k += 32)
             nlist[i * Nm + off + k] = k < nkeep ? inv[(int)(keys[k] & 0xFFFFFFull)] : -1;
-        if (lane == 0) nreal[i * T + b] = nkeep;
+        if (lane == 0) {
+            nreal[i * T + b] = nkeep;
+            if (rowcnt) rowcnt[(long)b * N + i] = nkeep + (nkeep < sel[b] ? 1 : 0);   // real rows + one padded-row representative
+        }
         truncated |= n > sel[b];
         off += sel[b];
         __syncwarp();
@@ -234,7 +245,11 @@ cudaError_t launch_nlist(const dp_model *m, long N, const Grid3 &g, char *ws, co
     k_nlist<<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, m->T, g, m->rc * m->rc, cap, (int *)(ws + L.bin_start),
                                                        (double *)(ws + L.xs), (int *)(ws + L.perm),
                                                        (int *)(ws + L.inv), m->Nm, sel4, (int *)(ws + L.nlist),
-                                                       (int *)(ws + L.nreal), (int *)(ws + L.status));
+                                                       (int *)(ws + L.nreal), m->prec == DP_FP64 ? nullptr : (int *)(ws + L.rowcnt),
+                                                       (int *)(ws + L.status));
+    if (m->prec != DP_FP64)
+        for (int b = 0; b < m->T; ++b)
+            k_scan<<<1, 1024, 0, st>>>((int)N, (int *)(ws + L.rowcnt) + (long)b * N, (int *)(ws + L.rowstart) + (long)b * (N + 1));
     return cudaGetLastError();
 }
 
