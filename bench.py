@@ -157,6 +157,8 @@ def main():
     ap.add_argument("--config", type=int, default=4,
                     help="BASELINE.json configs index (default: c4, copper 1,048,576 atoms MIX-16, the largest single-GPU config)")
     ap.add_argument("--all-configs", action="store_true", help="also time the other four configs (summary table in the JSON line)")
+    ap.add_argument("--precision", default=None, choices=["fp64", "mix32", "mix16"],
+                    help="override the config's precision (profiling aid; the default is the precision BASELINE.json names)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -184,6 +186,8 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     s = synth.config(args.config)
+    if args.precision:
+        s.precision = args.precision
     N = s.natoms
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > L2 (126 MB)
     st = torch.cuda.current_stream(dev)

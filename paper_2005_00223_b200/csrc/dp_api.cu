@@ -9,6 +9,7 @@
 
 #include "embed_mix.cuh"
 #include "embed_tc.cuh"
+#include "embed_tc2.cuh"
 
 namespace {
 
@@ -197,6 +198,41 @@ void build_embed_tc(const double *net, EmbedNetTC<NSW> *out) {
     }
 }
 
+// MIX-16 operand images of the warpgroup-per-tile kernels (embed_tc2.cuh): fp16 weights ("stored in half precision",
+// PAPER.md:125), biases as hi + lo rows multiplied by the constant-one columns, residual folds pre-summed in fp64.
+void build_embed_tc2(const double *net, EmbedNetTC2 *out) {
+    const double *W1 = net, *b1 = W1 + M0, *W2 = b1 + M0, *b2 = W2 + M0 * M1, *W3 = b2 + M1, *b3 = W3 + M1 * M2E;
+    std::memset(out, 0, sizeof(*out));
+    for (int e = 0; e < M0; ++e) { out->w1[e] = (float)W1[e]; out->b1[e] = (float)b1[e]; }
+    auto h = [](double x) { return __float2half_rn((float)x); };
+    for (int k = 0; k < T2_K1; ++k)
+        for (int n = 0; n < M1; ++n) {
+            double v = 0.0;
+            if (k < M0) v = W2[k * M1 + n];
+            else if (k == T2_ONE_HI) v = hpart(b2[n], 0);
+            else if (k == T2_ONE_LO) v = hpart(b2[n], 1);
+            out->W2[k >> 3][n][k & 7] = h(v);
+        }
+    for (int k = 0; k < T2_K2 + T2_K1; ++k)
+        for (int m = 0; m < M2E; ++m) {
+            double v = 0.0;
+            if (k < M1) v = W3[k * M2E + m];
+            else if (k >= T2_K2) {
+                const int e = k - T2_K2;
+                if (e < M0) v = W3[e * M2E + m] + W3[(e + M0) * M2E + m];
+                else if (e == T2_ONE_HI) v = hpart(b3[m], 0);
+                else if (e == T2_ONE_LO) v = hpart(b3[m], 1);
+            }
+            out->W3[k >> 3][m][k & 7] = h(v);
+        }
+    for (int k = 0; k < M2E; ++k) {          // k = layer-3 feature m
+        for (int f = 0; f < M1; ++f) out->W3T[k >> 3][f][k & 7] = h(W3[f * M2E + k]);
+        for (int e = 0; e < M0; ++e) out->W3T[k >> 3][64 + e][k & 7] = h(W3[e * M2E + k] + W3[(e + M0) * M2E + k]);
+    }
+    for (int k = 0; k < M1; ++k)             // k = layer-2 feature f
+        for (int e = 0; e < M0; ++e) out->W2T[k >> 3][e][k & 7] = h(W2[e * M1 + k]);
+}
+
 template <typename Tp>
 cudaError_t upload(const std::vector<Tp> &h, void **dev) {
     cudaError_t e = cudaMalloc(dev, h.size() * sizeof(Tp));
@@ -292,6 +328,11 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
         if (const char *e = std::getenv("DP_MIX16_FIT_NS")) { int v = std::atoi(e); if (v >= 1 && v <= 3) m->mix_fit_ns = v; }
         if (const char *e = std::getenv("DP_MIX16_FIT3_NS")) { int v = std::atoi(e); if (v >= 1 && v <= 3) m->mix_fit3_ns = v; }
     }
+    m->mix_ns_fwd = m->mix_ns; m->mix_nsc_fwd = m->mix_nsc;
+    if (prec == DP_MIX16) {
+        if (const char *e = std::getenv("DP_MIX16_NS_FWD")) { int v = std::atoi(e); if (v >= 1 && v <= 2) m->mix_ns_fwd = v; }
+        if (const char *e = std::getenv("DP_MIX16_NSC_FWD")) m->mix_nsc_fwd = std::atoi(e) == 3 ? 3 : 1;
+    }
     for (int b = 0; b < T; ++b) { m->sel[b] = sel[b]; m->off[b + 1] = m->off[b] + sel[b]; }
     int cap = 256;
     while (cap < 2 * maxsel) cap <<= 1;
@@ -329,8 +370,14 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
         for (int ab = 0; ab < T * T; ++ab) build_embed_tc<1>(w->embed + ab * ensz, &nets[ab]);
         ok(upload(nets, &m->embed_tc_dev));
     }
-    m->use_tc = 1;
-    if (const char *e = std::getenv("DP_EMBED_TC")) m->use_tc = std::atoi(e) ? 1 : 0;
+    if (prec == DP_MIX16) {
+        std::vector<EmbedNetTC2> nets((size_t)T * T);
+        for (int ab = 0; ab < T * T; ++ab) build_embed_tc2(w->embed + ab * ensz, &nets[ab]);
+        ok(upload(nets, &m->embed_tc2_dev));
+    }
+    // embedding forward: 0 = mma.sync kernels, 1 = first tcgen05 kernel, 2 = warpgroup-per-tile tcgen05 kernel (MIX-16)
+    m->use_tc = prec == DP_MIX16 ? 2 : 1;
+    if (const char *e = std::getenv("DP_EMBED_TC")) { int v = std::atoi(e); if (v >= 0 && v <= (prec == DP_MIX16 ? 2 : 1)) m->use_tc = v; }
     const int ND = M2E * 16, F = 240;
     const size_t fnsz = (size_t)ND * F + F + (size_t)F * F + F + (size_t)F * F + F + F + 1;
     std::vector<double> V1((size_t)T * ND * F), V2((size_t)T * F * F), V3((size_t)T * F * F), c1(T * F), c2(T * F),
@@ -365,7 +412,7 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
 
 void dp_destroy(dp_model *m) {
     if (!m) return;
-    void *ptrs[] = {m->type_map_dev, m->embed_frag_dev, m->embed_tc_dev, m->avg_dev, m->std_dev, m->ebias_dev, m->fitV1_dev, m->fitV2_dev,
+    void *ptrs[] = {m->type_map_dev, m->embed_frag_dev, m->embed_tc_dev, m->embed_tc2_dev, m->avg_dev, m->std_dev, m->ebias_dev, m->fitV1_dev, m->fitV2_dev,
                     m->fitV3_dev, m->fitc1_dev, m->fitc2_dev, m->fitc3_dev, m->fitv4_dev, m->fitc4_dev};
     for (void *p : ptrs) if (p) cudaFree(p);
     if (m->ev[0]) for (int k = 0; k <= DP_NPHASES; ++k) cudaEventDestroy(m->ev[k]);
@@ -405,7 +452,8 @@ int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *ty
     mark(1);
     const bool f64 = m->prec == DP_FP64;
     ok(f64 ? launch_embed_fwd_f64(m, natoms, g, ws, L, st)
-           : (m->use_tc ? launch_embed_fwd_tc(m, natoms, g, ws, L, st) : launch_embed_fwd_mix(m, natoms, g, ws, L, st)));
+           : (m->use_tc == 2 ? launch_embed_fwd_tc2(m, natoms, g, ws, L, st)
+              : (m->use_tc ? launch_embed_fwd_tc(m, natoms, g, ws, L, st) : launch_embed_fwd_mix(m, natoms, g, ws, L, st))));
     mark(2);
     ok(f64 ? launch_fit_f64(m, natoms, g, ws, L, st) : launch_fit_mix(m, natoms, g, ws, L, st));
     mark(3);

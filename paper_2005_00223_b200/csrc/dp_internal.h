@@ -47,6 +47,7 @@ struct dp_model {
     // device weights
     void *embed_frag_dev;           // T*T EmbedNetFrag<TW>
     void *embed_tc_dev;             // T*T EmbedNetTC<NSW> (mixed modes, tcgen05 path)
+    void *embed_tc2_dev;            // T*T EmbedNetTC2 (MIX-16, warpgroup-per-tile tcgen05 path)
     int use_tc;                     // mixed modes: embedding forward on tcgen05
     double *avg_dev, *std_dev;      // [T][4]
     double *ebias_dev;              // [T]
@@ -62,6 +63,7 @@ struct dp_model {
     // mixed-mode variant knobs: operand parts of the net MMAs (1 = fp16, 3 = split), of the contraction-type MMAs,
     // tanh.approx vs tanhf, and operand parts of fitting layers 1-2
     int mix_ns, mix_nsc, mix_tanh_approx, mix_fit_ns, mix_fit3_ns, mix_ns_bwd;
+    int mix_ns_fwd, mix_nsc_fwd;    // forward-kernel overrides of mix_ns / mix_nsc (precision study)
     int profile;
     cudaEvent_t ev[DP_NPHASES + 1];
 };
@@ -115,6 +117,8 @@ cudaError_t launch_finalize(const dp_model *m, long N, char *ws, const WsLayout 
 cudaError_t launch_embed_fwd_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_embed_bwd_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_embed_fwd_tc(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+cudaError_t launch_embed_fwd_tc2(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+cudaError_t launch_env_rows(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 int embed_smem_bytes_fwd_f64();
 int embed_smem_bytes_bwd_f64();

@@ -536,8 +536,8 @@ cudaError_t launch_bwd(const dp_model *m, long N, const Grid3 &g, char *ws, cons
 
 cudaError_t launch_embed_fwd_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
     if (m->prec == DP_MIX32) return launch_fwd<3, 3, false>(m, N, g, ws, L, st);
-    if (m->mix_ns == 1) return m->mix_nsc == 3 ? launch_fwd<1, 3, true>(m, N, g, ws, L, st) : launch_fwd<1, 1, true>(m, N, g, ws, L, st);
-    return m->mix_nsc == 3 ? launch_fwd<2, 3, true>(m, N, g, ws, L, st) : launch_fwd<2, 1, true>(m, N, g, ws, L, st);
+    if (m->mix_ns_fwd == 1) return m->mix_nsc_fwd == 3 ? launch_fwd<1, 3, true>(m, N, g, ws, L, st) : launch_fwd<1, 1, true>(m, N, g, ws, L, st);
+    return m->mix_nsc_fwd == 3 ? launch_fwd<2, 3, true>(m, N, g, ws, L, st) : launch_fwd<2, 1, true>(m, N, g, ws, L, st);
 }
 cudaError_t launch_embed_bwd_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
     if (m->prec == DP_MIX32) return launch_bwd<3, 3, false, 3>(m, N, g, ws, L, st);

@@ -407,6 +407,21 @@ EnvParams make_env(const dp_model *m, const Grid3 &g) {
     return ep;
 }
 
+}  // namespace
+
+// S3: compact fp32 environment rows for the tcgen05 embedding kernels
+cudaError_t launch_env_rows(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
+    int4 off4 = make_int4(m->off[0], m->off[1], m->off[2], m->off[3]);
+    k_env_rows<<<(unsigned)((N + 7) / 8), 256, 0, st>>>(N, m->T, g.ncell, m->Nm, sel4, off4, make_env(m, g), m->avg_dev, m->std_dev,
+                                                         (int *)(ws + L.bin_start), (double *)(ws + L.xs), (int *)(ws + L.nlist),
+                                                         (int *)(ws + L.nreal), (int *)(ws + L.rowstart),
+                                                         (float4 *)(ws + L.rows_rh), (int2 *)(ws + L.rows_id));
+    return cudaGetLastError();
+}
+
+namespace {
+
 template <int NS, bool APPROX>
 cudaError_t launch_fwd(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
     constexpr int NSW = NS == 3 ? 2 : 1;
@@ -415,10 +430,7 @@ cudaError_t launch_fwd(const dp_model *m, long N, const Grid3 &g, char *ws, cons
     if (!attr) { cudaFuncSetAttribute(k_embed_fwd_tc<NS, APPROX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr = true; }
     int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
     int4 off4 = make_int4(m->off[0], m->off[1], m->off[2], m->off[3]);
-    k_env_rows<<<(unsigned)((N + 7) / 8), 256, 0, st>>>(N, m->T, g.ncell, m->Nm, sel4, off4, make_env(m, g), m->avg_dev, m->std_dev,
-                                                         (int *)(ws + L.bin_start), (double *)(ws + L.xs), (int *)(ws + L.nlist),
-                                                         (int *)(ws + L.nreal), (int *)(ws + L.rowstart),
-                                                         (float4 *)(ws + L.rows_rh), (int2 *)(ws + L.rows_id));
+    launch_env_rows(m, N, g, ws, L, st);
     cudaMemsetAsync(ws + L.A, 0, sizeof(float) * (size_t)N * 4 * M2E, st);
     const int grid = m->num_sms * (NS == 2 ? 2 : 1);
     k_embed_fwd_tc<NS, APPROX><<<grid, 256, smem, st>>>(
