@@ -226,8 +226,8 @@ void build_embed_tc2(const double *net, EmbedNetTC2 *out) {
             out->W3[k >> 3][m][k & 7] = h(v);
         }
     for (int k = 0; k < M2E; ++k) {          // k = layer-3 feature m
-        for (int f = 0; f < M1; ++f) out->W3T[k >> 3][f][k & 7] = h(W3[f * M2E + k]);
-        for (int e = 0; e < M0; ++e) out->W3T[k >> 3][64 + e][k & 7] = h(W3[e * M2E + k] + W3[(e + M0) * M2E + k]);
+        for (int e = 0; e < M0; ++e) out->W3T[k >> 3][e][k & 7] = h(W3[e * M2E + k] + W3[(e + M0) * M2E + k]);
+        for (int f = 0; f < M1; ++f) out->W3T[k >> 3][32 + f][k & 7] = h(W3[f * M2E + k]);
     }
     for (int k = 0; k < M1; ++k)             // k = layer-2 feature f
         for (int e = 0; e < M0; ++e) out->W2T[k >> 3][e][k & 7] = h(W2[e * M1 + k]);
@@ -378,6 +378,9 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
     // embedding forward: 0 = mma.sync kernels, 1 = first tcgen05 kernel, 2 = warpgroup-per-tile tcgen05 kernel (MIX-16)
     m->use_tc = prec == DP_MIX16 ? 2 : 1;
     if (const char *e = std::getenv("DP_EMBED_TC")) { int v = std::atoi(e); if (v >= 0 && v <= (prec == DP_MIX16 ? 2 : 1)) m->use_tc = v; }
+    m->use_tc_bwd = prec == DP_MIX16 ? 1 : 0;
+    if (const char *e = std::getenv("DP_EMBED_TC_BWD")) m->use_tc_bwd = (prec == DP_MIX16 && std::atoi(e)) ? 1 : 0;
+    if (m->use_tc == 0) m->use_tc_bwd = 0;      // the tcgen05 backward reads the compact rows the tcgen05 forward builds
     const int ND = M2E * 16, F = 240;
     const size_t fnsz = (size_t)ND * F + F + (size_t)F * F + F + (size_t)F * F + F + F + 1;
     std::vector<double> V1((size_t)T * ND * F), V2((size_t)T * F * F), V3((size_t)T * F * F), c1(T * F), c2(T * F),
@@ -457,7 +460,8 @@ int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *ty
     mark(2);
     ok(f64 ? launch_fit_f64(m, natoms, g, ws, L, st) : launch_fit_mix(m, natoms, g, ws, L, st));
     mark(3);
-    ok(f64 ? launch_embed_bwd_f64(m, natoms, g, ws, L, st) : launch_embed_bwd_mix(m, natoms, g, ws, L, st));
+    ok(f64 ? launch_embed_bwd_f64(m, natoms, g, ws, L, st)
+           : (m->use_tc_bwd ? launch_embed_bwd_tc2(m, natoms, g, ws, L, st) : launch_embed_bwd_mix(m, natoms, g, ws, L, st)));
     mark(4);
     ok(launch_finalize(m, natoms, ws, L, energy_dev, atom_energy_dev, forces_dev, virial_dev, st));
     mark(5);

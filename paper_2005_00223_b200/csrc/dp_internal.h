@@ -49,6 +49,7 @@ struct dp_model {
     void *embed_tc_dev;             // T*T EmbedNetTC<NSW> (mixed modes, tcgen05 path)
     void *embed_tc2_dev;            // T*T EmbedNetTC2 (MIX-16, warpgroup-per-tile tcgen05 path)
     int use_tc;                     // mixed modes: embedding forward on tcgen05
+    int use_tc_bwd;                 // MIX-16: embedding backward on tcgen05
     double *avg_dev, *std_dev;      // [T][4]
     double *ebias_dev;              // [T]
     // fitting nets (per type): V1 [1600][240], V2, V3 [240][240] row-major in x out, biases, v4, c4
@@ -118,6 +119,7 @@ cudaError_t launch_embed_fwd_mix(const dp_model *m, long N, const Grid3 &g, char
 cudaError_t launch_embed_bwd_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_embed_fwd_tc(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_embed_fwd_tc2(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+cudaError_t launch_embed_bwd_tc2(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_env_rows(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 int embed_smem_bytes_fwd_f64();

@@ -3,6 +3,7 @@
 // accumulation in fp64; the embedding net on fp16 tensor-core MMAs with fp32 accumulation (operand splitting gives
 // single-precision products in MIX-32); tanh and tanh' in fp32; first embedding layer (K = 1) on the ALUs as in
 // the paper ("do not meet the size requirements for using Tensor Cores").  See embed_mix.cuh for the layouts.
+#include <cstdlib>
 #include "embed_mix.cuh"
 
 namespace {
@@ -287,7 +288,7 @@ k_embed_bwd_mix(int T, int ncell, int Nm, int4 sel4, EnvParams ep, const EmbedNe
                 const double *__restrict__ avg, const double *__restrict__ stdv, const int *__restrict__ bin_start,
                 const double *__restrict__ xs, const int *__restrict__ nlist, const int *__restrict__ nreal,
                 const uint32_t *__restrict__ gAf, const float *__restrict__ gscale, double *__restrict__ fsorted,
-                double *__restrict__ virial, unsigned long long *__restrict__ row_counter) {
+                double *__restrict__ virial, unsigned long long *__restrict__ row_counter, int dbg) {
     constexpr int NSW = ns_wparts(NS);
     extern __shared__ __align__(16) uint32_t smem_u[];
     EmbedNetFragH<NSW> *net = reinterpret_cast<EmbedNetFragH<NSW> *>(smem_u);
@@ -431,6 +432,10 @@ k_embed_bwd_mix(int T, int ncell, int Nm, int4 sel4, EnvParams ep, const EmbedNe
                         ds1 += __shfl_xor_sync(0xffffffffu, ds1, 1); ds1 += __shfl_xor_sync(0xffffffffu, ds1, 2);
 #pragma unroll
                         for (int k = 0; k < 4; ++k) dR[k] *= oscale;
+                        if (dbg & 2) { dR[0] = dR[1] = dR[2] = dR[3] = 0.f; }
+                        if (dbg & 16) { if (r == 0) { dR[1] = dR[3] = 0.f; } else { dR[0] = dR[1] = dR[2] = dR[3] = 0.f; } }
+                        if (dbg & 32) { if (r == 0) { dR[0] = dR[2] = 0.f; } }
+                        if (dbg & 1) { ds0 = ds1 = 0.f; }
                         if (r == 0) { dR[0] += ds0; dR[2] += ds1; }
                         __syncwarp();
                         if (r < 2) {
@@ -528,7 +533,7 @@ cudaError_t launch_bwd(const dp_model *m, long N, const Grid3 &g, char *ws, cons
         m->T, g.ncell, m->Nm, sel4, make_env(m, g), (const EmbedNetFragH<ns_wparts(NS)> *)m->embed_frag_dev, m->avg_dev,
         m->std_dev, (int *)(ws + L.bin_start), (double *)(ws + L.xs), (int *)(ws + L.nlist), (int *)(ws + L.nreal),
         (const uint32_t *)(ws + L.gAf), (const float *)(ws + L.gscale), (double *)(ws + L.fsorted),
-        (double *)(ws + L.virial), (unsigned long long *)(ws + L.status + 16));
+        (double *)(ws + L.virial), (unsigned long long *)(ws + L.status + 16), getenv("DP_DEBUG_BWD") ? atoi(getenv("DP_DEBUG_BWD")) : 0);
     return cudaGetLastError();
 }
 

@@ -145,7 +145,8 @@ struct TileMeta {
 };
 
 // Compact env rows (S3): one record per processed row, block b at row offset N*off[b]:
-//   rh = R^ (fp32, unweighted), id = {sorted atom, k | pad << 30}; rows of atom i start at rowstart[b][i].
+//   rh = R^ (fp32, unweighted), id = {sorted atom, neighbour j (sorted index)} for a real row and {sorted atom, -npad}
+//   for the representative of the npad padded slots; rows of atom i start at rowstart[b][i].
 __global__ void __launch_bounds__(256)
 k_env_rows(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, EnvParams ep, const double *__restrict__ avg,
            const double *__restrict__ stdv, const int *__restrict__ bin_start, const double *__restrict__ xs,
@@ -177,7 +178,7 @@ k_env_rows(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, EnvParams ep,
             }
             rows_rh[base + k] = make_float4((float)((Rt[0] - av[0]) / sd[0]), (float)((Rt[1] - av[1]) / sd[1]),
                                             (float)((Rt[2] - av[2]) / sd[2]), (float)((Rt[3] - av[3]) / sd[3]));
-            rows_id[base + k] = make_int2((int)i, k | (k >= nr ? (1 << 30) : 0));
+            rows_id[base + k] = make_int2((int)i, k < nr ? nlist[i * Nm + off[b] + k] : -(sel[b] - nr));
         }
     }
 }
@@ -249,7 +250,7 @@ k_embed_fwd_tc(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, const Emb
                         rh = rows_rh[rbase + r0 + row];
                         const int2 id = rows_id[rbase + r0 + row];
                         atom = id.x;
-                        wgt = (id.y >> 30) ? (float)(sel[b] - (id.y & 0x3FFFFFFF)) : 1.f;
+                        wgt = id.y < 0 ? (float)(-id.y) : 1.f;
                     }
                     sS[row] = rh.x;
                     if (row == 0) meta->atom0 = atom;

@@ -145,7 +145,7 @@ k_embed_fwd_tc2(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, const Em
             const int tile0 = (int)((long)ntiles * gw / G), tile1 = (int)((long)ntiles * (gw + 1) / G);
             int pending = -1;
             float4 nrh = make_float4(0.f, 0.f, 0.f, 0.f);
-            int2 nid = make_int2(-1, 0);
+            int2 nid = make_int2(-1, 1);
             if (tile0 < tile1) {
                 const int r0 = rs + tile0 * T2_ROWS;
                 if (r0 + t < re) { nrh = __ldg(&rows_rh[rbase + r0 + t]); nid = __ldg(&rows_id[rbase + r0 + t]); }
@@ -156,13 +156,13 @@ k_embed_fwd_tc2(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, const Em
                 const float4 rh = nrh;
                 const int2 id = nid;
                 nrh = make_float4(0.f, 0.f, 0.f, 0.f);
-                nid = make_int2(-1, 0);
+                nid = make_int2(-1, 1);
                 if (tile + 1 < tile1 && r0 + T2_ROWS + t < re) {
                     nrh = __ldg(&rows_rh[rbase + r0 + T2_ROWS + t]);
                     nid = __ldg(&rows_id[rbase + r0 + T2_ROWS + t]);
                 }
                 const int atom = id.x;
-                const float wgt = (id.y >> 30) ? (float)(sel[b] - (id.y & 0x3FFFFFFF)) : 1.f;
+                const float wgt = id.y < 0 ? (float)(-id.y) : 1.f;
                 if (t == 0) meta[0] = atom;
                 if (t == nrows - 1) meta[1] = atom;
                 // ---- E1: layer 1 on the ALUs ----

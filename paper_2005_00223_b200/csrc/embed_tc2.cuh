@@ -29,6 +29,6 @@ struct EmbedNetTC2 {
     __half W2[T2_K1 / 8][64][8];                 // layer 2: A = t1 block (K = 32), N = 64 (50 real)
     __half W3[(T2_K2 + T2_K1) / 8][112][8];      // layer 3: A = t2 block then t1 block (K = 96), N = 112 (100 real)
     // backward (A operands dz3 [K = 112], dz2 [K = 64])
-    __half W3T[T2_K3 / 8][96][8];                // n < 64: dy2[f] += dz3[m] W3[f][m];  n = 64 + e: dy1[e] += dz3[m] (W3[e][m] + W3[e+25][m])
+    __half W3T[T2_K3 / 8][96][8];                // n = e < 32: dy1[e] += dz3[m] (W3[e][m] + W3[e+25][m]);  n = 32 + f: dy2[f] += dz3[m] W3[f][m]
     __half W2T[T2_K2 / 8][32][8];                // dy1[e] += dz2[f] W2[e][f]
 };

@@ -1,0 +1,621 @@
+// S7 + S8 + S9 (embedding backward, ProdForce, ProdViral) on tcgen05 tensor cores, MIX-16.
+//
+// One warpgroup = one 128-row tile (thread = neighbour row = TMEM lane), two warpgroups per CTA, one CTA per SM.
+// The forward is recomputed (storing the tanh outputs would cost 94 GB at config 4) with the
+// activations carried as fp16 hi + lo pairs: the hi parts live in TMEM and feed tcgen05.mma as the A operand, the lo
+// parts in shared memory.  With t_l = tanh(z_l) and T = [t1 | t2 | t3] (embed_tc2.cuh) the residual folds are linear, so
+//   dR^[k][c]  = sum_col T[k][col] g~[c][col]                      (g~ = gA folded onto the T columns, per atom)
+//   dT[k][col] = sum_c R^[k][c] g~[c][col]                         (direct part of every layer's gradient)
+//   dz3 = dT3 (1 - t3^2);   dy2 = dT2 + dz3 W3^T;   dz2 = dy2 (1 - t2^2)
+//   dy1 = dT1 + dz3 (W3^T folded) + dz2 W2^T;   dz1 = dy1 (1 - t1^2);   ds^ = dz1 . w1
+// followed, per row, by the fp64 geometry derivative, the force scatter and the virial (S8, S9).
+// Per-atom operand images g~ (hi, lo) come from k_gA_img (the tail of the fitting backward), scaled by a power of two.
+#include <cstdlib>
+#include "embed_tc2.cuh"
+#include "tc_common.cuh"
+
+namespace {
+
+constexpr int NWG = 2;
+// TMEM columns per warpgroup
+constexpr int TM_T = 0;                        // T hi parts, packed fp16 pairs: t1 [0,16) t2 [16,48) t3 [48,104)
+constexpr int TM_Z = 112;                      // accumulator: z2 -> z3 -> dT3 -> [dy2 | dy1]      (112 columns)
+constexpr int TM_DR = 224;                     // dR^: 2 slots x 8 columns
+constexpr int TM_WG = 256;
+
+struct BwdSmem {
+    static constexpr int W2 = 0;                                   // [4][64][16 B]
+    static constexpr int W3 = W2 + 4 * 64 * 16;                    // [12][112][16 B]
+    static constexpr int W3T = W3 + 12 * 112 * 16;                 // [14][96][16 B]
+    static constexpr int W2T = W3T + 14 * 96 * 16;                 // [8][32][16 B]
+    static constexpr int VEC = W2T + 8 * 32 * 16;                  // w1[32] b1[32]
+    static constexpr int BARS = VEC + 256;
+    static constexpr int WG0 = ((BARS + 64 + 1023) / 1024) * 1024;
+    // per warpgroup
+    static constexpr int TLO = 0;                                  // T lo parts / dz2 / dz3: 26 chunks x 2 KB
+    static constexpr int RIMG = TLO + T2_CHUNKS * 2048;            // A of the direct products: [4][128][16 B]
+    static constexpr int QIMG = RIMG + 4 * 2048;                   // per slot two copies of the atom's gradient image C [208][16 B]:
+                                                                   // K-major B of the direct products (K = 16 per slot) and,
+                                                                   // viewed MN-major (chunks 0 and 2), B of the dR^ product (N = 16)
+    static constexpr int META = QIMG + 4 * T2_COLS * 16;
+    static constexpr int WG_BYTES = ((META + 512 + 127) / 128) * 128;
+    static constexpr int TOTAL = WG0 + NWG * WG_BYTES;
+};
+static_assert(BwdSmem::TOTAL <= 227 * 1024, "shared memory budget");
+
+__device__ __forceinline__ double min_image(double t, double L, double halfL) {
+    double s = t > halfL ? -1.0 : (t < -halfL ? 1.0 : 0.0);
+    return __dadd_rn(t, __dmul_rn(s, L));
+}
+struct EnvParams {
+    double rc, rc_smth, inv_range;
+    double L[3];
+};
+
+__device__ __forceinline__ void cp_async16(uint32_t sdst, const void *gsrc) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sdst), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// prefetch loads that the compiler must keep where they are written (issued one tile ahead of their use)
+__device__ __forceinline__ float4 ldv_f4(const float4 *p) {
+    float4 r;
+    asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ int2 ldv_i2(const int2 *p) {
+    int2 r;
+    asm volatile("ld.global.nc.v2.s32 {%0,%1}, [%2];" : "=r"(r.x), "=r"(r.y) : "l"(p));
+    return r;
+}
+
+__device__ __forceinline__ float2 unpack_h2(uint32_t v) {
+    return __half22float2(*reinterpret_cast<const __half2 *>(&v));
+}
+
+// 16 accumulator columns: t = tanh(z); hi parts -> 8 TMEM columns, lo parts -> two 16-byte chunks, 1 - t^2 -> dpk (fp16 pairs)
+__device__ __forceinline__ void act16(const uint32_t (&z)[16], uint32_t tm_dst, uint8_t *lo_row, int chunk, uint32_t *dpk) {
+    uint32_t hi[8], lo[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        const float x = tc::tanh_approx(__uint_as_float(z[2 * q])), y = tc::tanh_approx(__uint_as_float(z[2 * q + 1]));
+        tc::split_h2(x, y, hi[q], lo[q]);
+        dpk[q] = tc::pack_h2(fmaf(-x, x, 1.f), fmaf(-y, y, 1.f));
+    }
+    tc::st8(tm_dst, hi);
+    *reinterpret_cast<uint4 *>(lo_row + chunk * 2048) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+    *reinterpret_cast<uint4 *>(lo_row + (chunk + 1) * 2048) = make_uint4(lo[4], lo[5], lo[6], lo[7]);
+}
+// 16 gradient columns times 1 - t^2 -> fp16 -> two chunks
+__device__ __forceinline__ void grad16(const uint32_t (&g)[16], const uint32_t *dpk, uint8_t *row, int chunk) {
+    uint32_t o[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        const float2 d = unpack_h2(dpk[q]);
+        o[q] = tc::pack_h2(__uint_as_float(g[2 * q]) * d.x, __uint_as_float(g[2 * q + 1]) * d.y);
+    }
+    *reinterpret_cast<uint4 *>(row + chunk * 2048) = make_uint4(o[0], o[1], o[2], o[3]);
+    *reinterpret_cast<uint4 *>(row + (chunk + 1) * 2048) = make_uint4(o[4], o[5], o[6], o[7]);
+}
+
+// Per-atom operand image of the folded gradient g~[c][col] = fold(gA)[c][col] * 2^e, split in hi + lo fp16 parts:
+//   C [208][8] : per T column {hi[0..3], lo[0..3]} (16 bytes)
+// gA[c][m] = sum_a gD[m][a] A[c][a] + [m < 16] sum_m' gD[m'][m] A[c][m'], fp32.
+constexpr int GA_IMG_BYTES = T2_COLS * 16;    // 3,328 per atom
+__global__ void __launch_bounds__(128) k_gA_img(long N, const float *__restrict__ Amat, const float *__restrict__ gD,
+                                                 uint8_t *__restrict__ img, float *__restrict__ gscale) {
+    extern __shared__ float smg[];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const long i = blockIdx.x * 4L + wid;
+    if (i >= N) return;
+    float *sA = smg + wid * (4 * M2E + M2E * 16 + 4 * M2E);
+    float *sG = sA + 4 * M2E;
+    float *sO = sG + M2E * 16;
+    {
+        const float4 *a4 = reinterpret_cast<const float4 *>(Amat + i * 4 * M2E);
+        const float4 *g4 = reinterpret_cast<const float4 *>(gD + i * (M2E * 16));
+        for (int k = lane; k < M2E; k += 32) reinterpret_cast<float4 *>(sA)[k] = a4[k];
+        for (int k = lane; k < M2E * 4; k += 32) reinterpret_cast<float4 *>(sG)[k] = g4[k];
+    }
+    __syncwarp();
+    for (int idx = lane; idx < 4 * M2E; idx += 32) {
+        const int c = idx / M2E, m = idx % M2E;
+        float acc = 0.f;
+#pragma unroll
+        for (int ax = 0; ax < 16; ++ax) acc = fmaf(sG[m * 16 + ax], sA[c * M2E + ax], acc);
+        if (m < 16)
+            for (int mp = 0; mp < M2E; ++mp) acc = fmaf(sG[mp * 16 + m], sA[c * M2E + mp], acc);
+        sO[idx] = acc;
+    }
+    __syncwarp();
+    // fold onto the T columns (reuse sG as [4][208])
+    float mx = 0.f;
+    for (int idx = lane; idx < 4 * T2_COLS; idx += 32) {
+        const int c = idx / T2_COLS, col = idx % T2_COLS;
+        const float *o = sO + c * M2E;
+        float v = 0.f;
+        if (col < T2_O2) { if (col < M0) v = (o[col] + o[col + M0]) + (o[col + 2 * M0] + o[col + 3 * M0]); }
+        else if (col < T2_O3) { const int f = col - T2_O2; if (f < M1) v = o[f] + o[f + M1]; }
+        else { const int m = col - T2_O3; if (m < M2E) v = o[m]; }
+        sG[idx] = v;
+        mx = fmaxf(mx, fabsf(v));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    int ex = 0;
+    if (mx > 0.f) frexpf(mx, &ex);
+    const float sc = ldexpf(1.f, -ex);          // max |g~| in [0.5, 1)
+    if (lane == 0) gscale[i] = sc;
+    __syncwarp();
+    uint4 *C = reinterpret_cast<uint4 *>(img + i * (long)GA_IMG_BYTES);
+    for (int col = lane; col < T2_COLS; col += 32) {
+        uint32_t h01, l01, h23, l23;
+        tc::split_h2(sG[col] * sc, sG[T2_COLS + col] * sc, h01, l01);
+        tc::split_h2(sG[2 * T2_COLS + col] * sc, sG[3 * T2_COLS + col] * sc, h23, l23);
+        C[col] = make_uint4(h01, h23, l01, l23);
+    }
+}
+
+// hi parts -> 8 TMEM columns, lo parts -> two 16-byte chunks, 1 - t^2 -> dpk (fp16 pairs); t given in fp32
+__device__ __forceinline__ void emit16(const float (&y)[16], uint32_t tm_dst, uint8_t *lo_row, int chunk, uint32_t *dpk) {
+    uint32_t hi[8], lo[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        tc::split_h2(y[2 * q], y[2 * q + 1], hi[q], lo[q]);
+        dpk[q] = tc::pack_h2(fmaf(-y[2 * q], y[2 * q], 1.f), fmaf(-y[2 * q + 1], y[2 * q + 1], 1.f));
+    }
+    tc::st8(tm_dst, hi);
+    *reinterpret_cast<uint4 *>(lo_row + chunk * 2048) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+    *reinterpret_cast<uint4 *>(lo_row + (chunk + 1) * 2048) = make_uint4(lo[4], lo[5], lo[6], lo[7]);
+}
+__device__ __forceinline__ uint32_t hmul2(uint32_t a, uint32_t b) {
+    __half2 r = __hmul2(*reinterpret_cast<const __half2 *>(&a), *reinterpret_cast<const __half2 *>(&b));
+    return *reinterpret_cast<uint32_t *>(&r);
+}
+// 16 gradient columns (fp32 accumulators) times 1 - t^2 (fp16 pairs) -> fp16 -> two chunks
+__device__ __forceinline__ void gradh16(const uint32_t (&g)[16], const uint32_t *dpk, uint8_t *row, int chunk) {
+    uint32_t o[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) o[q] = hmul2(tc::pack_h2(__uint_as_float(g[2 * q]), __uint_as_float(g[2 * q + 1])), dpk[q]);
+    *reinterpret_cast<uint4 *>(row + chunk * 2048) = make_uint4(o[0], o[1], o[2], o[3]);
+    *reinterpret_cast<uint4 *>(row + (chunk + 1) * 2048) = make_uint4(o[4], o[5], o[6], o[7]);
+}
+
+constexpr int WGT = 128;       // threads per warpgroup: thread = row; every stage walks its two column halves h = 0, 1
+
+__global__ void __launch_bounds__(NWG * WGT, 1)
+k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, EnvParams ep, const EmbedNetTC2 *__restrict__ nets,
+                const double *__restrict__ stdv, const int *__restrict__ bin_start, const int *__restrict__ rowstart,
+                const float4 *__restrict__ rows_rh, const int2 *__restrict__ rows_id, const double *__restrict__ xs,
+                const uint8_t *__restrict__ gimg, const float *__restrict__ gscale, double *__restrict__ fsorted,
+                double *__restrict__ virial, unsigned long long *__restrict__ row_counter) {
+    using SL = BwdSmem;
+    extern __shared__ __align__(1024) uint8_t smem[];
+    __shared__ uint32_t tmem_base_s;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int wg = warp >> 2, t = tid & (WGT - 1), tw = t;
+    float *sw1 = reinterpret_cast<float *>(smem + SL::VEC), *sb1 = sw1 + 32;
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + SL::BARS);
+    uint8_t *wgs = smem + SL::WG0 + wg * SL::WG_BYTES;
+    uint8_t *lo_row = wgs + SL::TLO + t * 16;
+    const int off[4] = {off4.x, off4.y, off4.z, off4.w};
+    const double hx = 0.5 * ep.L[0], hy = 0.5 * ep.L[1], hz = 0.5 * ep.L[2];
+
+    if (tid == 0) {
+        for (int k = 0; k < NWG; ++k) tc::mbar_init(&bars[k], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tc::smem_u32(&tmem_base_s)), "n"(512));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    for (int k = tw; k < SL::WG_BYTES / 16; k += WGT) reinterpret_cast<uint4 *>(wgs)[k] = make_uint4(0u, 0u, 0u, 0u);
+    tc::fence_before();
+    __syncthreads();
+    tc::fence_after();
+    const uint32_t tmem = tmem_base_s + wg * TM_WG;
+    const uint32_t tm_lane = tmem + ((uint32_t)((warp & 3) * 32) << 16);
+    const uint32_t sbase = tc::smem_u32(smem);
+    const uint32_t s_tlo = tc::smem_u32(wgs + SL::TLO), s_rimg = tc::smem_u32(wgs + SL::RIMG);
+    const uint32_t s_qimg = tc::smem_u32(wgs + SL::QIMG);
+    uint64_t *bar = &bars[wg];
+    uint32_t ph = 0;
+    unsigned long long my_rows = 0;
+    double vir[9];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) vir[k] = 0.0;
+    // zero the T hi region once: its padding columns are read as K of the products and must stay finite (zero)
+    {
+        uint32_t z8[8] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
+#pragma unroll
+        for (int c = 0; c < 104; c += 8) tc::st8(tm_lane + TM_T + c, z8);
+    }
+    tc::wait_st();
+
+    auto sync_issue = [&]() {          // make this warpgroup's operand writes visible to the tensor core, then meet
+        tc::proxy_fence();
+        tc::fence_before();
+        tc::bar_sync(1 + wg, WGT);
+    };
+    auto wait_mma = [&]() {
+        tc::mbar_wait(bar, ph); ph ^= 1;
+        tc::fence_after();
+    };
+
+    for (int a = 0; a < T; ++a) {
+        const int ts0 = bin_start[a * ncell], ts1 = bin_start[(a + 1) * ncell];
+        if (ts0 == ts1) continue;
+        const float isd[4] = {(float)(1.0 / stdv[4 * a]), (float)(1.0 / stdv[4 * a + 1]), (float)(1.0 / stdv[4 * a + 2]),
+                              (float)(1.0 / stdv[4 * a + 3])};
+        for (int b = 0; b < T; ++b) {
+            const long rbase = N * (long)off[b];
+            const int rs = rowstart[(long)b * (N + 1) + ts0], re = rowstart[(long)b * (N + 1) + ts1];
+            const int ntiles = (re - rs + T2_ROWS - 1) / T2_ROWS;
+            __syncthreads();
+            {   // stage the (a, b) net
+                const EmbedNetTC2 *net = nets + (a * T + b);
+                const uint4 *src = reinterpret_cast<const uint4 *>(&net->W2[0][0][0]);
+                constexpr int NW = (4 * 64 + 12 * 112 + 14 * 96 + 8 * 32);
+                for (int k = tid; k < NW; k += NWG * WGT) reinterpret_cast<uint4 *>(smem + SL::W2)[k] = src[k];
+                if (tid < 64) sw1[tid] = reinterpret_cast<const float *>(net)[tid];
+            }
+            tc::proxy_fence();
+            __syncthreads();
+            const int G = gridDim.x * NWG, gw = blockIdx.x * NWG + wg;
+            const int tile0 = (int)((long)ntiles * gw / G), tile1 = (int)((long)ntiles * (gw + 1) / G);
+            float4 nrh = make_float4(0.f, 0.f, 0.f, 0.f);
+            int2 nid = make_int2(-1, -1);
+            int na0 = 0, naL = -1;                      // first and last atom of the next tile (uniform loads)
+            if (tile0 < tile1) {
+                const int r0 = rs + tile0 * T2_ROWS;
+                if (r0 + t < re) { nrh = ldv_f4(&rows_rh[rbase + r0 + t]); nid = ldv_i2(&rows_id[rbase + r0 + t]); }
+                na0 = ldv_i2(&rows_id[rbase + r0]).x;
+                naL = ldv_i2(&rows_id[rbase + min(r0 + T2_ROWS, re) - 1]).x;
+            }
+            for (int tile = tile0; tile < tile1; ++tile) {
+                const int r0 = rs + tile * T2_ROWS;
+                const int nrows = min(T2_ROWS, re - r0);
+                const float4 rh = nrh;
+                const int2 id = nid;
+                const int atom0 = na0, atomL = naL;
+                nrh = make_float4(0.f, 0.f, 0.f, 0.f);
+                nid = make_int2(-1, -1);
+                if (tile + 1 < tile1) {
+                    const int r1 = r0 + T2_ROWS;
+                    if (r1 + t < re) { nrh = ldv_f4(&rows_rh[rbase + r1 + t]); nid = ldv_i2(&rows_id[rbase + r1 + t]); }
+                    na0 = ldv_i2(&rows_id[rbase + r1]).x;
+                    naL = ldv_i2(&rows_id[rbase + min(r1 + T2_ROWS, re) - 1]).x;
+                }
+                const int atom = id.x;
+                // T2_NSLOT atoms per pass; a tile that spans more atoms (short neighbour blocks) is recomputed per pass
+                for (int p0 = atom0; p0 <= atomL; p0 += T2_NSLOT) {
+                    const bool in = atom >= p0 && atom - p0 < T2_NSLOT;
+                    const int slot = atom & (T2_NSLOT - 1);
+                    // operand images of this pass: R (A of the direct products) and the per-atom gradient images (async copies)
+                    {
+                        uint32_t rh01, rl01, rh23, rl23;
+                        tc::split_h2(rh.x, rh.y, rh01, rl01);
+                        tc::split_h2(rh.z, rh.w, rh23, rl23);
+                        const uint4 c0 = make_uint4(rh01, rh23, rh01, rh23), c1 = make_uint4(rl01, rl23, 0u, 0u), z4 = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+                        for (int s_ = 0; s_ < T2_NSLOT; ++s_) {
+                            const bool mine = in && slot == s_;
+                            *reinterpret_cast<uint4 *>(wgs + SL::RIMG + (2 * s_) * 2048 + t * 16) = mine ? c0 : z4;
+                            *reinterpret_cast<uint4 *>(wgs + SL::RIMG + (2 * s_ + 1) * 2048 + t * 16) = mine ? c1 : z4;
+                        }
+                    }
+                    for (int q = p0; q < p0 + T2_NSLOT && q <= atomL; ++q) {
+                        const int s_ = q & (T2_NSLOT - 1);
+                        const uint4 *C = reinterpret_cast<const uint4 *>(gimg + (long)q * GA_IMG_BYTES);
+                        for (int k = tw; k < T2_COLS; k += WGT) {
+                            cp_async16(s_qimg + (2 * s_) * (T2_COLS * 16) + k * 16, C + k);
+                            cp_async16(s_qimg + (2 * s_ + 1) * (T2_COLS * 16) + k * 16, C + k);
+                        }
+                    }
+                    uint32_t d1p[2][8], d2p[2][16], d3p[2][26];       // 1 - t^2 per column half (fp16 pairs)
+                    // ---- E1: layer 1 on the ALUs; h = 0: t1[0..16), h = 1: t1[16..25), ones, padding ----
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const float s = rh.x;
+                        float y[16];
+#pragma unroll
+                        for (int e = 0; e < 16; ++e) {
+                            const int ee = 16 * h + e;
+                            if (ee < 25) y[e] = tc::tanh_approx(fmaf(s, sw1[ee], sb1[ee]));
+                            else y[e] = ee <= 26 ? 1.f : 0.f;
+                        }
+                        emit16(y, tm_lane + TM_T + 8 * h, lo_row, 2 * h, d1p[h]);
+                    }
+                    tc::wait_st();
+                    sync_issue();
+                    if (tw == 0) {
+                        tc::fence_after();
+                        constexpr uint32_t id2 = tc::idesc(128, 64, false, false);
+#pragma unroll
+                        for (int ks = 0; ks < 2; ++ks) {
+                            const uint64_t db = tc::desc(sbase + SL::W2 + ks * 2 * (64 * 16), 64 * 16, 128);
+                            tc::mma_ts(tmem + TM_Z, tmem + TM_T + 8 * ks, db, id2, ks > 0);
+                            tc::mma_ss(tmem + TM_Z, tc::desc(s_tlo + ks * 2 * 2048, 2048, 128), db, id2, true);
+                        }
+                        tc::commit(bar);
+                    }
+                    wait_mma();
+                    // ---- E2: h = 0: t2[0..32), h = 1: t2[32..50) ----
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        uint8_t *img = lo_row + (T2_O2 / 8) * 2048;
+                        uint32_t z0[16], z1[16];
+                        tc::ld16(tm_lane + TM_Z + 32 * h, z0);
+                        if (h == 0) tc::ld16(tm_lane + TM_Z + 16, z1);
+                        else tc::ld2(tm_lane + TM_Z + 48, reinterpret_cast<uint32_t (&)[2]>(z1));
+                        tc::wait_ld();
+                        act16(z0, tm_lane + TM_T + 16 + 16 * h, img, 4 * h, d2p[h]);
+                        if (h == 0) {
+                            act16(z1, tm_lane + TM_T + 24, img, 2, d2p[h] + 8);
+                        } else {
+                            const float x = tc::tanh_approx(__uint_as_float(z1[0])), y = tc::tanh_approx(__uint_as_float(z1[1]));
+                            uint32_t hi, lo;
+                            tc::split_h2(x, y, hi, lo);
+                            d2p[h][8] = tc::pack_h2(fmaf(-x, x, 1.f), fmaf(-y, y, 1.f));
+                            tc::st4(tm_lane + TM_T + 40, hi, 0u, 0u, 0u);
+                            *reinterpret_cast<uint4 *>(img + 6 * 2048) = make_uint4(lo, 0u, 0u, 0u);
+                        }
+                    }
+                    tc::wait_st();
+                    sync_issue();
+                    if (tw == 0) {
+                        tc::fence_after();
+                        constexpr uint32_t id3 = tc::idesc(128, 112, false, false);
+#pragma unroll
+                        for (int ks = 0; ks < 6; ++ks) {
+                            const int acol = ks < 4 ? 16 + 8 * ks : 8 * (ks - 4);              // TMEM column of the hi part
+                            const int achunk = ks < 4 ? T2_O2 / 8 + 2 * ks : 2 * (ks - 4);     // chunk of the lo part
+                            const uint64_t db = tc::desc(sbase + SL::W3 + ks * 2 * (112 * 16), 112 * 16, 128);
+                            tc::mma_ts(tmem + TM_Z, tmem + TM_T + acol, db, id3, ks > 0);
+                            tc::mma_ss(tmem + TM_Z, tc::desc(s_tlo + achunk * 2048, 2048, 128), db, id3, true);
+                        }
+                        tc::commit(bar);
+                    }
+                    wait_mma();
+                    // ---- E3: h = 0: t3[0..48), h = 1: t3[48..100) ----
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        uint8_t *img = lo_row + (T2_O3 / 8 + 6 * h) * 2048;
+#pragma unroll
+                        for (int u = 0; u < 3; ++u) {
+                            uint32_t z0[16];
+                            tc::ld16(tm_lane + TM_Z + 48 * h + 16 * u, z0);
+                            tc::wait_ld();
+                            act16(z0, tm_lane + TM_T + 48 + 24 * h + 8 * u, img, 2 * u, d3p[h] + 8 * u);
+                        }
+                        if (h == 1) {
+                            uint32_t z3[4];
+                            tc::ld4(tm_lane + TM_Z + 96, z3);
+                            tc::wait_ld();
+                            const float x0 = tc::tanh_approx(__uint_as_float(z3[0])), x1 = tc::tanh_approx(__uint_as_float(z3[1]));
+                            const float x2 = tc::tanh_approx(__uint_as_float(z3[2])), x3 = tc::tanh_approx(__uint_as_float(z3[3]));
+                            uint32_t h0, l0, h1, l1;
+                            tc::split_h2(x0, x1, h0, l0); tc::split_h2(x2, x3, h1, l1);
+                            d3p[h][24] = tc::pack_h2(fmaf(-x0, x0, 1.f), fmaf(-x1, x1, 1.f));
+                            d3p[h][25] = tc::pack_h2(fmaf(-x2, x2, 1.f), fmaf(-x3, x3, 1.f));
+                            tc::st4(tm_lane + TM_T + 96, h0, h1, 0u, 0u);
+                            *reinterpret_cast<uint4 *>(img + 6 * 2048) = make_uint4(l0, l1, 0u, 0u);
+                        }
+                    }
+                    tc::wait_st();
+                    // ---- backward ----
+                    cp_async_wait_all();
+                    sync_issue();
+                    if (tw == 0) {
+                        tc::fence_after();
+                        constexpr uint32_t idr = tc::idesc(128, 8 * T2_NSLOT, false, true);
+#pragma unroll
+                        for (int ks = 0; ks < T2_COLS / 16; ++ks) {
+                            const uint64_t db = tc::desc(s_qimg + ks * 256, 128, 2 * T2_COLS * 16);
+                            tc::mma_ts(tmem + TM_DR, tmem + TM_T + 8 * ks, db, idr, ks > 0);
+                            tc::mma_ss(tmem + TM_DR, tc::desc(s_tlo + ks * 2 * 2048, 2048, 128), db, idr, true);
+                        }
+                        constexpr uint32_t idg = tc::idesc(128, T2_K3, false, false);
+#pragma unroll
+                        for (int ks = 0; ks < T2_NSLOT; ++ks)
+                            tc::mma_ss(tmem + TM_Z, tc::desc(s_rimg + ks * 2 * 2048, 2048, 128),
+                                       tc::desc(s_qimg + T2_O3 * 16 + ks * 2 * (T2_COLS * 16), T2_COLS * 16, 128), idg, ks > 0);
+                        tc::commit(bar);
+                    }
+                    // prefetch the geometry of this row while the products run
+                    const bool real = in && id.y >= 0;
+                    double xj = 0.0, yj = 0.0, zj = 0.0, xc = 0.0, yc = 0.0, zc = 0.0;
+                    float gsc = 1.f;
+                    if (real) {
+                        const int j = id.y;
+                        xj = xs[3 * (long)j]; yj = xs[3 * (long)j + 1]; zj = xs[3 * (long)j + 2];
+                        xc = xs[3 * (long)atom]; yc = xs[3 * (long)atom + 1]; zc = xs[3 * (long)atom + 2];
+                        gsc = __ldg(&gscale[atom]);
+                    }
+                    wait_mma();
+                    // ---- E4: dR^ of this row; dz3 = dT3 (1 - t3^2) -> t3 block of the lo image ----
+                    float dR[4];
+                    {
+                        uint32_t v[16];                      // both slots: tcgen05.ld takes one warp-uniform address
+                        tc::ld16(tm_lane + TM_DR, v);
+#pragma unroll
+                        for (int h = 0; h < 2; ++h) {
+                            uint8_t *img = lo_row + (T2_O3 / 8 + 6 * h) * 2048;
+#pragma unroll
+                            for (int u = 0; u < 3; ++u) {
+                                uint32_t g0[16];
+                                tc::ld16(tm_lane + TM_Z + 48 * h + 16 * u, g0);
+                                tc::wait_ld();
+                                gradh16(g0, d3p[h] + 8 * u, img, 2 * u);
+                            }
+                            if (h == 1) {
+                                uint32_t g3[4];
+                                tc::ld4(tm_lane + TM_Z + 96, g3);
+                                tc::wait_ld();
+                                *reinterpret_cast<uint4 *>(img + 6 * 2048) =
+                                    make_uint4(hmul2(tc::pack_h2(__uint_as_float(g3[0]), __uint_as_float(g3[1])), d3p[h][24]),
+                                               hmul2(tc::pack_h2(__uint_as_float(g3[2]), __uint_as_float(g3[3])), d3p[h][25]), 0u, 0u);
+                            }
+                        }
+#pragma unroll
+                        for (int c = 0; c < 4; ++c)
+                            dR[c] = slot ? __uint_as_float(v[8 + c]) + __uint_as_float(v[12 + c]) : __uint_as_float(v[c]) + __uint_as_float(v[4 + c]);
+                    }
+                    sync_issue();
+                    if (tw == 0) {
+                        tc::fence_after();
+                        // dy2 first (the next stage needs it) ...
+                        constexpr uint32_t idy2 = tc::idesc(128, 64, false, false);
+#pragma unroll
+                        for (int ks = 0; ks < T2_NSLOT; ++ks)      // direct part dT2 -> accumulator columns [32,96)
+                            tc::mma_ss(tmem + TM_Z + 32, tc::desc(s_rimg + ks * 2 * 2048, 2048, 128),
+                                       tc::desc(s_qimg + T2_O2 * 16 + ks * 2 * (T2_COLS * 16), T2_COLS * 16, 128), idy2, ks > 0);
+#pragma unroll
+                        for (int ks = 0; ks < T2_K3 / 16; ++ks)
+                            tc::mma_ss(tmem + TM_Z + 32, tc::desc(s_tlo + (T2_O3 / 8 + 2 * ks) * 2048, 2048, 128),
+                                       tc::desc(sbase + SL::W3T + 32 * 16 + ks * 2 * (96 * 16), 96 * 16, 128), idy2, true);
+                        tc::commit(bar);
+                        // ... then the part of dy1 that does not depend on dz2 (waited for with the last stage)
+                        constexpr uint32_t idy1 = tc::idesc(128, 32, false, false);
+#pragma unroll
+                        for (int ks = 0; ks < T2_NSLOT; ++ks)      // direct part dT1 -> accumulator columns [0,32)
+                            tc::mma_ss(tmem + TM_Z, tc::desc(s_rimg + ks * 2 * 2048, 2048, 128),
+                                       tc::desc(s_qimg + ks * 2 * (T2_COLS * 16), T2_COLS * 16, 128), idy1, ks > 0);
+#pragma unroll
+                        for (int ks = 0; ks < T2_K3 / 16; ++ks)
+                            tc::mma_ss(tmem + TM_Z, tc::desc(s_tlo + (T2_O3 / 8 + 2 * ks) * 2048, 2048, 128),
+                                       tc::desc(sbase + SL::W3T + ks * 2 * (96 * 16), 96 * 16, 128), idy1, true);
+                    }
+                    wait_mma();
+                    // ---- E5: dz2 = dy2 (1 - t2^2) -> t2 block of the lo image ----
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        uint8_t *img = lo_row + (T2_O2 / 8) * 2048;
+                        uint32_t g0[16], g1[16];
+                        tc::ld16(tm_lane + TM_Z + 32 + 32 * h, g0);
+                        if (h == 0) tc::ld16(tm_lane + TM_Z + 48, g1);
+                        else tc::ld2(tm_lane + TM_Z + 80, reinterpret_cast<uint32_t (&)[2]>(g1));
+                        tc::wait_ld();
+                        gradh16(g0, d2p[h], img, 4 * h);
+                        if (h == 0) gradh16(g1, d2p[h] + 8, img, 2);
+                        else *reinterpret_cast<uint4 *>(img + 6 * 2048) =
+                                 make_uint4(hmul2(tc::pack_h2(__uint_as_float(g1[0]), __uint_as_float(g1[1])), d2p[h][8]), 0u, 0u, 0u);
+                    }
+                    sync_issue();
+                    if (tw == 0) {
+                        tc::fence_after();
+                        constexpr uint32_t id1 = tc::idesc(128, 32, false, false);
+#pragma unroll
+                        for (int ks = 0; ks < T2_K2 / 16; ++ks)
+                            tc::mma_ss(tmem + TM_Z, tc::desc(s_tlo + (T2_O2 / 8 + 2 * ks) * 2048, 2048, 128),
+                                       tc::desc(sbase + SL::W2T + ks * 2 * (32 * 16), 32 * 16, 128), id1, true);
+                        tc::commit(bar);
+                    }
+                    wait_mma();
+                    // ---- E6: ds^ = sum_e dy1 (1 - t1^2) w1; gradient of the environment row; S8 + S9 in fp64 ----
+                    {
+                        float ds = 0.f;
+#pragma unroll
+                        for (int h = 0; h < 2; ++h) {
+                            uint32_t g0[16];
+                            tc::ld16(tm_lane + TM_Z + 16 * h, g0);
+                            tc::wait_ld();
+#pragma unroll
+                            for (int q = 0; q < 8; ++q) {
+                                const float2 d = unpack_h2(d1p[h][q]);
+                                if (16 * h + 2 * q < 25) ds = fmaf(__uint_as_float(g0[2 * q]) * d.x, sw1[16 * h + 2 * q], ds);
+                                if (16 * h + 2 * q + 1 < 25) ds = fmaf(__uint_as_float(g0[2 * q + 1]) * d.y, sw1[16 * h + 2 * q + 1], ds);
+                            }
+                        }
+                        double gk[3] = {0.0, 0.0, 0.0};
+                        if (real) {
+                            const float osc = 1.0f / ((float)Nm * gsc);
+                            const double g0_ = (double)((dR[0] + ds) * osc * isd[0]), g1_ = (double)(dR[1] * osc * isd[1]);
+                            const double g2_ = (double)(dR[2] * osc * isd[2]), g3_ = (double)(dR[3] * osc * isd[3]);
+                            const int j = id.y;
+                            const double dx = min_image(xj - xc, ep.L[0], hx);
+                            const double dy = min_image(yj - yc, ep.L[1], hy);
+                            const double dz = min_image(zj - zc, ep.L[2], hz);
+                            const double r2 = dx * dx + dy * dy + dz * dz;
+                            const double r = sqrt(r2), ir = 1.0 / r;
+                            double w = 1.0, dw = 0.0;
+                            if (r >= ep.rc_smth) {
+                                if (r < ep.rc) {
+                                    const double u = (r - ep.rc_smth) * ep.inv_range;
+                                    w = u * u * u * (-6.0 * u * u + 15.0 * u - 10.0) + 1.0;
+                                    dw = -30.0 * u * u * (u - 1.0) * (u - 1.0) * ep.inv_range;
+                                } else {
+                                    w = 0.0;
+                                }
+                            }
+                            const double s = w * ir;
+                            const double sp = dw * ir - w * ir * ir;          // ds/dr
+                            const double gd = g1_ * dx + g2_ * dy + g3_ * dz;
+                            const double coef = (sp * ir - s * ir * ir) * ir;
+                            const double c0 = g0_ * sp * ir + coef * gd, c1 = s * ir;
+                            gk[0] = c0 * dx + c1 * g1_;
+                            gk[1] = c0 * dy + c1 * g2_;
+                            gk[2] = c0 * dz + c1 * g3_;
+#pragma unroll
+                            for (int bb = 0; bb < 3; ++bb) atomicAdd(&fsorted[3 * (long)j + bb], -gk[bb]);
+                            vir[0] -= dx * gk[0]; vir[1] -= dx * gk[1]; vir[2] -= dx * gk[2];
+                            vir[3] -= dy * gk[0]; vir[4] -= dy * gk[1]; vir[5] -= dy * gk[2];
+                            vir[6] -= dz * gk[0]; vir[7] -= dz * gk[1]; vir[8] -= dz * gk[2];
+                        }
+                        // centre atom: one atomic per warp when all its real rows belong to the same atom
+                        {
+                            const unsigned rm = __ballot_sync(0xffffffffu, real);
+                            if (rm) {
+                                const int a0 = __shfl_sync(0xffffffffu, atom, __ffs(rm) - 1);
+                                if (__all_sync(0xffffffffu, !real || atom == a0)) {
+#pragma unroll
+                                    for (int bb = 0; bb < 3; ++bb) {
+                                        double v = gk[bb];
+#pragma unroll
+                                        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                                        if (lane == 0) atomicAdd(&fsorted[3 * (long)a0 + bb], v);
+                                    }
+                                } else if (real) {
+#pragma unroll
+                                    for (int bb = 0; bb < 3; ++bb) atomicAdd(&fsorted[3 * (long)atom + bb], gk[bb]);
+                                }
+                            }
+                        }
+                    }
+                }   // passes
+                if (tw == 0) my_rows += (unsigned long long)nrows;
+            }
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < 9; ++k) {
+        double v = vir[k];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0 && v != 0.0) atomicAdd(&virial[k], v);
+    }
+    tc::fence_before();
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base_s), "n"(512));
+    if (tw == 0 && my_rows) atomicAdd(row_counter, my_rows);
+}
+
+}  // namespace
+
+cudaError_t launch_embed_bwd_tc2(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    static bool attr = false;
+    if (!attr) { cudaFuncSetAttribute(k_embed_bwd_tc2, cudaFuncAttributeMaxDynamicSharedMemorySize, BwdSmem::TOTAL); attr = true; }
+    int4 off4 = make_int4(m->off[0], m->off[1], m->off[2], m->off[3]);
+    EnvParams ep;
+    ep.rc = m->rc; ep.rc_smth = m->rc_smth; ep.inv_range = 1.0 / (m->rc - m->rc_smth);
+    ep.L[0] = g.L[0]; ep.L[1] = g.L[1]; ep.L[2] = g.L[2];
+    const int smem_ga = 4 * (4 * M2E + M2E * 16 + 4 * M2E) * 4;
+    k_gA_img<<<(unsigned)((N + 3) / 4), 128, smem_ga, st>>>(N, (const float *)(ws + L.A), (const float *)(ws + L.gD),
+                                                             (uint8_t *)(ws + L.gAf), (float *)(ws + L.gscale));
+    k_embed_bwd_tc2<<<m->num_sms, NWG * WGT, BwdSmem::TOTAL, st>>>(
+        N, m->T, g.ncell, m->Nm, off4, ep, (const EmbedNetTC2 *)m->embed_tc2_dev, m->std_dev, (int *)(ws + L.bin_start),
+        (int *)(ws + L.rowstart), (const float4 *)(ws + L.rows_rh), (const int2 *)(ws + L.rows_id), (double *)(ws + L.xs),
+        (const uint8_t *)(ws + L.gAf), (const float *)(ws + L.gscale), (double *)(ws + L.fsorted), (double *)(ws + L.virial),
+        (unsigned long long *)(ws + L.status + 16));
+    return cudaGetLastError();
+}

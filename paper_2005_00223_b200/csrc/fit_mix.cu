@@ -331,6 +331,7 @@ cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, 
     launch_gemm<4>(ns12, false, p, g240, st);
     p.A = gz1; p.N = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.out0 = D; p.ldo = ND;
     launch_gemm<5>(ns12, false, p, g1600, st);
+    if (m->use_tc_bwd) return cudaGetLastError();     // the tcgen05 backward builds its own operand images of gA
     const int smem = 4 * (4 * M2E + M2E * 16 + 4 * M2E) * 4;
     if (m->mix_nsc == 1) k_gA_f<1><<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, Amat, D, (uint32_t *)(ws + L.gAf), (float *)(ws + L.gscale));
     else k_gA_f<2><<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, Amat, D, (uint32_t *)(ws + L.gAf), (float *)(ws + L.gscale));
