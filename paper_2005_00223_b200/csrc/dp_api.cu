@@ -406,6 +406,16 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
         ok(upload(f32(c1), &m->fitc1_dev)); ok(upload(f32(c2), &m->fitc2_dev)); ok(upload(f32(c3), &m->fitc3_dev));
         ok(upload(f32(v4), &m->fitv4_dev)); ok(upload(f32(c4), &m->fitc4_dev));
     }
+    // tcgen05 fitting GEMMs: fp16 weight images; used when every fitting product carries its activations as hi + lo and
+    // its weights as single fp16 values (the MIX-16 default)
+    m->use_fit_tc = (prec == DP_MIX16 && m->mix_fit_ns == 2 && m->mix_fit3_ns == 2) ? 1 : 0;
+    if (const char *e = std::getenv("DP_FIT_TC")) if (!std::atoi(e)) m->use_fit_tc = 0;
+    if (m->use_fit_tc) {
+        std::vector<__half> img((size_t)T * fit_tc_type_elems());
+        for (int a = 0; a < T; ++a)
+            fit_tc_build_type(&V1[(size_t)a * ND * F], &V2[(size_t)a * F * F], &V3[(size_t)a * F * F], &img[(size_t)a * fit_tc_type_elems()]);
+        ok(upload(img, &m->fit_tc_img_dev));
+    }
     std::vector<double> avg(w->avg, w->avg + 4 * T), sd(w->std, w->std + 4 * T), eb(w->ebias, w->ebias + T);
     ok(upload(avg, (void **)&m->avg_dev)); ok(upload(sd, (void **)&m->std_dev)); ok(upload(eb, (void **)&m->ebias_dev));
     if (e != cudaSuccess) { dp_destroy(m); return DP_ECUDA; }
@@ -415,7 +425,7 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
 
 void dp_destroy(dp_model *m) {
     if (!m) return;
-    void *ptrs[] = {m->type_map_dev, m->embed_frag_dev, m->embed_tc_dev, m->embed_tc2_dev, m->avg_dev, m->std_dev, m->ebias_dev, m->fitV1_dev, m->fitV2_dev,
+    void *ptrs[] = {m->type_map_dev, m->embed_frag_dev, m->embed_tc_dev, m->embed_tc2_dev, m->fit_tc_img_dev, m->avg_dev, m->std_dev, m->ebias_dev, m->fitV1_dev, m->fitV2_dev,
                     m->fitV3_dev, m->fitc1_dev, m->fitc2_dev, m->fitc3_dev, m->fitv4_dev, m->fitc4_dev};
     for (void *p : ptrs) if (p) cudaFree(p);
     if (m->ev[0]) for (int k = 0; k <= DP_NPHASES; ++k) cudaEventDestroy(m->ev[k]);

@@ -50,6 +50,8 @@ struct dp_model {
     void *embed_tc2_dev;            // T*T EmbedNetTC2 (MIX-16, warpgroup-per-tile tcgen05 path)
     int use_tc;                     // mixed modes: embedding forward on tcgen05
     int use_tc_bwd;                 // MIX-16: embedding backward on tcgen05
+    int use_fit_tc;                 // mixed modes with activation-split fitting products: fitting GEMMs on tcgen05
+    void *fit_tc_img_dev;           // T x six fp16 weight images (fit_tc.cu)
     double *avg_dev, *std_dev;      // [T][4]
     double *ebias_dev;              // [T]
     // fitting nets (per type): V1 [1600][240], V2, V3 [240][240] row-major in x out, biases, v4, c4
@@ -120,6 +122,11 @@ cudaError_t launch_embed_bwd_mix(const dp_model *m, long N, const Grid3 &g, char
 cudaError_t launch_embed_fwd_tc(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_embed_fwd_tc2(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_embed_bwd_tc2(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+cudaError_t fit_tc_gemm(int mode, bool apx, const dp_model *m, const Grid3 &g, const int *bin_start, const float *A, int lda,
+                        const float *bias, const float *v4, const float *aux0, const float *aux1, float *out0, float *out1,
+                        int ldo, cudaStream_t st);
+size_t fit_tc_type_elems();
+void fit_tc_build_type(const double *V1, const double *V2, const double *V3, struct __half *out);
 cudaError_t launch_env_rows(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 int embed_smem_bytes_fwd_f64();

@@ -319,6 +319,15 @@ cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, 
     p.K = ND; p.N = F; p.A = D; p.lda = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.ldb = F; p.bias = c1;
     p.out0 = h1; p.ldo = F;
     const dim3 g240(F / BN, gy, T), g1600(ND / BN, gy, T);
+    if (m->use_fit_tc) {      // tcgen05 GEMMs (fit_tc.cu), same products, buffers and epilogues
+        fit_tc_gemm(0, apx, m, g, bin_start, D, ND, c1, nullptr, nullptr, nullptr, h1, nullptr, F, st);
+        fit_tc_gemm(1, apx, m, g, bin_start, h1, F, c2, nullptr, h1, nullptr, t2, h2, F, st);
+        fit_tc_gemm(2, false, m, g, bin_start, h2, F, c3, v4, h2, nullptr, gz3, h3, F, st);
+        k_energy_f<<<nb8, 256, 0, st>>>(N, T, g.ncell, bin_start, h3, v4, c4, m->ebias_dev, (double *)(ws + L.eatom));
+        fit_tc_gemm(3, false, m, g, bin_start, gz3, F, nullptr, v4, t2, nullptr, g2, gz2, F, st);
+        fit_tc_gemm(4, false, m, g, bin_start, gz2, F, nullptr, nullptr, g2, h1, gz1, nullptr, F, st);
+        fit_tc_gemm(5, false, m, g, bin_start, gz1, F, nullptr, nullptr, nullptr, nullptr, D, nullptr, ND, st);
+    } else {
     launch_gemm<0>(ns12, apx, p, g240, st);
     p.K = F; p.A = h1; p.lda = F; p.B = V2; p.b_type_stride = (long)F * F; p.bias = c2; p.aux0 = h1; p.out0 = t2; p.out1 = h2;
     launch_gemm<1>(ns12, apx, p, g240, st);
@@ -331,6 +340,7 @@ cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, 
     launch_gemm<4>(ns12, false, p, g240, st);
     p.A = gz1; p.N = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.out0 = D; p.ldo = ND;
     launch_gemm<5>(ns12, false, p, g1600, st);
+    }
     if (m->use_tc_bwd) return cudaGetLastError();     // the tcgen05 backward builds its own operand images of gA
     const int smem = 4 * (4 * M2E + M2E * 16 + 4 * M2E) * 4;
     if (m->mix_nsc == 1) k_gA_f<1><<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, Amat, D, (uint32_t *)(ws + L.gAf), (float *)(ws + L.gscale));

@@ -1,0 +1,325 @@
+// S6 (fitting net forward + backward GEMMs) on tcgen05 tensor cores, mixed-precision modes.
+//
+// One persistent, warp-specialised GEMM kernel C[rows x N] = A[rows x K] . B[K x N] per layer product, batched over the
+// atoms of each centre type (row ranges from the device-side type boundaries, no host sync):
+//   warp 0      : streams the weight images B (fp16, pre-tiled at dp_create) with cp.async.bulk + mbarrier transactions
+//   warp 1      : issues tcgen05.mma (one thread); accumulators in TMEM, double buffered (2 x BN columns)
+//   warps 2-9   : A producers: fp32 activations from global memory -> fp16 hi + lo operand images in shared memory
+//                 (activations are carried as hi + lo pairs: single-precision activations on fp16 tensor cores)
+//   warps 10-13 : epilogue: tcgen05.ld, bias / tanh / residual / tanh' per MODE, fp32 results to global memory
+// K = 1600 (first layer) streams A and B chunk by chunk; K = 240 keeps the A tile resident and streams B over the N tiles.
+#include <cuda_fp16.h>
+#include "dp_internal.h"
+#include "tc_common.cuh"
+
+namespace {
+
+constexpr int BM = 128;
+constexpr int KC = 80;                    // K chunk: 5 k-steps of 16
+constexpr int SUB = KC / 8;               // 16-byte sub-chunks per K chunk
+constexpr int A_SUB_STRIDE = BM * 16 + 16;   // bytes between sub-chunks of the A image (+16: conflict-free producer stores)
+constexpr int A_PART = SUB * A_SUB_STRIDE;   // one part (hi or lo) of one K chunk
+constexpr int NPROD = 256, NEPI = 128;
+constexpr int NTHREADS = 64 + NPROD + NEPI;
+
+template <int KTOT, int NTOT>
+struct Cfg {
+    static constexpr bool RESIDENT = KTOT == 240;            // the A tile stays in shared memory for all N tiles
+    static constexpr int BN = NTOT == 240 ? 240 : 160;
+    static constexpr int NTILES = NTOT / BN;
+    static constexpr int NKC = KTOT / KC;
+    static constexpr int NA = RESIDENT ? NKC : 2;            // A buffers
+    static constexpr int B_STAGE = KC * BN * 2;
+    static constexpr int A_BUF = 2 * A_PART;                 // hi + lo
+    static constexpr int OFF_A = 0;
+    static constexpr int OFF_B = ((NA * A_BUF + 1023) / 1024) * 1024;
+    static constexpr int OFF_BAR = OFF_B + 2 * B_STAGE;
+    static constexpr int TOTAL = OFF_BAR + 256;
+    static constexpr int TM_BUF = 256;                       // TMEM columns per accumulator buffer
+    static_assert(KTOT % KC == 0 && NTOT % BN == 0 && BN % 16 == 0, "tile shapes");
+    static_assert(TOTAL <= 227 * 1024, "shared memory budget");
+};
+
+struct FitTcArgs {
+    int T, ncell;
+    const int *bin_start;
+    const float *A; int lda;
+    const __half *Bimg; long b_type_stride;      // elements per type
+    const float *bias; const float *v4;          // [T][240]
+    const float *aux0; const float *aux1;
+    float *out0; float *out1; int ldo;
+};
+
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(tc::smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(tc::smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t sdst, const void *gsrc, uint32_t bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(sdst), "l"(gsrc), "r"(bytes), "r"(tc::smem_u32(bar)) : "memory");
+}
+
+// row tile -> (type, first row, end of the type's rows)
+__device__ __forceinline__ bool tile_rows(const FitTcArgs &p, int tile, int &a, int &row0, int &rend) {
+    for (a = 0; a < p.T; ++a) {
+        const int ts0 = p.bin_start[a * p.ncell], ts1 = p.bin_start[(a + 1) * p.ncell];
+        const int nt = (ts1 - ts0 + BM - 1) / BM;
+        if (tile < nt) { row0 = ts0 + tile * BM; rend = ts1; return true; }
+        tile -= nt;
+    }
+    return false;
+}
+
+// MODE (epilogue), as in the mma.sync kernels of fit_mix.cu:
+//   0: out0 = tanh(acc + bias)                                   (h1)
+//   1: t = tanh(acc + bias); out0 = t; out1 = aux0 + t           (t2, h2 = h1 + t2)
+//   2: t = tanhf(acc + bias); out0 = v4 (1 - t^2); out1 = aux0 + t   (gz3, h3 = h2 + t3)
+//   3: g = v4 + acc; out0 = g; out1 = g (1 - aux0^2)             (gh2, gz2;  aux0 = t2)
+//   4: g = aux0 + acc; out0 = g (1 - aux1^2)                     (gz1;  aux0 = gh2, aux1 = h1)
+//   5: out0 = acc                                                (gD)
+template <int MODE, int KTOT, int NTOT, bool APPROX>
+__global__ void __launch_bounds__(NTHREADS, 1) k_fit_tc(FitTcArgs p) {
+    using C = Cfg<KTOT, NTOT>;
+    extern __shared__ __align__(1024) uint8_t smem[];
+    __shared__ uint32_t tmem_base_s;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + C::OFF_BAR);
+    uint64_t *b_full = bars, *b_empty = bars + 2, *a_full = bars + 4, *a_empty = bars + 4 + C::NA;
+    uint64_t *acc_full = bars + 4 + 2 * C::NA, *acc_empty = acc_full + 2;
+    if (tid == 0) {
+        for (int k = 0; k < 2; ++k) { tc::mbar_init(&b_full[k], 1); tc::mbar_init(&b_empty[k], 1); }
+        for (int k = 0; k < C::NA; ++k) { tc::mbar_init(&a_full[k], NPROD / 32); tc::mbar_init(&a_empty[k], 1); }
+        for (int k = 0; k < 2; ++k) { tc::mbar_init(&acc_full[k], 1); tc::mbar_init(&acc_empty[k], NEPI / 32); }
+        asm volatile("fence.mbarrier_init.release.cluster;");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tc::smem_u32(&tmem_base_s)), "n"(512));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    tc::fence_before();
+    __syncthreads();
+    tc::fence_after();
+    const uint32_t tmem = tmem_base_s;
+    const uint32_t sbase = tc::smem_u32(smem);
+    int ntiles_total = 0;
+    for (int a = 0; a < p.T; ++a) ntiles_total += (p.bin_start[(a + 1) * p.ncell] - p.bin_start[a * p.ncell] + BM - 1) / BM;
+
+    if (warp == 0) {
+        // ---------------------------------------------------------------- B loader
+        if (lane == 0) {
+            uint32_t step = 0;
+            for (int tile = blockIdx.x; tile < ntiles_total; tile += gridDim.x) {
+                int a, row0, rend;
+                tile_rows(p, tile, a, row0, rend);
+                const __half *Bw = p.Bimg + a * p.b_type_stride;
+                for (int nt = 0; nt < C::NTILES; ++nt)
+                    for (int kc = 0; kc < C::NKC; ++kc, ++step) {
+                        const int st = step & 1;
+                        tc::mbar_wait(&b_empty[st], ((step >> 1) & 1) ^ 1);
+                        mbar_expect_tx(&b_full[st], C::B_STAGE);
+                        bulk_g2s(sbase + C::OFF_B + st * C::B_STAGE, Bw + ((long)nt * C::NKC + kc) * (KC * C::BN), C::B_STAGE, &b_full[st]);
+                    }
+            }
+        }
+    } else if (warp == 1) {
+        // ---------------------------------------------------------------- MMA issuer
+        if (lane == 0) {
+            constexpr uint32_t idesc = tc::idesc(128, C::BN, false, false);
+            uint32_t step = 0, astep = 0, accn = 0, it = 0;
+            for (int tile = blockIdx.x; tile < ntiles_total; tile += gridDim.x, ++it) {
+                for (int nt = 0; nt < C::NTILES; ++nt, ++accn) {
+                    const int buf = accn & 1;
+                    tc::mbar_wait(&acc_empty[buf], ((accn >> 1) & 1) ^ 1);
+                    tc::fence_after();
+                    for (int kc = 0; kc < C::NKC; ++kc, ++step) {
+                        const int st = step & 1;
+                        int ab;
+                        if (C::RESIDENT) { ab = kc; tc::mbar_wait(&a_full[ab], it & 1); }
+                        else { ab = astep & 1; tc::mbar_wait(&a_full[ab], (astep >> 1) & 1); }
+                        tc::mbar_wait(&b_full[st], (step >> 1) & 1);
+                        tc::fence_after();
+                        const uint32_t a_hi = sbase + C::OFF_A + ab * C::A_BUF, b_img = sbase + C::OFF_B + st * C::B_STAGE;
+#pragma unroll
+                        for (int part = 0; part < 2; ++part)
+#pragma unroll
+                            for (int ks = 0; ks < KC / 16; ++ks)
+                                tc::mma_ss(tmem + buf * C::TM_BUF, tc::desc(a_hi + part * A_PART + ks * 2 * A_SUB_STRIDE, A_SUB_STRIDE, 128),
+                                           tc::desc(b_img + ks * 2 * (C::BN * 16), C::BN * 16, 128), idesc, (kc | part | ks) != 0);
+                        tc::commit(&b_empty[st]);
+                        if (!C::RESIDENT) { tc::commit(&a_empty[ab]); ++astep; }
+                        else if (nt == C::NTILES - 1) tc::commit(&a_empty[ab]);
+                    }
+                    tc::commit(&acc_full[buf]);
+                }
+            }
+        }
+    } else if (warp < 2 + NPROD / 32) {
+        // ---------------------------------------------------------------- A producers
+        const int pt = tid - 64;
+        uint32_t astep = 0, it = 0;
+        for (int tile = blockIdx.x; tile < ntiles_total; tile += gridDim.x, ++it) {
+            int a, row0, rend;
+            tile_rows(p, tile, a, row0, rend);
+            for (int kc = 0; kc < C::NKC; ++kc, ++astep) {
+                int ab;
+                if (C::RESIDENT) { ab = kc; tc::mbar_wait(&a_empty[ab], (it & 1) ^ 1); }
+                else { ab = astep & 1; tc::mbar_wait(&a_empty[ab], ((astep >> 1) & 1) ^ 1); }
+                uint8_t *img = smem + C::OFF_A + ab * C::A_BUF;
+                // item = (row, sub-chunk): 8 consecutive fp32 -> one 16-byte hi chunk and one lo chunk
+#pragma unroll
+                for (int j = 0; j < BM * SUB / NPROD; ++j) {
+                    const int idx = pt + j * NPROD;
+                    const int r = idx / SUB, sub = idx % SUB;
+                    float4 x0 = make_float4(0.f, 0.f, 0.f, 0.f), x1 = x0;
+                    if (row0 + r < rend) {
+                        const float4 *src = reinterpret_cast<const float4 *>(p.A + (long)(row0 + r) * p.lda + kc * KC + sub * 8);
+                        x0 = __ldg(src); x1 = __ldg(src + 1);
+                    }
+                    uint4 hi, lo;
+                    tc::split_h2(x0.x, x0.y, hi.x, lo.x); tc::split_h2(x0.z, x0.w, hi.y, lo.y);
+                    tc::split_h2(x1.x, x1.y, hi.z, lo.z); tc::split_h2(x1.z, x1.w, hi.w, lo.w);
+                    *reinterpret_cast<uint4 *>(img + sub * A_SUB_STRIDE + r * 16) = hi;
+                    *reinterpret_cast<uint4 *>(img + A_PART + sub * A_SUB_STRIDE + r * 16) = lo;
+                }
+                tc::proxy_fence();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&a_full[ab]);
+            }
+        }
+    } else {
+        // ---------------------------------------------------------------- epilogue (thread = row)
+        const int q = warp & 3, r = q * 32 + lane;
+        const uint32_t tm_lane = tmem + ((uint32_t)(q * 32) << 16);
+        uint32_t accn = 0;
+        for (int tile = blockIdx.x; tile < ntiles_total; tile += gridDim.x) {
+            int a, row0, rend;
+            tile_rows(p, tile, a, row0, rend);
+            const bool ok = row0 + r < rend;
+            const float *bias = p.bias ? p.bias + a * 240 : nullptr;
+            const float *v4 = p.v4 ? p.v4 + a * 240 : nullptr;
+            for (int nt = 0; nt < C::NTILES; ++nt, ++accn) {
+                const int buf = accn & 1;
+                tc::mbar_wait(&acc_full[buf], (accn >> 1) & 1);
+                tc::fence_after();
+                const long o = (long)(row0 + r) * p.ldo + nt * C::BN;
+#pragma unroll 1
+                for (int c0 = 0; c0 < C::BN; c0 += 16) {
+                    uint32_t v[16];
+                    tc::ld16(tm_lane + buf * C::TM_BUF + c0, v);
+                    tc::wait_ld();
+                    if (ok) {
+#pragma unroll
+                        for (int g4 = 0; g4 < 4; ++g4) {
+                            const int c = c0 + 4 * g4;
+                            float x[4] = {__uint_as_float(v[4 * g4]), __uint_as_float(v[4 * g4 + 1]), __uint_as_float(v[4 * g4 + 2]),
+                                          __uint_as_float(v[4 * g4 + 3])};
+                            float r0[4], r1[4];
+                            if (MODE == 0) {
+                                const float4 b = *reinterpret_cast<const float4 *>(bias + c);
+                                const float bb[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+                                for (int k = 0; k < 4; ++k) r0[k] = APPROX ? tc::tanh_approx(x[k] + bb[k]) : tanhf(x[k] + bb[k]);
+                            } else if (MODE == 1 || MODE == 2) {
+                                const float4 b = *reinterpret_cast<const float4 *>(bias + c);
+                                const float4 hh = *reinterpret_cast<const float4 *>(p.aux0 + o + c);
+                                const float bb[4] = {b.x, b.y, b.z, b.w}, hv[4] = {hh.x, hh.y, hh.z, hh.w};
+                                float vv[4] = {0.f, 0.f, 0.f, 0.f};
+                                if (MODE == 2) { const float4 w = *reinterpret_cast<const float4 *>(v4 + c); vv[0] = w.x; vv[1] = w.y; vv[2] = w.z; vv[3] = w.w; }
+#pragma unroll
+                                for (int k = 0; k < 4; ++k) {
+                                    const float t = (MODE == 1 && APPROX) ? tc::tanh_approx(x[k] + bb[k]) : tanhf(x[k] + bb[k]);
+                                    r0[k] = MODE == 1 ? t : vv[k] * (1.f - t * t);
+                                    r1[k] = hv[k] + t;
+                                }
+                            } else if (MODE == 3) {
+                                const float4 w = *reinterpret_cast<const float4 *>(v4 + c);
+                                const float4 tt = *reinterpret_cast<const float4 *>(p.aux0 + o + c);
+                                const float vv[4] = {w.x, w.y, w.z, w.w}, tv[4] = {tt.x, tt.y, tt.z, tt.w};
+#pragma unroll
+                                for (int k = 0; k < 4; ++k) { r0[k] = vv[k] + x[k]; r1[k] = r0[k] * (1.f - tv[k] * tv[k]); }
+                            } else if (MODE == 4) {
+                                const float4 gg = *reinterpret_cast<const float4 *>(p.aux0 + o + c);
+                                const float4 hh = *reinterpret_cast<const float4 *>(p.aux1 + o + c);
+                                const float gv[4] = {gg.x, gg.y, gg.z, gg.w}, hv[4] = {hh.x, hh.y, hh.z, hh.w};
+#pragma unroll
+                                for (int k = 0; k < 4; ++k) r0[k] = (gv[k] + x[k]) * (1.f - hv[k] * hv[k]);
+                            } else {
+#pragma unroll
+                                for (int k = 0; k < 4; ++k) r0[k] = x[k];
+                            }
+                            *reinterpret_cast<float4 *>(p.out0 + o + c) = make_float4(r0[0], r0[1], r0[2], r0[3]);
+                            if (MODE >= 1 && MODE <= 3) *reinterpret_cast<float4 *>(p.out1 + o + c) = make_float4(r1[0], r1[1], r1[2], r1[3]);
+                        }
+                    }
+                }
+                tc::fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&acc_empty[buf]);
+            }
+        }
+    }
+    tc::fence_before();
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(512));
+}
+
+template <int MODE, int KTOT, int NTOT, bool APPROX>
+void launch(const FitTcArgs &p, int grid, cudaStream_t st) {
+    using C = Cfg<KTOT, NTOT>;
+    static bool attr = false;
+    if (!attr) { cudaFuncSetAttribute(k_fit_tc<MODE, KTOT, NTOT, APPROX>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::TOTAL); attr = true; }
+    k_fit_tc<MODE, KTOT, NTOT, APPROX><<<grid, NTHREADS, C::TOTAL, st>>>(p);
+}
+
+}  // namespace
+
+// Host side: weight images.  For product g the image of type a is [NTILES][NKC][KC/8][BN][8] fp16 with
+// element (nt, kc, sub, n, kk) = B[k = kc*KC + sub*8 + kk][nt*BN + n].
+size_t fit_tc_image_elems(int K, int Nn) { return (size_t)K * Nn; }
+void fit_tc_build_image(const double *W, int ldw, bool transpose, int K, int Nn, __half *out) {
+    const int BN = Nn == 240 ? 240 : 160;
+    const int ntl = Nn / BN, nkc = K / KC;
+    for (int nt = 0; nt < ntl; ++nt)
+        for (int kc = 0; kc < nkc; ++kc)
+            for (int sub = 0; sub < SUB; ++sub)
+                for (int n = 0; n < BN; ++n)
+                    for (int kk = 0; kk < 8; ++kk) {
+                        const int k = kc * KC + sub * 8 + kk, nn = nt * BN + n;
+                        const double v = transpose ? W[(size_t)nn * ldw + k] : W[(size_t)k * ldw + nn];
+                        out[((((size_t)nt * nkc + kc) * SUB + sub) * BN + n) * 8 + kk] = __float2half_rn((float)v);
+                    }
+}
+
+// offsets (elements) of the six product images inside one type's block: g0 V1, g1 V2, g2 V3, g3 V3^T, g4 V2^T, g5 V1^T
+static const size_t FIT_TC_OFF[7] = {0, 1600 * 240, 1600 * 240 + 240 * 240, 1600 * 240 + 2 * 240 * 240, 1600 * 240 + 3 * 240 * 240,
+                                     1600 * 240 + 4 * 240 * 240, 2 * 1600 * 240 + 4 * 240 * 240};
+size_t fit_tc_type_elems() { return FIT_TC_OFF[6]; }
+void fit_tc_build_type(const double *V1, const double *V2, const double *V3, __half *out) {
+    fit_tc_build_image(V1, 240, false, 1600, 240, out + FIT_TC_OFF[0]);
+    fit_tc_build_image(V2, 240, false, 240, 240, out + FIT_TC_OFF[1]);
+    fit_tc_build_image(V3, 240, false, 240, 240, out + FIT_TC_OFF[2]);
+    fit_tc_build_image(V3, 240, true, 240, 240, out + FIT_TC_OFF[3]);
+    fit_tc_build_image(V2, 240, true, 240, 240, out + FIT_TC_OFF[4]);
+    fit_tc_build_image(V1, 240, true, 240, 1600, out + FIT_TC_OFF[5]);
+}
+
+cudaError_t fit_tc_gemm(int mode, bool apx, const dp_model *m, const Grid3 &g, const int *bin_start, const float *A, int lda,
+                        const float *bias, const float *v4, const float *aux0, const float *aux1, float *out0, float *out1,
+                        int ldo, cudaStream_t st) {
+    FitTcArgs p{};
+    p.T = m->T; p.ncell = g.ncell; p.bin_start = bin_start; p.A = A; p.lda = lda;
+    p.Bimg = (const __half *)m->fit_tc_img_dev + FIT_TC_OFF[mode]; p.b_type_stride = (long)FIT_TC_OFF[6];
+    p.bias = bias; p.v4 = v4; p.aux0 = aux0; p.aux1 = aux1; p.out0 = out0; p.out1 = out1; p.ldo = ldo;
+    const int grid = m->num_sms;
+    switch (mode) {
+        case 0: if (apx) launch<0, 1600, 240, true>(p, grid, st); else launch<0, 1600, 240, false>(p, grid, st); break;
+        case 1: if (apx) launch<1, 240, 240, true>(p, grid, st); else launch<1, 240, 240, false>(p, grid, st); break;
+        case 2: launch<2, 240, 240, false>(p, grid, st); break;
+        case 3: launch<3, 240, 240, false>(p, grid, st); break;
+        case 4: launch<4, 240, 240, false>(p, grid, st); break;
+        default: launch<5, 240, 1600, false>(p, grid, st); break;
+    }
+    return cudaGetLastError();
+}
