@@ -39,6 +39,7 @@ WsLayout ws_layout(const dp_model *m, long N) {
         L.rowstart = take(sizeof(int) * ((size_t)N + 1) * m->T);
         L.rows_rh = take(sizeof(float) * 4 * (size_t)N * m->Nm);     // block b starts at row offset N*off[b]
         L.rows_id = take(sizeof(int) * 2 * (size_t)N * m->Nm);
+        if (m->prec == DP_MIX16) L.rows_g = take(sizeof(float) * 4 * (size_t)N * m->Nm);
     }
     const size_t esz = m->prec == DP_FP64 ? sizeof(double) : sizeof(float);
     L.A = take(esz * (size_t)N * 4 * M2E);

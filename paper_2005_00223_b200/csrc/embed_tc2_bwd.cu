@@ -10,11 +10,18 @@
 //   dy1 = dT1 + dz3 (W3^T folded) + dz2 W2^T;   dz1 = dy1 (1 - t1^2);   ds^ = dz1 . w1
 // followed, per row, by the fp64 geometry derivative, the force scatter and the virial (S8, S9).
 // Per-atom operand images g~ (hi, lo) come from k_gA_img (the tail of the fitting backward), scaled by a power of two.
+#include <cstdio>
 #include <cstdlib>
 #include "embed_tc2.cuh"
 #include "tc_common.cuh"
 
 namespace {
+
+#ifdef DP_BWD_TIMING
+#define DP_TICK(i) do { if (dbg_t) { long long now_ = clock64(); tacc[i] += now_ - tlast; tlast = now_; } } while (0)
+#else
+#define DP_TICK(i) do { } while (0)
+#endif
 
 constexpr int NWG = 2;
 // TMEM columns per warpgroup
@@ -38,7 +45,7 @@ struct BwdSmem {
                                                                    // K-major B of the direct products (K = 16 per slot) and,
                                                                    // viewed MN-major (chunks 0 and 2), B of the dR^ product (N = 16)
     static constexpr int META = QIMG + 4 * T2_COLS * 16;
-    static constexpr int WG_BYTES = ((META + 512 + 127) / 128) * 128;
+    static constexpr int WG_BYTES = ((META + 2 * 3072 + 127) / 128) * 128;   // META: two stages of prefetched row data
     static constexpr int TOTAL = WG0 + NWG * WG_BYTES;
 };
 static_assert(BwdSmem::TOTAL <= 227 * 1024, "shared memory budget");
@@ -54,6 +61,9 @@ struct EnvParams {
 
 __device__ __forceinline__ void cp_async16(uint32_t sdst, const void *gsrc) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sdst), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async8(uint32_t sdst, const void *gsrc) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sdst), "l"(gsrc) : "memory");
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
@@ -227,11 +237,11 @@ __device__ __forceinline__ void gradh16(const uint32_t (&g)[16], const uint32_t 
 constexpr int WGT = 128;       // threads per warpgroup: thread = row; every stage walks its two column halves h = 0, 1
 
 __global__ void __launch_bounds__(NWG * WGT, 1)
-k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, EnvParams ep, const EmbedNetTC2 *__restrict__ nets,
+k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *__restrict__ nets,
                 const double *__restrict__ stdv, const int *__restrict__ bin_start, const int *__restrict__ rowstart,
-                const float4 *__restrict__ rows_rh, const int2 *__restrict__ rows_id, const double *__restrict__ xs,
-                const uint8_t *__restrict__ gimg, const float *__restrict__ gscale, double *__restrict__ fsorted,
-                double *__restrict__ virial, unsigned long long *__restrict__ row_counter) {
+                const float4 *__restrict__ rows_rh, const int2 *__restrict__ rows_id, const uint8_t *__restrict__ gimg,
+                const float *__restrict__ gscale, float4 *__restrict__ rows_g, unsigned long long *__restrict__ row_counter,
+                long long *__restrict__ tdbg) {
     using SL = BwdSmem;
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ uint32_t tmem_base_s;
@@ -242,7 +252,6 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, EnvParams ep, const
     uint8_t *wgs = smem + SL::WG0 + wg * SL::WG_BYTES;
     uint8_t *lo_row = wgs + SL::TLO + t * 16;
     const int off[4] = {off4.x, off4.y, off4.z, off4.w};
-    const double hx = 0.5 * ep.L[0], hy = 0.5 * ep.L[1], hz = 0.5 * ep.L[2];
 
     if (tid == 0) {
         for (int k = 0; k < NWG; ++k) tc::mbar_init(&bars[k], 1);
@@ -261,12 +270,19 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, EnvParams ep, const
     const uint32_t sbase = tc::smem_u32(smem);
     const uint32_t s_tlo = tc::smem_u32(wgs + SL::TLO), s_rimg = tc::smem_u32(wgs + SL::RIMG);
     const uint32_t s_qimg = tc::smem_u32(wgs + SL::QIMG);
+    // operand descriptors are built once; every MMA adds a compile-time offset
+    const uint64_t d_tlo = tc::desc(s_tlo, 2048, 128), d_rimg = tc::desc(s_rimg, 2048, 128);
+    const uint64_t d_qk = tc::desc(s_qimg, T2_COLS * 16, 128), d_qmn = tc::desc(s_qimg, 128, 2 * T2_COLS * 16);
+    const uint64_t d_w2 = tc::desc(sbase + SL::W2, 64 * 16, 128), d_w3 = tc::desc(sbase + SL::W3, 112 * 16, 128);
+    const uint64_t d_w3t = tc::desc(sbase + SL::W3T, 96 * 16, 128), d_w2t = tc::desc(sbase + SL::W2T, 32 * 16, 128);
     uint64_t *bar = &bars[wg];
     uint32_t ph = 0;
     unsigned long long my_rows = 0;
-    double vir[9];
-#pragma unroll
-    for (int k = 0; k < 9; ++k) vir[k] = 0.0;
+#ifdef DP_BWD_TIMING
+    const bool dbg_t = tdbg && blockIdx.x == 0 && tid == 0;
+    long long tacc[20], tlast = clock64();
+    for (int k = 0; k < 20; ++k) tacc[k] = 0;
+#endif
     // zero the T hi region once: its padding columns are read as K of the products and must stay finite (zero)
     {
         uint32_t z8[8] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
@@ -306,30 +322,34 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, EnvParams ep, const
             __syncthreads();
             const int G = gridDim.x * NWG, gw = blockIdx.x * NWG + wg;
             const int tile0 = (int)((long)ntiles * gw / G), tile1 = (int)((long)ntiles * (gw + 1) / G);
-            float4 nrh = make_float4(0.f, 0.f, 0.f, 0.f);
-            int2 nid = make_int2(-1, -1);
-            int na0 = 0, naL = -1;                      // first and last atom of the next tile (uniform loads)
+            // Row data (R^, {atom, j}) is prefetched one tile ahead with cp.async into a two-stage buffer: stage = tile parity.
+            auto prefetch_rows = [&](int first_row, int stage) {
+                uint8_t *pf = wgs + SL::META + stage * 3072;
+                if (first_row + t < re) {
+                    cp_async16(tc::smem_u32(pf + t * 16), &rows_rh[rbase + first_row + t]);
+                    cp_async8(tc::smem_u32(pf + 2048 + t * 8), &rows_id[rbase + first_row + t]);
+                } else {
+                    *reinterpret_cast<float4 *>(pf + t * 16) = make_float4(0.f, 0.f, 0.f, 0.f);
+                    *reinterpret_cast<int2 *>(pf + 2048 + t * 8) = make_int2(-1, -1);
+                }
+            };
             if (tile0 < tile1) {
-                const int r0 = rs + tile0 * T2_ROWS;
-                if (r0 + t < re) { nrh = ldv_f4(&rows_rh[rbase + r0 + t]); nid = ldv_i2(&rows_id[rbase + r0 + t]); }
-                na0 = ldv_i2(&rows_id[rbase + r0]).x;
-                naL = ldv_i2(&rows_id[rbase + min(r0 + T2_ROWS, re) - 1]).x;
+                prefetch_rows(rs + tile0 * T2_ROWS, tile0 & 1);
+                cp_async_wait_all();
             }
+            tc::bar_sync(1 + wg, WGT);
             for (int tile = tile0; tile < tile1; ++tile) {
                 const int r0 = rs + tile * T2_ROWS;
                 const int nrows = min(T2_ROWS, re - r0);
-                const float4 rh = nrh;
-                const int2 id = nid;
-                const int atom0 = na0, atomL = naL;
-                nrh = make_float4(0.f, 0.f, 0.f, 0.f);
-                nid = make_int2(-1, -1);
-                if (tile + 1 < tile1) {
-                    const int r1 = r0 + T2_ROWS;
-                    if (r1 + t < re) { nrh = ldv_f4(&rows_rh[rbase + r1 + t]); nid = ldv_i2(&rows_id[rbase + r1 + t]); }
-                    na0 = ldv_i2(&rows_id[rbase + r1]).x;
-                    naL = ldv_i2(&rows_id[rbase + min(r1 + T2_ROWS, re) - 1]).x;
-                }
+                const uint8_t *pf = wgs + SL::META + (tile & 1) * 3072;
+                const float4 rh = *reinterpret_cast<const float4 *>(pf + t * 16);
+                const int2 id = *reinterpret_cast<const int2 *>(pf + 2048 + t * 8);
+                const int atom0 = reinterpret_cast<const int2 *>(pf + 2048)[0].x;
+                const int atomL = reinterpret_cast<const int2 *>(pf + 2048)[nrows - 1].x;
+                // next tile: lands before this tile's backward stage (cp.async.wait_all + warpgroup barrier there)
+                if (tile + 1 < tile1) prefetch_rows(r0 + T2_ROWS, (tile + 1) & 1);
                 const int atom = id.x;
+                DP_TICK(17);
                 // T2_NSLOT atoms per pass; a tile that spans more atoms (short neighbour blocks) is recomputed per pass
                 for (int p0 = atom0; p0 <= atomL; p0 += T2_NSLOT) {
                     const bool in = atom >= p0 && atom - p0 < T2_NSLOT;
@@ -347,6 +367,7 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, EnvParams ep, const
                             *reinterpret_cast<uint4 *>(wgs + SL::RIMG + (2 * s_ + 1) * 2048 + t * 16) = mine ? c1 : z4;
                         }
                     }
+                    DP_TICK(18);
                     for (int q = p0; q < p0 + T2_NSLOT && q <= atomL; ++q) {
                         const int s_ = q & (T2_NSLOT - 1);
                         const uint4 *C = reinterpret_cast<const uint4 *>(gimg + (long)q * GA_IMG_BYTES);
@@ -356,6 +377,7 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, EnvParams ep, const
                         }
                     }
                     uint32_t d1p[2][8], d2p[2][16], d3p[2][26];       // 1 - t^2 per column half (fp16 pairs)
+                    DP_TICK(0);
                     // ---- E1: layer 1 on the ALUs; h = 0: t1[0..16), h = 1: t1[16..25), ones, padding ----
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
@@ -370,19 +392,22 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, EnvParams ep, const
                         emit16(y, tm_lane + TM_T + 8 * h, lo_row, 2 * h, d1p[h]);
                     }
                     tc::wait_st();
+                    DP_TICK(1);
                     sync_issue();
                     if (tw == 0) {
                         tc::fence_after();
                         constexpr uint32_t id2 = tc::idesc(128, 64, false, false);
 #pragma unroll
                         for (int ks = 0; ks < 2; ++ks) {
-                            const uint64_t db = tc::desc(sbase + SL::W2 + ks * 2 * (64 * 16), 64 * 16, 128);
+                            const uint64_t db = tc::desc_at(d_w2, ks * 2 * (64 * 16));
                             tc::mma_ts(tmem + TM_Z, tmem + TM_T + 8 * ks, db, id2, ks > 0);
-                            tc::mma_ss(tmem + TM_Z, tc::desc(s_tlo + ks * 2 * 2048, 2048, 128), db, id2, true);
+                            tc::mma_ss(tmem + TM_Z, tc::desc_at(d_tlo, ks * 2 * 2048), db, id2, true);
                         }
                         tc::commit(bar);
                     }
+                    DP_TICK(2);
                     wait_mma();
+                    DP_TICK(3);
                     // ---- E2: h = 0: t2[0..32), h = 1: t2[32..50) ----
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
@@ -405,6 +430,7 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, EnvParams ep, const
                         }
                     }
                     tc::wait_st();
+                    DP_TICK(4);
                     sync_issue();
                     if (tw == 0) {
                         tc::fence_after();
@@ -413,13 +439,15 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, EnvParams ep, const
                         for (int ks = 0; ks < 6; ++ks) {
                             const int acol = ks < 4 ? 16 + 8 * ks : 8 * (ks - 4);              // TMEM column of the hi part
                             const int achunk = ks < 4 ? T2_O2 / 8 + 2 * ks : 2 * (ks - 4);     // chunk of the lo part
-                            const uint64_t db = tc::desc(sbase + SL::W3 + ks * 2 * (112 * 16), 112 * 16, 128);
+                            const uint64_t db = tc::desc_at(d_w3, ks * 2 * (112 * 16));
                             tc::mma_ts(tmem + TM_Z, tmem + TM_T + acol, db, id3, ks > 0);
-                            tc::mma_ss(tmem + TM_Z, tc::desc(s_tlo + achunk * 2048, 2048, 128), db, id3, true);
+                            tc::mma_ss(tmem + TM_Z, tc::desc_at(d_tlo, achunk * 2048), db, id3, true);
                         }
                         tc::commit(bar);
                     }
+                    DP_TICK(5);
                     wait_mma();
+                    DP_TICK(6);
                     // ---- E3: h = 0: t3[0..48), h = 1: t3[48..100) ----
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
@@ -448,34 +476,28 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, EnvParams ep, const
                     tc::wait_st();
                     // ---- backward ----
                     cp_async_wait_all();
+                    DP_TICK(7);
                     sync_issue();
                     if (tw == 0) {
                         tc::fence_after();
                         constexpr uint32_t idr = tc::idesc(128, 8 * T2_NSLOT, false, true);
 #pragma unroll
                         for (int ks = 0; ks < T2_COLS / 16; ++ks) {
-                            const uint64_t db = tc::desc(s_qimg + ks * 256, 128, 2 * T2_COLS * 16);
+                            const uint64_t db = tc::desc_at(d_qmn, ks * 256);
                             tc::mma_ts(tmem + TM_DR, tmem + TM_T + 8 * ks, db, idr, ks > 0);
-                            tc::mma_ss(tmem + TM_DR, tc::desc(s_tlo + ks * 2 * 2048, 2048, 128), db, idr, true);
+                            tc::mma_ss(tmem + TM_DR, tc::desc_at(d_tlo, ks * 2 * 2048), db, idr, true);
                         }
                         constexpr uint32_t idg = tc::idesc(128, T2_K3, false, false);
 #pragma unroll
                         for (int ks = 0; ks < T2_NSLOT; ++ks)
-                            tc::mma_ss(tmem + TM_Z, tc::desc(s_rimg + ks * 2 * 2048, 2048, 128),
-                                       tc::desc(s_qimg + T2_O3 * 16 + ks * 2 * (T2_COLS * 16), T2_COLS * 16, 128), idg, ks > 0);
+                            tc::mma_ss(tmem + TM_Z, tc::desc_at(d_rimg, ks * 2 * 2048), tc::desc_at(d_qk, T2_O3 * 16 + ks * 2 * (T2_COLS * 16)), idg, ks > 0);
                         tc::commit(bar);
                     }
-                    // prefetch the geometry of this row while the products run
-                    const bool real = in && id.y >= 0;
-                    double xj = 0.0, yj = 0.0, zj = 0.0, xc = 0.0, yc = 0.0, zc = 0.0;
                     float gsc = 1.f;
-                    if (real) {
-                        const int j = id.y;
-                        xj = xs[3 * (long)j]; yj = xs[3 * (long)j + 1]; zj = xs[3 * (long)j + 2];
-                        xc = xs[3 * (long)atom]; yc = xs[3 * (long)atom + 1]; zc = xs[3 * (long)atom + 2];
-                        gsc = __ldg(&gscale[atom]);
-                    }
+                    if (in) gsc = __ldg(&gscale[atom]);
+                    DP_TICK(8);
                     wait_mma();
+                    DP_TICK(9);
                     // ---- E4: dR^ of this row; dz3 = dT3 (1 - t3^2) -> t3 block of the lo image ----
                     float dR[4];
                     {
@@ -504,6 +526,7 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, EnvParams ep, const
                         for (int c = 0; c < 4; ++c)
                             dR[c] = slot ? __uint_as_float(v[8 + c]) + __uint_as_float(v[12 + c]) : __uint_as_float(v[c]) + __uint_as_float(v[4 + c]);
                     }
+                    DP_TICK(10);
                     sync_issue();
                     if (tw == 0) {
                         tc::fence_after();
@@ -511,25 +534,23 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, EnvParams ep, const
                         constexpr uint32_t idy2 = tc::idesc(128, 64, false, false);
 #pragma unroll
                         for (int ks = 0; ks < T2_NSLOT; ++ks)      // direct part dT2 -> accumulator columns [32,96)
-                            tc::mma_ss(tmem + TM_Z + 32, tc::desc(s_rimg + ks * 2 * 2048, 2048, 128),
-                                       tc::desc(s_qimg + T2_O2 * 16 + ks * 2 * (T2_COLS * 16), T2_COLS * 16, 128), idy2, ks > 0);
+                            tc::mma_ss(tmem + TM_Z + 32, tc::desc_at(d_rimg, ks * 2 * 2048), tc::desc_at(d_qk, T2_O2 * 16 + ks * 2 * (T2_COLS * 16)), idy2, ks > 0);
 #pragma unroll
                         for (int ks = 0; ks < T2_K3 / 16; ++ks)
-                            tc::mma_ss(tmem + TM_Z + 32, tc::desc(s_tlo + (T2_O3 / 8 + 2 * ks) * 2048, 2048, 128),
-                                       tc::desc(sbase + SL::W3T + 32 * 16 + ks * 2 * (96 * 16), 96 * 16, 128), idy2, true);
+                            tc::mma_ss(tmem + TM_Z + 32, tc::desc_at(d_tlo, (T2_O3 / 8 + 2 * ks) * 2048), tc::desc_at(d_w3t, 32 * 16 + ks * 2 * (96 * 16)), idy2, true);
                         tc::commit(bar);
                         // ... then the part of dy1 that does not depend on dz2 (waited for with the last stage)
                         constexpr uint32_t idy1 = tc::idesc(128, 32, false, false);
 #pragma unroll
                         for (int ks = 0; ks < T2_NSLOT; ++ks)      // direct part dT1 -> accumulator columns [0,32)
-                            tc::mma_ss(tmem + TM_Z, tc::desc(s_rimg + ks * 2 * 2048, 2048, 128),
-                                       tc::desc(s_qimg + ks * 2 * (T2_COLS * 16), T2_COLS * 16, 128), idy1, ks > 0);
+                            tc::mma_ss(tmem + TM_Z, tc::desc_at(d_rimg, ks * 2 * 2048), tc::desc_at(d_qk, ks * 2 * (T2_COLS * 16)), idy1, ks > 0);
 #pragma unroll
                         for (int ks = 0; ks < T2_K3 / 16; ++ks)
-                            tc::mma_ss(tmem + TM_Z, tc::desc(s_tlo + (T2_O3 / 8 + 2 * ks) * 2048, 2048, 128),
-                                       tc::desc(sbase + SL::W3T + ks * 2 * (96 * 16), 96 * 16, 128), idy1, true);
+                            tc::mma_ss(tmem + TM_Z, tc::desc_at(d_tlo, (T2_O3 / 8 + 2 * ks) * 2048), tc::desc_at(d_w3t, ks * 2 * (96 * 16)), idy1, true);
                     }
+                    DP_TICK(11);
                     wait_mma();
+                    DP_TICK(12);
                     // ---- E5: dz2 = dy2 (1 - t2^2) -> t2 block of the lo image ----
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
@@ -544,17 +565,19 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, EnvParams ep, const
                         else *reinterpret_cast<uint4 *>(img + 6 * 2048) =
                                  make_uint4(hmul2(tc::pack_h2(__uint_as_float(g1[0]), __uint_as_float(g1[1])), d2p[h][8]), 0u, 0u, 0u);
                     }
+                    DP_TICK(13);
                     sync_issue();
                     if (tw == 0) {
                         tc::fence_after();
                         constexpr uint32_t id1 = tc::idesc(128, 32, false, false);
 #pragma unroll
                         for (int ks = 0; ks < T2_K2 / 16; ++ks)
-                            tc::mma_ss(tmem + TM_Z, tc::desc(s_tlo + (T2_O2 / 8 + 2 * ks) * 2048, 2048, 128),
-                                       tc::desc(sbase + SL::W2T + ks * 2 * (32 * 16), 32 * 16, 128), id1, true);
+                            tc::mma_ss(tmem + TM_Z, tc::desc_at(d_tlo, (T2_O2 / 8 + 2 * ks) * 2048), tc::desc_at(d_w2t, ks * 2 * (32 * 16)), id1, true);
                         tc::commit(bar);
                     }
+                    DP_TICK(14);
                     wait_mma();
+                    DP_TICK(15);
                     // ---- E6: ds^ = sum_e dy1 (1 - t1^2) w1; gradient of the environment row; S8 + S9 in fp64 ----
                     {
                         float ds = 0.f;
@@ -570,77 +593,119 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, EnvParams ep, const
                                 if (16 * h + 2 * q + 1 < 25) ds = fmaf(__uint_as_float(g0[2 * q + 1]) * d.y, sw1[16 * h + 2 * q + 1], ds);
                             }
                         }
-                        double gk[3] = {0.0, 0.0, 0.0};
-                        if (real) {
+                        // gradient of E with respect to this row of the environment matrix R~ (S8 + S9 run in k_prod_force_virial)
+                        if (in) {
                             const float osc = 1.0f / ((float)Nm * gsc);
-                            const double g0_ = (double)((dR[0] + ds) * osc * isd[0]), g1_ = (double)(dR[1] * osc * isd[1]);
-                            const double g2_ = (double)(dR[2] * osc * isd[2]), g3_ = (double)(dR[3] * osc * isd[3]);
-                            const int j = id.y;
-                            const double dx = min_image(xj - xc, ep.L[0], hx);
-                            const double dy = min_image(yj - yc, ep.L[1], hy);
-                            const double dz = min_image(zj - zc, ep.L[2], hz);
-                            const double r2 = dx * dx + dy * dy + dz * dz;
-                            const double r = sqrt(r2), ir = 1.0 / r;
-                            double w = 1.0, dw = 0.0;
-                            if (r >= ep.rc_smth) {
-                                if (r < ep.rc) {
-                                    const double u = (r - ep.rc_smth) * ep.inv_range;
-                                    w = u * u * u * (-6.0 * u * u + 15.0 * u - 10.0) + 1.0;
-                                    dw = -30.0 * u * u * (u - 1.0) * (u - 1.0) * ep.inv_range;
-                                } else {
-                                    w = 0.0;
-                                }
-                            }
-                            const double s = w * ir;
-                            const double sp = dw * ir - w * ir * ir;          // ds/dr
-                            const double gd = g1_ * dx + g2_ * dy + g3_ * dz;
-                            const double coef = (sp * ir - s * ir * ir) * ir;
-                            const double c0 = g0_ * sp * ir + coef * gd, c1 = s * ir;
-                            gk[0] = c0 * dx + c1 * g1_;
-                            gk[1] = c0 * dy + c1 * g2_;
-                            gk[2] = c0 * dz + c1 * g3_;
-#pragma unroll
-                            for (int bb = 0; bb < 3; ++bb) atomicAdd(&fsorted[3 * (long)j + bb], -gk[bb]);
-                            vir[0] -= dx * gk[0]; vir[1] -= dx * gk[1]; vir[2] -= dx * gk[2];
-                            vir[3] -= dy * gk[0]; vir[4] -= dy * gk[1]; vir[5] -= dy * gk[2];
-                            vir[6] -= dz * gk[0]; vir[7] -= dz * gk[1]; vir[8] -= dz * gk[2];
-                        }
-                        // centre atom: one atomic per warp when all its real rows belong to the same atom
-                        {
-                            const unsigned rm = __ballot_sync(0xffffffffu, real);
-                            if (rm) {
-                                const int a0 = __shfl_sync(0xffffffffu, atom, __ffs(rm) - 1);
-                                if (__all_sync(0xffffffffu, !real || atom == a0)) {
-#pragma unroll
-                                    for (int bb = 0; bb < 3; ++bb) {
-                                        double v = gk[bb];
-#pragma unroll
-                                        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-                                        if (lane == 0) atomicAdd(&fsorted[3 * (long)a0 + bb], v);
-                                    }
-                                } else if (real) {
-#pragma unroll
-                                    for (int bb = 0; bb < 3; ++bb) atomicAdd(&fsorted[3 * (long)atom + bb], gk[bb]);
-                                }
-                            }
+                            rows_g[rbase + r0 + t] = make_float4((dR[0] + ds) * osc * isd[0], dR[1] * osc * isd[1], dR[2] * osc * isd[2],
+                                                                 dR[3] * osc * isd[3]);
                         }
                     }
+                    DP_TICK(16);
                 }   // passes
                 if (tw == 0) my_rows += (unsigned long long)nrows;
             }
         }
     }
+    tc::fence_before();
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base_s), "n"(512));
+    if (tw == 0 && my_rows) atomicAdd(row_counter, my_rows);
+#ifdef DP_BWD_TIMING
+    if (dbg_t) for (int k = 0; k < 20; ++k) tdbg[k] = tacc[k];
+#endif
+}
+
+
+// S8 + S9 (ProdForce, ProdViral): one thread per compact neighbour row.  g = dE/dR~ of the row (fp32, from
+// the backward kernel); the geometry derivative, the force scatter and the virial are fp64 (configs 3-4).
+__global__ void __launch_bounds__(256)
+k_prod_force_virial(long N, int T, int4 off4, int4 sel4, EnvParams ep, const int *__restrict__ rowstart,
+                    const int2 *__restrict__ rows_id, const float4 *__restrict__ rows_g, const double *__restrict__ xs,
+                    double *__restrict__ fsorted, double *__restrict__ virial) {
+    const int lane = threadIdx.x & 31;
+    const int off[4] = {off4.x, off4.y, off4.z, off4.w}, sel[4] = {sel4.x, sel4.y, sel4.z, sel4.w};
+    const double hx = 0.5 * ep.L[0], hy = 0.5 * ep.L[1], hz = 0.5 * ep.L[2];
+    double vir[9];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) vir[k] = 0.0;
+    for (int b = 0; b < T; ++b) {
+        const long rbase = N * (long)off[b];
+        const long nrows = rowstart[(long)b * (N + 1) + N];
+        (void)sel;
+        // whole warps walk the rows so that the warp-level reduction below is always convergent
+        for (long r0 = (blockIdx.x * (long)blockDim.x + threadIdx.x) - lane; r0 < nrows; r0 += (long)gridDim.x * blockDim.x) {
+            const long row = r0 + lane;
+            int2 id = make_int2(-1, -1);
+            if (row < nrows) id = __ldg(&rows_id[rbase + row]);
+            const bool real = id.y >= 0;
+            const int atom = id.x;
+            double gk[3] = {0.0, 0.0, 0.0};
+            if (real) {
+                const float4 g = __ldg(&rows_g[rbase + row]);
+                const int j = id.y;
+                const double dx = min_image(xs[3 * (long)j] - xs[3 * (long)atom], ep.L[0], hx);
+                const double dy = min_image(xs[3 * (long)j + 1] - xs[3 * (long)atom + 1], ep.L[1], hy);
+                const double dz = min_image(xs[3 * (long)j + 2] - xs[3 * (long)atom + 2], ep.L[2], hz);
+                const double r2 = dx * dx + dy * dy + dz * dz;
+                const double ir = rsqrt(r2), r = r2 * ir;
+                double w = 1.0, dw = 0.0;
+                if (r >= ep.rc_smth) {
+                    if (r < ep.rc) {
+                        const double u = (r - ep.rc_smth) * ep.inv_range;
+                        w = u * u * u * (-6.0 * u * u + 15.0 * u - 10.0) + 1.0;
+                        dw = -30.0 * u * u * (u - 1.0) * (u - 1.0) * ep.inv_range;
+                    } else {
+                        w = 0.0;
+                    }
+                }
+                const double s = w * ir;
+                const double sp = dw * ir - w * ir * ir;          // ds/dr
+                const double g0_ = g.x, g1_ = g.y, g2_ = g.z, g3_ = g.w;
+                const double gd = g1_ * dx + g2_ * dy + g3_ * dz;
+                const double coef = (sp * ir - s * ir * ir) * ir;
+                const double c0 = g0_ * sp * ir + coef * gd, c1 = s * ir;
+                gk[0] = c0 * dx + c1 * g1_;
+                gk[1] = c0 * dy + c1 * g2_;
+                gk[2] = c0 * dz + c1 * g3_;
+#pragma unroll
+                for (int bb = 0; bb < 3; ++bb) atomicAdd(&fsorted[3 * (long)j + bb], -gk[bb]);
+                vir[0] -= dx * gk[0]; vir[1] -= dx * gk[1]; vir[2] -= dx * gk[2];
+                vir[3] -= dy * gk[0]; vir[4] -= dy * gk[1]; vir[5] -= dy * gk[2];
+                vir[6] -= dz * gk[0]; vir[7] -= dz * gk[1]; vir[8] -= dz * gk[2];
+            }
+            // centre atom: one atomic per warp when all its real rows belong to the same atom
+            const unsigned rm = __ballot_sync(0xffffffffu, real);
+            if (rm) {
+                const int a0 = __shfl_sync(0xffffffffu, atom, __ffs(rm) - 1);
+                if (__all_sync(0xffffffffu, !real || atom == a0)) {
+#pragma unroll
+                    for (int bb = 0; bb < 3; ++bb) {
+                        double v = gk[bb];
+#pragma unroll
+                        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                        if (lane == 0) atomicAdd(&fsorted[3 * (long)a0 + bb], v);
+                    }
+                } else if (real) {
+#pragma unroll
+                    for (int bb = 0; bb < 3; ++bb) atomicAdd(&fsorted[3 * (long)atom + bb], gk[bb]);
+                }
+            }
+        }
+    }
+    __shared__ double red[8][9];
 #pragma unroll
     for (int k = 0; k < 9; ++k) {
         double v = vir[k];
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-        if (lane == 0 && v != 0.0) atomicAdd(&virial[k], v);
+        if (lane == 0) red[threadIdx.x >> 5][k] = v;
     }
-    tc::fence_before();
     __syncthreads();
-    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base_s), "n"(512));
-    if (tw == 0 && my_rows) atomicAdd(row_counter, my_rows);
+    if (threadIdx.x < 9) {
+        double v = 0.0;
+        for (int w = 0; w < 8; ++w) v += red[w][threadIdx.x];
+        if (v != 0.0) atomicAdd(&virial[threadIdx.x], v);
+    }
 }
 
 }  // namespace
@@ -659,10 +724,32 @@ cudaError_t launch_embed_bwd_tc2(const dp_model *m, long N, const Grid3 &g, char
     const int smem_ga = 4 * GA_WARP_FLOATS * 4;
     k_gA_img<<<(unsigned)((N + 3) / 4), 128, smem_ga, st>>>(N, (const float *)(ws + L.A), (const float *)(ws + L.gD),
                                                              (uint8_t *)(ws + L.gAf), (float *)(ws + L.gscale));
+    long long *tdbg = nullptr;
+#ifdef DP_BWD_TIMING
+    static long long *tbuf = nullptr;
+    if (!tbuf) cudaMalloc(&tbuf, 20 * sizeof(long long));
+    tdbg = tbuf;
+#endif
     k_embed_bwd_tc2<<<m->num_sms, NWG * WGT, BwdSmem::TOTAL, st>>>(
-        N, m->T, g.ncell, m->Nm, off4, ep, (const EmbedNetTC2 *)m->embed_tc2_dev, m->std_dev, (int *)(ws + L.bin_start),
-        (int *)(ws + L.rowstart), (const float4 *)(ws + L.rows_rh), (const int2 *)(ws + L.rows_id), (double *)(ws + L.xs),
-        (const uint8_t *)(ws + L.gAf), (const float *)(ws + L.gscale), (double *)(ws + L.fsorted), (double *)(ws + L.virial),
-        (unsigned long long *)(ws + L.status + 16));
+        N, m->T, g.ncell, m->Nm, off4, (const EmbedNetTC2 *)m->embed_tc2_dev, m->std_dev, (int *)(ws + L.bin_start),
+        (int *)(ws + L.rowstart), (const float4 *)(ws + L.rows_rh), (const int2 *)(ws + L.rows_id),
+        (const uint8_t *)(ws + L.gAf), (const float *)(ws + L.gscale), (float4 *)(ws + L.rows_g),
+        (unsigned long long *)(ws + L.status + 16), tdbg);
+    int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
+    k_prod_force_virial<<<m->num_sms * 8, 256, 0, st>>>(N, m->T, off4, sel4, ep, (int *)(ws + L.rowstart),
+                                                        (const int2 *)(ws + L.rows_id), (const float4 *)(ws + L.rows_g),
+                                                        (double *)(ws + L.xs), (double *)(ws + L.fsorted), (double *)(ws + L.virial));
+#ifdef DP_BWD_TIMING
+    if (tdbg) {
+        cudaStreamSynchronize(st);
+        long long h[20];
+        cudaMemcpy(h, tdbg, sizeof(h), cudaMemcpyDeviceToHost);
+        long long tot = 0;
+        for (int k = 0; k < 20; ++k) tot += h[k];
+        fprintf(stderr, "bwd phase cycles (WG0 of CTA 0), total %lld:", tot);
+        for (int k = 0; k < 20; ++k) fprintf(stderr, " %d:%.1f%%", k, 100.0 * h[k] / (double)tot);
+        fprintf(stderr, "\n");
+    }
+#endif
     return cudaGetLastError();
 }

@@ -19,6 +19,8 @@ __device__ __forceinline__ uint64_t desc(uint32_t saddr, uint32_t lbo_bytes, uin
     d |= (uint64_t)1 << 46;
     return d;
 }
+// descriptor of the same image at a byte offset (16-byte granularity; the address field must not overflow its 14 bits)
+__device__ __forceinline__ uint64_t desc_at(uint64_t d, uint32_t byte_off) { return d + (uint64_t)(byte_off >> 4); }
 // kind::f16 instruction descriptor: fp16 x fp16 -> fp32, M x N, optional MN-major operands
 __host__ __device__ constexpr uint32_t idesc(int M, int N, bool a_mn, bool b_mn) {
     return (1u << 4) | ((a_mn ? 1u : 0u) << 15) | ((b_mn ? 1u : 0u) << 16) | ((uint32_t)(N >> 3) << 17) |
