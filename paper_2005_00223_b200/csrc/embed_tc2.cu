@@ -58,7 +58,9 @@ k_embed_fwd_tc2(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, const Em
     using SL = FwdSmem;
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ uint32_t tmem_base_s;
-    const int tid = threadIdx.x, warp = tid >> 5, wg = warp >> 2, t = tid & 127;
+    const int tid = threadIdx.x, t = tid & 127;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0), wg = warp >> 2;     // warp-uniform (MMA operands in uniform registers)
+    const bool issuer_warp = (warp & 3) == 0;
     float *sw1 = reinterpret_cast<float *>(smem + SL::VEC), *sb1 = sw1 + 32;
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem + SL::BARS);
     uint8_t *wgs = smem + SL::WG0 + wg * SL::WG_BYTES;
@@ -83,10 +85,12 @@ k_embed_fwd_tc2(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, const Em
     tc::fence_before();
     __syncthreads();
     tc::fence_after();
-    const uint32_t tmem = tmem_base_s + wg * TM_WG;
+    const uint32_t tmem = __shfl_sync(0xffffffffu, tmem_base_s, 0) + wg * TM_WG;
     const uint32_t tm_lane = tmem + ((uint32_t)((warp & 3) * 32) << 16);
     const uint32_t sbase = tc::smem_u32(smem);
     const uint32_t s_timg = tc::smem_u32(wgs + SL::TIMG), s_rimg = tc::smem_u32(wgs + SL::RIMG);
+    const uint64_t d_timg = tc::desc(s_timg, 2048, 128), d_timg_mn = tc::desc(s_timg, 128, 2048), d_rimg_mn = tc::desc(s_rimg, 128, 2048);
+    const uint64_t d_w2 = tc::desc(sbase + SL::W2, 64 * 16, 128), d_w3 = tc::desc(sbase + SL::W3, 112 * 16, 128);
     uint64_t *bar = &bars[wg];
     uint32_t ph = 0;
     unsigned long long my_rows = 0;
@@ -183,13 +187,12 @@ k_embed_fwd_tc2(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, const Em
                 tc::fence_before();
                 tc::bar_sync(1 + wg, 128);
                 const int atom0 = meta[0], atomL = meta[1];
-                if (t == 0) {
+                if (issuer_warp && tc::elect_one()) {
                     tc::fence_after();
                     constexpr uint32_t id2 = tc::idesc(128, 64, false, false);
 #pragma unroll
                     for (int ks = 0; ks < 2; ++ks)
-                        tc::mma_ss(tmem + TM_Z, tc::desc(s_timg + ks * 2 * 2048, 2048, 128),
-                                   tc::desc(sbase + SL::W2 + ks * 2 * (64 * 16), 64 * 16, 128), id2, ks > 0);
+                        tc::mma_ss(tmem + TM_Z, tc::desc_at(d_timg, ks * 2 * 2048), tc::desc_at(d_w2, ks * 2 * (64 * 16)), id2, ks > 0);
                     tc::commit(bar);
                 }
                 // while layer 2 runs: retire the previous tile's last atom if this tile starts a new one
@@ -219,14 +222,13 @@ k_embed_fwd_tc2(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, const Em
                 tc::proxy_fence();
                 tc::fence_before();
                 tc::bar_sync(1 + wg, 128);
-                if (t == 0) {
+                if (issuer_warp && tc::elect_one()) {
                     tc::fence_after();
                     constexpr uint32_t id3 = tc::idesc(128, 112, false, false);
 #pragma unroll
                     for (int ks = 0; ks < 6; ++ks) {
                         const int achunk = ks < 4 ? T2_O2 / 8 + 2 * ks : 2 * (ks - 4);
-                        tc::mma_ss(tmem + TM_Z, tc::desc(s_timg + achunk * 2048, 2048, 128),
-                                   tc::desc(sbase + SL::W3 + ks * 2 * (112 * 16), 112 * 16, 128), id3, ks > 0);
+                        tc::mma_ss(tmem + TM_Z, tc::desc_at(d_timg, achunk * 2048), tc::desc_at(d_w3, ks * 2 * (112 * 16)), id3, ks > 0);
                     }
                     tc::commit(bar);
                 }
@@ -263,15 +265,14 @@ k_embed_fwd_tc2(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, const Em
                     tc::proxy_fence();
                     tc::fence_before();
                     tc::bar_sync(1 + wg, 128);
-                    if (t == 0) {
+                    if (issuer_warp && tc::elect_one()) {
                         tc::fence_after();
                         constexpr uint32_t idc = tc::idesc(128, 8 * T2_NSLOT, true, true);
 #pragma unroll
                         for (int half = 0; half < 2; ++half)
 #pragma unroll
                             for (int ks = 0; ks < T2_ROWS / 16; ++ks)
-                                tc::mma_ss(tmem + (half ? TM_D2 : TM_D1), tc::desc(s_timg + half * 16 * 2048 + ks * 256, 128, 2048),
-                                           tc::desc(s_rimg + ks * 256, 128, 2048), idc, true);
+                                tc::mma_ss(tmem + (half ? TM_D2 : TM_D1), tc::desc_at(d_timg_mn, half * 16 * 2048 + ks * 256), tc::desc_at(d_rimg_mn, ks * 256), idc, true);
                         tc::commit(bar);
                     }
                     tc::mbar_wait(bar, ph); ph ^= 1;

@@ -245,8 +245,10 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *
     using SL = BwdSmem;
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ uint32_t tmem_base_s;
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);      // warp-uniform: keeps the MMA operands in uniform registers
     const int wg = warp >> 2, t = tid & (WGT - 1), tw = t;
+    const bool issuer_warp = (warp & 3) == 0;
     float *sw1 = reinterpret_cast<float *>(smem + SL::VEC), *sb1 = sw1 + 32;
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem + SL::BARS);
     uint8_t *wgs = smem + SL::WG0 + wg * SL::WG_BYTES;
@@ -265,7 +267,7 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *
     tc::fence_before();
     __syncthreads();
     tc::fence_after();
-    const uint32_t tmem = tmem_base_s + wg * TM_WG;
+    const uint32_t tmem = __shfl_sync(0xffffffffu, tmem_base_s, 0) + wg * TM_WG;
     const uint32_t tm_lane = tmem + ((uint32_t)((warp & 3) * 32) << 16);
     const uint32_t sbase = tc::smem_u32(smem);
     const uint32_t s_tlo = tc::smem_u32(wgs + SL::TLO), s_rimg = tc::smem_u32(wgs + SL::RIMG);
@@ -394,7 +396,7 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *
                     tc::wait_st();
                     DP_TICK(1);
                     sync_issue();
-                    if (tw == 0) {
+                    if (issuer_warp && tc::elect_one()) {
                         tc::fence_after();
                         constexpr uint32_t id2 = tc::idesc(128, 64, false, false);
 #pragma unroll
@@ -432,7 +434,7 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *
                     tc::wait_st();
                     DP_TICK(4);
                     sync_issue();
-                    if (tw == 0) {
+                    if (issuer_warp && tc::elect_one()) {
                         tc::fence_after();
                         constexpr uint32_t id3 = tc::idesc(128, 112, false, false);
 #pragma unroll
@@ -478,7 +480,7 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *
                     cp_async_wait_all();
                     DP_TICK(7);
                     sync_issue();
-                    if (tw == 0) {
+                    if (issuer_warp && tc::elect_one()) {
                         tc::fence_after();
                         constexpr uint32_t idr = tc::idesc(128, 8 * T2_NSLOT, false, true);
 #pragma unroll
@@ -528,7 +530,7 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *
                     }
                     DP_TICK(10);
                     sync_issue();
-                    if (tw == 0) {
+                    if (issuer_warp && tc::elect_one()) {
                         tc::fence_after();
                         // dy2 first (the next stage needs it) ...
                         constexpr uint32_t idy2 = tc::idesc(128, 64, false, false);
@@ -567,7 +569,7 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *
                     }
                     DP_TICK(13);
                     sync_issue();
-                    if (tw == 0) {
+                    if (issuer_warp && tc::elect_one()) {
                         tc::fence_after();
                         constexpr uint32_t id1 = tc::idesc(128, 32, false, false);
 #pragma unroll

@@ -84,7 +84,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_fit_tc(FitTcArgs p) {
     using C = Cfg<KTOT, NTOT>;
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ uint32_t tmem_base_s;
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);       // warp-uniform role index
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem + C::OFF_BAR);
     uint64_t *b_full = bars, *b_empty = bars + 2, *a_full = bars + 4, *a_empty = bars + 4 + C::NA;
     uint64_t *acc_full = bars + 4 + 2 * C::NA, *acc_empty = acc_full + 2;
@@ -101,7 +102,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_fit_tc(FitTcArgs p) {
     tc::fence_before();
     __syncthreads();
     tc::fence_after();
-    const uint32_t tmem = tmem_base_s;
+    const uint32_t tmem = __shfl_sync(0xffffffffu, tmem_base_s, 0);
     const uint32_t sbase = tc::smem_u32(smem);
     int ntiles_total = 0;
     for (int a = 0; a < p.T; ++a) ntiles_total += (p.bin_start[(a + 1) * p.ncell] - p.bin_start[a * p.ncell] + BM - 1) / BM;
@@ -124,8 +125,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_fit_tc(FitTcArgs p) {
             }
         }
     } else if (warp == 1) {
-        // ---------------------------------------------------------------- MMA issuer
-        if (lane == 0) {
+        // ---------------------------------------------------------------- MMA issuer (whole warp walks the loop, one lane issues)
+        {
             constexpr uint32_t idesc = tc::idesc(128, C::BN, false, false);
             uint32_t step = 0, astep = 0, accn = 0, it = 0;
             for (int tile = blockIdx.x; tile < ntiles_total; tile += gridDim.x, ++it) {
@@ -140,18 +141,23 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_fit_tc(FitTcArgs p) {
                         else { ab = astep & 1; tc::mbar_wait(&a_full[ab], (astep >> 1) & 1); }
                         tc::mbar_wait(&b_full[st], (step >> 1) & 1);
                         tc::fence_after();
-                        const uint32_t a_hi = sbase + C::OFF_A + ab * C::A_BUF, b_img = sbase + C::OFF_B + st * C::B_STAGE;
+                        const uint64_t da = tc::desc(sbase + C::OFF_A + ab * C::A_BUF, A_SUB_STRIDE, 128);
+                        const uint64_t db = tc::desc(sbase + C::OFF_B + st * C::B_STAGE, C::BN * 16, 128);
+                        if (tc::elect_one()) {
 #pragma unroll
-                        for (int part = 0; part < 2; ++part)
+                            for (int part = 0; part < 2; ++part)
 #pragma unroll
-                            for (int ks = 0; ks < KC / 16; ++ks)
-                                tc::mma_ss(tmem + buf * C::TM_BUF, tc::desc(a_hi + part * A_PART + ks * 2 * A_SUB_STRIDE, A_SUB_STRIDE, 128),
-                                           tc::desc(b_img + ks * 2 * (C::BN * 16), C::BN * 16, 128), idesc, (kc | part | ks) != 0);
-                        tc::commit(&b_empty[st]);
-                        if (!C::RESIDENT) { tc::commit(&a_empty[ab]); ++astep; }
-                        else if (nt == C::NTILES - 1) tc::commit(&a_empty[ab]);
+                                for (int ks = 0; ks < KC / 16; ++ks)
+                                    tc::mma_ss(tmem + buf * C::TM_BUF, tc::desc_at(da, part * A_PART + ks * 2 * A_SUB_STRIDE),
+                                               tc::desc_at(db, ks * 2 * (C::BN * 16)), idesc, (kc | part | ks) != 0);
+                            tc::commit(&b_empty[st]);
+                            if (!C::RESIDENT || nt == C::NTILES - 1) tc::commit(&a_empty[ab]);
+                        }
+                        __syncwarp();
+                        if (!C::RESIDENT) ++astep;
                     }
-                    tc::commit(&acc_full[buf]);
+                    if (tc::elect_one()) tc::commit(&acc_full[buf]);
+                    __syncwarp();
                 }
             }
         }
