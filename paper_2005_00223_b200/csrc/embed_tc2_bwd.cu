@@ -67,18 +67,6 @@ __device__ __forceinline__ void cp_async8(uint32_t sdst, const void *gsrc) {
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-// prefetch loads that the compiler must keep where they are written (issued one tile ahead of their use)
-__device__ __forceinline__ float4 ldv_f4(const float4 *p) {
-    float4 r;
-    asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
-    return r;
-}
-__device__ __forceinline__ int2 ldv_i2(const int2 *p) {
-    int2 r;
-    asm volatile("ld.global.nc.v2.s32 {%0,%1}, [%2];" : "=r"(r.x), "=r"(r.y) : "l"(p));
-    return r;
-}
-
 __device__ __forceinline__ float2 unpack_h2(uint32_t v) {
     return __half22float2(*reinterpret_cast<const __half2 *>(&v));
 }
@@ -96,18 +84,6 @@ __device__ __forceinline__ void act16(const uint32_t (&z)[16], uint32_t tm_dst, 
     *reinterpret_cast<uint4 *>(lo_row + chunk * 2048) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
     *reinterpret_cast<uint4 *>(lo_row + (chunk + 1) * 2048) = make_uint4(lo[4], lo[5], lo[6], lo[7]);
 }
-// 16 gradient columns times 1 - t^2 -> fp16 -> two chunks
-__device__ __forceinline__ void grad16(const uint32_t (&g)[16], const uint32_t *dpk, uint8_t *row, int chunk) {
-    uint32_t o[8];
-#pragma unroll
-    for (int q = 0; q < 8; ++q) {
-        const float2 d = unpack_h2(dpk[q]);
-        o[q] = tc::pack_h2(__uint_as_float(g[2 * q]) * d.x, __uint_as_float(g[2 * q + 1]) * d.y);
-    }
-    *reinterpret_cast<uint4 *>(row + chunk * 2048) = make_uint4(o[0], o[1], o[2], o[3]);
-    *reinterpret_cast<uint4 *>(row + (chunk + 1) * 2048) = make_uint4(o[4], o[5], o[6], o[7]);
-}
-
 // Per-atom operand image of the folded gradient g~[c][col] = fold(gA)[c][col] * 2^e, split in hi + lo fp16 parts:
 //   C [208][8] : per T column {hi[0..3], lo[0..3]} (16 bytes)
 // gA[c][m] = sum_a gD[m][a] A[c][a] + [m < 16] sum_m' gD[m'][m] A[c][m'], fp32.
@@ -209,6 +185,52 @@ __global__ void __launch_bounds__(128) k_gA_img(long N, const float *__restrict_
     }
 }
 
+// Same image from gA itself (fp32 [N][4][100], written by the epilogue of the last fitting-backward GEMM, fit_tc.cu MODE 6).
+__global__ void __launch_bounds__(256) k_gA_fold(long N, const float *__restrict__ gA, uint8_t *__restrict__ img,
+                                                  float *__restrict__ gscale) {
+    __shared__ __align__(16) float sO_all[8][4 * M2E];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const long i = blockIdx.x * 8L + wid;
+    if (i >= N) return;
+    float *sO = sO_all[wid];
+    const float4 *g4 = reinterpret_cast<const float4 *>(gA + i * 4 * M2E);
+    for (int k = lane; k < M2E; k += 32) reinterpret_cast<float4 *>(sO)[k] = __ldg(g4 + k);
+    __syncwarp();
+    float v[7][4];
+    float mx = 0.f;
+#pragma unroll
+    for (int j = 0; j < 7; ++j) {
+        const int col = lane + 32 * j;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const float *o = sO + c * M2E;
+            float x = 0.f;
+            if (col < T2_O2) { if (col < M0) x = (o[col] + o[col + M0]) + (o[col + 2 * M0] + o[col + 3 * M0]); }
+            else if (col < T2_O3) { const int f = col - T2_O2; if (f < M1) x = o[f] + o[f + M1]; }
+            else if (col < T2_COLS) { const int m = col - T2_O3; if (m < M2E) x = o[m]; }
+            v[j][c] = x;
+            mx = fmaxf(mx, fabsf(x));
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    int ex = 0;
+    if (mx > 0.f) frexpf(mx, &ex);
+    const float sc = ldexpf(1.f, -ex);          // max |g~| in [0.5, 1)
+    if (lane == 0) gscale[i] = sc;
+    uint4 *C = reinterpret_cast<uint4 *>(img + i * (long)GA_IMG_BYTES);
+#pragma unroll
+    for (int j = 0; j < 7; ++j) {
+        const int col = lane + 32 * j;
+        if (col < T2_COLS) {
+            uint32_t h01, l01, h23, l23;
+            tc::split_h2(v[j][0] * sc, v[j][1] * sc, h01, l01);
+            tc::split_h2(v[j][2] * sc, v[j][3] * sc, h23, l23);
+            C[col] = make_uint4(h01, h23, l01, l23);
+        }
+    }
+}
+
 // hi parts -> 8 TMEM columns, lo parts -> two 16-byte chunks, 1 - t^2 -> dpk (fp16 pairs); t given in fp32
 __device__ __forceinline__ void emit16(const float (&y)[16], uint32_t tm_dst, uint8_t *lo_row, int chunk, uint32_t *dpk) {
     uint32_t hi[8], lo[8];
@@ -229,7 +251,14 @@ __device__ __forceinline__ uint32_t hmul2(uint32_t a, uint32_t b) {
 __device__ __forceinline__ void gradh16(const uint32_t (&g)[16], const uint32_t *dpk, uint8_t *row, int chunk) {
     uint32_t o[8];
 #pragma unroll
-    for (int q = 0; q < 8; ++q) o[q] = hmul2(tc::pack_h2(__uint_as_float(g[2 * q]), __uint_as_float(g[2 * q + 1])), dpk[q]);
+    for (int q = 0; q < 8; ++q) {
+#ifndef DP_GRAD_F16
+        const float2 d = unpack_h2(dpk[q]);
+        o[q] = tc::pack_h2(__uint_as_float(g[2 * q]) * d.x, __uint_as_float(g[2 * q + 1]) * d.y);
+#else
+        o[q] = hmul2(tc::pack_h2(__uint_as_float(g[2 * q]), __uint_as_float(g[2 * q + 1])), dpk[q]);
+#endif
+    }
     *reinterpret_cast<uint4 *>(row + chunk * 2048) = make_uint4(o[0], o[1], o[2], o[3]);
     *reinterpret_cast<uint4 *>(row + (chunk + 1) * 2048) = make_uint4(o[4], o[5], o[6], o[7]);
 }
@@ -245,7 +274,7 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *
     using SL = BwdSmem;
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ uint32_t tmem_base_s;
-    const int tid = threadIdx.x, lane = tid & 31;
+    const int tid = threadIdx.x;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);      // warp-uniform: keeps the MMA operands in uniform registers
     const int wg = warp >> 2, t = tid & (WGT - 1), tw = t;
     const bool issuer_warp = (warp & 3) == 0;
@@ -378,7 +407,8 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *
                             cp_async16(s_qimg + (2 * s_ + 1) * (T2_COLS * 16) + k * 16, C + k);
                         }
                     }
-                    uint32_t d1p[2][8], d2p[2][16], d3p[2][26];       // 1 - t^2 per column half (fp16 pairs)
+                    uint32_t d1p[2][8], d2p[2][16], d3p[2][26];       // 1 - t^2 per column half (fp16 pairs; only layer 3's are read back)
+                    float d2f[2][32], d1f[2][16];     // layers 1-2 keep 1 - t^2 in fp32: fp16 here costs 2x in force error
                     DP_TICK(0);
                     // ---- E1: layer 1 on the ALUs; h = 0: t1[0..16), h = 1: t1[16..25), ones, padding ----
 #pragma unroll
@@ -392,6 +422,8 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *
                             else y[e] = ee <= 26 ? 1.f : 0.f;
                         }
                         emit16(y, tm_lane + TM_T + 8 * h, lo_row, 2 * h, d1p[h]);
+#pragma unroll
+                        for (int q = 0; q < 16; ++q) d1f[h][q] = fmaf(-y[q], y[q], 1.f);
                     }
                     tc::wait_st();
                     DP_TICK(1);
@@ -420,6 +452,10 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *
                         else tc::ld2(tm_lane + TM_Z + 48, reinterpret_cast<uint32_t (&)[2]>(z1));
                         tc::wait_ld();
                         act16(z0, tm_lane + TM_T + 16 + 16 * h, img, 4 * h, d2p[h]);
+#pragma unroll
+                        for (int q = 0; q < 16; ++q) { const float tt = tc::tanh_approx(__uint_as_float(z0[q])); d2f[h][q] = fmaf(-tt, tt, 1.f); }
+#pragma unroll
+                        for (int q = 0; q < 16; ++q) { const float tt = tc::tanh_approx(__uint_as_float(z1[q & (h ? 1 : 15)])); d2f[h][16 + q] = fmaf(-tt, tt, 1.f); }
                         if (h == 0) {
                             act16(z1, tm_lane + TM_T + 24, img, 2, d2p[h] + 8);
                         } else {
@@ -562,10 +598,21 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *
                         if (h == 0) tc::ld16(tm_lane + TM_Z + 48, g1);
                         else tc::ld2(tm_lane + TM_Z + 80, reinterpret_cast<uint32_t (&)[2]>(g1));
                         tc::wait_ld();
-                        gradh16(g0, d2p[h], img, 4 * h);
-                        if (h == 0) gradh16(g1, d2p[h] + 8, img, 2);
-                        else *reinterpret_cast<uint4 *>(img + 6 * 2048) =
-                                 make_uint4(hmul2(tc::pack_h2(__uint_as_float(g1[0]), __uint_as_float(g1[1])), d2p[h][8]), 0u, 0u, 0u);
+                        {
+                            uint32_t o[8];
+#pragma unroll
+                            for (int q = 0; q < 8; ++q) o[q] = tc::pack_h2(__uint_as_float(g0[2 * q]) * d2f[h][2 * q], __uint_as_float(g0[2 * q + 1]) * d2f[h][2 * q + 1]);
+                            *reinterpret_cast<uint4 *>(img + (4 * h) * 2048) = make_uint4(o[0], o[1], o[2], o[3]);
+                            *reinterpret_cast<uint4 *>(img + (4 * h + 1) * 2048) = make_uint4(o[4], o[5], o[6], o[7]);
+                            if (h == 0) {
+#pragma unroll
+                                for (int q = 0; q < 8; ++q) o[q] = tc::pack_h2(__uint_as_float(g1[2 * q]) * d2f[h][16 + 2 * q], __uint_as_float(g1[2 * q + 1]) * d2f[h][16 + 2 * q + 1]);
+                                *reinterpret_cast<uint4 *>(img + 2 * 2048) = make_uint4(o[0], o[1], o[2], o[3]);
+                                *reinterpret_cast<uint4 *>(img + 3 * 2048) = make_uint4(o[4], o[5], o[6], o[7]);
+                            } else {
+                                *reinterpret_cast<uint4 *>(img + 6 * 2048) = make_uint4(tc::pack_h2(__uint_as_float(g1[0]) * d2f[h][16], __uint_as_float(g1[1]) * d2f[h][17]), 0u, 0u, 0u);
+                            }
+                        }
                     }
                     DP_TICK(13);
                     sync_issue();
@@ -590,7 +637,7 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *
                             tc::wait_ld();
 #pragma unroll
                             for (int q = 0; q < 8; ++q) {
-                                const float2 d = unpack_h2(d1p[h][q]);
+                                const float2 d = make_float2(d1f[h][2 * q], d1f[h][2 * q + 1]);
                                 if (16 * h + 2 * q < 25) ds = fmaf(__uint_as_float(g0[2 * q]) * d.x, sw1[16 * h + 2 * q], ds);
                                 if (16 * h + 2 * q + 1 < 25) ds = fmaf(__uint_as_float(g0[2 * q + 1]) * d.y, sw1[16 * h + 2 * q + 1], ds);
                             }
@@ -724,8 +771,11 @@ cudaError_t launch_embed_bwd_tc2(const dp_model *m, long N, const Grid3 &g, char
     ep.rc = m->rc; ep.rc_smth = m->rc_smth; ep.inv_range = 1.0 / (m->rc - m->rc_smth);
     ep.L[0] = g.L[0]; ep.L[1] = g.L[1]; ep.L[2] = g.L[2];
     const int smem_ga = 4 * GA_WARP_FLOATS * 4;
-    k_gA_img<<<(unsigned)((N + 3) / 4), 128, smem_ga, st>>>(N, (const float *)(ws + L.A), (const float *)(ws + L.gD),
-                                                             (uint8_t *)(ws + L.gAf), (float *)(ws + L.gscale));
+    if (m->use_fit_tc)      // the last fitting GEMM left gA itself in the gD buffer (fit_tc.cu MODE 6)
+        k_gA_fold<<<(unsigned)((N + 7) / 8), 256, 0, st>>>(N, (const float *)(ws + L.gD), (uint8_t *)(ws + L.gAf), (float *)(ws + L.gscale));
+    else
+        k_gA_img<<<(unsigned)((N + 3) / 4), 128, smem_ga, st>>>(N, (const float *)(ws + L.A), (const float *)(ws + L.gD),
+                                                                 (uint8_t *)(ws + L.gAf), (float *)(ws + L.gscale));
     long long *tdbg = nullptr;
 #ifdef DP_BWD_TIMING
     static long long *tbuf = nullptr;

@@ -4,6 +4,7 @@
 // MIX-16: layers 1 and 2 (and their backward products) NS = 1, the third 240x240 layer NS = 3 and the output layer in
 // fp32 ("in the last layer of the fitting net, both data storage and arithmetic operations are kept in single
 // precision", reading Q16).  MIX-32: NS = 3 everywhere.  Activations are stored in fp32.
+#include <cstdlib>
 #include "embed_mix.cuh"
 
 namespace {
@@ -326,7 +327,10 @@ cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, 
         k_energy_f<<<nb8, 256, 0, st>>>(N, T, g.ncell, bin_start, h3, v4, c4, m->ebias_dev, (double *)(ws + L.eatom));
         fit_tc_gemm(3, false, m, g, bin_start, gz3, F, nullptr, v4, t2, nullptr, g2, gz2, F, st);
         fit_tc_gemm(4, false, m, g, bin_start, gz2, F, nullptr, nullptr, g2, h1, gz1, nullptr, F, st);
-        fit_tc_gemm(5, false, m, g, bin_start, gz1, F, nullptr, nullptr, nullptr, nullptr, D, nullptr, ND, st);
+        if (m->use_tc_bwd)   // gA in the epilogue: D receives gA [N][4][100], the gD tensor is never written
+            fit_tc_gemm(6, false, m, g, bin_start, gz1, F, nullptr, nullptr, Amat, nullptr, D, nullptr, ND, st);
+        else
+            fit_tc_gemm(5, false, m, g, bin_start, gz1, F, nullptr, nullptr, nullptr, nullptr, D, nullptr, ND, st);
     } else {
     launch_gemm<0>(ns12, apx, p, g240, st);
     p.K = F; p.A = h1; p.lda = F; p.B = V2; p.b_type_stride = (long)F * F; p.bias = c2; p.aux0 = h1; p.out0 = t2; p.out1 = h2;
@@ -335,11 +339,12 @@ cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, 
     launch_gemm<2>(ns3, false, p, g240, st);
     k_energy_f<<<nb8, 256, 0, st>>>(N, T, g.ncell, bin_start, h3, v4, c4, m->ebias_dev, (double *)(ws + L.eatom));
     p.A = gz3; p.B = V3; p.aux0 = t2; p.out0 = g2; p.out1 = gz2;
-    launch_gemm<3>(ns3, false, p, g240, st);
+    const int nsb = std::getenv("DP_MIX16_FIT_BWD_NS") ? std::atoi(std::getenv("DP_MIX16_FIT_BWD_NS")) : 0;   // precision study
+    launch_gemm<3>(nsb ? nsb : ns3, false, p, g240, st);
     p.A = gz2; p.B = V2; p.aux0 = g2; p.aux1 = h1; p.out0 = gz1; p.out1 = nullptr;
-    launch_gemm<4>(ns12, false, p, g240, st);
+    launch_gemm<4>(nsb ? nsb : ns12, false, p, g240, st);
     p.A = gz1; p.N = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.out0 = D; p.ldo = ND;
-    launch_gemm<5>(ns12, false, p, g1600, st);
+    launch_gemm<5>(nsb ? nsb : ns12, false, p, g1600, st);
     }
     if (m->use_tc_bwd) return cudaGetLastError();     // the tcgen05 backward builds its own operand images of gA
     const int smem = 4 * (4 * M2E + M2E * 16 + 4 * M2E) * 4;

@@ -19,8 +19,10 @@ constexpr int KC = 80;                    // K chunk: 5 k-steps of 16
 constexpr int SUB = KC / 8;               // 16-byte sub-chunks per K chunk
 constexpr int A_SUB_STRIDE = BM * 16 + 16;   // bytes between sub-chunks of the A image (+16: conflict-free producer stores)
 constexpr int A_PART = SUB * A_SUB_STRIDE;   // one part (hi or lo) of one K chunk
-constexpr int NPROD = 256, NEPI = 128;
-constexpr int NTHREADS = 64 + NPROD + NEPI;
+constexpr int NPROD = 256;
+// epilogue threads: one per row; MODE 6 (gA in the epilogue) uses two per row, each owning two of the four components c
+__host__ __device__ constexpr int nepi(int mode) { return mode == 6 ? 256 : 128; }
+__host__ __device__ constexpr int nthreads(int mode) { return 64 + NPROD + nepi(mode); }
 
 template <int KTOT, int NTOT>
 struct Cfg {
@@ -30,10 +32,11 @@ struct Cfg {
     static constexpr int NKC = KTOT / KC;
     static constexpr int NA = RESIDENT ? NKC : 2;            // A buffers
     static constexpr int B_STAGE = KC * BN * 2;
+    static constexpr int NSTAGE = NTOT == 1600 ? 4 : 2;      // B pipeline depth (short N = 160 stages need more copies in flight)
     static constexpr int A_BUF = 2 * A_PART;                 // hi + lo
     static constexpr int OFF_A = 0;
     static constexpr int OFF_B = ((NA * A_BUF + 1023) / 1024) * 1024;
-    static constexpr int OFF_BAR = OFF_B + 2 * B_STAGE;
+    static constexpr int OFF_BAR = OFF_B + NSTAGE * B_STAGE;
     static constexpr int TOTAL = OFF_BAR + 256;
     static constexpr int TM_BUF = 256;                       // TMEM columns per accumulator buffer
     static_assert(KTOT % KC == 0 && NTOT % BN == 0 && BN % 16 == 0, "tile shapes");
@@ -79,18 +82,21 @@ __device__ __forceinline__ bool tile_rows(const FitTcArgs &p, int tile, int &a, 
 //   3: g = v4 + acc; out0 = g; out1 = g (1 - aux0^2)             (gh2, gz2;  aux0 = t2)
 //   4: g = aux0 + acc; out0 = g (1 - aux1^2)                     (gz1;  aux0 = gh2, aux1 = h1)
 //   5: out0 = acc                                                (gD)
+//   6: gD is consumed in registers: out0[row][c][m] = gA[c][m] = sum_a gD[m][a] A[c][a] + [m < 16] sum_m' gD[m'][m] A[c][m']
+//      (aux0 = A [rows][4][100]); the gD tensor never reaches memory
 template <int MODE, int KTOT, int NTOT, bool APPROX>
-__global__ void __launch_bounds__(NTHREADS, 1) k_fit_tc(FitTcArgs p) {
+__global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
+    constexpr int NEPI = nepi(MODE);
     using C = Cfg<KTOT, NTOT>;
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ uint32_t tmem_base_s;
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);       // warp-uniform role index
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem + C::OFF_BAR);
-    uint64_t *b_full = bars, *b_empty = bars + 2, *a_full = bars + 4, *a_empty = bars + 4 + C::NA;
-    uint64_t *acc_full = bars + 4 + 2 * C::NA, *acc_empty = acc_full + 2;
+    uint64_t *b_full = bars, *b_empty = bars + C::NSTAGE, *a_full = bars + 2 * C::NSTAGE, *a_empty = a_full + C::NA;
+    uint64_t *acc_full = a_empty + C::NA, *acc_empty = acc_full + 2;
     if (tid == 0) {
-        for (int k = 0; k < 2; ++k) { tc::mbar_init(&b_full[k], 1); tc::mbar_init(&b_empty[k], 1); }
+        for (int k = 0; k < C::NSTAGE; ++k) { tc::mbar_init(&b_full[k], 1); tc::mbar_init(&b_empty[k], 1); }
         for (int k = 0; k < C::NA; ++k) { tc::mbar_init(&a_full[k], NPROD / 32); tc::mbar_init(&a_empty[k], 1); }
         for (int k = 0; k < 2; ++k) { tc::mbar_init(&acc_full[k], 1); tc::mbar_init(&acc_empty[k], NEPI / 32); }
         asm volatile("fence.mbarrier_init.release.cluster;");
@@ -117,8 +123,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_fit_tc(FitTcArgs p) {
                 const __half *Bw = p.Bimg + a * p.b_type_stride;
                 for (int nt = 0; nt < C::NTILES; ++nt)
                     for (int kc = 0; kc < C::NKC; ++kc, ++step) {
-                        const int st = step & 1;
-                        tc::mbar_wait(&b_empty[st], ((step >> 1) & 1) ^ 1);
+                        const int st = step % C::NSTAGE;
+                        tc::mbar_wait(&b_empty[st], ((step / C::NSTAGE) & 1) ^ 1);
                         mbar_expect_tx(&b_full[st], C::B_STAGE);
                         bulk_g2s(sbase + C::OFF_B + st * C::B_STAGE, Bw + ((long)nt * C::NKC + kc) * (KC * C::BN), C::B_STAGE, &b_full[st]);
                     }
@@ -135,11 +141,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_fit_tc(FitTcArgs p) {
                     tc::mbar_wait(&acc_empty[buf], ((accn >> 1) & 1) ^ 1);
                     tc::fence_after();
                     for (int kc = 0; kc < C::NKC; ++kc, ++step) {
-                        const int st = step & 1;
+                        const int st = step % C::NSTAGE;
                         int ab;
                         if (C::RESIDENT) { ab = kc; tc::mbar_wait(&a_full[ab], it & 1); }
                         else { ab = astep & 1; tc::mbar_wait(&a_full[ab], (astep >> 1) & 1); }
-                        tc::mbar_wait(&b_full[st], (step >> 1) & 1);
+                        tc::mbar_wait(&b_full[st], (step / C::NSTAGE) & 1);
                         tc::fence_after();
                         const uint64_t da = tc::desc(sbase + C::OFF_A + ab * C::A_BUF, A_SUB_STRIDE, 128);
                         const uint64_t db = tc::desc(sbase + C::OFF_B + st * C::B_STAGE, C::BN * 16, 128);
@@ -205,6 +211,69 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_fit_tc(FitTcArgs p) {
             const bool ok = row0 + r < rend;
             const float *bias = p.bias ? p.bias + a * 240 : nullptr;
             const float *v4 = p.v4 ? p.v4 + a * 240 : nullptr;
+            if (MODE == 6) {
+                // thread (row, ch): components c = 2 ch, 2 ch + 1.  Per 16 accumulator columns = gD[m][0..16) of one m.
+                const int ch = ((warp - 2 - NPROD / 32) >> 2) & 1;
+                const float *Arow = p.aux0 + (long)(ok ? row0 + r : row0) * 400 + 2 * ch * 100;
+                float *Grow = p.out0 + (long)(row0 + r) * 400 + 2 * ch * 100;
+                float a16[2][16], acc2[2][16];
+#pragma unroll
+                for (int c = 0; c < 2; ++c)
+#pragma unroll
+                    for (int k4 = 0; k4 < 4; ++k4) {
+                        const float4 v = __ldg(reinterpret_cast<const float4 *>(Arow + c * 100) + k4);
+                        a16[c][4 * k4] = v.x; a16[c][4 * k4 + 1] = v.y; a16[c][4 * k4 + 2] = v.z; a16[c][4 * k4 + 3] = v.w;
+                        acc2[c][4 * k4] = acc2[c][4 * k4 + 1] = acc2[c][4 * k4 + 2] = acc2[c][4 * k4 + 3] = 0.f;
+                    }
+                float4 am0 = make_float4(0.f, 0.f, 0.f, 0.f), am1 = am0, go0 = am0, go1 = am0;
+                for (int nt = 0; nt < C::NTILES; ++nt, ++accn) {
+                    const int buf = accn & 1;
+                    tc::mbar_wait(&acc_full[buf], (accn >> 1) & 1);
+                    tc::fence_after();
+#pragma unroll
+                    for (int mm = 0; mm < C::BN / 16; ++mm) {
+                        const int m = nt * (C::BN / 16) + mm;            // BN / 16 = 10: the unrolled mm gives m & 3 statically per nt parity
+                        uint32_t v[16];
+                        tc::ld16(tm_lane + buf * C::TM_BUF + 16 * mm, v);
+                        if ((m & 3) == 0) {
+                            am0 = __ldg(reinterpret_cast<const float4 *>(Arow + m));
+                            am1 = __ldg(reinterpret_cast<const float4 *>(Arow + 100 + m));
+                        }
+                        tc::wait_ld();
+                        const float a0 = (m & 3) == 0 ? am0.x : (m & 3) == 1 ? am0.y : (m & 3) == 2 ? am0.z : am0.w;
+                        const float a1 = (m & 3) == 0 ? am1.x : (m & 3) == 1 ? am1.y : (m & 3) == 2 ? am1.z : am1.w;
+                        float g0 = 0.f, g1 = 0.f;
+#pragma unroll
+                        for (int ax = 0; ax < 16; ++ax) {
+                            const float gd = __uint_as_float(v[ax]);
+                            g0 = fmaf(gd, a16[0][ax], g0);
+                            g1 = fmaf(gd, a16[1][ax], g1);
+                            acc2[0][ax] = fmaf(gd, a0, acc2[0][ax]);
+                            acc2[1][ax] = fmaf(gd, a1, acc2[1][ax]);
+                        }
+                        if ((m & 3) == 0) { go0.x = g0; go1.x = g1; }
+                        else if ((m & 3) == 1) { go0.y = g0; go1.y = g1; }
+                        else if ((m & 3) == 2) { go0.z = g0; go1.z = g1; }
+                        else {
+                            go0.w = g0; go1.w = g1;
+                            if (ok) {
+                                *reinterpret_cast<float4 *>(Grow + m - 3) = go0;
+                                *reinterpret_cast<float4 *>(Grow + 100 + m - 3) = go1;
+                            }
+                        }
+                    }
+                    tc::fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&acc_empty[buf]);
+                }
+                if (ok) {
+#pragma unroll
+                    for (int c = 0; c < 2; ++c)
+#pragma unroll
+                        for (int ax = 0; ax < 16; ++ax) Grow[c * 100 + ax] += acc2[c][ax];
+                }
+                continue;
+            }
             for (int nt = 0; nt < C::NTILES; ++nt, ++accn) {
                 const int buf = accn & 1;
                 tc::mbar_wait(&acc_full[buf], (accn >> 1) & 1);
@@ -276,7 +345,7 @@ void launch(const FitTcArgs &p, int grid, cudaStream_t st) {
     using C = Cfg<KTOT, NTOT>;
     static bool attr = false;
     if (!attr) { cudaFuncSetAttribute(k_fit_tc<MODE, KTOT, NTOT, APPROX>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::TOTAL); attr = true; }
-    k_fit_tc<MODE, KTOT, NTOT, APPROX><<<grid, NTHREADS, C::TOTAL, st>>>(p);
+    k_fit_tc<MODE, KTOT, NTOT, APPROX><<<grid, nthreads(MODE), C::TOTAL, st>>>(p);
 }
 
 }  // namespace
@@ -316,7 +385,7 @@ cudaError_t fit_tc_gemm(int mode, bool apx, const dp_model *m, const Grid3 &g, c
                         int ldo, cudaStream_t st) {
     FitTcArgs p{};
     p.T = m->T; p.ncell = g.ncell; p.bin_start = bin_start; p.A = A; p.lda = lda;
-    p.Bimg = (const __half *)m->fit_tc_img_dev + FIT_TC_OFF[mode]; p.b_type_stride = (long)FIT_TC_OFF[6];
+    p.Bimg = (const __half *)m->fit_tc_img_dev + FIT_TC_OFF[mode > 5 ? 5 : mode]; p.b_type_stride = (long)FIT_TC_OFF[6];
     p.bias = bias; p.v4 = v4; p.aux0 = aux0; p.aux1 = aux1; p.out0 = out0; p.out1 = out1; p.ldo = ldo;
     const int grid = m->num_sms;
     switch (mode) {
@@ -325,7 +394,8 @@ cudaError_t fit_tc_gemm(int mode, bool apx, const dp_model *m, const Grid3 &g, c
         case 2: launch<2, 240, 240, false>(p, grid, st); break;
         case 3: launch<3, 240, 240, false>(p, grid, st); break;
         case 4: launch<4, 240, 240, false>(p, grid, st); break;
-        default: launch<5, 240, 1600, false>(p, grid, st); break;
+        case 5: launch<5, 240, 1600, false>(p, grid, st); break;
+        default: launch<6, 240, 1600, false>(p, grid, st); break;
     }
     return cudaGetLastError();
 }
