@@ -83,6 +83,7 @@ struct WsLayout {
     size_t perm;        // int[N]  sorted -> user
     size_t inv;         // int[N]  user -> sorted
     size_t xs;          // double[N][3] wrapped coords, sorted order
+    size_t xsf;         // float4[N] the same, rounded to fp32 (conservative pre-filter of the neighbour search)
     size_t xw;          // double[N][3] wrapped coords, user order
     size_t nlist;       // int[N][Nm] sorted-space indices
     size_t nreal;       // int[N][T]
@@ -106,6 +107,7 @@ struct Grid3 {
     double L[3];
     double inv_cw[3];   // nc / L
     int ncell;
+    int reach;          // neighbour cells searched per direction: 1 (cell edge >= rc) or 2 (cell edge >= rc/2)
 };
 
 // launchers (each returns cudaGetLastError())

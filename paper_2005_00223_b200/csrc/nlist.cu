@@ -3,6 +3,7 @@
 // 64-bit key per element (binary restatement, reading Q11).  Bit-exact against the
 // oracle: the arithmetic that decides list membership and order uses explicit round-to-nearest intrinsics so
 // that nvcc cannot contract it differently from the reading N2 of DESIGN.md.
+#include <cstdlib>
 #include "dp_internal.h"
 
 namespace {
@@ -97,7 +98,7 @@ __global__ void k_scatter(long N, const int *__restrict__ atom_bin, const int *_
 // order every bin by user index (makes the internal order, hence every later summation order, reproducible)
 __global__ void k_bin_sort(long N, const int *__restrict__ atom_bin, const int *__restrict__ bin_start,
                            const int *__restrict__ tmp_order, const double *__restrict__ xw, int *__restrict__ perm,
-                           int *__restrict__ inv, double *__restrict__ xs) {
+                           int *__restrict__ inv, double *__restrict__ xs, float4 *__restrict__ xsf) {
     long s = blockIdx.x * (long)blockDim.x + threadIdx.x;
     if (s >= N) return;
     int u = tmp_order[s];
@@ -111,6 +112,7 @@ __global__ void k_bin_sort(long N, const int *__restrict__ atom_bin, const int *
     xs[3 * (long)dst + 0] = xw[3 * (long)u + 0];
     xs[3 * (long)dst + 1] = xw[3 * (long)u + 1];
     xs[3 * (long)dst + 2] = xw[3 * (long)u + 2];
+    xsf[dst] = make_float4((float)xw[3 * (long)u + 0], (float)xw[3 * (long)u + 1], (float)xw[3 * (long)u + 2], 0.f);
 }
 
 __device__ __forceinline__ double min_image(double t, double L, double halfL) {
@@ -133,9 +135,10 @@ k_nlist(long N, int T, Grid3 g, double rc2, int cap, const int *__restrict__ bin
     const double xi = xs[3 * i], yi = xs[3 * i + 1], zi = xs[3 * i + 2];
     const int cx = cell_of(xi, g.inv_cw[0], g.nc[0]), cy = cell_of(yi, g.inv_cw[1], g.nc[1]),
               cz = cell_of(zi, g.inv_cw[2], g.nc[2]);
-    const int lo0 = g.nc[0] >= 3 ? -1 : 0, hi0 = g.nc[0] >= 2 ? 1 : 0;
-    const int lo1 = g.nc[1] >= 3 ? -1 : 0, hi1 = g.nc[1] >= 2 ? 1 : 0;
-    const int lo2 = g.nc[2] >= 3 ? -1 : 0, hi2 = g.nc[2] >= 2 ? 1 : 0;
+    const int R_ = g.reach;       // reach 2 is only chosen for grids with >= 5 cells per axis
+    const int lo0 = R_ == 2 ? -2 : (g.nc[0] >= 3 ? -1 : 0), hi0 = R_ == 2 ? 2 : (g.nc[0] >= 2 ? 1 : 0);
+    const int lo1 = R_ == 2 ? -2 : (g.nc[1] >= 3 ? -1 : 0), hi1 = R_ == 2 ? 2 : (g.nc[1] >= 2 ? 1 : 0);
+    const int lo2 = R_ == 2 ? -2 : (g.nc[2] >= 3 ? -1 : 0), hi2 = R_ == 2 ? 2 : (g.nc[2] >= 2 ? 1 : 0);
     const double hx = 0.5 * g.L[0], hy = 0.5 * g.L[1], hz = 0.5 * g.L[2];
     bool truncated = false;
     int off = 0;
@@ -203,6 +206,186 @@ k_nlist(long N, int T, Grid3 g, double rc2, int cap, const int *__restrict__ bin
     if (truncated && lane == 0) atomicAdd(&status[1], 1);
 }
 
+// ---- second-generation list kernel ----------------------------------------------------------------------------------
+// Bitonic sort of 32 R keys held R per lane (element index = lane * R + r): strides below R are register exchanges,
+// larger strides are warp shuffles.  Ascending.
+template <int R>
+__device__ __forceinline__ void warp_sort_regs(unsigned long long (&key)[R], int lane) {
+#pragma unroll
+    for (int k = 2; k <= 32 * R; k <<= 1) {
+#pragma unroll
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            if (j < R) {
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const int q = r ^ j;
+                    if (q > r) {
+                        const bool asc = (((lane * R + r) & k) == 0);
+                        const unsigned long long a = key[r], c = key[q];
+                        const bool sw = (a > c) == asc;
+                        key[r] = sw ? c : a;
+                        key[q] = sw ? a : c;
+                    }
+                }
+            } else {
+                const int jl = j / R;
+                const bool lower = (lane & jl) == 0;
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const bool asc = (((lane * R + r) & k) == 0);
+                    const unsigned long long a = key[r];
+                    const unsigned long long o = __shfl_xor_sync(0xffffffffu, a, jl);
+                    const bool take_min = asc == lower;
+                    key[r] = take_min ? (a < o ? a : o) : (a > o ? a : o);
+                }
+            }
+        }
+    }
+}
+
+template <int R>
+__device__ __forceinline__ void sort_and_emit(const unsigned long long *keys, int n, int lane, int selb, const int *__restrict__ inv,
+                                              int *__restrict__ out) {
+    unsigned long long key[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) { const int idx = lane * R + r; key[r] = idx < n ? keys[idx] : ~0ull; }
+    warp_sort_regs<R>(key, lane);
+    const int nkeep = n < selb ? n : selb;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int rank = lane * R + r;
+        if (rank < selb) out[rank] = rank < nkeep ? inv[(int)(key[r] & 0xFFFFFFull)] : -1;
+    }
+    for (int k = 32 * R + lane; k < selb; k += 32) out[k] = -1;
+}
+
+// One warp per (sorted) atom.  Pass 1: fp32 distances on the fp32 copy of the coordinates select candidates conservatively
+// (margin covers the rounding of the copy), ballot-compacted into shared memory.  Pass 2: the exact test and the 64-bit key
+// (canonical fp64 arithmetic of DESIGN.md reading N2) on the few survivors only.  Sort in registers.
+__global__ void __launch_bounds__(128, 8)
+k_nlist2(long N, int T, Grid3 g, double rc2, float rc2f_margin, int cap, const int *__restrict__ bin_start,
+         const double *__restrict__ xs, const float4 *__restrict__ xsf, const int *__restrict__ perm,
+         const int *__restrict__ inv, int Nm, int4 sel4, int *__restrict__ nlist, int *__restrict__ nreal,
+         int *__restrict__ rowcnt, int *__restrict__ status) {
+    extern __shared__ unsigned long long keys_all[];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const long i = blockIdx.x * 4L + wid;
+    if (i >= N) return;
+    unsigned long long *keys = keys_all + (size_t)wid * cap;
+    const int sel[4] = {sel4.x, sel4.y, sel4.z, sel4.w};
+    const double xi = xs[3 * i], yi = xs[3 * i + 1], zi = xs[3 * i + 2];
+    const float4 pf = xsf[i];
+    const int cx = cell_of(xi, g.inv_cw[0], g.nc[0]), cy = cell_of(yi, g.inv_cw[1], g.nc[1]),
+              cz = cell_of(zi, g.inv_cw[2], g.nc[2]);
+    const int R_ = g.reach;       // reach 2 is only chosen for grids with >= 5 cells per axis
+    const int lo0 = R_ == 2 ? -2 : (g.nc[0] >= 3 ? -1 : 0), hi0 = R_ == 2 ? 2 : (g.nc[0] >= 2 ? 1 : 0);
+    const int lo1 = R_ == 2 ? -2 : (g.nc[1] >= 3 ? -1 : 0), hi1 = R_ == 2 ? 2 : (g.nc[1] >= 2 ? 1 : 0);
+    const int lo2 = R_ == 2 ? -2 : (g.nc[2] >= 3 ? -1 : 0), hi2 = R_ == 2 ? 2 : (g.nc[2] >= 2 ? 1 : 0);
+    const double hx = 0.5 * g.L[0], hy = 0.5 * g.L[1], hz = 0.5 * g.L[2];
+    const float Lx = (float)g.L[0], Ly = (float)g.L[1], Lz = (float)g.L[2];
+    const float hxf = 0.5f * Lx, hyf = 0.5f * Ly, hzf = 0.5f * Lz;
+    bool truncated = false;
+    int off = 0;
+    for (int b = 0; b < T; ++b) {
+        // ---- pass 1: conservative fp32 filter ----
+        int n1 = 0;
+        for (int ox = lo0; ox <= hi0; ++ox) {
+            int ax = cx + ox; ax += ax < 0 ? g.nc[0] : 0; ax -= ax >= g.nc[0] ? g.nc[0] : 0;
+            for (int oy = lo1; oy <= hi1; ++oy) {
+                int ay = cy + oy; ay += ay < 0 ? g.nc[1] : 0; ay -= ay >= g.nc[1] ? g.nc[1] : 0;
+                // the z cells of one (x, y) column are consecutive bins: one run unless the column wraps
+                const int colb = b * g.ncell + (ax * g.nc[1] + ay) * g.nc[2];
+                const bool one_run = cz + lo2 >= 0 && cz + hi2 < g.nc[2];
+                for (int oz = lo2; oz <= hi2; ++oz) {
+                    int s0, s1;
+                    if (one_run) {
+                        s0 = bin_start[colb + cz + lo2]; s1 = bin_start[colb + cz + hi2 + 1];
+                        oz = hi2;
+                    } else {
+                        int az = cz + oz; az += az < 0 ? g.nc[2] : 0; az -= az >= g.nc[2] ? g.nc[2] : 0;
+                        s0 = bin_start[colb + az]; s1 = bin_start[colb + az + 1];
+                    }
+                    for (int base = s0; base < s1; base += 32) {
+                        const int s = base + lane;
+                        bool ok = false;
+                        if (s < s1 && s != i) {
+                            const float4 q = __ldg(&xsf[s]);
+                            float dx = q.x - pf.x, dy = q.y - pf.y, dz = q.z - pf.z;
+                            dx -= dx > hxf ? Lx : 0.f; dx += dx < -hxf ? Lx : 0.f;
+                            dy -= dy > hyf ? Ly : 0.f; dy += dy < -hyf ? Ly : 0.f;
+                            dz -= dz > hzf ? Lz : 0.f; dz += dz < -hzf ? Lz : 0.f;
+                            ok = fmaf(dz, dz, fmaf(dy, dy, dx * dx)) < rc2f_margin;
+                        }
+                        const unsigned mask = __ballot_sync(0xffffffffu, ok);
+                        const int pos = n1 + __popc(mask & ((1u << lane) - 1u));
+                        if (ok && pos < cap) keys[pos] = (unsigned long long)s;
+                        n1 += __popc(mask);
+                    }
+                }
+            }
+        }
+        if (n1 > cap) { if (lane == 0) atomicOr(&status[0], 2); n1 = cap; }
+        __syncwarp();
+        // ---- pass 2: exact test + key on the survivors, compacted in place ----
+        int n = 0;
+        for (int base = 0; base < n1; base += 32) {
+            const int k = base + lane;
+            bool ok = false;
+            unsigned long long key = 0;
+            if (k < n1) {
+                const int s = (int)keys[k];
+                double dx = min_image(__dsub_rn(xs[3 * (long)s], xi), g.L[0], hx);
+                double dy = min_image(__dsub_rn(xs[3 * (long)s + 1], yi), g.L[1], hy);
+                double dz = min_image(__dsub_rn(xs[3 * (long)s + 2], zi), g.L[2], hz);
+                double r2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
+                if (r2 < rc2) {
+                    ok = true;
+                    key = (__double2ull_rd(r2 * 536870912.0) << 24) | (unsigned long long)perm[s];
+                }
+            }
+            const unsigned mask = __ballot_sync(0xffffffffu, ok);      // every lane has read its entry: in-place write is safe
+            if (ok) keys[n + __popc(mask & ((1u << lane) - 1u))] = key;
+            n += __popc(mask);
+        }
+        __syncwarp();
+        int *out = nlist + i * Nm + off;
+        if (n <= 32) sort_and_emit<1>(keys, n, lane, sel[b], inv, out);
+        else if (n <= 64) sort_and_emit<2>(keys, n, lane, sel[b], inv, out);
+        else if (n <= 128) sort_and_emit<4>(keys, n, lane, sel[b], inv, out);
+        else if (n <= 256) sort_and_emit<8>(keys, n, lane, sel[b], inv, out);
+        else {
+            int P = 512;
+            while (P < n) P <<= 1;
+            for (int k = n + lane; k < P; k += 32) keys[k] = ~0ull;
+            __syncwarp();
+            for (int k = 2; k <= P; k <<= 1) {
+                for (int j = k >> 1; j > 0; j >>= 1) {
+                    for (int idx = lane; idx < P; idx += 32) {
+                        const int ixj = idx ^ j;
+                        if (ixj > idx) {
+                            const unsigned long long a = keys[idx], c = keys[ixj];
+                            const bool asc = (idx & k) == 0;
+                            if ((a > c) == asc) { keys[idx] = c; keys[ixj] = a; }
+                        }
+                    }
+                    __syncwarp();
+                }
+            }
+            const int nkeep = n < sel[b] ? n : sel[b];
+            for (int k = lane; k < sel[b]; k += 32) out[k] = k < nkeep ? inv[(int)(keys[k] & 0xFFFFFFull)] : -1;
+        }
+        const int nkeep = n < sel[b] ? n : sel[b];
+        if (lane == 0) {
+            nreal[i * T + b] = nkeep;
+            if (rowcnt) rowcnt[(long)b * N + i] = nkeep + (nkeep < sel[b] ? 1 : 0);
+        }
+        truncated |= n > sel[b];
+        off += sel[b];
+        __syncwarp();
+    }
+    if (truncated && lane == 0) atomicAdd(&status[1], 1);
+}
+
 __global__ void k_get_nlist(long N, int Nm, const int *__restrict__ nlist, const int *__restrict__ perm,
                             int *__restrict__ out) {
     long t = blockIdx.x * (long)blockDim.x + threadIdx.x;
@@ -229,7 +412,7 @@ cudaError_t launch_build_cells(const dp_model *m, long N, const double *coords, 
     k_scatter<<<nb, 256, 0, st>>>(N, (int *)(ws + L.atom_bin), start, cursor, (int *)(ws + L.tmp_order));
     k_bin_sort<<<nb, 256, 0, st>>>(N, (int *)(ws + L.atom_bin), start, (int *)(ws + L.tmp_order),
                                    (double *)(ws + L.xw), (int *)(ws + L.perm), (int *)(ws + L.inv),
-                                   (double *)(ws + L.xs));
+                                   (double *)(ws + L.xs), (float4 *)(ws + L.xsf));
     return cudaGetLastError();
 }
 
@@ -242,6 +425,20 @@ cudaError_t launch_nlist(const dp_model *m, long N, const Grid3 &g, char *ws, co
         attr_set = true;
     }
     int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
+    // fp32 pre-filter margin: the fp32 copy is off by <= ulp(L)/2 per coordinate, the fp32 arithmetic by a few ulp of rc^2
+    double Lmax = g.L[0] > g.L[1] ? g.L[0] : g.L[1];
+    Lmax = Lmax > g.L[2] ? Lmax : g.L[2];
+    const float rc2f = (float)(m->rc * m->rc * (1.0 + 1e-5) + 8.0 * m->rc * Lmax * 1.2e-7 + 1e-6);
+    static const bool legacy = std::getenv("DP_NLIST_V1") != nullptr;
+    if (!legacy) {
+        static bool attr2 = false;
+        if (!attr2) { cudaFuncSetAttribute(k_nlist2, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 4096 * 8); attr2 = true; }
+        k_nlist2<<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, m->T, g, m->rc * m->rc, rc2f, cap, (int *)(ws + L.bin_start),
+                                                            (double *)(ws + L.xs), (const float4 *)(ws + L.xsf), (int *)(ws + L.perm),
+                                                            (int *)(ws + L.inv), m->Nm, sel4, (int *)(ws + L.nlist),
+                                                            (int *)(ws + L.nreal), m->prec == DP_FP64 ? nullptr : (int *)(ws + L.rowcnt),
+                                                            (int *)(ws + L.status));
+    } else
     k_nlist<<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, m->T, g, m->rc * m->rc, cap, (int *)(ws + L.bin_start),
                                                        (double *)(ws + L.xs), (int *)(ws + L.perm),
                                                        (int *)(ws + L.inv), m->Nm, sel4, (int *)(ws + L.nlist),
