@@ -314,14 +314,14 @@ cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, 
     const unsigned gy = (unsigned)((N + BM - 1) / BM);
     const unsigned nb8 = (unsigned)((N + 7) / 8);
 
-    k_descr_f<<<nb8, 256, 0, st>>>(N, Amat, D);
+    if (!m->use_fit_tc) k_descr_f<<<nb8, 256, 0, st>>>(N, Amat, D);     // the tcgen05 first-layer GEMM forms D in its operand producer
     FitArgsF p{};
     p.ncell = g.ncell; p.bin_start = bin_start; p.v4 = v4; p.v4_type_stride = F; p.bias_type_stride = F;
     p.K = ND; p.N = F; p.A = D; p.lda = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.ldb = F; p.bias = c1;
     p.out0 = h1; p.ldo = F;
     const dim3 g240(F / BN, gy, T), g1600(ND / BN, gy, T);
     if (m->use_fit_tc) {      // tcgen05 GEMMs (fit_tc.cu), same products, buffers and epilogues
-        fit_tc_gemm(0, apx, m, g, bin_start, D, ND, c1, nullptr, nullptr, nullptr, h1, nullptr, F, st);
+        fit_tc_gemm(0, apx, m, g, bin_start, Amat, 4 * M2E, c1, nullptr, nullptr, nullptr, h1, nullptr, F, st);
         fit_tc_gemm(1, apx, m, g, bin_start, h1, F, c2, nullptr, h1, nullptr, t2, h2, F, st);
         fit_tc_gemm(2, false, m, g, bin_start, h2, F, c3, v4, h2, nullptr, gz3, h3, F, st);
         k_energy_f<<<nb8, 256, 0, st>>>(N, T, g.ncell, bin_start, h3, v4, c4, m->ebias_dev, (double *)(ws + L.eatom));

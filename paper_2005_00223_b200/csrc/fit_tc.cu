@@ -174,14 +174,48 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
         for (int tile = blockIdx.x; tile < ntiles_total; tile += gridDim.x, ++it) {
             int a, row0, rend;
             tile_rows(p, tile, a, row0, rend);
+            // MODE 0: the A operand is the descriptor D[m*16 + a] = sum_c A[c][m] A[c][a] (S5), formed here from the
+            // 4 x 100 matrix A_i (p.A, lda = 400): D never reaches memory.  Thread = (row, half of the axis range a).
+            constexpr bool DESCR = MODE == 0;
+            const int dr = pt & (BM - 1), dah = pt >> 7;
+            const bool drow_ok = row0 + dr < rend;
+            const float *Ai = p.A + (long)(drow_ok ? row0 + dr : row0) * 400;
+            float ax8[4][8];
+            if (DESCR) {
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const float4 u0 = __ldg(reinterpret_cast<const float4 *>(Ai + c * 100 + 8 * dah));
+                    const float4 u1 = __ldg(reinterpret_cast<const float4 *>(Ai + c * 100 + 8 * dah + 4));
+                    ax8[c][0] = u0.x; ax8[c][1] = u0.y; ax8[c][2] = u0.z; ax8[c][3] = u0.w;
+                    ax8[c][4] = u1.x; ax8[c][5] = u1.y; ax8[c][6] = u1.z; ax8[c][7] = u1.w;
+                }
+            }
             for (int kc = 0; kc < C::NKC; ++kc, ++astep) {
                 int ab;
                 if (C::RESIDENT) { ab = kc; tc::mbar_wait(&a_empty[ab], (it & 1) ^ 1); }
                 else { ab = astep & 1; tc::mbar_wait(&a_empty[ab], ((astep >> 1) & 1) ^ 1); }
                 uint8_t *img = smem + C::OFF_A + ab * C::A_BUF;
+                if (DESCR) {
+                    // chunk kc covers m = 5 kc .. 5 kc + 4 (KC / 16 = 5 values of m, 16 axis columns each)
+#pragma unroll
+                    for (int mm = 0; mm < KC / 16; ++mm) {
+                        const int m = kc * (KC / 16) + mm;
+                        const float a0 = __ldg(Ai + m), a1 = __ldg(Ai + 100 + m), a2 = __ldg(Ai + 200 + m), a3 = __ldg(Ai + 300 + m);
+                        float d[8];
+#pragma unroll
+                        for (int j = 0; j < 8; ++j)
+                            d[j] = drow_ok ? fmaf(a3, ax8[3][j], fmaf(a2, ax8[2][j], fmaf(a1, ax8[1][j], a0 * ax8[0][j]))) : 0.f;
+                        uint4 hi, lo;
+                        tc::split_h2(d[0], d[1], hi.x, lo.x); tc::split_h2(d[2], d[3], hi.y, lo.y);
+                        tc::split_h2(d[4], d[5], hi.z, lo.z); tc::split_h2(d[6], d[7], hi.w, lo.w);
+                        const int sub = 2 * mm + dah;
+                        *reinterpret_cast<uint4 *>(img + sub * A_SUB_STRIDE + dr * 16) = hi;
+                        *reinterpret_cast<uint4 *>(img + A_PART + sub * A_SUB_STRIDE + dr * 16) = lo;
+                    }
+                }
                 // item = (row, sub-chunk): 8 consecutive fp32 -> one 16-byte hi chunk and one lo chunk
 #pragma unroll
-                for (int j = 0; j < BM * SUB / NPROD; ++j) {
+                for (int j = 0; j < (DESCR ? 0 : BM * SUB / NPROD); ++j) {
                     const int idx = pt + j * NPROD;
                     const int r = idx / SUB, sub = idx % SUB;
                     float4 x0 = make_float4(0.f, 0.f, 0.f, 0.f), x1 = x0;
