@@ -19,10 +19,11 @@ constexpr int KC = 80;                    // K chunk: 5 k-steps of 16
 constexpr int SUB = KC / 8;               // 16-byte sub-chunks per K chunk
 constexpr int A_SUB_STRIDE = BM * 16 + 16;   // bytes between sub-chunks of the A image (+16: conflict-free producer stores)
 constexpr int A_PART = SUB * A_SUB_STRIDE;   // one part (hi or lo) of one K chunk
-constexpr int NPROD = 256;
+// producer threads (MODE 6 produces its resident A tile once per row tile: fewer producers leave registers to its epilogue)
+__host__ __device__ constexpr int nprod(int mode) { return mode == 6 ? 128 : 256; }
 // epilogue threads: one per row; MODE 6 (gA in the epilogue) uses two per row, each owning two of the four components c
 __host__ __device__ constexpr int nepi(int mode) { return mode == 6 ? 256 : 128; }
-__host__ __device__ constexpr int nthreads(int mode) { return 64 + NPROD + nepi(mode); }
+__host__ __device__ constexpr int nthreads(int mode) { return 64 + nprod(mode) + nepi(mode); }
 
 template <int KTOT, int NTOT>
 struct Cfg {
@@ -86,7 +87,7 @@ __device__ __forceinline__ bool tile_rows(const FitTcArgs &p, int tile, int &a, 
 //      (aux0 = A [rows][4][100]); the gD tensor never reaches memory
 template <int MODE, int KTOT, int NTOT, bool APPROX>
 __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
-    constexpr int NEPI = nepi(MODE);
+    constexpr int NEPI = nepi(MODE), NPROD = nprod(MODE);
     using C = Cfg<KTOT, NTOT>;
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ uint32_t tmem_base_s;
