@@ -21,8 +21,9 @@ constexpr int A_SUB_STRIDE = BM * 16 + 16;   // bytes between sub-chunks of the 
 constexpr int A_PART = SUB * A_SUB_STRIDE;   // one part (hi or lo) of one K chunk
 // producer threads (MODE 6 produces its resident A tile once per row tile: fewer producers leave registers to its epilogue)
 __host__ __device__ constexpr int nprod(int mode) { return mode == 6 ? 128 : 256; }
-// epilogue threads: one per row; MODE 6 (gA in the epilogue) uses two per row, each owning two of the four components c
-__host__ __device__ constexpr int nepi(int mode) { return mode == 6 ? 256 : 128; }
+// epilogue threads: two per row.  MODE 6 (gA in the epilogue): each owns two of the four components c; other modes: each owns
+// every other group of 16 columns (the epilogues are bound by the latency of their global loads: twice the loads in flight)
+__host__ __device__ constexpr int nepi(int mode) { return 256; }
 __host__ __device__ constexpr int nthreads(int mode) { return 64 + nprod(mode) + nepi(mode); }
 
 template <int KTOT, int NTOT>
@@ -314,8 +315,22 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                 tc::mbar_wait(&acc_full[buf], (accn >> 1) & 1);
                 tc::fence_after();
                 const long o = (long)(row0 + r) * p.ldo + nt * C::BN;
+                const int half = ((warp - 2 - NPROD / 32) >> 2) & 1;
+                float4 a0c[4], a1c[4], a0n[4], a1n[4];
+                auto load_aux = [&](int c0, float4 (&a0)[4], float4 (&a1)[4]) {     // auxiliary operands of one 16-column group
+#pragma unroll
+                    for (int g4 = 0; g4 < 4; ++g4) {
+                        a0[g4] = make_float4(0.f, 0.f, 0.f, 0.f); a1[g4] = a0[g4];
+                        if (ok && c0 < C::BN) {
+                            if (MODE >= 1 && MODE <= 4) a0[g4] = __ldg(reinterpret_cast<const float4 *>(p.aux0 + o + c0 + 4 * g4));
+                            if (MODE == 4) a1[g4] = __ldg(reinterpret_cast<const float4 *>(p.aux1 + o + c0 + 4 * g4));
+                        }
+                    }
+                };
+                load_aux(16 * half, a0c, a1c);
 #pragma unroll 1
-                for (int c0 = 0; c0 < C::BN; c0 += 16) {
+                for (int c0 = 16 * half; c0 < C::BN; c0 += 32) {
+                    load_aux(c0 + 32, a0n, a1n);          // one group ahead
                     uint32_t v[16];
                     tc::ld16(tm_lane + buf * C::TM_BUF + c0, v);
                     tc::wait_ld();
@@ -333,7 +348,7 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                                 for (int k = 0; k < 4; ++k) r0[k] = APPROX ? tc::tanh_approx(x[k] + bb[k]) : tanhf(x[k] + bb[k]);
                             } else if (MODE == 1 || MODE == 2) {
                                 const float4 b = *reinterpret_cast<const float4 *>(bias + c);
-                                const float4 hh = *reinterpret_cast<const float4 *>(p.aux0 + o + c);
+                                const float4 hh = a0c[g4];
                                 const float bb[4] = {b.x, b.y, b.z, b.w}, hv[4] = {hh.x, hh.y, hh.z, hh.w};
                                 float vv[4] = {0.f, 0.f, 0.f, 0.f};
                                 if (MODE == 2) { const float4 w = *reinterpret_cast<const float4 *>(v4 + c); vv[0] = w.x; vv[1] = w.y; vv[2] = w.z; vv[3] = w.w; }
@@ -345,13 +360,13 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                                 }
                             } else if (MODE == 3) {
                                 const float4 w = *reinterpret_cast<const float4 *>(v4 + c);
-                                const float4 tt = *reinterpret_cast<const float4 *>(p.aux0 + o + c);
+                                const float4 tt = a0c[g4];
                                 const float vv[4] = {w.x, w.y, w.z, w.w}, tv[4] = {tt.x, tt.y, tt.z, tt.w};
 #pragma unroll
                                 for (int k = 0; k < 4; ++k) { r0[k] = vv[k] + x[k]; r1[k] = r0[k] * (1.f - tv[k] * tv[k]); }
                             } else if (MODE == 4) {
-                                const float4 gg = *reinterpret_cast<const float4 *>(p.aux0 + o + c);
-                                const float4 hh = *reinterpret_cast<const float4 *>(p.aux1 + o + c);
+                                const float4 gg = a0c[g4];
+                                const float4 hh = a1c[g4];
                                 const float gv[4] = {gg.x, gg.y, gg.z, gg.w}, hv[4] = {hh.x, hh.y, hh.z, hh.w};
 #pragma unroll
                                 for (int k = 0; k < 4; ++k) r0[k] = (gv[k] + x[k]) * (1.f - hv[k] * hv[k]);
@@ -363,6 +378,8 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                             if (MODE >= 1 && MODE <= 3) *reinterpret_cast<float4 *>(p.out1 + o + c) = make_float4(r1[0], r1[1], r1[2], r1[3]);
                         }
                     }
+#pragma unroll
+                    for (int g4 = 0; g4 < 4; ++g4) { a0c[g4] = a0n[g4]; a1c[g4] = a1n[g4]; }
                 }
                 tc::fence_before();
                 __syncwarp();
