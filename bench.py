@@ -29,8 +29,12 @@ FLOP_ROW_FWD = 12550 + 800          # embedding GEMMs forward + contraction forw
 FLOP_ROW_BWD = 12550 + 1600         # embedding GEMMs backward + contraction backward, per neighbour row
 FLOP_ATOM_FIT = 2036160             # fitting fwd + bwd + descriptor fwd/bwd, per atom
 FP64_OVER_BF16_NOMINAL = 45.0 / 2250.0
+# tensor-core flops the MIX-16 backward kernel actually executes per 128-row tile (M = 128, 2 flop per MAC):
+# layer 2 (hi+lo) 2*32*64, layer 3 2*96*112, dR 2*208*16, dT3 32*112, dT2+dz3 W3^T (32+112)*64, dT1+dz3 W3f (32+112)*32, dz2 W2^T 64*32
+EXEC_FLOP_ROW_BWD = 2 * (2 * 32 * 64 + 2 * 96 * 112 + 2 * 208 * 16 + 32 * 112 + 144 * 64 + 144 * 32 + 64 * 32)
+MUFU_TANH_PEAK = 16 * 148 * 1.965e9          # tanh.approx.f32 per second, measured
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, one ncu --set full capture per config (profiles/)
-TRAFFIC = {}   # guide's nominal dense ratio: B200 FP64 tensor 45 TF vs bf16 2250 TF
+TRAFFIC = {"c4_cu1048576": 8.045858e9 + 3.012969e9}   # k_embed_bwd_tc2, profiles/r01_c4_bwd_tc2_ncu.md
 
 
 def peaks():
@@ -134,7 +138,7 @@ def time_config(binding, torch, s, dev, steps, warmup, flush, profile=True):
         model.compute(coords, types, s.box, out=out)
     model.profile_enable(True)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
-    phases = np.zeros(5)
+    phases = np.zeros(6)
     torch.cuda.synchronize(dev)
     for k in range(steps):
         flush.fill_(k & 0xFF)                      # L2 flush, outside the timed events
@@ -252,11 +256,12 @@ def main():
         else:
             peak = pk["bf16_sus"]
             peak_src = f"{pk['src']}: dense bf16 sustained (fp16 has the same nominal rate)"
-            kname = "k_embed_bwd_mix"
+            kname = "k_embed_bwd_tc2" if s.precision == "mix16" else "k_embed_bwd_mix"
         dom_flops = real_rows * FLOP_ROW_BWD
-        ach = dom_flops / (phases[3] * 1e-3) / 1e12
+        ach = dom_flops / (phases[5] * 1e-3) / 1e12           # phases[5]: CUDA events around the backward kernel alone
         kern = {"nlist_ms": phases[0], "embed_fwd_ms": phases[1], "fit_ms": phases[2], "embed_bwd_ms": phases[3],
-                "finalize_ms": phases[4],
+                "finalize_ms": phases[4], "embed_bwd_kernel_ms": phases[5],
+                "tanh_per_s_bwd_kernel": rows_b * 175 / (phases[5] * 1e-3),
                 "embed_fwd_tflops": real_rows * FLOP_ROW_FWD / (phases[1] * 1e-3) / 1e12,
                 "fit_tflops": N * FLOP_ATOM_FIT / (phases[2] * 1e-3) / 1e12,
                 "embed_bwd_tflops": ach,
@@ -278,7 +283,11 @@ def main():
                              "unit": "TFLOP/s", "frac": ach / peak, "traffic": TRAFFIC.get(s.name),
                              "peak_source": peak_src,
                              "flops_per_launch": dom_flops,
-                             "note": "algorithmic backward flops (14,150 per real neighbour row); the in-kernel forward recompute is not credited"},
+                             "executed_tflops": (rows_b * EXEC_FLOP_ROW_BWD / (phases[5] * 1e-3) / 1e12) if s.precision == "mix16" else None,
+                             "mufu_tanh_frac": (rows_b * 175 / (phases[5] * 1e-3)) / MUFU_TANH_PEAK,
+                             "note": "algorithmic backward flops (14,150 per real neighbour row); the in-kernel forward recompute, "
+                                     "the hi/lo operand splitting and the K/N padding are executed (executed_tflops) but not credited; "
+                                     "mufu_tanh_frac = tanh issued by this kernel / measured MUFU.TANH peak (16 per clock per SM)"},
                 "kernels": kern}
         if args.all_configs and world == 1:
             summ = {}
