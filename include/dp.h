@@ -105,8 +105,9 @@ int dp_last_row_counts(dp_model *m, long *rows_forward, long *rows_backward);
 /* Optional per-phase device timing of dp_compute (CUDA events recorded on the caller's stream; off by default).
  * dp_profile_read synchronises the last compute and returns DP_NPHASES durations in milliseconds:
  * [0] cell binning + neighbour list (S1,S2), [1] embedding forward + contraction (S3-S5), [2] fitting net
- * forward + backward (S6), [3] embedding backward + ProdForce + ProdViral (S7-S9), [4] finalize. */
-#define DP_NPHASES 5
+ * forward + backward (S6), [3] embedding backward + ProdForce + ProdViral (S7-S9), [4] finalize,
+ * [5] the embedding-backward kernel alone (a part of [3]; equal to [3] where one kernel does all of S7-S9). */
+#define DP_NPHASES 6
 int dp_profile_enable(dp_model *m, int on);
 int dp_profile_read(dp_model *m, double *ms_host);
 

@@ -169,7 +169,7 @@ class DPModel:
 
     def profile_read(self):
         """Per-phase milliseconds of the last compute: nlist, embed_fwd, fit, embed_bwd, finalize."""
-        ms = np.zeros(5)
+        ms = np.zeros(6)
         rc = lib().dp_profile_read(self._h, _dptr(ms))
         if rc != 0:
             raise DPError(rc, "dp_profile_read")

@@ -440,7 +440,7 @@ void dp_destroy(dp_model *m) {
     void *ptrs[] = {m->type_map_dev, m->embed_frag_dev, m->embed_tc_dev, m->embed_tc2_dev, m->fit_tc_img_dev, m->avg_dev, m->std_dev, m->ebias_dev, m->fitV1_dev, m->fitV2_dev,
                     m->fitV3_dev, m->fitc1_dev, m->fitc2_dev, m->fitc3_dev, m->fitv4_dev, m->fitc4_dev};
     for (void *p : ptrs) if (p) cudaFree(p);
-    if (m->ev[0]) for (int k = 0; k <= DP_NPHASES; ++k) cudaEventDestroy(m->ev[k]);
+    if (m->ev[0]) for (int k = 0; k < DP_NEVENTS; ++k) cudaEventDestroy(m->ev[k]);
     delete m;
 }
 
@@ -449,7 +449,12 @@ size_t dp_workspace_bytes(const dp_model *m, long natoms) {
     return ws_layout(m, natoms).total;
 }
 
-int dp_launches_per_compute(const dp_model *m) { return m ? 17 : 0; }
+int dp_launches_per_compute(const dp_model *m) {
+    if (!m) return 0;
+    // MIX-16 tcgen05 path: 4 binning + list + T row scans + env rows + forward + 7 fitting + image fold + backward + force/virial + finalize
+    if (m->use_tc == 2 && m->use_tc_bwd && m->use_fit_tc) return 18 + m->T;
+    return 17;
+}
 
 int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *types_dev, const double *box_host,
                void *workspace_dev, size_t workspace_bytes, void *cuda_stream, double *energy_dev,
@@ -494,7 +499,7 @@ int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *ty
 int dp_profile_enable(dp_model *m, int on) {
     if (!m) return DP_EINVAL;
     if (on && !m->ev[0]) {
-        for (int k = 0; k <= DP_NPHASES; ++k)
+        for (int k = 0; k < DP_NEVENTS; ++k)
             if (cudaEventCreate(&m->ev[k]) != cudaSuccess) return DP_ECUDA;
     }
     m->profile = on ? 1 : 0;
@@ -503,11 +508,17 @@ int dp_profile_enable(dp_model *m, int on) {
 
 int dp_profile_read(dp_model *m, double *ms_host) {
     if (!m || !ms_host || !m->profile || !m->last_ws) return DP_EINVAL;
-    if (cudaEventSynchronize(m->ev[DP_NPHASES]) != cudaSuccess) return DP_ECUDA;
-    for (int k = 0; k < DP_NPHASES; ++k) {
+    if (cudaEventSynchronize(m->ev[5]) != cudaSuccess) return DP_ECUDA;
+    for (int k = 0; k < 5; ++k) {
         float ms = 0.f;
         if (cudaEventElapsedTime(&ms, m->ev[k], m->ev[k + 1]) != cudaSuccess) return DP_ECUDA;
         ms_host[k] = ms;
+    }
+    ms_host[5] = ms_host[3];
+    if (m->use_tc_bwd) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, m->ev[6], m->ev[7]) != cudaSuccess) return DP_ECUDA;
+        ms_host[5] = ms;
     }
     return DP_OK;
 }

@@ -6,6 +6,7 @@
 #include "../../include/dp.h"
 
 #define DP_MAX_TYPES 4
+#define DP_NEVENTS 8
 #define DP_WARPS_PER_CTA 8
 
 // ---------------------------------------------------------------- shapes fixed by this build (dp.h: widths (25,50,100))
@@ -68,7 +69,7 @@ struct dp_model {
     int mix_ns, mix_nsc, mix_tanh_approx, mix_fit_ns, mix_fit3_ns, mix_ns_bwd;
     int mix_ns_fwd, mix_nsc_fwd;    // forward-kernel overrides of mix_ns / mix_nsc (precision study)
     int profile;
-    cudaEvent_t ev[DP_NPHASES + 1];
+    cudaEvent_t ev[8];                // ev[0..5]: phase boundaries; ev[6], ev[7]: around the MIX-16 tcgen05 backward kernel
 };
 
 // Workspace carve-up (all offsets 256-byte aligned), filled by dp_ws_layout().

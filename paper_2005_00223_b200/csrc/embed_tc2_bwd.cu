@@ -782,11 +782,13 @@ cudaError_t launch_embed_bwd_tc2(const dp_model *m, long N, const Grid3 &g, char
     if (!tbuf) cudaMalloc(&tbuf, 20 * sizeof(long long));
     tdbg = tbuf;
 #endif
+    if (m->profile) cudaEventRecord(m->ev[6], st);
     k_embed_bwd_tc2<<<m->num_sms, NWG * WGT, BwdSmem::TOTAL, st>>>(
         N, m->T, g.ncell, m->Nm, off4, (const EmbedNetTC2 *)m->embed_tc2_dev, m->std_dev, (int *)(ws + L.bin_start),
         (int *)(ws + L.rowstart), (const float4 *)(ws + L.rows_rh), (const int2 *)(ws + L.rows_id),
         (const uint8_t *)(ws + L.gAf), (const float *)(ws + L.gscale), (float4 *)(ws + L.rows_g),
         (unsigned long long *)(ws + L.status + 16), tdbg);
+    if (m->profile) cudaEventRecord(m->ev[7], st);
     int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
     k_prod_force_virial<<<m->num_sms * 8, 256, 0, st>>>(N, m->T, off4, sel4, ep, (int *)(ws + L.rowstart),
                                                         (const int2 *)(ws + L.rows_id), (const float4 *)(ws + L.rows_g),
