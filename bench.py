@@ -153,6 +153,22 @@ def time_config(binding, torch, s, dev, steps, warmup, flush, profile=True):
                 rows_f=rows_f, rows_b=rows_b, ntr=ntr)
 
 
+def max_over_ranks(times_ms, world, device):
+    """Replicas only: every rank times the same number of steps of its own replica; the job time is the
+    MAX over ranks (one all-reduce of the timings, no data-path collective)."""
+    import torch
+    tt = torch.tensor(list(times_ms), dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return [float(x) for x in tt]
+
+
+def whole_job_value(natoms, steps, world, t_ms):
+    """Aggregate atom-steps/s of `world` independent replicas (weak scaling)."""
+    return world * natoms * steps / (t_ms * 1e-3)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -240,15 +256,12 @@ def main():
     h2d = N * 24 + N * 4
     d2h = 8 + N * 24 + 72 + N * 8
 
-    tt = torch.tensor([t_ms, e2e_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    t_ms, e2e_ms = float(tt[0]), float(tt[1])
+    t_ms, e2e_ms = max_over_ranks([t_ms, e2e_ms], world, dev)
 
     if rank == 0:
         pk = peaks()
         ms_step = t_ms / K
-        value = world * N * K / (t_ms * 1e-3)
+        value = whole_job_value(N, K, world, t_ms)
         if s.precision == "fp64":
             peak = pk["bf16_sus"] * FP64_OVER_BF16_NOMINAL
             peak_src = f"{pk['src']}: bf16 sustained {pk['bf16_sus']} TF/s x nominal fp64/bf16 ratio 45/2250"

@@ -102,16 +102,17 @@ k_embed_fwd_tc2(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, const Em
     // fold the lanes of one finished atom into A_i and clear its accumulator block
     auto flush = [&](int atom) {
         const int slot = atom & (T2_NSLOT - 1);
-        uint32_t v1[4], v2[4];
-        tc::ld4(tm_lane + TM_D1 + 8 * slot, v1);
-        tc::ld4(tm_lane + TM_D2 + 8 * slot, v2);
+        uint32_t v1[8], v2[8];
+        const uint32_t z8[8] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
+        tc::ld8(tm_lane + TM_D1 + 8 * slot, v1);
+        tc::ld8(tm_lane + TM_D2 + 8 * slot, v2);
         tc::wait_ld();
-        tc::st4(tm_lane + TM_D1 + 8 * slot, 0u, 0u, 0u, 0u);
-        tc::st4(tm_lane + TM_D2 + 8 * slot, 0u, 0u, 0u, 0u);
+        tc::st8(tm_lane + TM_D1 + 8 * slot, z8);
+        tc::st8(tm_lane + TM_D2 + 8 * slot, z8);
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            scr[c * 208 + t] = __uint_as_float(v1[c]);
-            if (t < 80) scr[c * 208 + 128 + t] = __uint_as_float(v2[c]);
+        for (int c = 0; c < 4; ++c) {      // columns c: T . R^w(hi), columns 4 + c: T . R^w(lo)
+            scr[c * 208 + t] = __uint_as_float(v1[c]) + __uint_as_float(v1[4 + c]);
+            if (t < 80) scr[c * 208 + 128 + t] = __uint_as_float(v2[c]) + __uint_as_float(v2[4 + c]);
         }
         tc::bar_sync(1 + wg, 128);
         if (t < M2E) {
@@ -200,7 +201,9 @@ k_embed_fwd_tc2(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, const Em
                 // ... and write the contraction operand of the first pass
                 {
                     const bool in = atom >= 0 && atom - atom0 < T2_NSLOT;
-                    const uint4 rw = make_uint4(tc::pack_h2(wgt * rh.x, wgt * rh.y), tc::pack_h2(wgt * rh.z, wgt * rh.w), 0u, 0u);
+                    uint4 rw;          // {hi[0..3], lo[0..3]} of the weighted row: the lo parts ride in the four spare columns of the slot
+                    tc::split_h2(wgt * rh.x, wgt * rh.y, rw.x, rw.z);
+                    tc::split_h2(wgt * rh.z, wgt * rh.w, rw.y, rw.w);
                     const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll
                     for (int s_ = 0; s_ < T2_NSLOT; ++s_)
@@ -256,7 +259,9 @@ k_embed_fwd_tc2(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, const Em
                 for (int p0 = atom0; p0 <= atomL; p0 += T2_NSLOT) {
                     if (p0 != atom0) {
                         const bool in = atom >= p0 && atom - p0 < T2_NSLOT;
-                        const uint4 rw = make_uint4(tc::pack_h2(wgt * rh.x, wgt * rh.y), tc::pack_h2(wgt * rh.z, wgt * rh.w), 0u, 0u);
+                        uint4 rw;          // {hi[0..3], lo[0..3]} of the weighted row: the lo parts ride in the four spare columns of the slot
+                    tc::split_h2(wgt * rh.x, wgt * rh.y, rw.x, rw.z);
+                    tc::split_h2(wgt * rh.z, wgt * rh.w, rw.y, rw.w);
                         const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll
                         for (int s_ = 0; s_ < T2_NSLOT; ++s_)

@@ -147,3 +147,45 @@ def test_config3_mix32_full_size_sampled():
 def test_config4_mix16_full_size_sampled():
     """copper 1,048,576 atoms, MIX-16, shuffled atom order; sampled oracle centres."""
     _sampled_check(4, nsample=48, tol=5e-3, tolEi=1e-3)
+
+
+# ------------------------------------------------------------------ MIX-16 tcgen05 path: edge cases of the tiling
+def test_mix16_overflow_blocks_have_no_padded_row():
+    """every block over-full (no padded-row representative), rows per atom = sel: tiles span two atoms exactly"""
+    s = synth.copper(5, 0.05, 77, sel=(100,))
+    o = oracle.evaluate(s.coords, s.types, s.box, s.model)
+    g = _gpu_eval(s, "mix16")
+    assert np.array_equal(g["nlist"], o["nlist"]) and g["n_truncated"] == 500
+    # Outside the five BASELINE configs the 5e-3 bound is not guaranteed: with only 100 rows per atom the single-fp16
+    # activations of the forward kernel average less (measured 5.2e-3; DESIGN.md section 6.1).  The bound here is 2x.
+    _check_forces(g, o, 1e-2)
+    assert g["rows"] == (500 * 100, 500 * 100)            # forward and backward push the same compact rows
+
+
+def test_mix16_short_blocks_many_atoms_per_tile():
+    """water with generous capacities: 128-row tiles span up to ~6 atoms (several passes per tile in the backward),
+    ragged tails in all four (centre, neighbour) blocks"""
+    s = synth.water(216, 18.7, 5, sel=(50, 100))
+    o = oracle.evaluate(s.coords, s.types, s.box, s.model)
+    g = _gpu_eval(s, "mix16")
+    assert np.array_equal(g["nlist"], o["nlist"])
+    _check_forces(g, o, 5e-3)
+    vmax = np.abs(o["virial"]).max()
+    assert np.abs(g["virial"] - o["virial"]).max() <= 5e-3 * vmax
+    assert abs(g["energy"][0] - o["energy"]) / s.natoms <= 1e-3
+
+
+def test_profile_slots_and_launch_count():
+    import torch
+    from paper_2005_00223_b200 import binding
+    s = synth.config(0)
+    m = binding.DPModel(s.model, "mix16")
+    c, t = torch.from_numpy(s.coords).cuda(), torch.from_numpy(s.types).cuda()
+    m.compute(c, t, s.box)
+    m.profile_enable(True)
+    m.compute(c, t, s.box)
+    ms = m.profile_read()
+    assert ms.shape == (6,) and (ms >= 0).all()
+    assert 0 < ms[5] <= ms[3]                  # the backward kernel alone is a part of the backward phase
+    assert m.launches_per_compute() == 19      # one type: 18 + T
+    m.close()
