@@ -158,9 +158,9 @@ k_env_rows(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, EnvParams ep,
     const int sel[4] = {sel4.x, sel4.y, sel4.z, sel4.w}, off[4] = {off4.x, off4.y, off4.z, off4.w};
     int a = 0;
     for (int t = 1; t < T; ++t) a += i >= bin_start[t * ncell];
-    double av[4], sd[4];
+    double av[4], isd[4];
 #pragma unroll
-    for (int c = 0; c < 4; ++c) { av[c] = avg[4 * a + c]; sd[c] = stdv[4 * a + c]; }
+    for (int c = 0; c < 4; ++c) { av[c] = avg[4 * a + c]; isd[c] = 1.0 / stdv[4 * a + c]; }
     const double xi = xs[3 * i], yi = xs[3 * i + 1], zi = xs[3 * i + 2];
     const double hx = 0.5 * ep.L[0], hy = 0.5 * ep.L[1], hz = 0.5 * ep.L[2];
     for (int b = 0; b < T; ++b) {
@@ -174,10 +174,24 @@ k_env_rows(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, EnvParams ep,
                 const double dx = min_image(xs[3 * (long)j] - xi, ep.L[0], hx);
                 const double dy = min_image(xs[3 * (long)j + 1] - yi, ep.L[1], hy);
                 const double dz = min_image(xs[3 * (long)j + 2] - zi, ep.L[2], hz);
-                env_row(ep, dx, dy, dz, Rt);
+                // fp64 environment row with one reciprocal square root instead of a square root and four divisions
+                // (the result is rounded to fp32 below; PAPER.md:125 keeps the environment matrix in double)
+                const double r2 = dx * dx + dy * dy + dz * dz;
+                const double ir = rsqrt(r2), r = r2 * ir;
+                double w = 1.0;
+                if (r >= ep.rc_smth) {
+                    if (r < ep.rc) {
+                        const double u = (r - ep.rc_smth) * ep.inv_range;
+                        w = u * u * u * (-6.0 * u * u + 15.0 * u - 10.0) + 1.0;
+                    } else {
+                        w = 0.0;
+                    }
+                }
+                const double sr = w * ir, q = sr * ir;
+                Rt[0] = sr; Rt[1] = q * dx; Rt[2] = q * dy; Rt[3] = q * dz;
             }
-            rows_rh[base + k] = make_float4((float)((Rt[0] - av[0]) / sd[0]), (float)((Rt[1] - av[1]) / sd[1]),
-                                            (float)((Rt[2] - av[2]) / sd[2]), (float)((Rt[3] - av[3]) / sd[3]));
+            rows_rh[base + k] = make_float4((float)((Rt[0] - av[0]) * isd[0]), (float)((Rt[1] - av[1]) * isd[1]),
+                                            (float)((Rt[2] - av[2]) * isd[2]), (float)((Rt[3] - av[3]) * isd[3]));
             rows_id[base + k] = make_int2((int)i, k < nr ? nlist[i * Nm + off[b] + k] : -(sel[b] - nr));
         }
     }
