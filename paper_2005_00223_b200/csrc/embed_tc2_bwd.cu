@@ -247,20 +247,16 @@ __device__ __forceinline__ uint32_t hmul2(uint32_t a, uint32_t b) {
     __half2 r = __hmul2(*reinterpret_cast<const __half2 *>(&a), *reinterpret_cast<const __half2 *>(&b));
     return *reinterpret_cast<uint32_t *>(&r);
 }
-// 16 gradient columns (fp32 accumulators) times 1 - t^2 (fp16 pairs) -> fp16 -> two chunks
-__device__ __forceinline__ void gradh16(const uint32_t (&g)[16], const uint32_t *dpk, uint8_t *row, int chunk) {
+// 16 gradient columns (fp32 accumulators) times 1 - t^2 (fp16 pairs) -> fp16 pairs -> 8 TMEM columns (A operand of the
+// next product: dz3 / dz2 overwrite the hi parts of t3 / t2, which are dead once dR^ = T g~ has been formed)
+__device__ __forceinline__ void gradh16(const uint32_t (&g)[16], const uint32_t *dpk, uint32_t tm_dst) {
     uint32_t o[8];
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
-#ifndef DP_GRAD_F16
         const float2 d = unpack_h2(dpk[q]);
         o[q] = tc::pack_h2(__uint_as_float(g[2 * q]) * d.x, __uint_as_float(g[2 * q + 1]) * d.y);
-#else
-        o[q] = hmul2(tc::pack_h2(__uint_as_float(g[2 * q]), __uint_as_float(g[2 * q + 1])), dpk[q]);
-#endif
     }
-    *reinterpret_cast<uint4 *>(row + chunk * 2048) = make_uint4(o[0], o[1], o[2], o[3]);
-    *reinterpret_cast<uint4 *>(row + (chunk + 1) * 2048) = make_uint4(o[4], o[5], o[6], o[7]);
+    tc::st8(tm_dst, o);
 }
 
 constexpr int WGT = 128;       // threads per warpgroup: thread = row; every stage walks its two column halves h = 0, 1
@@ -536,33 +532,33 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *
                     DP_TICK(8);
                     wait_mma();
                     DP_TICK(9);
-                    // ---- E4: dR^ of this row; dz3 = dT3 (1 - t3^2) -> t3 block of the lo image ----
+                    // ---- E4: dR^ of this row; dz3 = dT3 (1 - t3^2) -> TMEM, over the hi parts of t3 ----
                     float dR[4];
                     {
                         uint32_t v[16];                      // both slots: tcgen05.ld takes one warp-uniform address
                         tc::ld16(tm_lane + TM_DR, v);
 #pragma unroll
                         for (int h = 0; h < 2; ++h) {
-                            uint8_t *img = lo_row + (T2_O3 / 8 + 6 * h) * 2048;
 #pragma unroll
                             for (int u = 0; u < 3; ++u) {
                                 uint32_t g0[16];
                                 tc::ld16(tm_lane + TM_Z + 48 * h + 16 * u, g0);
                                 tc::wait_ld();
-                                gradh16(g0, d3p[h] + 8 * u, img, 2 * u);
+                                gradh16(g0, d3p[h] + 8 * u, tm_lane + TM_T + 48 + 24 * h + 8 * u);
                             }
                             if (h == 1) {
                                 uint32_t g3[4];
                                 tc::ld4(tm_lane + TM_Z + 96, g3);
                                 tc::wait_ld();
-                                *reinterpret_cast<uint4 *>(img + 6 * 2048) =
-                                    make_uint4(hmul2(tc::pack_h2(__uint_as_float(g3[0]), __uint_as_float(g3[1])), d3p[h][24]),
-                                               hmul2(tc::pack_h2(__uint_as_float(g3[2]), __uint_as_float(g3[3])), d3p[h][25]), 0u, 0u);
+                                const float2 da = unpack_h2(d3p[h][24]), db = unpack_h2(d3p[h][25]);
+                                tc::st4(tm_lane + TM_T + 96, tc::pack_h2(__uint_as_float(g3[0]) * da.x, __uint_as_float(g3[1]) * da.y),
+                                        tc::pack_h2(__uint_as_float(g3[2]) * db.x, __uint_as_float(g3[3]) * db.y), 0u, 0u);
                             }
                         }
 #pragma unroll
                         for (int c = 0; c < 4; ++c)
                             dR[c] = slot ? __uint_as_float(v[8 + c]) + __uint_as_float(v[12 + c]) : __uint_as_float(v[c]) + __uint_as_float(v[4 + c]);
+                        tc::wait_st();
                     }
                     DP_TICK(10);
                     sync_issue();
@@ -575,7 +571,7 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *
                             tc::mma_ss(tmem + TM_Z + 32, tc::desc_at(d_rimg, ks * 2 * 2048), tc::desc_at(d_qk, T2_O2 * 16 + ks * 2 * (T2_COLS * 16)), idy2, ks > 0);
 #pragma unroll
                         for (int ks = 0; ks < T2_K3 / 16; ++ks)
-                            tc::mma_ss(tmem + TM_Z + 32, tc::desc_at(d_tlo, (T2_O3 / 8 + 2 * ks) * 2048), tc::desc_at(d_w3t, 32 * 16 + ks * 2 * (96 * 16)), idy2, true);
+                            tc::mma_ts(tmem + TM_Z + 32, tmem + TM_T + 48 + 8 * ks, tc::desc_at(d_w3t, 32 * 16 + ks * 2 * (96 * 16)), idy2, true);
                         tc::commit(bar);
                         // ... then the part of dy1 that does not depend on dz2 (waited for with the last stage)
                         constexpr uint32_t idy1 = tc::idesc(128, 32, false, false);
@@ -584,36 +580,32 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *
                             tc::mma_ss(tmem + TM_Z, tc::desc_at(d_rimg, ks * 2 * 2048), tc::desc_at(d_qk, ks * 2 * (T2_COLS * 16)), idy1, ks > 0);
 #pragma unroll
                         for (int ks = 0; ks < T2_K3 / 16; ++ks)
-                            tc::mma_ss(tmem + TM_Z, tc::desc_at(d_tlo, (T2_O3 / 8 + 2 * ks) * 2048), tc::desc_at(d_w3t, ks * 2 * (96 * 16)), idy1, true);
+                            tc::mma_ts(tmem + TM_Z, tmem + TM_T + 48 + 8 * ks, tc::desc_at(d_w3t, ks * 2 * (96 * 16)), idy1, true);
                     }
                     DP_TICK(11);
                     wait_mma();
                     DP_TICK(12);
-                    // ---- E5: dz2 = dy2 (1 - t2^2) -> t2 block of the lo image ----
+                    // ---- E5: dz2 = dy2 (1 - t2^2) -> TMEM, over the hi parts of t2 ----
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
-                        uint8_t *img = lo_row + (T2_O2 / 8) * 2048;
                         uint32_t g0[16], g1[16];
                         tc::ld16(tm_lane + TM_Z + 32 + 32 * h, g0);
                         if (h == 0) tc::ld16(tm_lane + TM_Z + 48, g1);
                         else tc::ld2(tm_lane + TM_Z + 80, reinterpret_cast<uint32_t (&)[2]>(g1));
                         tc::wait_ld();
-                        {
-                            uint32_t o[8];
+                        uint32_t o[8];
 #pragma unroll
-                            for (int q = 0; q < 8; ++q) o[q] = tc::pack_h2(__uint_as_float(g0[2 * q]) * d2f[h][2 * q], __uint_as_float(g0[2 * q + 1]) * d2f[h][2 * q + 1]);
-                            *reinterpret_cast<uint4 *>(img + (4 * h) * 2048) = make_uint4(o[0], o[1], o[2], o[3]);
-                            *reinterpret_cast<uint4 *>(img + (4 * h + 1) * 2048) = make_uint4(o[4], o[5], o[6], o[7]);
-                            if (h == 0) {
+                        for (int q = 0; q < 8; ++q) o[q] = tc::pack_h2(__uint_as_float(g0[2 * q]) * d2f[h][2 * q], __uint_as_float(g0[2 * q + 1]) * d2f[h][2 * q + 1]);
+                        tc::st8(tm_lane + TM_T + 16 + 16 * h, o);
+                        if (h == 0) {
 #pragma unroll
-                                for (int q = 0; q < 8; ++q) o[q] = tc::pack_h2(__uint_as_float(g1[2 * q]) * d2f[h][16 + 2 * q], __uint_as_float(g1[2 * q + 1]) * d2f[h][16 + 2 * q + 1]);
-                                *reinterpret_cast<uint4 *>(img + 2 * 2048) = make_uint4(o[0], o[1], o[2], o[3]);
-                                *reinterpret_cast<uint4 *>(img + 3 * 2048) = make_uint4(o[4], o[5], o[6], o[7]);
-                            } else {
-                                *reinterpret_cast<uint4 *>(img + 6 * 2048) = make_uint4(tc::pack_h2(__uint_as_float(g1[0]) * d2f[h][16], __uint_as_float(g1[1]) * d2f[h][17]), 0u, 0u, 0u);
-                            }
+                            for (int q = 0; q < 8; ++q) o[q] = tc::pack_h2(__uint_as_float(g1[2 * q]) * d2f[h][16 + 2 * q], __uint_as_float(g1[2 * q + 1]) * d2f[h][16 + 2 * q + 1]);
+                            tc::st8(tm_lane + TM_T + 24, o);
+                        } else {
+                            tc::st4(tm_lane + TM_T + 40, tc::pack_h2(__uint_as_float(g1[0]) * d2f[h][16], __uint_as_float(g1[1]) * d2f[h][17]), 0u, 0u, 0u);
                         }
                     }
+                    tc::wait_st();
                     DP_TICK(13);
                     sync_issue();
                     if (issuer_warp && tc::elect_one()) {
@@ -621,7 +613,7 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *
                         constexpr uint32_t id1 = tc::idesc(128, 32, false, false);
 #pragma unroll
                         for (int ks = 0; ks < T2_K2 / 16; ++ks)
-                            tc::mma_ss(tmem + TM_Z, tc::desc_at(d_tlo, (T2_O2 / 8 + 2 * ks) * 2048), tc::desc_at(d_w2t, ks * 2 * (32 * 16)), id1, true);
+                            tc::mma_ts(tmem + TM_Z, tmem + TM_T + 16 + 8 * ks, tc::desc_at(d_w2t, ks * 2 * (32 * 16)), id1, true);
                         tc::commit(bar);
                     }
                     DP_TICK(14);
