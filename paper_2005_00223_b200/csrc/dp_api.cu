@@ -451,8 +451,9 @@ size_t dp_workspace_bytes(const dp_model *m, long natoms) {
 
 int dp_launches_per_compute(const dp_model *m) {
     if (!m) return 0;
-    // MIX-16 tcgen05 path: 4 binning + list + T row scans + env rows + forward + 7 fitting + image fold + backward + force/virial + finalize
-    if (m->use_tc == 2 && m->use_tc_bwd && m->use_fit_tc) return 18 + m->T;
+    // MIX-16 tcgen05 path: 4 binning + list + T row scans + env rows + forward + 3 fitting (first layer, fused 240 x 240 chain,
+    // last product with gA) + image fold + backward + force/virial + finalize
+    if (m->use_tc == 2 && m->use_tc_bwd && m->use_fit_tc) return 14 + m->T;
     return 17;
 }
 

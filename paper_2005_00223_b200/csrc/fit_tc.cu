@@ -392,6 +392,256 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(512));
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// The four 240 x 240 products of the fitting net in ONE kernel (layers 2, 3 forward, their backward):
+//   S1: t2 = tanh(h1 V2 + c2), h2 = h1 + t2         S2: t3 = tanh(h2 V3 + c3), h3 = h2 + t3, E_i = h3.v4 + c4 + ebias,
+//   S3: gh2 = v4 + gz3 V3^T, gz2 = gh2 (1 - t2^2)        gz3 = v4 (1 - t3^2)
+//   S4: gh1 = gh2 + gz2 V2^T, gz1 = gh1 (1 - h1^2)  -> global (A operand of the last product, MODE 6)
+// One 128-row tile per CTA at a time; the operand of every stage is written by the previous epilogue straight into the
+// shared-memory operand image (hi + lo fp16), 1 - t2^2 waits in TMEM (fp32), gh2 stays in the accumulator and the S4
+// product accumulates on top of it.  h1 is read from global memory twice (S1 operand, S4 epilogue), prefetched into
+// registers under the preceding MMAs; nothing else of the chain touches HBM.
+// Warps: 0 weight loader (cp.async.bulk), 1 MMA issuer, 2-9 epilogue / operand producers: thread (row, half of the columns).
+struct FitChainArgs {
+    int T, ncell;
+    const int *bin_start;
+    const float *h1;                      // [rows][240]
+    const __half *Bimg; long b_type_stride;
+    const float *c2, *c3, *v4, *c4;       // [T][240], c4 [T]
+    const double *ebias;                  // [T]
+    float *gz1;                           // [rows][240]
+    double *eatom;                        // [rows]
+};
+constexpr int CH_THREADS = 64 + 256;
+constexpr int CH_BN = 240, CH_NKC = 3, CH_BSTAGE = KC * CH_BN * 2;
+constexpr int CH_OFF_B = ((CH_NKC * 2 * A_PART + 1023) / 1024) * 1024;
+constexpr int CH_OFF_BAR = CH_OFF_B + 2 * CH_BSTAGE;
+constexpr int CH_OFF_RED = CH_OFF_BAR + 128;                 // float [2][128] energy partial sums
+constexpr int CH_TOTAL = CH_OFF_RED + 2 * 128 * 4;
+constexpr int CH_TM_ACC = 0, CH_TM_D2 = 256;                 // TMEM: accumulator [0,240), 1 - t2^2 (fp32) [256,496)
+static_assert(CH_TOTAL <= 227 * 1024, "shared memory budget");
+
+template <bool APPROX>
+__global__ void __launch_bounds__(CH_THREADS, 1) k_fit_chain(FitChainArgs p) {
+    extern __shared__ __align__(1024) uint8_t smem[];
+    __shared__ uint32_t tmem_base_s;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + CH_OFF_BAR);
+    uint64_t *b_full = bars, *b_empty = bars + 2, *a_ready = bars + 4, *acc_ready = bars + 5;
+    float *red = reinterpret_cast<float *>(smem + CH_OFF_RED);
+    if (tid == 0) {
+        for (int k = 0; k < 2; ++k) { tc::mbar_init(&b_full[k], 1); tc::mbar_init(&b_empty[k], 1); }
+        tc::mbar_init(a_ready, 8);
+        tc::mbar_init(acc_ready, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tc::smem_u32(&tmem_base_s)), "n"(512));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    tc::fence_before();
+    __syncthreads();
+    tc::fence_after();
+    const uint32_t tmem = __shfl_sync(0xffffffffu, tmem_base_s, 0);
+    const uint32_t sbase = tc::smem_u32(smem);
+    int ntiles_total = 0;
+    for (int a = 0; a < p.T; ++a) ntiles_total += (p.bin_start[(a + 1) * p.ncell] - p.bin_start[a * p.ncell] + BM - 1) / BM;
+    auto tile_of = [&](int tile, int &a, int &row0, int &rend) {
+        for (a = 0; a < p.T; ++a) {
+            const int ts0 = p.bin_start[a * p.ncell], ts1 = p.bin_start[(a + 1) * p.ncell];
+            const int nt = (ts1 - ts0 + BM - 1) / BM;
+            if (tile < nt) { row0 = ts0 + tile * BM; rend = ts1; return; }
+            tile -= nt;
+        }
+    };
+    // weight images of the four stages inside one type's block (FIT_TC_OFF[1..4]): V2, V3, V3^T, V2^T
+    const long img_off[4] = {1600L * 240, 1600L * 240 + 240L * 240, 1600L * 240 + 2L * 240 * 240, 1600L * 240 + 3L * 240 * 240};
+
+    if (warp == 0) {
+        // ---------------------------------------------------------------- weight loader
+        if (lane == 0) {
+            uint32_t step = 0;
+            for (int tile = blockIdx.x; tile < ntiles_total; tile += gridDim.x) {
+                int a, row0, rend;
+                tile_of(tile, a, row0, rend);
+                const __half *Bw = p.Bimg + a * p.b_type_stride;
+                for (int sidx = 0; sidx < 4; ++sidx)
+                    for (int kc = 0; kc < CH_NKC; ++kc, ++step) {
+                        const int st = step & 1;
+                        tc::mbar_wait(&b_empty[st], ((step >> 1) & 1) ^ 1);
+                        mbar_expect_tx(&b_full[st], CH_BSTAGE);
+                        bulk_g2s(sbase + CH_OFF_B + st * CH_BSTAGE, Bw + img_off[sidx] + (long)kc * (KC * CH_BN), CH_BSTAGE, &b_full[st]);
+                    }
+            }
+        }
+    } else if (warp == 1) {
+        // ---------------------------------------------------------------- MMA issuer
+        constexpr uint32_t idesc = tc::idesc(128, CH_BN, false, false);
+        uint32_t step = 0, stage = 0;
+        for (int tile = blockIdx.x; tile < ntiles_total; tile += gridDim.x)
+            for (int sidx = 0; sidx < 4; ++sidx, ++stage) {
+                tc::mbar_wait(a_ready, stage & 1);
+                tc::fence_after();
+                for (int kc = 0; kc < CH_NKC; ++kc, ++step) {
+                    const int st = step & 1;
+                    tc::mbar_wait(&b_full[st], (step >> 1) & 1);
+                    tc::fence_after();
+                    const uint64_t da = tc::desc(sbase + kc * 2 * A_PART, A_SUB_STRIDE, 128);
+                    const uint64_t db = tc::desc(sbase + CH_OFF_B + st * CH_BSTAGE, CH_BN * 16, 128);
+                    if (tc::elect_one()) {
+#pragma unroll
+                        for (int part = 0; part < 2; ++part)
+#pragma unroll
+                            for (int ks = 0; ks < KC / 16; ++ks)       // S4 accumulates on gh2, left in TMEM by the S3 epilogue
+                                tc::mma_ss(tmem + CH_TM_ACC, tc::desc_at(da, part * A_PART + ks * 2 * A_SUB_STRIDE),
+                                           tc::desc_at(db, ks * 2 * (CH_BN * 16)), idesc, sidx == 3 || (kc | part | ks) != 0);
+                        tc::commit(&b_empty[st]);
+                    }
+                    __syncwarp();
+                }
+                if (tc::elect_one()) tc::commit(acc_ready);
+                __syncwarp();
+            }
+    } else {
+        // ---------------------------------------------------------------- epilogue / operand producers: thread = (row, column half)
+        const int q4 = warp & 3, r = q4 * 32 + lane, hc = ((warp - 2) >> 2) & 1;
+        const uint32_t tm_lane = tmem + ((uint32_t)(q4 * 32) << 16);
+        uint32_t stage = 0;
+        // 8 consecutive values of this row -> the hi and lo 16-byte chunks of column group j (columns 120 hc + 8 j ..)
+        auto put_group = [&](int j, const float (&x)[8]) {
+            const int g = 15 * hc + j, kc = g / SUB, sub = g % SUB;
+            uint8_t *dst = smem + kc * 2 * A_PART + sub * A_SUB_STRIDE + r * 16;
+            uint4 hi, lo;
+            tc::split_h2(x[0], x[1], hi.x, lo.x); tc::split_h2(x[2], x[3], hi.y, lo.y);
+            tc::split_h2(x[4], x[5], hi.z, lo.z); tc::split_h2(x[6], x[7], hi.w, lo.w);
+            *reinterpret_cast<uint4 *>(dst) = hi;
+            *reinterpret_cast<uint4 *>(dst + A_PART) = lo;
+        };
+        auto publish = [&]() {        // operand image (and TMEM stores) of this warp are complete: one arrival per warp
+            tc::wait_st();
+            tc::proxy_fence();
+            tc::fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(a_ready);
+        };
+        auto wait_acc = [&]() {
+            tc::mbar_wait(acc_ready, stage & 1);
+            ++stage;
+            tc::fence_after();
+        };
+        for (int tile = blockIdx.x; tile < ntiles_total; tile += gridDim.x) {
+            int a, row0, rend;
+            tile_of(tile, a, row0, rend);
+            const bool ok = row0 + r < rend;
+            const float *h1row = p.h1 + (long)(ok ? row0 + r : row0) * 240 + 120 * hc;
+            const float *c2 = p.c2 + a * 240 + 120 * hc, *c3 = p.c3 + a * 240 + 120 * hc, *v4 = p.v4 + a * 240 + 120 * hc;
+            float H[120];
+            // ---- operand of S1: h1 ----
+#pragma unroll
+            for (int k4 = 0; k4 < 30; ++k4) {
+                float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (ok) v = __ldg(reinterpret_cast<const float4 *>(h1row) + k4);
+                H[4 * k4] = v.x; H[4 * k4 + 1] = v.y; H[4 * k4 + 2] = v.z; H[4 * k4 + 3] = v.w;
+            }
+#pragma unroll
+            for (int j = 0; j < 15; ++j) {
+                const float x[8] = {H[8 * j], H[8 * j + 1], H[8 * j + 2], H[8 * j + 3], H[8 * j + 4], H[8 * j + 5], H[8 * j + 6], H[8 * j + 7]};
+                put_group(j, x);
+            }
+            publish();
+            // ---- S1: t2 = tanh(acc + c2); 1 - t2^2 -> TMEM; h2 = h1 + t2 -> operand of S2 ----
+            wait_acc();
+#pragma unroll
+            for (int j = 0; j < 15; ++j) {
+                uint32_t v[8], d[8];
+                tc::ld8(tm_lane + CH_TM_ACC + 120 * hc + 8 * j, v);
+                tc::wait_ld();
+                float x[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    const float z = __uint_as_float(v[q]) + __ldg(c2 + 8 * j + q);
+                    const float t = APPROX ? tc::tanh_approx(z) : tanhf(z);
+                    d[q] = __float_as_uint(fmaf(-t, t, 1.f));
+                    H[8 * j + q] += t;
+                    x[q] = H[8 * j + q];
+                }
+                tc::st8(tm_lane + CH_TM_D2 + 120 * hc + 8 * j, d);
+                put_group(j, x);
+            }
+            publish();
+            // ---- S2: t3 = tanh(acc + c3); h3 = h2 + t3 -> E_i; gz3 = v4 (1 - t3^2) -> operand of S3 ----
+            wait_acc();
+            float esum = 0.f;
+#pragma unroll
+            for (int j = 0; j < 15; ++j) {
+                uint32_t v[8];
+                tc::ld8(tm_lane + CH_TM_ACC + 120 * hc + 8 * j, v);
+                tc::wait_ld();
+                float x[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    const float w = __ldg(v4 + 8 * j + q);
+                    const float t = tanhf(__uint_as_float(v[q]) + __ldg(c3 + 8 * j + q));
+                    esum = fmaf(H[8 * j + q] + t, w, esum);
+                    x[q] = w * fmaf(-t, t, 1.f);
+                }
+                put_group(j, x);
+            }
+            red[hc * 128 + r] = esum;
+            tc::bar_sync(1, 256);
+            if (hc == 0 && ok) p.eatom[row0 + r] = (double)(red[r] + red[128 + r] + __ldg(p.c4 + a)) + p.ebias[a];
+            publish();
+            // ---- S3: gh2 = v4 + acc (left in the accumulator); gz2 = gh2 (1 - t2^2) -> operand of S4 ----
+            wait_acc();
+#pragma unroll
+            for (int j = 0; j < 15; ++j) {
+                uint32_t v[8], d[8], o[8];
+                tc::ld8(tm_lane + CH_TM_ACC + 120 * hc + 8 * j, v);
+                tc::ld8(tm_lane + CH_TM_D2 + 120 * hc + 8 * j, d);
+                tc::wait_ld();
+                float x[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    const float gh = __ldg(v4 + 8 * j + q) + __uint_as_float(v[q]);
+                    o[q] = __float_as_uint(gh);
+                    x[q] = gh * __uint_as_float(d[q]);
+                }
+                tc::st8(tm_lane + CH_TM_ACC + 120 * hc + 8 * j, o);
+                put_group(j, x);
+            }
+            publish();
+            // h1 again (for 1 - h1^2), in flight under the S4 products
+#pragma unroll
+            for (int k4 = 0; k4 < 30; ++k4) {
+                float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (ok) v = __ldg(reinterpret_cast<const float4 *>(h1row) + k4);
+                H[4 * k4] = v.x; H[4 * k4 + 1] = v.y; H[4 * k4 + 2] = v.z; H[4 * k4 + 3] = v.w;
+            }
+            // ---- S4: gh1 = acc (= gh2 + gz2 V2^T); gz1 = gh1 (1 - h1^2) -> global ----
+            wait_acc();
+            float *gzrow = p.gz1 + (long)(row0 + r) * 240 + 120 * hc;
+#pragma unroll
+            for (int j = 0; j < 15; ++j) {
+                uint32_t v[8];
+                tc::ld8(tm_lane + CH_TM_ACC + 120 * hc + 8 * j, v);
+                tc::wait_ld();
+                float x[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) x[q] = __uint_as_float(v[q]) * fmaf(-H[8 * j + q], H[8 * j + q], 1.f);
+                if (ok) {
+                    *reinterpret_cast<float4 *>(gzrow + 8 * j) = make_float4(x[0], x[1], x[2], x[3]);
+                    *reinterpret_cast<float4 *>(gzrow + 8 * j + 4) = make_float4(x[4], x[5], x[6], x[7]);
+                }
+            }
+            tc::fence_before();      // the accumulator reads above precede the next tile's products (ordered by its first publish)
+        }
+    }
+    tc::fence_before();
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(512));
+}
+
 template <int MODE, int KTOT, int NTOT, bool APPROX>
 void launch(const FitTcArgs &p, int grid, cudaStream_t st) {
     using C = Cfg<KTOT, NTOT>;
@@ -449,5 +699,23 @@ cudaError_t fit_tc_gemm(int mode, bool apx, const dp_model *m, const Grid3 &g, c
         case 5: launch<5, 240, 1600, false>(p, grid, st); break;
         default: launch<6, 240, 1600, false>(p, grid, st); break;
     }
+    return cudaGetLastError();
+}
+
+// layers 2-3 forward, energy, and their backward in one kernel (k_fit_chain)
+cudaError_t fit_tc_chain(bool apx, const dp_model *m, const Grid3 &g, const int *bin_start, const float *h1, const float *c2,
+                         const float *c3, const float *v4, const float *c4, float *gz1, double *eatom, cudaStream_t st) {
+    FitChainArgs p{};
+    p.T = m->T; p.ncell = g.ncell; p.bin_start = bin_start; p.h1 = h1;
+    p.Bimg = (const __half *)m->fit_tc_img_dev; p.b_type_stride = (long)FIT_TC_OFF[6];
+    p.c2 = c2; p.c3 = c3; p.v4 = v4; p.c4 = c4; p.ebias = m->ebias_dev; p.gz1 = gz1; p.eatom = eatom;
+    static bool attr = false;
+    if (!attr) {
+        cudaFuncSetAttribute(k_fit_chain<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, CH_TOTAL);
+        cudaFuncSetAttribute(k_fit_chain<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, CH_TOTAL);
+        attr = true;
+    }
+    if (apx) k_fit_chain<true><<<m->num_sms, CH_THREADS, CH_TOTAL, st>>>(p);
+    else k_fit_chain<false><<<m->num_sms, CH_THREADS, CH_TOTAL, st>>>(p);
     return cudaGetLastError();
 }
