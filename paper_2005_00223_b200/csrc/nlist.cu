@@ -207,22 +207,43 @@ k_nlist(long N, int T, Grid3 g, double rc2, int cap, const int *__restrict__ bin
 }
 
 // ---- second-generation list kernel ----------------------------------------------------------------------------------
-// Bitonic sort of 32 R keys held R per lane (element index = lane * R + r): strides below R are register exchanges,
-// larger strides are warp shuffles.  Ascending.
+// Bitonic sort of 32 R keys held R per lane (element index = lane * R + r), every merge ascending: the first stage of a
+// merge of width k pairs idx with idx ^ (k - 1), the following ones idx with idx ^ j.  Strides below R are register
+// exchanges, larger ones warp shuffles; the smaller key always goes to the smaller index (one 64-bit compare per element).
 template <int R>
 __device__ __forceinline__ void warp_sort_regs(unsigned long long (&key)[R], int lane) {
 #pragma unroll
     for (int k = 2; k <= 32 * R; k <<= 1) {
+        // flip stage
+        if (k <= R) {
 #pragma unroll
-        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int r = 0; r < R; ++r) {
+                const int q = r ^ (k - 1);
+                if (q > r) {
+                    const unsigned long long a = key[r], c = key[q];
+                    const bool sw = a > c;
+                    key[r] = sw ? c : a;
+                    key[q] = sw ? a : c;
+                }
+            }
+        } else {
+            const int jl = k / R - 1;
+            const bool lower = (lane & (k / (2 * R))) == 0;
+            unsigned long long o[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) o[r] = __shfl_xor_sync(0xffffffffu, key[R - 1 - r], jl);
+#pragma unroll
+            for (int r = 0; r < R; ++r) key[r] = ((key[r] < o[r]) == lower) ? key[r] : o[r];
+        }
+#pragma unroll
+        for (int j = k >> 2; j > 0; j >>= 1) {
             if (j < R) {
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
                     const int q = r ^ j;
                     if (q > r) {
-                        const bool asc = (((lane * R + r) & k) == 0);
                         const unsigned long long a = key[r], c = key[q];
-                        const bool sw = (a > c) == asc;
+                        const bool sw = a > c;
                         key[r] = sw ? c : a;
                         key[q] = sw ? a : c;
                     }
@@ -232,11 +253,9 @@ __device__ __forceinline__ void warp_sort_regs(unsigned long long (&key)[R], int
                 const bool lower = (lane & jl) == 0;
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
-                    const bool asc = (((lane * R + r) & k) == 0);
                     const unsigned long long a = key[r];
                     const unsigned long long o = __shfl_xor_sync(0xffffffffu, a, jl);
-                    const bool take_min = asc == lower;
-                    key[r] = take_min ? (a < o ? a : o) : (a > o ? a : o);
+                    key[r] = ((a < o) == lower) ? a : o;
                 }
             }
         }
@@ -262,19 +281,39 @@ __device__ __forceinline__ void sort_and_emit(const unsigned long long *keys, in
 // One warp per (sorted) atom.  Pass 1: fp32 distances on the fp32 copy of the coordinates select candidates conservatively
 // (margin covers the rounding of the copy), ballot-compacted into shared memory.  Pass 2: the exact test and the 64-bit key
 // (canonical fp64 arithmetic of DESIGN.md reading N2) on the few survivors only.  Sort in registers.
+//
+// Pass 1 walks one flat candidate range: the z cells of an (x, y) column are consecutive bins, so a column is one run of
+// sorted atoms (two when it wraps around the box); lane c < 25 looks up the runs of column c, a warp scan turns the run
+// lengths into a table {end of the run in the flat range, first atom - start in the flat range}, and the warp then
+// tests 32 consecutive flat positions per iteration with every lane busy.
+struct NlistF32 {
+    float L[3], invL[3];
+    float rc2_margin;
+};
+__device__ __forceinline__ int warp_incl_scan(int v, int lane) {
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int o = __shfl_up_sync(0xffffffffu, v, d);
+        v += lane >= d ? o : 0;
+    }
+    return v;
+}
 __global__ void __launch_bounds__(128, 8)
-k_nlist2(long N, int T, Grid3 g, double rc2, float rc2f_margin, int cap, const int *__restrict__ bin_start,
+k_nlist2(long N, int T, Grid3 g, double rc2, NlistF32 gf, int cap, const int *__restrict__ bin_start,
          const double *__restrict__ xs, const float4 *__restrict__ xsf, const int *__restrict__ perm,
          const int *__restrict__ inv, int Nm, int4 sel4, int *__restrict__ nlist, int *__restrict__ nreal,
          int *__restrict__ rowcnt, int *__restrict__ status) {
     extern __shared__ unsigned long long keys_all[];
+    __shared__ int2 runtab_all[4][66];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const long i = blockIdx.x * 4L + wid;
     if (i >= N) return;
     unsigned long long *keys = keys_all + (size_t)wid * cap;
+    int2 *runtab = runtab_all[wid];
     const int sel[4] = {sel4.x, sel4.y, sel4.z, sel4.w};
     const double xi = xs[3 * i], yi = xs[3 * i + 1], zi = xs[3 * i + 2];
     const float4 pf = xsf[i];
+    const int ii = (int)i;
     const int cx = cell_of(xi, g.inv_cw[0], g.nc[0]), cy = cell_of(yi, g.inv_cw[1], g.nc[1]),
               cz = cell_of(zi, g.inv_cw[2], g.nc[2]);
     const int R_ = g.reach;       // reach 2 is only chosen for grids with >= 5 cells per axis
@@ -282,47 +321,66 @@ k_nlist2(long N, int T, Grid3 g, double rc2, float rc2f_margin, int cap, const i
     const int lo1 = R_ == 2 ? -2 : (g.nc[1] >= 3 ? -1 : 0), hi1 = R_ == 2 ? 2 : (g.nc[1] >= 2 ? 1 : 0);
     const int lo2 = R_ == 2 ? -2 : (g.nc[2] >= 3 ? -1 : 0), hi2 = R_ == 2 ? 2 : (g.nc[2] >= 2 ? 1 : 0);
     const double hx = 0.5 * g.L[0], hy = 0.5 * g.L[1], hz = 0.5 * g.L[2];
-    const float Lx = (float)g.L[0], Ly = (float)g.L[1], Lz = (float)g.L[2];
-    const float hxf = 0.5f * Lx, hyf = 0.5f * Ly, hzf = 0.5f * Lz;
+    // this lane's column (first z bin of it, relative to the type's bins) and the z cell ranges A (in the box) and B (wrapped)
+    const int ny = hi1 - lo1 + 1, ncol = (hi0 - lo0 + 1) * ny;       // <= 25
+    int colrel = 0;
+    if (lane < ncol) {
+        int ax = cx + lo0 + lane / ny; ax += ax < 0 ? g.nc[0] : 0; ax -= ax >= g.nc[0] ? g.nc[0] : 0;
+        int ay = cy + lo1 + lane % ny; ay += ay < 0 ? g.nc[1] : 0; ay -= ay >= g.nc[1] ? g.nc[1] : 0;
+        colrel = (ax * g.nc[1] + ay) * g.nc[2];
+    }
+    const int zlo = cz + lo2, zhi = cz + hi2;
+    const int za0 = zlo < 0 ? 0 : zlo, za1 = zhi >= g.nc[2] ? g.nc[2] - 1 : zhi;
+    int zb0 = 0, zb1 = -1;
+    if (zlo < 0) { zb0 = zlo + g.nc[2]; zb1 = g.nc[2] - 1; }
+    else if (zhi >= g.nc[2]) { zb0 = 0; zb1 = zhi - g.nc[2]; }
+    const unsigned lt = (1u << lane) - 1u;
     bool truncated = false;
     int off = 0;
     for (int b = 0; b < T; ++b) {
+        // ---- run table ----
+        int sA = 0, lenA = 0, sB = 0, lenB = 0;
+        if (lane < ncol) {
+            const int *bs = bin_start + b * g.ncell + colrel;
+            sA = bs[za0]; lenA = bs[za1 + 1] - sA;
+            if (zb1 >= zb0) { sB = bs[zb0]; lenB = bs[zb1 + 1] - sB; }
+        }
+        const unsigned mA = __ballot_sync(0xffffffffu, lenA > 0), mB = __ballot_sync(0xffffffffu, lenB > 0);
+        const int inA = warp_incl_scan(lenA, lane);
+        const int totA = __shfl_sync(0xffffffffu, inA, 31);
+        int total = totA;
+        if (lenA > 0) runtab[__popc(mA & lt)] = make_int2(inA, sA - (inA - lenA));
+        int nrun = __popc(mA);
+        if (mB) {
+            const int inB = warp_incl_scan(lenB, lane);
+            if (lenB > 0) runtab[nrun + __popc(mB & lt)] = make_int2(totA + inB, sB - (totA + inB - lenB));
+            total += __shfl_sync(0xffffffffu, inB, 31);
+            nrun += __popc(mB);
+        }
+        if (lane == 0) runtab[nrun] = make_int2(0x7fffffff, 0);
+        __syncwarp();
         // ---- pass 1: conservative fp32 filter ----
-        int n1 = 0;
-        for (int ox = lo0; ox <= hi0; ++ox) {
-            int ax = cx + ox; ax += ax < 0 ? g.nc[0] : 0; ax -= ax >= g.nc[0] ? g.nc[0] : 0;
-            for (int oy = lo1; oy <= hi1; ++oy) {
-                int ay = cy + oy; ay += ay < 0 ? g.nc[1] : 0; ay -= ay >= g.nc[1] ? g.nc[1] : 0;
-                // the z cells of one (x, y) column are consecutive bins: one run unless the column wraps
-                const int colb = b * g.ncell + (ax * g.nc[1] + ay) * g.nc[2];
-                const bool one_run = cz + lo2 >= 0 && cz + hi2 < g.nc[2];
-                for (int oz = lo2; oz <= hi2; ++oz) {
-                    int s0, s1;
-                    if (one_run) {
-                        s0 = bin_start[colb + cz + lo2]; s1 = bin_start[colb + cz + hi2 + 1];
-                        oz = hi2;
-                    } else {
-                        int az = cz + oz; az += az < 0 ? g.nc[2] : 0; az -= az >= g.nc[2] ? g.nc[2] : 0;
-                        s0 = bin_start[colb + az]; s1 = bin_start[colb + az + 1];
-                    }
-                    for (int base = s0; base < s1; base += 32) {
-                        const int s = base + lane;
-                        bool ok = false;
-                        if (s < s1 && s != i) {
-                            const float4 q = __ldg(&xsf[s]);
-                            float dx = q.x - pf.x, dy = q.y - pf.y, dz = q.z - pf.z;
-                            dx -= dx > hxf ? Lx : 0.f; dx += dx < -hxf ? Lx : 0.f;
-                            dy -= dy > hyf ? Ly : 0.f; dy += dy < -hyf ? Ly : 0.f;
-                            dz -= dz > hzf ? Lz : 0.f; dz += dz < -hzf ? Lz : 0.f;
-                            ok = fmaf(dz, dz, fmaf(dy, dy, dx * dx)) < rc2f_margin;
-                        }
-                        const unsigned mask = __ballot_sync(0xffffffffu, ok);
-                        const int pos = n1 + __popc(mask & ((1u << lane) - 1u));
-                        if (ok && pos < cap) keys[pos] = (unsigned long long)s;
-                        n1 += __popc(mask);
-                    }
-                }
+        int n1 = 0, r = 0;
+        int2 e = runtab[0];
+        for (int base = 0; base < total; base += 32) {
+            const int idx = base + lane;
+            while (idx >= e.x) e = runtab[++r];
+            const int s = idx + e.y;
+            bool ok = false;
+            if (idx < total && s != ii) {
+                const float4 q = __ldg(&xsf[s]);
+                float dx = q.x - pf.x, dy = q.y - pf.y, dz = q.z - pf.z;
+                // minimum image: d - L rint(d / L), rint through the 1.5 * 2^23 shift
+                const float tx = fmaf(dx, gf.invL[0], 12582912.f) - 12582912.f;
+                const float ty = fmaf(dy, gf.invL[1], 12582912.f) - 12582912.f;
+                const float tz = fmaf(dz, gf.invL[2], 12582912.f) - 12582912.f;
+                dx = fmaf(-tx, gf.L[0], dx); dy = fmaf(-ty, gf.L[1], dy); dz = fmaf(-tz, gf.L[2], dz);
+                ok = fmaf(dz, dz, fmaf(dy, dy, dx * dx)) < gf.rc2_margin;
             }
+            const unsigned mask = __ballot_sync(0xffffffffu, ok);
+            const int pos = n1 + __popc(mask & lt);
+            if (ok && pos < cap) keys[pos] = (unsigned long long)s;
+            n1 += __popc(mask);
         }
         if (n1 > cap) { if (lane == 0) atomicOr(&status[0], 2); n1 = cap; }
         __syncwarp();
@@ -428,12 +486,15 @@ cudaError_t launch_nlist(const dp_model *m, long N, const Grid3 &g, char *ws, co
     // fp32 pre-filter margin: the fp32 copy is off by <= ulp(L)/2 per coordinate, the fp32 arithmetic by a few ulp of rc^2
     double Lmax = g.L[0] > g.L[1] ? g.L[0] : g.L[1];
     Lmax = Lmax > g.L[2] ? Lmax : g.L[2];
-    const float rc2f = (float)(m->rc * m->rc * (1.0 + 1e-5) + 8.0 * m->rc * Lmax * 1.2e-7 + 1e-6);
+    // (and the fp32 minimum image d - L rint(d / L) by another ulp(L))
+    NlistF32 gf;
+    for (int d = 0; d < 3; ++d) { gf.L[d] = (float)g.L[d]; gf.invL[d] = (float)(1.0 / g.L[d]); }
+    gf.rc2_margin = (float)(m->rc * m->rc * (1.0 + 1e-5) + 12.0 * m->rc * Lmax * 1.2e-7 + 1e-6);
     static const bool legacy = std::getenv("DP_NLIST_V1") != nullptr;
     if (!legacy) {
         static bool attr2 = false;
         if (!attr2) { cudaFuncSetAttribute(k_nlist2, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 4096 * 8); attr2 = true; }
-        k_nlist2<<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, m->T, g, m->rc * m->rc, rc2f, cap, (int *)(ws + L.bin_start),
+        k_nlist2<<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, m->T, g, m->rc * m->rc, gf, cap, (int *)(ws + L.bin_start),
                                                             (double *)(ws + L.xs), (const float4 *)(ws + L.xsf), (int *)(ws + L.perm),
                                                             (int *)(ws + L.inv), m->Nm, sel4, (int *)(ws + L.nlist),
                                                             (int *)(ws + L.nreal), m->prec == DP_FP64 ? nullptr : (int *)(ws + L.rowcnt),
