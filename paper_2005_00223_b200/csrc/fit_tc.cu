@@ -29,19 +29,26 @@ __host__ __device__ constexpr int nthreads(int mode) { return 64 + nprod(mode) +
 template <int KTOT, int NTOT>
 struct Cfg {
     static constexpr bool RESIDENT = KTOT == 240;            // the A tile stays in shared memory for all N tiles
+    // K chunk.  K = 1600 (the descriptor producer): 64 = 4 values of m, so that A_i[c][4 kc .. 4 kc + 3] is one aligned float4
+    static constexpr int KCH = KTOT == 1600 ? 64 : KC;
+    static constexpr int SUBS = KCH / 8;
+    // bytes between sub-chunks of the A image.  K = 1600: the two threads of a row are neighbouring lanes and write
+    // sub-chunks 2 mm and 2 mm + 1: 64 bytes of padding put them on disjoint banks
+    static constexpr int ASS = KTOT == 1600 ? BM * 16 + 64 : A_SUB_STRIDE;
+    static constexpr int A_PARTC = SUBS * ASS;               // one part (hi or lo) of one K chunk
     static constexpr int BN = NTOT == 240 ? 240 : 160;
     static constexpr int NTILES = NTOT / BN;
-    static constexpr int NKC = KTOT / KC;
-    static constexpr int NA = RESIDENT ? NKC : 2;            // A buffers
-    static constexpr int B_STAGE = KC * BN * 2;
-    static constexpr int NSTAGE = NTOT == 1600 ? 4 : 2;      // B pipeline depth (short N = 160 stages need more copies in flight)
-    static constexpr int A_BUF = 2 * A_PART;                 // hi + lo
+    static constexpr int NKC = KTOT / KCH;
+    static constexpr int NA = RESIDENT ? NKC : 3;            // A buffers
+    static constexpr int B_STAGE = KCH * BN * 2;
+    static constexpr int NSTAGE = NTOT == 1600 ? 4 : (KTOT == 1600 ? 3 : 2);   // B pipeline depth (short stages need more copies in flight)
+    static constexpr int A_BUF = 2 * A_PARTC;                // hi + lo
     static constexpr int OFF_A = 0;
     static constexpr int OFF_B = ((NA * A_BUF + 1023) / 1024) * 1024;
     static constexpr int OFF_BAR = OFF_B + NSTAGE * B_STAGE;
     static constexpr int TOTAL = OFF_BAR + 256;
     static constexpr int TM_BUF = 256;                       // TMEM columns per accumulator buffer
-    static_assert(KTOT % KC == 0 && NTOT % BN == 0 && BN % 16 == 0, "tile shapes");
+    static_assert(KTOT % KCH == 0 && NTOT % BN == 0 && BN % 16 == 0, "tile shapes");
     static_assert(TOTAL <= 227 * 1024, "shared memory budget");
 };
 
@@ -128,7 +135,7 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                         const int st = step % C::NSTAGE;
                         tc::mbar_wait(&b_empty[st], ((step / C::NSTAGE) & 1) ^ 1);
                         mbar_expect_tx(&b_full[st], C::B_STAGE);
-                        bulk_g2s(sbase + C::OFF_B + st * C::B_STAGE, Bw + ((long)nt * C::NKC + kc) * (KC * C::BN), C::B_STAGE, &b_full[st]);
+                        bulk_g2s(sbase + C::OFF_B + st * C::B_STAGE, Bw + ((long)nt * C::NKC + kc) * (C::KCH * C::BN), C::B_STAGE, &b_full[st]);
                     }
             }
         }
@@ -146,17 +153,17 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                         const int st = step % C::NSTAGE;
                         int ab;
                         if (C::RESIDENT) { ab = kc; tc::mbar_wait(&a_full[ab], it & 1); }
-                        else { ab = astep & 1; tc::mbar_wait(&a_full[ab], (astep >> 1) & 1); }
+                        else { ab = astep % C::NA; tc::mbar_wait(&a_full[ab], (astep / C::NA) & 1); }
                         tc::mbar_wait(&b_full[st], (step / C::NSTAGE) & 1);
                         tc::fence_after();
-                        const uint64_t da = tc::desc(sbase + C::OFF_A + ab * C::A_BUF, A_SUB_STRIDE, 128);
+                        const uint64_t da = tc::desc(sbase + C::OFF_A + ab * C::A_BUF, C::ASS, 128);
                         const uint64_t db = tc::desc(sbase + C::OFF_B + st * C::B_STAGE, C::BN * 16, 128);
                         if (tc::elect_one()) {
 #pragma unroll
                             for (int part = 0; part < 2; ++part)
 #pragma unroll
-                                for (int ks = 0; ks < KC / 16; ++ks)
-                                    tc::mma_ss(tmem + buf * C::TM_BUF, tc::desc_at(da, part * A_PART + ks * 2 * A_SUB_STRIDE),
+                                for (int ks = 0; ks < C::KCH / 16; ++ks)
+                                    tc::mma_ss(tmem + buf * C::TM_BUF, tc::desc_at(da, part * C::A_PARTC + ks * 2 * C::ASS),
                                                tc::desc_at(db, ks * 2 * (C::BN * 16)), idesc, (kc | part | ks) != 0);
                             tc::commit(&b_empty[st]);
                             if (!C::RESIDENT || nt == C::NTILES - 1) tc::commit(&a_empty[ab]);
@@ -179,10 +186,11 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
             // MODE 0: the A operand is the descriptor D[m*16 + a] = sum_c A[c][m] A[c][a] (S5), formed here from the
             // 4 x 100 matrix A_i (p.A, lda = 400): D never reaches memory.  Thread = (row, half of the axis range a).
             constexpr bool DESCR = MODE == 0;
-            const int dr = pt & (BM - 1), dah = pt >> 7;
+            const int dr = pt >> 1, dah = pt & 1;       // neighbouring lanes share a row: their loads coalesce in L1
             const bool drow_ok = row0 + dr < rend;
             const float *Ai = p.A + (long)(drow_ok ? row0 + dr : row0) * 400;
             float ax8[4][8];
+            float4 nx[4];                               // A_i[c][4 kc .. 4 kc + 3] of the next chunk (prefetched)
             if (DESCR) {
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
@@ -190,19 +198,32 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                     const float4 u1 = __ldg(reinterpret_cast<const float4 *>(Ai + c * 100 + 8 * dah + 4));
                     ax8[c][0] = u0.x; ax8[c][1] = u0.y; ax8[c][2] = u0.z; ax8[c][3] = u0.w;
                     ax8[c][4] = u1.x; ax8[c][5] = u1.y; ax8[c][6] = u1.z; ax8[c][7] = u1.w;
+                    nx[c] = u0;
+                }
+                if (dah) {
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) nx[c] = __ldg(reinterpret_cast<const float4 *>(Ai + c * 100));
                 }
             }
             for (int kc = 0; kc < C::NKC; ++kc, ++astep) {
+                float4 cur[4];
+                if (DESCR) {
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        cur[c] = nx[c];
+                        if (kc + 1 < C::NKC) nx[c] = __ldg(reinterpret_cast<const float4 *>(Ai + c * 100 + 4 * (kc + 1)));
+                    }
+                }
                 int ab;
                 if (C::RESIDENT) { ab = kc; tc::mbar_wait(&a_empty[ab], (it & 1) ^ 1); }
-                else { ab = astep & 1; tc::mbar_wait(&a_empty[ab], ((astep >> 1) & 1) ^ 1); }
+                else { ab = astep % C::NA; tc::mbar_wait(&a_empty[ab], ((astep / C::NA) & 1) ^ 1); }
                 uint8_t *img = smem + C::OFF_A + ab * C::A_BUF;
                 if (DESCR) {
-                    // chunk kc covers m = 5 kc .. 5 kc + 4 (KC / 16 = 5 values of m, 16 axis columns each)
+                    // chunk kc covers m = 4 kc .. 4 kc + 3 (KCH / 16 = 4 values of m, 16 axis columns each)
 #pragma unroll
-                    for (int mm = 0; mm < KC / 16; ++mm) {
-                        const int m = kc * (KC / 16) + mm;
-                        const float a0 = __ldg(Ai + m), a1 = __ldg(Ai + 100 + m), a2 = __ldg(Ai + 200 + m), a3 = __ldg(Ai + 300 + m);
+                    for (int mm = 0; mm < C::KCH / 16; ++mm) {
+                        const float a0 = reinterpret_cast<const float *>(&cur[0])[mm], a1 = reinterpret_cast<const float *>(&cur[1])[mm];
+                        const float a2 = reinterpret_cast<const float *>(&cur[2])[mm], a3 = reinterpret_cast<const float *>(&cur[3])[mm];
                         float d[8];
 #pragma unroll
                         for (int j = 0; j < 8; ++j)
@@ -211,25 +232,25 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                         tc::split_h2(d[0], d[1], hi.x, lo.x); tc::split_h2(d[2], d[3], hi.y, lo.y);
                         tc::split_h2(d[4], d[5], hi.z, lo.z); tc::split_h2(d[6], d[7], hi.w, lo.w);
                         const int sub = 2 * mm + dah;
-                        *reinterpret_cast<uint4 *>(img + sub * A_SUB_STRIDE + dr * 16) = hi;
-                        *reinterpret_cast<uint4 *>(img + A_PART + sub * A_SUB_STRIDE + dr * 16) = lo;
+                        *reinterpret_cast<uint4 *>(img + sub * C::ASS + dr * 16) = hi;
+                        *reinterpret_cast<uint4 *>(img + C::A_PARTC + sub * C::ASS + dr * 16) = lo;
                     }
                 }
                 // item = (row, sub-chunk): 8 consecutive fp32 -> one 16-byte hi chunk and one lo chunk
 #pragma unroll
-                for (int j = 0; j < (DESCR ? 0 : BM * SUB / NPROD); ++j) {
+                for (int j = 0; j < (DESCR ? 0 : BM * C::SUBS / NPROD); ++j) {
                     const int idx = pt + j * NPROD;
-                    const int r = idx / SUB, sub = idx % SUB;
+                    const int r = idx / C::SUBS, sub = idx % C::SUBS;
                     float4 x0 = make_float4(0.f, 0.f, 0.f, 0.f), x1 = x0;
                     if (row0 + r < rend) {
-                        const float4 *src = reinterpret_cast<const float4 *>(p.A + (long)(row0 + r) * p.lda + kc * KC + sub * 8);
+                        const float4 *src = reinterpret_cast<const float4 *>(p.A + (long)(row0 + r) * p.lda + kc * C::KCH + sub * 8);
                         x0 = __ldg(src); x1 = __ldg(src + 1);
                     }
                     uint4 hi, lo;
                     tc::split_h2(x0.x, x0.y, hi.x, lo.x); tc::split_h2(x0.z, x0.w, hi.y, lo.y);
                     tc::split_h2(x1.x, x1.y, hi.z, lo.z); tc::split_h2(x1.z, x1.w, hi.w, lo.w);
-                    *reinterpret_cast<uint4 *>(img + sub * A_SUB_STRIDE + r * 16) = hi;
-                    *reinterpret_cast<uint4 *>(img + A_PART + sub * A_SUB_STRIDE + r * 16) = lo;
+                    *reinterpret_cast<uint4 *>(img + sub * C::ASS + r * 16) = hi;
+                    *reinterpret_cast<uint4 *>(img + C::A_PARTC + sub * C::ASS + r * 16) = lo;
                 }
                 tc::proxy_fence();
                 __syncwarp();
