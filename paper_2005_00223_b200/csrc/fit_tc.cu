@@ -8,6 +8,7 @@
 //                 (activations are carried as hi + lo pairs: single-precision activations on fp16 tensor cores)
 //   warps 10-13 : epilogue: tcgen05.ld, bias / tanh / residual / tanh' per MODE, fp32 results to global memory
 // K = 1600 (first layer) streams A and B chunk by chunk; K = 240 keeps the A tile resident and streams B over the N tiles.
+#include <cstdio>
 #include <cuda_fp16.h>
 #include "dp_internal.h"
 #include "tc_common.cuh"
@@ -20,7 +21,7 @@ constexpr int SUB = KC / 8;               // 16-byte sub-chunks per K chunk
 constexpr int A_SUB_STRIDE = BM * 16 + 16;   // bytes between sub-chunks of the A image (+16: conflict-free producer stores)
 constexpr int A_PART = SUB * A_SUB_STRIDE;   // one part (hi or lo) of one K chunk
 // producer threads (MODE 6 produces its resident A tile once per row tile: fewer producers leave registers to its epilogue)
-__host__ __device__ constexpr int nprod(int mode) { return mode == 6 ? 128 : 256; }
+__host__ __device__ constexpr int nprod(int mode) { return mode == 6 ? 64 : 256; }
 // epilogue threads: two per row.  MODE 6 (gA in the epilogue): each owns two of the four components c; other modes: each owns
 // every other group of 16 columns (the epilogues are bound by the latency of their global loads: twice the loads in flight)
 __host__ __device__ constexpr int nepi(int mode) { return 256; }
@@ -93,6 +94,12 @@ __device__ __forceinline__ bool tile_rows(const FitTcArgs &p, int tile, int &a, 
 //   5: out0 = acc                                                (gD)
 //   6: gD is consumed in registers: out0[row][c][m] = gA[c][m] = sum_a gD[m][a] A[c][a] + [m < 16] sum_m' gD[m'][m] A[c][m']
 //      (aux0 = A [rows][4][100]); the gD tensor never reaches memory
+#ifdef DP_FIT_TIMING
+__device__ long long fit_dbg[8];
+#define FT(i) do { long long n_ = clock64(); if (blockIdx.x == 0) ft[i] += n_ - ftl; ftl = n_; } while (0)
+#else
+#define FT(i) do { } while (0)
+#endif
 template <int MODE, int KTOT, int NTOT, bool APPROX>
 __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
     constexpr int NEPI = nepi(MODE), NPROD = nprod(MODE);
@@ -144,18 +151,25 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
         {
             constexpr uint32_t idesc = tc::idesc(128, C::BN, false, false);
             uint32_t step = 0, astep = 0, accn = 0, it = 0;
+#ifdef DP_FIT_TIMING
+            long long ft[8] = {0, 0, 0, 0, 0, 0, 0, 0}, ftl = clock64();
+#endif
             for (int tile = blockIdx.x; tile < ntiles_total; tile += gridDim.x, ++it) {
                 for (int nt = 0; nt < C::NTILES; ++nt, ++accn) {
                     const int buf = accn & 1;
+                    FT(0);
                     tc::mbar_wait(&acc_empty[buf], ((accn >> 1) & 1) ^ 1);
                     tc::fence_after();
+                    FT(1);
                     for (int kc = 0; kc < C::NKC; ++kc, ++step) {
                         const int st = step % C::NSTAGE;
                         int ab;
                         if (C::RESIDENT) { ab = kc; tc::mbar_wait(&a_full[ab], it & 1); }
                         else { ab = astep % C::NA; tc::mbar_wait(&a_full[ab], (astep / C::NA) & 1); }
+                        FT(2);
                         tc::mbar_wait(&b_full[st], (step / C::NSTAGE) & 1);
                         tc::fence_after();
+                        FT(3);
                         const uint64_t da = tc::desc(sbase + C::OFF_A + ab * C::A_BUF, C::ASS, 128);
                         const uint64_t db = tc::desc(sbase + C::OFF_B + st * C::B_STAGE, C::BN * 16, 128);
                         if (tc::elect_one()) {
@@ -169,17 +183,24 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                             if (!C::RESIDENT || nt == C::NTILES - 1) tc::commit(&a_empty[ab]);
                         }
                         __syncwarp();
+                        FT(4);
                         if (!C::RESIDENT) ++astep;
                     }
                     if (tc::elect_one()) tc::commit(&acc_full[buf]);
                     __syncwarp();
                 }
             }
+#ifdef DP_FIT_TIMING
+            if (blockIdx.x == 0 && lane == 0) for (int k = 0; k < 5; ++k) fit_dbg[k] = ft[k];
+#endif
         }
     } else if (warp < 2 + NPROD / 32) {
         // ---------------------------------------------------------------- A producers
         const int pt = tid - 64;
         uint32_t astep = 0, it = 0;
+#ifdef DP_FIT_TIMING
+        long long ft[8] = {0, 0, 0, 0, 0, 0, 0, 0}, ftl = clock64();
+#endif
         for (int tile = blockIdx.x; tile < ntiles_total; tile += gridDim.x, ++it) {
             int a, row0, rend;
             tile_rows(p, tile, a, row0, rend);
@@ -215,8 +236,10 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                     }
                 }
                 int ab;
+                FT(5);
                 if (C::RESIDENT) { ab = kc; tc::mbar_wait(&a_empty[ab], (it & 1) ^ 1); }
                 else { ab = astep % C::NA; tc::mbar_wait(&a_empty[ab], ((astep / C::NA) & 1) ^ 1); }
+                FT(6);
                 uint8_t *img = smem + C::OFF_A + ab * C::A_BUF;
                 if (DESCR) {
                     // chunk kc covers m = 4 kc .. 4 kc + 3 (KCH / 16 = 4 values of m, 16 axis columns each)
@@ -257,6 +280,10 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                 if (lane == 0) mbar_arrive(&a_full[ab]);
             }
         }
+#ifdef DP_FIT_TIMING
+        FT(5);
+        if (blockIdx.x == 0 && tid == 64) { fit_dbg[5] = ft[5]; fit_dbg[6] = ft[6]; }
+#endif
     } else {
         // ---------------------------------------------------------------- epilogue (thread = row)
         const int q = warp & 3, r = q * 32 + lane;
@@ -282,38 +309,49 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                         a16[c][4 * k4] = v.x; a16[c][4 * k4 + 1] = v.y; a16[c][4 * k4 + 2] = v.z; a16[c][4 * k4 + 3] = v.w;
                         acc2[c][4 * k4] = acc2[c][4 * k4 + 1] = acc2[c][4 * k4 + 2] = acc2[c][4 * k4 + 3] = 0.f;
                     }
-                float4 am0 = make_float4(0.f, 0.f, 0.f, 0.f), am1 = am0, go0 = am0, go1 = am0;
+                // A_i[c][m .. m + 3] is loaded one group of four m ahead of its use, the accumulator columns one group of 16 ahead
+                float4 am0, am1, an0, an1, go0 = make_float4(0.f, 0.f, 0.f, 0.f), go1 = go0;
+                an0 = __ldg(reinterpret_cast<const float4 *>(Arow));
+                an1 = __ldg(reinterpret_cast<const float4 *>(Arow + 100));
+                am0 = an0; am1 = an1;
                 for (int nt = 0; nt < C::NTILES; ++nt, ++accn) {
                     const int buf = accn & 1;
                     tc::mbar_wait(&acc_full[buf], (accn >> 1) & 1);
                     tc::fence_after();
+                    uint32_t v[2][16];
+                    tc::ld16(tm_lane + buf * C::TM_BUF, v[0]);
 #pragma unroll
                     for (int mm = 0; mm < C::BN / 16; ++mm) {
                         const int m = nt * (C::BN / 16) + mm;            // BN / 16 = 10: the unrolled mm gives m & 3 statically per nt parity
-                        uint32_t v[16];
-                        tc::ld16(tm_lane + buf * C::TM_BUF + 16 * mm, v);
                         if ((m & 3) == 0) {
-                            am0 = __ldg(reinterpret_cast<const float4 *>(Arow + m));
-                            am1 = __ldg(reinterpret_cast<const float4 *>(Arow + 100 + m));
+                            am0 = an0; am1 = an1;
+                            if (m + 4 < 100) {
+                                an0 = __ldg(reinterpret_cast<const float4 *>(Arow + m + 4));
+                                an1 = __ldg(reinterpret_cast<const float4 *>(Arow + 100 + m + 4));
+                            }
                         }
                         tc::wait_ld();
+                        if (mm + 1 < C::BN / 16) tc::ld16(tm_lane + buf * C::TM_BUF + 16 * (mm + 1), v[(mm + 1) & 1]);
                         const float a0 = (m & 3) == 0 ? am0.x : (m & 3) == 1 ? am0.y : (m & 3) == 2 ? am0.z : am0.w;
                         const float a1 = (m & 3) == 0 ? am1.x : (m & 3) == 1 ? am1.y : (m & 3) == 2 ? am1.z : am1.w;
                         float g0 = 0.f, g1 = 0.f;
 #pragma unroll
                         for (int ax = 0; ax < 16; ++ax) {
-                            const float gd = __uint_as_float(v[ax]);
+                            const float gd = __uint_as_float(v[mm & 1][ax]);
                             g0 = fmaf(gd, a16[0][ax], g0);
                             g1 = fmaf(gd, a16[1][ax], g1);
                             acc2[0][ax] = fmaf(gd, a0, acc2[0][ax]);
                             acc2[1][ax] = fmaf(gd, a1, acc2[1][ax]);
                         }
+                        // m < 16: the first term joins the second one in registers (written once, after the last N tile)
+                        if (nt == 0) { acc2[0][mm] += g0; acc2[1][mm] += g1; }
+                        else if (nt == 1 && mm < 16 - C::BN / 16) { acc2[0][(C::BN / 16 + mm) & 15] += g0; acc2[1][(C::BN / 16 + mm) & 15] += g1; }
                         if ((m & 3) == 0) { go0.x = g0; go1.x = g1; }
                         else if ((m & 3) == 1) { go0.y = g0; go1.y = g1; }
                         else if ((m & 3) == 2) { go0.z = g0; go1.z = g1; }
                         else {
                             go0.w = g0; go1.w = g1;
-                            if (ok) {
+                            if (ok && m >= 16) {
                                 *reinterpret_cast<float4 *>(Grow + m - 3) = go0;
                                 *reinterpret_cast<float4 *>(Grow + 100 + m - 3) = go1;
                             }
@@ -327,7 +365,9 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
 #pragma unroll
                     for (int c = 0; c < 2; ++c)
 #pragma unroll
-                        for (int ax = 0; ax < 16; ++ax) Grow[c * 100 + ax] += acc2[c][ax];
+                        for (int k4 = 0; k4 < 4; ++k4)
+                            *reinterpret_cast<float4 *>(Grow + c * 100 + 4 * k4) =
+                                make_float4(acc2[c][4 * k4], acc2[c][4 * k4 + 1], acc2[c][4 * k4 + 2], acc2[c][4 * k4 + 3]);
                 }
                 continue;
             }
@@ -669,6 +709,17 @@ void launch(const FitTcArgs &p, int grid, cudaStream_t st) {
     static bool attr = false;
     if (!attr) { cudaFuncSetAttribute(k_fit_tc<MODE, KTOT, NTOT, APPROX>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::TOTAL); attr = true; }
     k_fit_tc<MODE, KTOT, NTOT, APPROX><<<grid, nthreads(MODE), C::TOTAL, st>>>(p);
+#ifdef DP_FIT_TIMING
+    {
+        cudaStreamSynchronize(st);
+        long long h[8];
+        cudaMemcpyFromSymbol(h, fit_dbg, sizeof(h));
+        long long tot = 0;
+        for (int k = 0; k < 5; ++k) tot += h[k];
+        fprintf(stderr, "fit_tc mode %d MMA warp cycles %lld: other %.1f%% acc_empty %.1f%% a_full %.1f%% b_full %.1f%% issue %.1f%%; producer: work %.1f%% wait a_empty %.1f%%\n", MODE, tot,
+                100.0 * h[0] / tot, 100.0 * h[1] / tot, 100.0 * h[2] / tot, 100.0 * h[3] / tot, 100.0 * h[4] / tot, 100.0 * h[5] / tot, 100.0 * h[6] / tot);
+    }
+#endif
 }
 
 }  // namespace
