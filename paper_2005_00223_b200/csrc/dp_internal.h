@@ -130,7 +130,7 @@ cudaError_t fit_tc_gemm(int mode, bool apx, const dp_model *m, const Grid3 &g, c
                         const float *bias, const float *v4, const float *aux0, const float *aux1, float *out0, float *out1,
                         int ldo, cudaStream_t st);
 cudaError_t fit_tc_chain(bool apx, const dp_model *m, const Grid3 &g, const int *bin_start, const float *h1, const float *c2,
-                         const float *c3, const float *v4, const float *c4, float *gz1, double *eatom, cudaStream_t st);
+                         const float *c3, const float *v4, const float *c4, float *gz1, uint8_t *gz1img, double *eatom, cudaStream_t st);
 size_t fit_tc_type_elems();
 void fit_tc_build_type(const double *V1, const double *V2, const double *V3, struct __half *out);
 cudaError_t launch_env_rows(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);

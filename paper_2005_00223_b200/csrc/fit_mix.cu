@@ -323,8 +323,12 @@ cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, 
     if (m->use_fit_tc) {      // tcgen05 GEMMs (fit_tc.cu), same products, buffers and epilogues
         fit_tc_gemm(0, apx, m, g, bin_start, Amat, 4 * M2E, c1, nullptr, nullptr, nullptr, h1, nullptr, F, st);
         static const bool unfused = std::getenv("DP_FIT_UNFUSED") != nullptr;
+        // fused path with the gA epilogue: gz1 goes to the last product as ready-made hi + lo fp16 tile images (they fit in the
+        // unused activation buffers 2 S .. 4 S: 967.5 bytes per row plus one tile per type)
+        const bool gz_img = !unfused && m->use_tc_bwd;
         if (!unfused) {      // the four 240 x 240 products and the energy in one kernel
-            fit_tc_chain(apx, m, g, bin_start, h1, c2, c3, v4, c4, gz1, (double *)(ws + L.eatom), st);
+            fit_tc_chain(apx, m, g, bin_start, h1, c2, c3, v4, c4, gz1, gz_img ? reinterpret_cast<uint8_t *>(gz1) : nullptr,
+                         (double *)(ws + L.eatom), st);
         } else {
         fit_tc_gemm(1, apx, m, g, bin_start, h1, F, c2, nullptr, h1, nullptr, t2, h2, F, st);
         fit_tc_gemm(2, false, m, g, bin_start, h2, F, c3, v4, h2, nullptr, gz3, h3, F, st);
@@ -333,7 +337,7 @@ cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, 
         fit_tc_gemm(4, false, m, g, bin_start, gz2, F, nullptr, nullptr, g2, h1, gz1, nullptr, F, st);
         }
         if (m->use_tc_bwd)   // gA in the epilogue: D receives gA [N][4][100], the gD tensor is never written
-            fit_tc_gemm(6, false, m, g, bin_start, gz1, F, nullptr, nullptr, Amat, nullptr, D, nullptr, ND, st);
+            fit_tc_gemm(6, false, m, g, bin_start, gz_img ? nullptr : gz1, F, nullptr, nullptr, Amat, gz_img ? gz1 : nullptr, D, nullptr, ND, st);
         else
             fit_tc_gemm(5, false, m, g, bin_start, gz1, F, nullptr, nullptr, nullptr, nullptr, D, nullptr, ND, st);
     } else {

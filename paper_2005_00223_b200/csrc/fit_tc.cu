@@ -20,8 +20,11 @@ constexpr int KC = 80;                    // K chunk: 5 k-steps of 16
 constexpr int SUB = KC / 8;               // 16-byte sub-chunks per K chunk
 constexpr int A_SUB_STRIDE = BM * 16 + 16;   // bytes between sub-chunks of the A image (+16: conflict-free producer stores)
 constexpr int A_PART = SUB * A_SUB_STRIDE;   // one part (hi or lo) of one K chunk
+// gz1 as the tcgen05 A operand of the last product, written by k_fit_chain tile by tile in the shared-memory layout of
+// k_fit_tc<6>: [K chunk 3][hi, lo][sub-chunk 10][row 128 (+ pad)][16 B]; one cp.async.bulk per K chunk brings it in
+constexpr int GZ_TILE_BYTES = 3 * 2 * A_PART;
 // producer threads (MODE 6 produces its resident A tile once per row tile: fewer producers leave registers to its epilogue)
-__host__ __device__ constexpr int nprod(int mode) { return mode == 6 ? 64 : 256; }
+__host__ __device__ constexpr int nprod(int mode) { return mode == 6 ? 32 : 256; }
 // epilogue threads: two per row.  MODE 6 (gA in the epilogue): each owns two of the four components c; other modes: each owns
 // every other group of 16 columns (the epilogues are bound by the latency of their global loads: twice the loads in flight)
 __host__ __device__ constexpr int nepi(int mode) { return 256; }
@@ -57,6 +60,7 @@ struct FitTcArgs {
     int T, ncell;
     const int *bin_start;
     const float *A; int lda;
+    const uint8_t *Aimg;                         // MODE 6: the A operand as pre-built hi + lo fp16 tile images (k_fit_chain), or null
     const __half *Bimg; long b_type_stride;      // elements per type
     const float *bias; const float *v4;          // [T][240]
     const float *aux0; const float *aux1;
@@ -204,6 +208,16 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
         for (int tile = blockIdx.x; tile < ntiles_total; tile += gridDim.x, ++it) {
             int a, row0, rend;
             tile_rows(p, tile, a, row0, rend);
+            if (MODE == 6 && p.Aimg) {      // the operand image exists already: one bulk copy per K chunk
+                if (lane == 0)
+                    for (int kc = 0; kc < C::NKC; ++kc) {
+                        tc::mbar_wait(&a_empty[kc], (it & 1) ^ 1);
+                        mbar_expect_tx(&a_full[kc], C::A_BUF);
+                        bulk_g2s(sbase + C::OFF_A + kc * C::A_BUF, p.Aimg + (size_t)tile * GZ_TILE_BYTES + kc * C::A_BUF, C::A_BUF, &a_full[kc]);
+                    }
+                __syncwarp();
+                continue;
+            }
             // MODE 0: the A operand is the descriptor D[m*16 + a] = sum_c A[c][m] A[c][a] (S5), formed here from the
             // 4 x 100 matrix A_i (p.A, lda = 400): D never reaches memory.  Thread = (row, half of the axis range a).
             constexpr bool DESCR = MODE == 0;
@@ -470,7 +484,8 @@ struct FitChainArgs {
     const __half *Bimg; long b_type_stride;
     const float *c2, *c3, *v4, *c4;       // [T][240], c4 [T]
     const double *ebias;                  // [T]
-    float *gz1;                           // [rows][240]
+    float *gz1;                           // [rows][240] (fp32), or
+    uint8_t *gz1img;                      // per 128-row tile the hi + lo fp16 operand image of the last product (GZ_TILE_BYTES)
     double *eatom;                        // [rows]
 };
 constexpr int CH_THREADS = 64 + 256;
@@ -682,6 +697,7 @@ __global__ void __launch_bounds__(CH_THREADS, 1) k_fit_chain(FitChainArgs p) {
             // ---- S4: gh1 = acc (= gh2 + gz2 V2^T); gz1 = gh1 (1 - h1^2) -> global ----
             wait_acc();
             float *gzrow = p.gz1 + (long)(row0 + r) * 240 + 120 * hc;
+            uint8_t *gzimg = p.gz1img + (size_t)tile * GZ_TILE_BYTES + r * 16;
 #pragma unroll
             for (int j = 0; j < 15; ++j) {
                 uint32_t v[8];
@@ -689,8 +705,16 @@ __global__ void __launch_bounds__(CH_THREADS, 1) k_fit_chain(FitChainArgs p) {
                 tc::wait_ld();
                 float x[8];
 #pragma unroll
-                for (int q = 0; q < 8; ++q) x[q] = __uint_as_float(v[q]) * fmaf(-H[8 * j + q], H[8 * j + q], 1.f);
-                if (ok) {
+                for (int q = 0; q < 8; ++q) x[q] = ok ? __uint_as_float(v[q]) * fmaf(-H[8 * j + q], H[8 * j + q], 1.f) : 0.f;
+                if (p.gz1img) {
+                    const int g = 15 * hc + j, kc = g / SUB, sub = g % SUB;
+                    uint4 hi, lo;
+                    tc::split_h2(x[0], x[1], hi.x, lo.x); tc::split_h2(x[2], x[3], hi.y, lo.y);
+                    tc::split_h2(x[4], x[5], hi.z, lo.z); tc::split_h2(x[6], x[7], hi.w, lo.w);
+                    uint8_t *dst = gzimg + kc * 2 * A_PART + sub * A_SUB_STRIDE;
+                    *reinterpret_cast<uint4 *>(dst) = hi;
+                    *reinterpret_cast<uint4 *>(dst + A_PART) = lo;
+                } else if (ok) {
                     *reinterpret_cast<float4 *>(gzrow + 8 * j) = make_float4(x[0], x[1], x[2], x[3]);
                     *reinterpret_cast<float4 *>(gzrow + 8 * j + 4) = make_float4(x[4], x[5], x[6], x[7]);
                 }
@@ -761,6 +785,7 @@ cudaError_t fit_tc_gemm(int mode, bool apx, const dp_model *m, const Grid3 &g, c
     p.T = m->T; p.ncell = g.ncell; p.bin_start = bin_start; p.A = A; p.lda = lda;
     p.Bimg = (const __half *)m->fit_tc_img_dev + FIT_TC_OFF[mode > 5 ? 5 : mode]; p.b_type_stride = (long)FIT_TC_OFF[6];
     p.bias = bias; p.v4 = v4; p.aux0 = aux0; p.aux1 = aux1; p.out0 = out0; p.out1 = out1; p.ldo = ldo;
+    if (mode == 6 && A == nullptr) { p.Aimg = reinterpret_cast<const uint8_t *>(aux1); p.aux1 = nullptr; }   // operand image from k_fit_chain
     const int grid = m->num_sms;
     switch (mode) {
         case 0: if (apx) launch<0, 1600, 240, true>(p, grid, st); else launch<0, 1600, 240, false>(p, grid, st); break;
@@ -776,11 +801,11 @@ cudaError_t fit_tc_gemm(int mode, bool apx, const dp_model *m, const Grid3 &g, c
 
 // layers 2-3 forward, energy, and their backward in one kernel (k_fit_chain)
 cudaError_t fit_tc_chain(bool apx, const dp_model *m, const Grid3 &g, const int *bin_start, const float *h1, const float *c2,
-                         const float *c3, const float *v4, const float *c4, float *gz1, double *eatom, cudaStream_t st) {
+                         const float *c3, const float *v4, const float *c4, float *gz1, uint8_t *gz1img, double *eatom, cudaStream_t st) {
     FitChainArgs p{};
     p.T = m->T; p.ncell = g.ncell; p.bin_start = bin_start; p.h1 = h1;
     p.Bimg = (const __half *)m->fit_tc_img_dev; p.b_type_stride = (long)FIT_TC_OFF[6];
-    p.c2 = c2; p.c3 = c3; p.v4 = v4; p.c4 = c4; p.ebias = m->ebias_dev; p.gz1 = gz1; p.eatom = eatom;
+    p.c2 = c2; p.c3 = c3; p.v4 = v4; p.c4 = c4; p.ebias = m->ebias_dev; p.gz1 = gz1; p.gz1img = gz1img; p.eatom = eatom;
     static bool attr = false;
     if (!attr) {
         cudaFuncSetAttribute(k_fit_chain<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, CH_TOTAL);
