@@ -25,9 +25,9 @@ constexpr int A_PART = SUB * A_SUB_STRIDE;   // one part (hi or lo) of one K chu
 constexpr int GZ_TILE_BYTES = 3 * 2 * A_PART;
 // producer threads (MODE 6 produces its resident A tile once per row tile: fewer producers leave registers to its epilogue)
 __host__ __device__ constexpr int nprod(int mode) { return mode == 6 ? 32 : 256; }
-// epilogue threads: two per row.  MODE 6 (gA in the epilogue): each owns two of the four components c; other modes: each owns
-// every other group of 16 columns (the epilogues are bound by the latency of their global loads: twice the loads in flight)
-__host__ __device__ constexpr int nepi(int mode) { return 256; }
+// epilogue threads.  MODE 6 (gA in the epilogue): four per row, one per component c; other modes: two per row, each owns
+// every other group of 16 columns (the epilogues are bound by the latency of their loads: more of them in flight)
+__host__ __device__ constexpr int nepi(int mode) { return mode == 6 ? 512 : 256; }
 __host__ __device__ constexpr int nthreads(int mode) { return 64 + nprod(mode) + nepi(mode); }
 
 template <int KTOT, int NTOT>
@@ -310,24 +310,22 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
             const float *bias = p.bias ? p.bias + a * 240 : nullptr;
             const float *v4 = p.v4 ? p.v4 + a * 240 : nullptr;
             if (MODE == 6) {
-                // thread (row, ch): components c = 2 ch, 2 ch + 1.  Per 16 accumulator columns = gD[m][0..16) of one m.
-                const int ch = ((warp - 2 - NPROD / 32) >> 2) & 1;
-                const float *Arow = p.aux0 + (long)(ok ? row0 + r : row0) * 400 + 2 * ch * 100;
-                float *Grow = p.out0 + (long)(row0 + r) * 400 + 2 * ch * 100;
-                float a16[2][16], acc2[2][16];
+                // thread (row, c): one of the four components.  Per 16 accumulator columns = gD[m][0..16) of one m.
+                // (four threads per row: the epilogue is bound by its load-to-use latencies, not by the FMA pipe)
+                const int c = ((warp - 2 - NPROD / 32) >> 2) & 3;
+                const float *Arow = p.aux0 + (long)(ok ? row0 + r : row0) * 400 + c * 100;
+                float *Grow = p.out0 + (long)(row0 + r) * 400 + c * 100;
+                float a16[16], acc2[16];
 #pragma unroll
-                for (int c = 0; c < 2; ++c)
-#pragma unroll
-                    for (int k4 = 0; k4 < 4; ++k4) {
-                        const float4 v = __ldg(reinterpret_cast<const float4 *>(Arow + c * 100) + k4);
-                        a16[c][4 * k4] = v.x; a16[c][4 * k4 + 1] = v.y; a16[c][4 * k4 + 2] = v.z; a16[c][4 * k4 + 3] = v.w;
-                        acc2[c][4 * k4] = acc2[c][4 * k4 + 1] = acc2[c][4 * k4 + 2] = acc2[c][4 * k4 + 3] = 0.f;
-                    }
+                for (int k4 = 0; k4 < 4; ++k4) {
+                    const float4 v = __ldg(reinterpret_cast<const float4 *>(Arow) + k4);
+                    a16[4 * k4] = v.x; a16[4 * k4 + 1] = v.y; a16[4 * k4 + 2] = v.z; a16[4 * k4 + 3] = v.w;
+                    acc2[4 * k4] = acc2[4 * k4 + 1] = acc2[4 * k4 + 2] = acc2[4 * k4 + 3] = 0.f;
+                }
                 // A_i[c][m .. m + 3] is loaded one group of four m ahead of its use, the accumulator columns one group of 16 ahead
-                float4 am0, am1, an0, an1, go0 = make_float4(0.f, 0.f, 0.f, 0.f), go1 = go0;
+                float4 am0, an0, go0 = make_float4(0.f, 0.f, 0.f, 0.f);
                 an0 = __ldg(reinterpret_cast<const float4 *>(Arow));
-                an1 = __ldg(reinterpret_cast<const float4 *>(Arow + 100));
-                am0 = an0; am1 = an1;
+                am0 = an0;
                 for (int nt = 0; nt < C::NTILES; ++nt, ++accn) {
                     const int buf = accn & 1;
                     tc::mbar_wait(&acc_full[buf], (accn >> 1) & 1);
@@ -338,37 +336,31 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                     for (int mm = 0; mm < C::BN / 16; ++mm) {
                         const int m = nt * (C::BN / 16) + mm;            // BN / 16 = 10: the unrolled mm gives m & 3 statically per nt parity
                         if ((m & 3) == 0) {
-                            am0 = an0; am1 = an1;
-                            if (m + 4 < 100) {
-                                an0 = __ldg(reinterpret_cast<const float4 *>(Arow + m + 4));
-                                an1 = __ldg(reinterpret_cast<const float4 *>(Arow + 100 + m + 4));
-                            }
+                            am0 = an0;
+                            if (m + 4 < 100) an0 = __ldg(reinterpret_cast<const float4 *>(Arow + m + 4));
                         }
                         tc::wait_ld();
                         if (mm + 1 < C::BN / 16) tc::ld16(tm_lane + buf * C::TM_BUF + 16 * (mm + 1), v[(mm + 1) & 1]);
                         const float a0 = (m & 3) == 0 ? am0.x : (m & 3) == 1 ? am0.y : (m & 3) == 2 ? am0.z : am0.w;
-                        const float a1 = (m & 3) == 0 ? am1.x : (m & 3) == 1 ? am1.y : (m & 3) == 2 ? am1.z : am1.w;
-                        float g0 = 0.f, g1 = 0.f;
+                        float g0 = 0.f, g1 = 0.f;      // two partial sums: half the dependent-FMA chain
 #pragma unroll
-                        for (int ax = 0; ax < 16; ++ax) {
-                            const float gd = __uint_as_float(v[mm & 1][ax]);
-                            g0 = fmaf(gd, a16[0][ax], g0);
-                            g1 = fmaf(gd, a16[1][ax], g1);
-                            acc2[0][ax] = fmaf(gd, a0, acc2[0][ax]);
-                            acc2[1][ax] = fmaf(gd, a1, acc2[1][ax]);
+                        for (int ax = 0; ax < 16; ax += 2) {
+                            const float gd0 = __uint_as_float(v[mm & 1][ax]), gd1 = __uint_as_float(v[mm & 1][ax + 1]);
+                            g0 = fmaf(gd0, a16[ax], g0);
+                            g1 = fmaf(gd1, a16[ax + 1], g1);
+                            acc2[ax] = fmaf(gd0, a0, acc2[ax]);
+                            acc2[ax + 1] = fmaf(gd1, a0, acc2[ax + 1]);
                         }
+                        g0 += g1;
                         // m < 16: the first term joins the second one in registers (written once, after the last N tile)
-                        if (nt == 0) { acc2[0][mm] += g0; acc2[1][mm] += g1; }
-                        else if (nt == 1 && mm < 16 - C::BN / 16) { acc2[0][(C::BN / 16 + mm) & 15] += g0; acc2[1][(C::BN / 16 + mm) & 15] += g1; }
-                        if ((m & 3) == 0) { go0.x = g0; go1.x = g1; }
-                        else if ((m & 3) == 1) { go0.y = g0; go1.y = g1; }
-                        else if ((m & 3) == 2) { go0.z = g0; go1.z = g1; }
+                        if (nt == 0) acc2[mm] += g0;
+                        else if (nt == 1 && mm < 16 - C::BN / 16) acc2[(C::BN / 16 + mm) & 15] += g0;
+                        if ((m & 3) == 0) go0.x = g0;
+                        else if ((m & 3) == 1) go0.y = g0;
+                        else if ((m & 3) == 2) go0.z = g0;
                         else {
-                            go0.w = g0; go1.w = g1;
-                            if (ok && m >= 16) {
-                                *reinterpret_cast<float4 *>(Grow + m - 3) = go0;
-                                *reinterpret_cast<float4 *>(Grow + 100 + m - 3) = go1;
-                            }
+                            go0.w = g0;
+                            if (ok && m >= 16) *reinterpret_cast<float4 *>(Grow + m - 3) = go0;
                         }
                     }
                     tc::fence_before();
@@ -377,11 +369,8 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                 }
                 if (ok) {
 #pragma unroll
-                    for (int c = 0; c < 2; ++c)
-#pragma unroll
-                        for (int k4 = 0; k4 < 4; ++k4)
-                            *reinterpret_cast<float4 *>(Grow + c * 100 + 4 * k4) =
-                                make_float4(acc2[c][4 * k4], acc2[c][4 * k4 + 1], acc2[c][4 * k4 + 2], acc2[c][4 * k4 + 3]);
+                    for (int k4 = 0; k4 < 4; ++k4)
+                        *reinterpret_cast<float4 *>(Grow + 4 * k4) = make_float4(acc2[4 * k4], acc2[4 * k4 + 1], acc2[4 * k4 + 2], acc2[4 * k4 + 3]);
                 }
                 continue;
             }
