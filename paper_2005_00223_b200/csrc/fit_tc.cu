@@ -224,15 +224,15 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
             const int dr = pt >> 1, dah = pt & 1;       // neighbouring lanes share a row: their loads coalesce in L1
             const bool drow_ok = row0 + dr < rend;
             const float *Ai = p.A + (long)(drow_ok ? row0 + dr : row0) * 400;
-            float ax8[4][8];
+            tc::f32x2 axp[4][4];                        // A_i[c][8 dah + 2 jp, + 1] as packed pairs
             float4 nx[4];                               // A_i[c][4 kc .. 4 kc + 3] of the next chunk (prefetched)
             if (DESCR) {
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
                     const float4 u0 = __ldg(reinterpret_cast<const float4 *>(Ai + c * 100 + 8 * dah));
                     const float4 u1 = __ldg(reinterpret_cast<const float4 *>(Ai + c * 100 + 8 * dah + 4));
-                    ax8[c][0] = u0.x; ax8[c][1] = u0.y; ax8[c][2] = u0.z; ax8[c][3] = u0.w;
-                    ax8[c][4] = u1.x; ax8[c][5] = u1.y; ax8[c][6] = u1.z; ax8[c][7] = u1.w;
+                    axp[c][0] = tc::pk2(u0.x, u0.y); axp[c][1] = tc::pk2(u0.z, u0.w);
+                    axp[c][2] = tc::pk2(u1.x, u1.y); axp[c][3] = tc::pk2(u1.z, u1.w);
                     nx[c] = u0;
                 }
                 if (dah) {
@@ -261,10 +261,14 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                     for (int mm = 0; mm < C::KCH / 16; ++mm) {
                         const float a0 = reinterpret_cast<const float *>(&cur[0])[mm], a1 = reinterpret_cast<const float *>(&cur[1])[mm];
                         const float a2 = reinterpret_cast<const float *>(&cur[2])[mm], a3 = reinterpret_cast<const float *>(&cur[3])[mm];
+                        const tc::f32x2 s0 = tc::pk2(a0, a0), s1 = tc::pk2(a1, a1), s2 = tc::pk2(a2, a2), s3 = tc::pk2(a3, a3);
                         float d[8];
 #pragma unroll
-                        for (int j = 0; j < 8; ++j)
-                            d[j] = drow_ok ? fmaf(a3, ax8[3][j], fmaf(a2, ax8[2][j], fmaf(a1, ax8[1][j], a0 * ax8[0][j]))) : 0.f;
+                        for (int jp = 0; jp < 4; ++jp) {
+                            const tc::f32x2 dp = tc::fma2(s3, axp[3][jp], tc::fma2(s2, axp[2][jp], tc::fma2(s1, axp[1][jp], tc::mul2(s0, axp[0][jp]))));
+                            tc::upk2(dp, d[2 * jp], d[2 * jp + 1]);
+                            if (!drow_ok) d[2 * jp] = d[2 * jp + 1] = 0.f;
+                        }
                         uint4 hi, lo;
                         tc::split_h2(d[0], d[1], hi.x, lo.x); tc::split_h2(d[2], d[3], hi.y, lo.y);
                         tc::split_h2(d[4], d[5], hi.z, lo.z); tc::split_h2(d[6], d[7], hi.w, lo.w);
