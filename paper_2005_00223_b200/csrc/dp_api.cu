@@ -32,6 +32,7 @@ WsLayout ws_layout(const dp_model *m, long N) {
     L.inv = take(sizeof(int) * (size_t)N);
     L.xs = take(sizeof(double) * 3 * (size_t)N);
     L.xsf = take(sizeof(float) * 4 * (size_t)N);
+    L.scan_tmp = take(sizeof(int) * 2 * ((nbins > (size_t)N ? nbins : (size_t)N) / 4096 + 4));
     L.xw = take(sizeof(double) * 3 * (size_t)N);
     L.nlist = take(sizeof(int) * (size_t)N * m->Nm);
     L.nreal = take(sizeof(int) * (size_t)N * m->T);
@@ -451,10 +452,10 @@ size_t dp_workspace_bytes(const dp_model *m, long natoms) {
 
 int dp_launches_per_compute(const dp_model *m) {
     if (!m) return 0;
-    // MIX-16 tcgen05 path: 4 binning + list + T row scans + env rows + forward + 3 fitting (first layer, fused 240 x 240 chain,
-    // last product with gA) + image fold + backward + force/virial + finalize
-    if (m->use_tc == 2 && m->use_tc_bwd && m->use_fit_tc) return 14 + m->T;
-    return 17;
+    // MIX-16 tcgen05 path: 6 binning (wrap, 3-launch bin scan, scatter, sort) + list + T row scans of 3 launches + env rows +
+    // forward + 3 fitting (first layer, fused 240 x 240 chain, last product with gA) + image fold + backward + force/virial + finalize
+    if (m->use_tc == 2 && m->use_tc_bwd && m->use_fit_tc) return 16 + 3 * m->T;
+    return 19;
 }
 
 int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *types_dev, const double *box_host,

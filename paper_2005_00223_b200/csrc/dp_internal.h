@@ -88,6 +88,7 @@ struct WsLayout {
     size_t xw;          // double[N][3] wrapped coords, user order
     size_t nlist;       // int[N][Nm] sorted-space indices
     size_t nreal;       // int[N][T]
+    size_t scan_tmp;    // scratch of the two-level scans
     size_t rowcnt;      // int[T][N]   rows per (neighbour type, atom): real + one padded-row representative (mixed modes)
     size_t rowstart;    // int[T][N+1] exclusive prefix of rowcnt over the sorted atoms
     size_t rows_rh;     // float4[T][N*sel_b...] compact env rows R^ (mixed modes, tcgen05 path)

@@ -86,6 +86,69 @@ __global__ void k_scan(int n, const int *__restrict__ cnt, int *__restrict__ sta
     if (threadIdx.x == 0) start[n] = carry;
 }
 
+// Two-level scan for long arrays: tile sums, the single-block scan above over the sums, then each tile scans itself.
+constexpr int SCAN_TILE = 4096;        // 1024 threads x 4 elements
+__global__ void __launch_bounds__(1024) k_scan_sums(int n, const int *__restrict__ cnt, int *__restrict__ sums) {
+    __shared__ int ws[32];
+    const int i0 = blockIdx.x * SCAN_TILE + 4 * threadIdx.x;
+    int v = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) v += i0 + k < n ? cnt[i0 + k] : 0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        v = ws[threadIdx.x];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (threadIdx.x == 0) sums[blockIdx.x] = v;
+    }
+}
+__global__ void __launch_bounds__(1024) k_scan_tiles(int n, const int *__restrict__ cnt, const int *__restrict__ tile_start,
+                                                      int *__restrict__ start) {
+    __shared__ int warp_sums[32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int i0 = blockIdx.x * SCAN_TILE + 4 * threadIdx.x;
+    int v[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) v[k] = i0 + k < n ? cnt[i0 + k] : 0;
+    const int tsum = v[0] + v[1] + v[2] + v[3];
+    int x = tsum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int y = __shfl_up_sync(0xffffffffu, x, o);
+        if (lane >= o) x += y;
+    }
+    if (lane == 31) warp_sums[wid] = x;
+    __syncthreads();
+    if (wid == 0) {
+        int s = warp_sums[lane];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int y = __shfl_up_sync(0xffffffffu, s, o);
+            if (lane >= o) s += y;
+        }
+        warp_sums[lane] = s;
+    }
+    __syncthreads();
+    int prefix = tile_start[blockIdx.x] + (wid ? warp_sums[wid - 1] : 0) + x - tsum;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        if (i0 + k < n) start[i0 + k] = prefix;
+        prefix += v[k];
+    }
+    if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) start[n] = tile_start[gridDim.x];
+}
+// exclusive scan of cnt[0..n) -> start[0..n] (three launches; tmp holds 2 * (n / SCAN_TILE + 2) ints)
+void launch_scan(int n, const int *cnt, int *start, int *tmp, cudaStream_t st) {
+    const int nt = (n + SCAN_TILE - 1) / SCAN_TILE;
+    int *sums = tmp, *tile_start = tmp + nt + 1;
+    k_scan_sums<<<nt, 1024, 0, st>>>(n, cnt, sums);
+    k_scan<<<1, 1024, 0, st>>>(nt, sums, tile_start);
+    k_scan_tiles<<<nt, 1024, 0, st>>>(n, cnt, tile_start, start);
+}
+
 __global__ void k_scatter(long N, const int *__restrict__ atom_bin, const int *__restrict__ bin_start,
                           int *__restrict__ cursor, int *__restrict__ tmp_order) {
     long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
@@ -466,7 +529,7 @@ cudaError_t launch_build_cells(const dp_model *m, long N, const double *coords, 
     const int nb = (int)((N + 255) / 256);
     k_wrap_bin<<<nb, 256, 0, st>>>(N, coords, types, m->type_map_dev, m->n_type_map, g, (double *)(ws + L.xw),
                                    (int *)(ws + L.atom_bin), cnt, status);
-    k_scan<<<1, 1024, 0, st>>>(nbins, cnt, start);
+    launch_scan(nbins, cnt, start, (int *)(ws + L.scan_tmp), st);
     k_scatter<<<nb, 256, 0, st>>>(N, (int *)(ws + L.atom_bin), start, cursor, (int *)(ws + L.tmp_order));
     k_bin_sort<<<nb, 256, 0, st>>>(N, (int *)(ws + L.atom_bin), start, (int *)(ws + L.tmp_order),
                                    (double *)(ws + L.xw), (int *)(ws + L.perm), (int *)(ws + L.inv),
@@ -507,7 +570,7 @@ cudaError_t launch_nlist(const dp_model *m, long N, const Grid3 &g, char *ws, co
                                                        (int *)(ws + L.status));
     if (m->prec != DP_FP64)
         for (int b = 0; b < m->T; ++b)
-            k_scan<<<1, 1024, 0, st>>>((int)N, (int *)(ws + L.rowcnt) + (long)b * N, (int *)(ws + L.rowstart) + (long)b * (N + 1));
+            launch_scan((int)N, (int *)(ws + L.rowcnt) + (long)b * N, (int *)(ws + L.rowstart) + (long)b * (N + 1), (int *)(ws + L.scan_tmp), st);
     return cudaGetLastError();
 }
 
