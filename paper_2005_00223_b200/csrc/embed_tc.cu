@@ -167,13 +167,22 @@ k_env_rows(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, EnvParams ep,
         const int nr = nreal[i * T + b];
         const int tot = nr + (nr < sel[b] ? 1 : 0);
         const long base = N * (long)off[b] + rowstart[(long)b * (N + 1) + i];
+        // software pipeline over the lane's rows: list entries two rows ahead, coordinates one row ahead of the arithmetic
+        const int *nl = nlist + i * Nm + off[b];
+        int jn0 = lane < nr ? nl[lane] : -1, jn1 = lane + 32 < nr ? nl[lane + 32] : -1;
+        double xn = 0.0, yn = 0.0, zn = 0.0;
+        if (jn0 >= 0) { xn = xs[3 * (long)jn0]; yn = xs[3 * (long)jn0 + 1]; zn = xs[3 * (long)jn0 + 2]; }
         for (int k = lane; k < tot; k += 32) {
+            const int j = jn0;
+            const double xj = xn, yj = yn, zj = zn;
+            jn0 = jn1;
+            jn1 = k + 64 < nr ? nl[k + 64] : -1;
+            if (jn0 >= 0) { xn = xs[3 * (long)jn0]; yn = xs[3 * (long)jn0 + 1]; zn = xs[3 * (long)jn0 + 2]; }
             double Rt[4] = {0.0, 0.0, 0.0, 0.0};
             if (k < nr) {
-                const int j = nlist[i * Nm + off[b] + k];
-                const double dx = min_image(xs[3 * (long)j] - xi, ep.L[0], hx);
-                const double dy = min_image(xs[3 * (long)j + 1] - yi, ep.L[1], hy);
-                const double dz = min_image(xs[3 * (long)j + 2] - zi, ep.L[2], hz);
+                const double dx = min_image(xj - xi, ep.L[0], hx);
+                const double dy = min_image(yj - yi, ep.L[1], hy);
+                const double dz = min_image(zj - zi, ep.L[2], hz);
                 // fp64 environment row with one reciprocal square root instead of a square root and four divisions
                 // (the result is rounded to fp32 below; PAPER.md:125 keeps the environment matrix in double)
                 const double r2 = dx * dx + dy * dy + dz * dz;
@@ -192,7 +201,7 @@ k_env_rows(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, EnvParams ep,
             }
             rows_rh[base + k] = make_float4((float)((Rt[0] - av[0]) * isd[0]), (float)((Rt[1] - av[1]) * isd[1]),
                                             (float)((Rt[2] - av[2]) * isd[2]), (float)((Rt[3] - av[3]) * isd[3]));
-            rows_id[base + k] = make_int2((int)i, k < nr ? nlist[i * Nm + off[b] + k] : -(sel[b] - nr));
+            rows_id[base + k] = make_int2((int)i, k < nr ? j : -(sel[b] - nr));
         }
     }
 }
