@@ -48,7 +48,9 @@ WsLayout ws_layout(const dp_model *m, long N) {
     if (m->prec == DP_FP64) L.gAf = take(sizeof(double) * (size_t)N * 3 * NT3 * 32);
     else L.gAf = take(sizeof(uint32_t) * (size_t)N * 2 * 28 * 32);
     L.gscale = take(sizeof(float) * (size_t)N);
-    L.fit_act = take(esz * (size_t)N * 240 * 7);
+    // (MIX-16: buffers 2..6 also hold the gz1 operand images, one per 128-row tile and at least one per type: the pad
+    // covers systems with fewer rows than a tile)
+    L.fit_act = take(esz * (size_t)N * 240 * 7 + (m->prec == DP_MIX16 ? ((size_t)m->T + 1) * FIT_GZ_TILE_BYTES : 0));
     L.gD = take(esz * (size_t)N * M2E * 16);
     L.eatom = take(sizeof(double) * (size_t)N);
     L.fsorted = take(sizeof(double) * 3 * (size_t)N);

@@ -11,6 +11,8 @@
 
 // ---------------------------------------------------------------- shapes fixed by this build (dp.h: widths (25,50,100))
 constexpr int M0 = 25, M1 = 50, M2E = 100;   // embedding widths
+// bytes of one 128-row hi + lo fp16 operand image of gz1 (fit_tc.cu: k_fit_chain -> k_fit_tc<6>)
+constexpr size_t FIT_GZ_TILE_BYTES = 3 * 2 * 10 * (128 * 16 + 16);
 constexpr int KC1 = 7;                       // ceil(M0/4) k-chunks of layer-1 output
 constexpr int NT2 = 7;                       // 8-wide tiles of layer-2 output (56 positions, 50 real)
 constexpr int NT3 = 14;                      // 8-wide tiles of layer-3 output (112 positions, 100 real)

@@ -23,6 +23,7 @@ constexpr int A_PART = SUB * A_SUB_STRIDE;   // one part (hi or lo) of one K chu
 // gz1 as the tcgen05 A operand of the last product, written by k_fit_chain tile by tile in the shared-memory layout of
 // k_fit_tc<6>: [K chunk 3][hi, lo][sub-chunk 10][row 128 (+ pad)][16 B]; one cp.async.bulk per K chunk brings it in
 constexpr int GZ_TILE_BYTES = 3 * 2 * A_PART;
+static_assert((size_t)GZ_TILE_BYTES == FIT_GZ_TILE_BYTES, "workspace layout (dp_api.cu) sizes the gz1 images");
 // producer threads (MODE 6 produces its resident A tile once per row tile: fewer producers leave registers to its epilogue)
 __host__ __device__ constexpr int nprod(int mode) { return mode == 6 ? 32 : 256; }
 // epilogue threads.  MODE 6 (gA in the epilogue): four per row, one per component c; other modes: two per row, each owns

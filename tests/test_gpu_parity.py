@@ -175,6 +175,18 @@ def test_mix16_short_blocks_many_atoms_per_tile():
     assert abs(g["energy"][0] - o["energy"]) / s.natoms <= 1e-3
 
 
+@pytest.mark.parametrize("prec,tol", [("fp64", 1e-10), ("mix32", 1e-4), ("mix16", 5e-3)])
+def test_tiny_two_type_cluster_fewer_rows_than_a_tile(prec, tol):
+    """12 atoms of two types in a 40 A box: every (centre, neighbour) block is a fraction of one 128-row tile, the
+    per-type fitting batches are 6 rows, the cell grid is mostly empty (workspace and tile-image sizing at tiny N)"""
+    s = synth.cluster(12, 5, ntypes=2)
+    o = oracle.evaluate(s.coords, s.types, s.box, s.model)
+    g = _gpu_eval(s, prec)
+    assert np.array_equal(g["nlist"], o["nlist"])
+    _check_forces(g, o, tol)
+    assert abs(g["energy"][0] - o["energy"]) <= (1e-12 if prec == "fp64" else 1e-3) * abs(o["energy"])
+
+
 def test_profile_slots_and_launch_count():
     import torch
     from paper_2005_00223_b200 import binding
