@@ -454,10 +454,18 @@ size_t dp_workspace_bytes(const dp_model *m, long natoms) {
 
 int dp_launches_per_compute(const dp_model *m) {
     if (!m) return 0;
-    // MIX-16 tcgen05 path: 6 binning (wrap, 3-launch bin scan, scatter, sort) + list + T row scans of 3 launches + env rows +
-    // forward + 3 fitting (first layer, fused 240 x 240 chain, last product with gA) + image fold + backward + force/virial + finalize
-    if (m->use_tc == 2 && m->use_tc_bwd && m->use_fit_tc) return 16 + 3 * m->T;
-    return 19;
+    // default paths (the DP_* debug switches that split or merge kernels are not counted)
+    int n = 6 + 1;                                   // wrap, 3-launch bin scan, scatter, bin sort; list
+    if (m->prec == DP_FP64) {
+        n += 1 + 9 + 1;                              // forward; descriptor, 6 GEMMs, energy, gA; backward (with S8, S9)
+    } else {
+        n += 3 * m->T;                               // row prefix sums, one 3-launch scan per neighbour type
+        n += m->use_tc ? 2 : 1;                      // environment rows + tcgen05 forward, or the mma.sync forward
+        if (m->use_fit_tc) n += 3 + (m->use_tc_bwd ? 0 : 1);   // first layer, fused 240 x 240 chain, last product (+ gA fragments)
+        else n += m->use_tc_bwd ? 8 : 9;             // descriptor, 6 GEMMs, energy (+ gA fragments)
+        n += m->use_tc_bwd ? 3 : 1;                  // gA fold / images, tcgen05 backward, force + virial; or the mma.sync backward
+    }
+    return n + 1;                                    // finalize
 }
 
 int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *types_dev, const double *box_host,
