@@ -111,6 +111,23 @@ int dp_last_row_counts(dp_model *m, long *rows_forward, long *rows_backward);
 int dp_profile_enable(dp_model *m, int on);
 int dp_profile_read(dp_model *m, double *ms_host);
 
+/* Velocity-Verlet MD loop around dp_compute (section VI-A: "the MD equations are numerically
+ * integrated by the velocity-Verlet scheme for 500 steps (the energy and forces are evaluated for 501 times)").
+ * One evaluation at the input coordinates, then nsteps times: v += (dt/2) a; x += dt v; evaluate; v += (dt/2) a,
+ * with a = F / m * 9.648533216e-3 A/fs^2 per (eV/A)/amu (CODATA 2018 e / amu * 1e-10).  nsteps + 1 evaluations.
+ *   coords_dev [natoms][3] fp64, in: x(0), out: x(nsteps dt) (not wrapped);  vel_dev [natoms][3] fp64 in A/fs, in/out;
+ *   types_dev as dp_compute;  mass_host[n_mass] amu per USER type (1 <= n_mass <= 8, all > 0);
+ *   dt_fs > 0 in femtoseconds;  workspace / stream / box as dp_compute (every evaluation rebuilds the neighbour list:
+ *   the paper's list with a 2 A buffer updated every 50 steps is not built);
+ *   forces_dev [natoms][3]: forces at the final coordinates;  thermo_dev [nsteps + 1][2] fp64: potential energy E and
+ *   kinetic energy sum 1/2 m v^2 (both eV) after evaluation 0 .. nsteps;  virial_dev [9] or NULL: virial of the last
+ *   evaluation.  Only enqueues on cuda_stream (no host synchronisation, no allocation); dp_status afterwards reports the
+ *   LAST evaluation.  Errors as dp_compute; DP_EINVAL for bad masses, dt_fs or nsteps < 0. */
+int dp_md_run(dp_model *m, long natoms, double *coords_dev, double *vel_dev, const int *types_dev,
+              const double *mass_host, int n_mass, const double *box_host, double dt_fs, int nsteps,
+              void *workspace_dev, size_t workspace_bytes, void *cuda_stream, double *forces_dev,
+              double *thermo_dev, double *virial_dev);
+
 void dp_destroy(dp_model *m);
 const char *dp_strerror(int code);
 

@@ -7,7 +7,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdp_b200.so")
-SOURCES = ["dp_api.cu", "nlist.cu", "embed_f64.cu", "fit_f64.cu", "embed_mix.cu", "fit_mix.cu", "embed_tc.cu", "embed_tc2.cu", "embed_tc2_bwd.cu", "fit_tc.cu"]
+SOURCES = ["dp_api.cu", "nlist.cu", "embed_f64.cu", "fit_f64.cu", "embed_mix.cu", "fit_mix.cu", "embed_tc.cu", "embed_tc2.cu", "embed_tc2_bwd.cu", "fit_tc.cu", "md.cu"]
 NVCC_FLAGS = os.environ.get("DP_EXTRA_NVCC", "").split() + ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--shared", "-cudart", "shared"]
 

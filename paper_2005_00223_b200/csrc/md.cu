@@ -1,0 +1,80 @@
+// Velocity-Verlet MD loop around dp_compute ("the MD equations are numerically
+// integrated by the velocity-Verlet scheme for 500 steps (the energy and forces are evaluated for 501 times)").
+// Everything is enqueued on the caller's stream: no host synchronisation, no allocation; the neighbour list is rebuilt by
+// every evaluation (the paper's 2 A skin list with an update every 50 steps is not built yet).
+#include "dp_internal.h"
+
+namespace {
+
+// acceleration of 1 eV/A on 1 amu in A/fs^2: (e / amu) * 1e-10 (CODATA 2018: e = 1.602176634e-19 C, amu = 1.66053906660e-27 kg)
+constexpr double ACC = 1.602176634e-19 / 1.66053906660e-27 * 1.0e-10;
+constexpr int MD_MAX_MASS = 8;
+struct Masses {
+    int n;
+    double m[MD_MAX_MASS];
+};
+
+// v += hk F / m  (hk = dt/2 * ACC, 0 for none);  x += dt v  (DRIFT);  kinetic energy sum 1/2 m v^2 / ACC in eV (KE)
+template <bool DRIFT, bool KE>
+__global__ void __launch_bounds__(256) k_md(long N, double *__restrict__ x, double *__restrict__ v,
+                                            const double *__restrict__ F, const int *__restrict__ types, Masses ms,
+                                            double hk, double dt, double *__restrict__ ke_out) {
+    double ke = 0.0;
+    for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < N; i += (long)gridDim.x * blockDim.x) {
+        const int ty = types[i];
+        if (ty < 0 || ty >= ms.n) continue;                 // dp_compute flags the type (DP_ETYPE); the atom stays put
+        const double mass = ms.m[ty], c = hk / mass;
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            double vb = v[3 * i + b];
+            if (hk != 0.0) vb = fma(c, F[3 * i + b], vb);
+            v[3 * i + b] = vb;
+            if (DRIFT) x[3 * i + b] = fma(dt, vb, x[3 * i + b]);
+            if (KE) ke = fma(0.5 * mass * vb, vb, ke);
+        }
+    }
+    if (KE) {
+        __shared__ double red[8];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) ke += __shfl_xor_sync(0xffffffffu, ke, o);
+        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = ke;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double s = 0.0;
+            for (int w = 0; w < 8; ++w) s += red[w];
+            atomicAdd(ke_out, s / ACC);
+        }
+    }
+}
+
+}  // namespace
+
+extern "C" int dp_md_run(dp_model *m, long natoms, double *coords_dev, double *vel_dev, const int *types_dev,
+                         const double *mass_host, int n_mass, const double *box_host, double dt_fs, int nsteps,
+                         void *workspace_dev, size_t workspace_bytes, void *cuda_stream, double *forces_dev,
+                         double *thermo_dev, double *virial_dev) {
+    if (!m || natoms <= 0 || !coords_dev || !vel_dev || !types_dev || !mass_host || n_mass <= 0 || n_mass > MD_MAX_MASS ||
+        !box_host || !(dt_fs > 0.0) || nsteps < 0 || !forces_dev || !thermo_dev)
+        return DP_EINVAL;
+    Masses ms;
+    ms.n = n_mass;
+    for (int k = 0; k < MD_MAX_MASS; ++k) ms.m[k] = k < n_mass ? mass_host[k] : 1.0;
+    for (int k = 0; k < n_mass; ++k) if (!(ms.m[k] > 0.0)) return DP_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const unsigned grid = (unsigned)((natoms + 255) / 256 < 148L * 8 ? (natoms + 255) / 256 : 148L * 8);
+    const double hk = 0.5 * dt_fs * ACC;
+    if (cudaMemsetAsync(thermo_dev, 0, sizeof(double) * 2 * ((size_t)nsteps + 1), st) != cudaSuccess) return DP_ECUDA;
+    int rc = dp_compute(m, natoms, coords_dev, types_dev, box_host, workspace_dev, workspace_bytes, cuda_stream, thermo_dev,
+                        nullptr, forces_dev, nsteps == 0 ? virial_dev : nullptr);
+    if (rc != DP_OK) return rc;
+    k_md<false, true><<<grid, 256, 0, st>>>(natoms, coords_dev, vel_dev, forces_dev, types_dev, ms, 0.0, dt_fs, thermo_dev + 1);
+    for (int s = 1; s <= nsteps; ++s) {
+        k_md<true, false><<<grid, 256, 0, st>>>(natoms, coords_dev, vel_dev, forces_dev, types_dev, ms, hk, dt_fs, nullptr);
+        rc = dp_compute(m, natoms, coords_dev, types_dev, box_host, workspace_dev, workspace_bytes, cuda_stream,
+                        thermo_dev + 2 * s, nullptr, forces_dev, s == nsteps ? virial_dev : nullptr);
+        if (rc != DP_OK) return rc;
+        k_md<false, true><<<grid, 256, 0, st>>>(natoms, coords_dev, vel_dev, forces_dev, types_dev, ms, hk, dt_fs,
+                                                 thermo_dev + 2 * s + 1);
+    }
+    return cudaGetLastError() == cudaSuccess ? DP_OK : DP_ECUDA;
+}

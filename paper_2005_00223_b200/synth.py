@@ -288,3 +288,20 @@ def small_fcc(ncell: int, seed: int, sigma: float = 0.05, a: float = 3.634, rc: 
     model = make_model(ntypes, rc, rc_smth, sel, seed + 1000, avg, std)
     box = np.diag([L, L, L]).reshape(9).astype(np.float64)
     return System(f"fcc{n}", np.ascontiguousarray(x), types, box, model, "fp64")
+
+
+# ----------------------------------------------------------------------------- MD inputs
+MASS_AMU = {"cu": (63.546,), "water": (15.999, 1.008)}     # per user type: copper; water O, H
+
+
+def boltzmann_velocities(types: np.ndarray, masses, temperature: float, seed: int) -> np.ndarray:
+    """Seeded velocities [N,3] in Angstrom/fs "randomly initialized subjected to the Boltzmann distribution"
+    (330 K): each component ~ N(0, kB T / m), total momentum removed.  An input recipe only: the
+    integrator arithmetic lives in csrc/md.cu and, independently, in oracle/md_oracle.py."""
+    kb = 8.617333262e-5                                     # eV/K
+    ev_per_amu_a2_fs2 = 1.0 / 9.648533216e-3                # 1 amu A^2/fs^2 in eV
+    rng = np.random.Generator(np.random.PCG64(seed))
+    m = np.asarray(masses, dtype=np.float64)[np.asarray(types)]
+    v = rng.standard_normal((len(m), 3)) * np.sqrt(kb * temperature / (m * ev_per_amu_a2_fs2))[:, None]
+    v -= (m[:, None] * v).sum(axis=0) / m.sum()
+    return np.ascontiguousarray(v)

@@ -1,0 +1,72 @@
+"""dp_md_run (velocity-Verlet loop) against the MD oracle, through the C ABI (-m gpu)."""
+import numpy as np
+import pytest
+
+from oracle import md_oracle
+from paper_2005_00223_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+
+def _gpu_md(s, v, masses, dt, nsteps, precision):
+    import torch
+    from paper_2005_00223_b200 import binding
+    m = binding.DPModel(s.model, precision)
+    c = torch.from_numpy(s.coords.copy()).cuda()
+    vel = torch.from_numpy(v.copy()).cuda()
+    t = torch.from_numpy(s.types).cuda()
+    out = m.md_run(c, vel, t, masses, s.box, dt, nsteps)
+    rc, _ = m.status()
+    assert rc == 0
+    torch.cuda.synchronize()
+    res = {k: x.cpu().numpy() for k, x in out.items()}
+    res["coords"], res["vel"] = c.cpu().numpy(), vel.cpu().numpy()
+    m.close()
+    return res
+
+
+@pytest.mark.parametrize("idx,dt,nsteps", [(0, 1.0, 6), (1, 0.5, 4)])      # copper 1.0 fs, water 0.5 fs
+def test_md_trajectory_fp64_matches_oracle(idx, dt, nsteps):
+    s = synth.config(idx)
+    masses = synth.MASS_AMU["cu" if idx == 0 else "water"]
+    v = synth.boltzmann_velocities(s.types, masses, 330.0, 4242 + idx)
+    o = md_oracle.run(s.coords, v, s.types, masses, s.box, s.model, dt, nsteps)
+    g = _gpu_md(s, v, masses, dt, nsteps, "fp64")
+    assert np.abs(g["coords"] - o["coords"]).max() <= 1e-11
+    vr = np.sqrt((o["vel"] ** 2).mean())
+    assert np.abs(g["vel"] - o["vel"]).max() <= 1e-10 * vr
+    fr = np.sqrt((o["forces"] ** 2).mean())
+    assert np.abs(g["forces"] - o["forces"]).max() <= 1e-9 * fr       # forces at positions that differ by rounding
+    assert np.abs(g["thermo"][:, 0] - o["thermo"][:, 0]).max() <= 1e-12 * abs(o["thermo"][0, 0])
+    assert np.abs(g["thermo"][:, 1] - o["thermo"][:, 1]).max() <= 1e-11 * o["thermo"][0, 1]
+    assert np.abs(g["virial"] - o["virial"]).max() <= 1e-9 * np.abs(o["virial"]).max()
+    assert np.abs(o["coords"] - s.coords).max() > 1e-3
+
+
+def test_md_zero_steps_is_one_evaluation_and_bad_arguments():
+    import torch
+    from paper_2005_00223_b200 import binding
+    s = synth.config(0)
+    v = synth.boltzmann_velocities(s.types, (63.546,), 330.0, 1)
+    g = _gpu_md(s, v, (63.546,), 1.0, 0, "fp64")
+    assert np.array_equal(g["coords"], s.coords) and np.array_equal(g["vel"], v)
+    assert g["thermo"].shape == (1, 2)
+    m = binding.DPModel(s.model, "fp64")
+    c = torch.from_numpy(s.coords.copy()).cuda(); vel = torch.from_numpy(v.copy()).cuda(); t = torch.from_numpy(s.types).cuda()
+    for masses, dt, n in [((0.0,), 1.0, 1), ((63.5,), 0.0, 1), ((63.5,), 1.0, -1)]:
+        with pytest.raises(binding.DPError) as e:
+            m.md_run(c, vel, t, masses, s.box, dt, n)
+        assert e.value.code == -1
+    m.close()
+
+
+def test_md_mix16_conserves_total_energy():
+    # the benchmark precision on config 0's geometry: 20 steps of 1 fs; the total energy must stay put far better than
+    # its parts move (mixed-precision forces are not exactly conservative: bound the drift, PAPER.md:127 discusses it)
+    s = synth.config(0)
+    masses = (1.0,)                                                   # light atoms so that the dynamics matter in 20 fs
+    v = synth.boltzmann_velocities(s.types, masses, 30.0, 7)
+    g = _gpu_md(s, v, masses, 1.0, 20, "mix16")
+    e = g["thermo"].sum(axis=1)
+    moved = np.ptp(g["thermo"][:, 1])
+    assert moved > 0 and np.abs(e - e[0]).max() < 0.05 * moved, (np.abs(e - e[0]).max(), moved)
