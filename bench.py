@@ -181,6 +181,8 @@ def main():
                     help="override the config's precision (profiling aid; the default is the precision BASELINE.json names)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--md-steps", type=int, default=10,
+                    help="also time an MD loop of this many velocity-Verlet steps (dp_md_run; 0 = skip; N = 1 only)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -258,6 +260,32 @@ def main():
 
     t_ms, e2e_ms = max_over_ranks([t_ms, e2e_ms], world, dev)
 
+    # the paper's own time-to-solution: MD loop time / steps, one dp_md_run of md_steps steps
+    md = None
+    if world == 1 and args.md_steps > 0:
+        try:
+            kind = "water" if s.model.ntypes == 2 else "cu"
+            dt_fs = 0.5 if kind == "water" else 1.0
+            vel = torch.from_numpy(synth.boltzmann_velocities(s.types, synth.MASS_AMU[kind], 330.0, 99)).to(dev)
+            xmd = coords.clone()
+            model.md_run(xmd, vel, types, synth.MASS_AMU[kind], s.box, dt_fs, 1)          # warm-up
+            barrier()
+            m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            m0.record(st)
+            mo = model.md_run(xmd, vel, types, synth.MASS_AMU[kind], s.box, dt_fs, args.md_steps)
+            m1.record(st)
+            barrier()
+            rc_md, _ = model.status()
+            th = mo["thermo"].cpu().numpy()
+            md_ms = m0.elapsed_time(m1)
+            md = {"steps": args.md_steps, "evaluations": args.md_steps + 1, "dt_fs": dt_fs, "temperature_K": 330.0,
+                  "loop_ms_per_step": md_ms / args.md_steps, "s_per_step_per_atom": md_ms * 1e-3 / args.md_steps / N,
+                  "status": rc_md, "e_total_first_last_eV": [float(th[0].sum()), float(th[-1].sum())],
+                  "e_kin_first_eV": float(th[0, 1]),
+                  "note": "velocity Verlet, list rebuilt by every evaluation, no L2 flush between steps"}
+        except Exception as ex:      # the MD leg never takes the bench line down
+            md = {"error": repr(ex)}
+
     if rank == 0:
         pk = peaks()
         ms_step = t_ms / K
@@ -302,6 +330,8 @@ def main():
                                      "the hi/lo operand splitting and the K/N padding are executed (executed_tflops) but not credited; "
                                      "mufu_tanh_frac = tanh issued by this kernel / measured MUFU.TANH peak (16 per clock per SM)"},
                 "kernels": kern}
+        if md is not None:
+            line["md"] = md
         if args.all_configs and world == 1:
             summ = {}
             for idx in range(5):
