@@ -44,7 +44,8 @@ typedef enum {
     DP_ETYPE = -4,    /* an atom type outside type_map (detected on device, reported by dp_status)            */
     DP_ECUDA = -5,    /* CUDA runtime error or no device                                                      */
     DP_ENEIGH = -6,   /* an atom has more candidates inside rc than the sort buffer holds (dp_status)         */
-    DP_EUNSUPPORTED = -7 /* precision mode / shape not built                                                 */
+    DP_EUNSUPPORTED = -7, /* precision mode / shape not built                                                */
+    DP_ESKIN = -8     /* dp_md_run with a buffered list: an atom moved > skin/2 since the list was built (dp_status) */
 } dp_error;
 
 /* Host-side description of one model; read only during dp_create (weights are copied and converted once,
@@ -117,16 +118,23 @@ int dp_profile_read(dp_model *m, double *ms_host);
  * with a = F / m * 9.648533216e-3 A/fs^2 per (eV/A)/amu (CODATA 2018 e / amu * 1e-10).  nsteps + 1 evaluations.
  *   coords_dev [natoms][3] fp64, in: x(0), out: x(nsteps dt) (not wrapped);  vel_dev [natoms][3] fp64 in A/fs, in/out;
  *   types_dev as dp_compute;  mass_host[n_mass] amu per USER type (1 <= n_mass <= 8, all > 0);
- *   dt_fs > 0 in femtoseconds;  workspace / stream / box as dp_compute (every evaluation rebuilds the neighbour list:
- *   the paper's list with a 2 A buffer updated every 50 steps is not built);
+ *   dt_fs > 0 in femtoseconds;  box / stream as dp_compute;
+ *   skin (A) and rebuild_every: with skin > 0 and rebuild_every > 1 the neighbour search keeps, per atom and type, the
+ *   candidates within rc + skin of the last cell search and repeats that search every rebuild_every evaluations
+ *   ("The neighbor list with a 2 A buffer region is updated every 50 steps"); in between a step re-tests the
+ *   candidates exactly, re-sorts and truncates, so the formatted list is the same as without the buffer as long as no atom
+ *   moved more than skin/2 since the last search (checked on the device: DP_ESKIN from dp_status).  skin = 0 or
+ *   rebuild_every <= 1: every evaluation searches the cells.
+ *   workspace_dev: >= dp_md_workspace_bytes(m, natoms, skin) bytes (skin = 0 if not buffered), 256-byte aligned;
  *   forces_dev [natoms][3]: forces at the final coordinates;  thermo_dev [nsteps + 1][2] fp64: potential energy E and
  *   kinetic energy sum 1/2 m v^2 (both eV) after evaluation 0 .. nsteps;  virial_dev [9] or NULL: virial of the last
  *   evaluation.  Only enqueues on cuda_stream (no host synchronisation, no allocation); dp_status afterwards reports the
- *   LAST evaluation.  Errors as dp_compute; DP_EINVAL for bad masses, dt_fs or nsteps < 0. */
+ *   LAST evaluation.  Errors as dp_compute; DP_EINVAL for bad masses, dt_fs, skin < 0, nsteps < 0 or rebuild_every < 0. */
+size_t dp_md_workspace_bytes(const dp_model *m, long natoms, double skin);
 int dp_md_run(dp_model *m, long natoms, double *coords_dev, double *vel_dev, const int *types_dev,
               const double *mass_host, int n_mass, const double *box_host, double dt_fs, int nsteps,
-              void *workspace_dev, size_t workspace_bytes, void *cuda_stream, double *forces_dev,
-              double *thermo_dev, double *virial_dev);
+              double skin, int rebuild_every, void *workspace_dev, size_t workspace_bytes, void *cuda_stream,
+              double *forces_dev, double *thermo_dev, double *virial_dev);
 
 void dp_destroy(dp_model *m);
 const char *dp_strerror(int code);

@@ -18,7 +18,7 @@ DP_FP64, DP_MIX32, DP_MIX16 = 0, 1, 2
 PRECISIONS = {"fp64": DP_FP64, "mix32": DP_MIX32, "mix16": DP_MIX16}
 EXPORTS = ["dp_create", "dp_workspace_bytes", "dp_compute", "dp_get_nlist", "dp_status",
            "dp_launches_per_compute", "dp_last_row_counts", "dp_profile_enable", "dp_profile_read", "dp_md_run",
-           "dp_destroy", "dp_strerror"]
+           "dp_md_workspace_bytes",           "dp_destroy", "dp_strerror"]
 
 
 class DPError(RuntimeError):
@@ -65,7 +65,10 @@ def lib():
         L.dp_profile_read.restype = C.c_int
         L.dp_profile_read.argtypes = [vp, dp]
         L.dp_md_run.restype = C.c_int
-        L.dp_md_run.argtypes = [vp, C.c_long, vp, vp, vp, dp, C.c_int, dp, C.c_double, C.c_int, vp, C.c_size_t, vp, vp, vp, vp]
+        L.dp_md_run.argtypes = [vp, C.c_long, vp, vp, vp, dp, C.c_int, dp, C.c_double, C.c_int, C.c_double, C.c_int, vp,
+                                C.c_size_t, vp, vp, vp, vp]
+        L.dp_md_workspace_bytes.restype = C.c_size_t
+        L.dp_md_workspace_bytes.argtypes = [vp, C.c_long, C.c_double]
         L.dp_destroy.restype = None
         L.dp_destroy.argtypes = [vp]
         _lib = L
@@ -142,16 +145,24 @@ class DPModel:
         self._n = n
         return out
 
-    def md_run(self, coords, vel, types, masses, box, dt_fs, nsteps, stream=None, want_virial=True):
+    def md_run(self, coords, vel, types, masses, box, dt_fs, nsteps, skin=0.0, rebuild_every=0, stream=None,
+               want_virial=True):
         """Velocity-Verlet loop (dp_md_run): coords, vel [N,3] f64 cuda are advanced IN PLACE by nsteps steps of dt_fs;
-        masses: amu per user type.  Enqueues only; returns forces [N,3], thermo [nsteps+1,2] (E_pot, E_kin in eV), virial."""
+        masses: amu per user type; skin > 0 and rebuild_every > 1: buffered neighbour list.
+        Enqueues only; returns forces [N,3], thermo [nsteps+1,2] (E_pot, E_kin in eV), virial."""
         import torch
         for x in (coords, vel):
             assert x.is_cuda and x.dtype == torch.float64 and x.is_contiguous()
         assert types.is_cuda and types.dtype == torch.int32 and types.is_contiguous()
         n = int(coords.shape[0])
         dev = coords.device
-        ws = self._workspace(n, dev)
+        buffered = skin > 0.0 and rebuild_every > 1
+        need = int(lib().dp_md_workspace_bytes(self._h, n, float(skin) if buffered else 0.0))
+        if need == 0:
+            raise DPError(-1, "dp_md_workspace_bytes")
+        if self._ws is None or self._ws.numel() < need or self._ws.device != dev:
+            self._ws = torch.empty(need, dtype=torch.uint8, device=dev)
+        ws = self._ws
         out = dict(forces=torch.empty((n, 3), dtype=torch.float64, device=dev),
                    thermo=torch.empty((int(nsteps) + 1, 2), dtype=torch.float64, device=dev),
                    virial=torch.empty(9, dtype=torch.float64, device=dev))
@@ -159,7 +170,8 @@ class DPModel:
         mh = np.ascontiguousarray(masses, dtype=np.float64)
         st = stream if stream is not None else torch.cuda.current_stream(dev)
         rc = lib().dp_md_run(self._h, n, coords.data_ptr(), vel.data_ptr(), types.data_ptr(), _dptr(mh), int(mh.shape[0]),
-                             _dptr(boxh), float(dt_fs), int(nsteps), ws.data_ptr(), ws.numel(), st.cuda_stream,
+                             _dptr(boxh), float(dt_fs), int(nsteps), float(skin), int(rebuild_every), ws.data_ptr(), ws.numel(),
+                             st.cuda_stream,
                              out["forces"].data_ptr(), out["thermo"].data_ptr(),
                              out["virial"].data_ptr() if want_virial else None)
         if rc != 0:

@@ -65,18 +65,20 @@ bool make_grid(const dp_model *m, long N, const double *box, Grid3 *g) {
     const long cap = ncell_max_for(N);
     // half-width cells (edge >= rc/2, 5 x 5 x 5 neighbourhood: 58 % of the candidates of the 3 x 3 x 3 search) when the grid
     // then has at least 5 cells per axis and fits the bin arrays; else cells of edge >= rc
+    // the MD loop's buffered list searches rc + skin (every call of one dp_md_run uses the same grid)
+    const double rl = m->rc + (m->list_mode ? m->md_skin : 0.0);
     g->reach = 2;
     for (int a = 0; a < 3; ++a) {
         if (!(Ls[a] >= 2.0 * m->rc)) return false;
         g->L[a] = Ls[a];
-        g->nc[a] = (int)std::floor(Ls[a] / (0.5 * m->rc * (1.0 + 1e-9)));
+        g->nc[a] = (int)std::floor(Ls[a] / (0.5 * rl * (1.0 + 1e-9)));
         if (g->nc[a] < 5) g->reach = 1;
     }
     if ((long)g->nc[0] * g->nc[1] * g->nc[2] > cap) g->reach = 1;
     if (std::getenv("DP_NLIST_REACH1")) g->reach = 1;
     if (g->reach == 1)
         for (int a = 0; a < 3; ++a) {
-            int nc = (int)std::floor(Ls[a] / (m->rc * (1.0 + 1e-9)));
+            int nc = (int)std::floor(Ls[a] / (rl * (1.0 + 1e-9)));
             g->nc[a] = nc < 1 ? 1 : nc;
         }
     while ((long)g->nc[0] * g->nc[1] * g->nc[2] > cap) {
@@ -305,6 +307,7 @@ const char *dp_strerror(int code) {
         case DP_ECUDA: return "CUDA error or no device";
         case DP_ENEIGH: return "too many neighbour candidates for the sort buffer";
         case DP_EUNSUPPORTED: return "precision mode or shape not supported by this build";
+        case DP_ESKIN: return "an atom moved more than skin/2 since the buffered neighbour list was built";
         default: return "unknown error";
     }
 }
@@ -489,7 +492,8 @@ int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *ty
     ok(cudaMemsetAsync(energy_dev, 0, sizeof(double), st));
     auto mark = [&](int k) { if (m->profile) ok(cudaEventRecord(m->ev[k], st)); };
     mark(0);
-    ok(launch_build_cells(m, natoms, coords_dev, types_dev, g, ws, L, st));
+    ok(m->list_mode == 2 ? launch_regather(m, natoms, coords_dev, g, ws, L, st)
+                         : launch_build_cells(m, natoms, coords_dev, types_dev, g, ws, L, st));
     ok(launch_nlist(m, natoms, g, ws, L, st));
     mark(1);
     const bool f64 = m->prec == DP_FP64;
@@ -551,6 +555,7 @@ int dp_status(dp_model *m, long *n_truncated_atoms) {
     if (n_truncated_atoms) *n_truncated_atoms = st[1];
     if (st[0] & 1) return DP_ETYPE;
     if (st[0] & 2) return DP_ENEIGH;
+    if (st[0] & 4) return DP_ESKIN;
     return DP_OK;
 }
 

@@ -71,6 +71,11 @@ struct dp_model {
     int mix_ns, mix_nsc, mix_tanh_approx, mix_fit_ns, mix_fit3_ns, mix_ns_bwd;
     int mix_ns_fwd, mix_nsc_fwd;    // forward-kernel overrides of mix_ns / mix_nsc (precision study)
     int profile;
+    // buffered neighbour list of the MD loop (md.cu sets these around its dp_compute calls; 0 / null otherwise)
+    int list_mode;                  // 0: search the cells every call; 1: search with rc + skin and store candidates; 2: reuse them
+    double md_skin;
+    int *md_cand, *md_candcnt;      // [T][N][sort_cap], [T][N] in the MD part of the workspace
+    double *md_xref;                // [N][3] coordinates at the last list build (user order)
     cudaEvent_t ev[8];                // ev[0..5]: phase boundaries; ev[6], ev[7]: around the MIX-16 tcgen05 backward kernel
 };
 
@@ -117,6 +122,8 @@ struct Grid3 {
 // launchers (each returns cudaGetLastError())
 cudaError_t launch_build_cells(const dp_model *m, long N, const double *coords, const int *types, const Grid3 &g,
                                char *ws, const WsLayout &L, cudaStream_t st);
+cudaError_t launch_regather(const dp_model *m, long N, const double *coords, const Grid3 &g, char *ws, const WsLayout &L,
+                            cudaStream_t st);
 cudaError_t launch_nlist(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_get_nlist(const dp_model *m, long N, char *ws, const WsLayout &L, int *out, cudaStream_t st);
 cudaError_t launch_embed_fwd_f64(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);

@@ -1,7 +1,8 @@
 // Velocity-Verlet MD loop around dp_compute ("the MD equations are numerically
 // integrated by the velocity-Verlet scheme for 500 steps (the energy and forces are evaluated for 501 times)").
 // Everything is enqueued on the caller's stream: no host synchronisation, no allocation; the neighbour list is rebuilt by
-// every evaluation (the paper's 2 A skin list with an update every 50 steps is not built yet).
+// every evaluation, or (skin > 0, rebuild_every > 1) kept as a buffered candidate list for rebuild_every evaluations as in the
+// paper (2 A buffer, update every 50 steps); then a step only re-tests, re-sorts and truncates (nlist.cu).
 #include "dp_internal.h"
 
 namespace {
@@ -49,32 +50,70 @@ __global__ void __launch_bounds__(256) k_md(long N, double *__restrict__ x, doub
 
 }  // namespace
 
+namespace {
+struct MdWs { size_t base, cand, candcnt, xref, total; };
+MdWs md_layout(const dp_model *m, long N, double skin) {
+    MdWs w{};
+    auto al = [](size_t x) { return (x + 255) & ~(size_t)255; };
+    w.base = al(dp_workspace_bytes(m, N));
+    w.total = w.base;
+    if (skin > 0.0) {
+        w.cand = w.total; w.total = al(w.total + sizeof(int) * (size_t)m->T * (size_t)N * (size_t)m->sort_cap);
+        w.candcnt = w.total; w.total = al(w.total + sizeof(int) * (size_t)m->T * (size_t)N);
+        w.xref = w.total; w.total = al(w.total + sizeof(double) * 3 * (size_t)N);
+    }
+    return w;
+}
+}  // namespace
+
+extern "C" size_t dp_md_workspace_bytes(const dp_model *m, long natoms, double skin) {
+    if (!m || natoms <= 0 || !(skin >= 0.0) || dp_workspace_bytes(m, natoms) == 0) return 0;
+    return md_layout(m, natoms, skin).total;
+}
+
 extern "C" int dp_md_run(dp_model *m, long natoms, double *coords_dev, double *vel_dev, const int *types_dev,
                          const double *mass_host, int n_mass, const double *box_host, double dt_fs, int nsteps,
-                         void *workspace_dev, size_t workspace_bytes, void *cuda_stream, double *forces_dev,
-                         double *thermo_dev, double *virial_dev) {
+                         double skin, int rebuild_every, void *workspace_dev, size_t workspace_bytes, void *cuda_stream,
+                         double *forces_dev, double *thermo_dev, double *virial_dev) {
     if (!m || natoms <= 0 || !coords_dev || !vel_dev || !types_dev || !mass_host || n_mass <= 0 || n_mass > MD_MAX_MASS ||
-        !box_host || !(dt_fs > 0.0) || nsteps < 0 || !forces_dev || !thermo_dev)
+        !box_host || !(dt_fs > 0.0) || nsteps < 0 || !forces_dev || !thermo_dev || !(skin >= 0.0) || rebuild_every < 0 ||
+        !workspace_dev)
         return DP_EINVAL;
     Masses ms;
     ms.n = n_mass;
     for (int k = 0; k < MD_MAX_MASS; ++k) ms.m[k] = k < n_mass ? mass_host[k] : 1.0;
     for (int k = 0; k < n_mass; ++k) if (!(ms.m[k] > 0.0)) return DP_EINVAL;
+    const bool buffered = skin > 0.0 && rebuild_every > 1;
+    const MdWs W = md_layout(m, natoms, buffered ? skin : 0.0);
+    if (W.base == 0) return DP_EINVAL;
+    if (workspace_bytes < W.total) return DP_ENOMEM;
+    char *ws = (char *)workspace_dev;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const unsigned grid = (unsigned)((natoms + 255) / 256 < 148L * 8 ? (natoms + 255) / 256 : 148L * 8);
     const double hk = 0.5 * dt_fs * ACC;
     if (cudaMemsetAsync(thermo_dev, 0, sizeof(double) * 2 * ((size_t)nsteps + 1), st) != cudaSuccess) return DP_ECUDA;
-    int rc = dp_compute(m, natoms, coords_dev, types_dev, box_host, workspace_dev, workspace_bytes, cuda_stream, thermo_dev,
-                        nullptr, forces_dev, nsteps == 0 ? virial_dev : nullptr);
-    if (rc != DP_OK) return rc;
-    k_md<false, true><<<grid, 256, 0, st>>>(natoms, coords_dev, vel_dev, forces_dev, types_dev, ms, 0.0, dt_fs, thermo_dev + 1);
-    for (int s = 1; s <= nsteps; ++s) {
-        k_md<true, false><<<grid, 256, 0, st>>>(natoms, coords_dev, vel_dev, forces_dev, types_dev, ms, hk, dt_fs, nullptr);
-        rc = dp_compute(m, natoms, coords_dev, types_dev, box_host, workspace_dev, workspace_bytes, cuda_stream,
-                        thermo_dev + 2 * s, nullptr, forces_dev, s == nsteps ? virial_dev : nullptr);
-        if (rc != DP_OK) return rc;
-        k_md<false, true><<<grid, 256, 0, st>>>(natoms, coords_dev, vel_dev, forces_dev, types_dev, ms, hk, dt_fs,
-                                                 thermo_dev + 2 * s + 1);
+    if (buffered) {
+        m->md_skin = skin;
+        m->md_cand = (int *)(ws + W.cand); m->md_candcnt = (int *)(ws + W.candcnt); m->md_xref = (double *)(ws + W.xref);
     }
+    int rc = DP_OK;
+    for (int s = 0; s <= nsteps && rc == DP_OK; ++s) {
+        if (s > 0)
+            k_md<true, false><<<grid, 256, 0, st>>>(natoms, coords_dev, vel_dev, forces_dev, types_dev, ms, hk, dt_fs, nullptr);
+        if (buffered) {
+            m->list_mode = (s % rebuild_every == 0) ? 1 : 2;
+            if (m->list_mode == 1 &&
+                cudaMemcpyAsync(m->md_xref, coords_dev, sizeof(double) * 3 * (size_t)natoms, cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+                rc = DP_ECUDA;
+        }
+        if (rc == DP_OK)
+            rc = dp_compute(m, natoms, coords_dev, types_dev, box_host, workspace_dev, W.base, cuda_stream, thermo_dev + 2 * s,
+                            nullptr, forces_dev, s == nsteps ? virial_dev : nullptr);
+        if (rc == DP_OK)
+            k_md<false, true><<<grid, 256, 0, st>>>(natoms, coords_dev, vel_dev, forces_dev, types_dev, ms, s > 0 ? hk : 0.0,
+                                                     dt_fs, thermo_dev + 2 * s + 1);
+    }
+    m->list_mode = 0; m->md_skin = 0.0; m->md_cand = nullptr; m->md_candcnt = nullptr; m->md_xref = nullptr;
+    if (rc != DP_OK) return rc;
     return cudaGetLastError() == cudaSuccess ? DP_OK : DP_ECUDA;
 }

@@ -361,11 +361,16 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
     }
     return v;
 }
+// MODE 0: every call searches the cells.  MODE 1 / 2: the MD loop's buffered list ("neighbor list with a 2 A
+// buffer region ... updated every 50 steps"): MODE 1 searches the cells with rc + skin in pass 1 and also stores the
+// survivors (sorted-space atom indices, cap per atom and type); MODE 2 skips the cells and pass 1 and starts from the
+// stored candidates.  Pass 2 (exact test, key), sort and truncation are the same every step, so the list stays bit-exact.
+template <int MODE>
 __global__ void __launch_bounds__(128, 8)
 k_nlist2(long N, int T, Grid3 g, double rc2, NlistF32 gf, int cap, const int *__restrict__ bin_start,
          const double *__restrict__ xs, const float4 *__restrict__ xsf, const int *__restrict__ perm,
          const int *__restrict__ inv, int Nm, int4 sel4, int *__restrict__ nlist, int *__restrict__ nreal,
-         int *__restrict__ rowcnt, int *__restrict__ status) {
+         int *__restrict__ rowcnt, int *__restrict__ status, int *__restrict__ cand, int *__restrict__ candcnt) {
     extern __shared__ unsigned long long keys_all[];
     __shared__ int2 runtab_all[4][66];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -401,6 +406,12 @@ k_nlist2(long N, int T, Grid3 g, double rc2, NlistF32 gf, int cap, const int *__
     bool truncated = false;
     int off = 0;
     for (int b = 0; b < T; ++b) {
+        int n1 = 0;
+        if (MODE == 2) {
+            n1 = candcnt[(long)b * N + i];
+            const int *cs = cand + ((long)b * N + i) * cap;
+            for (int k = lane; k < n1; k += 32) keys[k] = (unsigned long long)cs[k];
+        } else {
         // ---- run table ----
         int sA = 0, lenA = 0, sB = 0, lenB = 0;
         if (lane < ncol) {
@@ -423,7 +434,7 @@ k_nlist2(long N, int T, Grid3 g, double rc2, NlistF32 gf, int cap, const int *__
         if (lane == 0) runtab[nrun] = make_int2(0x7fffffff, 0);
         __syncwarp();
         // ---- pass 1: conservative fp32 filter ----
-        int n1 = 0, r = 0;
+        int r = 0;
         int2 e = runtab[0];
         for (int base = 0; base < total; base += 32) {
             const int idx = base + lane;
@@ -446,6 +457,13 @@ k_nlist2(long N, int T, Grid3 g, double rc2, NlistF32 gf, int cap, const int *__
             n1 += __popc(mask);
         }
         if (n1 > cap) { if (lane == 0) atomicOr(&status[0], 2); n1 = cap; }
+        __syncwarp();
+        if (MODE == 1) {
+            int *cs = cand + ((long)b * N + i) * cap;
+            for (int k = lane; k < n1; k += 32) cs[k] = (int)keys[k];
+            if (lane == 0) candcnt[(long)b * N + i] = n1;
+        }
+        }
         __syncwarp();
         // ---- pass 2: exact test + key on the survivors, compacted in place ----
         int n = 0;
@@ -517,7 +535,35 @@ __global__ void k_get_nlist(long N, int Nm, const int *__restrict__ nlist, const
     out[(long)perm[i] * Nm + k] = v >= 0 ? perm[v] : -1;
 }
 
+// Reuse step of the buffered list: the sorted order of the last cell build is kept, only the coordinates are refreshed
+// (canonical wrap as k_wrap_bin).  An atom that moved more than skin / 2 since the build breaks the superset guarantee.
+__global__ void k_regather(long N, const double *__restrict__ coords, const int *__restrict__ perm, Grid3 g,
+                           const double *__restrict__ xref, double half_skin2, double *__restrict__ xs,
+                           float4 *__restrict__ xsf, int *__restrict__ status) {
+    long s = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    const long u = perm[s];
+    double w[3], d2 = 0.0;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double x = coords[3 * u + a], d = x - xref[3 * u + a];
+        w[a] = wrap_coord(x, g.L[a]);
+        d2 += d * d;
+        xs[3 * s + a] = w[a];
+    }
+    xsf[s] = make_float4((float)w[0], (float)w[1], (float)w[2], 0.f);
+    if (d2 > half_skin2) atomicOr(&status[0], 4);
+}
+
 }  // namespace
+
+cudaError_t launch_regather(const dp_model *m, long N, const double *coords, const Grid3 &g, char *ws, const WsLayout &L,
+                            cudaStream_t st) {
+    k_regather<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(N, coords, (int *)(ws + L.perm), g, m->md_xref,
+                                                           0.25 * m->md_skin * m->md_skin, (double *)(ws + L.xs),
+                                                           (float4 *)(ws + L.xsf), (int *)(ws + L.status));
+    return cudaGetLastError();
+}
 
 cudaError_t launch_build_cells(const dp_model *m, long N, const double *coords, const int *types, const Grid3 &g,
                                char *ws, const WsLayout &L, cudaStream_t st) {
@@ -552,16 +598,23 @@ cudaError_t launch_nlist(const dp_model *m, long N, const Grid3 &g, char *ws, co
     // (and the fp32 minimum image d - L rint(d / L) by another ulp(L))
     NlistF32 gf;
     for (int d = 0; d < 3; ++d) { gf.L[d] = (float)g.L[d]; gf.invL[d] = (float)(1.0 / g.L[d]); }
-    gf.rc2_margin = (float)(m->rc * m->rc * (1.0 + 1e-5) + 12.0 * m->rc * Lmax * 1.2e-7 + 1e-6);
+    const double rl = m->rc + (m->list_mode ? m->md_skin : 0.0);      // search radius of pass 1
+    gf.rc2_margin = (float)(rl * rl * (1.0 + 1e-5) + 12.0 * rl * Lmax * 1.2e-7 + 1e-6);
     static const bool legacy = std::getenv("DP_NLIST_V1") != nullptr;
     if (!legacy) {
         static bool attr2 = false;
-        if (!attr2) { cudaFuncSetAttribute(k_nlist2, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 4096 * 8); attr2 = true; }
-        k_nlist2<<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, m->T, g, m->rc * m->rc, gf, cap, (int *)(ws + L.bin_start),
-                                                            (double *)(ws + L.xs), (const float4 *)(ws + L.xsf), (int *)(ws + L.perm),
-                                                            (int *)(ws + L.inv), m->Nm, sel4, (int *)(ws + L.nlist),
-                                                            (int *)(ws + L.nreal), m->prec == DP_FP64 ? nullptr : (int *)(ws + L.rowcnt),
-                                                            (int *)(ws + L.status));
+        if (!attr2) {
+            cudaFuncSetAttribute(k_nlist2<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 4096 * 8);
+            cudaFuncSetAttribute(k_nlist2<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 4096 * 8);
+            cudaFuncSetAttribute(k_nlist2<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 4096 * 8);
+            attr2 = true;
+        }
+        auto kern = m->list_mode == 1 ? k_nlist2<1> : (m->list_mode == 2 ? k_nlist2<2> : k_nlist2<0>);
+        kern<<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, m->T, g, m->rc * m->rc, gf, cap, (int *)(ws + L.bin_start),
+                                                        (double *)(ws + L.xs), (const float4 *)(ws + L.xsf), (int *)(ws + L.perm),
+                                                        (int *)(ws + L.inv), m->Nm, sel4, (int *)(ws + L.nlist),
+                                                        (int *)(ws + L.nreal), m->prec == DP_FP64 ? nullptr : (int *)(ws + L.rowcnt),
+                                                        (int *)(ws + L.status), m->md_cand, m->md_candcnt);
     } else
     k_nlist<<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, m->T, g, m->rc * m->rc, cap, (int *)(ws + L.bin_start),
                                                        (double *)(ws + L.xs), (int *)(ws + L.perm),

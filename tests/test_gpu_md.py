@@ -8,18 +8,22 @@ from paper_2005_00223_b200 import synth
 pytestmark = pytest.mark.gpu
 
 
-def _gpu_md(s, v, masses, dt, nsteps, precision):
+def _gpu_md(s, v, masses, dt, nsteps, precision, skin=0.0, rebuild_every=0, want_status=False):
     import torch
     from paper_2005_00223_b200 import binding
     m = binding.DPModel(s.model, precision)
     c = torch.from_numpy(s.coords.copy()).cuda()
     vel = torch.from_numpy(v.copy()).cuda()
     t = torch.from_numpy(s.types).cuda()
-    out = m.md_run(c, vel, t, masses, s.box, dt, nsteps)
+    out = m.md_run(c, vel, t, masses, s.box, dt, nsteps, skin=skin, rebuild_every=rebuild_every)
     rc, _ = m.status()
+    if want_status:
+        m.close()
+        return rc
     assert rc == 0
     torch.cuda.synchronize()
     res = {k: x.cpu().numpy() for k, x in out.items()}
+    res["nlist"] = m.get_nlist().cpu().numpy()
     res["coords"], res["vel"] = c.cpu().numpy(), vel.cpu().numpy()
     m.close()
     return res
@@ -70,3 +74,42 @@ def test_md_mix16_conserves_total_energy():
     e = g["thermo"].sum(axis=1)
     moved = np.ptp(g["thermo"][:, 1])
     assert moved > 0 and np.abs(e - e[0]).max() < 0.05 * moved, (np.abs(e - e[0]).max(), moved)
+
+
+@pytest.mark.parametrize("idx,dt,nsteps,every", [(0, 1.0, 7, 3), (1, 0.5, 5, 4)])
+def test_md_buffered_list_gives_the_same_trajectory_and_list(idx, dt, nsteps, every):
+    # 2 A buffer; list searches at evaluations 0, every, 2 every, ...; the steps between re-test the stored
+    # candidates.  The formatted list of the LAST evaluation (a reuse step) must still be the oracle's, bit for bit.
+    from oracle import oracle
+    s = synth.config(idx)
+    masses = synth.MASS_AMU["cu" if idx == 0 else "water"]
+    v = synth.boltzmann_velocities(s.types, masses, 330.0, 4242 + idx)
+    o = md_oracle.run(s.coords, v, s.types, masses, s.box, s.model, dt, nsteps)
+    g = _gpu_md(s, v, masses, dt, nsteps, "fp64", skin=2.0, rebuild_every=every)
+    assert nsteps % every != 0
+    assert np.abs(g["coords"] - o["coords"]).max() <= 1e-11
+    assert np.abs(g["vel"] - o["vel"]).max() <= 1e-10 * np.sqrt((o["vel"] ** 2).mean())
+    assert np.abs(g["thermo"][:, 0] - o["thermo"][:, 0]).max() <= 1e-12 * abs(o["thermo"][0, 0])
+    fin = oracle.evaluate(g["coords"], s.types, s.box, s.model)
+    assert np.array_equal(g["nlist"], fin["nlist"])
+    fr = np.sqrt((fin["forces"] ** 2).mean())
+    assert np.abs(g["forces"] - fin["forces"]).max() <= 1e-10 * fr
+
+
+def test_md_buffered_list_reports_an_atom_that_outran_the_buffer():
+    s = synth.config(0)
+    v = synth.boltzmann_velocities(s.types, (63.546,), 330.0, 1)
+    v[17] = [0.3, 0.0, 0.0]                      # 0.3 A/fs: 1.5 A after 5 fs, beyond half of a 2 A buffer
+    assert _gpu_md(s, v, (63.546,), 1.0, 5, "fp64", skin=2.0, rebuild_every=50, want_status=True) == -8
+    assert _gpu_md(s, v, (63.546,), 1.0, 2, "fp64", skin=2.0, rebuild_every=50, want_status=True) == 0
+
+
+def test_md_buffered_list_mix16_matches_unbuffered_energies():
+    s = synth.config(0)
+    masses = (1.0,)
+    v = synth.boltzmann_velocities(s.types, masses, 30.0, 7)
+    a = _gpu_md(s, v, masses, 1.0, 12, "mix16")
+    b = _gpu_md(s, v, masses, 1.0, 12, "mix16", skin=2.0, rebuild_every=5)
+    swing = np.ptp(a["thermo"][:, 1])
+    assert np.abs(a["thermo"] - b["thermo"]).max() < 1e-3 * swing
+    assert np.array_equal(a["nlist"], b["nlist"]) or np.abs(a["coords"] - b["coords"]).max() > 0
