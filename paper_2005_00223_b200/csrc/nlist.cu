@@ -273,8 +273,8 @@ k_nlist(long N, int T, Grid3 g, double rc2, int cap, const int *__restrict__ bin
 // Bitonic sort of 32 R keys held R per lane (element index = lane * R + r), every merge ascending: the first stage of a
 // merge of width k pairs idx with idx ^ (k - 1), the following ones idx with idx ^ j.  Strides below R are register
 // exchanges, larger ones warp shuffles; the smaller key always goes to the smaller index (one 64-bit compare per element).
-template <int R>
-__device__ __forceinline__ void warp_sort_regs(unsigned long long (&key)[R], int lane) {
+template <int R, typename K>
+__device__ __forceinline__ void warp_sort_regs(K (&key)[R], int lane) {
 #pragma unroll
     for (int k = 2; k <= 32 * R; k <<= 1) {
         // flip stage
@@ -283,7 +283,7 @@ __device__ __forceinline__ void warp_sort_regs(unsigned long long (&key)[R], int
             for (int r = 0; r < R; ++r) {
                 const int q = r ^ (k - 1);
                 if (q > r) {
-                    const unsigned long long a = key[r], c = key[q];
+                    const K a = key[r], c = key[q];
                     const bool sw = a > c;
                     key[r] = sw ? c : a;
                     key[q] = sw ? a : c;
@@ -292,7 +292,7 @@ __device__ __forceinline__ void warp_sort_regs(unsigned long long (&key)[R], int
         } else {
             const int jl = k / R - 1;
             const bool lower = (lane & (k / (2 * R))) == 0;
-            unsigned long long o[R];
+            K o[R];
 #pragma unroll
             for (int r = 0; r < R; ++r) o[r] = __shfl_xor_sync(0xffffffffu, key[R - 1 - r], jl);
 #pragma unroll
@@ -305,7 +305,7 @@ __device__ __forceinline__ void warp_sort_regs(unsigned long long (&key)[R], int
                 for (int r = 0; r < R; ++r) {
                     const int q = r ^ j;
                     if (q > r) {
-                        const unsigned long long a = key[r], c = key[q];
+                        const K a = key[r], c = key[q];
                         const bool sw = a > c;
                         key[r] = sw ? c : a;
                         key[q] = sw ? a : c;
@@ -316,8 +316,8 @@ __device__ __forceinline__ void warp_sort_regs(unsigned long long (&key)[R], int
                 const bool lower = (lane & jl) == 0;
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
-                    const unsigned long long a = key[r];
-                    const unsigned long long o = __shfl_xor_sync(0xffffffffu, a, jl);
+                    const K a = key[r];
+                    const K o = __shfl_xor_sync(0xffffffffu, a, jl);
                     key[r] = ((a < o) == lower) ? a : o;
                 }
             }
@@ -328,10 +328,27 @@ __device__ __forceinline__ void warp_sort_regs(unsigned long long (&key)[R], int
 template <int R>
 __device__ __forceinline__ void sort_and_emit(const unsigned long long *keys, int n, int lane, int selb, const int *__restrict__ inv,
                                               int *__restrict__ out) {
+    // Sort 32-bit proxies {top 24 bits of the quantised r^2, position in keys[]} with min / max, fetch the 64-bit keys in
+    // that order and verify it; only a warp whose proxies tie (equal r^2 to 2^-17 A^2, e.g. a perfect lattice)
+    // re-sorts the 64-bit keys.  The emitted order is always the exact key order.
     unsigned long long key[R];
+    {
+        uint32_t pk[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) { const int idx = lane * R + r; key[r] = idx < n ? keys[idx] : ~0ull; }
-    warp_sort_regs<R>(key, lane);
+        for (int r = 0; r < R; ++r) {
+            const int idx = lane * R + r;
+            pk[r] = idx < n ? (((uint32_t)(keys[idx] >> 36) << 8) | (uint32_t)idx) : 0xFFFFFFFFu;   // key = q << 24 | j, q < 2^36
+        }
+        warp_sort_regs<R>(pk, lane);
+        bool bad = false;
+#pragma unroll
+        for (int r = 0; r < R; ++r) key[r] = pk[r] != 0xFFFFFFFFu ? keys[pk[r] & 255u] : ~0ull;
+#pragma unroll
+        for (int r = 0; r + 1 < R; ++r) bad |= key[r] > key[r + 1];
+        const unsigned long long nxt = __shfl_down_sync(0xffffffffu, key[0], 1);
+        bad |= lane < 31 && key[R - 1] > nxt;
+        if (__any_sync(0xffffffffu, bad)) warp_sort_regs<R>(key, lane);
+    }
     const int nkeep = n < selb ? n : selb;
 #pragma unroll
     for (int r = 0; r < R; ++r) {
@@ -351,8 +368,19 @@ __device__ __forceinline__ void sort_and_emit(const unsigned long long *keys, in
 // tests 32 consecutive flat positions per iteration with every lane busy.
 struct NlistF32 {
     float L[3], invL[3];
-    float rc2_margin;
+    float rc2_margin;        // pass-1 radius of the cell search (rc, or rc + skin when the candidates are stored), with margin
+    float rc2_margin_rc;     // rc with margin: pass 1 over stored candidates (MODE 2)
 };
+// conservative fp32 test of sorted atom s against the centre pf (minimum image: d - L rint(d / L), rint through the 1.5 * 2^23 shift)
+__device__ __forceinline__ bool near_f32(const float4 *__restrict__ xsf, int s, const float4 &pf, const NlistF32 &gf, float r2m) {
+    const float4 q = __ldg(&xsf[s]);
+    float dx = q.x - pf.x, dy = q.y - pf.y, dz = q.z - pf.z;
+    const float tx = fmaf(dx, gf.invL[0], 12582912.f) - 12582912.f;
+    const float ty = fmaf(dy, gf.invL[1], 12582912.f) - 12582912.f;
+    const float tz = fmaf(dz, gf.invL[2], 12582912.f) - 12582912.f;
+    dx = fmaf(-tx, gf.L[0], dx); dy = fmaf(-ty, gf.L[1], dy); dz = fmaf(-tz, gf.L[2], dz);
+    return fmaf(dz, dz, fmaf(dy, dy, dx * dx)) < r2m;
+}
 __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
@@ -408,9 +436,18 @@ k_nlist2(long N, int T, Grid3 g, double rc2, NlistF32 gf, int cap, const int *__
     for (int b = 0; b < T; ++b) {
         int n1 = 0;
         if (MODE == 2) {
-            n1 = candcnt[(long)b * N + i];
+            // ---- pass 1 over the stored candidates (they were within rc + skin at the last cell search) ----
+            const int total = candcnt[(long)b * N + i];
             const int *cs = cand + ((long)b * N + i) * cap;
-            for (int k = lane; k < n1; k += 32) keys[k] = (unsigned long long)cs[k];
+            for (int base = 0; base < total; base += 32) {
+                const int idx = base + lane;
+                int s = 0;
+                bool ok = false;
+                if (idx < total) { s = cs[idx]; ok = near_f32(xsf, s, pf, gf, gf.rc2_margin_rc); }
+                const unsigned mask = __ballot_sync(0xffffffffu, ok);
+                if (ok) keys[n1 + __popc(mask & lt)] = (unsigned long long)s;
+                n1 += __popc(mask);
+            }
         } else {
         // ---- run table ----
         int sA = 0, lenA = 0, sB = 0, lenB = 0;
@@ -441,16 +478,7 @@ k_nlist2(long N, int T, Grid3 g, double rc2, NlistF32 gf, int cap, const int *__
             while (idx >= e.x) e = runtab[++r];
             const int s = idx + e.y;
             bool ok = false;
-            if (idx < total && s != ii) {
-                const float4 q = __ldg(&xsf[s]);
-                float dx = q.x - pf.x, dy = q.y - pf.y, dz = q.z - pf.z;
-                // minimum image: d - L rint(d / L), rint through the 1.5 * 2^23 shift
-                const float tx = fmaf(dx, gf.invL[0], 12582912.f) - 12582912.f;
-                const float ty = fmaf(dy, gf.invL[1], 12582912.f) - 12582912.f;
-                const float tz = fmaf(dz, gf.invL[2], 12582912.f) - 12582912.f;
-                dx = fmaf(-tx, gf.L[0], dx); dy = fmaf(-ty, gf.L[1], dy); dz = fmaf(-tz, gf.L[2], dz);
-                ok = fmaf(dz, dz, fmaf(dy, dy, dx * dx)) < gf.rc2_margin;
-            }
+            if (idx < total && s != ii) ok = near_f32(xsf, s, pf, gf, gf.rc2_margin);
             const unsigned mask = __ballot_sync(0xffffffffu, ok);
             const int pos = n1 + __popc(mask & lt);
             if (ok && pos < cap) keys[pos] = (unsigned long long)s;
@@ -600,6 +628,7 @@ cudaError_t launch_nlist(const dp_model *m, long N, const Grid3 &g, char *ws, co
     for (int d = 0; d < 3; ++d) { gf.L[d] = (float)g.L[d]; gf.invL[d] = (float)(1.0 / g.L[d]); }
     const double rl = m->rc + (m->list_mode ? m->md_skin : 0.0);      // search radius of pass 1
     gf.rc2_margin = (float)(rl * rl * (1.0 + 1e-5) + 12.0 * rl * Lmax * 1.2e-7 + 1e-6);
+    gf.rc2_margin_rc = (float)(m->rc * m->rc * (1.0 + 1e-5) + 12.0 * m->rc * Lmax * 1.2e-7 + 1e-6);
     static const bool legacy = std::getenv("DP_NLIST_V1") != nullptr;
     if (!legacy) {
         static bool attr2 = false;

@@ -201,3 +201,14 @@ def test_profile_slots_and_launch_count():
     assert 0 < ms[5] <= ms[3]                  # the backward kernel alone is a part of the backward phase
     assert m.launches_per_compute() == 19      # one type: 16 + 3 T (every scan is three launches)
     m.close()
+
+
+def test_perfect_lattice_ties_are_ordered_by_index():
+    # ideal FCC: every shell is a set of exactly equal distances; the order inside a shell is the index order (PAPER.md:113:
+    # the index sits in the low digits of the key).  Exercises the 64-bit re-sort behind the 32-bit proxy sort of the list kernel.
+    s = synth.copper(5, 0.0, 12345, name="fcc_ideal")
+    o = oracle.evaluate(s.coords, s.types, s.box, s.model)
+    for prec in ("fp64", "mix16"):
+        g = _gpu_eval(s, prec)
+        assert np.array_equal(g["nlist"], o["nlist"])
+    assert (o["nlist"] >= 0).sum(axis=1).min() >= 170
