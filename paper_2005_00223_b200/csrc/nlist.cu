@@ -326,14 +326,15 @@ __device__ __forceinline__ void warp_sort_regs(K (&key)[R], int lane) {
 }
 
 template <int R>
-__device__ __forceinline__ void sort_and_emit(const unsigned long long *keys, int n, int lane, int selb, const int *__restrict__ inv,
-                                              int *__restrict__ out) {
+__device__ __forceinline__ void sort_and_emit(const unsigned long long *keys, const int *sidx, int n, int lane, int selb,
+                                              const int *__restrict__ inv, int *__restrict__ out) {
     // Sort 32-bit proxies {top 24 bits of the quantised r^2, position in keys[]} with min / max, fetch the 64-bit keys in
     // that order and verify it; only a warp whose proxies tie (equal r^2 to 2^-17 A^2, e.g. a perfect lattice)
     // re-sorts the 64-bit keys.  The emitted order is always the exact key order.
     unsigned long long key[R];
+    uint32_t pk[R];
+    bool resorted;
     {
-        uint32_t pk[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int idx = lane * R + r;
@@ -347,13 +348,15 @@ __device__ __forceinline__ void sort_and_emit(const unsigned long long *keys, in
         for (int r = 0; r + 1 < R; ++r) bad |= key[r] > key[r + 1];
         const unsigned long long nxt = __shfl_down_sync(0xffffffffu, key[0], 1);
         bad |= lane < 31 && key[R - 1] > nxt;
-        if (__any_sync(0xffffffffu, bad)) warp_sort_regs<R>(key, lane);
+        resorted = __any_sync(0xffffffffu, bad);
+        if (resorted) warp_sort_regs<R>(key, lane);
     }
     const int nkeep = n < selb ? n : selb;
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const int rank = lane * R + r;
-        if (rank < selb) out[rank] = rank < nkeep ? inv[(int)(key[r] & 0xFFFFFFull)] : -1;
+        // sorted-space index of the neighbour: kept beside the key by pass 2 (proxy order), or through inv after a re-sort
+        if (rank < selb) out[rank] = rank < nkeep ? (resorted ? inv[(int)(key[r] & 0xFFFFFFull)] : sidx[pk[r] & 255u]) : -1;
     }
     for (int k = 32 * R + lane; k < selb; k += 32) out[k] = -1;
 }
@@ -405,6 +408,7 @@ k_nlist2(long N, int T, Grid3 g, double rc2, NlistF32 gf, int cap, const int *__
     const long i = blockIdx.x * 4L + wid;
     if (i >= N) return;
     unsigned long long *keys = keys_all + (size_t)wid * cap;
+    int *sidx = reinterpret_cast<int *>(keys_all + (size_t)4 * cap) + (size_t)wid * cap;   // sorted-space index beside every key
     int2 *runtab = runtab_all[wid];
     const int sel[4] = {sel4.x, sel4.y, sel4.z, sel4.w};
     const double xi = xs[3 * i], yi = xs[3 * i + 1], zi = xs[3 * i + 2];
@@ -499,8 +503,9 @@ k_nlist2(long N, int T, Grid3 g, double rc2, NlistF32 gf, int cap, const int *__
             const int k = base + lane;
             bool ok = false;
             unsigned long long key = 0;
+            int s = 0;
             if (k < n1) {
-                const int s = (int)keys[k];
+                s = (int)keys[k];
                 double dx = min_image(__dsub_rn(xs[3 * (long)s], xi), g.L[0], hx);
                 double dy = min_image(__dsub_rn(xs[3 * (long)s + 1], yi), g.L[1], hy);
                 double dz = min_image(__dsub_rn(xs[3 * (long)s + 2], zi), g.L[2], hz);
@@ -511,15 +516,15 @@ k_nlist2(long N, int T, Grid3 g, double rc2, NlistF32 gf, int cap, const int *__
                 }
             }
             const unsigned mask = __ballot_sync(0xffffffffu, ok);      // every lane has read its entry: in-place write is safe
-            if (ok) keys[n + __popc(mask & ((1u << lane) - 1u))] = key;
+            if (ok) { const int p = n + __popc(mask & ((1u << lane) - 1u)); keys[p] = key; sidx[p] = s; }
             n += __popc(mask);
         }
         __syncwarp();
         int *out = nlist + i * Nm + off;
-        if (n <= 32) sort_and_emit<1>(keys, n, lane, sel[b], inv, out);
-        else if (n <= 64) sort_and_emit<2>(keys, n, lane, sel[b], inv, out);
-        else if (n <= 128) sort_and_emit<4>(keys, n, lane, sel[b], inv, out);
-        else if (n <= 256) sort_and_emit<8>(keys, n, lane, sel[b], inv, out);
+        if (n <= 32) sort_and_emit<1>(keys, sidx, n, lane, sel[b], inv, out);
+        else if (n <= 64) sort_and_emit<2>(keys, sidx, n, lane, sel[b], inv, out);
+        else if (n <= 128) sort_and_emit<4>(keys, sidx, n, lane, sel[b], inv, out);
+        else if (n <= 256) sort_and_emit<8>(keys, sidx, n, lane, sel[b], inv, out);
         else {
             int P = 512;
             while (P < n) P <<= 1;
@@ -613,10 +618,10 @@ cudaError_t launch_build_cells(const dp_model *m, long N, const double *coords, 
 
 cudaError_t launch_nlist(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
     const int cap = m->sort_cap;
-    const size_t smem = (size_t)4 * cap * sizeof(unsigned long long);
+    const size_t smem = (size_t)4 * cap * (sizeof(unsigned long long) + sizeof(int));   // keys + sorted-space indices
     static bool attr_set = false;
     if (!attr_set) {
-        cudaFuncSetAttribute(k_nlist, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 4096 * 8);
+        cudaFuncSetAttribute(k_nlist, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 4096 * 12);
         attr_set = true;
     }
     int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
@@ -633,9 +638,9 @@ cudaError_t launch_nlist(const dp_model *m, long N, const Grid3 &g, char *ws, co
     if (!legacy) {
         static bool attr2 = false;
         if (!attr2) {
-            cudaFuncSetAttribute(k_nlist2<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 4096 * 8);
-            cudaFuncSetAttribute(k_nlist2<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 4096 * 8);
-            cudaFuncSetAttribute(k_nlist2<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 4096 * 8);
+            cudaFuncSetAttribute(k_nlist2<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 4096 * 12);
+            cudaFuncSetAttribute(k_nlist2<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 4096 * 12);
+            cudaFuncSetAttribute(k_nlist2<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 4096 * 12);
             attr2 = true;
         }
         auto kern = m->list_mode == 1 ? k_nlist2<1> : (m->list_mode == 2 ? k_nlist2<2> : k_nlist2<0>);
