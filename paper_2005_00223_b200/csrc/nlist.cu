@@ -375,13 +375,17 @@ struct NlistF32 {
     float rc2_margin_rc;     // rc with margin: pass 1 over stored candidates (MODE 2)
 };
 // conservative fp32 test of sorted atom s against the centre pf (minimum image: d - L rint(d / L), rint through the 1.5 * 2^23 shift)
+// WRAP = false: the caller knows that the plain difference is the minimum image (interior centre, see k_nlist2)
+template <bool WRAP = true>
 __device__ __forceinline__ bool near_f32(const float4 *__restrict__ xsf, int s, const float4 &pf, const NlistF32 &gf, float r2m) {
     const float4 q = __ldg(&xsf[s]);
     float dx = q.x - pf.x, dy = q.y - pf.y, dz = q.z - pf.z;
-    const float tx = fmaf(dx, gf.invL[0], 12582912.f) - 12582912.f;
-    const float ty = fmaf(dy, gf.invL[1], 12582912.f) - 12582912.f;
-    const float tz = fmaf(dz, gf.invL[2], 12582912.f) - 12582912.f;
-    dx = fmaf(-tx, gf.L[0], dx); dy = fmaf(-ty, gf.L[1], dy); dz = fmaf(-tz, gf.L[2], dz);
+    if (WRAP) {
+        const float tx = fmaf(dx, gf.invL[0], 12582912.f) - 12582912.f;
+        const float ty = fmaf(dy, gf.invL[1], 12582912.f) - 12582912.f;
+        const float tz = fmaf(dz, gf.invL[2], 12582912.f) - 12582912.f;
+        dx = fmaf(-tx, gf.L[0], dx); dy = fmaf(-ty, gf.L[1], dy); dz = fmaf(-tz, gf.L[2], dz);
+    }
     return fmaf(dz, dz, fmaf(dy, dy, dx * dx)) < r2m;
 }
 __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
@@ -435,6 +439,10 @@ k_nlist2(long N, int T, Grid3 g, double rc2, NlistF32 gf, int cap, const int *__
     if (zlo < 0) { zb0 = zlo + g.nc[2]; zb1 = g.nc[2] - 1; }
     else if (zhi >= g.nc[2]) { zb0 = 0; zb1 = zhi - g.nc[2]; }
     const unsigned lt = (1u << lane) - 1u;
+    // Interior centre: the searched cells do not wrap on any axis and span less than half the box ((reach + 1) cell widths
+    // < L / 2), so the plain coordinate difference of every candidate is its minimum image: pass 1 skips the wrap arithmetic.
+    const bool interior = cx + lo0 >= 0 && cx + hi0 < g.nc[0] && cy + lo1 >= 0 && cy + hi1 < g.nc[1] && zlo >= 0 && zhi < g.nc[2] &&
+                          g.nc[0] > 2 * (R_ + 1) && g.nc[1] > 2 * (R_ + 1) && g.nc[2] > 2 * (R_ + 1);
     bool truncated = false;
     int off = 0;
     for (int b = 0; b < T; ++b) {
@@ -482,7 +490,7 @@ k_nlist2(long N, int T, Grid3 g, double rc2, NlistF32 gf, int cap, const int *__
             while (idx >= e.x) e = runtab[++r];
             const int s = idx + e.y;
             bool ok = false;
-            if (idx < total && s != ii) ok = near_f32(xsf, s, pf, gf, gf.rc2_margin);
+            if (idx < total && s != ii) ok = interior ? near_f32<false>(xsf, s, pf, gf, gf.rc2_margin) : near_f32<true>(xsf, s, pf, gf, gf.rc2_margin);
             const unsigned mask = __ballot_sync(0xffffffffu, ok);
             const int pos = n1 + __popc(mask & lt);
             if (ok && pos < cap) keys[pos] = (unsigned long long)s;
