@@ -485,27 +485,32 @@ k_nlist2(long N, int T, Grid3 g, double rc2, NlistF32 gf, int cap, const int *__
         // ---- pass 1: conservative fp32 filter ----
         int r = 0;
         int2 e = runtab[0];
-        // two candidates per lane and iteration (both gathers in flight); a position past the range tests the centre itself
-        for (int base = 0; base < total; base += 64) {
-            const int idx0 = base + lane, idx1 = idx0 + 32;
-            while (idx0 >= e.x) e = runtab[++r];
-            const int s0 = idx0 < total ? idx0 + e.y : ii;
-            while (idx1 >= e.x) e = runtab[++r];
-            const int s1 = idx1 < total ? idx1 + e.y : ii;
-            bool ok0, ok1;
-            if (interior) {
-                ok0 = near_f32<false>(xsf, s0, pf, gf, gf.rc2_margin);
-                ok1 = near_f32<false>(xsf, s1, pf, gf, gf.rc2_margin);
-            } else {
-                ok0 = near_f32<true>(xsf, s0, pf, gf, gf.rc2_margin);
-                ok1 = near_f32<true>(xsf, s1, pf, gf, gf.rc2_margin);
+        // PU candidates per lane and iteration (their gathers in flight together); a position past the range tests the centre itself
+        constexpr int PU = 4;
+        for (int base = 0; base < total; base += 32 * PU) {
+            int sv[PU];
+            bool okv[PU];
+#pragma unroll
+            for (int u = 0; u < PU; ++u) {
+                const int idx = base + 32 * u + lane;
+                while (idx >= e.x) e = runtab[++r];
+                sv[u] = idx < total ? idx + e.y : ii;
             }
-            ok0 &= s0 != ii; ok1 &= s1 != ii;
-            const unsigned mask0 = __ballot_sync(0xffffffffu, ok0), mask1 = __ballot_sync(0xffffffffu, ok1);
-            const int pos0 = n1 + __popc(mask0 & lt), pos1 = n1 + __popc(mask0) + __popc(mask1 & lt);
-            if (ok0 && pos0 < cap) keys[pos0] = (unsigned long long)s0;
-            if (ok1 && pos1 < cap) keys[pos1] = (unsigned long long)s1;
-            n1 += __popc(mask0) + __popc(mask1);
+            if (interior) {
+#pragma unroll
+                for (int u = 0; u < PU; ++u) okv[u] = near_f32<false>(xsf, sv[u], pf, gf, gf.rc2_margin);
+            } else {
+#pragma unroll
+                for (int u = 0; u < PU; ++u) okv[u] = near_f32<true>(xsf, sv[u], pf, gf, gf.rc2_margin);
+            }
+#pragma unroll
+            for (int u = 0; u < PU; ++u) {
+                const bool ok = okv[u] && sv[u] != ii;
+                const unsigned mask = __ballot_sync(0xffffffffu, ok);
+                const int pos = n1 + __popc(mask & lt);
+                if (ok && pos < cap) keys[pos] = (unsigned long long)sv[u];
+                n1 += __popc(mask);
+            }
         }
         if (n1 > cap) { if (lane == 0) atomicOr(&status[0], 2); n1 = cap; }
         __syncwarp();
