@@ -521,27 +521,35 @@ k_nlist2(long N, int T, Grid3 g, double rc2, NlistF32 gf, int cap, const int *__
         }
         }
         __syncwarp();
-        // ---- pass 2: exact test + key on the survivors, compacted in place ----
+        // ---- pass 2: exact test + key on the survivors, compacted in place; two entries per lane and iteration with
+        // unconditional gathers (an entry past the end tests the centre itself and is dropped) ----
         int n = 0;
-        for (int base = 0; base < n1; base += 32) {
-            const int k = base + lane;
-            bool ok = false;
-            unsigned long long key = 0;
-            int s = 0;
-            if (k < n1) {
-                s = (int)keys[k];
-                double dx = min_image(__dsub_rn(xs[3 * (long)s], xi), g.L[0], hx);
-                double dy = min_image(__dsub_rn(xs[3 * (long)s + 1], yi), g.L[1], hy);
-                double dz = min_image(__dsub_rn(xs[3 * (long)s + 2], zi), g.L[2], hz);
-                double r2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
-                if (r2 < rc2) {
-                    ok = true;
-                    key = (__double2ull_rd(r2 * 536870912.0) << 24) | (unsigned long long)perm[s];
-                }
+        for (int base = 0; base < n1; base += 64) {
+            int sv[2];
+            double r2v[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const int k = base + 32 * u + lane;
+                sv[u] = k < n1 ? (int)keys[k] : ii;
             }
-            const unsigned mask = __ballot_sync(0xffffffffu, ok);      // every lane has read its entry: in-place write is safe
-            if (ok) { const int p = n + __popc(mask & ((1u << lane) - 1u)); keys[p] = key; sidx[p] = s; }
-            n += __popc(mask);
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const long s3 = 3 * (long)sv[u];
+                const double dx = min_image(__dsub_rn(xs[s3], xi), g.L[0], hx);
+                const double dy = min_image(__dsub_rn(xs[s3 + 1], yi), g.L[1], hy);
+                const double dz = min_image(__dsub_rn(xs[s3 + 2], zi), g.L[2], hz);
+                r2v[u] = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
+            }
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const bool ok = r2v[u] < rc2 && sv[u] != ii;
+                unsigned long long key = 0;
+                if (ok) key = (__double2ull_rd(r2v[u] * 536870912.0) << 24) | (unsigned long long)perm[sv[u]];
+                // every lane has read both of its entries, and this batch writes below the entries of the next one
+                const unsigned mask = __ballot_sync(0xffffffffu, ok);
+                if (ok) { const int p = n + __popc(mask & lt); keys[p] = key; sidx[p] = sv[u]; }
+                n += __popc(mask);
+            }
         }
         __syncwarp();
         int *out = nlist + i * Nm + off;
