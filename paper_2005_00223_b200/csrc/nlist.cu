@@ -451,14 +451,20 @@ k_nlist2(long N, int T, Grid3 g, double rc2, NlistF32 gf, int cap, const int *__
             // ---- pass 1 over the stored candidates (they were within rc + skin at the last cell search) ----
             const int total = candcnt[(long)b * N + i];
             const int *cs = cand + ((long)b * N + i) * cap;
-            for (int base = 0; base < total; base += 32) {
-                const int idx = base + lane;
-                int s = 0;
-                bool ok = false;
-                if (idx < total) { s = cs[idx]; ok = near_f32(xsf, s, pf, gf, gf.rc2_margin_rc); }
-                const unsigned mask = __ballot_sync(0xffffffffu, ok);
-                if (ok) keys[n1 + __popc(mask & lt)] = (unsigned long long)s;
-                n1 += __popc(mask);
+            for (int base = 0; base < total; base += 128) {       // four candidates per lane and iteration, as in the cell search
+                int sv[4];
+                bool okv[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) { const int idx = base + 32 * u + lane; sv[u] = idx < total ? cs[idx] : ii; }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) okv[u] = near_f32(xsf, sv[u], pf, gf, gf.rc2_margin_rc);
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const bool ok = okv[u] && sv[u] != ii;
+                    const unsigned mask = __ballot_sync(0xffffffffu, ok);
+                    if (ok) keys[n1 + __popc(mask & lt)] = (unsigned long long)sv[u];
+                    n1 += __popc(mask);
+                }
             }
         } else {
         // ---- run table ----
