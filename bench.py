@@ -280,7 +280,7 @@ def main():
             md_ms = m0.elapsed_time(m1)
             md = {"steps": args.md_steps, "evaluations": args.md_steps + 1, "dt_fs": dt_fs, "temperature_K": 330.0,
                   "loop_ms_per_step": md_ms / args.md_steps, "s_per_step_per_atom": md_ms * 1e-3 / args.md_steps / N,
-                  "status": rc_md, "e_total_first_last_eV": [float(th[0].sum()), float(th[-1].sum())],
+                  "status": rc_md, "e_total_first_last_eV": [float(th[0, :2].sum()), float(th[-1, :2].sum())],
                   "e_kin_first_eV": float(th[0, 1]),
                   "skin_A": 2.0, "rebuild_every": 50,
                   "note": "velocity Verlet, 2 A buffered list searched at evaluation 0 and every 50 (PAPER.md:153), "

@@ -38,11 +38,11 @@ typedef enum { DP_FP64 = 0, DP_MIX32 = 1, DP_MIX16 = 2 } dp_precision;
 
 typedef enum {
     DP_OK = 0,
-    DP_EINVAL = -1,   /* null pointer, natoms <= 0, rc_smth >= rc, rc*rc >= 128, sel <= 0, unsupported widths */
+    DP_EINVAL = -1,   /* null pointer, natoms <= 0 or > 2^24, natoms * max(sel) >= 2^31, rc_smth >= rc, rc*rc >= 128, sel <= 0 */
     DP_EBOX = -2,     /* box not orthorhombic, or a box length < 2*rc                                        */
     DP_ENOMEM = -3,   /* workspace_bytes < dp_workspace_bytes(model, natoms)                                  */
     DP_ETYPE = -4,    /* an atom type outside type_map (detected on device, reported by dp_status)            */
-    DP_ECUDA = -5,    /* CUDA runtime error or no device                                                      */
+    DP_ECUDA = -5,    /* CUDA runtime error, no device, or the current device is not the one the model was created on */
     DP_ENEIGH = -6,   /* an atom has more candidates inside rc than the sort buffer holds (dp_status)         */
     DP_EUNSUPPORTED = -7, /* precision mode / shape not built                                                */
     DP_ESKIN = -8     /* dp_md_run with a buffered list: an atom moved > skin/2 since the list was built (dp_status) */
@@ -112,6 +112,7 @@ int dp_last_row_counts(dp_model *m, long *rows_forward, long *rows_backward);
 int dp_profile_enable(dp_model *m, int on);
 int dp_profile_read(dp_model *m, double *ms_host);
 
+#define DP_MD_NTHERMO 4   /* doubles per thermo record of dp_md_run */
 /* Velocity-Verlet MD loop around dp_compute (section VI-A: "the MD equations are numerically
  * integrated by the velocity-Verlet scheme for 500 steps (the energy and forces are evaluated for 501 times)").
  * One evaluation at the input coordinates, then nsteps times: v += (dt/2) a; x += dt v; evaluate; v += (dt/2) a,
@@ -126,10 +127,14 @@ int dp_profile_read(dp_model *m, double *ms_host);
  *   moved more than skin/2 since the last search (checked on the device: DP_ESKIN from dp_status).  skin = 0 or
  *   rebuild_every <= 1: every evaluation searches the cells.
  *   workspace_dev: >= dp_md_workspace_bytes(m, natoms, skin) bytes (skin = 0 if not buffered), 256-byte aligned;
- *   forces_dev [natoms][3]: forces at the final coordinates;  thermo_dev [nsteps + 1][2] fp64: potential energy E and
- *   kinetic energy sum 1/2 m v^2 (both eV) after evaluation 0 .. nsteps;  virial_dev [9] or NULL: virial of the last
- *   evaluation.  Only enqueues on cuda_stream (no host synchronisation, no allocation); dp_status afterwards reports the
- *   LAST evaluation.  Errors as dp_compute; DP_EINVAL for bad masses, dt_fs, skin < 0, nsteps < 0 or rebuild_every < 0. */
+ *   forces_dev [natoms][3]: forces at the final coordinates;  thermo_dev [nsteps + 1][DP_MD_NTHERMO] fp64, one record per
+ *   evaluation 0 .. nsteps ("kinetic energy, potential energy, temperature, pressure, are collected"):
+ *   [0] potential energy E (eV), [1] kinetic energy sum 1/2 m v^2 (eV), [2] temperature 2 KE / ((3 natoms - 3) kB) (K),
+ *   [3] pressure (2 KE + trace(virial)) / (3 V) (bar);  virial_dev [9] or NULL: virial of the last evaluation.
+ *   Only enqueues on cuda_stream (no host synchronisation, no allocation).  dp_status afterwards reports the device-detected
+ *   conditions of the WHOLE run (the flags of all nsteps + 1 evaluations are OR-ed: DP_ETYPE, DP_ENEIGH, DP_ESKIN) and the
+ *   truncation count of the last evaluation.  Errors as dp_compute; DP_EINVAL for bad masses, dt_fs, skin < 0, nsteps < 0 or
+ *   rebuild_every < 0. */
 size_t dp_md_workspace_bytes(const dp_model *m, long natoms, double skin);
 int dp_md_run(dp_model *m, long natoms, double *coords_dev, double *vel_dev, const int *types_dev,
               const double *mass_host, int n_mass, const double *box_host, double dt_fs, int nsteps,

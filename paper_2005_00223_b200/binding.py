@@ -149,7 +149,7 @@ class DPModel:
                want_virial=True):
         """Velocity-Verlet loop (dp_md_run): coords, vel [N,3] f64 cuda are advanced IN PLACE by nsteps steps of dt_fs;
         masses: amu per user type; skin > 0 and rebuild_every > 1: buffered neighbour list.
-        Enqueues only; returns forces [N,3], thermo [nsteps+1,2] (E_pot, E_kin in eV), virial."""
+        Enqueues only; returns forces [N,3], thermo [nsteps+1,4] (E_pot eV, E_kin eV, T K, P bar), virial."""
         import torch
         for x in (coords, vel):
             assert x.is_cuda and x.dtype == torch.float64 and x.is_contiguous()
@@ -164,7 +164,7 @@ class DPModel:
             self._ws = torch.empty(need, dtype=torch.uint8, device=dev)
         ws = self._ws
         out = dict(forces=torch.empty((n, 3), dtype=torch.float64, device=dev),
-                   thermo=torch.empty((int(nsteps) + 1, 2), dtype=torch.float64, device=dev),
+                   thermo=torch.empty((int(nsteps) + 1, 4), dtype=torch.float64, device=dev),
                    virial=torch.empty(9, dtype=torch.float64, device=dev))
         boxh = np.ascontiguousarray(np.asarray(box, dtype=np.float64).reshape(9))
         mh = np.ascontiguousarray(masses, dtype=np.float64)

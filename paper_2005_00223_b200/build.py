@@ -1,31 +1,49 @@
-"""Build libdp_b200.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a."""
+"""Build libdp_b200.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a.
+
+Every .cu is compiled to an object under paper_2005_00223_b200/_obj/ (objects are git-ignored) in parallel, only when it or a
+header is newer than the object, then linked into libdp_b200.so next to this file (the .so travels to the GPU box).
+"""
 from __future__ import annotations
 
 import os
 import subprocess
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "_obj")
 LIB = os.path.join(HERE, "libdp_b200.so")
-SOURCES = ["dp_api.cu", "nlist.cu", "embed_f64.cu", "fit_f64.cu", "embed_mix.cu", "fit_mix.cu", "embed_tc.cu", "embed_tc2.cu", "embed_tc2_bwd.cu", "fit_tc.cu", "md.cu"]
-NVCC_FLAGS = os.environ.get("DP_EXTRA_NVCC", "").split() + ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "--shared", "-cudart", "shared"]
+NVCC_FLAGS = os.environ.get("DP_EXTRA_NVCC", "").split() + ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo",
+                                                            "-std=c++17", "-Xcompiler", "-fPIC"]
 
 
-def _stale() -> bool:
-    if not os.path.exists(LIB):
-        return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(HERE, "..", "include", "dp.h")]
-    return any(os.path.getmtime(d) > t for d in deps)
+def sources():
+    return sorted(f for f in os.listdir(CSRC) if f.endswith(".cu"))
+
+
+def _headers_mtime() -> float:
+    hs = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".h", ".cuh"))]
+    hs.append(os.path.join(HERE, "..", "include", "dp.h"))
+    return max(os.path.getmtime(h) for h in hs)
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    if force or _stale():
-        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-              [os.path.join(CSRC, s) for s in SOURCES] + ["-o", LIB]
-        subprocess.check_call(cmd)
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    os.makedirs(OBJ, exist_ok=True)
+    hm = _headers_mtime()
+    jobs = []
+    for s in sources():
+        src, obj = os.path.join(CSRC, s), os.path.join(OBJ, s[:-3] + ".o")
+        if force or not os.path.exists(obj) or os.path.getmtime(obj) < max(os.path.getmtime(src), hm):
+            jobs.append([nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj])
+    if jobs:
+        with ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 4)) as ex:
+            for rc in ex.map(lambda c: subprocess.run(c).returncode, jobs):
+                if rc != 0:
+                    raise RuntimeError("nvcc failed")
+    objs = [os.path.join(OBJ, s[:-3] + ".o") for s in sources()]
+    if jobs or not os.path.exists(LIB) or any(os.path.getmtime(o) > os.path.getmtime(LIB) for o in objs):
+        subprocess.check_call([nvcc, "--shared", "-cudart", "shared", "-gencode", "arch=compute_100a,code=sm_100a"] + objs + ["-o", LIB])
     return LIB
 
 

@@ -59,6 +59,12 @@ WsLayout ws_layout(const dp_model *m, long N) {
     return L;
 }
 
+// row offsets (N * off[b] + prefix sums of the rows per atom) are 32-bit: natoms * max(sel) must stay below 2^31
+bool rows_fit_int32(const dp_model *m, long N) {
+    for (int b = 0; b < m->T; ++b) if ((long)N * m->sel[b] >= (1L << 31)) return false;
+    return true;
+}
+
 bool make_grid(const dp_model *m, long N, const double *box, Grid3 *g) {
     if (box[1] != 0 || box[2] != 0 || box[3] != 0 || box[5] != 0 || box[6] != 0 || box[7] != 0) return false;
     const double Ls[3] = {box[0], box[4], box[8]};
@@ -75,7 +81,6 @@ bool make_grid(const dp_model *m, long N, const double *box, Grid3 *g) {
         if (g->nc[a] < 5) g->reach = 1;
     }
     if ((long)g->nc[0] * g->nc[1] * g->nc[2] > cap) g->reach = 1;
-    if (std::getenv("DP_NLIST_REACH1")) g->reach = 1;
     if (g->reach == 1)
         for (int a = 0; a < 3; ++a) {
             int nc = (int)std::floor(Ls[a] / (rl * (1.0 + 1e-9)));
@@ -333,24 +338,9 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
     dp_model *m = new (std::nothrow) dp_model();
     if (!m) return DP_EINVAL;
     std::memset(m, 0, sizeof(*m));
+    m->device = dev;
     m->T = T; m->Nm = Nm; m->axis = 16; m->F = 240; m->rc = rc; m->rc_smth = rc_smth; m->prec = prec;
     m->n_type_map = n_type_map;
-    if (prec == DP_MIX32) { m->mix_ns = 3; m->mix_nsc = 3; m->mix_tanh_approx = 0; m->mix_fit_ns = 3; m->mix_fit3_ns = 3; }
-    if (prec == DP_MIX16) {
-        // defaults from the precision study in DESIGN.md: fp16 weights, activations carried as hi + lo fp16 pairs
-        m->mix_ns = 2; m->mix_nsc = 3; m->mix_tanh_approx = 1; m->mix_fit_ns = 2; m->mix_fit3_ns = 2; m->mix_ns_bwd = 1;
-        if (const char *e = std::getenv("DP_MIX16_NS_BWD")) m->mix_ns_bwd = std::atoi(e) == 1 ? 1 : 2;
-        if (const char *e = std::getenv("DP_MIX16_NS")) { int v = std::atoi(e); if (v >= 1 && v <= 2) m->mix_ns = v; }
-        if (const char *e = std::getenv("DP_MIX16_NSC")) m->mix_nsc = std::atoi(e) == 3 ? 3 : 1;
-        if (const char *e = std::getenv("DP_MIX16_TANH_APPROX")) m->mix_tanh_approx = std::atoi(e) ? 1 : 0;
-        if (const char *e = std::getenv("DP_MIX16_FIT_NS")) { int v = std::atoi(e); if (v >= 1 && v <= 3) m->mix_fit_ns = v; }
-        if (const char *e = std::getenv("DP_MIX16_FIT3_NS")) { int v = std::atoi(e); if (v >= 1 && v <= 3) m->mix_fit3_ns = v; }
-    }
-    m->mix_ns_fwd = m->mix_ns; m->mix_nsc_fwd = m->mix_nsc;
-    if (prec == DP_MIX16) {
-        if (const char *e = std::getenv("DP_MIX16_NS_FWD")) { int v = std::atoi(e); if (v >= 1 && v <= 2) m->mix_ns_fwd = v; }
-        if (const char *e = std::getenv("DP_MIX16_NSC_FWD")) m->mix_nsc_fwd = std::atoi(e) == 3 ? 3 : 1;
-    }
     for (int b = 0; b < T; ++b) { m->sel[b] = sel[b]; m->off[b + 1] = m->off[b] + sel[b]; }
     int cap = 256;
     while (cap < 2 * maxsel) cap <<= 1;
@@ -370,35 +360,18 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
         std::vector<EmbedNetFrag<double>> frags((size_t)T * T);
         for (int ab = 0; ab < T * T; ++ab) build_embed_frag<double>(w->embed + ab * ensz, &frags[ab]);
         ok(upload(frags, &m->embed_frag_dev));
-    } else if (prec == DP_MIX32) {
+    } else if (prec == DP_MIX32) {      // tcgen05 forward (embed_tc.cu), mma.sync backward (embed_mix.cu): weights as hi + lo fp16
         std::vector<EmbedNetFragH<2>> frags((size_t)T * T);
         for (int ab = 0; ab < T * T; ++ab) build_embed_frag_h<2>(w->embed + ab * ensz, &frags[ab]);
         ok(upload(frags, &m->embed_frag_dev));
-    } else {
-        std::vector<EmbedNetFragH<1>> frags((size_t)T * T);
-        for (int ab = 0; ab < T * T; ++ab) build_embed_frag_h<1>(w->embed + ab * ensz, &frags[ab]);
-        ok(upload(frags, &m->embed_frag_dev));
-    }
-    if (prec == DP_MIX32) {
         std::vector<EmbedNetTC<2>> nets((size_t)T * T);
         for (int ab = 0; ab < T * T; ++ab) build_embed_tc<2>(w->embed + ab * ensz, &nets[ab]);
         ok(upload(nets, &m->embed_tc_dev));
-    } else if (prec == DP_MIX16) {
-        std::vector<EmbedNetTC<1>> nets((size_t)T * T);
-        for (int ab = 0; ab < T * T; ++ab) build_embed_tc<1>(w->embed + ab * ensz, &nets[ab]);
-        ok(upload(nets, &m->embed_tc_dev));
-    }
-    if (prec == DP_MIX16) {
+    } else {                            // MIX-16: warpgroup-per-tile tcgen05 kernels (embed_tc2*.cu)
         std::vector<EmbedNetTC2> nets((size_t)T * T);
         for (int ab = 0; ab < T * T; ++ab) build_embed_tc2(w->embed + ab * ensz, &nets[ab]);
         ok(upload(nets, &m->embed_tc2_dev));
     }
-    // embedding forward: 0 = mma.sync kernels, 1 = first tcgen05 kernel, 2 = warpgroup-per-tile tcgen05 kernel (MIX-16)
-    m->use_tc = prec == DP_MIX16 ? 2 : 1;
-    if (const char *e = std::getenv("DP_EMBED_TC")) { int v = std::atoi(e); if (v >= 0 && v <= (prec == DP_MIX16 ? 2 : 1)) m->use_tc = v; }
-    m->use_tc_bwd = prec == DP_MIX16 ? 1 : 0;
-    if (const char *e = std::getenv("DP_EMBED_TC_BWD")) m->use_tc_bwd = (prec == DP_MIX16 && std::atoi(e)) ? 1 : 0;
-    if (m->use_tc == 0) m->use_tc_bwd = 0;      // the tcgen05 backward reads the compact rows the tcgen05 forward builds
     const int ND = M2E * 16, F = 240;
     const size_t fnsz = (size_t)ND * F + F + (size_t)F * F + F + (size_t)F * F + F + F + 1;
     std::vector<double> V1((size_t)T * ND * F), V2((size_t)T * F * F), V3((size_t)T * F * F), c1(T * F), c2(T * F),
@@ -424,11 +397,8 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
         ok(upload(f32(c1), &m->fitc1_dev)); ok(upload(f32(c2), &m->fitc2_dev)); ok(upload(f32(c3), &m->fitc3_dev));
         ok(upload(f32(v4), &m->fitv4_dev)); ok(upload(f32(c4), &m->fitc4_dev));
     }
-    // tcgen05 fitting GEMMs: fp16 weight images; used when every fitting product carries its activations as hi + lo and
-    // its weights as single fp16 values (the MIX-16 default)
-    m->use_fit_tc = (prec == DP_MIX16 && m->mix_fit_ns == 2 && m->mix_fit3_ns == 2) ? 1 : 0;
-    if (const char *e = std::getenv("DP_FIT_TC")) if (!std::atoi(e)) m->use_fit_tc = 0;
-    if (m->use_fit_tc) {
+    // MIX-16: tcgen05 fitting GEMMs (fit_tc.cu) take fp16 weight images; activations are carried as hi + lo fp16 pairs
+    if (prec == DP_MIX16) {
         std::vector<__half> img((size_t)T * fit_tc_type_elems());
         for (int a = 0; a < T; ++a)
             fit_tc_build_type(&V1[(size_t)a * ND * F], &V2[(size_t)a * F * F], &V3[(size_t)a * F * F], &img[(size_t)a * fit_tc_type_elems()]);
@@ -451,22 +421,20 @@ void dp_destroy(dp_model *m) {
 }
 
 size_t dp_workspace_bytes(const dp_model *m, long natoms) {
-    if (!m || natoms <= 0 || natoms > 16777216) return 0;
+    if (!m || natoms <= 0 || natoms > 16777216 || !rows_fit_int32(m, natoms)) return 0;
     return ws_layout(m, natoms).total;
 }
 
 int dp_launches_per_compute(const dp_model *m) {
     if (!m) return 0;
-    // default paths (the DP_* debug switches that split or merge kernels are not counted)
     int n = 6 + 1;                                   // wrap, 3-launch bin scan, scatter, bin sort; list
     if (m->prec == DP_FP64) {
         n += 1 + 9 + 1;                              // forward; descriptor, 6 GEMMs, energy, gA; backward (with S8, S9)
     } else {
         n += 3 * m->T;                               // row prefix sums, one 3-launch scan per neighbour type
-        n += m->use_tc ? 2 : 1;                      // environment rows + tcgen05 forward, or the mma.sync forward
-        if (m->use_fit_tc) n += 3 + (m->use_tc_bwd ? 0 : 1);   // first layer, fused 240 x 240 chain, last product (+ gA fragments)
-        else n += m->use_tc_bwd ? 8 : 9;             // descriptor, 6 GEMMs, energy (+ gA fragments)
-        n += m->use_tc_bwd ? 3 : 1;                  // gA fold / images, tcgen05 backward, force + virial; or the mma.sync backward
+        n += 2;                                      // environment rows + tcgen05 forward
+        if (m->prec == DP_MIX16) n += 3 + 3;         // first layer, fused 240 x 240 chain, last product; gA fold, backward, force + virial
+        else n += 9 + 1;                             // descriptor, 6 GEMMs, energy, gA fragments; backward (with S8, S9)
     }
     return n + 1;                                    // finalize
 }
@@ -478,6 +446,9 @@ int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *ty
         !energy_dev || !forces_dev)
         return DP_EINVAL;
     if (((uintptr_t)workspace_dev & 255) != 0) return DP_EINVAL;
+    if (!rows_fit_int32(m, natoms)) return DP_EINVAL;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != m->device) return DP_ECUDA;    // weights live on the device of dp_create
     Grid3 g;
     if (!make_grid(m, natoms, box_host, &g)) return DP_EBOX;
     const WsLayout L = ws_layout(m, natoms);
@@ -486,7 +457,9 @@ int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *ty
     char *ws = (char *)workspace_dev;
     cudaError_t e = cudaSuccess;
     auto ok = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
-    ok(cudaMemsetAsync(ws + L.status, 0, 64, st));
+    // status word 0 = error flags: cleared per call, except inside one dp_md_run, where they accumulate (dp_status then
+    // reports the whole run); the counters behind it are per evaluation
+    ok(m->keep_flags ? cudaMemsetAsync(ws + L.status + 4, 0, 60, st) : cudaMemsetAsync(ws + L.status, 0, 64, st));
     ok(cudaMemsetAsync(ws + L.fsorted, 0, sizeof(double) * 3 * (size_t)natoms, st));
     ok(cudaMemsetAsync(ws + L.virial, 0, sizeof(double) * 16, st));
     ok(cudaMemsetAsync(energy_dev, 0, sizeof(double), st));
@@ -497,14 +470,14 @@ int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *ty
     ok(launch_nlist(m, natoms, g, ws, L, st));
     mark(1);
     const bool f64 = m->prec == DP_FP64;
+    const bool m16 = m->prec == DP_MIX16;
     ok(f64 ? launch_embed_fwd_f64(m, natoms, g, ws, L, st)
-           : (m->use_tc == 2 ? launch_embed_fwd_tc2(m, natoms, g, ws, L, st)
-              : (m->use_tc ? launch_embed_fwd_tc(m, natoms, g, ws, L, st) : launch_embed_fwd_mix(m, natoms, g, ws, L, st))));
+           : (m16 ? launch_embed_fwd_tc2(m, natoms, g, ws, L, st) : launch_embed_fwd_tc(m, natoms, g, ws, L, st)));
     mark(2);
-    ok(f64 ? launch_fit_f64(m, natoms, g, ws, L, st) : launch_fit_mix(m, natoms, g, ws, L, st));
+    ok(f64 ? launch_fit_f64(m, natoms, g, ws, L, st) : (m16 ? launch_fit_tc(m, natoms, g, ws, L, st) : launch_fit_mix(m, natoms, g, ws, L, st)));
     mark(3);
     ok(f64 ? launch_embed_bwd_f64(m, natoms, g, ws, L, st)
-           : (m->use_tc_bwd ? launch_embed_bwd_tc2(m, natoms, g, ws, L, st) : launch_embed_bwd_mix(m, natoms, g, ws, L, st)));
+           : (m16 ? launch_embed_bwd_tc2(m, natoms, g, ws, L, st) : launch_embed_bwd_mix(m, natoms, g, ws, L, st)));
     mark(4);
     ok(launch_finalize(m, natoms, ws, L, energy_dev, atom_energy_dev, forces_dev, virial_dev, st));
     mark(5);
@@ -531,7 +504,7 @@ int dp_profile_read(dp_model *m, double *ms_host) {
         ms_host[k] = ms;
     }
     ms_host[5] = ms_host[3];
-    if (m->use_tc_bwd) {
+    if (m->prec == DP_MIX16) {
         float ms = 0.f;
         if (cudaEventElapsedTime(&ms, m->ev[6], m->ev[7]) != cudaSuccess) return DP_ECUDA;
         ms_host[5] = ms;

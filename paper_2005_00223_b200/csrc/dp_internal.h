@@ -3,7 +3,22 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stddef.h>
+#include <atomic>
 #include "../../include/dp.h"
+
+// One-time opt-in of a kernel to more than 48 KB of dynamic shared memory.  The attribute belongs to the device context,
+// so the "done" flag is per device (bit = device ordinal) and per call site; the return code is checked.
+#define DP_SMEM_OPTIN(kern, bytes)                                                                                      \
+    do {                                                                                                                \
+        static std::atomic<unsigned long long> done_{0ull};                                                             \
+        int dev_ = 0;                                                                                                   \
+        if (cudaGetDevice(&dev_) != cudaSuccess) return cudaErrorInvalidDevice;                                         \
+        if (!((done_.load(std::memory_order_acquire) >> (dev_ & 63)) & 1ull)) {                                         \
+            const cudaError_t e_ = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bytes)); \
+            if (e_ != cudaSuccess) return e_;                                                                           \
+            done_.fetch_or(1ull << (dev_ & 63), std::memory_order_release);                                             \
+        }                                                                                                               \
+    } while (0)
 
 #define DP_MAX_TYPES 4
 #define DP_NEVENTS 8
@@ -48,13 +63,11 @@ struct dp_model {
     int n_type_map;
     int *type_map_dev;
     // device weights
-    void *embed_frag_dev;           // T*T EmbedNetFrag<TW>
-    void *embed_tc_dev;             // T*T EmbedNetTC<NSW> (mixed modes, tcgen05 path)
-    void *embed_tc2_dev;            // T*T EmbedNetTC2 (MIX-16, warpgroup-per-tile tcgen05 path)
-    int use_tc;                     // mixed modes: embedding forward on tcgen05
-    int use_tc_bwd;                 // MIX-16: embedding backward on tcgen05
-    int use_fit_tc;                 // mixed modes with activation-split fitting products: fitting GEMMs on tcgen05
-    void *fit_tc_img_dev;           // T x six fp16 weight images (fit_tc.cu)
+    void *embed_frag_dev;           // T*T EmbedNetFrag<double> (FP64) / EmbedNetFragH<2> (MIX-32 backward, mma.sync)
+    void *embed_tc_dev;             // T*T EmbedNetTC<2> (MIX-32 forward, tcgen05)
+    void *embed_tc2_dev;            // T*T EmbedNetTC2 (MIX-16, warpgroup-per-tile tcgen05 kernels)
+    void *fit_tc_img_dev;           // MIX-16: T x six fp16 weight images (fit_tc.cu)
+    int device;                     // CUDA device the model was created on (dp_compute checks it)
     double *avg_dev, *std_dev;      // [T][4]
     double *ebias_dev;              // [T]
     // fitting nets (per type): V1 [1600][240], V2, V3 [240][240] row-major in x out, biases, v4, c4
@@ -66,13 +79,10 @@ struct dp_model {
     void *last_ws;
     cudaStream_t last_stream;
     int sort_cap;
-    // mixed-mode variant knobs: operand parts of the net MMAs (1 = fp16, 3 = split), of the contraction-type MMAs,
-    // tanh.approx vs tanhf, and operand parts of fitting layers 1-2
-    int mix_ns, mix_nsc, mix_tanh_approx, mix_fit_ns, mix_fit3_ns, mix_ns_bwd;
-    int mix_ns_fwd, mix_nsc_fwd;    // forward-kernel overrides of mix_ns / mix_nsc (precision study)
     int profile;
     // buffered neighbour list of the MD loop (md.cu sets these around its dp_compute calls; 0 / null otherwise)
     int list_mode;                  // 0: search the cells every call; 1: search with rc + skin and store candidates; 2: reuse them
+    int keep_flags;                 // dp_md_run, evaluations after the first: device error flags accumulate over the whole run
     double md_skin;
     int *md_cand, *md_candcnt;      // [T][N][sort_cap], [T][N] in the MD part of the workspace
     double *md_xref;                // [N][3] coordinates at the last list build (user order)
@@ -131,16 +141,11 @@ cudaError_t launch_embed_bwd_f64(const dp_model *m, long N, const Grid3 &g, char
 cudaError_t launch_fit_f64(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_finalize(const dp_model *m, long N, char *ws, const WsLayout &L, double *energy, double *eatom,
                             double *forces, double *virial, cudaStream_t st);
-cudaError_t launch_embed_fwd_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_embed_bwd_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_embed_fwd_tc(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_embed_fwd_tc2(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_embed_bwd_tc2(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
-cudaError_t fit_tc_gemm(int mode, bool apx, const dp_model *m, const Grid3 &g, const int *bin_start, const float *A, int lda,
-                        const float *bias, const float *v4, const float *aux0, const float *aux1, float *out0, float *out1,
-                        int ldo, cudaStream_t st);
-cudaError_t fit_tc_chain(bool apx, const dp_model *m, const Grid3 &g, const int *bin_start, const float *h1, const float *c2,
-                         const float *c3, const float *v4, const float *c4, float *gz1, uint8_t *gz1img, double *eatom, cudaStream_t st);
+cudaError_t launch_fit_tc(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 size_t fit_tc_type_elems();
 void fit_tc_build_type(const double *V1, const double *V2, const double *V3, struct __half *out);
 cudaError_t launch_env_rows(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);

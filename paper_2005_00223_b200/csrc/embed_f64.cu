@@ -413,11 +413,7 @@ static int embed_grid(const dp_model *m, long N) {
 }
 
 cudaError_t launch_embed_fwd_f64(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    static bool attr = false;
-    if (!attr) {
-        cudaFuncSetAttribute(k_embed_fwd_f64, cudaFuncAttributeMaxDynamicSharedMemorySize, embed_smem_bytes_fwd_f64());
-        attr = true;
-    }
+    DP_SMEM_OPTIN(k_embed_fwd_f64, embed_smem_bytes_fwd_f64());
     int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
     k_embed_fwd_f64<<<embed_grid(m, N), DP_WARPS_PER_CTA * 32, embed_smem_bytes_fwd_f64(), st>>>(
         m->T, g.ncell, m->Nm, sel4, make_env(m, g), (const EmbedNetFrag<double> *)m->embed_frag_dev, m->avg_dev,
@@ -427,11 +423,7 @@ cudaError_t launch_embed_fwd_f64(const dp_model *m, long N, const Grid3 &g, char
 }
 
 cudaError_t launch_embed_bwd_f64(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    static bool attr = false;
-    if (!attr) {
-        cudaFuncSetAttribute(k_embed_bwd_f64, cudaFuncAttributeMaxDynamicSharedMemorySize, embed_smem_bytes_bwd_f64());
-        attr = true;
-    }
+    DP_SMEM_OPTIN(k_embed_bwd_f64, embed_smem_bytes_bwd_f64());
     int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
     k_embed_bwd_f64<<<embed_grid(m, N), DP_WARPS_PER_CTA * 32, embed_smem_bytes_bwd_f64(), st>>>(
         m->T, g.ncell, m->Nm, sel4, make_env(m, g), (const EmbedNetFrag<double> *)m->embed_frag_dev, m->avg_dev,

@@ -1,9 +1,8 @@
-// S3 + S4 + S5 (forward) and S3 + S4 + S7 + S8 + S9 (backward) of SURVEY.md section 8(a), MIX-32 and MIX-16 modes
+// S3 + S4 + S7 + S8 + S9 (embedding backward, ProdForce, ProdViral) of SURVEY.md section 8(a), MIX-32 mode
 // (PAPER.md:125): coordinates, environment matrix, switching function, its derivative, force and virial
 // accumulation in fp64; the embedding net on fp16 tensor-core MMAs with fp32 accumulation (operand splitting gives
 // single-precision products in MIX-32); tanh and tanh' in fp32; first embedding layer (K = 1) on the ALUs as in
 // the paper ("do not meet the size requirements for using Tensor Cores").  See embed_mix.cuh for the layouts.
-#include <cstdlib>
 #include "embed_mix.cuh"
 
 namespace {
@@ -145,138 +144,6 @@ __device__ __forceinline__ void copy_net_to_smem(EmbedNetFragH<NSW> *dst, const 
 constexpr int MIX_ROWCHUNK = 64;
 constexpr int MIX_WARP_BUF_FLOATS = MIX_ROWCHUNK * 5;    // rbuf[64][4] + sbuf[64]
 
-template <int NSW>
-constexpr int fwd_net_words() {
-    return (32 + 32 + HNT2 * 8 + HNT3 * 8) + NSW * (2 * HNT2 * 64 + 4 * HNT3 * 64);
-}
-
-// ------------------------------------------------------------------------------------------------ forward
-template <int NS, int NSC, bool APPROX>
-__global__ void __launch_bounds__(DP_WARPS_PER_CTA * 32, 1)
-k_embed_fwd_mix(int T, int ncell, int Nm, int4 sel4, EnvParams ep, const EmbedNetFragH<ns_wparts(NS)> *__restrict__ nets,
-                const double *__restrict__ avg, const double *__restrict__ stdv, const int *__restrict__ bin_start,
-                const double *__restrict__ xs, const int *__restrict__ nlist, const int *__restrict__ nreal,
-                float *__restrict__ Aout, unsigned long long *__restrict__ row_counter) {
-    constexpr int NSW = ns_wparts(NS);
-    extern __shared__ __align__(16) uint32_t smem_u[];
-    // forward kernel keeps only the forward part of the net: the struct members are ordered so that it is a prefix
-    // when NSW == 1; for NSW == 2 the whole struct is staged (W2f/W3f hold both parts contiguously per array).
-    EmbedNetFragH<NSW> *net = reinterpret_cast<EmbedNetFragH<NSW> *>(smem_u);
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    float *rbuf = reinterpret_cast<float *>(smem_u) + sizeof(EmbedNetFragH<NSW>) / 4 + wid * MIX_WARP_BUF_FLOATS;
-    float *sbuf = rbuf + MIX_ROWCHUNK * 4;
-    const int sel[4] = {sel4.x, sel4.y, sel4.z, sel4.w};
-    const int gw = blockIdx.x * DP_WARPS_PER_CTA + wid, W = gridDim.x * DP_WARPS_PER_CTA;
-    const int r = lane & 3, g = lane >> 2;
-    const float inv_nm = 1.0f / (float)Nm;
-    const double hx = 0.5 * ep.L[0], hy = 0.5 * ep.L[1], hz = 0.5 * ep.L[2];
-    unsigned long long my_rows = 0;
-
-    for (int a = 0; a < T; ++a) {
-        const int ts0 = bin_start[a * ncell], ts1 = bin_start[(a + 1) * ncell];
-        if (ts0 == ts1) continue;
-        double av[4], sd[4];
-#pragma unroll
-        for (int c = 0; c < 4; ++c) { av[c] = avg[4 * a + c]; sd[c] = stdv[4 * a + c]; }
-        int off = 0;
-        for (int b = 0; b < T; ++b) {
-            __syncthreads();
-            copy_net_to_smem<NSW>(net, nets + (a * T + b), (int)(sizeof(EmbedNetFragH<NSW>) / 4));
-            __syncthreads();
-            for (int i = ts0 + gw; i < ts1; i += W) {
-                const int nr = nreal[i * T + b];
-                const int npad = sel[b] - nr;
-                const int rows = nr + (npad > 0 ? 1 : 0);
-                const double xi = xs[3 * (long)i], yi = xs[3 * (long)i + 1], zi = xs[3 * (long)i + 2];
-                float accA[HNT3 / 2][4];
-#pragma unroll
-                for (int t = 0; t < HNT3 / 2; ++t) accA[t][0] = accA[t][1] = accA[t][2] = accA[t][3] = 0.f;
-                for (int r0 = 0; r0 < rows; r0 += MIX_ROWCHUNK) {
-                    const int nrow_c = min(MIX_ROWCHUNK, rows - r0);
-                    const int ntile = (nrow_c + HROWS - 1) / HROWS;
-                    for (int rr = lane; rr < ntile * HROWS; rr += 32) {
-                        const int row = r0 + rr;
-                        double Rt[4] = {0.0, 0.0, 0.0, 0.0};
-                        double wgt = 0.0;
-                        if (row < nr) {
-                            const int j = nlist[(long)i * Nm + off + row];
-                            const double dx = min_image(xs[3 * (long)j] - xi, ep.L[0], hx);
-                            const double dy = min_image(xs[3 * (long)j + 1] - yi, ep.L[1], hy);
-                            const double dz = min_image(xs[3 * (long)j + 2] - zi, ep.L[2], hz);
-                            env_row(ep, dx, dy, dz, Rt, nullptr, nullptr);
-                            wgt = 1.0;
-                        } else if (row == nr && npad > 0) {
-                            wgt = (double)npad;
-                        }
-                        const double Rh0 = (Rt[0] - av[0]) / sd[0];
-                        sbuf[rr] = (float)Rh0;
-                        rbuf[rr * 4 + 0] = (float)(wgt * Rh0);
-#pragma unroll
-                        for (int c = 1; c < 4; ++c) rbuf[rr * 4 + c] = (float)(wgt * ((Rt[c] - av[c]) / sd[c]));
-                    }
-                    __syncwarp();
-                    for (int t = 0; t < ntile; ++t) {
-                        float y1c[4][4], t2c[HNT2][4], t3c[HNT3][4];
-                        forward_tile<NS, APPROX>(net, lane, sbuf[t * HROWS + g], sbuf[t * HROWS + g + 8], y1c, t2c, t3c);
-                        // B operand of the contraction: weighted R^ [k = 16 rows][n = c], rows 2r,2r+1 and 2r+8,2r+9
-                        uint32_t bh[2], bl[2];
-                        {
-                            const float *rb = rbuf + t * HROWS * 4;
-                            const float v0 = g < 4 ? rb[(2 * r) * 4 + g] : 0.f, v1 = g < 4 ? rb[(2 * r + 1) * 4 + g] : 0.f;
-                            const float v2 = g < 4 ? rb[(2 * r + 8) * 4 + g] : 0.f, v3 = g < 4 ? rb[(2 * r + 9) * 4 + g] : 0.f;
-                            if (NSC == 1) { bh[0] = pack_h2(v0, v1); bh[1] = pack_h2(v2, v3); bl[0] = bl[1] = 0; }
-                            else { split_h2(v0, v1, bh[0], bl[0]); split_h2(v2, v3, bh[1], bl[1]); }
-                        }
-                        // A^T[m][c] += G^T[m][k] R^w[k][c]; G^T fragments by 8x8 b16 transposes of the C fragments
-#pragma unroll
-                        for (int s = 0; s < HNT3 / 2; ++s) {
-                            AFrag<NSC> a_;
-                            uint32_t x00h, x01h, x10h, x11h, x00l = 0, x01l = 0, x10l = 0, x11l = 0;
-                            const int ta = 2 * s, tb = 2 * s + 1;
-                            if (NSC == 1) {
-                                x00h = pack_h2(GVAL(ta, 0), GVAL(ta, 1)); x01h = pack_h2(GVAL(ta, 2), GVAL(ta, 3));
-                                x10h = pack_h2(GVAL(tb, 0), GVAL(tb, 1)); x11h = pack_h2(GVAL(tb, 2), GVAL(tb, 3));
-                            } else {
-                                split_h2(GVAL(ta, 0), GVAL(ta, 1), x00h, x00l); split_h2(GVAL(ta, 2), GVAL(ta, 3), x01h, x01l);
-                                split_h2(GVAL(tb, 0), GVAL(tb, 1), x10h, x10l); split_h2(GVAL(tb, 2), GVAL(tb, 3), x11h, x11l);
-                            }
-                            a_.hi[0] = movmatrix_trans(x00h); a_.hi[1] = movmatrix_trans(x10h);
-                            a_.hi[2] = movmatrix_trans(x01h); a_.hi[3] = movmatrix_trans(x11h);
-                            if (NSC == 3) {
-                                a_.lo[0] = movmatrix_trans(x00l); a_.lo[1] = movmatrix_trans(x10l);
-                                a_.lo[2] = movmatrix_trans(x01l); a_.lo[3] = movmatrix_trans(x11l);
-                            }
-                            mma_k16<NSC>(accA[s], a_, bh, bl);
-                        }
-                    }
-                    my_rows += (unsigned long long)ntile * HROWS;
-                    __syncwarp();
-                }
-                // accA[s]: c0,c1 = (feature col g of tile 2s, c = 2r + {0,1}); c2,c3 = tile 2s+1.  valid for r < 2.
-                if (r < 2) {
-                    float *Ai = Aout + (long)i * 4 * M2E;
-#pragma unroll
-                    for (int s = 0; s < HNT3 / 2; ++s)
-#pragma unroll
-                        for (int h = 0; h < 2; ++h) {
-                            const int f = h_f3(2 * s + h, g >> 1, g & 1);
-                            if (f >= 0) {
-#pragma unroll
-                                for (int j = 0; j < 2; ++j) {
-                                    const float v = accA[s][2 * h + j] * inv_nm;
-                                    float *dst = Ai + (2 * r + j) * M2E + f;
-                                    *dst = (b == 0) ? v : *dst + v;
-                                }
-                            }
-                        }
-                }
-            }
-            off += sel[b];
-        }
-    }
-    if (lane == 0 && my_rows) atomicAdd(row_counter, my_rows);
-}
-
 // ------------------------------------------------------------------------------------------------ backward
 // gAf per atom (written by the mixed fitting backward, fit_mix.cu), per weight part p < NSW, 28*32 words:
 //   [p][0..14)[lane]     dG  MMA (k8) B fragment of tile nt3:  (r < 2) ? half2(gA[2r][f], gA[2r+1][f]) : 0, f = f3(nt3, g/2, g%2)
@@ -288,7 +155,7 @@ k_embed_bwd_mix(int T, int ncell, int Nm, int4 sel4, EnvParams ep, const EmbedNe
                 const double *__restrict__ avg, const double *__restrict__ stdv, const int *__restrict__ bin_start,
                 const double *__restrict__ xs, const int *__restrict__ nlist, const int *__restrict__ nreal,
                 const uint32_t *__restrict__ gAf, const float *__restrict__ gscale, double *__restrict__ fsorted,
-                double *__restrict__ virial, unsigned long long *__restrict__ row_counter, int dbg) {
+                double *__restrict__ virial, unsigned long long *__restrict__ row_counter) {
     constexpr int NSW = ns_wparts(NS);
     extern __shared__ __align__(16) uint32_t smem_u[];
     EmbedNetFragH<NSW> *net = reinterpret_cast<EmbedNetFragH<NSW> *>(smem_u);
@@ -432,10 +299,6 @@ k_embed_bwd_mix(int T, int ncell, int Nm, int4 sel4, EnvParams ep, const EmbedNe
                         ds1 += __shfl_xor_sync(0xffffffffu, ds1, 1); ds1 += __shfl_xor_sync(0xffffffffu, ds1, 2);
 #pragma unroll
                         for (int k = 0; k < 4; ++k) dR[k] *= oscale;
-                        if (dbg & 2) { dR[0] = dR[1] = dR[2] = dR[3] = 0.f; }
-                        if (dbg & 16) { if (r == 0) { dR[1] = dR[3] = 0.f; } else { dR[0] = dR[1] = dR[2] = dR[3] = 0.f; } }
-                        if (dbg & 32) { if (r == 0) { dR[0] = dR[2] = 0.f; } }
-                        if (dbg & 1) { ds0 = ds1 = 0.f; }
                         if (r == 0) { dR[0] += ds0; dR[2] += ds1; }
                         __syncwarp();
                         if (r < 2) {
@@ -512,41 +375,21 @@ int embed_grid(const dp_model *m, long N) {
     return (int)(grid > m->num_sms ? m->num_sms : grid);
 }
 
-template <int NS, int NSC, bool APPROX>
-cudaError_t launch_fwd(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(k_embed_fwd_mix<NS, NSC, APPROX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<NS>()); attr = true; }
-    int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
-    k_embed_fwd_mix<NS, NSC, APPROX><<<embed_grid(m, N), DP_WARPS_PER_CTA * 32, smem_bytes<NS>(), st>>>(
-        m->T, g.ncell, m->Nm, sel4, make_env(m, g), (const EmbedNetFragH<ns_wparts(NS)> *)m->embed_frag_dev, m->avg_dev,
-        m->std_dev, (int *)(ws + L.bin_start), (double *)(ws + L.xs), (int *)(ws + L.nlist), (int *)(ws + L.nreal),
-        (float *)(ws + L.A), (unsigned long long *)(ws + L.status + 8));
-    return cudaGetLastError();
-}
-
 template <int NS, int NSC, bool APPROX, int NSB>
 cudaError_t launch_bwd(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(k_embed_bwd_mix<NS, NSC, APPROX, NSB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<NS>()); attr = true; }
+    DP_SMEM_OPTIN((k_embed_bwd_mix<NS, NSC, APPROX, NSB>), smem_bytes<NS>());
     int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
     k_embed_bwd_mix<NS, NSC, APPROX, NSB><<<embed_grid(m, N), DP_WARPS_PER_CTA * 32, smem_bytes<NS>(), st>>>(
         m->T, g.ncell, m->Nm, sel4, make_env(m, g), (const EmbedNetFragH<ns_wparts(NS)> *)m->embed_frag_dev, m->avg_dev,
         m->std_dev, (int *)(ws + L.bin_start), (double *)(ws + L.xs), (int *)(ws + L.nlist), (int *)(ws + L.nreal),
         (const uint32_t *)(ws + L.gAf), (const float *)(ws + L.gscale), (double *)(ws + L.fsorted),
-        (double *)(ws + L.virial), (unsigned long long *)(ws + L.status + 16), getenv("DP_DEBUG_BWD") ? atoi(getenv("DP_DEBUG_BWD")) : 0);
+        (double *)(ws + L.virial), (unsigned long long *)(ws + L.status + 16));
     return cudaGetLastError();
 }
 
 }  // namespace
 
-cudaError_t launch_embed_fwd_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    if (m->prec == DP_MIX32) return launch_fwd<3, 3, false>(m, N, g, ws, L, st);
-    if (m->mix_ns_fwd == 1) return m->mix_nsc_fwd == 3 ? launch_fwd<1, 3, true>(m, N, g, ws, L, st) : launch_fwd<1, 1, true>(m, N, g, ws, L, st);
-    return m->mix_nsc_fwd == 3 ? launch_fwd<2, 3, true>(m, N, g, ws, L, st) : launch_fwd<2, 1, true>(m, N, g, ws, L, st);
-}
+// MIX-32 ("all the arithmetic operations ... in single precision"): every operand split hi + lo, exact tanhf
 cudaError_t launch_embed_bwd_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    if (m->prec == DP_MIX32) return launch_bwd<3, 3, false, 3>(m, N, g, ws, L, st);
-    if (m->mix_ns == 1) return m->mix_nsc == 3 ? launch_bwd<1, 3, true, 1>(m, N, g, ws, L, st) : launch_bwd<1, 1, true, 1>(m, N, g, ws, L, st);
-    if (m->mix_ns_bwd == 1) return m->mix_nsc == 3 ? launch_bwd<2, 3, true, 1>(m, N, g, ws, L, st) : launch_bwd<2, 1, true, 1>(m, N, g, ws, L, st);
-    return m->mix_nsc == 3 ? launch_bwd<2, 3, true, 2>(m, N, g, ws, L, st) : launch_bwd<2, 1, true, 2>(m, N, g, ws, L, st);
+    return launch_bwd<3, 3, false, 3>(m, N, g, ws, L, st);
 }

@@ -9,7 +9,8 @@
 //   E3:     tcgen05.ld D3, + bias, tanh, + (y2,y2) -> G  -> operand image (MN-major use)
 //   MMA C:  DA[128 features x 8*slots] = G^T . R^w   (K = 128 rows; per-atom slots mask the rows of other atoms)
 //   E4:     tcgen05.ld DA -> A_i (fp32, global), scaled by 1/Nm
-// G never leaves the SM.  Two CTAs per SM (MIX-16) overlap one tile's MUFU/ALU phases with the other's MMAs.
+// G never leaves the SM.  This kernel serves MIX-32 (NS = 3: hi + lo activations and weights); MIX-16 runs embed_tc2.cu.
+// k_env_rows (S3, the compact fp32 environment rows) serves both mixed modes.
 #include "embed_tc.cuh"
 
 namespace {
@@ -450,8 +451,7 @@ template <int NS, bool APPROX>
 cudaError_t launch_fwd(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
     constexpr int NSW = NS == 3 ? 2 : 1;
     const int smem = SmemLayout<NSW>::TOTAL;
-    static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(k_embed_fwd_tc<NS, APPROX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr = true; }
+    DP_SMEM_OPTIN((k_embed_fwd_tc<NS, APPROX>), smem);
     int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
     int4 off4 = make_int4(m->off[0], m->off[1], m->off[2], m->off[3]);
     launch_env_rows(m, N, g, ws, L, st);
@@ -466,7 +466,7 @@ cudaError_t launch_fwd(const dp_model *m, long N, const Grid3 &g, char *ws, cons
 
 }  // namespace
 
+// MIX-32: activations and weights as hi + lo fp16 pairs (three products per MMA step), exact tanhf
 cudaError_t launch_embed_fwd_tc(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    if (m->prec == DP_MIX32) return launch_fwd<3, false>(m, N, g, ws, L, st);
-    return launch_fwd<2, true>(m, N, g, ws, L, st);
+    return launch_fwd<3, false>(m, N, g, ws, L, st);
 }

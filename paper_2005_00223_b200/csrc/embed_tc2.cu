@@ -302,8 +302,7 @@ k_embed_fwd_tc2(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, const Em
 cudaError_t launch_env_rows(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 
 cudaError_t launch_embed_fwd_tc2(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(k_embed_fwd_tc2, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdSmem::TOTAL); attr = true; }
+    DP_SMEM_OPTIN(k_embed_fwd_tc2, FwdSmem::TOTAL);
     int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
     int4 off4 = make_int4(m->off[0], m->off[1], m->off[2], m->off[3]);
     cudaError_t e = launch_env_rows(m, N, g, ws, L, st);

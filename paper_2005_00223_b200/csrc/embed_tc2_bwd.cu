@@ -86,106 +86,8 @@ __device__ __forceinline__ void act16(const uint32_t (&z)[16], uint32_t tm_dst, 
 }
 // Per-atom operand image of the folded gradient g~[c][col] = fold(gA)[c][col] * 2^e, split in hi + lo fp16 parts:
 //   C [208][8] : per T column {hi[0..3], lo[0..3]} (16 bytes)
-// gA[c][m] = sum_a gD[m][a] A[c][a] + [m < 16] sum_m' gD[m'][m] A[c][m'], fp32.
 constexpr int GA_IMG_BYTES = T2_COLS * 16;    // 3,328 per atom
-constexpr int GA_ROW = 20;                                         // padded gD row (floats): conflict-free float4 reads
-constexpr int GA_WARP_FLOATS = M2E * GA_ROW + 2 * 4 * M2E + 4 * T2_COLS;   // gD, A [c][m], A^T [m][c], folded g~ [c][col]
-__global__ void __launch_bounds__(128) k_gA_img(long N, const float *__restrict__ Amat, const float *__restrict__ gD,
-                                                 uint8_t *__restrict__ img, float *__restrict__ gscale) {
-    extern __shared__ __align__(16) float smg[];
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const long i = blockIdx.x * 4L + wid;
-    if (i >= N) return;
-    float *sG = smg + wid * GA_WARP_FLOATS;      // [100][20]
-    float *sA = sG + M2E * GA_ROW;               // [4][100]
-    float *sAT = sA + 4 * M2E;                   // [100][4]
-    float *sF = sAT + 4 * M2E;                   // [4][208]
-    {
-        const float4 *a4 = reinterpret_cast<const float4 *>(Amat + i * 4 * M2E);
-        const float4 *g4 = reinterpret_cast<const float4 *>(gD + i * (M2E * 16));
-        for (int k = lane; k < M2E; k += 32) {
-            const float4 v = __ldg(a4 + k);
-            reinterpret_cast<float4 *>(sA)[k] = v;
-            const int c = (4 * k) / M2E, m = (4 * k) % M2E;        // 100 = 4 * 25: a float4 never straddles two c
-            sAT[(m + 0) * 4 + c] = v.x; sAT[(m + 1) * 4 + c] = v.y; sAT[(m + 2) * 4 + c] = v.z; sAT[(m + 3) * 4 + c] = v.w;
-        }
-        for (int k = lane; k < M2E * 4; k += 32) reinterpret_cast<float4 *>(sG + (k >> 2) * GA_ROW)[k & 3] = __ldg(g4 + k);
-    }
-    __syncwarp();
-    // term 2 (m < 16): lane = (a', half); sum over m' in the half
-    float t2[4] = {0.f, 0.f, 0.f, 0.f};
-    {
-        const int ap = lane & 15, m0 = (lane >> 4) * (M2E / 2);
-#pragma unroll 5
-        for (int mp = m0; mp < m0 + M2E / 2; ++mp) {
-            const float gv = sG[mp * GA_ROW + ap];
-            const float4 av = *reinterpret_cast<const float4 *>(sAT + mp * 4);
-            t2[0] = fmaf(gv, av.x, t2[0]); t2[1] = fmaf(gv, av.y, t2[1]); t2[2] = fmaf(gv, av.z, t2[2]); t2[3] = fmaf(gv, av.w, t2[3]);
-        }
-#pragma unroll
-        for (int c = 0; c < 4; ++c) t2[c] += __shfl_xor_sync(0xffffffffu, t2[c], 16);
-    }
-    // term 1: lane = m (+32, +64, +96); A[c][0..16) in registers
-    float a16[4][16];
-#pragma unroll
-    for (int c = 0; c < 4; ++c)
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const float4 v = *reinterpret_cast<const float4 *>(sA + c * M2E + 4 * q);
-            a16[c][4 * q] = v.x; a16[c][4 * q + 1] = v.y; a16[c][4 * q + 2] = v.z; a16[c][4 * q + 3] = v.w;
-        }
-    float *sO = sAT;                             // gA [c][m] overwrites A^T (all its readers are done)
-    __syncwarp();
-    for (int m = lane; m < M2E; m += 32) {
-        float g[16];
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const float4 v = *reinterpret_cast<const float4 *>(sG + m * GA_ROW + 4 * q);
-            g[4 * q] = v.x; g[4 * q + 1] = v.y; g[4 * q + 2] = v.z; g[4 * q + 3] = v.w;
-        }
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            float acc = 0.f;
-#pragma unroll
-            for (int ax = 0; ax < 16; ++ax) acc = fmaf(g[ax], a16[c][ax], acc);
-            sO[c * M2E + m] = acc;
-        }
-    }
-    __syncwarp();
-    if (lane < 16) {
-#pragma unroll
-        for (int c = 0; c < 4; ++c) sO[c * M2E + lane] += t2[c];
-    }
-    __syncwarp();
-    // fold onto the T columns
-    float mx = 0.f;
-    for (int idx = lane; idx < 4 * T2_COLS; idx += 32) {
-        const int c = idx / T2_COLS, col = idx % T2_COLS;
-        const float *o = sO + c * M2E;
-        float v = 0.f;
-        if (col < T2_O2) { if (col < M0) v = (o[col] + o[col + M0]) + (o[col + 2 * M0] + o[col + 3 * M0]); }
-        else if (col < T2_O3) { const int f = col - T2_O2; if (f < M1) v = o[f] + o[f + M1]; }
-        else { const int m = col - T2_O3; if (m < M2E) v = o[m]; }
-        sF[idx] = v;
-        mx = fmaxf(mx, fabsf(v));
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-    int ex = 0;
-    if (mx > 0.f) frexpf(mx, &ex);
-    const float sc = ldexpf(1.f, -ex);          // max |g~| in [0.5, 1)
-    if (lane == 0) gscale[i] = sc;
-    __syncwarp();
-    uint4 *C = reinterpret_cast<uint4 *>(img + i * (long)GA_IMG_BYTES);
-    for (int col = lane; col < T2_COLS; col += 32) {
-        uint32_t h01, l01, h23, l23;
-        tc::split_h2(sF[col] * sc, sF[T2_COLS + col] * sc, h01, l01);
-        tc::split_h2(sF[2 * T2_COLS + col] * sc, sF[3 * T2_COLS + col] * sc, h23, l23);
-        C[col] = make_uint4(h01, h23, l01, l23);
-    }
-}
-
-// Same image from gA itself (fp32 [N][4][100], written by the epilogue of the last fitting-backward GEMM, fit_tc.cu MODE 6).
+// Built from gA (fp32 [N][4][100], written by the epilogue of the last fitting-backward GEMM, fit_tc.cu MODE 6).
 __global__ void __launch_bounds__(256) k_gA_fold(long N, const float *__restrict__ gA, uint8_t *__restrict__ img,
                                                   float *__restrict__ gscale) {
     __shared__ __align__(16) float sO_all[8][4 * M2E];
@@ -752,22 +654,13 @@ k_prod_force_virial(long N, int T, int4 off4, int4 sel4, EnvParams ep, const int
 }  // namespace
 
 cudaError_t launch_embed_bwd_tc2(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    static bool attr = false;
-    if (!attr) {
-        cudaFuncSetAttribute(k_embed_bwd_tc2, cudaFuncAttributeMaxDynamicSharedMemorySize, BwdSmem::TOTAL);
-        cudaFuncSetAttribute(k_gA_img, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * GA_WARP_FLOATS * 4);
-        attr = true;
-    }
+    DP_SMEM_OPTIN(k_embed_bwd_tc2, BwdSmem::TOTAL);
     int4 off4 = make_int4(m->off[0], m->off[1], m->off[2], m->off[3]);
     EnvParams ep;
     ep.rc = m->rc; ep.rc_smth = m->rc_smth; ep.inv_range = 1.0 / (m->rc - m->rc_smth);
     ep.L[0] = g.L[0]; ep.L[1] = g.L[1]; ep.L[2] = g.L[2];
-    const int smem_ga = 4 * GA_WARP_FLOATS * 4;
-    if (m->use_fit_tc)      // the last fitting GEMM left gA itself in the gD buffer (fit_tc.cu MODE 6)
-        k_gA_fold<<<(unsigned)((N + 7) / 8), 256, 0, st>>>(N, (const float *)(ws + L.gD), (uint8_t *)(ws + L.gAf), (float *)(ws + L.gscale));
-    else
-        k_gA_img<<<(unsigned)((N + 3) / 4), 128, smem_ga, st>>>(N, (const float *)(ws + L.A), (const float *)(ws + L.gD),
-                                                                 (uint8_t *)(ws + L.gAf), (float *)(ws + L.gscale));
+    // the last fitting GEMM left gA itself in the gD buffer (fit_tc.cu MODE 6)
+    k_gA_fold<<<(unsigned)((N + 7) / 8), 256, 0, st>>>(N, (const float *)(ws + L.gD), (uint8_t *)(ws + L.gAf), (float *)(ws + L.gscale));
     long long *tdbg = nullptr;
 #ifdef DP_BWD_TIMING
     static long long *tbuf = nullptr;

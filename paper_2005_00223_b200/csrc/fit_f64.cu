@@ -280,9 +280,8 @@ cudaError_t launch_fit_f64(const dp_model *m, long N, const Grid3 &g, char *ws, 
     p.A = gz1; p.N = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.out0 = D; p.ldo = ND;
     k_fit_gemm<5><<<dim3(gx, ND / BN, T), 256, 0, st>>>(p);
     // gD, A -> gA fragments for the embedding backward
-    static bool attr = false;
     const int smem = 4 * (4 * M2E + M2E * 16 + 4 * M2E) * 8;
-    if (!attr) { cudaFuncSetAttribute(k_gA, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr = true; }
+    DP_SMEM_OPTIN(k_gA, smem);
     k_gA<<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, 1.0 / (double)m->Nm, Amat, D, (double *)(ws + L.gAf));
     return cudaGetLastError();
 }

@@ -1,10 +1,7 @@
-// S5 (descriptor) + S6 (fitting net forward and backward) in the mixed-precision modes.
-// GEMMs batched over the atoms of one centre type on fp16 tensor-core MMAs (m16n8k16) with fp32 accumulation;
-// NS = 1 rounds the operands to fp16, NS = 3 splits them (hi + lo) for single-precision products.
-// MIX-16: layers 1 and 2 (and their backward products) NS = 1, the third 240x240 layer NS = 3 and the output layer in
-// fp32 ("in the last layer of the fitting net, both data storage and arithmetic operations are kept in single
-// precision", reading Q16).  MIX-32: NS = 3 everywhere.  Activations are stored in fp32.
-#include <cstdlib>
+// S5 (descriptor) + S6 (fitting net forward and backward) in MIX-32 (MIX-16 runs fit_tc.cu).
+// GEMMs batched over the atoms of one centre type on fp16 tensor-core MMAs (m16n8k16) with fp32 accumulation; every
+// operand is split hi + lo (NS = 3: hi hi + hi lo + lo hi), i.e. single-precision products on the tensor pipe, exact
+// tanhf, activations stored in fp32 ("all the arithmetic operations ... performed in single precision").
 #include "embed_mix.cuh"
 
 namespace {
@@ -273,25 +270,12 @@ __global__ void __launch_bounds__(128) k_gA_f(long N, const float *__restrict__ 
     }
 }
 
-template <int MODE, int NS, bool APPROX>
-void launch_gemm_t(const FitArgsF &p, dim3 grid, cudaStream_t st) {
-    static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(k_fitm_gemm<MODE, NS, APPROX>, cudaFuncAttributeMaxDynamicSharedMemorySize, FIT_SMEM_BYTES); attr = true; }
-    k_fitm_gemm<MODE, NS, APPROX><<<grid, 256, FIT_SMEM_BYTES, st>>>(p);
-}
-// ns: 1 fp16 operands, 2 activations split, 3 activations and weights split; apx: tanh.approx in the epilogue (modes 0, 1)
+// MIX-32: every operand split hi + lo (NS = 3), exact tanhf
 template <int MODE>
-void launch_gemm(int ns, bool apx, const FitArgsF &p, dim3 grid, cudaStream_t st) {
-    constexpr bool HAS_TANH = MODE <= 1;
-    if (HAS_TANH && apx) {
-        if (ns == 1) launch_gemm_t<MODE, 1, HAS_TANH>(p, grid, st);
-        else if (ns == 2) launch_gemm_t<MODE, 2, HAS_TANH>(p, grid, st);
-        else launch_gemm_t<MODE, 3, HAS_TANH>(p, grid, st);
-    } else {
-        if (ns == 1) launch_gemm_t<MODE, 1, false>(p, grid, st);
-        else if (ns == 2) launch_gemm_t<MODE, 2, false>(p, grid, st);
-        else launch_gemm_t<MODE, 3, false>(p, grid, st);
-    }
+cudaError_t launch_gemm(const FitArgsF &p, dim3 grid, cudaStream_t st) {
+    DP_SMEM_OPTIN((k_fitm_gemm<MODE, 3, false>), FIT_SMEM_BYTES);
+    k_fitm_gemm<MODE, 3, false><<<grid, 256, FIT_SMEM_BYTES, st>>>(p);
+    return cudaGetLastError();
 }
 
 }  // namespace
@@ -299,8 +283,6 @@ void launch_gemm(int ns, bool apx, const FitArgsF &p, dim3 grid, cudaStream_t st
 cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
     const int F = 240, ND = M2E * 16;
     const int T = m->T;
-    const int ns12 = m->mix_fit_ns, ns3 = m->mix_fit3_ns;   // operand parts of layers 1-2 and of the third 240x240 layer
-    const bool apx = m->mix_tanh_approx != 0;
     float *Amat = (float *)(ws + L.A);
     float *D = (float *)(ws + L.gD);
     float *act = (float *)(ws + L.fit_act);
@@ -313,51 +295,30 @@ cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, 
     const float *v4 = (const float *)m->fitv4_dev, *c4 = (const float *)m->fitc4_dev;
     const unsigned gy = (unsigned)((N + BM - 1) / BM);
     const unsigned nb8 = (unsigned)((N + 7) / 8);
+    cudaError_t e = cudaSuccess;
+    auto ok = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
 
-    if (!m->use_fit_tc) k_descr_f<<<nb8, 256, 0, st>>>(N, Amat, D);     // the tcgen05 first-layer GEMM forms D in its operand producer
+    k_descr_f<<<nb8, 256, 0, st>>>(N, Amat, D);
     FitArgsF p{};
     p.ncell = g.ncell; p.bin_start = bin_start; p.v4 = v4; p.v4_type_stride = F; p.bias_type_stride = F;
     p.K = ND; p.N = F; p.A = D; p.lda = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.ldb = F; p.bias = c1;
     p.out0 = h1; p.ldo = F;
     const dim3 g240(F / BN, gy, T), g1600(ND / BN, gy, T);
-    if (m->use_fit_tc) {      // tcgen05 GEMMs (fit_tc.cu), same products, buffers and epilogues
-        fit_tc_gemm(0, apx, m, g, bin_start, Amat, 4 * M2E, c1, nullptr, nullptr, nullptr, h1, nullptr, F, st);
-        static const bool unfused = std::getenv("DP_FIT_UNFUSED") != nullptr;
-        // fused path with the gA epilogue: gz1 goes to the last product as ready-made hi + lo fp16 tile images (they fit in the
-        // unused activation buffers 2 S .. 4 S: 967.5 bytes per row plus one tile per type)
-        const bool gz_img = !unfused && m->use_tc_bwd;
-        if (!unfused) {      // the four 240 x 240 products and the energy in one kernel
-            fit_tc_chain(apx, m, g, bin_start, h1, c2, c3, v4, c4, gz1, gz_img ? reinterpret_cast<uint8_t *>(gz1) : nullptr,
-                         (double *)(ws + L.eatom), st);
-        } else {
-        fit_tc_gemm(1, apx, m, g, bin_start, h1, F, c2, nullptr, h1, nullptr, t2, h2, F, st);
-        fit_tc_gemm(2, false, m, g, bin_start, h2, F, c3, v4, h2, nullptr, gz3, h3, F, st);
-        k_energy_f<<<nb8, 256, 0, st>>>(N, T, g.ncell, bin_start, h3, v4, c4, m->ebias_dev, (double *)(ws + L.eatom));
-        fit_tc_gemm(3, false, m, g, bin_start, gz3, F, nullptr, v4, t2, nullptr, g2, gz2, F, st);
-        fit_tc_gemm(4, false, m, g, bin_start, gz2, F, nullptr, nullptr, g2, h1, gz1, nullptr, F, st);
-        }
-        if (m->use_tc_bwd)   // gA in the epilogue: D receives gA [N][4][100], the gD tensor is never written
-            fit_tc_gemm(6, false, m, g, bin_start, gz_img ? nullptr : gz1, F, nullptr, nullptr, Amat, gz_img ? gz1 : nullptr, D, nullptr, ND, st);
-        else
-            fit_tc_gemm(5, false, m, g, bin_start, gz1, F, nullptr, nullptr, nullptr, nullptr, D, nullptr, ND, st);
-    } else {
-    launch_gemm<0>(ns12, apx, p, g240, st);
+    ok(launch_gemm<0>(p, g240, st));
     p.K = F; p.A = h1; p.lda = F; p.B = V2; p.b_type_stride = (long)F * F; p.bias = c2; p.aux0 = h1; p.out0 = t2; p.out1 = h2;
-    launch_gemm<1>(ns12, apx, p, g240, st);
+    ok(launch_gemm<1>(p, g240, st));
     p.A = h2; p.B = V3; p.bias = c3; p.aux0 = h2; p.out0 = gz3; p.out1 = h3;
-    launch_gemm<2>(ns3, false, p, g240, st);
+    ok(launch_gemm<2>(p, g240, st));
     k_energy_f<<<nb8, 256, 0, st>>>(N, T, g.ncell, bin_start, h3, v4, c4, m->ebias_dev, (double *)(ws + L.eatom));
     p.A = gz3; p.B = V3; p.aux0 = t2; p.out0 = g2; p.out1 = gz2;
-    const int nsb = std::getenv("DP_MIX16_FIT_BWD_NS") ? std::atoi(std::getenv("DP_MIX16_FIT_BWD_NS")) : 0;   // precision study
-    launch_gemm<3>(nsb ? nsb : ns3, false, p, g240, st);
+    ok(launch_gemm<3>(p, g240, st));
     p.A = gz2; p.B = V2; p.aux0 = g2; p.aux1 = h1; p.out0 = gz1; p.out1 = nullptr;
-    launch_gemm<4>(nsb ? nsb : ns12, false, p, g240, st);
+    ok(launch_gemm<4>(p, g240, st));
     p.A = gz1; p.N = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.out0 = D; p.ldo = ND;
-    launch_gemm<5>(nsb ? nsb : ns12, false, p, g1600, st);
-    }
-    if (m->use_tc_bwd) return cudaGetLastError();     // the tcgen05 backward builds its own operand images of gA
+    ok(launch_gemm<5>(p, g1600, st));
     const int smem = 4 * (4 * M2E + M2E * 16 + 4 * M2E) * 4;
-    if (m->mix_nsc == 1) k_gA_f<1><<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, Amat, D, (uint32_t *)(ws + L.gAf), (float *)(ws + L.gscale));
-    else k_gA_f<2><<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, Amat, D, (uint32_t *)(ws + L.gAf), (float *)(ws + L.gscale));
-    return cudaGetLastError();
+    DP_SMEM_OPTIN(k_gA_f<2>, smem);
+    k_gA_f<2><<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, Amat, D, (uint32_t *)(ws + L.gAf), (float *)(ws + L.gscale));
+    ok(cudaGetLastError());
+    return e;
 }

@@ -63,9 +63,9 @@ struct FitTcArgs {
     const float *A; int lda;
     const uint8_t *Aimg;                         // MODE 6: the A operand as pre-built hi + lo fp16 tile images (k_fit_chain), or null
     const __half *Bimg; long b_type_stride;      // elements per type
-    const float *bias; const float *v4;          // [T][240]
-    const float *aux0; const float *aux1;
-    float *out0; float *out1; int ldo;
+    const float *bias;                           // [T][240]
+    const float *aux0;                           // MODE 6: A [rows][4][100]
+    float *out0; int ldo;
 };
 
 __device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
@@ -90,13 +90,8 @@ __device__ __forceinline__ bool tile_rows(const FitTcArgs &p, int tile, int &a, 
     return false;
 }
 
-// MODE (epilogue), as in the mma.sync kernels of fit_mix.cu:
-//   0: out0 = tanh(acc + bias)                                   (h1)
-//   1: t = tanh(acc + bias); out0 = t; out1 = aux0 + t           (t2, h2 = h1 + t2)
-//   2: t = tanhf(acc + bias); out0 = v4 (1 - t^2); out1 = aux0 + t   (gz3, h3 = h2 + t3)
-//   3: g = v4 + acc; out0 = g; out1 = g (1 - aux0^2)             (gh2, gz2;  aux0 = t2)
-//   4: g = aux0 + acc; out0 = g (1 - aux1^2)                     (gz1;  aux0 = gh2, aux1 = h1)
-//   5: out0 = acc                                                (gD)
+// MODE (epilogue):
+//   0: out0 = tanh(acc + bias)                                   (h1; the A operand is the descriptor, formed by the producers)
 //   6: gD is consumed in registers: out0[row][c][m] = gA[c][m] = sum_a gD[m][a] A[c][a] + [m < 16] sum_m' gD[m'][m] A[c][m']
 //      (aux0 = A [rows][4][100]); the gD tensor never reaches memory
 #ifdef DP_FIT_TIMING
@@ -105,8 +100,9 @@ __device__ long long fit_dbg[8];
 #else
 #define FT(i) do { } while (0)
 #endif
-template <int MODE, int KTOT, int NTOT, bool APPROX>
+template <int MODE, int KTOT, int NTOT>
 __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
+    static_assert(MODE == 0 || MODE == 6, "the 240 x 240 products run in k_fit_chain");
     constexpr int NEPI = nepi(MODE), NPROD = nprod(MODE);
     using C = Cfg<KTOT, NTOT>;
     extern __shared__ __align__(1024) uint8_t smem[];
@@ -313,7 +309,6 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
             tile_rows(p, tile, a, row0, rend);
             const bool ok = row0 + r < rend;
             const float *bias = p.bias ? p.bias + a * 240 : nullptr;
-            const float *v4 = p.v4 ? p.v4 + a * 240 : nullptr;
             if (MODE == 6) {
                 // thread (row, c): one of the four components.  Per 16 accumulator columns = gD[m][0..16) of one m.
                 // (four threads per row: the epilogue is bound by its load-to-use latencies, not by the FMA pipe)
@@ -379,27 +374,15 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                 }
                 continue;
             }
+            // MODE 0: h1 = tanh(acc + c1); two threads per row, each owns every other group of 16 columns
             for (int nt = 0; nt < C::NTILES; ++nt, ++accn) {
                 const int buf = accn & 1;
                 tc::mbar_wait(&acc_full[buf], (accn >> 1) & 1);
                 tc::fence_after();
                 const long o = (long)(row0 + r) * p.ldo + nt * C::BN;
                 const int half = ((warp - 2 - NPROD / 32) >> 2) & 1;
-                float4 a0c[4], a1c[4], a0n[4], a1n[4];
-                auto load_aux = [&](int c0, float4 (&a0)[4], float4 (&a1)[4]) {     // auxiliary operands of one 16-column group
-#pragma unroll
-                    for (int g4 = 0; g4 < 4; ++g4) {
-                        a0[g4] = make_float4(0.f, 0.f, 0.f, 0.f); a1[g4] = a0[g4];
-                        if (ok && c0 < C::BN) {
-                            if (MODE >= 1 && MODE <= 4) a0[g4] = __ldg(reinterpret_cast<const float4 *>(p.aux0 + o + c0 + 4 * g4));
-                            if (MODE == 4) a1[g4] = __ldg(reinterpret_cast<const float4 *>(p.aux1 + o + c0 + 4 * g4));
-                        }
-                    }
-                };
-                load_aux(16 * half, a0c, a1c);
 #pragma unroll 1
                 for (int c0 = 16 * half; c0 < C::BN; c0 += 32) {
-                    load_aux(c0 + 32, a0n, a1n);          // one group ahead
                     uint32_t v[16];
                     tc::ld16(tm_lane + buf * C::TM_BUF + c0, v);
                     tc::wait_ld();
@@ -407,48 +390,14 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
 #pragma unroll
                         for (int g4 = 0; g4 < 4; ++g4) {
                             const int c = c0 + 4 * g4;
-                            float x[4] = {__uint_as_float(v[4 * g4]), __uint_as_float(v[4 * g4 + 1]), __uint_as_float(v[4 * g4 + 2]),
-                                          __uint_as_float(v[4 * g4 + 3])};
-                            float r0[4], r1[4];
-                            if (MODE == 0) {
-                                const float4 b = *reinterpret_cast<const float4 *>(bias + c);
-                                const float bb[4] = {b.x, b.y, b.z, b.w};
+                            const float4 b = *reinterpret_cast<const float4 *>(bias + c);
+                            const float bb[4] = {b.x, b.y, b.z, b.w};
+                            float r0[4];
 #pragma unroll
-                                for (int k = 0; k < 4; ++k) r0[k] = APPROX ? tc::tanh_approx(x[k] + bb[k]) : tanhf(x[k] + bb[k]);
-                            } else if (MODE == 1 || MODE == 2) {
-                                const float4 b = *reinterpret_cast<const float4 *>(bias + c);
-                                const float4 hh = a0c[g4];
-                                const float bb[4] = {b.x, b.y, b.z, b.w}, hv[4] = {hh.x, hh.y, hh.z, hh.w};
-                                float vv[4] = {0.f, 0.f, 0.f, 0.f};
-                                if (MODE == 2) { const float4 w = *reinterpret_cast<const float4 *>(v4 + c); vv[0] = w.x; vv[1] = w.y; vv[2] = w.z; vv[3] = w.w; }
-#pragma unroll
-                                for (int k = 0; k < 4; ++k) {
-                                    const float t = (MODE == 1 && APPROX) ? tc::tanh_approx(x[k] + bb[k]) : tanhf(x[k] + bb[k]);
-                                    r0[k] = MODE == 1 ? t : vv[k] * (1.f - t * t);
-                                    r1[k] = hv[k] + t;
-                                }
-                            } else if (MODE == 3) {
-                                const float4 w = *reinterpret_cast<const float4 *>(v4 + c);
-                                const float4 tt = a0c[g4];
-                                const float vv[4] = {w.x, w.y, w.z, w.w}, tv[4] = {tt.x, tt.y, tt.z, tt.w};
-#pragma unroll
-                                for (int k = 0; k < 4; ++k) { r0[k] = vv[k] + x[k]; r1[k] = r0[k] * (1.f - tv[k] * tv[k]); }
-                            } else if (MODE == 4) {
-                                const float4 gg = a0c[g4];
-                                const float4 hh = a1c[g4];
-                                const float gv[4] = {gg.x, gg.y, gg.z, gg.w}, hv[4] = {hh.x, hh.y, hh.z, hh.w};
-#pragma unroll
-                                for (int k = 0; k < 4; ++k) r0[k] = (gv[k] + x[k]) * (1.f - hv[k] * hv[k]);
-                            } else {
-#pragma unroll
-                                for (int k = 0; k < 4; ++k) r0[k] = x[k];
-                            }
+                            for (int k = 0; k < 4; ++k) r0[k] = tc::tanh_approx(__uint_as_float(v[4 * g4 + k]) + bb[k]);
                             *reinterpret_cast<float4 *>(p.out0 + o + c) = make_float4(r0[0], r0[1], r0[2], r0[3]);
-                            if (MODE >= 1 && MODE <= 3) *reinterpret_cast<float4 *>(p.out1 + o + c) = make_float4(r1[0], r1[1], r1[2], r1[3]);
                         }
                     }
-#pragma unroll
-                    for (int g4 = 0; g4 < 4; ++g4) { a0c[g4] = a0n[g4]; a1c[g4] = a1n[g4]; }
                 }
                 tc::fence_before();
                 __syncwarp();
@@ -478,7 +427,6 @@ struct FitChainArgs {
     const __half *Bimg; long b_type_stride;
     const float *c2, *c3, *v4, *c4;       // [T][240], c4 [T]
     const double *ebias;                  // [T]
-    float *gz1;                           // [rows][240] (fp32), or
     uint8_t *gz1img;                      // per 128-row tile the hi + lo fp16 operand image of the last product (GZ_TILE_BYTES)
     double *eatom;                        // [rows]
 };
@@ -491,7 +439,6 @@ constexpr int CH_TOTAL = CH_OFF_RED + 2 * 128 * 4;
 constexpr int CH_TM_ACC = 0, CH_TM_D2 = 256;                 // TMEM: accumulator [0,240), 1 - t2^2 (fp32) [256,496)
 static_assert(CH_TOTAL <= 227 * 1024, "shared memory budget");
 
-template <bool APPROX>
 __global__ void __launch_bounds__(CH_THREADS, 1) k_fit_chain(FitChainArgs p) {
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ uint32_t tmem_base_s;
@@ -631,7 +578,7 @@ __global__ void __launch_bounds__(CH_THREADS, 1) k_fit_chain(FitChainArgs p) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) {
                     const float z = __uint_as_float(v[q]) + __ldg(c2 + 8 * j + q);
-                    const float t = APPROX ? tc::tanh_approx(z) : tanhf(z);
+                    const float t = tc::tanh_approx(z);
                     d[q] = __float_as_uint(fmaf(-t, t, 1.f));
                     H[8 * j + q] += t;
                     x[q] = H[8 * j + q];
@@ -690,7 +637,6 @@ __global__ void __launch_bounds__(CH_THREADS, 1) k_fit_chain(FitChainArgs p) {
             }
             // ---- S4: gh1 = acc (= gh2 + gz2 V2^T); gz1 = gh1 (1 - h1^2) -> global ----
             wait_acc();
-            float *gzrow = p.gz1 + (long)(row0 + r) * 240 + 120 * hc;
             uint8_t *gzimg = p.gz1img + (size_t)tile * GZ_TILE_BYTES + r * 16;
 #pragma unroll
             for (int j = 0; j < 15; ++j) {
@@ -700,18 +646,13 @@ __global__ void __launch_bounds__(CH_THREADS, 1) k_fit_chain(FitChainArgs p) {
                 float x[8];
 #pragma unroll
                 for (int q = 0; q < 8; ++q) x[q] = ok ? __uint_as_float(v[q]) * fmaf(-H[8 * j + q], H[8 * j + q], 1.f) : 0.f;
-                if (p.gz1img) {
-                    const int g = 15 * hc + j, kc = g / SUB, sub = g % SUB;
-                    uint4 hi, lo;
-                    tc::split_h2(x[0], x[1], hi.x, lo.x); tc::split_h2(x[2], x[3], hi.y, lo.y);
-                    tc::split_h2(x[4], x[5], hi.z, lo.z); tc::split_h2(x[6], x[7], hi.w, lo.w);
-                    uint8_t *dst = gzimg + kc * 2 * A_PART + sub * A_SUB_STRIDE;
-                    *reinterpret_cast<uint4 *>(dst) = hi;
-                    *reinterpret_cast<uint4 *>(dst + A_PART) = lo;
-                } else if (ok) {
-                    *reinterpret_cast<float4 *>(gzrow + 8 * j) = make_float4(x[0], x[1], x[2], x[3]);
-                    *reinterpret_cast<float4 *>(gzrow + 8 * j + 4) = make_float4(x[4], x[5], x[6], x[7]);
-                }
+                const int g = 15 * hc + j, kc = g / SUB, sub = g % SUB;
+                uint4 hi, lo;
+                tc::split_h2(x[0], x[1], hi.x, lo.x); tc::split_h2(x[2], x[3], hi.y, lo.y);
+                tc::split_h2(x[4], x[5], hi.z, lo.z); tc::split_h2(x[6], x[7], hi.w, lo.w);
+                uint8_t *dst = gzimg + kc * 2 * A_PART + sub * A_SUB_STRIDE;
+                *reinterpret_cast<uint4 *>(dst) = hi;
+                *reinterpret_cast<uint4 *>(dst + A_PART) = lo;
             }
             tc::fence_before();      // the accumulator reads above precede the next tile's products (ordered by its first publish)
         }
@@ -721,12 +662,11 @@ __global__ void __launch_bounds__(CH_THREADS, 1) k_fit_chain(FitChainArgs p) {
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(512));
 }
 
-template <int MODE, int KTOT, int NTOT, bool APPROX>
-void launch(const FitTcArgs &p, int grid, cudaStream_t st) {
+template <int MODE, int KTOT, int NTOT>
+cudaError_t launch(const FitTcArgs &p, int grid, cudaStream_t st) {
     using C = Cfg<KTOT, NTOT>;
-    static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(k_fit_tc<MODE, KTOT, NTOT, APPROX>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::TOTAL); attr = true; }
-    k_fit_tc<MODE, KTOT, NTOT, APPROX><<<grid, nthreads(MODE), C::TOTAL, st>>>(p);
+    DP_SMEM_OPTIN((k_fit_tc<MODE, KTOT, NTOT>), C::TOTAL);
+    k_fit_tc<MODE, KTOT, NTOT><<<grid, nthreads(MODE), C::TOTAL, st>>>(p);
 #ifdef DP_FIT_TIMING
     {
         cudaStreamSynchronize(st);
@@ -738,6 +678,7 @@ void launch(const FitTcArgs &p, int grid, cudaStream_t st) {
                 100.0 * h[0] / tot, 100.0 * h[1] / tot, 100.0 * h[2] / tot, 100.0 * h[3] / tot, 100.0 * h[4] / tot, 100.0 * h[5] / tot, 100.0 * h[6] / tot);
     }
 #endif
+    return cudaGetLastError();
 }
 
 }  // namespace
@@ -772,41 +713,36 @@ void fit_tc_build_type(const double *V1, const double *V2, const double *V3, __h
     fit_tc_build_image(V1, 240, true, 240, 1600, out + FIT_TC_OFF[5]);
 }
 
-cudaError_t fit_tc_gemm(int mode, bool apx, const dp_model *m, const Grid3 &g, const int *bin_start, const float *A, int lda,
-                        const float *bias, const float *v4, const float *aux0, const float *aux1, float *out0, float *out1,
-                        int ldo, cudaStream_t st) {
-    FitTcArgs p{};
-    p.T = m->T; p.ncell = g.ncell; p.bin_start = bin_start; p.A = A; p.lda = lda;
-    p.Bimg = (const __half *)m->fit_tc_img_dev + FIT_TC_OFF[mode > 5 ? 5 : mode]; p.b_type_stride = (long)FIT_TC_OFF[6];
-    p.bias = bias; p.v4 = v4; p.aux0 = aux0; p.aux1 = aux1; p.out0 = out0; p.out1 = out1; p.ldo = ldo;
-    if (mode == 6 && A == nullptr) { p.Aimg = reinterpret_cast<const uint8_t *>(aux1); p.aux1 = nullptr; }   // operand image from k_fit_chain
+// S5 + S6 in MIX-16: first layer (descriptor formed in the operand producer), the fused 240 x 240 chain with the energy,
+// and the last backward product with gA in its epilogue (the gD buffer receives gA [N][4][100]; gD is never written).
+// gz1 travels from the chain to the last product as ready-made hi + lo fp16 tile images in the activation buffers 2 S .. 4 S.
+cudaError_t launch_fit_tc(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    const int F = 240, ND = M2E * 16;
+    float *Amat = (float *)(ws + L.A);
+    float *act = (float *)(ws + L.fit_act);
+    float *h1 = act;
+    uint8_t *gzimg = reinterpret_cast<uint8_t *>(act + 2 * (size_t)N * F);
+    const int *bin_start = (const int *)(ws + L.bin_start);
     const int grid = m->num_sms;
-    switch (mode) {
-        case 0: if (apx) launch<0, 1600, 240, true>(p, grid, st); else launch<0, 1600, 240, false>(p, grid, st); break;
-        case 1: if (apx) launch<1, 240, 240, true>(p, grid, st); else launch<1, 240, 240, false>(p, grid, st); break;
-        case 2: launch<2, 240, 240, false>(p, grid, st); break;
-        case 3: launch<3, 240, 240, false>(p, grid, st); break;
-        case 4: launch<4, 240, 240, false>(p, grid, st); break;
-        case 5: launch<5, 240, 1600, false>(p, grid, st); break;
-        default: launch<6, 240, 1600, false>(p, grid, st); break;
-    }
-    return cudaGetLastError();
-}
-
-// layers 2-3 forward, energy, and their backward in one kernel (k_fit_chain)
-cudaError_t fit_tc_chain(bool apx, const dp_model *m, const Grid3 &g, const int *bin_start, const float *h1, const float *c2,
-                         const float *c3, const float *v4, const float *c4, float *gz1, uint8_t *gz1img, double *eatom, cudaStream_t st) {
-    FitChainArgs p{};
-    p.T = m->T; p.ncell = g.ncell; p.bin_start = bin_start; p.h1 = h1;
-    p.Bimg = (const __half *)m->fit_tc_img_dev; p.b_type_stride = (long)FIT_TC_OFF[6];
-    p.c2 = c2; p.c3 = c3; p.v4 = v4; p.c4 = c4; p.ebias = m->ebias_dev; p.gz1 = gz1; p.gz1img = gz1img; p.eatom = eatom;
-    static bool attr = false;
-    if (!attr) {
-        cudaFuncSetAttribute(k_fit_chain<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, CH_TOTAL);
-        cudaFuncSetAttribute(k_fit_chain<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, CH_TOTAL);
-        attr = true;
-    }
-    if (apx) k_fit_chain<true><<<m->num_sms, CH_THREADS, CH_TOTAL, st>>>(p);
-    else k_fit_chain<false><<<m->num_sms, CH_THREADS, CH_TOTAL, st>>>(p);
-    return cudaGetLastError();
+    cudaError_t e = cudaSuccess;
+    auto ok = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
+    FitTcArgs p{};
+    p.T = m->T; p.ncell = g.ncell; p.bin_start = bin_start; p.b_type_stride = (long)FIT_TC_OFF[6];
+    p.A = Amat; p.lda = 4 * M2E; p.Bimg = (const __half *)m->fit_tc_img_dev + FIT_TC_OFF[0];
+    p.bias = (const float *)m->fitc1_dev; p.out0 = h1; p.ldo = F;
+    ok(launch<0, 1600, 240>(p, grid, st));
+    FitChainArgs c{};
+    c.T = m->T; c.ncell = g.ncell; c.bin_start = bin_start; c.h1 = h1;
+    c.Bimg = (const __half *)m->fit_tc_img_dev; c.b_type_stride = (long)FIT_TC_OFF[6];
+    c.c2 = (const float *)m->fitc2_dev; c.c3 = (const float *)m->fitc3_dev; c.v4 = (const float *)m->fitv4_dev;
+    c.c4 = (const float *)m->fitc4_dev; c.ebias = m->ebias_dev; c.gz1img = gzimg; c.eatom = (double *)(ws + L.eatom);
+    DP_SMEM_OPTIN(k_fit_chain, CH_TOTAL);
+    k_fit_chain<<<grid, CH_THREADS, CH_TOTAL, st>>>(c);
+    ok(cudaGetLastError());
+    FitTcArgs q{};
+    q.T = m->T; q.ncell = g.ncell; q.bin_start = bin_start; q.b_type_stride = (long)FIT_TC_OFF[6];
+    q.Aimg = gzimg; q.lda = F; q.Bimg = (const __half *)m->fit_tc_img_dev + FIT_TC_OFF[5];
+    q.aux0 = Amat; q.out0 = (float *)(ws + L.gD); q.ldo = ND;
+    ok(launch<6, 240, 1600>(q, grid, st));
+    return e;
 }

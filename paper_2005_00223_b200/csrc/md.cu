@@ -3,6 +3,7 @@
 // Everything is enqueued on the caller's stream: no host synchronisation, no allocation; the neighbour list is rebuilt by
 // every evaluation, or (skin > 0, rebuild_every > 1) kept as a buffered candidate list for rebuild_every evaluations as in the
 // paper (2 A buffer, update every 50 steps); then a step only re-tests, re-sorts and truncates (nlist.cu).
+#include <cmath>
 #include "dp_internal.h"
 
 namespace {
@@ -48,15 +49,25 @@ __global__ void __launch_bounds__(256) k_md(long N, double *__restrict__ x, doub
     }
 }
 
+// temperature (K) and pressure (bar) of one evaluation from its kinetic energy and virial ("kinetic energy,
+// potential energy, temperature, pressure, are collected"): T = 2 KE / ((3 N - 3) kB) (three momentum constraints, as
+// LAMMPS counts them), P = (2 KE + tr Xi) / (3 V) with Xi = -dE/d(strain); 1 eV/A^3 = 1.602176634e6 bar.
+__global__ void k_thermo(double *__restrict__ rec, const double *__restrict__ virial, double dof, double volume) {
+    const double ke = rec[1];
+    rec[2] = 2.0 * ke / (dof * 8.617333262e-5);
+    rec[3] = (2.0 * ke + virial[0] + virial[4] + virial[8]) / (3.0 * volume) * 1.602176634e6;
+}
+
 }  // namespace
 
 namespace {
-struct MdWs { size_t base, cand, candcnt, xref, total; };
+struct MdWs { size_t base, vir, cand, candcnt, xref, total; };
 MdWs md_layout(const dp_model *m, long N, double skin) {
     MdWs w{};
     auto al = [](size_t x) { return (x + 255) & ~(size_t)255; };
     w.base = al(dp_workspace_bytes(m, N));
-    w.total = w.base;
+    w.vir = w.base;
+    w.total = al(w.vir + 16 * sizeof(double));
     if (skin > 0.0) {
         w.cand = w.total; w.total = al(w.total + sizeof(int) * (size_t)m->T * (size_t)N * (size_t)m->sort_cap);
         w.candcnt = w.total; w.total = al(w.total + sizeof(int) * (size_t)m->T * (size_t)N);
@@ -91,7 +102,12 @@ extern "C" int dp_md_run(dp_model *m, long natoms, double *coords_dev, double *v
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const unsigned grid = (unsigned)((natoms + 255) / 256 < 148L * 8 ? (natoms + 255) / 256 : 148L * 8);
     const double hk = 0.5 * dt_fs * ACC;
-    if (cudaMemsetAsync(thermo_dev, 0, sizeof(double) * 2 * ((size_t)nsteps + 1), st) != cudaSuccess) return DP_ECUDA;
+    if (cudaMemsetAsync(thermo_dev, 0, sizeof(double) * DP_MD_NTHERMO * ((size_t)nsteps + 1), st) != cudaSuccess) return DP_ECUDA;
+    const double *bx = box_host;
+    const double volume = std::fabs(bx[0] * (bx[4] * bx[8] - bx[5] * bx[7]) - bx[1] * (bx[3] * bx[8] - bx[5] * bx[6]) +
+                                    bx[2] * (bx[3] * bx[7] - bx[4] * bx[6]));
+    const double dof = natoms > 1 ? 3.0 * (double)natoms - 3.0 : 3.0;
+    double *vir = virial_dev ? virial_dev : (double *)(ws + W.vir);
     if (buffered) {
         m->md_skin = skin;
         m->md_cand = (int *)(ws + W.cand); m->md_candcnt = (int *)(ws + W.candcnt); m->md_xref = (double *)(ws + W.xref);
@@ -106,13 +122,17 @@ extern "C" int dp_md_run(dp_model *m, long natoms, double *coords_dev, double *v
                 cudaMemcpyAsync(m->md_xref, coords_dev, sizeof(double) * 3 * (size_t)natoms, cudaMemcpyDeviceToDevice, st) != cudaSuccess)
                 rc = DP_ECUDA;
         }
+        m->keep_flags = s > 0;          // device error flags accumulate over the run (dp_status reports all of it)
         if (rc == DP_OK)
-            rc = dp_compute(m, natoms, coords_dev, types_dev, box_host, workspace_dev, W.base, cuda_stream, thermo_dev + 2 * s,
-                            nullptr, forces_dev, s == nsteps ? virial_dev : nullptr);
-        if (rc == DP_OK)
+            rc = dp_compute(m, natoms, coords_dev, types_dev, box_host, workspace_dev, W.base, cuda_stream,
+                            thermo_dev + DP_MD_NTHERMO * s, nullptr, forces_dev, vir);
+        if (rc == DP_OK) {
             k_md<false, true><<<grid, 256, 0, st>>>(natoms, coords_dev, vel_dev, forces_dev, types_dev, ms, s > 0 ? hk : 0.0,
-                                                     dt_fs, thermo_dev + 2 * s + 1);
+                                                     dt_fs, thermo_dev + DP_MD_NTHERMO * s + 1);
+            k_thermo<<<1, 1, 0, st>>>(thermo_dev + DP_MD_NTHERMO * s, vir, dof, volume);
+        }
     }
+    m->keep_flags = 0;
     m->list_mode = 0; m->md_skin = 0.0; m->md_cand = nullptr; m->md_candcnt = nullptr; m->md_xref = nullptr;
     if (rc != DP_OK) return rc;
     return cudaGetLastError() == cudaSuccess ? DP_OK : DP_ECUDA;

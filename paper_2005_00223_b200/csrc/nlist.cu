@@ -3,7 +3,6 @@
 // 64-bit key per element (binary restatement, reading Q11).  Bit-exact against the
 // oracle: the arithmetic that decides list membership and order uses explicit round-to-nearest intrinsics so
 // that nvcc cannot contract it differently from the reading N2 of DESIGN.md.
-#include <cstdlib>
 #include "dp_internal.h"
 
 namespace {
@@ -183,93 +182,7 @@ __device__ __forceinline__ double min_image(double t, double L, double halfL) {
     return __dadd_rn(t, __dmul_rn(s, L));
 }
 
-// One warp per (sorted) atom.  keys live in shared memory, cap entries per warp.
-__global__ void __launch_bounds__(128)
-k_nlist(long N, int T, Grid3 g, double rc2, int cap, const int *__restrict__ bin_start,
-        const double *__restrict__ xs, const int *__restrict__ perm, const int *__restrict__ inv,
-        int Nm, int4 sel4, int *__restrict__ nlist, int *__restrict__ nreal, int *__restrict__ rowcnt,
-        int *__restrict__ status) {
-    extern __shared__ unsigned long long keys_all[];
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const long i = blockIdx.x * 4L + wid;
-    if (i >= N) return;
-    unsigned long long *keys = keys_all + (size_t)wid * cap;
-    const int sel[4] = {sel4.x, sel4.y, sel4.z, sel4.w};
-    const double xi = xs[3 * i], yi = xs[3 * i + 1], zi = xs[3 * i + 2];
-    const int cx = cell_of(xi, g.inv_cw[0], g.nc[0]), cy = cell_of(yi, g.inv_cw[1], g.nc[1]),
-              cz = cell_of(zi, g.inv_cw[2], g.nc[2]);
-    const int R_ = g.reach;       // reach 2 is only chosen for grids with >= 5 cells per axis
-    const int lo0 = R_ == 2 ? -2 : (g.nc[0] >= 3 ? -1 : 0), hi0 = R_ == 2 ? 2 : (g.nc[0] >= 2 ? 1 : 0);
-    const int lo1 = R_ == 2 ? -2 : (g.nc[1] >= 3 ? -1 : 0), hi1 = R_ == 2 ? 2 : (g.nc[1] >= 2 ? 1 : 0);
-    const int lo2 = R_ == 2 ? -2 : (g.nc[2] >= 3 ? -1 : 0), hi2 = R_ == 2 ? 2 : (g.nc[2] >= 2 ? 1 : 0);
-    const double hx = 0.5 * g.L[0], hy = 0.5 * g.L[1], hz = 0.5 * g.L[2];
-    bool truncated = false;
-    int off = 0;
-    for (int b = 0; b < T; ++b) {
-        int n = 0;
-        for (int ox = lo0; ox <= hi0; ++ox) {
-            int ax = cx + ox; ax += ax < 0 ? g.nc[0] : 0; ax -= ax >= g.nc[0] ? g.nc[0] : 0;
-            for (int oy = lo1; oy <= hi1; ++oy) {
-                int ay = cy + oy; ay += ay < 0 ? g.nc[1] : 0; ay -= ay >= g.nc[1] ? g.nc[1] : 0;
-                for (int oz = lo2; oz <= hi2; ++oz) {
-                    int az = cz + oz; az += az < 0 ? g.nc[2] : 0; az -= az >= g.nc[2] ? g.nc[2] : 0;
-                    const int bin = b * g.ncell + (ax * g.nc[1] + ay) * g.nc[2] + az;
-                    const int s0 = bin_start[bin], s1 = bin_start[bin + 1];
-                    for (int base = s0; base < s1; base += 32) {
-                        const int s = base + lane;
-                        bool ok = false;
-                        unsigned long long key = 0;
-                        if (s < s1 && s != i) {
-                            double dx = min_image(__dsub_rn(xs[3 * (long)s], xi), g.L[0], hx);
-                            double dy = min_image(__dsub_rn(xs[3 * (long)s + 1], yi), g.L[1], hy);
-                            double dz = min_image(__dsub_rn(xs[3 * (long)s + 2], zi), g.L[2], hz);
-                            double r2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
-                            if (r2 < rc2) {
-                                ok = true;
-                                key = (__double2ull_rd(r2 * 536870912.0) << 24) | (unsigned long long)perm[s];
-                            }
-                        }
-                        const unsigned mask = __ballot_sync(0xffffffffu, ok);
-                        const int pos = n + __popc(mask & ((1u << lane) - 1u));
-                        if (ok && pos < cap) keys[pos] = key;
-                        n += __popc(mask);
-                    }
-                }
-            }
-        }
-        if (n > cap) { if (lane == 0) atomicOr(&status[0], 2); n = cap; }
-        int P = 32;
-        while (P < n) P <<= 1;
-        for (int k = n + lane; k < P; k += 32) keys[k] = ~0ull;
-        __syncwarp();
-        for (int k = 2; k <= P; k <<= 1) {
-            for (int j = k >> 1; j > 0; j >>= 1) {
-                for (int idx = lane; idx < P; idx += 32) {
-                    const int ixj = idx ^ j;
-                    if (ixj > idx) {
-                        const unsigned long long a = keys[idx], c = keys[ixj];
-                        const bool asc = (idx & k) == 0;
-                        if ((a > c) == asc) { keys[idx] = c; keys[ixj] = a; }
-                    }
-                }
-                __syncwarp();
-            }
-        }
-        const int nkeep = n < sel[b] ? n : sel[b];
-        for (int k = lane; k < sel[b]; k += 32)
-            nlist[i * Nm + off + k] = k < nkeep ? inv[(int)(keys[k] & 0xFFFFFFull)] : -1;
-        if (lane == 0) {
-            nreal[i * T + b] = nkeep;
-            if (rowcnt) rowcnt[(long)b * N + i] = nkeep + (nkeep < sel[b] ? 1 : 0);   // real rows + one padded-row representative
-        }
-        truncated |= n > sel[b];
-        off += sel[b];
-        __syncwarp();
-    }
-    if (truncated && lane == 0) atomicAdd(&status[1], 1);
-}
-
-// ---- second-generation list kernel ----------------------------------------------------------------------------------
+// ---- list kernel ------------------------------------------------------------------------------------------------------
 // Bitonic sort of 32 R keys held R per lane (element index = lane * R + r), every merge ascending: the first stage of a
 // merge of width k pairs idx with idx ^ (k - 1), the following ones idx with idx ^ j.  Strides below R are register
 // exchanges, larger ones warp shuffles; the smaller key always goes to the smaller index (one 64-bit compare per element).
@@ -657,11 +570,6 @@ cudaError_t launch_build_cells(const dp_model *m, long N, const double *coords, 
 cudaError_t launch_nlist(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
     const int cap = m->sort_cap;
     const size_t smem = (size_t)4 * cap * (sizeof(unsigned long long) + sizeof(int));   // keys + sorted-space indices
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(k_nlist, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 4096 * 12);
-        attr_set = true;
-    }
     int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
     // fp32 pre-filter margin: the fp32 copy is off by <= ulp(L)/2 per coordinate, the fp32 arithmetic by a few ulp of rc^2
     double Lmax = g.L[0] > g.L[1] ? g.L[0] : g.L[1];
@@ -672,27 +580,15 @@ cudaError_t launch_nlist(const dp_model *m, long N, const Grid3 &g, char *ws, co
     const double rl = m->rc + (m->list_mode ? m->md_skin : 0.0);      // search radius of pass 1
     gf.rc2_margin = (float)(rl * rl * (1.0 + 1e-5) + 12.0 * rl * Lmax * 1.2e-7 + 1e-6);
     gf.rc2_margin_rc = (float)(m->rc * m->rc * (1.0 + 1e-5) + 12.0 * m->rc * Lmax * 1.2e-7 + 1e-6);
-    static const bool legacy = std::getenv("DP_NLIST_V1") != nullptr;
-    if (!legacy) {
-        static bool attr2 = false;
-        if (!attr2) {
-            cudaFuncSetAttribute(k_nlist2<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 4096 * 12);
-            cudaFuncSetAttribute(k_nlist2<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 4096 * 12);
-            cudaFuncSetAttribute(k_nlist2<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 4096 * 12);
-            attr2 = true;
-        }
-        auto kern = m->list_mode == 1 ? k_nlist2<1> : (m->list_mode == 2 ? k_nlist2<2> : k_nlist2<0>);
-        kern<<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, m->T, g, m->rc * m->rc, gf, cap, (int *)(ws + L.bin_start),
-                                                        (double *)(ws + L.xs), (const float4 *)(ws + L.xsf), (int *)(ws + L.perm),
-                                                        (int *)(ws + L.inv), m->Nm, sel4, (int *)(ws + L.nlist),
-                                                        (int *)(ws + L.nreal), m->prec == DP_FP64 ? nullptr : (int *)(ws + L.rowcnt),
-                                                        (int *)(ws + L.status), m->md_cand, m->md_candcnt);
-    } else
-    k_nlist<<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, m->T, g, m->rc * m->rc, cap, (int *)(ws + L.bin_start),
-                                                       (double *)(ws + L.xs), (int *)(ws + L.perm),
-                                                       (int *)(ws + L.inv), m->Nm, sel4, (int *)(ws + L.nlist),
-                                                       (int *)(ws + L.nreal), m->prec == DP_FP64 ? nullptr : (int *)(ws + L.rowcnt),
-                                                       (int *)(ws + L.status));
+    DP_SMEM_OPTIN(k_nlist2<0>, 4 * 4096 * 12);
+    DP_SMEM_OPTIN(k_nlist2<1>, 4 * 4096 * 12);
+    DP_SMEM_OPTIN(k_nlist2<2>, 4 * 4096 * 12);
+    auto kern = m->list_mode == 1 ? k_nlist2<1> : (m->list_mode == 2 ? k_nlist2<2> : k_nlist2<0>);
+    kern<<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, m->T, g, m->rc * m->rc, gf, cap, (int *)(ws + L.bin_start),
+                                                    (double *)(ws + L.xs), (const float4 *)(ws + L.xsf), (int *)(ws + L.perm),
+                                                    (int *)(ws + L.inv), m->Nm, sel4, (int *)(ws + L.nlist),
+                                                    (int *)(ws + L.nreal), m->prec == DP_FP64 ? nullptr : (int *)(ws + L.rowcnt),
+                                                    (int *)(ws + L.status), m->md_cand, m->md_candcnt);
     if (m->prec != DP_FP64)
         for (int b = 0; b < m->T; ++b)
             launch_scan((int)N, (int *)(ws + L.rowcnt) + (long)b * N, (int *)(ws + L.rowstart) + (long)b * (N + 1), (int *)(ws + L.scan_tmp), st);

@@ -12,12 +12,12 @@ from paper_2005_00223_b200 import synth
 pytestmark = pytest.mark.gpu
 
 
-def _gpu_eval(s, precision=None):
+def _gpu_eval(s, precision=None, type_map=None, user_types=None):
     import torch
     from paper_2005_00223_b200 import binding
-    m = binding.DPModel(s.model, precision or s.precision)
+    m = binding.DPModel(s.model, precision or s.precision, type_map=type_map)
     c = torch.from_numpy(s.coords).cuda()
-    t = torch.from_numpy(s.types).cuda()
+    t = torch.from_numpy(s.types if user_types is None else user_types).cuda()
     out = m.compute(c, t, s.box)
     rc, ntr = m.status()
     assert rc == 0, rc
@@ -51,7 +51,7 @@ def test_config_fp64_full_parity(idx):
     _check_fp64(g, o)
 
 
-def test_coordinates_outside_box_and_type_map():
+def test_coordinates_outside_box():
     s = synth.config(1)
     rng = np.random.default_rng(2)
     shift = rng.integers(-3, 4, size=(s.natoms, 3)) * 24.83
@@ -59,6 +59,67 @@ def test_coordinates_outside_box_and_type_map():
     o = oracle.evaluate(s.coords, s.types, s.box, s.model)
     g = _gpu_eval(s2)
     _check_fp64(g, o, tolE=2e-12, tolF=1e-9)     # coordinates differ by the rounding of the shift
+
+
+def test_non_identity_type_map_and_unmapped_type():
+    """user types 5 (-> model type 0, O) and 2 (-> model type 1, H) through a type_map with -1 holes; a user type that maps
+    to -1 (or lies outside the map) is reported by dp_status as DP_ETYPE (-4)."""
+    import torch
+    from paper_2005_00223_b200 import binding
+    s = synth.config(1)
+    tmap = np.array([-1, -1, 1, -1, -1, 0], dtype=np.int32)
+    ut = np.where(s.types == 0, 5, 2).astype(np.int32)
+    o = oracle.evaluate(s.coords, s.types, s.box, s.model)
+    g = _gpu_eval(s, type_map=tmap, user_types=ut)
+    _check_fp64(g, o)
+    for bad in (3, 6, -1):
+        ut2 = ut.copy()
+        ut2[17] = bad
+        m = binding.DPModel(s.model, "fp64", type_map=tmap)
+        m.compute(torch.from_numpy(s.coords).cuda(), torch.from_numpy(ut2).cuda(), s.box)
+        rc, _ = m.status()
+        m.close()
+        assert rc == -4, (bad, rc)
+
+
+def test_error_codes_through_the_c_abi():
+    """DP_EBOX (degenerate box), DP_ENOMEM (workspace one block short), DP_EINVAL (misaligned workspace, natoms <= 0),
+    DP_ENEIGH (more candidates inside rc than the sort buffer holds; device-detected, dp_status)."""
+    import ctypes as C
+    import torch
+    from paper_2005_00223_b200 import binding
+    s = synth.config(0)
+    m = binding.DPModel(s.model, "fp64")
+    c, t = torch.from_numpy(s.coords).cuda(), torch.from_numpy(s.types).cuda()
+    for box in (np.zeros(9), np.diag([18.17, -18.17, 18.17]).reshape(9)):
+        with pytest.raises(binding.DPError) as e:
+            m.compute(c, t, box)
+        assert e.value.code == -2
+    L = binding.lib()
+    need = m.workspace_bytes(s.natoms)
+    ws = torch.empty(need + 512, dtype=torch.uint8, device="cuda")
+    out = [torch.empty(k, dtype=torch.float64, device="cuda") for k in (1, s.natoms, 3 * s.natoms, 9)]
+    boxh = np.ascontiguousarray(s.box, dtype=np.float64)
+    bp = boxh.ctypes.data_as(C.POINTER(C.c_double))
+
+    def call(n, wsptr, wsbytes):
+        return L.dp_compute(m._h, n, c.data_ptr(), t.data_ptr(), bp, wsptr, wsbytes, None, out[0].data_ptr(), out[1].data_ptr(),
+                            out[2].data_ptr(), out[3].data_ptr())
+    base = (ws.data_ptr() + 255) & ~255
+    assert call(s.natoms, base, need) == 0
+    assert call(s.natoms, base, need - 256) == -3
+    assert call(s.natoms, base + 8, need) == -1
+    assert call(0, base, need) == -1
+    assert L.dp_workspace_bytes(m._h, 1 << 25) == 0 and L.dp_workspace_bytes(m._h, (1 << 24)) == 0   # 2^24 * 256 rows >= 2^31
+    torch.cuda.synchronize()
+    m.close()
+    # 298 neighbours inside rc = 9.5 A against a sort buffer of 256 (capacity 16)
+    s2 = synth.copper(6, 0.05, 3, rc=9.5, rc_smth=2.0, sel=(16,))
+    m = binding.DPModel(s2.model, "fp64")
+    m.compute(torch.from_numpy(s2.coords).cuda(), torch.from_numpy(s2.types).cuda(), s2.box)
+    rc, _ = m.status()
+    m.close()
+    assert rc == -6
 
 
 def test_overflow_keeps_nearest_and_counts():
@@ -97,12 +158,29 @@ def test_water_mix32_and_mix16_full_parity():
         assert np.abs(g["virial"] - o["virial"]).max() <= tol * vmax
 
 
+def _check_mixed(g, o, natoms, tol, tolE):
+    """list bit-exact; forces, virial within tol of RMS(F) / max|Xi|; energy within tolE eV per atom"""
+    assert np.array_equal(g["nlist"], o["nlist"]) and g["n_truncated"] == o["n_truncated"]
+    _check_forces(g, o, tol)
+    vmax = np.abs(o["virial"]).max()
+    assert np.abs(g["virial"] - o["virial"]).max() <= tol * vmax, np.abs(g["virial"] - o["virial"]).max() / vmax
+    assert abs(g["energy"][0] - o["energy"]) / natoms <= tolE
+    assert np.abs(g["atom_energy"] - o["atom_energy"]).max() <= 5 * tolE
+
+
 def test_copper_mix16_parity_config0_geometry():
     s = synth.config(0)
     o = oracle.evaluate(s.coords, s.types, s.box, s.model)
-    g = _gpu_eval(s, "mix16")
-    assert np.array_equal(g["nlist"], o["nlist"])
-    _check_forces(g, o, 5e-3)
+    _check_mixed(_gpu_eval(s, "mix16"), o, s.natoms, 5e-3, 1e-3)
+
+
+def test_copper_mix32_and_mix16_parity_config2_geometry():
+    """copper 13,500 atoms in both mixed modes against the full oracle: E, F, virial, list (MIX-32 on copper; the mixed-mode
+    virial on a system with more than a few tiles per type)"""
+    s = synth.config(2)
+    o = oracle.evaluate(s.coords, s.types, s.box, s.model)
+    _check_mixed(_gpu_eval(s, "mix32"), o, s.natoms, 1e-4, 2e-5)
+    _check_mixed(_gpu_eval(s, "mix16"), o, s.natoms, 5e-3, 1e-3)
 
 
 def _sampled_check(idx, nsample, tol, tolEi):
@@ -138,15 +216,55 @@ def test_config2_fp64_full_size():
     _check_fp64(g, o)
 
 
-def test_config3_mix32_full_size_sampled():
-    """water 110,592 atoms, MIX-32, in the launch configuration bench.py times; sampled oracle centres."""
-    ntr = _sampled_check(3, nsample=64, tol=1e-4, tolEi=2e-5)
-    assert ntr > 0            # the 97.4 A box over-fills a few blocks (DESIGN.md reading Q23)
+def test_config3_mix32_full_size_full_oracle():
+    """water 110,592 atoms, MIX-32, in the launch configuration bench.py times, against the FULL oracle (all atoms: E, every
+    force component, virial, every list row, the truncation count; about a minute of host time)."""
+    s = synth.config(3)
+    o = oracle.evaluate(s.coords, s.types, s.box, s.model)
+    g = _gpu_eval(s)
+    assert o["n_truncated"] > 0            # the 97.4 A box over-fills a few blocks (DESIGN.md reading Q23)
+    _check_mixed(g, o, s.natoms, 1e-4, 2e-5)
 
 
 def test_config4_mix16_full_size_sampled():
-    """copper 1,048,576 atoms, MIX-16, shuffled atom order; sampled oracle centres."""
-    _sampled_check(4, nsample=48, tol=5e-3, tolEi=1e-3)
+    """copper 1,048,576 atoms, MIX-16, shuffled atom order; 256 sample atoms, ~46k oracle centres."""
+    _sampled_check(4, nsample=256, tol=5e-3, tolEi=1e-3)
+
+
+def test_config4_mix16_full_size_against_stored_full_oracle():
+    """config 4 against tests/golden/c4_full.npz, written once by tests/golden/make_full_size_golden.py from a FULL oracle
+    evaluation (oracle/ only): every one of the 1,048,576 list rows by checksum, total E, the virial, the truncation count, and
+    the forces and atomic energies of a fixed 4,096-atom subset, at the MIX-16 tolerances (RMS(F) over all atoms)."""
+    import os
+    import sys
+    import torch
+    from paper_2005_00223_b200 import binding
+    gold_dir = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    sys.path.insert(0, gold_dir)
+    from make_full_size_golden import group_sums, row_hash
+    gd = np.load(os.path.join(gold_dir, "c4_full.npz"))
+    s = synth.config(4)
+    m = binding.DPModel(s.model, s.precision)
+    out = m.compute(torch.from_numpy(s.coords).cuda(), torch.from_numpy(s.types).cuda(), s.box)
+    rc, ntr = m.status()
+    assert rc == 0 and ntr == int(gd["n_truncated"])
+    nl = m.get_nlist().cpu().numpy()
+    F = out["forces"].cpu().numpy()
+    ea = out["atom_energy"].cpu().numpy()
+    E = float(out["energy"].item())
+    V = out["virial"].cpu().numpy()
+    m.close()
+    gs = group_sums(row_hash(nl))
+    bad = np.nonzero(gs != gd["nlist_group_sum"])[0]
+    assert bad.size == 0, f"{bad.size} groups of 16 list rows differ from the oracle, first group {bad[:4]}"
+    sub = gd["subset"]
+    rms = float(gd["rms_f"])
+    err = np.abs(F[sub] - gd["forces_subset"]).max()
+    assert err <= 5e-3 * rms, (err / rms)
+    assert np.abs(ea[sub] - gd["atom_energy_subset"]).max() <= 5e-3
+    assert abs(E - float(gd["energy"])) / s.natoms <= 1e-3
+    vmax = np.abs(gd["virial"]).max()
+    assert np.abs(V - gd["virial"]).max() <= 5e-3 * vmax, np.abs(V - gd["virial"]).max() / vmax
 
 
 # ------------------------------------------------------------------ MIX-16 tcgen05 path: edge cases of the tiling
@@ -156,9 +274,7 @@ def test_mix16_overflow_blocks_have_no_padded_row():
     o = oracle.evaluate(s.coords, s.types, s.box, s.model)
     g = _gpu_eval(s, "mix16")
     assert np.array_equal(g["nlist"], o["nlist"]) and g["n_truncated"] == 500
-    # Outside the five BASELINE configs the 5e-3 bound is not guaranteed: with only 100 rows per atom the single-fp16
-    # activations of the forward kernel average less (measured 5.2e-3).  The bound here is 2x.
-    _check_forces(g, o, 1e-2)
+    _check_forces(g, o, 5e-3)
     assert g["rows"] == (500 * 100, 500 * 100)            # forward and backward push the same compact rows
 
 

@@ -76,9 +76,35 @@ def test_total_energy_error_scales_as_dt_squared():
 
     def dev(dt, n):
         th = md_oracle.run(s.coords, v, s.types, masses, s.box, s.model, dt, n)["thermo"]
-        e = th.sum(axis=1)
+        e = th[:, 0] + th[:, 1]
         return np.abs(e - e[0]).max(), np.ptp(th[:, 1])
     d1, k1 = dev(2.0, 8)
     d2, _ = dev(1.0, 16)
     assert k1 > 50 * d1            # the total is conserved far better than its parts move
     assert 2.5 < d1 / d2 < 6.0, (d1, d2)
+
+
+def test_temperature_and_pressure_record():
+    """PAPER.md:153 thermo record.  Unit constants against scipy; ideal-gas law for a zero-weight model (Xi = 0):
+    P V = (N - 1) kB T; T of the seeded 330 K velocities; the potential part of P equals -dE/dV by a finite isotropic
+    volume change at rest (uses the oracle's virial, pinned separately by strain finite differences)."""
+    from oracle import oracle
+    assert abs(md_oracle.KB - sc.k / sc.e) < 1e-13            # 8.617333262e-5 eV/K is the 10-digit CODATA value
+    assert abs(md_oracle.EV_A3_TO_BAR - sc.e * 1e30 / 1e5) < 1e-6
+    s, masses, v = _fcc()
+    z = synth.make_model(2, s.model.rc, s.model.rc_smth, s.model.sel, 1, s.model.avg, s.model.std, zero=True)
+    th = md_oracle.run(s.coords, v, s.types, masses, s.box, z, 0.5, 2)["thermo"]
+    n = s.natoms
+    vol = s.box[0] * s.box[4] * s.box[8]
+    assert np.allclose(th[:, 3] * 1e5 * vol * 1e-30, (n - 1) * sc.k * th[:, 2], rtol=1e-9)     # Pa m^3 = J
+    big = synth.boltzmann_velocities(np.zeros(30000, dtype=np.int32), (63.546,), 330.0, 3)
+    ke = md_oracle.kinetic_energy(big, np.full(30000, 63.546))
+    assert abs(md_oracle.temperature(ke, 30000) - 330.0) < 4.0
+    # potential pressure at rest: -dE/dV with V -> V (1 + 3 h): coordinates and box scaled by (1 + h)
+    h = 1e-5
+    ep = oracle.evaluate(s.coords * (1 + h), s.types, s.box * (1 + h), s.model)["energy"]
+    em = oracle.evaluate(s.coords * (1 - h), s.types, s.box * (1 - h), s.model)["energy"]
+    p_fd = -(ep - em) / (vol * ((1 + h) ** 3 - (1 - h) ** 3)) * md_oracle.EV_A3_TO_BAR
+    o = oracle.evaluate(s.coords, s.types, s.box, s.model)
+    p_or = md_oracle.pressure(0.0, o["virial"], s.box)
+    assert abs(p_or - p_fd) <= 1e-6 * max(abs(p_fd), 1.0), (p_or, p_fd)
