@@ -3,6 +3,10 @@
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..4] [--impl ours|reference]
 
+The default run times config 4 (headline), then configs 0-3 (`configs_summary`, each with its own roofline and oracle
+timing), measures the arithmetic-pipe peaks it quotes (`peaks`, dp_measure_peaks) and runs the paper's MD protocol
+(`md`, PAPER.md:151-153).
+
 One "step" = one dp_compute (all of SURVEY.md section 8(a): cell list, formatted neighbour list, environment
 matrix, embedding net + contraction, fitting net forward/backward, embedding backward, ProdForce, ProdViral)
 on one seeded synthetic configuration.  The path does not shard (BASELINE north_star: one GPU, no
@@ -28,13 +32,13 @@ sys.path.insert(0, ROOT)
 FLOP_ROW_FWD = 12550 + 800          # embedding GEMMs forward + contraction forward, per neighbour row
 FLOP_ROW_BWD = 12550 + 1600         # embedding GEMMs backward + contraction backward, per neighbour row
 FLOP_ATOM_FIT = 2036160             # fitting fwd + bwd + descriptor fwd/bwd, per atom
-FP64_OVER_BF16_NOMINAL = 45.0 / 2250.0
 # tensor-core flops the MIX-16 backward kernel actually executes per 128-row tile (M = 128, 2 flop per MAC):
 # layer 2 (hi+lo) 2*32*64, layer 3 2*96*112, dR 2*208*16, dT3 32*112, dT2+dz3 W3^T (32+112)*64, dT1+dz3 W3f (32+112)*32, dz2 W2^T 64*32
 EXEC_FLOP_ROW_BWD = 2 * (2 * 32 * 64 + 2 * 96 * 112 + 2 * 208 * 16 + 32 * 112 + 144 * 64 + 144 * 32 + 64 * 32)
-MUFU_TANH_PEAK = 16 * 148 * 1.965e9          # tanh.approx.f32 per second, measured
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, one ncu --set full capture per config (profiles/)
-TRAFFIC = {"c4_cu1048576": 8.045858e9 + 3.012969e9}   # k_embed_bwd_tc2, profiles/r01_c4_bwd_tc2_ncu.md
+# ncu --set full captures of the dominant kernel per config (dram__bytes_read.sum + dram__bytes_write.sum per launch are in
+# these summaries; the bench line itself measures no DRAM traffic, so roofline.traffic is null and points here)
+TRAFFIC_PROFILE = {"c4_cu1048576": "profiles/r02_c4_bwd_tc2_ncu.md", "c2_cu13500": "profiles/r02_c2_embed_bwd_ncu.md",
+                   "c3_water110592": "profiles/r02_c3_embed_bwd_ncu.md"}
 
 
 def peaks():
@@ -119,9 +123,8 @@ def run_reference(args, s):
     print(json.dumps(line))
 
 
-def time_config(binding, torch, s, dev, steps, warmup, flush, profile=True):
+def time_config(binding, torch, s, dev, steps, warmup, flush):
     """Device-resident timing of one config: per-step CUDA events, L2 flush between steps, per-phase events."""
-    N = s.natoms
     model = binding.DPModel(s.model, s.precision)
     coords = torch.from_numpy(s.coords).to(dev)
     types = torch.from_numpy(s.types).to(dev)
@@ -153,6 +156,48 @@ def time_config(binding, torch, s, dev, steps, warmup, flush, profile=True):
                 rows_f=rows_f, rows_b=rows_b, ntr=ntr)
 
 
+def roofline_of(s, r, pk, mp):
+    """Roofline record of the dominant kernel (the embedding backward in every precision mode) of one timed config.
+    achieved = algorithmic flops of the kernel (SURVEY.md 8(d): 14,150 per REAL neighbour row) / its CUDA-event duration;
+    peak = the measured rate of the pipe its dtype runs on (pk: MEASURED_PEAKS.json, mp: dp_measure_peaks of this run)."""
+    ph = r["phases"]
+    dom_flops = r["real_rows"] * FLOP_ROW_BWD
+    ach = dom_flops / (ph[5] * 1e-3) / 1e12
+    if s.precision == "fp64":
+        kname, peak = "k_embed_bwd_f64 (S7-S9 in one kernel)", mp["dmma_tflops"]
+        peak_src = "measured in this run (dp_measure_peaks): fp64 tensor pipe, mma.sync m8n8k4 (DFMA shares the pipe: %.1f TF/s)" % mp["dfma_tflops"]
+    elif s.precision == "mix32":
+        kname, peak = "k_embed_bwd_mix (S7-S9 in one kernel)", mp["ffma_tflops"]
+        peak_src = ("measured in this run (dp_measure_peaks): fp32 FMA pipe, the pipe of single-precision arithmetic; the kernel "
+                    "forms its single-precision products as three fp16 mma.sync products (measured mma.sync rate %.0f TF/s)" % mp["hmma_sync_tflops"])
+    else:
+        kname, peak = "k_embed_bwd_tc2", pk["bf16_sus"]
+        peak_src = f"{pk['src']}: dense bf16 sustained (fp16 has the same nominal rate)"
+    rec = {"kernel": kname, "bound": "tensor", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+           "traffic": None, "traffic_profile": TRAFFIC_PROFILE.get(s.name), "peak_source": peak_src,
+           "flops_per_launch": dom_flops, "kernel_ms": ph[5]}
+    if s.precision != "fp64":
+        # the tanh of the recomputed forward, counted on the real rows only (175 per row), against the measured MUFU rate
+        rec["mufu_tanh_frac"] = (r["real_rows"] * 175 / (ph[5] * 1e-3)) / (mp["tanh_tera_per_s"] * 1e12)
+    if s.precision == "mix16":
+        rec["executed_tflops"] = r["rows_b"] * EXEC_FLOP_ROW_BWD / (ph[5] * 1e-3) / 1e12
+        rec["note"] = ("algorithmic backward flops (14,150 per real neighbour row); the in-kernel forward recompute, the hi/lo operand "
+                       "splitting and the K/N padding are executed (executed_tflops) but not credited; mufu_tanh_frac = tanh of the "
+                       "real rows / measured tanh.approx.f32 rate")
+    return rec
+
+
+def kernels_of(s, r, ms_step):
+    ph, N, rr = r["phases"], s.natoms, r["real_rows"]
+    return {"nlist_ms": ph[0], "embed_fwd_ms": ph[1], "fit_ms": ph[2], "embed_bwd_ms": ph[3], "finalize_ms": ph[4],
+            "embed_bwd_kernel_ms": ph[5],
+            "embed_fwd_tflops": rr * FLOP_ROW_FWD / (ph[1] * 1e-3) / 1e12,
+            "fit_tflops": N * FLOP_ATOM_FIT / (ph[2] * 1e-3) / 1e12,
+            "embed_bwd_tflops": rr * FLOP_ROW_BWD / (ph[5] * 1e-3) / 1e12,
+            "fused_embed_fwd_bwd_tflops": rr * (FLOP_ROW_FWD + FLOP_ROW_BWD) / ((ph[1] + ph[3]) * 1e-3) / 1e12,
+            "step_tflops": (rr * (FLOP_ROW_FWD + FLOP_ROW_BWD) + N * FLOP_ATOM_FIT) / (ms_step * 1e-3) / 1e12}
+
+
 def max_over_ranks(times_ms, world, device):
     """Replicas only: every rank times the same number of steps of its own replica; the job time is the
     MAX over ranks (one all-reduce of the timings, no data-path collective)."""
@@ -169,6 +214,49 @@ def whole_job_value(natoms, steps, world, t_ms):
     return world * natoms * steps / (t_ms * 1e-3)
 
 
+def spawn_replicas(ngpus: int, argv) -> int:
+    """`python bench.py --gpus N` outside torchrun: launch the N replica ranks ourselves (one process per GPU, NCCL only for
+    the max-over-ranks of the timings), exactly as the driver's torchrun line does."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={ngpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+    return subprocess.call(cmd)
+
+
+def md_leg(args, torch, synth, s, model, coords, types, dev, st, barrier):
+    """The paper's own time-to-solution: MD loop time / steps, one dp_md_run: velocity Verlet, 330 K,
+    2 A buffered list searched every 50 evaluations, thermo record (E_pot, E_kin, T, P) of every evaluation."""
+    N = s.natoms
+    kind = "water" if s.model.ntypes == 2 else "cu"
+    dt_fs = 0.5 if kind == "water" else 1.0
+    vel = torch.from_numpy(synth.boltzmann_velocities(s.types, synth.MASS_AMU[kind], 330.0, 99)).to(dev)
+    xmd = coords.clone()
+    model.md_run(xmd, vel, types, synth.MASS_AMU[kind], s.box, dt_fs, 1, skin=2.0, rebuild_every=50)   # warm-up
+    barrier()
+    m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    m0.record(st)
+    mo = model.md_run(xmd, vel, types, synth.MASS_AMU[kind], s.box, dt_fs, args.md_steps, skin=2.0, rebuild_every=50)
+    m1.record(st)
+    barrier()
+    rc_md, _ = model.status()
+    th = mo["thermo"].cpu().numpy()
+    md_ms = m0.elapsed_time(m1)
+    every = 20                                                     # PAPER.md:153: recorded every 20 time-steps
+    return {"steps": args.md_steps, "evaluations": args.md_steps + 1, "list_searches": args.md_steps // 50 + 1, "dt_fs": dt_fs,
+            "temperature_K": 330.0, "loop_ms_per_step": md_ms / args.md_steps,
+            "s_per_step_per_atom": md_ms * 1e-3 / args.md_steps / N, "status": rc_md,
+            "e_total_first_last_eV": [float(th[0, :2].sum()), float(th[-1, :2].sum())], "e_kin_first_eV": float(th[0, 1]),
+            "thermo_every_20_steps": {"step": list(range(0, args.md_steps + 1, every)),
+                                      "e_pot_eV": [float(x) for x in th[::every, 0]], "e_kin_eV": [float(x) for x in th[::every, 1]],
+                                      "temperature_K": [float(x) for x in th[::every, 2]],
+                                      "pressure_bar": [float(x) for x in th[::every, 3]]},
+            "skin_A": 2.0, "rebuild_every": 50,
+            "note": "velocity Verlet, 2 A buffered list searched at evaluation 0 and every 50 (PAPER.md:153), no L2 flush between steps"}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -176,15 +264,18 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4,
                     help="BASELINE.json configs index (default: c4, copper 1,048,576 atoms MIX-16, the largest single-GPU config)")
-    ap.add_argument("--all-configs", action="store_true", help="also time the other four configs (summary table in the JSON line)")
+    ap.add_argument("--no-summary", action="store_true", help="skip the configs_summary leg (the other four configs)")
     ap.add_argument("--precision", default=None, choices=["fp64", "mix32", "mix16"],
                     help="override the config's precision (profiling aid; the default is the precision BASELINE.json names)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--md-steps", type=int, default=20,
+    ap.add_argument("--md-steps", type=int, default=100,
                     help="also time an MD loop of this many velocity-Verlet steps (dp_md_run; 0 = skip; N = 1 only)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    if args.impl == "ours" and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        raise SystemExit(spawn_replicas(args.gpus, sys.argv[1:]))
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -229,7 +320,7 @@ def main():
     barrier()
     clocks = sampler.stop()
     model, coords, types, out = r["model"], r["coords"], r["types"], r["out"]
-    t_ms, phases, real_rows, rows_f, rows_b, ntr = r["t_ms"], r["phases"], r["real_rows"], r["rows_f"], r["rows_b"], r["ntr"]
+    t_ms = r["t_ms"]
 
     # end to end through the public API with HOST buffers: H2D of inputs, compute, D2H of results, every step
     res_h = dict(energy=torch.empty(1, dtype=torch.float64).pin_memory(),
@@ -260,98 +351,68 @@ def main():
 
     t_ms, e2e_ms = max_over_ranks([t_ms, e2e_ms], world, dev)
 
-    # the paper's own time-to-solution: MD loop time / steps, one dp_md_run of md_steps steps
     md = None
     if world == 1 and args.md_steps > 0:
         try:
-            kind = "water" if s.model.ntypes == 2 else "cu"
-            dt_fs = 0.5 if kind == "water" else 1.0
-            vel = torch.from_numpy(synth.boltzmann_velocities(s.types, synth.MASS_AMU[kind], 330.0, 99)).to(dev)
-            xmd = coords.clone()
-            model.md_run(xmd, vel, types, synth.MASS_AMU[kind], s.box, dt_fs, 1, skin=2.0, rebuild_every=50)   # warm-up
-            barrier()
-            m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            m0.record(st)
-            mo = model.md_run(xmd, vel, types, synth.MASS_AMU[kind], s.box, dt_fs, args.md_steps, skin=2.0, rebuild_every=50)
-            m1.record(st)
-            barrier()
-            rc_md, _ = model.status()
-            th = mo["thermo"].cpu().numpy()
-            md_ms = m0.elapsed_time(m1)
-            md = {"steps": args.md_steps, "evaluations": args.md_steps + 1, "dt_fs": dt_fs, "temperature_K": 330.0,
-                  "loop_ms_per_step": md_ms / args.md_steps, "s_per_step_per_atom": md_ms * 1e-3 / args.md_steps / N,
-                  "status": rc_md, "e_total_first_last_eV": [float(th[0, :2].sum()), float(th[-1, :2].sum())],
-                  "e_kin_first_eV": float(th[0, 1]),
-                  "skin_A": 2.0, "rebuild_every": 50,
-                  "note": "velocity Verlet, 2 A buffered list searched at evaluation 0 and every 50 (PAPER.md:153), "
-                          "no L2 flush between steps"}
+            md = md_leg(args, torch, synth, s, model, coords, types, dev, st, barrier)
         except Exception as ex:      # the MD leg never takes the bench line down
             md = {"error": repr(ex)}
 
     if rank == 0:
         pk = peaks()
+        mp = binding.measure_peaks()
         ms_step = t_ms / K
         value = whole_job_value(N, K, world, t_ms)
-        if s.precision == "fp64":
-            peak = pk["bf16_sus"] * FP64_OVER_BF16_NOMINAL
-            peak_src = f"{pk['src']}: bf16 sustained {pk['bf16_sus']} TF/s x nominal fp64/bf16 ratio 45/2250"
-            kname = "k_embed_bwd_f64"
-        else:
-            peak = pk["bf16_sus"]
-            peak_src = f"{pk['src']}: dense bf16 sustained (fp16 has the same nominal rate)"
-            kname = "k_embed_bwd_tc2" if s.precision == "mix16" else "k_embed_bwd_mix"
-        dom_flops = real_rows * FLOP_ROW_BWD
-        ach = dom_flops / (phases[5] * 1e-3) / 1e12           # phases[5]: CUDA events around the backward kernel alone
-        kern = {"nlist_ms": phases[0], "embed_fwd_ms": phases[1], "fit_ms": phases[2], "embed_bwd_ms": phases[3],
-                "finalize_ms": phases[4], "embed_bwd_kernel_ms": phases[5],
-                "tanh_per_s_bwd_kernel": rows_b * 175 / (phases[5] * 1e-3),
-                "embed_fwd_tflops": real_rows * FLOP_ROW_FWD / (phases[1] * 1e-3) / 1e12,
-                "fit_tflops": N * FLOP_ATOM_FIT / (phases[2] * 1e-3) / 1e12,
-                "embed_bwd_tflops": ach,
-                "step_tflops": (real_rows * (FLOP_ROW_FWD + FLOP_ROW_BWD) + N * FLOP_ATOM_FIT) / (ms_step * 1e-3) / 1e12}
         line = {"metric": "atom_steps_per_s", "value": value, "unit": "atom-steps/s", "n_gpus": world, "steps": K,
                 "warmup": args.warmup, "ms_per_step": ms_step, "s_per_step_per_atom": ms_step * 1e-3 / N,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": {"fp64": "f64", "mix32": "f32", "mix16": "f16"}[s.precision], "data": "synthetic",
                 "config": {"workload": s.name, "natoms": N, "precision": s.precision, "nm": s.model.nm,
-                           "real_neighbour_rows": real_rows, "rows_through_embedding_fwd": rows_f,
-                           "rows_through_embedding_bwd": rows_b, "n_truncated_atoms": ntr,
+                           "real_neighbour_rows": r["real_rows"], "rows_through_embedding_fwd": r["rows_f"],
+                           "rows_through_embedding_bwd": r["rows_b"], "n_truncated_atoms": r["ntr"],
                            "parallelism": "replicas only" if world > 1 else "single GPU",
                            "l2": "256 MB flush between timed steps, per-step CUDA events"},
                 "clocks": clocks,
                 "e2e": {"value": world * N * K / (e2e_ms * 1e-3), "unit": "atom-steps/s", "h2d_bytes_per_step": h2d,
                         "d2h_bytes_per_step": d2h},
                 "gpu_launches": model.launches_per_compute() * K,
-                "roofline": {"kernel": kname, "bound": "tensor", "achieved": ach, "peak": peak,
-                             "unit": "TFLOP/s", "frac": ach / peak, "traffic": TRAFFIC.get(s.name),
-                             "peak_source": peak_src,
-                             "flops_per_launch": dom_flops,
-                             "executed_tflops": (rows_b * EXEC_FLOP_ROW_BWD / (phases[5] * 1e-3) / 1e12) if s.precision == "mix16" else None,
-                             "mufu_tanh_frac": (rows_b * 175 / (phases[5] * 1e-3)) / MUFU_TANH_PEAK,
-                             "note": "algorithmic backward flops (14,150 per real neighbour row); the in-kernel forward recompute, "
-                                     "the hi/lo operand splitting and the K/N padding are executed (executed_tflops) but not credited; "
-                                     "mufu_tanh_frac = tanh issued by this kernel / measured MUFU.TANH peak (16 per clock per SM)"},
-                "kernels": kern}
+                "roofline": roofline_of(s, r, pk, mp),
+                "kernels": kernels_of(s, r, ms_step),
+                "peaks": {"hbm_gbs": pk["hbm"], "bf16_tflops_burst": pk["bf16"], "bf16_tflops_sustained": pk["bf16_sus"],
+                          "source_hbm_bf16": pk["src"], **mp,
+                          "source_pipes": "dp_measure_peaks in this run: 8 independent chains per thread, 8 x 256 threads per SM, CUDA events"}}
         if md is not None:
             line["md"] = md
-        if args.all_configs and world == 1:
-            summ = {}
-            for idx in range(5):
-                if idx == args.config:
-                    summ[s.name] = {"ms_per_step": ms_step, "atom_steps_per_s": value, "precision": s.precision}
-                    continue
-                s2 = synth.config(idx)
-                r2 = time_config(binding, torch, s2, dev, max(5, K), args.warmup, flush)
-                ms2 = r2["t_ms"] / max(5, K)
-                summ[s2.name] = {"ms_per_step": ms2, "atom_steps_per_s": s2.natoms / (ms2 * 1e-3), "precision": s2.precision,
-                                 "phases_ms": [round(float(x), 4) for x in r2["phases"]]}
-                r2["model"].close()
-            line["configs_summary"] = summ
         if world == 1 and not args.no_cpu_baseline:
             ncen = min(N, 16384)
             n, dt, cores = oracle_sample(s, ncen)
             line["cpu_baseline"] = {"value": n / dt, "unit": "atom-steps/s", "cores": cores, "kind": "oracle",
                                     "sample": f"{n} evenly spaced centre atoms of {s.name}, one evaluation ({dt:.1f} s)"}
+        if world == 1 and not args.no_summary:
+            # the other BASELINE configs: same timing method (warm-up, L2 flush, per-step events), own roofline and oracle timing
+            summ = {s.name: {"precision": s.precision, "natoms": N, "ms_per_step": ms_step, "atom_steps_per_s": value,
+                             "s_per_step_per_atom": ms_step * 1e-3 / N, "roofline_frac": line["roofline"]["frac"]}}
+            model.close()
+            del model, coords, types, out, cdev, tdev
+            torch.cuda.empty_cache()
+            for idx in range(5):
+                if idx == args.config:
+                    continue
+                s2 = synth.config(idx)
+                k2 = max(10, K)
+                r2 = time_config(binding, torch, s2, dev, k2, args.warmup, flush)
+                ms2 = r2["t_ms"] / k2
+                rec = {"precision": s2.precision, "natoms": s2.natoms, "steps": k2, "ms_per_step": ms2,
+                       "atom_steps_per_s": s2.natoms / (ms2 * 1e-3), "s_per_step_per_atom": ms2 * 1e-3 / s2.natoms,
+                       "real_neighbour_rows": r2["real_rows"], "n_truncated_atoms": r2["ntr"],
+                       "roofline": roofline_of(s2, r2, pk, mp), "kernels": kernels_of(s2, r2, ms2)}
+                r2["model"].close()
+                if not args.no_cpu_baseline:
+                    n2, dt2, cores2 = oracle_sample(s2, min(s2.natoms, 4096))
+                    rec["cpu_baseline"] = {"value": n2 / dt2, "unit": "atom-steps/s", "cores": cores2, "kind": "oracle",
+                                           "sample": f"{n2} evenly spaced centre atoms of {s2.name}, one evaluation ({dt2:.1f} s)"}
+                summ[s2.name] = rec
+            line["configs_summary"] = summ
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -141,6 +141,15 @@ int dp_md_run(dp_model *m, long natoms, double *coords_dev, double *vel_dev, con
               double skin, int rebuild_every, void *workspace_dev, size_t workspace_bytes, void *cuda_stream,
               double *forces_dev, double *thermo_dev, double *virial_dev);
 
+/* Measured peaks of the arithmetic pipes the path is bound by, for the roofline fractions of the benchmark (
+ * the paper reports its own GEMM efficiency against the hardware limit): a few milliseconds of synthetic
+ * single-instruction-kind kernels on the current device, timed with CUDA events on cuda_stream (synchronises; allocates 64
+ * bytes).  out_host[DP_NPEAKS]: [0] fp64 FMA TFLOP/s (DFMA), [1] fp64 tensor TFLOP/s (mma.sync m8n8k4), [2] fp32 FMA
+ * TFLOP/s (FFMA), [3] tanh.approx.f32 in 1e12 per second (MUFU), [4] fp16 mma.sync m16n8k16 TFLOP/s, [5] number of SMs.
+ * Not part of the evaluation path. */
+#define DP_NPEAKS 6
+int dp_measure_peaks(double *out_host, int n_out, void *cuda_stream);
+
 void dp_destroy(dp_model *m);
 const char *dp_strerror(int code);
 

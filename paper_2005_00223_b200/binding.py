@@ -18,7 +18,7 @@ DP_FP64, DP_MIX32, DP_MIX16 = 0, 1, 2
 PRECISIONS = {"fp64": DP_FP64, "mix32": DP_MIX32, "mix16": DP_MIX16}
 EXPORTS = ["dp_create", "dp_workspace_bytes", "dp_compute", "dp_get_nlist", "dp_status",
            "dp_launches_per_compute", "dp_last_row_counts", "dp_profile_enable", "dp_profile_read", "dp_md_run",
-           "dp_md_workspace_bytes",           "dp_destroy", "dp_strerror"]
+           "dp_md_workspace_bytes", "dp_measure_peaks", "dp_destroy", "dp_strerror"]
 
 
 class DPError(RuntimeError):
@@ -69,6 +69,8 @@ def lib():
                                 C.c_size_t, vp, vp, vp, vp]
         L.dp_md_workspace_bytes.restype = C.c_size_t
         L.dp_md_workspace_bytes.argtypes = [vp, C.c_long, C.c_double]
+        L.dp_measure_peaks.restype = C.c_int
+        L.dp_measure_peaks.argtypes = [dp, C.c_int, vp]
         L.dp_destroy.restype = None
         L.dp_destroy.argtypes = [vp]
         _lib = L
@@ -224,6 +226,18 @@ class DPModel:
             self.close()
         except Exception:
             pass
+
+
+def measure_peaks(stream=None) -> dict:
+    """dp_measure_peaks on the current device: measured DFMA / DMMA / FFMA / tanh.approx / mma.sync rates."""
+    import torch
+    out = np.zeros(6)
+    st = stream if stream is not None else torch.cuda.current_stream()
+    rc = lib().dp_measure_peaks(_dptr(out), 6, st.cuda_stream)
+    if rc != 0:
+        raise DPError(rc, "dp_measure_peaks")
+    return dict(dfma_tflops=out[0], dmma_tflops=out[1], ffma_tflops=out[2], tanh_tera_per_s=out[3],
+                hmma_sync_tflops=out[4], sms=int(out[5]))
 
 
 def compute_host(model_handle: DPModel, coords_np, types_np, box, device="cuda:0"):

@@ -371,6 +371,14 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
         std::vector<EmbedNetTC2> nets((size_t)T * T);
         for (int ab = 0; ab < T * T; ++ab) build_embed_tc2(w->embed + ab * ensz, &nets[ab]);
         ok(upload(nets, &m->embed_tc2_dev));
+        // short neighbour rows: the forward's rounding of the activations to one fp16 value averages over too few rows to
+        // hold the MIX-16 force tolerance (measured): carry them as hi + lo pairs there
+        m->fwd_split = Nm < 128 ? 1 : 0;
+        if (m->fwd_split) {
+            std::vector<EmbedNetTC<1>> n1((size_t)T * T);
+            for (int ab = 0; ab < T * T; ++ab) build_embed_tc<1>(w->embed + ab * ensz, &n1[ab]);
+            ok(upload(n1, &m->embed_tc_dev));
+        }
     }
     const int ND = M2E * 16, F = 240;
     const size_t fnsz = (size_t)ND * F + F + (size_t)F * F + F + (size_t)F * F + F + F + 1;
@@ -472,7 +480,7 @@ int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *ty
     const bool f64 = m->prec == DP_FP64;
     const bool m16 = m->prec == DP_MIX16;
     ok(f64 ? launch_embed_fwd_f64(m, natoms, g, ws, L, st)
-           : (m16 ? launch_embed_fwd_tc2(m, natoms, g, ws, L, st) : launch_embed_fwd_tc(m, natoms, g, ws, L, st)));
+           : (m16 && !m->fwd_split ? launch_embed_fwd_tc2(m, natoms, g, ws, L, st) : launch_embed_fwd_tc(m, natoms, g, ws, L, st)));
     mark(2);
     ok(f64 ? launch_fit_f64(m, natoms, g, ws, L, st) : (m16 ? launch_fit_tc(m, natoms, g, ws, L, st) : launch_fit_mix(m, natoms, g, ws, L, st)));
     mark(3);

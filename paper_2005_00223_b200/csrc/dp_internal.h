@@ -64,7 +64,8 @@ struct dp_model {
     int *type_map_dev;
     // device weights
     void *embed_frag_dev;           // T*T EmbedNetFrag<double> (FP64) / EmbedNetFragH<2> (MIX-32 backward, mma.sync)
-    void *embed_tc_dev;             // T*T EmbedNetTC<2> (MIX-32 forward, tcgen05)
+    void *embed_tc_dev;             // T*T EmbedNetTC<2> (MIX-32 forward, tcgen05) / EmbedNetTC<1> (MIX-16 with fwd_split)
+    int fwd_split;                  // MIX-16, Nm < 128: forward with hi + lo activations (embed_tc.cu) instead of embed_tc2.cu
     void *embed_tc2_dev;            // T*T EmbedNetTC2 (MIX-16, warpgroup-per-tile tcgen05 kernels)
     void *fit_tc_img_dev;           // MIX-16: T x six fp16 weight images (fit_tc.cu)
     int device;                     // CUDA device the model was created on (dp_compute checks it)

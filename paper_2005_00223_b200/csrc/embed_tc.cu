@@ -9,7 +9,8 @@
 //   E3:     tcgen05.ld D3, + bias, tanh, + (y2,y2) -> G  -> operand image (MN-major use)
 //   MMA C:  DA[128 features x 8*slots] = G^T . R^w   (K = 128 rows; per-atom slots mask the rows of other atoms)
 //   E4:     tcgen05.ld DA -> A_i (fp32, global), scaled by 1/Nm
-// G never leaves the SM.  This kernel serves MIX-32 (NS = 3: hi + lo activations and weights); MIX-16 runs embed_tc2.cu.
+// G never leaves the SM.  This kernel serves MIX-32 (NS = 3: hi + lo activations and weights) and MIX-16 models with
+// Nm < 128 (NS = 2: hi + lo activations); MIX-16 otherwise runs embed_tc2.cu.
 // k_env_rows (S3, the compact fp32 environment rows) serves both mixed modes.
 #include "embed_tc.cuh"
 
@@ -466,7 +467,10 @@ cudaError_t launch_fwd(const dp_model *m, long N, const Grid3 &g, char *ws, cons
 
 }  // namespace
 
-// MIX-32: activations and weights as hi + lo fp16 pairs (three products per MMA step), exact tanhf
+// MIX-32: activations and weights as hi + lo fp16 pairs (three products per MMA step), exact tanhf.
+// MIX-16 models with a short neighbour row (Nm < 128, dp_model::fwd_split): activations as hi + lo pairs, fp16 weights,
+// tanh.approx; the single-fp16 activations of embed_tc2.cu average over too few rows there.
 cudaError_t launch_embed_fwd_tc(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    return launch_fwd<3, false>(m, N, g, ws, L, st);
+    if (m->prec == DP_MIX32) return launch_fwd<3, false>(m, N, g, ws, L, st);
+    return launch_fwd<2, true>(m, N, g, ws, L, st);
 }

@@ -37,3 +37,15 @@ def test_single_rank_is_identity():
     import bench
     assert bench.max_over_ranks([3.5, 7.25], 1, torch.device("cpu")) == [3.5, 7.25]
     assert bench.whole_job_value(500, 10, 1, 2.0) == 500 * 10 / 2.0e-3
+
+
+def test_gpus_flag_spawns_one_rank_per_gpu(monkeypatch):
+    """`python bench.py --gpus N` outside torchrun launches N ranks itself (same line as the driver's torchrun call)."""
+    sys.path.insert(0, ROOT)
+    import bench
+    seen = {}
+    monkeypatch.setattr(bench.subprocess, "call", lambda cmd: seen.setdefault("cmd", cmd) and 0)
+    assert bench.spawn_replicas(4, ["--gpus", "4", "--steps", "2"]) == 0
+    cmd = seen["cmd"]
+    assert "torch.distributed.run" in cmd and "--nproc-per-node=4" in cmd and "127.0.0.1" in cmd
+    assert cmd[-4:] == ["--gpus", "4", "--steps", "2"] and cmd[-5].endswith("bench.py")
