@@ -166,26 +166,62 @@ double oracle_fit_net(const double *net, int nd, int f0, int f1, int f2, const d
     return e;
 }
 
+/* N2t: general (triclinic) cell, rows a, b, c of the row-major 3 x 3 box H.  Inverse by cofactors, each entry one
+ * expression (compiled without contraction), so that any implementation that writes the same expressions gets the same bits. */
+static void box_inverse(const double *H, double *Hi, double *vol) {
+    const double c00 = H[4] * H[8] - H[5] * H[7], c01 = H[5] * H[6] - H[3] * H[8], c02 = H[3] * H[7] - H[4] * H[6];
+    const double det = H[0] * c00 + H[1] * c01 + H[2] * c02;
+    Hi[0] = c00 / det; Hi[1] = (H[2] * H[7] - H[1] * H[8]) / det; Hi[2] = (H[1] * H[5] - H[2] * H[4]) / det;
+    Hi[3] = c01 / det; Hi[4] = (H[0] * H[8] - H[2] * H[6]) / det; Hi[5] = (H[2] * H[3] - H[0] * H[5]) / det;
+    Hi[6] = c02 / det; Hi[7] = (H[1] * H[6] - H[0] * H[7]) / det; Hi[8] = (H[0] * H[4] - H[1] * H[3]) / det;
+    *vol = fabs(det);
+}
+
+/* N2t canonical wrap of a point into the cell: fractional coordinates t_k = x . Hinv[:,k] (fma chain, x0 first),
+ * n_k = floor(t_k), xw = x - n_0 a - n_1 b - n_2 c (fma chain, a first).  Exposed for the pins. */
+void oracle_wrap_triclinic(const double *H, const double *x, double *xw) {
+    double Hi[9], vol;
+    box_inverse(H, Hi, &vol);
+    double n[3];
+    for (int k = 0; k < 3; ++k) n[k] = floor(fma(x[2], Hi[6 + k], fma(x[1], Hi[3 + k], x[0] * Hi[k])));
+    for (int c = 0; c < 3; ++c) xw[c] = fma(-n[2], H[6 + c], fma(-n[1], H[3 + c], fma(-n[0], H[c], x[c])));
+}
+
 /* N1-N3: formatted neighbour rows of the listed centres by brute force over all atoms and all images.
- * box: orthorhombic, row-major 3x3 with zero off-diagonals (returns -2 otherwise).
+ * box: row-major 3 x 3, rows a, b, c.  Orthorhombic (zero off-diagonals): wrap N2 per axis, shift s * L per axis.
+ * General cell (reading N2t, the multi-component / arbitrary-cell systems of PAPER.md:107 and the ghost region of
+ * Fig. 1(a)): wrap N2t, shift vector v_c = fma(s_2, c_c, fma(s_1, b_c, s_0 * a_c)), image range per axis
+ * ceil(rc / h_k) with h_k the height of the cell perpendicular to the other two edges; d = (xw_j - xw_i) + v as in N2.
  * types: MODEL types in [0,T).  nlist_out [ncenters][Nm] user indices, -1 pad.  dvec_out [ncenters][Nm][3]
  * (may be NULL).  ntrunc_out (may be NULL): number of listed centres with at least one over-full block.
- * The only pruning is per axis, |d_axis| >= rc => r2 >= rc*rc, which cannot change the result. */
+ * The only pruning (orthorhombic path) is per axis, |d_axis| >= rc => r2 >= rc*rc, which cannot change the result. */
 int oracle_nlist(long N, const double *coords, const int *types, const double *box, double rc, int T,
                  const int *sel, long ncenters, const long *centers, int *nlist_out, double *dvec_out,
                  long *ntrunc_out) {
-    if (box[1] != 0 || box[2] != 0 || box[3] != 0 || box[5] != 0 || box[6] != 0 || box[7] != 0) return -2;
+    const int ortho = !(box[1] != 0 || box[2] != 0 || box[3] != 0 || box[5] != 0 || box[6] != 0 || box[7] != 0);
     const double L[3] = {box[0], box[4], box[8]};
-    if (!(L[0] > 0 && L[1] > 0 && L[2] > 0) || !(rc * rc < 128.0) || T < 1 || T > 16 || N > 16777216) return -1;
+    if (!(rc * rc < 128.0) || T < 1 || T > 16 || N > 16777216) return -1;
+    if (ortho && !(L[0] > 0 && L[1] > 0 && L[2] > 0)) return -1;
     int Nm = 0;
     int off[17];
     for (int b = 0; b < T; ++b) { off[b] = Nm; Nm += sel[b]; }
     off[T] = Nm;
     int nimg[3];
-    for (int a = 0; a < 3; ++a) nimg[a] = (int)ceil(rc / L[a]);
     double *xw = (double *)malloc(sizeof(double) * 3 * (size_t)N);
-    for (long i = 0; i < N; ++i)
-        for (int a = 0; a < 3; ++a) xw[3 * i + a] = oracle_wrap(coords[3 * i + a], L[a]);
+    if (ortho) {
+        for (int a = 0; a < 3; ++a) nimg[a] = (int)ceil(rc / L[a]);
+        for (long i = 0; i < N; ++i)
+            for (int a = 0; a < 3; ++a) xw[3 * i + a] = oracle_wrap(coords[3 * i + a], L[a]);
+    } else {
+        double Hi[9], vol;
+        box_inverse(box, Hi, &vol);
+        if (!(vol > 0)) { free(xw); return -2; }
+        for (int k = 0; k < 3; ++k) {       /* h_k = V / |e_{k+1} x e_{k+2}| = 1 / |column k of Hinv| */
+            const double h = 1.0 / sqrt(Hi[k] * Hi[k] + Hi[3 + k] * Hi[3 + k] + Hi[6 + k] * Hi[6 + k]);
+            nimg[k] = (int)ceil(rc / h);
+        }
+        for (long i = 0; i < N; ++i) oracle_wrap_triclinic(box, coords + 3 * i, xw + 3 * i);
+    }
     const double rc2 = rc * rc;
     long ntrunc = 0;
 #pragma omp parallel for schedule(dynamic, 4) reduction(+ : ntrunc)
@@ -195,14 +231,30 @@ int oracle_nlist(long N, const double *coords, const int *types, const double *b
         nb_t *nb = (nb_t *)malloc(cap * sizeof(nb_t));
         for (long j = 0; j < N; ++j) {
             for (int sx = -nimg[0]; sx <= nimg[0]; ++sx) {
-                double dx = (xw[3 * j + 0] - xw[3 * i + 0]) + (double)sx * L[0];
-                if (fabs(dx) >= rc) continue;
+                double dx = 0.0;
+                if (ortho) {
+                    dx = (xw[3 * j + 0] - xw[3 * i + 0]) + (double)sx * L[0];
+                    if (fabs(dx) >= rc) continue;
+                }
                 for (int sy = -nimg[1]; sy <= nimg[1]; ++sy) {
-                    double dy = (xw[3 * j + 1] - xw[3 * i + 1]) + (double)sy * L[1];
-                    if (fabs(dy) >= rc) continue;
+                    double dy = 0.0;
+                    if (ortho) {
+                        dy = (xw[3 * j + 1] - xw[3 * i + 1]) + (double)sy * L[1];
+                        if (fabs(dy) >= rc) continue;
+                    }
                     for (int sz = -nimg[2]; sz <= nimg[2]; ++sz) {
                         if (j == i && sx == 0 && sy == 0 && sz == 0) continue;
-                        double dz = (xw[3 * j + 2] - xw[3 * i + 2]) + (double)sz * L[2];
+                        double dz;
+                        if (ortho) {
+                            dz = (xw[3 * j + 2] - xw[3 * i + 2]) + (double)sz * L[2];
+                        } else {
+                            double v[3];
+                            for (int c = 0; c < 3; ++c)
+                                v[c] = fma((double)sz, box[6 + c], fma((double)sy, box[3 + c], (double)sx * box[c]));
+                            dx = (xw[3 * j + 0] - xw[3 * i + 0]) + v[0];
+                            dy = (xw[3 * j + 1] - xw[3 * i + 1]) + v[1];
+                            dz = (xw[3 * j + 2] - xw[3 * i + 2]) + v[2];
+                        }
                         double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
                         if (!(r2 < rc2)) continue;
                         if (n == cap) { cap *= 2; nb = (nb_t *)realloc(nb, cap * sizeof(nb_t)); }

@@ -38,6 +38,8 @@ def lib():
         L.oracle_key.argtypes = [C.c_int, C.c_double, C.c_int]
         L.oracle_wrap.restype = C.c_double
         L.oracle_wrap.argtypes = [C.c_double, C.c_double]
+        L.oracle_wrap_triclinic.restype = None
+        L.oracle_wrap_triclinic.argtypes = [dp, dp, dp]
         L.oracle_switch.restype = C.c_double
         L.oracle_switch.argtypes = [C.c_double, C.c_double, C.c_double, dp]
         L.oracle_env_row.restype = None
@@ -79,6 +81,14 @@ def key(type_j: int, r2: float, j: int) -> int:
 
 def wrap(x: float, L: float) -> float:
     return float(lib().oracle_wrap(x, L))
+
+
+def wrap_triclinic(box, x) -> np.ndarray:
+    box = np.ascontiguousarray(box, dtype=np.float64).reshape(9)
+    x = np.ascontiguousarray(x, dtype=np.float64).reshape(3)
+    out = np.zeros(3)
+    lib().oracle_wrap_triclinic(_d(box), _d(x), _d(out))
+    return out
 
 
 def switch(r: float, rc_smth: float, rc: float):
