@@ -39,8 +39,9 @@ typedef enum { DP_FP64 = 0, DP_MIX32 = 1, DP_MIX16 = 2 } dp_precision;
 typedef enum {
     DP_OK = 0,
     DP_EINVAL = -1,   /* null pointer, natoms <= 0 or > 2^24, natoms * max(sel) >= 2^31, rc_smth >= rc, rc*rc >= 128, sel <= 0 */
-    DP_EBOX = -2,     /* box not orthorhombic, or a box length < 2*rc                                        */
-    DP_ENOMEM = -3,   /* workspace_bytes < dp_workspace_bytes(model, natoms)                                  */
+    DP_EBOX = -2,     /* degenerate box: zero volume, or so small that more than 7 images per axis lie inside rc   */
+    DP_ENOMEM = -3,   /* workspace_bytes < dp_workspace_bytes(model, natoms, box); or (dp_status) more periodic
+                         images than the extended atom arrays hold (strongly non-uniform density in a small cell)   */
     DP_ETYPE = -4,    /* an atom type outside type_map (detected on device, reported by dp_status)            */
     DP_ECUDA = -5,    /* CUDA runtime error, no device, or the current device is not the one the model was created on */
     DP_ENEIGH = -6,   /* an atom has more candidates inside rc than the sort buffer holds (dp_status)         */
@@ -54,7 +55,7 @@ typedef enum {
  * Layer rule (Fig. 1(e),(f)): out == 2*in -> y = (x,x) + tanh(xW+b); out == in -> y = x + tanh(xW+b);
  * otherwise y = tanh(xW+b).  The last fitting layer is linear. */
 typedef struct {
-    int ntypes;              /* T, 1..4                                                                    */
+    int ntypes;              /* T, 1..16 (the type field of the sort key has 4 bits)          */
     int embed_widths[3];     /* (m0, m1, m2); this build supports (25, 50, 100) only                       */
     int axis;                /* M2 (16): D = A^T A[:, :M2]                                                   */
     int fit_widths[3];       /* (240, 240, 240)                                                             */
@@ -72,12 +73,16 @@ typedef struct {
 int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_type_map, double rc,
               double rc_smth, const int *sel, dp_precision prec);
 
-/* Bytes of device workspace dp_compute needs for up to natoms atoms (0 on invalid arguments). */
-size_t dp_workspace_bytes(const dp_model *m, long natoms);
+/* Bytes of device workspace dp_compute needs for natoms atoms in the box box_host[9] (0 on invalid arguments).
+ * box_host == NULL: any orthorhombic box with every length >= 2 rc (the minimum-image path).  A general (triclinic) cell or
+ * an edge shorter than 2 rc makes the periodic images explicit ghost atoms (Fig. 1(a)) and needs room for them:
+ * pass the box. */
+size_t dp_workspace_bytes(const dp_model *m, long natoms, const double *box_host);
 
 /* One evaluation.  coords_dev [natoms][3] fp64 (may lie outside the box; wrapped canonically),
- * types_dev [natoms] int32 USER types, box_host[9] row-major rows a,b,c (orthorhombic, lengths >= 2 rc),
- * workspace_dev: >= dp_workspace_bytes, 256-byte aligned, contents undefined on entry and exit,
+ * types_dev [natoms] int32 USER types, box_host[9] row-major rows a,b,c: any non-degenerate cell (orthorhombic boxes with
+ * every length >= 2 rc use the minimum image; general cells and shorter edges use explicit ghost images),
+ * workspace_dev: >= dp_workspace_bytes(m, natoms, box_host), 256-byte aligned, contents undefined on entry and exit,
  * cuda_stream: a cudaStream_t (NULL = default stream).
  * Outputs (device, fp64): energy_dev[1]; atom_energy_dev[natoms] or NULL; forces_dev[natoms][3];
  * virial_dev[9] row-major, Xi_ab = -sum d_a (dE/dd_b) = -dE/d(strain_ab), or NULL.
@@ -126,7 +131,8 @@ int dp_profile_read(dp_model *m, double *ms_host);
  *   candidates exactly, re-sorts and truncates, so the formatted list is the same as without the buffer as long as no atom
  *   moved more than skin/2 since the last search (checked on the device: DP_ESKIN from dp_status).  skin = 0 or
  *   rebuild_every <= 1: every evaluation searches the cells.
- *   workspace_dev: >= dp_md_workspace_bytes(m, natoms, skin) bytes (skin = 0 if not buffered), 256-byte aligned;
+ *   workspace_dev: >= dp_md_workspace_bytes(m, natoms, skin, box_host) bytes (skin = 0 if not buffered), 256-byte aligned;
+ *   (the buffered list needs the minimum-image path: in a general cell or with an edge < 2 rc every evaluation searches);
  *   forces_dev [natoms][3]: forces at the final coordinates;  thermo_dev [nsteps + 1][DP_MD_NTHERMO] fp64, one record per
  *   evaluation 0 .. nsteps ("kinetic energy, potential energy, temperature, pressure, are collected"):
  *   [0] potential energy E (eV), [1] kinetic energy sum 1/2 m v^2 (eV), [2] temperature 2 KE / ((3 natoms - 3) kB) (K),
@@ -135,7 +141,7 @@ int dp_profile_read(dp_model *m, double *ms_host);
  *   conditions of the WHOLE run (the flags of all nsteps + 1 evaluations are OR-ed: DP_ETYPE, DP_ENEIGH, DP_ESKIN) and the
  *   truncation count of the last evaluation.  Errors as dp_compute; DP_EINVAL for bad masses, dt_fs, skin < 0, nsteps < 0 or
  *   rebuild_every < 0. */
-size_t dp_md_workspace_bytes(const dp_model *m, long natoms, double skin);
+size_t dp_md_workspace_bytes(const dp_model *m, long natoms, double skin, const double *box_host);
 int dp_md_run(dp_model *m, long natoms, double *coords_dev, double *vel_dev, const int *types_dev,
               const double *mass_host, int n_mass, const double *box_host, double dt_fs, int nsteps,
               double skin, int rebuild_every, void *workspace_dev, size_t workspace_bytes, void *cuda_stream,

@@ -49,7 +49,7 @@ def lib():
         L.dp_create.argtypes = [C.POINTER(vp), C.POINTER(_Weights), C.POINTER(C.c_int), C.c_int, C.c_double,
                                 C.c_double, C.POINTER(C.c_int), C.c_int]
         L.dp_workspace_bytes.restype = C.c_size_t
-        L.dp_workspace_bytes.argtypes = [vp, C.c_long]
+        L.dp_workspace_bytes.argtypes = [vp, C.c_long, dp]
         L.dp_compute.restype = C.c_int
         L.dp_compute.argtypes = [vp, C.c_long, vp, vp, dp, vp, C.c_size_t, vp, vp, vp, vp, vp]
         L.dp_get_nlist.restype = C.c_int
@@ -68,7 +68,7 @@ def lib():
         L.dp_md_run.argtypes = [vp, C.c_long, vp, vp, vp, dp, C.c_int, dp, C.c_double, C.c_int, C.c_double, C.c_int, vp,
                                 C.c_size_t, vp, vp, vp, vp]
         L.dp_md_workspace_bytes.restype = C.c_size_t
-        L.dp_md_workspace_bytes.argtypes = [vp, C.c_long, C.c_double]
+        L.dp_md_workspace_bytes.argtypes = [vp, C.c_long, C.c_double, dp]
         L.dp_measure_peaks.restype = C.c_int
         L.dp_measure_peaks.argtypes = [dp, C.c_int, vp]
         L.dp_destroy.restype = None
@@ -108,17 +108,20 @@ class DPModel:
         self._ws = None
         self._n = 0
 
-    def workspace_bytes(self, natoms: int) -> int:
-        return int(lib().dp_workspace_bytes(self._h, natoms))
+    def workspace_bytes(self, natoms: int, box=None) -> int:
+        if box is None:
+            return int(lib().dp_workspace_bytes(self._h, natoms, None))
+        boxh = np.ascontiguousarray(np.asarray(box, dtype=np.float64).reshape(9))
+        return int(lib().dp_workspace_bytes(self._h, natoms, _dptr(boxh)))
 
     def launches_per_compute(self) -> int:
         return int(lib().dp_launches_per_compute(self._h))
 
-    def _workspace(self, natoms: int, device):
+    def _workspace(self, natoms: int, device, box=None):
         import torch
-        need = self.workspace_bytes(natoms)
+        need = self.workspace_bytes(natoms, box)
         if need == 0:
-            raise DPError(-1, "dp_workspace_bytes")
+            raise DPError(-2 if self.workspace_bytes(natoms) else -1, "dp_workspace_bytes")
         if self._ws is None or self._ws.numel() < need or self._ws.device != device:
             self._ws = torch.empty(need, dtype=torch.uint8, device=device)
         return self._ws
@@ -130,7 +133,7 @@ class DPModel:
         assert coords.is_contiguous() and types.is_contiguous()
         n = int(coords.shape[0])
         dev = coords.device
-        ws = self._workspace(n, dev)
+        ws = self._workspace(n, dev, box)
         if out is None:
             out = dict(energy=torch.empty(1, dtype=torch.float64, device=dev),
                        atom_energy=torch.empty(n, dtype=torch.float64, device=dev),
@@ -159,7 +162,8 @@ class DPModel:
         n = int(coords.shape[0])
         dev = coords.device
         buffered = skin > 0.0 and rebuild_every > 1
-        need = int(lib().dp_md_workspace_bytes(self._h, n, float(skin) if buffered else 0.0))
+        boxh = np.ascontiguousarray(np.asarray(box, dtype=np.float64).reshape(9))
+        need = int(lib().dp_md_workspace_bytes(self._h, n, float(skin) if buffered else 0.0, _dptr(boxh)))
         if need == 0:
             raise DPError(-1, "dp_md_workspace_bytes")
         if self._ws is None or self._ws.numel() < need or self._ws.device != dev:

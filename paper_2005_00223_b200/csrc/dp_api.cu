@@ -17,23 +17,33 @@ inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 long ncell_max_for(long N) { return N < 512 ? 512 : N; }
 
-WsLayout ws_layout(const dp_model *m, long N) {
+// NE: capacity of the arrays that a neighbour index can address (NE = N without ghosts, Grid3::cap_ext in ghost mode)
+WsLayout ws_layout(const dp_model *m, long N, long NE) {
     WsLayout L{};
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t r = o; o = align256(o + bytes); return r; };
-    const size_t nbins = (size_t)m->T * (size_t)ncell_max_for(N);
+    const bool ghost = NE > N;
+    const size_t nbins = (ghost ? 2 : 1) * (size_t)m->T * (size_t)ncell_max_for(N);
     L.status = take(64);
     L.bin_count = take(sizeof(int) * (nbins + 1));
     L.bin_start = take(sizeof(int) * (nbins + 1));
     L.bin_cursor = take(sizeof(int) * nbins);
-    L.atom_bin = take(sizeof(int) * (size_t)N);
-    L.tmp_order = take(sizeof(int) * (size_t)N);
-    L.perm = take(sizeof(int) * (size_t)N);
+    L.atom_bin = take(sizeof(int) * (size_t)NE);
+    L.tmp_order = take(sizeof(int) * (size_t)NE);
+    L.perm = take(sizeof(int) * (size_t)NE);
     L.inv = take(sizeof(int) * (size_t)N);
-    L.xs = take(sizeof(double) * 3 * (size_t)N);
+    L.xs = take(sizeof(double) * 3 * (size_t)NE);
     L.xsf = take(sizeof(float) * 4 * (size_t)N);
     L.scan_tmp = take(sizeof(int) * 2 * ((nbins > (size_t)N ? nbins : (size_t)N) / 4096 + 4));
-    L.xw = take(sizeof(double) * 3 * (size_t)N);
+    L.xw = take(sizeof(double) * 3 * (size_t)NE);
+    if (ghost) {
+        L.ext_owner = take(sizeof(int) * (size_t)NE);
+        L.ext_code = take(sizeof(int) * (size_t)NE);
+        L.ext_base = take(sizeof(int) * (size_t)NE);
+        L.ext_scode = take(sizeof(int) * (size_t)NE);
+        L.gcnt = take(sizeof(int) * (size_t)N);
+        L.gstart = take(sizeof(int) * ((size_t)N + 1));
+    }
     L.nlist = take(sizeof(int) * (size_t)N * m->Nm);
     L.nreal = take(sizeof(int) * (size_t)N * m->T);
     if (m->prec != DP_FP64) {
@@ -53,7 +63,7 @@ WsLayout ws_layout(const dp_model *m, long N) {
     L.fit_act = take(esz * (size_t)N * 240 * 7 + (m->prec == DP_MIX16 ? ((size_t)m->T + 1) * FIT_GZ_TILE_BYTES : 0));
     L.gD = take(esz * (size_t)N * M2E * 16);
     L.eatom = take(sizeof(double) * (size_t)N);
-    L.fsorted = take(sizeof(double) * 3 * (size_t)N);
+    L.fsorted = take(sizeof(double) * 3 * (size_t)NE);
     L.virial = take(sizeof(double) * 16);
     L.total = o;
     return L;
@@ -65,17 +75,69 @@ bool rows_fit_int32(const dp_model *m, long N) {
     return true;
 }
 
+// Cell grid of one evaluation.  Orthorhombic boxes with every length >= 2 rc take the minimum-image path (nlist.cu);
+// everything else (a general cell, or an edge shorter than 2 rc) takes the ghost path (ghost.cu).  false: degenerate box.
 bool make_grid(const dp_model *m, long N, const double *box, Grid3 *g) {
-    if (box[1] != 0 || box[2] != 0 || box[3] != 0 || box[5] != 0 || box[6] != 0 || box[7] != 0) return false;
+    *g = Grid3{};
+    const bool ortho = !(box[1] != 0 || box[2] != 0 || box[3] != 0 || box[5] != 0 || box[6] != 0 || box[7] != 0);
     const double Ls[3] = {box[0], box[4], box[8]};
     const long cap = ncell_max_for(N);
+    bool small = false;
+    if (ortho)
+        for (int a = 0; a < 3; ++a) {
+            if (!(Ls[a] > 0.0)) return false;
+            if (!(Ls[a] >= 2.0 * m->rc)) small = true;
+        }
+    if (!ortho || small) {
+        // ---- ghost mode.  Inverse by cofactors, one expression per entry: the same expressions as the oracle (reading N2t)
+        const double *H = box;
+        double *Hi = g->Hinv;
+        const double c00 = H[4] * H[8] - H[5] * H[7], c01 = H[5] * H[6] - H[3] * H[8], c02 = H[3] * H[7] - H[4] * H[6];
+        const double det = H[0] * c00 + H[1] * c01 + H[2] * c02;
+        if (!(std::fabs(det) > 0.0) || !std::isfinite(det)) return false;
+        Hi[0] = c00 / det; Hi[1] = (H[2] * H[7] - H[1] * H[8]) / det; Hi[2] = (H[1] * H[5] - H[2] * H[4]) / det;
+        Hi[3] = c01 / det; Hi[4] = (H[0] * H[8] - H[2] * H[6]) / det; Hi[5] = (H[2] * H[3] - H[0] * H[5]) / det;
+        Hi[6] = c02 / det; Hi[7] = (H[1] * H[6] - H[0] * H[7]) / det; Hi[8] = (H[0] * H[4] - H[1] * H[3]) / det;
+        g->ghost = 1; g->ortho = ortho ? 1 : 0; g->reach = 1;
+        double images = 1.0, ratio = 1.0;
+        for (int k = 0; k < 3; ++k) {
+            // h_k: height of the cell perpendicular to the other two edges (= L_k for a diagonal box)
+            const double h = ortho ? Ls[k] : 1.0 / std::sqrt(Hi[k] * Hi[k] + Hi[3 + k] * Hi[3 + k] + Hi[6 + k] * Hi[6 + k]);
+            const int ni = (int)std::ceil(m->rc / h);
+            if (ni > 7) return false;                       // image shifts are packed in 4 bits
+            g->nimg[k] = ni;
+            const double mk = m->rc / h * (1.0 + 1e-9) + 1e-12;     // slab width in fractional units, with margin
+            g->flo[k] = -mk;
+            g->nc[k] = (int)std::floor((1.0 + 2.0 * mk) / mk);     // cells of fractional width >= mk: neighbours within +-1 cell
+            if (g->nc[k] < 1) g->nc[k] = 1;
+            images *= 2.0 * ni + 1.0;
+            ratio *= 1.0 + 2.0 * mk;
+            g->L[k] = 1e300;                                 // downstream kernels: no minimum-image step
+            g->inv_cw[k] = 0.0;
+        }
+        for (int k = 0; k < 9; ++k) g->H[k] = box[k];
+        while ((long)g->nc[0] * g->nc[1] * g->nc[2] > cap) {
+            int big = 0;
+            for (int a = 1; a < 3; ++a) if (g->nc[a] > g->nc[big]) big = a;
+            g->nc[big] -= 1;
+        }
+        for (int k = 0; k < 3; ++k) g->fcw[k] = (double)g->nc[k] / (1.0 - 2.0 * g->flo[k]);
+        g->ncell = g->nc[0] * g->nc[1] * g->nc[2];
+        // capacity of the extended arrays: never more than every image of every atom; twice the uniform-density expectation
+        // otherwise (an overflow is detected on the device and reported as DP_ENOMEM by dp_status)
+        const double all = (double)N * images, est = 2.0 * (double)N * ratio + 1024.0;
+        const double ce = all < est ? all : est;
+        if (ce > 16777216.0) return false;
+        g->cap_ext = (long)ce > N ? (long)ce : N + 1;
+        return true;
+    }
     // half-width cells (edge >= rc/2, 5 x 5 x 5 neighbourhood: 58 % of the candidates of the 3 x 3 x 3 search) when the grid
     // then has at least 5 cells per axis and fits the bin arrays; else cells of edge >= rc
     // the MD loop's buffered list searches rc + skin (every call of one dp_md_run uses the same grid)
     const double rl = m->rc + (m->list_mode ? m->md_skin : 0.0);
     g->reach = 2;
+    g->cap_ext = N;
     for (int a = 0; a < 3; ++a) {
-        if (!(Ls[a] >= 2.0 * m->rc)) return false;
         g->L[a] = Ls[a];
         g->nc[a] = (int)std::floor(Ls[a] / (0.5 * rl * (1.0 + 1e-9)));
         if (g->nc[a] < 5) g->reach = 1;
@@ -306,7 +368,7 @@ const char *dp_strerror(int code) {
     switch (code) {
         case DP_OK: return "ok";
         case DP_EINVAL: return "invalid argument";
-        case DP_EBOX: return "box must be orthorhombic with every length >= 2*rc";
+        case DP_EBOX: return "degenerate box (zero volume, or more than 7 periodic images per axis inside rc)";
         case DP_ENOMEM: return "workspace too small";
         case DP_ETYPE: return "atom type outside type_map";
         case DP_ECUDA: return "CUDA error or no device";
@@ -428,9 +490,12 @@ void dp_destroy(dp_model *m) {
     delete m;
 }
 
-size_t dp_workspace_bytes(const dp_model *m, long natoms) {
+size_t dp_workspace_bytes(const dp_model *m, long natoms, const double *box_host) {
     if (!m || natoms <= 0 || natoms > 16777216 || !rows_fit_int32(m, natoms)) return 0;
-    return ws_layout(m, natoms).total;
+    if (!box_host) return ws_layout(m, natoms, natoms).total;
+    Grid3 g;
+    if (!make_grid(m, natoms, box_host, &g)) return 0;
+    return ws_layout(m, natoms, g.cap_ext).total;
 }
 
 int dp_launches_per_compute(const dp_model *m) {
@@ -459,7 +524,8 @@ int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *ty
     if (cudaGetDevice(&dev) != cudaSuccess || dev != m->device) return DP_ECUDA;    // weights live on the device of dp_create
     Grid3 g;
     if (!make_grid(m, natoms, box_host, &g)) return DP_EBOX;
-    const WsLayout L = ws_layout(m, natoms);
+    if (g.ghost && m->list_mode) return DP_EUNSUPPORTED;        // the buffered list of dp_md_run needs the minimum-image path
+    const WsLayout L = ws_layout(m, natoms, g.cap_ext);
     if (workspace_bytes < L.total) return DP_ENOMEM;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     char *ws = (char *)workspace_dev;
@@ -468,14 +534,19 @@ int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *ty
     // status word 0 = error flags: cleared per call, except inside one dp_md_run, where they accumulate (dp_status then
     // reports the whole run); the counters behind it are per evaluation
     ok(m->keep_flags ? cudaMemsetAsync(ws + L.status + 4, 0, 60, st) : cudaMemsetAsync(ws + L.status, 0, 64, st));
-    ok(cudaMemsetAsync(ws + L.fsorted, 0, sizeof(double) * 3 * (size_t)natoms, st));
+    ok(cudaMemsetAsync(ws + L.fsorted, 0, sizeof(double) * 3 * (size_t)g.cap_ext, st));
     ok(cudaMemsetAsync(ws + L.virial, 0, sizeof(double) * 16, st));
     ok(cudaMemsetAsync(energy_dev, 0, sizeof(double), st));
     auto mark = [&](int k) { if (m->profile) ok(cudaEventRecord(m->ev[k], st)); };
     mark(0);
-    ok(m->list_mode == 2 ? launch_regather(m, natoms, coords_dev, g, ws, L, st)
-                         : launch_build_cells(m, natoms, coords_dev, types_dev, g, ws, L, st));
-    ok(launch_nlist(m, natoms, g, ws, L, st));
+    if (g.ghost) {
+        ok(launch_build_ghost(m, natoms, coords_dev, types_dev, g, ws, L, st));
+        ok(launch_nlist_ghost(m, natoms, g, ws, L, st));
+    } else {
+        ok(m->list_mode == 2 ? launch_regather(m, natoms, coords_dev, g, ws, L, st)
+                             : launch_build_cells(m, natoms, coords_dev, types_dev, g, ws, L, st));
+        ok(launch_nlist(m, natoms, g, ws, L, st));
+    }
     mark(1);
     const bool f64 = m->prec == DP_FP64;
     const bool m16 = m->prec == DP_MIX16;
@@ -486,10 +557,11 @@ int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *ty
     mark(3);
     ok(f64 ? launch_embed_bwd_f64(m, natoms, g, ws, L, st)
            : (m16 ? launch_embed_bwd_tc2(m, natoms, g, ws, L, st) : launch_embed_bwd_mix(m, natoms, g, ws, L, st)));
+    if (g.ghost) ok(launch_fold_ghost(m, natoms, g, ws, L, st));
     mark(4);
     ok(launch_finalize(m, natoms, ws, L, energy_dev, atom_energy_dev, forces_dev, virial_dev, st));
     mark(5);
-    m->last_natoms = natoms; m->last_ws = workspace_dev; m->last_stream = st;
+    m->last_natoms = natoms; m->last_next = g.cap_ext; m->last_ws = workspace_dev; m->last_stream = st;
     return e == cudaSuccess ? DP_OK : DP_ECUDA;
 }
 
@@ -522,7 +594,7 @@ int dp_profile_read(dp_model *m, double *ms_host) {
 
 int dp_get_nlist(dp_model *m, int *nlist_dev, void *cuda_stream) {
     if (!m || !nlist_dev || !m->last_ws) return DP_EINVAL;
-    const WsLayout L = ws_layout(m, m->last_natoms);
+    const WsLayout L = ws_layout(m, m->last_natoms, m->last_next);
     cudaError_t e = launch_get_nlist(m, m->last_natoms, (char *)m->last_ws, L, nlist_dev, (cudaStream_t)cuda_stream);
     return e == cudaSuccess ? DP_OK : DP_ECUDA;
 }
@@ -531,10 +603,11 @@ int dp_status(dp_model *m, long *n_truncated_atoms) {
     if (!m || !m->last_ws) return DP_EINVAL;
     if (cudaStreamSynchronize(m->last_stream) != cudaSuccess) return DP_ECUDA;
     int st[2] = {0, 0};
-    const WsLayout L = ws_layout(m, m->last_natoms);
+    const WsLayout L = ws_layout(m, m->last_natoms, m->last_next);
     if (cudaMemcpy(st, (char *)m->last_ws + L.status, sizeof(st), cudaMemcpyDeviceToHost) != cudaSuccess) return DP_ECUDA;
     if (n_truncated_atoms) *n_truncated_atoms = st[1];
     if (st[0] & 1) return DP_ETYPE;
+    if (st[0] & 8) return DP_ENOMEM;         // ghost mode: more periodic images than the extended arrays hold
     if (st[0] & 2) return DP_ENEIGH;
     if (st[0] & 4) return DP_ESKIN;
     return DP_OK;
@@ -544,7 +617,7 @@ int dp_last_row_counts(dp_model *m, long *rows_forward, long *rows_backward) {
     if (!m || !m->last_ws) return DP_EINVAL;
     if (cudaStreamSynchronize(m->last_stream) != cudaSuccess) return DP_ECUDA;
     unsigned long long c[2] = {0, 0};
-    const WsLayout L = ws_layout(m, m->last_natoms);
+    const WsLayout L = ws_layout(m, m->last_natoms, m->last_next);
     if (cudaMemcpy(c, (char *)m->last_ws + L.status + 8, sizeof(c), cudaMemcpyDeviceToHost) != cudaSuccess) return DP_ECUDA;
     if (rows_forward) *rows_forward = (long)c[0];
     if (rows_backward) *rows_backward = (long)c[1];

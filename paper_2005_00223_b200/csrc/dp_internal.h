@@ -20,7 +20,7 @@
         }                                                                                                               \
     } while (0)
 
-#define DP_MAX_TYPES 4
+#define DP_MAX_TYPES 16
 #define DP_NEVENTS 8
 #define DP_WARPS_PER_CTA 8
 
@@ -77,6 +77,7 @@ struct dp_model {
     int num_sms;
     // state of the last compute
     long last_natoms;
+    long last_next;                 // capacity of the extended atom arrays of the last compute (= last_natoms without ghosts)
     void *last_ws;
     cudaStream_t last_stream;
     int sort_cap;
@@ -120,17 +121,51 @@ struct WsLayout {
     size_t eatom;       // double[N] sorted order
     size_t fsorted;     // double[N][3] sorted order
     size_t virial;      // double[9] + energy accumulators
+    // ghost mode: extended atom arrays (the per-atom arrays above that are indexed by a neighbour are sized cap_ext)
+    size_t ext_owner;   // int[cap_ext] user index of the owner of unsorted item u (u < N: the atom itself)
+    size_t ext_code;    // int[cap_ext] packed image shift of unsorted item u
+    size_t ext_base;    // int[cap_ext] sorted index of the owner of sorted item e
+    size_t ext_scode;   // int[cap_ext] packed image shift of sorted item e
+    size_t gcnt;        // int[N] ghosts per atom
+    size_t gstart;      // int[N+1]
 };
+
+// neighbour capacities per type and their prefix sums, passed to kernels by value (a __grid_constant__ parameter: indexed
+// dynamically straight from constant memory)
+struct TypeTab {
+    int sel[DP_MAX_TYPES];
+    int off[DP_MAX_TYPES + 1];
+};
+inline TypeTab make_typetab(const dp_model *m) {
+    TypeTab t{};
+    for (int b = 0; b < DP_MAX_TYPES; ++b) { t.sel[b] = b < m->T ? m->sel[b] : 0; t.off[b] = b <= m->T ? m->off[b] : m->off[m->T]; }
+    t.off[DP_MAX_TYPES] = m->off[m->T];
+    return t;
+}
 
 struct Grid3 {
     int nc[3];          // cells per axis
-    double L[3];
+    double L[3];        // box lengths (ghost mode: 1e300, which switches the minimum image off in every kernel)
     double inv_cw[3];   // nc / L
     int ncell;
     int reach;          // neighbour cells searched per direction: 1 (cell edge >= rc) or 2 (cell edge >= rc/2)
+    // ---- ghost mode (ghost.cu): general cell or a cell edge shorter than 2 rc; periodic images are explicit ghost atoms
+    int ghost;          // 0: orthorhombic box with every length >= 2 rc (minimum image, nlist.cu)
+    int ortho;          // ghost mode: the box is diagonal (reading N2: per-axis wrap and shift) or general (reading N2t)
+    double H[9];        // box rows a, b, c
+    double Hinv[9];     // x = f H, f = x Hinv
+    int nimg[3];        // images per axis: ceil(rc / h_k)
+    double flo[3];      // fractional coordinate of the low edge of the extended region: -(rc / h_k) (1 + 1e-9)
+    double fcw[3];      // cells per unit fractional length
+    long cap_ext;       // capacity of the extended (local + ghost) atom arrays
 };
 
 // launchers (each returns cudaGetLastError())
+void dp_launch_scan(int n, const int *cnt, int *start, int *tmp, cudaStream_t st);
+cudaError_t launch_build_ghost(const dp_model *m, long N, const double *coords, const int *types, const Grid3 &g, char *ws,
+                               const WsLayout &L, cudaStream_t st);
+cudaError_t launch_nlist_ghost(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+cudaError_t launch_fold_ghost(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_build_cells(const dp_model *m, long N, const double *coords, const int *types, const Grid3 &g,
                                char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_regather(const dp_model *m, long N, const double *coords, const Grid3 &g, char *ws, const WsLayout &L,

@@ -127,7 +127,7 @@ constexpr int WARP_BUF_DOUBLES = ROWCHUNK * 5;   // rbuf[ROWCHUNK][4] + sbuf[ROW
 
 // ------------------------------------------------------------------------------------------------ forward
 __global__ void __launch_bounds__(DP_WARPS_PER_CTA * 32, 1)
-k_embed_fwd_f64(int T, int ncell, int Nm, int4 sel4, EnvParams ep, const EmbedNetFrag<double> *__restrict__ nets,
+k_embed_fwd_f64(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, EnvParams ep, const EmbedNetFrag<double> *__restrict__ nets,
                 const double *__restrict__ avg, const double *__restrict__ stdv, const int *__restrict__ bin_start,
                 const double *__restrict__ xs, const int *__restrict__ nlist, const int *__restrict__ nreal,
                 double *__restrict__ Aout, unsigned long long *__restrict__ row_counter) {
@@ -136,7 +136,7 @@ k_embed_fwd_f64(int T, int ncell, int Nm, int4 sel4, EnvParams ep, const EmbedNe
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     double *rbuf = smem + FWD_NET_DOUBLES + wid * WARP_BUF_DOUBLES;
     double *sbuf = rbuf + ROWCHUNK * 4;
-    const int sel[4] = {sel4.x, sel4.y, sel4.z, sel4.w};
+    const int *sel = tt.sel;
     const int gw = blockIdx.x * DP_WARPS_PER_CTA + wid, W = gridDim.x * DP_WARPS_PER_CTA;
     const int r = lane & 3, q4 = lane >> 2;
     const double inv_nm = 1.0 / (double)Nm;
@@ -235,7 +235,7 @@ k_embed_fwd_f64(int T, int ncell, int Nm, int4 sel4, EnvParams ep, const EmbedNe
 //   [0..14)  : dG MMA   B fragment of tile nt3: lane -> gA[c = lane%4][feature3(nt3, (lane/4)/2, (lane/4)%2)]
 //   [14..42) : dR^ MMA  B fragment of chunk kc = 2*nt3 + j3: lane -> (lane/4 < 4) ? gA[c = lane/4][feature3(nt3, lane%4, j3)] : 0
 __global__ void __launch_bounds__(DP_WARPS_PER_CTA * 32, 1)
-k_embed_bwd_f64(int T, int ncell, int Nm, int4 sel4, EnvParams ep, const EmbedNetFrag<double> *__restrict__ nets,
+k_embed_bwd_f64(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, EnvParams ep, const EmbedNetFrag<double> *__restrict__ nets,
                 const double *__restrict__ avg, const double *__restrict__ stdv, const int *__restrict__ bin_start,
                 const double *__restrict__ xs, const int *__restrict__ nlist, const int *__restrict__ nreal,
                 const double *__restrict__ gAf, double *__restrict__ fsorted, double *__restrict__ virial,
@@ -245,7 +245,7 @@ k_embed_bwd_f64(int T, int ncell, int Nm, int4 sel4, EnvParams ep, const EmbedNe
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     double *rbuf = smem + BWD_NET_DOUBLES + wid * WARP_BUF_DOUBLES;
     double *sbuf = rbuf + ROWCHUNK * 4;
-    const int sel[4] = {sel4.x, sel4.y, sel4.z, sel4.w};
+    const int *sel = tt.sel;
     const int gw = blockIdx.x * DP_WARPS_PER_CTA + wid, W = gridDim.x * DP_WARPS_PER_CTA;
     const int r = lane & 3, q4 = lane >> 2;
     const double hx = 0.5 * ep.L[0], hy = 0.5 * ep.L[1], hz = 0.5 * ep.L[2];
@@ -414,9 +414,9 @@ static int embed_grid(const dp_model *m, long N) {
 
 cudaError_t launch_embed_fwd_f64(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
     DP_SMEM_OPTIN(k_embed_fwd_f64, embed_smem_bytes_fwd_f64());
-    int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
+    const TypeTab tt = make_typetab(m);
     k_embed_fwd_f64<<<embed_grid(m, N), DP_WARPS_PER_CTA * 32, embed_smem_bytes_fwd_f64(), st>>>(
-        m->T, g.ncell, m->Nm, sel4, make_env(m, g), (const EmbedNetFrag<double> *)m->embed_frag_dev, m->avg_dev,
+        m->T, g.ncell, m->Nm, tt, make_env(m, g), (const EmbedNetFrag<double> *)m->embed_frag_dev, m->avg_dev,
         m->std_dev, (int *)(ws + L.bin_start), (double *)(ws + L.xs), (int *)(ws + L.nlist), (int *)(ws + L.nreal),
         (double *)(ws + L.A), (unsigned long long *)(ws + L.status + 8));
     return cudaGetLastError();
@@ -424,9 +424,9 @@ cudaError_t launch_embed_fwd_f64(const dp_model *m, long N, const Grid3 &g, char
 
 cudaError_t launch_embed_bwd_f64(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
     DP_SMEM_OPTIN(k_embed_bwd_f64, embed_smem_bytes_bwd_f64());
-    int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
+    const TypeTab tt = make_typetab(m);
     k_embed_bwd_f64<<<embed_grid(m, N), DP_WARPS_PER_CTA * 32, embed_smem_bytes_bwd_f64(), st>>>(
-        m->T, g.ncell, m->Nm, sel4, make_env(m, g), (const EmbedNetFrag<double> *)m->embed_frag_dev, m->avg_dev,
+        m->T, g.ncell, m->Nm, tt, make_env(m, g), (const EmbedNetFrag<double> *)m->embed_frag_dev, m->avg_dev,
         m->std_dev, (int *)(ws + L.bin_start), (double *)(ws + L.xs), (int *)(ws + L.nlist), (int *)(ws + L.nreal),
         (double *)(ws + L.gAf), (double *)(ws + L.fsorted), (double *)(ws + L.virial),
         (unsigned long long *)(ws + L.status + 16));

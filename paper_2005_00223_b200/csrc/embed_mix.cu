@@ -151,7 +151,7 @@ constexpr int MIX_WARP_BUF_FLOATS = MIX_ROWCHUNK * 5;    // rbuf[64][4] + sbuf[6
 // all scaled by gscale[i] (a power of two that brings max|gA| near 1); results are multiplied by 1/(Nm*gscale).
 template <int NS, int NSC, bool APPROX, int NSB>
 __global__ void __launch_bounds__(DP_WARPS_PER_CTA * 32, 1)
-k_embed_bwd_mix(int T, int ncell, int Nm, int4 sel4, EnvParams ep, const EmbedNetFragH<ns_wparts(NS)> *__restrict__ nets,
+k_embed_bwd_mix(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, EnvParams ep, const EmbedNetFragH<ns_wparts(NS)> *__restrict__ nets,
                 const double *__restrict__ avg, const double *__restrict__ stdv, const int *__restrict__ bin_start,
                 const double *__restrict__ xs, const int *__restrict__ nlist, const int *__restrict__ nreal,
                 const uint32_t *__restrict__ gAf, const float *__restrict__ gscale, double *__restrict__ fsorted,
@@ -162,7 +162,7 @@ k_embed_bwd_mix(int T, int ncell, int Nm, int4 sel4, EnvParams ep, const EmbedNe
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     float *rbuf = reinterpret_cast<float *>(smem_u) + sizeof(EmbedNetFragH<NSW>) / 4 + wid * MIX_WARP_BUF_FLOATS;
     float *sbuf = rbuf + MIX_ROWCHUNK * 4;
-    const int sel[4] = {sel4.x, sel4.y, sel4.z, sel4.w};
+    const int *sel = tt.sel;
     const int gw = blockIdx.x * DP_WARPS_PER_CTA + wid, W = gridDim.x * DP_WARPS_PER_CTA;
     const int r = lane & 3, g = lane >> 2;
     const double hx = 0.5 * ep.L[0], hy = 0.5 * ep.L[1], hz = 0.5 * ep.L[2];
@@ -378,9 +378,9 @@ int embed_grid(const dp_model *m, long N) {
 template <int NS, int NSC, bool APPROX, int NSB>
 cudaError_t launch_bwd(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
     DP_SMEM_OPTIN((k_embed_bwd_mix<NS, NSC, APPROX, NSB>), smem_bytes<NS>());
-    int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
+    const TypeTab tt = make_typetab(m);
     k_embed_bwd_mix<NS, NSC, APPROX, NSB><<<embed_grid(m, N), DP_WARPS_PER_CTA * 32, smem_bytes<NS>(), st>>>(
-        m->T, g.ncell, m->Nm, sel4, make_env(m, g), (const EmbedNetFragH<ns_wparts(NS)> *)m->embed_frag_dev, m->avg_dev,
+        m->T, g.ncell, m->Nm, tt, make_env(m, g), (const EmbedNetFragH<ns_wparts(NS)> *)m->embed_frag_dev, m->avg_dev,
         m->std_dev, (int *)(ws + L.bin_start), (double *)(ws + L.xs), (int *)(ws + L.nlist), (int *)(ws + L.nreal),
         (const uint32_t *)(ws + L.gAf), (const float *)(ws + L.gscale), (double *)(ws + L.fsorted),
         (double *)(ws + L.virial), (unsigned long long *)(ws + L.status + 16));

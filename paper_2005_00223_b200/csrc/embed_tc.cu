@@ -150,14 +150,14 @@ struct TileMeta {
 //   rh = R^ (fp32, unweighted), id = {sorted atom, neighbour j (sorted index)} for a real row and {sorted atom, -npad}
 //   for the representative of the npad padded slots; rows of atom i start at rowstart[b][i].
 __global__ void __launch_bounds__(256)
-k_env_rows(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, EnvParams ep, const double *__restrict__ avg,
+k_env_rows(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, EnvParams ep, const double *__restrict__ avg,
            const double *__restrict__ stdv, const int *__restrict__ bin_start, const double *__restrict__ xs,
            const int *__restrict__ nlist, const int *__restrict__ nreal, const int *__restrict__ rowstart,
            float4 *__restrict__ rows_rh, int2 *__restrict__ rows_id) {
     const int lane = threadIdx.x & 31;
     const long i = blockIdx.x * 8L + (threadIdx.x >> 5);
     if (i >= N) return;
-    const int sel[4] = {sel4.x, sel4.y, sel4.z, sel4.w}, off[4] = {off4.x, off4.y, off4.z, off4.w};
+    const int *sel = tt.sel, *off = tt.off;
     int a = 0;
     for (int t = 1; t < T; ++t) a += i >= bin_start[t * ncell];
     double av[4], isd[4];
@@ -210,7 +210,7 @@ k_env_rows(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, EnvParams ep,
 
 template <int NS, bool APPROX>
 __global__ void __launch_bounds__(256, (NS == 2 ? 2 : 1))
-k_embed_fwd_tc(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, const EmbedNetTC<(NS == 3 ? 2 : 1)> *__restrict__ nets,
+k_embed_fwd_tc(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, const EmbedNetTC<(NS == 3 ? 2 : 1)> *__restrict__ nets,
                const int *__restrict__ bin_start, const int *__restrict__ rowstart, const float4 *__restrict__ rows_rh,
                const int2 *__restrict__ rows_id, float *__restrict__ Aout, unsigned long long *__restrict__ row_counter) {
     constexpr int NSW = NS == 3 ? 2 : 1;
@@ -223,7 +223,7 @@ k_embed_fwd_tc(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, const Emb
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem + SL::BARS);
     const int tid = threadIdx.x, warp = tid >> 5;
     const int row = tid & 127, h = tid >> 7;
-    const int sel[4] = {sel4.x, sel4.y, sel4.z, sel4.w}, off[4] = {off4.x, off4.y, off4.z, off4.w};
+    const int *sel = tt.sel, *off = tt.off;
     const float inv_nm = 1.0f / (float)Nm;
 
     if (tid == 0) {
@@ -437,9 +437,8 @@ EnvParams make_env(const dp_model *m, const Grid3 &g) {
 
 // S3: compact fp32 environment rows for the tcgen05 embedding kernels
 cudaError_t launch_env_rows(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
-    int4 off4 = make_int4(m->off[0], m->off[1], m->off[2], m->off[3]);
-    k_env_rows<<<(unsigned)((N + 7) / 8), 256, 0, st>>>(N, m->T, g.ncell, m->Nm, sel4, off4, make_env(m, g), m->avg_dev, m->std_dev,
+    const TypeTab tt = make_typetab(m);
+    k_env_rows<<<(unsigned)((N + 7) / 8), 256, 0, st>>>(N, m->T, g.ncell, m->Nm, tt, make_env(m, g), m->avg_dev, m->std_dev,
                                                          (int *)(ws + L.bin_start), (double *)(ws + L.xs), (int *)(ws + L.nlist),
                                                          (int *)(ws + L.nreal), (int *)(ws + L.rowstart),
                                                          (float4 *)(ws + L.rows_rh), (int2 *)(ws + L.rows_id));
@@ -453,13 +452,12 @@ cudaError_t launch_fwd(const dp_model *m, long N, const Grid3 &g, char *ws, cons
     constexpr int NSW = NS == 3 ? 2 : 1;
     const int smem = SmemLayout<NSW>::TOTAL;
     DP_SMEM_OPTIN((k_embed_fwd_tc<NS, APPROX>), smem);
-    int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
-    int4 off4 = make_int4(m->off[0], m->off[1], m->off[2], m->off[3]);
+    const TypeTab tt = make_typetab(m);
     launch_env_rows(m, N, g, ws, L, st);
     cudaMemsetAsync(ws + L.A, 0, sizeof(float) * (size_t)N * 4 * M2E, st);
     const int grid = m->num_sms * (NS == 2 ? 2 : 1);
     k_embed_fwd_tc<NS, APPROX><<<grid, 256, smem, st>>>(
-        N, m->T, g.ncell, m->Nm, sel4, off4, (const EmbedNetTC<NSW> *)m->embed_tc_dev, (int *)(ws + L.bin_start),
+        N, m->T, g.ncell, m->Nm, tt, (const EmbedNetTC<NSW> *)m->embed_tc_dev, (int *)(ws + L.bin_start),
         (int *)(ws + L.rowstart), (const float4 *)(ws + L.rows_rh), (const int2 *)(ws + L.rows_id), (float *)(ws + L.A),
         (unsigned long long *)(ws + L.status + 8));
     return cudaGetLastError();

@@ -52,7 +52,7 @@ __device__ __forceinline__ void tanh16_store(const uint32_t (&z)[16], uint8_t *i
 }
 
 __global__ void __launch_bounds__(NWG * 128, 1)
-k_embed_fwd_tc2(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, const EmbedNetTC2 *__restrict__ nets,
+k_embed_fwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, const EmbedNetTC2 *__restrict__ nets,
                 const int *__restrict__ bin_start, const int *__restrict__ rowstart, const float4 *__restrict__ rows_rh,
                 const int2 *__restrict__ rows_id, float *__restrict__ Aout, unsigned long long *__restrict__ row_counter) {
     using SL = FwdSmem;
@@ -67,7 +67,7 @@ k_embed_fwd_tc2(long N, int T, int ncell, int Nm, int4 sel4, int4 off4, const Em
     uint8_t *timg_row = wgs + SL::TIMG + t * 16;            // this row's 16-byte slot of chunk 0
     float *scr = reinterpret_cast<float *>(wgs + SL::SCR);
     int *meta = reinterpret_cast<int *>(wgs + SL::META);
-    const int sel[4] = {sel4.x, sel4.y, sel4.z, sel4.w}, off[4] = {off4.x, off4.y, off4.z, off4.w};
+    const int *sel = tt.sel, *off = tt.off;
     const float inv_nm = 1.0f / (float)Nm;
 
     if (tid == 0) {
@@ -303,13 +303,12 @@ cudaError_t launch_env_rows(const dp_model *m, long N, const Grid3 &g, char *ws,
 
 cudaError_t launch_embed_fwd_tc2(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
     DP_SMEM_OPTIN(k_embed_fwd_tc2, FwdSmem::TOTAL);
-    int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
-    int4 off4 = make_int4(m->off[0], m->off[1], m->off[2], m->off[3]);
+    const TypeTab tt = make_typetab(m);
     cudaError_t e = launch_env_rows(m, N, g, ws, L, st);
     if (e != cudaSuccess) return e;
     cudaMemsetAsync(ws + L.A, 0, sizeof(float) * (size_t)N * 4 * M2E, st);
     k_embed_fwd_tc2<<<m->num_sms, NWG * 128, FwdSmem::TOTAL, st>>>(
-        N, m->T, g.ncell, m->Nm, sel4, off4, (const EmbedNetTC2 *)m->embed_tc2_dev, (int *)(ws + L.bin_start),
+        N, m->T, g.ncell, m->Nm, tt, (const EmbedNetTC2 *)m->embed_tc2_dev, (int *)(ws + L.bin_start),
         (int *)(ws + L.rowstart), (const float4 *)(ws + L.rows_rh), (const int2 *)(ws + L.rows_id), (float *)(ws + L.A),
         (unsigned long long *)(ws + L.status + 8));
     return cudaGetLastError();

@@ -164,7 +164,7 @@ __device__ __forceinline__ void gradh16(const uint32_t (&g)[16], const uint32_t 
 constexpr int WGT = 128;       // threads per warpgroup: thread = row; every stage walks its two column halves h = 0, 1
 
 __global__ void __launch_bounds__(NWG * WGT, 1)
-k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *__restrict__ nets,
+k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, const EmbedNetTC2 *__restrict__ nets,
                 const double *__restrict__ stdv, const int *__restrict__ bin_start, const int *__restrict__ rowstart,
                 const float4 *__restrict__ rows_rh, const int2 *__restrict__ rows_id, const uint8_t *__restrict__ gimg,
                 const float *__restrict__ gscale, float4 *__restrict__ rows_g, unsigned long long *__restrict__ row_counter,
@@ -180,7 +180,7 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem + SL::BARS);
     uint8_t *wgs = smem + SL::WG0 + wg * SL::WG_BYTES;
     uint8_t *lo_row = wgs + SL::TLO + t * 16;
-    const int off[4] = {off4.x, off4.y, off4.z, off4.w};
+    const int *off = tt.off;
 
     if (tid == 0) {
         for (int k = 0; k < NWG; ++k) tc::mbar_init(&bars[k], 1);
@@ -562,11 +562,11 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, int4 off4, const EmbedNetTC2 *
 // S8 + S9 (ProdForce, ProdViral): one thread per compact neighbour row.  g = dE/dR~ of the row (fp32, from
 // the backward kernel); the geometry derivative, the force scatter and the virial are fp64 (configs 3-4).
 __global__ void __launch_bounds__(256)
-k_prod_force_virial(long N, int T, int4 off4, int4 sel4, EnvParams ep, const int *__restrict__ rowstart,
+k_prod_force_virial(long N, int T, const __grid_constant__ TypeTab tt, EnvParams ep, const int *__restrict__ rowstart,
                     const int2 *__restrict__ rows_id, const float4 *__restrict__ rows_g, const double *__restrict__ xs,
                     double *__restrict__ fsorted, double *__restrict__ virial) {
     const int lane = threadIdx.x & 31;
-    const int off[4] = {off4.x, off4.y, off4.z, off4.w}, sel[4] = {sel4.x, sel4.y, sel4.z, sel4.w};
+    const int *sel = tt.sel, *off = tt.off;
     const double hx = 0.5 * ep.L[0], hy = 0.5 * ep.L[1], hz = 0.5 * ep.L[2];
     double vir[9];
 #pragma unroll
@@ -655,7 +655,7 @@ k_prod_force_virial(long N, int T, int4 off4, int4 sel4, EnvParams ep, const int
 
 cudaError_t launch_embed_bwd_tc2(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
     DP_SMEM_OPTIN(k_embed_bwd_tc2, BwdSmem::TOTAL);
-    int4 off4 = make_int4(m->off[0], m->off[1], m->off[2], m->off[3]);
+    const TypeTab tt = make_typetab(m);
     EnvParams ep;
     ep.rc = m->rc; ep.rc_smth = m->rc_smth; ep.inv_range = 1.0 / (m->rc - m->rc_smth);
     ep.L[0] = g.L[0]; ep.L[1] = g.L[1]; ep.L[2] = g.L[2];
@@ -669,13 +669,12 @@ cudaError_t launch_embed_bwd_tc2(const dp_model *m, long N, const Grid3 &g, char
 #endif
     if (m->profile) cudaEventRecord(m->ev[6], st);
     k_embed_bwd_tc2<<<m->num_sms, NWG * WGT, BwdSmem::TOTAL, st>>>(
-        N, m->T, g.ncell, m->Nm, off4, (const EmbedNetTC2 *)m->embed_tc2_dev, m->std_dev, (int *)(ws + L.bin_start),
+        N, m->T, g.ncell, m->Nm, tt, (const EmbedNetTC2 *)m->embed_tc2_dev, m->std_dev, (int *)(ws + L.bin_start),
         (int *)(ws + L.rowstart), (const float4 *)(ws + L.rows_rh), (const int2 *)(ws + L.rows_id),
         (const uint8_t *)(ws + L.gAf), (const float *)(ws + L.gscale), (float4 *)(ws + L.rows_g),
         (unsigned long long *)(ws + L.status + 16), tdbg);
     if (m->profile) cudaEventRecord(m->ev[7], st);
-    int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
-    k_prod_force_virial<<<m->num_sms * 8, 256, 0, st>>>(N, m->T, off4, sel4, ep, (int *)(ws + L.rowstart),
+    k_prod_force_virial<<<m->num_sms * 8, 256, 0, st>>>(N, m->T, tt, ep, (int *)(ws + L.rowstart),
                                                         (const int2 *)(ws + L.rows_id), (const float4 *)(ws + L.rows_g),
                                                         (double *)(ws + L.xs), (double *)(ws + L.fsorted), (double *)(ws + L.virial));
 #ifdef DP_BWD_TIMING

@@ -62,10 +62,10 @@ __global__ void k_thermo(double *__restrict__ rec, const double *__restrict__ vi
 
 namespace {
 struct MdWs { size_t base, vir, cand, candcnt, xref, total; };
-MdWs md_layout(const dp_model *m, long N, double skin) {
+MdWs md_layout(const dp_model *m, long N, double skin, const double *box) {
     MdWs w{};
     auto al = [](size_t x) { return (x + 255) & ~(size_t)255; };
-    w.base = al(dp_workspace_bytes(m, N));
+    w.base = al(dp_workspace_bytes(m, N, box));
     w.vir = w.base;
     w.total = al(w.vir + 16 * sizeof(double));
     if (skin > 0.0) {
@@ -77,9 +77,9 @@ MdWs md_layout(const dp_model *m, long N, double skin) {
 }
 }  // namespace
 
-extern "C" size_t dp_md_workspace_bytes(const dp_model *m, long natoms, double skin) {
-    if (!m || natoms <= 0 || !(skin >= 0.0) || dp_workspace_bytes(m, natoms) == 0) return 0;
-    return md_layout(m, natoms, skin).total;
+extern "C" size_t dp_md_workspace_bytes(const dp_model *m, long natoms, double skin, const double *box_host) {
+    if (!m || natoms <= 0 || !(skin >= 0.0) || dp_workspace_bytes(m, natoms, box_host) == 0) return 0;
+    return md_layout(m, natoms, skin, box_host).total;
 }
 
 extern "C" int dp_md_run(dp_model *m, long natoms, double *coords_dev, double *vel_dev, const int *types_dev,
@@ -94,8 +94,12 @@ extern "C" int dp_md_run(dp_model *m, long natoms, double *coords_dev, double *v
     ms.n = n_mass;
     for (int k = 0; k < MD_MAX_MASS; ++k) ms.m[k] = k < n_mass ? mass_host[k] : 1.0;
     for (int k = 0; k < n_mass; ++k) if (!(ms.m[k] > 0.0)) return DP_EINVAL;
-    const bool buffered = skin > 0.0 && rebuild_every > 1;
-    const MdWs W = md_layout(m, natoms, buffered ? skin : 0.0);
+    // the buffered list lives on the minimum-image path: a general cell or an edge shorter than 2 rc searches every step
+    // (a stored candidate is re-tested at its nearest image, which is the only image that can be inside rc when L >= 2 rc)
+    bool mi_box = box_host[1] == 0 && box_host[2] == 0 && box_host[3] == 0 && box_host[5] == 0 && box_host[6] == 0 && box_host[7] == 0;
+    for (int a = 0; a < 3; ++a) mi_box = mi_box && box_host[4 * a] >= 2.0 * m->rc;
+    const bool buffered = skin > 0.0 && rebuild_every > 1 && mi_box;
+    const MdWs W = md_layout(m, natoms, buffered ? skin : 0.0, box_host);
     if (W.base == 0) return DP_EINVAL;
     if (workspace_bytes < W.total) return DP_ENOMEM;
     char *ws = (char *)workspace_dev;

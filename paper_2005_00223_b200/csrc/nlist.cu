@@ -140,7 +140,7 @@ __global__ void __launch_bounds__(1024) k_scan_tiles(int n, const int *__restric
     if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) start[n] = tile_start[gridDim.x];
 }
 // exclusive scan of cnt[0..n) -> start[0..n] (three launches; tmp holds 2 * (n / SCAN_TILE + 2) ints)
-void launch_scan(int n, const int *cnt, int *start, int *tmp, cudaStream_t st) {
+inline void launch_scan(int n, const int *cnt, int *start, int *tmp, cudaStream_t st) {
     const int nt = (n + SCAN_TILE - 1) / SCAN_TILE;
     int *sums = tmp, *tile_start = tmp + nt + 1;
     k_scan_sums<<<nt, 1024, 0, st>>>(n, cnt, sums);
@@ -317,7 +317,7 @@ template <int MODE>
 __global__ void __launch_bounds__(128, 8)
 k_nlist2(long N, int T, Grid3 g, double rc2, NlistF32 gf, int cap, const int *__restrict__ bin_start,
          const double *__restrict__ xs, const float4 *__restrict__ xsf, const int *__restrict__ perm,
-         const int *__restrict__ inv, int Nm, int4 sel4, int *__restrict__ nlist, int *__restrict__ nreal,
+         const int *__restrict__ inv, int Nm, const __grid_constant__ TypeTab tt, int *__restrict__ nlist, int *__restrict__ nreal,
          int *__restrict__ rowcnt, int *__restrict__ status, int *__restrict__ cand, int *__restrict__ candcnt) {
     extern __shared__ unsigned long long keys_all[];
     __shared__ int2 runtab_all[4][66];
@@ -327,7 +327,7 @@ k_nlist2(long N, int T, Grid3 g, double rc2, NlistF32 gf, int cap, const int *__
     unsigned long long *keys = keys_all + (size_t)wid * cap;
     int *sidx = reinterpret_cast<int *>(keys_all + (size_t)4 * cap) + (size_t)wid * cap;   // sorted-space index beside every key
     int2 *runtab = runtab_all[wid];
-    const int sel[4] = {sel4.x, sel4.y, sel4.z, sel4.w};
+    const int *sel = tt.sel;
     const double xi = xs[3 * i], yi = xs[3 * i + 1], zi = xs[3 * i + 2];
     const float4 pf = xsf[i];
     const int ii = (int)i;
@@ -541,6 +541,8 @@ __global__ void k_regather(long N, const double *__restrict__ coords, const int 
 
 }  // namespace
 
+void dp_launch_scan(int n, const int *cnt, int *start, int *tmp, cudaStream_t st) { launch_scan(n, cnt, start, tmp, st); }
+
 cudaError_t launch_regather(const dp_model *m, long N, const double *coords, const Grid3 &g, char *ws, const WsLayout &L,
                             cudaStream_t st) {
     k_regather<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(N, coords, (int *)(ws + L.perm), g, m->md_xref,
@@ -570,7 +572,7 @@ cudaError_t launch_build_cells(const dp_model *m, long N, const double *coords, 
 cudaError_t launch_nlist(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
     const int cap = m->sort_cap;
     const size_t smem = (size_t)4 * cap * (sizeof(unsigned long long) + sizeof(int));   // keys + sorted-space indices
-    int4 sel4 = make_int4(m->sel[0], m->sel[1], m->sel[2], m->sel[3]);
+    const TypeTab tt = make_typetab(m);
     // fp32 pre-filter margin: the fp32 copy is off by <= ulp(L)/2 per coordinate, the fp32 arithmetic by a few ulp of rc^2
     double Lmax = g.L[0] > g.L[1] ? g.L[0] : g.L[1];
     Lmax = Lmax > g.L[2] ? Lmax : g.L[2];
@@ -586,7 +588,7 @@ cudaError_t launch_nlist(const dp_model *m, long N, const Grid3 &g, char *ws, co
     auto kern = m->list_mode == 1 ? k_nlist2<1> : (m->list_mode == 2 ? k_nlist2<2> : k_nlist2<0>);
     kern<<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, m->T, g, m->rc * m->rc, gf, cap, (int *)(ws + L.bin_start),
                                                     (double *)(ws + L.xs), (const float4 *)(ws + L.xsf), (int *)(ws + L.perm),
-                                                    (int *)(ws + L.inv), m->Nm, sel4, (int *)(ws + L.nlist),
+                                                    (int *)(ws + L.inv), m->Nm, tt, (int *)(ws + L.nlist),
                                                     (int *)(ws + L.nreal), m->prec == DP_FP64 ? nullptr : (int *)(ws + L.rowcnt),
                                                     (int *)(ws + L.status), m->md_cand, m->md_candcnt);
     if (m->prec != DP_FP64)

@@ -22,5 +22,5 @@ def test_strerror_and_argument_validation_without_gpu():
     L = binding.lib()
     assert L.dp_strerror(0) == b"ok"
     assert b"box" in L.dp_strerror(-2)
-    assert L.dp_workspace_bytes(None, 100) == 0
+    assert L.dp_workspace_bytes(None, 100, None) == 0
     assert L.dp_create(None, None, None, 0, 6.0, 0.5, None, 0) == -1     # DP_EINVAL before any CUDA call

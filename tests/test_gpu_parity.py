@@ -110,7 +110,7 @@ def test_error_codes_through_the_c_abi():
     assert call(s.natoms, base, need - 256) == -3
     assert call(s.natoms, base + 8, need) == -1
     assert call(0, base, need) == -1
-    assert L.dp_workspace_bytes(m._h, 1 << 25) == 0 and L.dp_workspace_bytes(m._h, (1 << 24)) == 0   # 2^24 * 256 rows >= 2^31
+    assert L.dp_workspace_bytes(m._h, 1 << 25, None) == 0 and L.dp_workspace_bytes(m._h, (1 << 24), None) == 0   # 2^24 * 256 rows >= 2^31
     torch.cuda.synchronize()
     m.close()
     # 298 neighbours inside rc = 9.5 A against a sort buffer of 256 (capacity 16)
