@@ -29,16 +29,25 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 # algorithmic flops (FMA = 2, tanh not counted, no credit for padding or recomputation)
-FLOP_ROW_FWD = 12550 + 800          # embedding GEMMs forward + contraction forward, per neighbour row
+FLOP_ROW_FWD = 12550 + 800          # embedding GEMMs forward + contraction forward, per neighbour row   (widths 25, 50, 100)
 FLOP_ROW_BWD = 12550 + 1600         # embedding GEMMs backward + contraction backward, per neighbour row
 FLOP_ATOM_FIT = 2036160             # fitting fwd + bwd + descriptor fwd/bwd, per atom
+
+
+def flops_of(model):
+    """(per-row forward, per-row backward, per-atom fitting + descriptor, tanh per row) for the model's network widths."""
+    m0, m1, m2 = model.embed_widths
+    f0, f1, f2 = model.fit_widths
+    gemm = 2 * (m0 + m0 * m1 + m1 * m2)
+    fit = 2 * (m2 * model.axis * f0 + f0 * f1 + f1 * f2 + f2)
+    return gemm + 2 * 4 * m2, gemm + 4 * 4 * m2, 2 * fit + 3 * 2 * 4 * m2 * model.axis, m0 + m1 + m2
 # tensor-core flops the MIX-16 backward kernel actually executes per 128-row tile (M = 128, 2 flop per MAC; DESIGN.md 6):
 # layer 2 (hi+lo) 2*32*64, layer 3 2*96*112, dR 2*208*16, dT3 32*112, dT2+dz3 W3^T (32+112)*64, dT1+dz3 W3f (32+112)*32, dz2 W2^T 64*32
 EXEC_FLOP_ROW_BWD = 2 * (2 * 32 * 64 + 2 * 96 * 112 + 2 * 208 * 16 + 32 * 112 + 144 * 64 + 144 * 32 + 64 * 32)
 # ncu --set full captures of the dominant kernel per config (dram__bytes_read.sum + dram__bytes_write.sum per launch are in
 # these summaries; the bench line itself measures no DRAM traffic, so roofline.traffic is null and points here)
-TRAFFIC_PROFILE = {"c4_cu1048576": "profiles/r02_c4_bwd_tc2_ncu.md", "c2_cu13500": "profiles/r02_c2_embed_bwd_ncu.md",
-                   "c3_water110592": "profiles/r02_c3_embed_bwd_ncu.md"}
+TRAFFIC_PROFILE = {"c4_cu1048576": "profiles/r02_c4_bwd_tc2_ncu.md", "c2_cu13500": "profiles/r02_c2_bwd_f64_ncu.md",
+                   "c3_water110592": "profiles/r02_c3_bwd_mix_ncu.md"}
 
 
 def peaks():
@@ -161,7 +170,8 @@ def roofline_of(s, r, pk, mp):
     achieved = algorithmic flops of the kernel (SURVEY.md 8(d): 14,150 per REAL neighbour row) / its CUDA-event duration;
     peak = the measured rate of the pipe its dtype runs on (pk: MEASURED_PEAKS.json, mp: dp_measure_peaks of this run)."""
     ph = r["phases"]
-    dom_flops = r["real_rows"] * FLOP_ROW_BWD
+    _, frow_b, _, tanh_row = flops_of(s.model)
+    dom_flops = r["real_rows"] * frow_b
     ach = dom_flops / (ph[5] * 1e-3) / 1e12
     if s.precision == "fp64":
         kname, peak = "k_embed_bwd_f64 (S7-S9 in one kernel)", mp["dmma_tflops"]
@@ -178,7 +188,7 @@ def roofline_of(s, r, pk, mp):
            "flops_per_launch": dom_flops, "kernel_ms": ph[5]}
     if s.precision != "fp64":
         # the tanh of the recomputed forward, counted on the real rows only (175 per row), against the measured MUFU rate
-        rec["mufu_tanh_frac"] = (r["real_rows"] * 175 / (ph[5] * 1e-3)) / (mp["tanh_tera_per_s"] * 1e12)
+        rec["mufu_tanh_frac"] = (r["real_rows"] * tanh_row / (ph[5] * 1e-3)) / (mp["tanh_tera_per_s"] * 1e12)
     if s.precision == "mix16":
         rec["executed_tflops"] = r["rows_b"] * EXEC_FLOP_ROW_BWD / (ph[5] * 1e-3) / 1e12
         rec["note"] = ("algorithmic backward flops (14,150 per real neighbour row); the in-kernel forward recompute, the hi/lo operand "
@@ -189,6 +199,7 @@ def roofline_of(s, r, pk, mp):
 
 def kernels_of(s, r, ms_step):
     ph, N, rr = r["phases"], s.natoms, r["real_rows"]
+    FLOP_ROW_FWD, FLOP_ROW_BWD, FLOP_ATOM_FIT, _ = flops_of(s.model)
     return {"nlist_ms": ph[0], "embed_fwd_ms": ph[1], "fit_ms": ph[2], "embed_bwd_ms": ph[3], "finalize_ms": ph[4],
             "embed_bwd_kernel_ms": ph[5],
             "embed_fwd_tflops": rr * FLOP_ROW_FWD / (ph[1] * 1e-3) / 1e12,
@@ -262,8 +273,9 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=4,
-                    help="BASELINE.json configs index (default: c4, copper 1,048,576 atoms MIX-16, the largest single-GPU config)")
+    ap.add_argument("--config", default="4",
+                    help="BASELINE.json configs index 0..4 (default: 4 = copper 1,048,576 atoms MIX-16, the largest single-GPU "
+                         "config), or paper_cu / paper_water: the paper's network shape (32, 64, 128), capacity 512 / 144 (PAPER.md:151)")
     ap.add_argument("--no-summary", action="store_true", help="skip the configs_summary leg (the other four configs)")
     ap.add_argument("--precision", default=None, choices=["fp64", "mix32", "mix16"],
                     help="override the config's precision (profiling aid; the default is the precision BASELINE.json names)")
@@ -282,9 +294,15 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
 
     from paper_2005_00223_b200 import synth
+
+    def workload():
+        if args.config in ("paper_cu", "paper_water"):
+            return synth.paper_config(args.config, args.precision or "fp64")
+        return synth.config(int(args.config))
+
     if args.impl == "reference":
         if rank == 0:
-            run_reference(args, synth.config(args.config))
+            run_reference(args, workload())
         return
 
     import torch
@@ -298,7 +316,7 @@ def main():
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=dev)
 
-    s = synth.config(args.config)
+    s = workload()
     if args.precision:
         s.precision = args.precision
     N = s.natoms
@@ -388,7 +406,7 @@ def main():
             n, dt, cores = oracle_sample(s, ncen)
             line["cpu_baseline"] = {"value": n / dt, "unit": "atom-steps/s", "cores": cores, "kind": "oracle",
                                     "sample": f"{n} evenly spaced centre atoms of {s.name}, one evaluation ({dt:.1f} s)"}
-        if world == 1 and not args.no_summary:
+        if world == 1 and not args.no_summary and args.config == "4":
             # the other BASELINE configs: same timing method (warm-up, L2 flush, per-step events), own roofline and oracle timing
             summ = {s.name: {"precision": s.precision, "natoms": N, "ms_per_step": ms_step, "atom_steps_per_s": value,
                              "s_per_step_per_atom": ms_step * 1e-3 / N, "roofline_frac": line["roofline"]["frac"]}}
@@ -396,7 +414,7 @@ def main():
             del model, coords, types, out, cdev, tdev
             torch.cuda.empty_cache()
             for idx in range(5):
-                if idx == args.config:
+                if idx == 4:
                     continue
                 s2 = synth.config(idx)
                 k2 = max(10, K)

@@ -54,14 +54,15 @@ WsLayout ws_layout(const dp_model *m, long N, long NE) {
         if (m->prec == DP_MIX16) L.rows_g = take(sizeof(float) * 4 * (size_t)N * m->Nm);
     }
     const size_t esz = m->prec == DP_FP64 ? sizeof(double) : sizeof(float);
-    L.A = take(esz * (size_t)N * 4 * M2E);
-    if (m->prec == DP_FP64) L.gAf = take(sizeof(double) * (size_t)N * 3 * NT3 * 32);
+    const int nt3 = 2 * ((m->m0 + 3) / 4);          // EmbW<W>::NT3
+    L.A = take(esz * (size_t)N * 4 * m->m2);
+    if (m->prec == DP_FP64) L.gAf = take(sizeof(double) * (size_t)N * 3 * nt3 * 32);
     else L.gAf = take(sizeof(uint32_t) * (size_t)N * 2 * 28 * 32);
     L.gscale = take(sizeof(float) * (size_t)N);
     // (MIX-16: buffers 2..6 also hold the gz1 operand images, one per 128-row tile and at least one per type: the pad
     // covers systems with fewer rows than a tile)
     L.fit_act = take(esz * (size_t)N * 240 * 7 + (m->prec == DP_MIX16 ? ((size_t)m->T + 1) * FIT_GZ_TILE_BYTES : 0));
-    L.gD = take(esz * (size_t)N * M2E * 16);
+    L.gD = take(esz * (size_t)N * m->m2 * 16);
     L.eatom = take(sizeof(double) * (size_t)N);
     L.fsorted = take(sizeof(double) * 3 * (size_t)NE);
     L.virial = take(sizeof(double) * 16);
@@ -77,6 +78,9 @@ bool rows_fit_int32(const dp_model *m, long N) {
 
 // Cell grid of one evaluation.  Orthorhombic boxes with every length >= 2 rc take the minimum-image path (nlist.cu);
 // everything else (a general cell, or an edge shorter than 2 rc) takes the ghost path (ghost.cu).  false: degenerate box.
+// (32, 64, 128) networks: which precision modes have kernels for them
+bool paper_shape_supported(dp_precision prec) { return prec == DP_FP64; }
+
 bool make_grid(const dp_model *m, long N, const double *box, Grid3 *g) {
     *g = Grid3{};
     const bool ortho = !(box[1] != 0 || box[2] != 0 || box[3] != 0 || box[5] != 0 || box[6] != 0 || box[7] != 0);
@@ -159,11 +163,11 @@ bool make_grid(const dp_model *m, long N, const double *box, Grid3 *g) {
 }
 
 // logical feature maps of the register-chained embedding net (dp_internal.h)
-inline int f2map(int nt, int r, int j) { int e = 4 * nt + r; return e < M0 ? e + M0 * j : -1; }
-inline int f3map(int nt3, int r, int j3) { int f = f2map(nt3 >> 1, r, nt3 & 1); return f < 0 ? -1 : f + M1 * j3; }
-
-template <typename TW>
-void build_embed_frag(const double *net, EmbedNetFrag<TW> *out) {
+template <typename TW, int W>
+void build_embed_frag(const double *net, EmbedNetFrag<TW, W> *out) {
+    constexpr int M0 = EmbW<W>::M0, M1 = EmbW<W>::M1, M2E = EmbW<W>::M2E, KC1 = EmbW<W>::KC1, NT2 = EmbW<W>::NT2, NT3 = EmbW<W>::NT3, NT1 = EmbW<W>::NT1;
+    auto f2map = [](int nt, int r, int j) { int e = 4 * nt + r; return e < M0 ? e + M0 * j : -1; };
+    auto f3map = [&](int nt3, int r, int j3) { int f = f2map(nt3 >> 1, r, nt3 & 1); return f < 0 ? -1 : f + M1 * j3; };
     const double *W1 = net, *b1 = W1 + M0, *W2 = b1 + M0, *b2 = W2 + M0 * M1, *W3 = b2 + M1, *b3 = W3 + M1 * M2E;
     std::memset(out, 0, sizeof(*out));
     for (int kc = 0; kc < KC1; ++kc)
@@ -196,11 +200,11 @@ void build_embed_frag(const double *net, EmbedNetFrag<TW> *out) {
                 if (fin >= 0 && fo >= 0) out->W3Tf[(kc * NT2 + nt2) * 32 + l] = (TW)W3[fin * M2E + fo];
             }
     for (int kc = 0; kc < 2 * NT2; ++kc)
-        for (int nt1 = 0; nt1 < 4; ++nt1)
+        for (int nt1 = 0; nt1 < NT1; ++nt1)
             for (int l = 0; l < 32; ++l) {
                 int fo = f2map(kc >> 1, l & 3, kc & 1), n = l >> 2;
                 int kc1 = 2 * nt1 + (n & 1), e = 4 * kc1 + (n >> 1);
-                if (kc1 < KC1 && e < M0 && fo >= 0) out->W2Tf[(kc * 4 + nt1) * 32 + l] = (TW)W2[e * M1 + fo];
+                if (kc1 < KC1 && e < M0 && fo >= 0) out->W2Tf[(kc * NT1 + nt1) * 32 + l] = (TW)W2[e * M1 + fo];
             }
 }
 
@@ -386,9 +390,12 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
     const int T = w->ntypes;
     if (T < 1 || T > DP_MAX_TYPES) return DP_EINVAL;
     if (!(rc > 0) || !(rc_smth >= 0) || !(rc_smth < rc) || !(rc * rc < 128.0)) return DP_EINVAL;
-    if (w->embed_widths[0] != M0 || w->embed_widths[1] != M1 || w->embed_widths[2] != M2E || w->axis != 16 ||
+    // embedding widths (W, 2 W, 4 W) with W = 25 (BASELINE configs) or W = 32 (the paper's own networks)
+    const int W0 = w->embed_widths[0];
+    if ((W0 != 25 && W0 != 32) || w->embed_widths[1] != 2 * W0 || w->embed_widths[2] != 4 * W0 || w->axis != 16 ||
         w->fit_widths[0] != 240 || w->fit_widths[1] != 240 || w->fit_widths[2] != 240)
         return DP_EUNSUPPORTED;
+    if (W0 == 32 && !paper_shape_supported(prec)) return DP_EUNSUPPORTED;
     if (prec != DP_FP64 && prec != DP_MIX32 && prec != DP_MIX16) return DP_EINVAL;
     int maxsel = 0, Nm = 0;
     for (int b = 0; b < T; ++b) { if (sel[b] <= 0) return DP_EINVAL; Nm += sel[b]; if (sel[b] > maxsel) maxsel = sel[b]; }
@@ -402,6 +409,7 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
     std::memset(m, 0, sizeof(*m));
     m->device = dev;
     m->T = T; m->Nm = Nm; m->axis = 16; m->F = 240; m->rc = rc; m->rc_smth = rc_smth; m->prec = prec;
+    m->m0 = W0; m->m1 = 2 * W0; m->m2 = 4 * W0;
     m->n_type_map = n_type_map;
     for (int b = 0; b < T; ++b) { m->sel[b] = sel[b]; m->off[b + 1] = m->off[b] + sel[b]; }
     int cap = 256;
@@ -417,10 +425,14 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
     auto ok = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
     std::vector<int> tm(type_map, type_map + n_type_map);
     ok(upload(tm, (void **)&m->type_map_dev));
-    const size_t ensz = (size_t)M0 + M0 + M0 * M1 + M1 + M1 * M2E + M2E;
-    if (prec == DP_FP64) {
-        std::vector<EmbedNetFrag<double>> frags((size_t)T * T);
-        for (int ab = 0; ab < T * T; ++ab) build_embed_frag<double>(w->embed + ab * ensz, &frags[ab]);
+    const size_t ensz = (size_t)W0 + W0 + (size_t)W0 * 2 * W0 + 2 * W0 + (size_t)2 * W0 * 4 * W0 + 4 * W0;
+    if (prec == DP_FP64 && W0 == 32) {
+        std::vector<EmbedNetFrag<double, 32>> frags((size_t)T * T);
+        for (int ab = 0; ab < T * T; ++ab) build_embed_frag<double, 32>(w->embed + ab * ensz, &frags[ab]);
+        ok(upload(frags, &m->embed_frag_dev));
+    } else if (prec == DP_FP64) {
+        std::vector<EmbedNetFrag<double, 25>> frags((size_t)T * T);
+        for (int ab = 0; ab < T * T; ++ab) build_embed_frag<double, 25>(w->embed + ab * ensz, &frags[ab]);
         ok(upload(frags, &m->embed_frag_dev));
     } else if (prec == DP_MIX32) {      // tcgen05 forward (embed_tc.cu), mma.sync backward (embed_mix.cu): weights as hi + lo fp16
         std::vector<EmbedNetFragH<2>> frags((size_t)T * T);
@@ -442,7 +454,7 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
             ok(upload(n1, &m->embed_tc_dev));
         }
     }
-    const int ND = M2E * 16, F = 240;
+    const int ND = m->m2 * 16, F = 240;
     const size_t fnsz = (size_t)ND * F + F + (size_t)F * F + F + (size_t)F * F + F + F + 1;
     std::vector<double> V1((size_t)T * ND * F), V2((size_t)T * F * F), V3((size_t)T * F * F), c1(T * F), c2(T * F),
         c3(T * F), v4(T * F), c4(T);

@@ -34,21 +34,33 @@ constexpr int NT3 = 14;                      // 8-wide tiles of layer-3 output (
 constexpr int M2P = NT3 * 8;                 // padded G width
 constexpr int ROWCHUNK = 64;                 // neighbour rows staged per pre-pass / post-pass
 
+// Width-dependent constants of the register-chained (mma.sync) kernels for embedding widths (W, 2 W, 4 W); W = 25 is the
+// BASELINE shape, W = 32 the paper's ("the embedding nets are of size (32, 64, 128)").
+template <int W>
+struct EmbW {
+    static constexpr int M0 = W, M1 = 2 * W, M2E = 4 * W;
+    static constexpr int KC1 = (W + 3) / 4;          // k-chunks of 4 of the layer-1 output
+    static constexpr int NT2 = KC1;                  // 8-wide tiles of the layer-2 output
+    static constexpr int NT3 = 2 * KC1;              // 8-wide tiles of the layer-3 output
+    static constexpr int NT1 = (KC1 + 1) / 2;        // 8-wide tiles of the layer-1 slots (backward of layer 2)
+};
+
 // Fragment-ordered embedding net (one per (centre type, neighbour type)), element type TW.
 // Logical feature <-> internal position maps:
 //   layer-1 slot (kc,r)        : e  = 4*kc + r                       (valid if < 25)
 //   layer-2 position (nt,r,j)  : f2 = (4*nt + r) + 25*j              (valid if 4*nt+r < 25)
 //   layer-3 position (nt3,r,j3): f3 = f2(nt3/2, r, nt3%2) + 50*j3    (valid if f2 valid)
-template <typename TW>
+template <typename TW, int W = 25>
 struct EmbedNetFrag {
-    TW w1[KC1 * 4];                 // by slot
-    TW b1[KC1 * 4];
-    TW b2[NT2 * 8];                 // by position nt*8 + 2r + j
-    TW b3[NT3 * 8];
-    TW W2f[KC1 * NT2 * 32];         // forward B fragments  [kc][nt][lane]
-    TW W3f[NT3 * NT3 * 32];         // forward B fragments  [kc'=2nt2+j2][nt3][lane]
-    TW W3Tf[2 * NT3 * NT2 * 32];    // backward B fragments [kc=2nt3+j3][nt2][lane]
-    TW W2Tf[NT3 * 4 * 32];          // backward B fragments [kc=2nt2+j2][nt1][lane]
+    using E = EmbW<W>;
+    TW w1[E::KC1 * 4];                      // by slot
+    TW b1[E::KC1 * 4];
+    TW b2[E::NT2 * 8];                      // by position nt*8 + 2r + j
+    TW b3[E::NT3 * 8];
+    TW W2f[E::KC1 * E::NT2 * 32];           // forward B fragments  [kc][nt][lane]
+    TW W3f[E::NT3 * E::NT3 * 32];           // forward B fragments  [kc'=2nt2+j2][nt3][lane]
+    TW W3Tf[2 * E::NT3 * E::NT2 * 32];      // backward B fragments [kc=2nt3+j3][nt2][lane]
+    TW W2Tf[E::NT3 * E::NT1 * 32];          // backward B fragments [kc=2nt2+j2][nt1][lane]
 };
 
 struct dp_model {
@@ -56,6 +68,7 @@ struct dp_model {
     int sel[DP_MAX_TYPES];
     int off[DP_MAX_TYPES + 1];
     int Nm;
+    int m0, m1, m2;                 // embedding widths (W, 2 W, 4 W): (25, 50, 100) or (32, 64, 128)
     int axis;                       // 16
     int F;                          // fitting width 240
     double rc, rc_smth;
@@ -186,5 +199,3 @@ size_t fit_tc_type_elems();
 void fit_tc_build_type(const double *V1, const double *V2, const double *V3, struct __half *out);
 cudaError_t launch_env_rows(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
-int embed_smem_bytes_fwd_f64();
-int embed_smem_bytes_bwd_f64();

@@ -61,8 +61,11 @@ __device__ __forceinline__ void env_row(const EnvParams &p, double dx, double dy
 //   y1[kc]  layer-1 output, slot (kc, r=lane%4)
 //   t2[p]   tanh of layer-2 pre-activation at position p = 2*nt2 + j2 ;  y2[p] = y1[p>>1] + t2[p]
 //   t3[q]   tanh of layer-3 pre-activation at position q = 2*nt3 + j3 ;  G[q]  = y2[q>>1] + t3[q]
-__device__ __forceinline__ void embed_forward_tile(const EmbedNetFrag<double> *__restrict__ net, int lane, double s,
-                                                   double (&y1)[KC1], double (&t2)[2 * NT2], double (&t3)[2 * NT3]) {
+template <int W>
+__device__ __forceinline__ void embed_forward_tile(const EmbedNetFrag<double, W> *__restrict__ net, int lane, double s,
+                                                   double (&y1)[EmbW<W>::KC1], double (&t2)[2 * EmbW<W>::NT2], double (&t3)[2 * EmbW<W>::NT3]) {
+    constexpr int M0 = EmbW<W>::M0, M1 = EmbW<W>::M1, M2E = EmbW<W>::M2E, KC1 = EmbW<W>::KC1, NT2 = EmbW<W>::NT2, NT3 = EmbW<W>::NT3, NT1 = EmbW<W>::NT1;
+    (void)M0; (void)M1; (void)M2E; (void)KC1; (void)NT2; (void)NT3; (void)NT1;
     const int r = lane & 3;
 #pragma unroll
     for (int kc = 0; kc < KC1; ++kc) y1[kc] = dp_tanh(fma(s, net->w1[4 * kc + r], net->b1[4 * kc + r]));
@@ -112,32 +115,40 @@ __device__ __forceinline__ void embed_forward_tile(const EmbedNetFrag<double> *_
 }
 
 // logical layer-3 feature of internal position (nt3, r, j3); -1 for padding
+template <int W>
 __device__ __forceinline__ int feature3(int nt3, int r, int j3) {
     const int e = 4 * (nt3 >> 1) + r;
-    return e < M0 ? e + M0 * (nt3 & 1) + M1 * j3 : -1;
+    return e < W ? e + W * (nt3 & 1) + 2 * W * j3 : -1;
 }
 
 __device__ __forceinline__ void copy_to_smem(double *dst, const double *__restrict__ src, int n) {
     for (int k = threadIdx.x; k < n; k += blockDim.x) dst[k] = src[k];
 }
 
-constexpr int FWD_NET_DOUBLES = KC1 * 4 * 2 + NT2 * 8 + NT3 * 8 + KC1 * NT2 * 32 + NT3 * NT3 * 32;
-constexpr int BWD_NET_DOUBLES = (int)(sizeof(EmbedNetFrag<double>) / sizeof(double));
+template <int W> __host__ __device__ constexpr int fwd_net_doubles() {
+    using E = EmbW<W>;
+    return E::KC1 * 4 * 2 + E::NT2 * 8 + E::NT3 * 8 + E::KC1 * E::NT2 * 32 + E::NT3 * E::NT3 * 32;
+}
+template <int W> __host__ __device__ constexpr int bwd_net_doubles() { return (int)(sizeof(EmbedNetFrag<double, W>) / sizeof(double)); }
 constexpr int WARP_BUF_DOUBLES = ROWCHUNK * 5;   // rbuf[ROWCHUNK][4] + sbuf[ROWCHUNK]
 
 // ------------------------------------------------------------------------------------------------ forward
+template <int W>
 __global__ void __launch_bounds__(DP_WARPS_PER_CTA * 32, 1)
-k_embed_fwd_f64(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, EnvParams ep, const EmbedNetFrag<double> *__restrict__ nets,
+k_embed_fwd_f64(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, EnvParams ep, const EmbedNetFrag<double, W> *__restrict__ nets,
                 const double *__restrict__ avg, const double *__restrict__ stdv, const int *__restrict__ bin_start,
                 const double *__restrict__ xs, const int *__restrict__ nlist, const int *__restrict__ nreal,
                 double *__restrict__ Aout, unsigned long long *__restrict__ row_counter) {
+    constexpr int M0 = EmbW<W>::M0, M1 = EmbW<W>::M1, M2E = EmbW<W>::M2E, KC1 = EmbW<W>::KC1, NT2 = EmbW<W>::NT2, NT3 = EmbW<W>::NT3, NT1 = EmbW<W>::NT1;
+    (void)M0; (void)M1; (void)M2E; (void)KC1; (void)NT2; (void)NT3; (void)NT1;
+    constexpr int FWD_NET_DOUBLES = fwd_net_doubles<W>();
     extern __shared__ __align__(16) double smem[];
-    EmbedNetFrag<double> *net = reinterpret_cast<EmbedNetFrag<double> *>(smem);
+    EmbedNetFrag<double, W> *net = reinterpret_cast<EmbedNetFrag<double, W> *>(smem);
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     double *rbuf = smem + FWD_NET_DOUBLES + wid * WARP_BUF_DOUBLES;
     double *sbuf = rbuf + ROWCHUNK * 4;
     const int *sel = tt.sel;
-    const int gw = blockIdx.x * DP_WARPS_PER_CTA + wid, W = gridDim.x * DP_WARPS_PER_CTA;
+    const int gw = blockIdx.x * DP_WARPS_PER_CTA + wid, NW = gridDim.x * DP_WARPS_PER_CTA;
     const int r = lane & 3, q4 = lane >> 2;
     const double inv_nm = 1.0 / (double)Nm;
     const double hx = 0.5 * ep.L[0], hy = 0.5 * ep.L[1], hz = 0.5 * ep.L[2];
@@ -154,7 +165,7 @@ k_embed_fwd_f64(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, En
             __syncthreads();
             copy_to_smem(smem, reinterpret_cast<const double *>(nets + (a * T + b)), FWD_NET_DOUBLES);
             __syncthreads();
-            for (int i = ts0 + gw; i < ts1; i += W) {
+            for (int i = ts0 + gw; i < ts1; i += NW) {
                 const int nr = nreal[i * T + b];
                 const int npad = sel[b] - nr;
                 const int rows = nr + (npad > 0 ? 1 : 0);
@@ -189,7 +200,7 @@ k_embed_fwd_f64(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, En
                     __syncwarp();
                     for (int t = 0; t < ntile; ++t) {
                         double y1[KC1], t2[2 * NT2], t3[2 * NT3];
-                        embed_forward_tile(net, lane, sbuf[t * 8 + q4], y1, t2, t3);
+                        embed_forward_tile<W>(net, lane, sbuf[t * 8 + q4], y1, t2, t3);
                         // G in C-fragment layout -> B fragments of the contraction A^T[c][m] += R^[k][c] G[k][m]
 #pragma unroll
                         for (int g = 0; g < 2; ++g) {
@@ -215,7 +226,7 @@ k_embed_fwd_f64(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, En
                     for (int nt3 = 0; nt3 < NT3; ++nt3) {
 #pragma unroll
                         for (int j = 0; j < 2; ++j) {
-                            const int f = feature3(nt3, r, j);
+                            const int f = feature3<W>(nt3, r, j);
                             if (f >= 0) {
                                 const double v = accA[nt3][j] * inv_nm;
                                 Ai[f] = (b == 0) ? v : Ai[f] + v;
@@ -234,19 +245,23 @@ k_embed_fwd_f64(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, En
 // gAf: per atom 42 fragments of 32 doubles, already scaled by 1/Nm (written by the fitting backward):
 //   [0..14)  : dG MMA   B fragment of tile nt3: lane -> gA[c = lane%4][feature3(nt3, (lane/4)/2, (lane/4)%2)]
 //   [14..42) : dR^ MMA  B fragment of chunk kc = 2*nt3 + j3: lane -> (lane/4 < 4) ? gA[c = lane/4][feature3(nt3, lane%4, j3)] : 0
+template <int W>
 __global__ void __launch_bounds__(DP_WARPS_PER_CTA * 32, 1)
-k_embed_bwd_f64(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, EnvParams ep, const EmbedNetFrag<double> *__restrict__ nets,
+k_embed_bwd_f64(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, EnvParams ep, const EmbedNetFrag<double, W> *__restrict__ nets,
                 const double *__restrict__ avg, const double *__restrict__ stdv, const int *__restrict__ bin_start,
                 const double *__restrict__ xs, const int *__restrict__ nlist, const int *__restrict__ nreal,
                 const double *__restrict__ gAf, double *__restrict__ fsorted, double *__restrict__ virial,
                 unsigned long long *__restrict__ row_counter) {
+    constexpr int M0 = EmbW<W>::M0, M1 = EmbW<W>::M1, M2E = EmbW<W>::M2E, KC1 = EmbW<W>::KC1, NT2 = EmbW<W>::NT2, NT3 = EmbW<W>::NT3, NT1 = EmbW<W>::NT1;
+    (void)M0; (void)M1; (void)M2E; (void)KC1; (void)NT2; (void)NT3; (void)NT1;
+    constexpr int BWD_NET_DOUBLES = bwd_net_doubles<W>();
     extern __shared__ __align__(16) double smem[];
-    EmbedNetFrag<double> *net = reinterpret_cast<EmbedNetFrag<double> *>(smem);
+    EmbedNetFrag<double, W> *net = reinterpret_cast<EmbedNetFrag<double, W> *>(smem);
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     double *rbuf = smem + BWD_NET_DOUBLES + wid * WARP_BUF_DOUBLES;
     double *sbuf = rbuf + ROWCHUNK * 4;
     const int *sel = tt.sel;
-    const int gw = blockIdx.x * DP_WARPS_PER_CTA + wid, W = gridDim.x * DP_WARPS_PER_CTA;
+    const int gw = blockIdx.x * DP_WARPS_PER_CTA + wid, NW = gridDim.x * DP_WARPS_PER_CTA;
     const int r = lane & 3, q4 = lane >> 2;
     const double hx = 0.5 * ep.L[0], hy = 0.5 * ep.L[1], hz = 0.5 * ep.L[2];
     unsigned long long my_rows = 0;
@@ -265,7 +280,7 @@ k_embed_bwd_f64(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, En
             __syncthreads();
             copy_to_smem(smem, reinterpret_cast<const double *>(nets + (a * T + b)), BWD_NET_DOUBLES);
             __syncthreads();
-            for (int i = ts0 + gw; i < ts1; i += W) {
+            for (int i = ts0 + gw; i < ts1; i += NW) {
                 const int nr = nreal[i * T + b];
                 const double xi = xs[3 * (long)i], yi = xs[3 * (long)i + 1], zi = xs[3 * (long)i + 2];
                 const double *gf = gAf + (long)i * (3 * NT3 * 32);
@@ -290,7 +305,7 @@ k_embed_bwd_f64(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, En
                     __syncwarp();
                     for (int t = 0; t < ntile; ++t) {
                         double y1[KC1], t2[2 * NT2], t3[2 * NT3];
-                        embed_forward_tile(net, lane, sbuf[t * 8 + q4], y1, t2, t3);
+                        embed_forward_tile<W>(net, lane, sbuf[t * 8 + q4], y1, t2, t3);
                         const double rfrag = rbuf[(t * 8 + q4) * 4 + r];
                         // dR^[row][c] = sum_m gA[c][m] G[row][m]      (C frag: c = 2r + {0,1}, valid for r < 2)
                         double dR0 = 0.0, dR1 = 0.0;
@@ -317,17 +332,16 @@ k_embed_bwd_f64(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, En
                                 dmma(dy2[2 * nt2], dy2[2 * nt2 + 1], t3[kc], net->W3Tf[(kc * NT2 + nt2) * 32 + lane]);
                         }
                         // dz2 = dy2 (1 - t2^2) ; residual dy1[kc1] = dy2[2 kc1] + dy2[2 kc1 + 1]
-                        double dy1[8];
+                        double dy1[2 * NT1];
 #pragma unroll
-                        for (int kc1 = 0; kc1 < KC1; ++kc1) dy1[kc1] = dy2[2 * kc1] + dy2[2 * kc1 + 1];
-                        dy1[7] = 0.0;
+                        for (int kc1 = 0; kc1 < 2 * NT1; ++kc1) dy1[kc1] = kc1 < KC1 ? dy2[2 * kc1] + dy2[2 * kc1 + 1] : 0.0;
 #pragma unroll
                         for (int p = 0; p < 2 * NT2; ++p) dy2[p] *= (1.0 - t2[p] * t2[p]);
 #pragma unroll
                         for (int kc = 0; kc < 2 * NT2; ++kc) {
 #pragma unroll
-                            for (int nt1 = 0; nt1 < 4; ++nt1)
-                                dmma(dy1[2 * nt1], dy1[2 * nt1 + 1], dy2[kc], net->W2Tf[(kc * 4 + nt1) * 32 + lane]);
+                            for (int nt1 = 0; nt1 < NT1; ++nt1)
+                                dmma(dy1[2 * nt1], dy1[2 * nt1 + 1], dy2[kc], net->W2Tf[(kc * NT1 + nt1) * 32 + lane]);
                         }
                         // layer 1: ds = sum_e dy1[e] (1 - y1[e]^2) W1[e]
                         double ds = 0.0;
@@ -404,31 +418,41 @@ EnvParams make_env(const dp_model *m, const Grid3 &g) {
 
 }  // namespace
 
-int embed_smem_bytes_fwd_f64() { return (FWD_NET_DOUBLES + DP_WARPS_PER_CTA * WARP_BUF_DOUBLES) * 8; }
-int embed_smem_bytes_bwd_f64() { return (BWD_NET_DOUBLES + DP_WARPS_PER_CTA * WARP_BUF_DOUBLES) * 8; }
+template <int W> constexpr int smem_fwd() { return (fwd_net_doubles<W>() + DP_WARPS_PER_CTA * WARP_BUF_DOUBLES) * 8; }
+template <int W> constexpr int smem_bwd() { return (bwd_net_doubles<W>() + DP_WARPS_PER_CTA * WARP_BUF_DOUBLES) * 8; }
 
 static int embed_grid(const dp_model *m, long N) {
     long grid = (N + DP_WARPS_PER_CTA - 1) / DP_WARPS_PER_CTA;
     return (int)(grid > m->num_sms ? m->num_sms : grid);
 }
 
-cudaError_t launch_embed_fwd_f64(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    DP_SMEM_OPTIN(k_embed_fwd_f64, embed_smem_bytes_fwd_f64());
+template <int W>
+static cudaError_t launch_fwd_w(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    DP_SMEM_OPTIN(k_embed_fwd_f64<W>, smem_fwd<W>());
     const TypeTab tt = make_typetab(m);
-    k_embed_fwd_f64<<<embed_grid(m, N), DP_WARPS_PER_CTA * 32, embed_smem_bytes_fwd_f64(), st>>>(
-        m->T, g.ncell, m->Nm, tt, make_env(m, g), (const EmbedNetFrag<double> *)m->embed_frag_dev, m->avg_dev,
+    k_embed_fwd_f64<W><<<embed_grid(m, N), DP_WARPS_PER_CTA * 32, smem_fwd<W>(), st>>>(
+        m->T, g.ncell, m->Nm, tt, make_env(m, g), (const EmbedNetFrag<double, W> *)m->embed_frag_dev, m->avg_dev,
         m->std_dev, (int *)(ws + L.bin_start), (double *)(ws + L.xs), (int *)(ws + L.nlist), (int *)(ws + L.nreal),
         (double *)(ws + L.A), (unsigned long long *)(ws + L.status + 8));
     return cudaGetLastError();
 }
 
-cudaError_t launch_embed_bwd_f64(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    DP_SMEM_OPTIN(k_embed_bwd_f64, embed_smem_bytes_bwd_f64());
+template <int W>
+static cudaError_t launch_bwd_w(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    DP_SMEM_OPTIN(k_embed_bwd_f64<W>, smem_bwd<W>());
     const TypeTab tt = make_typetab(m);
-    k_embed_bwd_f64<<<embed_grid(m, N), DP_WARPS_PER_CTA * 32, embed_smem_bytes_bwd_f64(), st>>>(
-        m->T, g.ncell, m->Nm, tt, make_env(m, g), (const EmbedNetFrag<double> *)m->embed_frag_dev, m->avg_dev,
+    k_embed_bwd_f64<W><<<embed_grid(m, N), DP_WARPS_PER_CTA * 32, smem_bwd<W>(), st>>>(
+        m->T, g.ncell, m->Nm, tt, make_env(m, g), (const EmbedNetFrag<double, W> *)m->embed_frag_dev, m->avg_dev,
         m->std_dev, (int *)(ws + L.bin_start), (double *)(ws + L.xs), (int *)(ws + L.nlist), (int *)(ws + L.nreal),
         (double *)(ws + L.gAf), (double *)(ws + L.fsorted), (double *)(ws + L.virial),
         (unsigned long long *)(ws + L.status + 16));
     return cudaGetLastError();
+}
+
+cudaError_t launch_embed_fwd_f64(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    return m->m0 == 32 ? launch_fwd_w<32>(m, N, g, ws, L, st) : launch_fwd_w<25>(m, N, g, ws, L, st);
+}
+
+cudaError_t launch_embed_bwd_f64(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    return m->m0 == 32 ? launch_bwd_w<32>(m, N, g, ws, L, st) : launch_bwd_w<25>(m, N, g, ws, L, st);
 }

@@ -71,12 +71,14 @@ __global__ void __launch_bounds__(256) k_fit_gemm(FitArgs p) {
         if (!BT) {
             for (int c = tid; c < BK * (BN / 2); c += 256) {
                 const int k = c / (BN / 2), cc = c % (BN / 2);
-                cp_async16(Bs + k * BS_STRIDE + 2 * cc, Bw + (long)(k0 + k) * p.ldb + n0 + 2 * cc, true);
+                const bool okn = n0 + 2 * cc < p.N;
+                cp_async16(Bs + k * BS_STRIDE + 2 * cc, Bw + (long)(k0 + k) * p.ldb + (okn ? n0 + 2 * cc : 0), okn);
             }
         } else {
             for (int c = tid; c < BN * (BK / 2); c += 256) {
                 const int n = c >> 3, c8 = c & 7;
-                cp_async16(Bs + n * BT_STRIDE + 2 * c8, Bw + (long)(n0 + n) * p.ldb + k0 + 2 * c8, true);
+                const bool okn = n0 + n < p.N;
+                cp_async16(Bs + n * BT_STRIDE + 2 * c8, Bw + (long)(okn ? n0 + n : 0) * p.ldb + k0 + 2 * c8, okn);
             }
         }
         cp_async_commit();
@@ -121,6 +123,7 @@ __global__ void __launch_bounds__(256) k_fit_gemm(FitArgs p) {
 #pragma unroll
         for (int nt = 0; nt < 5; ++nt) {
             const int col = n0 + wn * 40 + nt * 8 + 2 * r;
+            if (col >= p.N) continue;          // N = 16 m2 need not be a multiple of the tile width
             const long o = (long)row * p.ldo + col;
             double v0 = acc[mt][nt][0], v1 = acc[mt][nt][1];
             if (MODE == 0) {
@@ -158,7 +161,9 @@ __global__ void __launch_bounds__(256) k_fit_gemm(FitArgs p) {
 }
 
 // D[i][m*16 + a] = sum_c A[i][c][m] A[i][c][a]    (N6, Q6, Q7); one warp per atom
+template <int W>
 __global__ void __launch_bounds__(256) k_descr(long N, const double *__restrict__ Amat, double *__restrict__ D) {
+    constexpr int M2E = EmbW<W>::M2E;
     __shared__ double sA[8][4 * M2E];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const long i = blockIdx.x * 8L + wid;
@@ -196,15 +201,18 @@ __global__ void __launch_bounds__(256) k_energy(long N, int T, int ncell, const 
     if (lane == 0) eatom[i] = acc + c4[a] + ebias[a];
 }
 
+template <int W>
 __device__ __forceinline__ int feature3(int nt3, int r, int j3) {
     const int e = 4 * (nt3 >> 1) + r;
-    return e < M0 ? e + M0 * (nt3 & 1) + M1 * j3 : -1;
+    return e < W ? e + W * (nt3 & 1) + 2 * W * j3 : -1;
 }
 
 // gA[c][m] = sum_a gD[m][a] A[c][a] + [m < 16] sum_m' gD[m'][m] A[c][m']   (N8), written as the MMA fragments the
 // embedding backward consumes (layout in embed_f64.cu), pre-scaled by 1/Nm.  One warp per atom.
+template <int W>
 __global__ void __launch_bounds__(128) k_gA(long N, double inv_nm, const double *__restrict__ Amat,
                                             const double *__restrict__ gD, double *__restrict__ gAf) {
+    constexpr int M2E = EmbW<W>::M2E, NT3 = EmbW<W>::NT3;
     extern __shared__ double smg[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const long i = blockIdx.x * 4L + wid;
@@ -228,18 +236,20 @@ __global__ void __launch_bounds__(128) k_gA(long N, double inv_nm, const double 
     double *out = gAf + i * (3 * NT3 * 32);
     const int q4 = lane >> 2, r = lane & 3;
     for (int nt3 = 0; nt3 < NT3; ++nt3) {
-        const int f = feature3(nt3, q4 >> 1, q4 & 1);
+        const int f = feature3<W>(nt3, q4 >> 1, q4 & 1);
         out[nt3 * 32 + lane] = f >= 0 ? sO[r * M2E + f] : 0.0;
     }
     for (int kc = 0; kc < 2 * NT3; ++kc) {
-        const int f = feature3(kc >> 1, r, kc & 1);
+        const int f = feature3<W>(kc >> 1, r, kc & 1);
         out[(NT3 + kc) * 32 + lane] = (f >= 0 && q4 < 4) ? sO[q4 * M2E + f] : 0.0;
     }
 }
 
 }  // namespace
 
-cudaError_t launch_fit_f64(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+template <int W>
+static cudaError_t launch_fit_w(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    constexpr int M2E = EmbW<W>::M2E;
     const int F = 240, ND = M2E * 16;
     const int T = m->T;
     double *Amat = (double *)(ws + L.A);
@@ -255,7 +265,7 @@ cudaError_t launch_fit_f64(const dp_model *m, long N, const Grid3 &g, char *ws, 
     const unsigned gx = (unsigned)((N + BM - 1) / BM);
     const unsigned nb8 = (unsigned)((N + 7) / 8);
 
-    k_descr<<<nb8, 256, 0, st>>>(N, Amat, D);
+    k_descr<W><<<nb8, 256, 0, st>>>(N, Amat, D);
 
     FitArgs p{};
     p.ncell = g.ncell; p.bin_start = bin_start; p.v4 = v4; p.v4_type_stride = F; p.bias_type_stride = F;
@@ -278,10 +288,14 @@ cudaError_t launch_fit_f64(const dp_model *m, long N, const Grid3 &g, char *ws, 
     k_fit_gemm<4><<<dim3(gx, F / BN, T), 256, 0, st>>>(p);
     // layer 1 backward: gD = gz1 V1^T
     p.A = gz1; p.N = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.out0 = D; p.ldo = ND;
-    k_fit_gemm<5><<<dim3(gx, ND / BN, T), 256, 0, st>>>(p);
+    k_fit_gemm<5><<<dim3(gx, (ND + BN - 1) / BN, T), 256, 0, st>>>(p);
     // gD, A -> gA fragments for the embedding backward
     const int smem = 4 * (4 * M2E + M2E * 16 + 4 * M2E) * 8;
-    DP_SMEM_OPTIN(k_gA, smem);
-    k_gA<<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, 1.0 / (double)m->Nm, Amat, D, (double *)(ws + L.gAf));
+    DP_SMEM_OPTIN(k_gA<W>, smem);
+    k_gA<W><<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, 1.0 / (double)m->Nm, Amat, D, (double *)(ws + L.gAf));
     return cudaGetLastError();
+}
+
+cudaError_t launch_fit_f64(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    return m->m0 == 32 ? launch_fit_w<32>(m, N, g, ws, L, st) : launch_fit_w<25>(m, N, g, ws, L, st);
 }

@@ -36,6 +36,16 @@ CU_STD = (0.093189, 0.060746, 0.060746, 0.060746)
 WATER_AVG = ((0.0511, 0.0, 0.0, 0.0), (0.0499, 0.0, 0.0, 0.0))
 WATER_STD = ((0.1404, 0.0863, 0.0863, 0.0863), (0.1287, 0.0797, 0.0797, 0.0797))
 
+# The paper's own network shape (section VI-A): embedding nets (32, 64, 128), fitting nets (240, 240, 240),
+# neighbour capacities 512 (copper) and 144 (water: 48 O + 96 H).  Normalisation constants: the same statistics taken over
+# the larger capacities (padded slots count as zero rows): copper from the ideal-FCC shell sums (sum s = 12.50524,
+# sum s^2 = 2.83400 over 512 slots), water rescaled from the config-1 statistics (138 -> 144 slots).
+PAPER_EMBED_WIDTHS = (32, 64, 128)
+PAPER_CU_AVG = (0.024424, 0.0, 0.0, 0.0)
+PAPER_CU_STD = (0.070275, 0.042954, 0.042954, 0.042954)
+PAPER_WATER_AVG = ((0.04897, 0.0, 0.0, 0.0), (0.04782, 0.0, 0.0, 0.0))
+PAPER_WATER_STD = ((0.13782, 0.08448, 0.08448, 0.08448), (0.12638, 0.07802, 0.07802, 0.07802))
+
 
 @dataclasses.dataclass
 class Model:
@@ -158,7 +168,7 @@ def fcc_positions(ncell: int, a: float = 3.634) -> np.ndarray:
 
 def copper(ncell: int, sigma: float, seed: int, shuffle: bool = False, a: float = 3.634,
            rc: float = 8.0, rc_smth: float = 2.0, sel=(256,), precision="fp64",
-           name=None) -> System:
+           name=None, embed_widths=EMBED_WIDTHS, avg=CU_AVG, std=CU_STD) -> System:
     rng = np.random.default_rng(seed)
     x = fcc_positions(ncell, a)
     x = x + sigma * rng.standard_normal(x.shape)
@@ -166,7 +176,7 @@ def copper(ncell: int, sigma: float, seed: int, shuffle: bool = False, a: float 
         x = x[rng.permutation(x.shape[0])]
     L = ncell * a
     box = np.diag([L, L, L]).reshape(9).astype(np.float64)
-    model = make_model(1, rc, rc_smth, sel, seed + 1000, CU_AVG, CU_STD)
+    model = make_model(1, rc, rc_smth, sel, seed + 1000, avg, std, embed_widths=embed_widths)
     return System(name or f"cu{x.shape[0]}", np.ascontiguousarray(x),
                   np.zeros(x.shape[0], dtype=np.int32), box, model, precision)
 
@@ -217,7 +227,7 @@ def _random_rotations(n: int, rng) -> np.ndarray:
 
 
 def water(nmol: int, L: float, seed: int, rc: float = 6.0, rc_smth: float = 0.5,
-          sel=(46, 92), precision="fp64", name=None) -> System:
+          sel=(46, 92), precision="fp64", name=None, embed_widths=EMBED_WIDTHS, avg=WATER_AVG, std=WATER_STD) -> System:
     rng = np.random.default_rng(seed)
     O = _rsa_sites(nmol, L, 2.5, rng)
     R = _random_rotations(nmol, rng)
@@ -229,7 +239,7 @@ def water(nmol: int, L: float, seed: int, rc: float = 6.0, rc_smth: float = 0.5,
     x = np.stack([O, H1, H2], axis=1).reshape(-1, 3)        # O,H,H per molecule
     types = np.tile(np.array([0, 1, 1], dtype=np.int32), nmol)
     box = np.diag([L, L, L]).reshape(9).astype(np.float64)
-    model = make_model(2, rc, rc_smth, sel, seed + 1000, WATER_AVG, WATER_STD)
+    model = make_model(2, rc, rc_smth, sel, seed + 1000, avg, std, embed_widths=embed_widths)
     return System(name or f"water{3 * nmol}", np.ascontiguousarray(x), types, box, model, precision)
 
 
@@ -250,6 +260,30 @@ def config(idx: int) -> System:
     if idx == 4:
         return copper(64, 0.1, SEED0 + 4, shuffle=True, name="c4_cu1048576", precision="mix16")
     raise ValueError(idx)
+
+
+# ----------------------------------------------------------------------------- the paper's network shape
+def paper_copper(ncell: int, seed: int, sigma: float = 0.05, shuffle: bool = False, precision="fp64", name=None) -> System:
+    """Copper with the paper's networks: embedding (32, 64, 128), capacity 512, rc 8 A."""
+    return copper(ncell, sigma, seed, shuffle=shuffle, sel=(512,), precision=precision, name=name or f"paper_cu{4 * ncell ** 3}",
+                  embed_widths=PAPER_EMBED_WIDTHS, avg=PAPER_CU_AVG, std=PAPER_CU_STD)
+
+
+def paper_water(nmol: int, L: float, seed: int, precision="fp64", name=None) -> System:
+    """Water with the paper's networks: embedding (32, 64, 128), capacity 144 = 48 O + 96 H, rc 6 A."""
+    return water(nmol, L, seed, sel=(48, 96), precision=precision, name=name or f"paper_water{3 * nmol}",
+                 embed_widths=PAPER_EMBED_WIDTHS, avg=PAPER_WATER_AVG, std=PAPER_WATER_STD)
+
+
+def paper_config(name: str, precision="fp64") -> System:
+    """Bench workloads at the paper's network shape: 'paper_cu' copper 32^3 cells = 131,072 atoms, 'paper_water' 36,864
+    molecules = 110,592 atoms in the config-3 box (the paper's single-GPU runs: 4,860 Cu / 24,576 water atoms on a V100,
+    PAPER.md Fig. 4; scaled to one B200)."""
+    if name == "paper_cu":
+        return paper_copper(32, SEED0 + 10, sigma=0.05, shuffle=True, precision=precision, name="paper_cu131072")
+    if name == "paper_water":
+        return paper_water(36864, 97.4, SEED0 + 11, precision=precision, name="paper_water110592")
+    raise ValueError(name)
 
 
 # ----------------------------------------------------------------------------- tiny systems for self-tests
