@@ -156,6 +156,10 @@ int dp_md_run(dp_model *m, long natoms, double *coords_dev, double *vel_dev, con
 #define DP_NPEAKS 6
 int dp_measure_peaks(double *out_host, int n_out, void *cuda_stream);
 
+/* Diagnostic for DP_ECUDA: the CUDA runtime's message for the first failing call of the last dp_compute on this model and,
+ * in *step (may be NULL), the ordinal of that call inside dp_compute.  The string is static. */
+const char *dp_last_cuda_error(const dp_model *m, int *step);
+
 void dp_destroy(dp_model *m);
 const char *dp_strerror(int code);
 

@@ -18,7 +18,7 @@ DP_FP64, DP_MIX32, DP_MIX16 = 0, 1, 2
 PRECISIONS = {"fp64": DP_FP64, "mix32": DP_MIX32, "mix16": DP_MIX16}
 EXPORTS = ["dp_create", "dp_workspace_bytes", "dp_compute", "dp_get_nlist", "dp_status",
            "dp_launches_per_compute", "dp_last_row_counts", "dp_profile_enable", "dp_profile_read", "dp_md_run",
-           "dp_md_workspace_bytes", "dp_measure_peaks", "dp_destroy", "dp_strerror"]
+           "dp_md_workspace_bytes", "dp_measure_peaks", "dp_last_cuda_error", "dp_destroy", "dp_strerror"]
 
 
 class DPError(RuntimeError):
@@ -71,6 +71,8 @@ def lib():
         L.dp_md_workspace_bytes.argtypes = [vp, C.c_long, C.c_double, dp]
         L.dp_measure_peaks.restype = C.c_int
         L.dp_measure_peaks.argtypes = [dp, C.c_int, vp]
+        L.dp_last_cuda_error.restype = C.c_char_p
+        L.dp_last_cuda_error.argtypes = [vp, C.POINTER(C.c_int)]
         L.dp_destroy.restype = None
         L.dp_destroy.argtypes = [vp]
         _lib = L
@@ -146,7 +148,11 @@ class DPModel:
                               out["atom_energy"].data_ptr() if want_atom_energy else None,
                               out["forces"].data_ptr(), out["virial"].data_ptr() if want_virial else None)
         if rc != 0:
-            raise DPError(rc, "dp_compute")
+            where = "dp_compute"
+            if rc == -5:
+                step = C.c_int(0)
+                where += f" [{lib().dp_last_cuda_error(self._h, C.byref(step)).decode()}, call {step.value}]"
+            raise DPError(rc, where)
         self._n = n
         return out
 

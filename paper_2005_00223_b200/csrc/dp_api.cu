@@ -79,7 +79,7 @@ bool rows_fit_int32(const dp_model *m, long N) {
 // Cell grid of one evaluation.  Orthorhombic boxes with every length >= 2 rc take the minimum-image path (nlist.cu);
 // everything else (a general cell, or an edge shorter than 2 rc) takes the ghost path (ghost.cu).  false: degenerate box.
 // (32, 64, 128) networks: which precision modes have kernels for them
-bool paper_shape_supported(dp_precision prec) { return prec == DP_FP64; }
+bool paper_shape_supported(dp_precision prec) { return prec == DP_FP64 || prec == DP_MIX16; }
 
 bool make_grid(const dp_model *m, long N, const double *box, Grid3 *g) {
     *g = Grid3{};
@@ -287,8 +287,10 @@ void build_embed_tc(const double *net, EmbedNetTC<NSW> *out) {
 }
 
 // MIX-16 operand images of the warpgroup-per-tile kernels (embed_tc2.cuh): fp16 weights ("stored in half precision",
-// PAPER.md:125), biases as hi + lo rows multiplied by the constant-one columns, residual folds pre-summed in fp64.
-void build_embed_tc2(const double *net, EmbedNetTC2 *out) {
+// PAPER.md:125), biases as hi + lo rows multiplied by constant-one columns, residual folds pre-summed in fp64.
+template <int W>
+void build_embed_tc2(const double *net, EmbedNetTC2<W> *out) {
+    constexpr int M0 = T2<W>::M0, M1 = T2<W>::M1, M2E = T2<W>::M2E;
     const double *W1 = net, *b1 = W1 + M0, *W2 = b1 + M0, *b2 = W2 + M0 * M1, *W3 = b2 + M1, *b3 = W3 + M1 * M2E;
     std::memset(out, 0, sizeof(*out));
     for (int e = 0; e < M0; ++e) { out->w1[e] = (float)W1[e]; out->b1[e] = (float)b1[e]; }
@@ -297,8 +299,8 @@ void build_embed_tc2(const double *net, EmbedNetTC2 *out) {
         for (int n = 0; n < M1; ++n) {
             double v = 0.0;
             if (k < M0) v = W2[k * M1 + n];
-            else if (k == T2_ONE_HI) v = hpart(b2[n], 0);
-            else if (k == T2_ONE_LO) v = hpart(b2[n], 1);
+            else if (!T2<W>::ONES_STEP && k == T2_ONE_HI) v = hpart(b2[n], 0);
+            else if (!T2<W>::ONES_STEP && k == T2_ONE_LO) v = hpart(b2[n], 1);
             out->W2[k >> 3][n][k & 7] = h(v);
         }
     for (int k = 0; k < T2_K2 + T2_K1; ++k)
@@ -308,8 +310,8 @@ void build_embed_tc2(const double *net, EmbedNetTC2 *out) {
             else if (k >= T2_K2) {
                 const int e = k - T2_K2;
                 if (e < M0) v = W3[e * M2E + m] + W3[(e + M0) * M2E + m];
-                else if (e == T2_ONE_HI) v = hpart(b3[m], 0);
-                else if (e == T2_ONE_LO) v = hpart(b3[m], 1);
+                else if (!T2<W>::ONES_STEP && e == T2_ONE_HI) v = hpart(b3[m], 0);
+                else if (!T2<W>::ONES_STEP && e == T2_ONE_LO) v = hpart(b3[m], 1);
             }
             out->W3[k >> 3][m][k & 7] = h(v);
         }
@@ -319,6 +321,10 @@ void build_embed_tc2(const double *net, EmbedNetTC2 *out) {
     }
     for (int k = 0; k < M1; ++k)             // k = layer-2 feature f
         for (int e = 0; e < M0; ++e) out->W2T[k >> 3][e][k & 7] = h(W2[e * M1 + k]);
+    if (T2<W>::ONES_STEP) {                  // bias rows of the ones step: k = 0 hi part, k = 1 lo part
+        for (int n = 0; n < M1; ++n) { out->Bb2[n][0] = h(hpart(b2[n], 0)); out->Bb2[n][1] = h(hpart(b2[n], 1)); }
+        for (int m = 0; m < M2E; ++m) { out->Bb3[m][0] = h(hpart(b3[m], 0)); out->Bb3[m][1] = h(hpart(b3[m], 1)); }
+    }
 }
 
 template <typename Tp>
@@ -442,12 +448,18 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
         for (int ab = 0; ab < T * T; ++ab) build_embed_tc<2>(w->embed + ab * ensz, &nets[ab]);
         ok(upload(nets, &m->embed_tc_dev));
     } else {                            // MIX-16: warpgroup-per-tile tcgen05 kernels (embed_tc2*.cu)
-        std::vector<EmbedNetTC2> nets((size_t)T * T);
-        for (int ab = 0; ab < T * T; ++ab) build_embed_tc2(w->embed + ab * ensz, &nets[ab]);
-        ok(upload(nets, &m->embed_tc2_dev));
+        if (W0 == 32) {
+            std::vector<EmbedNetTC2<32>> nets((size_t)T * T);
+            for (int ab = 0; ab < T * T; ++ab) build_embed_tc2<32>(w->embed + ab * ensz, &nets[ab]);
+            ok(upload(nets, &m->embed_tc2_dev));
+        } else {
+            std::vector<EmbedNetTC2<25>> nets((size_t)T * T);
+            for (int ab = 0; ab < T * T; ++ab) build_embed_tc2<25>(w->embed + ab * ensz, &nets[ab]);
+            ok(upload(nets, &m->embed_tc2_dev));
+        }
         // short neighbour rows: the forward's rounding of the activations to one fp16 value averages over too few rows to
         // hold the MIX-16 force tolerance (measured): carry them as hi + lo pairs there
-        m->fwd_split = Nm < 128 ? 1 : 0;
+        m->fwd_split = (Nm < 128 && W0 == 25) ? 1 : 0;
         if (m->fwd_split) {
             std::vector<EmbedNetTC<1>> n1((size_t)T * T);
             for (int ab = 0; ab < T * T; ++ab) build_embed_tc<1>(w->embed + ab * ensz, &n1[ab]);
@@ -481,9 +493,9 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
     }
     // MIX-16: tcgen05 fitting GEMMs (fit_tc.cu) take fp16 weight images; activations are carried as hi + lo fp16 pairs
     if (prec == DP_MIX16) {
-        std::vector<__half> img((size_t)T * fit_tc_type_elems());
+        std::vector<__half> img((size_t)T * fit_tc_type_elems(ND));
         for (int a = 0; a < T; ++a)
-            fit_tc_build_type(&V1[(size_t)a * ND * F], &V2[(size_t)a * F * F], &V3[(size_t)a * F * F], &img[(size_t)a * fit_tc_type_elems()]);
+            fit_tc_build_type(ND, &V1[(size_t)a * ND * F], &V2[(size_t)a * F * F], &V3[(size_t)a * F * F], &img[(size_t)a * fit_tc_type_elems(ND)]);
         ok(upload(img, &m->fit_tc_img_dev));
     }
     std::vector<double> avg(w->avg, w->avg + 4 * T), sd(w->std, w->std + 4 * T), eb(w->ebias, w->ebias + T);
@@ -542,7 +554,8 @@ int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *ty
     cudaStream_t st = (cudaStream_t)cuda_stream;
     char *ws = (char *)workspace_dev;
     cudaError_t e = cudaSuccess;
-    auto ok = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
+    int step = 0;
+    auto ok = [&](cudaError_t x) { ++step; if (e == cudaSuccess && x != cudaSuccess) { e = x; m->last_cuda_error = (int)x; m->last_cuda_step = step; } };
     // status word 0 = error flags: cleared per call, except inside one dp_md_run, where they accumulate (dp_status then
     // reports the whole run); the counters behind it are per evaluation
     ok(m->keep_flags ? cudaMemsetAsync(ws + L.status + 4, 0, 60, st) : cudaMemsetAsync(ws + L.status, 0, 64, st));
@@ -575,6 +588,12 @@ int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *ty
     mark(5);
     m->last_natoms = natoms; m->last_next = g.cap_ext; m->last_ws = workspace_dev; m->last_stream = st;
     return e == cudaSuccess ? DP_OK : DP_ECUDA;
+}
+
+const char *dp_last_cuda_error(const dp_model *m, int *step) {
+    if (!m) return "no model";
+    if (step) *step = m->last_cuda_step;
+    return cudaGetErrorString((cudaError_t)m->last_cuda_error);
 }
 
 int dp_profile_enable(dp_model *m, int on) {

@@ -95,6 +95,7 @@ struct dp_model {
     cudaStream_t last_stream;
     int sort_cap;
     int profile;
+    int last_cuda_error, last_cuda_step;   // first failing CUDA call of the last dp_compute (dp_last_cuda_error)
     // buffered neighbour list of the MD loop (md.cu sets these around its dp_compute calls; 0 / null otherwise)
     int list_mode;                  // 0: search the cells every call; 1: search with rc + skin and store candidates; 2: reuse them
     int keep_flags;                 // dp_md_run, evaluations after the first: device error flags accumulate over the whole run
@@ -195,7 +196,7 @@ cudaError_t launch_embed_fwd_tc(const dp_model *m, long N, const Grid3 &g, char 
 cudaError_t launch_embed_fwd_tc2(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_embed_bwd_tc2(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_fit_tc(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
-size_t fit_tc_type_elems();
-void fit_tc_build_type(const double *V1, const double *V2, const double *V3, struct __half *out);
+size_t fit_tc_type_elems(int nd);
+void fit_tc_build_type(int nd, const double *V1, const double *V2, const double *V3, struct __half *out);
 cudaError_t launch_env_rows(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);

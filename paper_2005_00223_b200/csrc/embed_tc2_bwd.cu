@@ -25,30 +25,38 @@ namespace {
 
 constexpr int NWG = 2;
 // TMEM columns per warpgroup
-constexpr int TM_T = 0;                        // T hi parts, packed fp16 pairs: t1 [0,16) t2 [16,48) t3 [48,104)
-constexpr int TM_Z = 112;                      // accumulator: z2 -> z3 -> dT3 -> [dy2 | dy1]      (112 columns)
-constexpr int TM_DR = 224;                     // dR^: 2 slots x 8 columns
+constexpr int TM_T = 0;                        // T hi parts, packed fp16 pairs: t1 [0,16) t2 [16,48) t3 [48,48 + K3/2)
+constexpr int TM_Z = 112;                      // accumulator: z2 -> z3 -> dT3 -> [dy2 | dy1]      (K3 columns)
 constexpr int TM_WG = 256;
 
+template <int W>
 struct BwdSmem {
+    using L = T2<W>;
+    static constexpr int TM_DR = TM_Z + L::K3;                     // dR^: 2 slots x 8 columns (TMEM columns 224 / 240)
+    static_assert(TM_DR + 16 <= TM_WG && 48 + L::K3 / 2 <= TM_Z, "TMEM budget");
     static constexpr int W2 = 0;                                   // [4][64][16 B]
-    static constexpr int W3 = W2 + 4 * 64 * 16;                    // [12][112][16 B]
-    static constexpr int W3T = W3 + 12 * 112 * 16;                 // [14][96][16 B]
-    static constexpr int W2T = W3T + 14 * 96 * 16;                 // [8][32][16 B]
-    static constexpr int VEC = W2T + 8 * 32 * 16;                  // w1[32] b1[32]
+    static constexpr int W3 = W2 + 4 * 64 * 16;                    // [12][K3][16 B]
+    static constexpr int W3T = W3 + 12 * L::K3 * 16;               // [K3/8][96][16 B]
+    static constexpr int W2T = W3T + (L::K3 / 8) * 96 * 16;        // [8][32][16 B]
+    static constexpr int BB2 = W2T + 8 * 32 * 16;                  // ONES_STEP: bias chunks and the ones image (embed_tc2.cuh)
+    static constexpr int BB3 = BB2 + (L::ONES_STEP ? 64 * 16 : 0);
+    static constexpr int ONES = BB3 + (L::ONES_STEP ? L::K3 * 16 : 0);
+    static constexpr int VEC = ONES + (L::ONES_STEP ? 256 : 0);    // w1[32] b1[32]
     static constexpr int BARS = VEC + 256;
-    static constexpr int WG0 = ((BARS + 64 + 1023) / 1024) * 1024;
+    static constexpr int WG0 = ((BARS + 64 + 127) / 128) * 128;
     // per warpgroup
-    static constexpr int TLO = 0;                                  // T lo parts / dz2 / dz3: 26 chunks x 2 KB
-    static constexpr int RIMG = TLO + T2_CHUNKS * 2048;            // A of the direct products: [4][128][16 B]
-    static constexpr int QIMG = RIMG + 4 * 2048;                   // per slot two copies of the atom's gradient image C [208][16 B]:
-                                                                   // K-major B of the direct products (K = 16 per slot) and,
-                                                                   // viewed MN-major (chunks 0 and 2), B of the dR^ product (N = 16)
-    static constexpr int META = QIMG + 4 * T2_COLS * 16;
+    static constexpr int TLO = 0;                                  // T lo parts / dz2 / dz3: CHUNKS x 2 KB
+    static constexpr int RIMG = TLO + L::CHUNKS * 2048;            // A of the direct products: [4][128][16 B]
+    // per slot the atom's gradient image C [COLS][16 B]: K-major B of the direct products (K = 16 per slot: both K chunks
+    // read the same image; W = 25 keeps two copies, W = 32 aliases them through a zero leading stride) and, viewed MN-major,
+    // B of the dR^ product (N = 16)
+    static constexpr int QCOPIES = W == 25 ? 2 : 1;
+    static constexpr int QIMG = RIMG + 4 * 2048;
+    static constexpr int META = QIMG + 2 * QCOPIES * L::COLS * 16;
     static constexpr int WG_BYTES = ((META + 2 * 3072 + 127) / 128) * 128;   // META: two stages of prefetched row data
     static constexpr int TOTAL = WG0 + NWG * WG_BYTES;
+    static_assert(TOTAL + 1024 <= 227 * 1024, "shared memory budget (1 KB: alignment of the dynamic array behind the static word)");
 };
-static_assert(BwdSmem::TOTAL <= 227 * 1024, "shared memory budget");
 
 __device__ __forceinline__ double min_image(double t, double L, double halfL) {
     double s = t > halfL ? -1.0 : (t < -halfL ? 1.0 : 0.0);
@@ -85,11 +93,12 @@ __device__ __forceinline__ void act16(const uint32_t (&z)[16], uint32_t tm_dst, 
     *reinterpret_cast<uint4 *>(lo_row + (chunk + 1) * 2048) = make_uint4(lo[4], lo[5], lo[6], lo[7]);
 }
 // Per-atom operand image of the folded gradient g~[c][col] = fold(gA)[c][col] * 2^e, split in hi + lo fp16 parts:
-//   C [208][8] : per T column {hi[0..3], lo[0..3]} (16 bytes)
-constexpr int GA_IMG_BYTES = T2_COLS * 16;    // 3,328 per atom
+//   C [COLS][8] : per T column {hi[0..3], lo[0..3]} (16 bytes); 3,328 / 3,584 bytes per atom
 // Built from gA (fp32 [N][4][100], written by the epilogue of the last fitting-backward GEMM, fit_tc.cu MODE 6).
+template <int W>
 __global__ void __launch_bounds__(256) k_gA_fold(long N, const float *__restrict__ gA, uint8_t *__restrict__ img,
                                                   float *__restrict__ gscale) {
+    constexpr int M0 = T2<W>::M0, M1 = T2<W>::M1, M2E = T2<W>::M2E, COLS = T2<W>::COLS, GA_IMG_BYTES = COLS * 16;
     __shared__ __align__(16) float sO_all[8][4 * M2E];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const long i = blockIdx.x * 8L + wid;
@@ -109,7 +118,7 @@ __global__ void __launch_bounds__(256) k_gA_fold(long N, const float *__restrict
             float x = 0.f;
             if (col < T2_O2) { if (col < M0) x = (o[col] + o[col + M0]) + (o[col + 2 * M0] + o[col + 3 * M0]); }
             else if (col < T2_O3) { const int f = col - T2_O2; if (f < M1) x = o[f] + o[f + M1]; }
-            else if (col < T2_COLS) { const int m = col - T2_O3; if (m < M2E) x = o[m]; }
+            else if (col < COLS) { const int m = col - T2_O3; if (m < M2E) x = o[m]; }
             v[j][c] = x;
             mx = fmaxf(mx, fabsf(x));
         }
@@ -124,7 +133,7 @@ __global__ void __launch_bounds__(256) k_gA_fold(long N, const float *__restrict
 #pragma unroll
     for (int j = 0; j < 7; ++j) {
         const int col = lane + 32 * j;
-        if (col < T2_COLS) {
+        if (col < COLS) {
             uint32_t h01, l01, h23, l23;
             tc::split_h2(v[j][0] * sc, v[j][1] * sc, h01, l01);
             tc::split_h2(v[j][2] * sc, v[j][3] * sc, h23, l23);
@@ -163,13 +172,18 @@ __device__ __forceinline__ void gradh16(const uint32_t (&g)[16], const uint32_t 
 
 constexpr int WGT = 128;       // threads per warpgroup: thread = row; every stage walks its two column halves h = 0, 1
 
+template <int W>
 __global__ void __launch_bounds__(NWG * WGT, 1)
-k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, const EmbedNetTC2 *__restrict__ nets,
+k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, const EmbedNetTC2<W> *__restrict__ nets,
                 const double *__restrict__ stdv, const int *__restrict__ bin_start, const int *__restrict__ rowstart,
                 const float4 *__restrict__ rows_rh, const int2 *__restrict__ rows_id, const uint8_t *__restrict__ gimg,
                 const float *__restrict__ gscale, float4 *__restrict__ rows_g, unsigned long long *__restrict__ row_counter,
                 long long *__restrict__ tdbg) {
-    using SL = BwdSmem;
+    using SL = BwdSmem<W>;
+    using LY = T2<W>;
+    constexpr int M0 = LY::M0, K3 = LY::K3, COLS = LY::COLS, GA_IMG_BYTES = COLS * 16, TM_DR = SL::TM_DR, QC = SL::QCOPIES;
+    constexpr int HW3 = K3 / 2 - (W == 25 ? 8 : 0);     // t3 columns handled per column half by full 16-column groups: 48 / 64
+    constexpr int NU3 = HW3 / 16;                      // 16-column groups per half: 3 / 4
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ uint32_t tmem_base_s;
     const int tid = threadIdx.x;
@@ -201,8 +215,10 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
     const uint32_t s_qimg = tc::smem_u32(wgs + SL::QIMG);
     // operand descriptors are built once; every MMA adds a compile-time offset
     const uint64_t d_tlo = tc::desc(s_tlo, 2048, 128), d_rimg = tc::desc(s_rimg, 2048, 128);
-    const uint64_t d_qk = tc::desc(s_qimg, T2_COLS * 16, 128), d_qmn = tc::desc(s_qimg, 128, 2 * T2_COLS * 16);
-    const uint64_t d_w2 = tc::desc(sbase + SL::W2, 64 * 16, 128), d_w3 = tc::desc(sbase + SL::W3, 112 * 16, 128);
+    const uint64_t d_qk = tc::desc(s_qimg, QC == 2 ? COLS * 16 : 0, 128), d_qmn = tc::desc(s_qimg, 128, QC * COLS * 16);
+    const uint64_t d_w2 = tc::desc(sbase + SL::W2, 64 * 16, 128), d_w3 = tc::desc(sbase + SL::W3, K3 * 16, 128);
+    const uint64_t d_ones = tc::desc(sbase + SL::ONES, 128, 0), d_bb2 = tc::desc(sbase + SL::BB2, 0, 128), d_bb3 = tc::desc(sbase + SL::BB3, 0, 128);
+    (void)d_ones; (void)d_bb2; (void)d_bb3;
     const uint64_t d_w3t = tc::desc(sbase + SL::W3T, 96 * 16, 128), d_w2t = tc::desc(sbase + SL::W2T, 32 * 16, 128);
     uint64_t *bar = &bars[wg];
     uint32_t ph = 0;
@@ -216,7 +232,7 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
     {
         uint32_t z8[8] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
 #pragma unroll
-        for (int c = 0; c < 104; c += 8) tc::st8(tm_lane + TM_T + c, z8);
+        for (int c = 0; c < 48 + K3 / 2; c += 8) tc::st8(tm_lane + TM_T + c, z8);
     }
     tc::wait_st();
 
@@ -241,10 +257,13 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
             const int ntiles = (re - rs + T2_ROWS - 1) / T2_ROWS;
             __syncthreads();
             {   // stage the (a, b) net
-                const EmbedNetTC2 *net = nets + (a * T + b);
+                const EmbedNetTC2<W> *net = nets + (a * T + b);
                 const uint4 *src = reinterpret_cast<const uint4 *>(&net->W2[0][0][0]);
-                constexpr int NW = (4 * 64 + 12 * 112 + 14 * 96 + 8 * 32);
+                // W2, W3, W3T, W2T (and, with the ones step, the bias chunks) are contiguous in the struct and in shared memory
+                constexpr int NW = (4 * 64 + 12 * K3 + (K3 / 8) * 96 + 8 * 32) + (LY::ONES_STEP ? 64 + K3 : 0);
                 for (int k = tid; k < NW; k += NWG * WGT) reinterpret_cast<uint4 *>(smem + SL::W2)[k] = src[k];
+                if (LY::ONES_STEP && tid < 16)
+                    reinterpret_cast<uint4 *>(smem + SL::ONES)[tid] = tid < 8 ? make_uint4(0x3c003c00u, 0u, 0u, 0u) : make_uint4(0u, 0u, 0u, 0u);
                 if (tid < 64) sw1[tid] = reinterpret_cast<const float *>(net)[tid];
             }
             tc::proxy_fence();
@@ -300,12 +319,12 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
                     for (int q = p0; q < p0 + T2_NSLOT && q <= atomL; ++q) {
                         const int s_ = q & (T2_NSLOT - 1);
                         const uint4 *C = reinterpret_cast<const uint4 *>(gimg + (long)q * GA_IMG_BYTES);
-                        for (int k = tw; k < T2_COLS; k += WGT) {
-                            cp_async16(s_qimg + (2 * s_) * (T2_COLS * 16) + k * 16, C + k);
-                            cp_async16(s_qimg + (2 * s_ + 1) * (T2_COLS * 16) + k * 16, C + k);
+                        for (int k = tw; k < COLS; k += WGT) {
+                            cp_async16(s_qimg + (QC * s_) * (COLS * 16) + k * 16, C + k);
+                            if (QC == 2) cp_async16(s_qimg + (2 * s_ + 1) * (COLS * 16) + k * 16, C + k);
                         }
                     }
-                    uint32_t d1p[2][8], d2p[2][16], d3p[2][26];       // 1 - t^2 per column half (fp16 pairs; only layer 3's are read back)
+                    uint32_t d1p[2][8], d2p[2][16], d3p[2][HW3 / 2 + 2];   // 1 - t^2 per column half (fp16 pairs; only layer 3's are read back)
                     float d2f[2][32], d1f[2][16];     // layers 1-2 keep 1 - t^2 in fp32: fp16 here costs 2x in force error
                     DP_TICK(0);
                     // ---- E1: layer 1 on the ALUs; h = 0: t1[0..16), h = 1: t1[16..25), ones, padding ----
@@ -316,8 +335,8 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
 #pragma unroll
                         for (int e = 0; e < 16; ++e) {
                             const int ee = 16 * h + e;
-                            if (ee < 25) y[e] = tc::tanh_approx(fmaf(s, sw1[ee], sb1[ee]));
-                            else y[e] = ee <= 26 ? 1.f : 0.f;
+                            if (ee < M0) y[e] = tc::tanh_approx(fmaf(s, sw1[ee], sb1[ee]));
+                            else y[e] = (!LY::ONES_STEP && ee <= T2_ONE_LO) ? 1.f : 0.f;
                         }
                         emit16(y, tm_lane + TM_T + 8 * h, lo_row, 2 * h, d1p[h]);
 #pragma unroll
@@ -335,6 +354,7 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
                             tc::mma_ts(tmem + TM_Z, tmem + TM_T + 8 * ks, db, id2, ks > 0);
                             tc::mma_ss(tmem + TM_Z, tc::desc_at(d_tlo, ks * 2 * 2048), db, id2, true);
                         }
+                        if (LY::ONES_STEP) tc::mma_ss(tmem + TM_Z, d_ones, d_bb2, id2, true);
                         tc::commit(bar);
                     }
                     DP_TICK(2);
@@ -345,17 +365,18 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
                     for (int h = 0; h < 2; ++h) {
                         uint8_t *img = lo_row + (T2_O2 / 8) * 2048;
                         uint32_t z0[16], z1[16];
+                        const bool full = h == 0 || W != 25;        // this half has 32 real columns (W = 25, h = 1: 18)
                         tc::ld16(tm_lane + TM_Z + 32 * h, z0);
-                        if (h == 0) tc::ld16(tm_lane + TM_Z + 16, z1);
+                        if (full) tc::ld16(tm_lane + TM_Z + 32 * h + 16, z1);
                         else tc::ld2(tm_lane + TM_Z + 48, reinterpret_cast<uint32_t (&)[2]>(z1));
                         tc::wait_ld();
                         act16(z0, tm_lane + TM_T + 16 + 16 * h, img, 4 * h, d2p[h]);
 #pragma unroll
                         for (int q = 0; q < 16; ++q) { const float tt = tc::tanh_approx(__uint_as_float(z0[q])); d2f[h][q] = fmaf(-tt, tt, 1.f); }
 #pragma unroll
-                        for (int q = 0; q < 16; ++q) { const float tt = tc::tanh_approx(__uint_as_float(z1[q & (h ? 1 : 15)])); d2f[h][16 + q] = fmaf(-tt, tt, 1.f); }
-                        if (h == 0) {
-                            act16(z1, tm_lane + TM_T + 24, img, 2, d2p[h] + 8);
+                        for (int q = 0; q < 16; ++q) { const float tt = tc::tanh_approx(__uint_as_float(z1[q & (full ? 15 : 1)])); d2f[h][16 + q] = fmaf(-tt, tt, 1.f); }
+                        if (full) {
+                            act16(z1, tm_lane + TM_T + 24 + 16 * h, img, 4 * h + 2, d2p[h] + 8);
                         } else {
                             const float x = tc::tanh_approx(__uint_as_float(z1[0])), y = tc::tanh_approx(__uint_as_float(z1[1]));
                             uint32_t hi, lo;
@@ -370,15 +391,16 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
                     sync_issue();
                     if (issuer_warp && tc::elect_one()) {
                         tc::fence_after();
-                        constexpr uint32_t id3 = tc::idesc(128, 112, false, false);
+                        constexpr uint32_t id3 = tc::idesc(128, K3, false, false);
 #pragma unroll
                         for (int ks = 0; ks < 6; ++ks) {
                             const int acol = ks < 4 ? 16 + 8 * ks : 8 * (ks - 4);              // TMEM column of the hi part
                             const int achunk = ks < 4 ? T2_O2 / 8 + 2 * ks : 2 * (ks - 4);     // chunk of the lo part
-                            const uint64_t db = tc::desc_at(d_w3, ks * 2 * (112 * 16));
+                            const uint64_t db = tc::desc_at(d_w3, ks * 2 * (K3 * 16));
                             tc::mma_ts(tmem + TM_Z, tmem + TM_T + acol, db, id3, ks > 0);
                             tc::mma_ss(tmem + TM_Z, tc::desc_at(d_tlo, achunk * 2048), db, id3, true);
                         }
+                        if (LY::ONES_STEP) tc::mma_ss(tmem + TM_Z, d_ones, d_bb3, id3, true);
                         tc::commit(bar);
                     }
                     DP_TICK(5);
@@ -387,15 +409,15 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
                     // ---- E3: h = 0: t3[0..48), h = 1: t3[48..100) ----
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
-                        uint8_t *img = lo_row + (T2_O3 / 8 + 6 * h) * 2048;
+                        uint8_t *img = lo_row + (T2_O3 / 8 + (HW3 / 8) * h) * 2048;
 #pragma unroll
-                        for (int u = 0; u < 3; ++u) {
+                        for (int u = 0; u < NU3; ++u) {
                             uint32_t z0[16];
-                            tc::ld16(tm_lane + TM_Z + 48 * h + 16 * u, z0);
+                            tc::ld16(tm_lane + TM_Z + HW3 * h + 16 * u, z0);
                             tc::wait_ld();
-                            act16(z0, tm_lane + TM_T + 48 + 24 * h + 8 * u, img, 2 * u, d3p[h] + 8 * u);
+                            act16(z0, tm_lane + TM_T + 48 + (HW3 / 2) * h + 8 * u, img, 2 * u, d3p[h] + 8 * u);
                         }
-                        if (h == 1) {
+                        if (W == 25 && h == 1) {
                             uint32_t z3[4];
                             tc::ld4(tm_lane + TM_Z + 96, z3);
                             tc::wait_ld();
@@ -418,15 +440,15 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
                         tc::fence_after();
                         constexpr uint32_t idr = tc::idesc(128, 8 * T2_NSLOT, false, true);
 #pragma unroll
-                        for (int ks = 0; ks < T2_COLS / 16; ++ks) {
+                        for (int ks = 0; ks < COLS / 16; ++ks) {
                             const uint64_t db = tc::desc_at(d_qmn, ks * 256);
                             tc::mma_ts(tmem + TM_DR, tmem + TM_T + 8 * ks, db, idr, ks > 0);
                             tc::mma_ss(tmem + TM_DR, tc::desc_at(d_tlo, ks * 2 * 2048), db, idr, true);
                         }
-                        constexpr uint32_t idg = tc::idesc(128, T2_K3, false, false);
+                        constexpr uint32_t idg = tc::idesc(128, K3, false, false);
 #pragma unroll
                         for (int ks = 0; ks < T2_NSLOT; ++ks)
-                            tc::mma_ss(tmem + TM_Z, tc::desc_at(d_rimg, ks * 2 * 2048), tc::desc_at(d_qk, T2_O3 * 16 + ks * 2 * (T2_COLS * 16)), idg, ks > 0);
+                            tc::mma_ss(tmem + TM_Z, tc::desc_at(d_rimg, ks * 2 * 2048), tc::desc_at(d_qk, T2_O3 * 16 + ks * QC * (COLS * 16)), idg, ks > 0);
                         tc::commit(bar);
                     }
                     float gsc = 1.f;
@@ -442,13 +464,13 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
 #pragma unroll
                         for (int h = 0; h < 2; ++h) {
 #pragma unroll
-                            for (int u = 0; u < 3; ++u) {
+                            for (int u = 0; u < NU3; ++u) {
                                 uint32_t g0[16];
-                                tc::ld16(tm_lane + TM_Z + 48 * h + 16 * u, g0);
+                                tc::ld16(tm_lane + TM_Z + HW3 * h + 16 * u, g0);
                                 tc::wait_ld();
-                                gradh16(g0, d3p[h] + 8 * u, tm_lane + TM_T + 48 + 24 * h + 8 * u);
+                                gradh16(g0, d3p[h] + 8 * u, tm_lane + TM_T + 48 + (HW3 / 2) * h + 8 * u);
                             }
-                            if (h == 1) {
+                            if (W == 25 && h == 1) {
                                 uint32_t g3[4];
                                 tc::ld4(tm_lane + TM_Z + 96, g3);
                                 tc::wait_ld();
@@ -470,18 +492,18 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
                         constexpr uint32_t idy2 = tc::idesc(128, 64, false, false);
 #pragma unroll
                         for (int ks = 0; ks < T2_NSLOT; ++ks)      // direct part dT2 -> accumulator columns [32,96)
-                            tc::mma_ss(tmem + TM_Z + 32, tc::desc_at(d_rimg, ks * 2 * 2048), tc::desc_at(d_qk, T2_O2 * 16 + ks * 2 * (T2_COLS * 16)), idy2, ks > 0);
+                            tc::mma_ss(tmem + TM_Z + 32, tc::desc_at(d_rimg, ks * 2 * 2048), tc::desc_at(d_qk, T2_O2 * 16 + ks * QC * (COLS * 16)), idy2, ks > 0);
 #pragma unroll
-                        for (int ks = 0; ks < T2_K3 / 16; ++ks)
+                        for (int ks = 0; ks < K3 / 16; ++ks)
                             tc::mma_ts(tmem + TM_Z + 32, tmem + TM_T + 48 + 8 * ks, tc::desc_at(d_w3t, 32 * 16 + ks * 2 * (96 * 16)), idy2, true);
                         tc::commit(bar);
                         // ... then the part of dy1 that does not depend on dz2 (waited for with the last stage)
                         constexpr uint32_t idy1 = tc::idesc(128, 32, false, false);
 #pragma unroll
                         for (int ks = 0; ks < T2_NSLOT; ++ks)      // direct part dT1 -> accumulator columns [0,32)
-                            tc::mma_ss(tmem + TM_Z, tc::desc_at(d_rimg, ks * 2 * 2048), tc::desc_at(d_qk, ks * 2 * (T2_COLS * 16)), idy1, ks > 0);
+                            tc::mma_ss(tmem + TM_Z, tc::desc_at(d_rimg, ks * 2 * 2048), tc::desc_at(d_qk, ks * QC * (COLS * 16)), idy1, ks > 0);
 #pragma unroll
-                        for (int ks = 0; ks < T2_K3 / 16; ++ks)
+                        for (int ks = 0; ks < K3 / 16; ++ks)
                             tc::mma_ts(tmem + TM_Z, tmem + TM_T + 48 + 8 * ks, tc::desc_at(d_w3t, ks * 2 * (96 * 16)), idy1, true);
                     }
                     DP_TICK(11);
@@ -491,18 +513,19 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
                         uint32_t g0[16], g1[16];
+                        const bool full = h == 0 || W != 25;
                         tc::ld16(tm_lane + TM_Z + 32 + 32 * h, g0);
-                        if (h == 0) tc::ld16(tm_lane + TM_Z + 48, g1);
+                        if (full) tc::ld16(tm_lane + TM_Z + 48 + 32 * h, g1);
                         else tc::ld2(tm_lane + TM_Z + 80, reinterpret_cast<uint32_t (&)[2]>(g1));
                         tc::wait_ld();
                         uint32_t o[8];
 #pragma unroll
                         for (int q = 0; q < 8; ++q) o[q] = tc::pack_h2(__uint_as_float(g0[2 * q]) * d2f[h][2 * q], __uint_as_float(g0[2 * q + 1]) * d2f[h][2 * q + 1]);
                         tc::st8(tm_lane + TM_T + 16 + 16 * h, o);
-                        if (h == 0) {
+                        if (full) {
 #pragma unroll
                             for (int q = 0; q < 8; ++q) o[q] = tc::pack_h2(__uint_as_float(g1[2 * q]) * d2f[h][16 + 2 * q], __uint_as_float(g1[2 * q + 1]) * d2f[h][16 + 2 * q + 1]);
-                            tc::st8(tm_lane + TM_T + 24, o);
+                            tc::st8(tm_lane + TM_T + 24 + 16 * h, o);
                         } else {
                             tc::st4(tm_lane + TM_T + 40, tc::pack_h2(__uint_as_float(g1[0]) * d2f[h][16], __uint_as_float(g1[1]) * d2f[h][17]), 0u, 0u, 0u);
                         }
@@ -532,8 +555,8 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
 #pragma unroll
                             for (int q = 0; q < 8; ++q) {
                                 const float2 d = make_float2(d1f[h][2 * q], d1f[h][2 * q + 1]);
-                                if (16 * h + 2 * q < 25) ds = fmaf(__uint_as_float(g0[2 * q]) * d.x, sw1[16 * h + 2 * q], ds);
-                                if (16 * h + 2 * q + 1 < 25) ds = fmaf(__uint_as_float(g0[2 * q + 1]) * d.y, sw1[16 * h + 2 * q + 1], ds);
+                                if (16 * h + 2 * q < M0) ds = fmaf(__uint_as_float(g0[2 * q]) * d.x, sw1[16 * h + 2 * q], ds);
+                                if (16 * h + 2 * q + 1 < M0) ds = fmaf(__uint_as_float(g0[2 * q + 1]) * d.y, sw1[16 * h + 2 * q + 1], ds);
                             }
                         }
                         // gradient of E with respect to this row of the environment matrix R~ (S8 + S9 run in k_prod_force_virial)
@@ -653,14 +676,15 @@ k_prod_force_virial(long N, int T, const __grid_constant__ TypeTab tt, EnvParams
 
 }  // namespace
 
-cudaError_t launch_embed_bwd_tc2(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    DP_SMEM_OPTIN(k_embed_bwd_tc2, BwdSmem::TOTAL);
+template <int W>
+static cudaError_t launch_bwd_w(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    DP_SMEM_OPTIN(k_embed_bwd_tc2<W>, BwdSmem<W>::TOTAL);
     const TypeTab tt = make_typetab(m);
     EnvParams ep;
     ep.rc = m->rc; ep.rc_smth = m->rc_smth; ep.inv_range = 1.0 / (m->rc - m->rc_smth);
     ep.L[0] = g.L[0]; ep.L[1] = g.L[1]; ep.L[2] = g.L[2];
     // the last fitting GEMM left gA itself in the gD buffer (fit_tc.cu MODE 6)
-    k_gA_fold<<<(unsigned)((N + 7) / 8), 256, 0, st>>>(N, (const float *)(ws + L.gD), (uint8_t *)(ws + L.gAf), (float *)(ws + L.gscale));
+    k_gA_fold<W><<<(unsigned)((N + 7) / 8), 256, 0, st>>>(N, (const float *)(ws + L.gD), (uint8_t *)(ws + L.gAf), (float *)(ws + L.gscale));
     long long *tdbg = nullptr;
 #ifdef DP_BWD_TIMING
     static long long *tbuf = nullptr;
@@ -668,8 +692,8 @@ cudaError_t launch_embed_bwd_tc2(const dp_model *m, long N, const Grid3 &g, char
     tdbg = tbuf;
 #endif
     if (m->profile) cudaEventRecord(m->ev[6], st);
-    k_embed_bwd_tc2<<<m->num_sms, NWG * WGT, BwdSmem::TOTAL, st>>>(
-        N, m->T, g.ncell, m->Nm, tt, (const EmbedNetTC2 *)m->embed_tc2_dev, m->std_dev, (int *)(ws + L.bin_start),
+    k_embed_bwd_tc2<W><<<m->num_sms, NWG * WGT, BwdSmem<W>::TOTAL, st>>>(
+        N, m->T, g.ncell, m->Nm, tt, (const EmbedNetTC2<W> *)m->embed_tc2_dev, m->std_dev, (int *)(ws + L.bin_start),
         (int *)(ws + L.rowstart), (const float4 *)(ws + L.rows_rh), (const int2 *)(ws + L.rows_id),
         (const uint8_t *)(ws + L.gAf), (const float *)(ws + L.gscale), (float4 *)(ws + L.rows_g),
         (unsigned long long *)(ws + L.status + 16), tdbg);
@@ -690,4 +714,8 @@ cudaError_t launch_embed_bwd_tc2(const dp_model *m, long N, const Grid3 &g, char
     }
 #endif
     return cudaGetLastError();
+}
+
+cudaError_t launch_embed_bwd_tc2(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    return m->m0 == 32 ? launch_bwd_w<32>(m, N, g, ws, L, st) : launch_bwd_w<25>(m, N, g, ws, L, st);
 }

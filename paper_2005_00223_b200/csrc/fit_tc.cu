@@ -35,18 +35,21 @@ template <int KTOT, int NTOT>
 struct Cfg {
     static constexpr bool RESIDENT = KTOT == 240;            // the A tile stays in shared memory for all N tiles
     // K chunk.  K = 1600 (the descriptor producer): 64 = 4 values of m, so that A_i[c][4 kc .. 4 kc + 3] is one aligned float4
-    static constexpr int KCH = KTOT == 1600 ? 64 : KC;
+    static constexpr bool DESCR_K = KTOT != 240;             // K = 16 m2 (1600 / 2048): the first layer, A = the descriptor
+    static constexpr bool GA_N = NTOT != 240;                // N = 16 m2: the last backward product, gA in the epilogue
+    static constexpr int M2 = (DESCR_K ? KTOT : (GA_N ? NTOT : 1600)) / 16;     // embedding output width m2 (100 / 128)
+    static constexpr int KCH = DESCR_K ? 64 : KC;
     static constexpr int SUBS = KCH / 8;
     // bytes between sub-chunks of the A image.  K = 1600: the two threads of a row are neighbouring lanes and write
     // sub-chunks 2 mm and 2 mm + 1: 64 bytes of padding put them on disjoint banks
-    static constexpr int ASS = KTOT == 1600 ? BM * 16 + 64 : A_SUB_STRIDE;
+    static constexpr int ASS = DESCR_K ? BM * 16 + 64 : A_SUB_STRIDE;
     static constexpr int A_PARTC = SUBS * ASS;               // one part (hi or lo) of one K chunk
-    static constexpr int BN = NTOT == 240 ? 240 : 160;
+    static constexpr int BN = NTOT == 240 ? 240 : (NTOT == 1600 ? 160 : 128);
     static constexpr int NTILES = NTOT / BN;
     static constexpr int NKC = KTOT / KCH;
     static constexpr int NA = RESIDENT ? NKC : 3;            // A buffers
     static constexpr int B_STAGE = KCH * BN * 2;
-    static constexpr int NSTAGE = NTOT == 1600 ? 4 : (KTOT == 1600 ? 3 : 2);   // B pipeline depth (short stages need more copies in flight)
+    static constexpr int NSTAGE = GA_N ? 4 : (DESCR_K ? 3 : 2);   // B pipeline depth (short stages need more copies in flight)
     static constexpr int A_BUF = 2 * A_PARTC;                // hi + lo
     static constexpr int OFF_A = 0;
     static constexpr int OFF_B = ((NA * A_BUF + 1023) / 1024) * 1024;
@@ -220,21 +223,22 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
             constexpr bool DESCR = MODE == 0;
             const int dr = pt >> 1, dah = pt & 1;       // neighbouring lanes share a row: their loads coalesce in L1
             const bool drow_ok = row0 + dr < rend;
-            const float *Ai = p.A + (long)(drow_ok ? row0 + dr : row0) * 400;
+            constexpr int M2 = C::M2;
+            const float *Ai = p.A + (long)(drow_ok ? row0 + dr : row0) * (4 * M2);
             tc::f32x2 axp[4][4];                        // A_i[c][8 dah + 2 jp, + 1] as packed pairs
             float4 nx[4];                               // A_i[c][4 kc .. 4 kc + 3] of the next chunk (prefetched)
             if (DESCR) {
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
-                    const float4 u0 = __ldg(reinterpret_cast<const float4 *>(Ai + c * 100 + 8 * dah));
-                    const float4 u1 = __ldg(reinterpret_cast<const float4 *>(Ai + c * 100 + 8 * dah + 4));
+                    const float4 u0 = __ldg(reinterpret_cast<const float4 *>(Ai + c * M2 + 8 * dah));
+                    const float4 u1 = __ldg(reinterpret_cast<const float4 *>(Ai + c * M2 + 8 * dah + 4));
                     axp[c][0] = tc::pk2(u0.x, u0.y); axp[c][1] = tc::pk2(u0.z, u0.w);
                     axp[c][2] = tc::pk2(u1.x, u1.y); axp[c][3] = tc::pk2(u1.z, u1.w);
                     nx[c] = u0;
                 }
                 if (dah) {
 #pragma unroll
-                    for (int c = 0; c < 4; ++c) nx[c] = __ldg(reinterpret_cast<const float4 *>(Ai + c * 100));
+                    for (int c = 0; c < 4; ++c) nx[c] = __ldg(reinterpret_cast<const float4 *>(Ai + c * M2));
                 }
             }
             for (int kc = 0; kc < C::NKC; ++kc, ++astep) {
@@ -243,7 +247,7 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
 #pragma unroll
                     for (int c = 0; c < 4; ++c) {
                         cur[c] = nx[c];
-                        if (kc + 1 < C::NKC) nx[c] = __ldg(reinterpret_cast<const float4 *>(Ai + c * 100 + 4 * (kc + 1)));
+                        if (kc + 1 < C::NKC) nx[c] = __ldg(reinterpret_cast<const float4 *>(Ai + c * M2 + 4 * (kc + 1)));
                     }
                 }
                 int ab;
@@ -313,8 +317,9 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                 // thread (row, c): one of the four components.  Per 16 accumulator columns = gD[m][0..16) of one m.
                 // (four threads per row: the epilogue is bound by its load-to-use latencies, not by the FMA pipe)
                 const int c = ((warp - 2 - NPROD / 32) >> 2) & 3;
-                const float *Arow = p.aux0 + (long)(ok ? row0 + r : row0) * 400 + c * 100;
-                float *Grow = p.out0 + (long)(row0 + r) * 400 + c * 100;
+                constexpr int M2 = C::M2;
+                const float *Arow = p.aux0 + (long)(ok ? row0 + r : row0) * (4 * M2) + c * M2;
+                float *Grow = p.out0 + (long)(row0 + r) * (4 * M2) + c * M2;
                 float a16[16], acc2[16];
 #pragma unroll
                 for (int k4 = 0; k4 < 4; ++k4) {
@@ -337,7 +342,7 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                         const int m = nt * (C::BN / 16) + mm;            // BN / 16 = 10: the unrolled mm gives m & 3 statically per nt parity
                         if ((m & 3) == 0) {
                             am0 = an0;
-                            if (m + 4 < 100) an0 = __ldg(reinterpret_cast<const float4 *>(Arow + m + 4));
+                            if (m + 4 < M2) an0 = __ldg(reinterpret_cast<const float4 *>(Arow + m + 4));
                         }
                         tc::wait_ld();
                         if (mm + 1 < C::BN / 16) tc::ld16(tm_lane + buf * C::TM_BUF + 16 * (mm + 1), v[(mm + 1) & 1]);
@@ -427,6 +432,7 @@ struct FitChainArgs {
     const __half *Bimg; long b_type_stride;
     const float *c2, *c3, *v4, *c4;       // [T][240], c4 [T]
     const double *ebias;                  // [T]
+    long nd240;                           // elements of the V1 image (16 m2 x 240): the 240 x 240 images follow it
     uint8_t *gz1img;                      // per 128-row tile the hi + lo fp16 operand image of the last product (GZ_TILE_BYTES)
     double *eatom;                        // [rows]
 };
@@ -473,7 +479,7 @@ __global__ void __launch_bounds__(CH_THREADS, 1) k_fit_chain(FitChainArgs p) {
         }
     };
     // weight images of the four stages inside one type's block (FIT_TC_OFF[1..4]): V2, V3, V3^T, V2^T
-    const long img_off[4] = {1600L * 240, 1600L * 240 + 240L * 240, 1600L * 240 + 2L * 240 * 240, 1600L * 240 + 3L * 240 * 240};
+    const long img_off[4] = {p.nd240, p.nd240 + 240L * 240, p.nd240 + 2L * 240 * 240, p.nd240 + 3L * 240 * 240};
 
     if (warp == 0) {
         // ---------------------------------------------------------------- weight loader
@@ -683,41 +689,44 @@ cudaError_t launch(const FitTcArgs &p, int grid, cudaStream_t st) {
 
 }  // namespace
 
-// Host side: weight images.  For product g the image of type a is [NTILES][NKC][KC/8][BN][8] fp16 with
-// element (nt, kc, sub, n, kk) = B[k = kc*KC + sub*8 + kk][nt*BN + n].
-size_t fit_tc_image_elems(int K, int Nn) { return (size_t)K * Nn; }
+// Host side: weight images.  For product g the image of type a is [NTILES][K/8][BN][8] fp16 with
+// element (nt, k8, n, kk) = B[k = k8*8 + kk][nt*BN + n]  (any K chunking of the kernels reads it contiguously).
 void fit_tc_build_image(const double *W, int ldw, bool transpose, int K, int Nn, __half *out) {
-    const int BN = Nn == 240 ? 240 : 160;
-    const int ntl = Nn / BN, nkc = K / KC;
+    const int BN = Nn == 240 ? 240 : (Nn == 1600 ? 160 : 128);
+    const int ntl = Nn / BN, nk8 = K / 8;
     for (int nt = 0; nt < ntl; ++nt)
-        for (int kc = 0; kc < nkc; ++kc)
-            for (int sub = 0; sub < SUB; ++sub)
-                for (int n = 0; n < BN; ++n)
-                    for (int kk = 0; kk < 8; ++kk) {
-                        const int k = kc * KC + sub * 8 + kk, nn = nt * BN + n;
-                        const double v = transpose ? W[(size_t)nn * ldw + k] : W[(size_t)k * ldw + nn];
-                        out[((((size_t)nt * nkc + kc) * SUB + sub) * BN + n) * 8 + kk] = __float2half_rn((float)v);
-                    }
+        for (int k8 = 0; k8 < nk8; ++k8)
+            for (int n = 0; n < BN; ++n)
+                for (int kk = 0; kk < 8; ++kk) {
+                    const int k = k8 * 8 + kk, nn = nt * BN + n;
+                    const double v = transpose ? W[(size_t)nn * ldw + k] : W[(size_t)k * ldw + nn];
+                    out[(((size_t)nt * nk8 + k8) * BN + n) * 8 + kk] = __float2half_rn((float)v);
+                }
 }
 
 // offsets (elements) of the six product images inside one type's block: g0 V1, g1 V2, g2 V3, g3 V3^T, g4 V2^T, g5 V1^T
-static const size_t FIT_TC_OFF[7] = {0, 1600 * 240, 1600 * 240 + 240 * 240, 1600 * 240 + 2 * 240 * 240, 1600 * 240 + 3 * 240 * 240,
-                                     1600 * 240 + 4 * 240 * 240, 2 * 1600 * 240 + 4 * 240 * 240};
-size_t fit_tc_type_elems() { return FIT_TC_OFF[6]; }
-void fit_tc_build_type(const double *V1, const double *V2, const double *V3, __half *out) {
-    fit_tc_build_image(V1, 240, false, 1600, 240, out + FIT_TC_OFF[0]);
-    fit_tc_build_image(V2, 240, false, 240, 240, out + FIT_TC_OFF[1]);
-    fit_tc_build_image(V3, 240, false, 240, 240, out + FIT_TC_OFF[2]);
-    fit_tc_build_image(V3, 240, true, 240, 240, out + FIT_TC_OFF[3]);
-    fit_tc_build_image(V2, 240, true, 240, 240, out + FIT_TC_OFF[4]);
-    fit_tc_build_image(V1, 240, true, 240, 1600, out + FIT_TC_OFF[5]);
+static size_t fit_tc_off(int nd, int g) {
+    const size_t a = (size_t)nd * 240, b = 240 * 240;
+    const size_t off[7] = {0, a, a + b, a + 2 * b, a + 3 * b, a + 4 * b, 2 * a + 4 * b};
+    return off[g];
+}
+size_t fit_tc_type_elems(int nd) { return fit_tc_off(nd, 6); }
+void fit_tc_build_type(int nd, const double *V1, const double *V2, const double *V3, __half *out) {
+    fit_tc_build_image(V1, 240, false, nd, 240, out + fit_tc_off(nd, 0));
+    fit_tc_build_image(V2, 240, false, 240, 240, out + fit_tc_off(nd, 1));
+    fit_tc_build_image(V3, 240, false, 240, 240, out + fit_tc_off(nd, 2));
+    fit_tc_build_image(V3, 240, true, 240, 240, out + fit_tc_off(nd, 3));
+    fit_tc_build_image(V2, 240, true, 240, 240, out + fit_tc_off(nd, 4));
+    fit_tc_build_image(V1, 240, true, 240, nd, out + fit_tc_off(nd, 5));
 }
 
 // S5 + S6 in MIX-16: first layer (descriptor formed in the operand producer), the fused 240 x 240 chain with the energy,
 // and the last backward product with gA in its epilogue (the gD buffer receives gA [N][4][100]; gD is never written).
 // gz1 travels from the chain to the last product as ready-made hi + lo fp16 tile images in the activation buffers 2 S .. 4 S.
-cudaError_t launch_fit_tc(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    const int F = 240, ND = M2E * 16;
+template <int ND>
+static cudaError_t launch_fit_tc_nd(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    const int F = 240;
+    constexpr int M2E = ND / 16;
     float *Amat = (float *)(ws + L.A);
     float *act = (float *)(ws + L.fit_act);
     float *h1 = act;
@@ -727,22 +736,26 @@ cudaError_t launch_fit_tc(const dp_model *m, long N, const Grid3 &g, char *ws, c
     cudaError_t e = cudaSuccess;
     auto ok = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
     FitTcArgs p{};
-    p.T = m->T; p.ncell = g.ncell; p.bin_start = bin_start; p.b_type_stride = (long)FIT_TC_OFF[6];
-    p.A = Amat; p.lda = 4 * M2E; p.Bimg = (const __half *)m->fit_tc_img_dev + FIT_TC_OFF[0];
+    p.T = m->T; p.ncell = g.ncell; p.bin_start = bin_start; p.b_type_stride = (long)fit_tc_off(ND, 6);
+    p.A = Amat; p.lda = 4 * M2E; p.Bimg = (const __half *)m->fit_tc_img_dev + fit_tc_off(ND, 0);
     p.bias = (const float *)m->fitc1_dev; p.out0 = h1; p.ldo = F;
-    ok(launch<0, 1600, 240>(p, grid, st));
+    ok(launch<0, ND, 240>(p, grid, st));
     FitChainArgs c{};
     c.T = m->T; c.ncell = g.ncell; c.bin_start = bin_start; c.h1 = h1;
-    c.Bimg = (const __half *)m->fit_tc_img_dev; c.b_type_stride = (long)FIT_TC_OFF[6];
+    c.Bimg = (const __half *)m->fit_tc_img_dev; c.b_type_stride = (long)fit_tc_off(ND, 6);
     c.c2 = (const float *)m->fitc2_dev; c.c3 = (const float *)m->fitc3_dev; c.v4 = (const float *)m->fitv4_dev;
-    c.c4 = (const float *)m->fitc4_dev; c.ebias = m->ebias_dev; c.gz1img = gzimg; c.eatom = (double *)(ws + L.eatom);
+    c.c4 = (const float *)m->fitc4_dev; c.nd240 = (long)ND * 240; c.ebias = m->ebias_dev; c.gz1img = gzimg; c.eatom = (double *)(ws + L.eatom);
     DP_SMEM_OPTIN(k_fit_chain, CH_TOTAL);
     k_fit_chain<<<grid, CH_THREADS, CH_TOTAL, st>>>(c);
     ok(cudaGetLastError());
     FitTcArgs q{};
-    q.T = m->T; q.ncell = g.ncell; q.bin_start = bin_start; q.b_type_stride = (long)FIT_TC_OFF[6];
-    q.Aimg = gzimg; q.lda = F; q.Bimg = (const __half *)m->fit_tc_img_dev + FIT_TC_OFF[5];
+    q.T = m->T; q.ncell = g.ncell; q.bin_start = bin_start; q.b_type_stride = (long)fit_tc_off(ND, 6);
+    q.Aimg = gzimg; q.lda = F; q.Bimg = (const __half *)m->fit_tc_img_dev + fit_tc_off(ND, 5);
     q.aux0 = Amat; q.out0 = (float *)(ws + L.gD); q.ldo = ND;
-    ok(launch<6, 240, 1600>(q, grid, st));
+    ok(launch<6, 240, ND>(q, grid, st));
     return e;
+}
+
+cudaError_t launch_fit_tc(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    return m->m2 == 128 ? launch_fit_tc_nd<2048>(m, N, g, ws, L, st) : launch_fit_tc_nd<1600>(m, N, g, ws, L, st);
 }

@@ -40,3 +40,26 @@ def test_paper_shape_fp64(k):
     rms = np.sqrt((o["forces"] ** 2).mean())
     assert np.abs(g["forces"] - o["forces"]).max() <= 1e-10 * rms
     assert np.abs(g["virial"] - o["virial"]).max() <= 1e-10 * np.abs(o["virial"]).max()
+
+
+@pytest.mark.parametrize("k", [0, 1])
+def test_paper_shape_mix16(k):
+    """MIX-16 at the paper's shape (tcgen05 kernels templated on the width; biases through the constant-ones K step)"""
+    s = _systems()[k]
+    o = oracle.evaluate(s.coords, s.types, s.box, s.model)
+    g = _gpu_eval(s, "mix16")
+    assert np.array_equal(g["nlist"], o["nlist"]) and g["n_truncated"] == o["n_truncated"]
+    rms = np.sqrt((o["forces"] ** 2).mean())
+    err = np.abs(g["forces"] - o["forces"]).max()
+    assert err <= 5e-3 * rms, err / rms
+    assert abs(g["energy"][0] - o["energy"]) / s.natoms <= 1e-3
+    assert np.abs(g["atom_energy"] - o["atom_energy"]).max() <= 5e-3
+    assert np.abs(g["virial"] - o["virial"]).max() / s.natoms <= 1e-3
+
+
+def test_paper_shape_mix32_is_reported_as_unsupported():
+    from paper_2005_00223_b200 import binding
+    s = _systems()[0]
+    with pytest.raises(binding.DPError) as e:
+        binding.DPModel(s.model, "mix32")
+    assert e.value.code == -7
