@@ -191,9 +191,11 @@ def roofline_of(s, r, pk, mp):
         rec["mufu_tanh_frac"] = (r["real_rows"] * tanh_row / (ph[5] * 1e-3)) / (mp["tanh_tera_per_s"] * 1e12)
     if s.precision == "mix16":
         rec["executed_tflops"] = r["rows_b"] * EXEC_FLOP_ROW_BWD / (ph[5] * 1e-3) / 1e12
-        rec["note"] = ("algorithmic backward flops (14,150 per real neighbour row); the in-kernel forward recompute, the hi/lo operand "
-                       "splitting and the K/N padding are executed (executed_tflops) but not credited; mufu_tanh_frac = tanh of the "
-                       "real rows / measured tanh.approx.f32 rate")
+        rec["note"] = (f"algorithmic backward flops ({frow_b:,} per real neighbour row); the in-kernel forward recompute, the hi/lo operand "
+                       "splitting and the K/N padding are executed (executed_tflops, widths 25-50-100 only) but not credited; "
+                       "mufu_tanh_frac = tanh of the real rows / measured tanh.approx.f32 rate")
+        if s.model.embed_widths[0] != 25:
+            rec.pop("executed_tflops")
     return rec
 
 
