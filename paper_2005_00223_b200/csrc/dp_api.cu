@@ -57,7 +57,7 @@ WsLayout ws_layout(const dp_model *m, long N, long NE) {
     const int nt3 = 2 * ((m->m0 + 3) / 4);          // EmbW<W>::NT3
     L.A = take(esz * (size_t)N * 4 * m->m2);
     if (m->prec == DP_FP64) L.gAf = take(sizeof(double) * (size_t)N * 3 * nt3 * 32);
-    else L.gAf = take(sizeof(uint32_t) * (size_t)N * 2 * 28 * 32);
+    else L.gAf = take(sizeof(uint32_t) * (size_t)N * 2 * (2 * nt3) * 32);     // MIX-32 fragments / MIX-16 operand image (smaller)
     L.gscale = take(sizeof(float) * (size_t)N);
     // (MIX-16: buffers 2..6 also hold the gz1 operand images, one per 128-row tile and at least one per type: the pad
     // covers systems with fewer rows than a tile)
@@ -79,7 +79,7 @@ bool rows_fit_int32(const dp_model *m, long N) {
 // Cell grid of one evaluation.  Orthorhombic boxes with every length >= 2 rc take the minimum-image path (nlist.cu);
 // everything else (a general cell, or an edge shorter than 2 rc) takes the ghost path (ghost.cu).  false: degenerate box.
 // (32, 64, 128) networks: which precision modes have kernels for them
-bool paper_shape_supported(dp_precision prec) { return prec == DP_FP64 || prec == DP_MIX16; }
+bool paper_shape_supported(dp_precision prec) { return prec == DP_FP64 || prec == DP_MIX16 || prec == DP_MIX32; }
 
 bool make_grid(const dp_model *m, long N, const double *box, Grid3 *g) {
     *g = Grid3{};
@@ -218,8 +218,11 @@ inline float hpart(double x, int part) {
     return part == 0 ? hi : xf - hi;
 }
 
-template <int NSW>
-void build_embed_frag_h(const double *net, EmbedNetFragH<NSW> *out) {
+template <int NSW, int W>
+void build_embed_frag_h(const double *net, EmbedNetFragH<NSW, W> *out) {
+    constexpr int M0 = HW<W>::M0, M1 = HW<W>::M1, M2E = HW<W>::M2E, HNT2 = HW<W>::HNT2, HNT3 = HW<W>::HNT3;
+    auto h_f2 = [](int nt, int r, int j) { return ::h_f2<W>(nt, r, j); };
+    auto h_f3 = [](int nt3, int r, int j3) { return ::h_f3<W>(nt3, r, j3); };
     const double *W1 = net, *b1 = W1 + M0, *W2 = b1 + M0, *b2 = W2 + M0 * M1, *W3 = b2 + M1, *b3 = W3 + M1 * M2E;
     std::memset(out, 0, sizeof(*out));
     for (int e = 0; e < M0; ++e) { out->w1[e] = (float)W1[e]; out->b1[e] = (float)b1[e]; }
@@ -251,7 +254,7 @@ void build_embed_frag_h(const double *net, EmbedNetFragH<NSW> *out) {
                         out->W3f[p][s][nt3][l][h] = hbits2(hpart(w3(h_f2(t, r, 0), fo), p), hpart(w3(h_f2(t, r, 1), fo), p));
                     }
             // layer 3 backward: K positions of G (tile 2s + h, r, j3); N position of y2 (nt2, g/2, g%2)
-            for (int s = 0; s < 7; ++s)
+            for (int s = 0; s < HNT3 / 2; ++s)
                 for (int nt2 = 0; nt2 < HNT2; ++nt2)
                     for (int h = 0; h < 2; ++h) {
                         int t = 2 * s + h, fi = h_f2(nt2, g >> 1, g & 1);
@@ -269,8 +272,12 @@ void build_embed_frag_h(const double *net, EmbedNetFragH<NSW> *out) {
         }
 }
 
-template <int NSW>
+template <int NSW, int W>
 void build_embed_tc(const double *net, EmbedNetTC<NSW> *out) {
+    constexpr int M0 = W, M1 = 2 * W, M2E = 4 * W;
+    auto tc_e_of_p1 = [](int p1) { return ::tc_e_of_p1<W>(p1); };
+    auto tc_f_of_n = [](int n) { return ::tc_f_of_n<W>(n); };
+    auto tc_m_of_c3 = [](int c) { return ::tc_m_of_c3<W>(c); };
     const double *W1 = net, *b1 = W1 + M0, *W2 = b1 + M0, *b2 = W2 + M0 * M1, *W3 = b2 + M1, *b3 = W3 + M1 * M2E;
     std::memset(out, 0, sizeof(*out));
     for (int p1 = 0; p1 < TC_K1; ++p1) { int e = tc_e_of_p1(p1); if (e >= 0) { out->w1[p1] = (float)W1[e]; out->b1[p1] = (float)b1[e]; } }
@@ -441,11 +448,18 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
         for (int ab = 0; ab < T * T; ++ab) build_embed_frag<double, 25>(w->embed + ab * ensz, &frags[ab]);
         ok(upload(frags, &m->embed_frag_dev));
     } else if (prec == DP_MIX32) {      // tcgen05 forward (embed_tc.cu), mma.sync backward (embed_mix.cu): weights as hi + lo fp16
-        std::vector<EmbedNetFragH<2>> frags((size_t)T * T);
-        for (int ab = 0; ab < T * T; ++ab) build_embed_frag_h<2>(w->embed + ab * ensz, &frags[ab]);
-        ok(upload(frags, &m->embed_frag_dev));
         std::vector<EmbedNetTC<2>> nets((size_t)T * T);
-        for (int ab = 0; ab < T * T; ++ab) build_embed_tc<2>(w->embed + ab * ensz, &nets[ab]);
+        if (W0 == 32) {
+            std::vector<EmbedNetFragH<2, 32>> frags((size_t)T * T);
+            for (int ab = 0; ab < T * T; ++ab) build_embed_frag_h<2, 32>(w->embed + ab * ensz, &frags[ab]);
+            ok(upload(frags, &m->embed_frag_dev));
+            for (int ab = 0; ab < T * T; ++ab) build_embed_tc<2, 32>(w->embed + ab * ensz, &nets[ab]);
+        } else {
+            std::vector<EmbedNetFragH<2, 25>> frags((size_t)T * T);
+            for (int ab = 0; ab < T * T; ++ab) build_embed_frag_h<2, 25>(w->embed + ab * ensz, &frags[ab]);
+            ok(upload(frags, &m->embed_frag_dev));
+            for (int ab = 0; ab < T * T; ++ab) build_embed_tc<2, 25>(w->embed + ab * ensz, &nets[ab]);
+        }
         ok(upload(nets, &m->embed_tc_dev));
     } else {                            // MIX-16: warpgroup-per-tile tcgen05 kernels (embed_tc2*.cu)
         if (W0 == 32) {
@@ -462,7 +476,7 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
         m->fwd_split = (Nm < 128 && W0 == 25) ? 1 : 0;
         if (m->fwd_split) {
             std::vector<EmbedNetTC<1>> n1((size_t)T * T);
-            for (int ab = 0; ab < T * T; ++ab) build_embed_tc<1>(w->embed + ab * ensz, &n1[ab]);
+            for (int ab = 0; ab < T * T; ++ab) build_embed_tc<1, 25>(w->embed + ab * ensz, &n1[ab]);
             ok(upload(n1, &m->embed_tc_dev));
         }
     }

@@ -43,10 +43,13 @@ __device__ __forceinline__ void env_row(const EnvParams &p, double dx, double dy
 //   y1c[t][2row+j] : layer-1 slot q = 2t + j              t2c[nt] : tanh of layer-2 pre-activation
 //   y2 = y1c[nt/2][2row + nt%2] + t2c[nt][.]              t3c[nt3]: tanh of layer-3 pre-activation
 //   G  = y2(nt3/2)[2row + nt3%2] + t3c[nt3][.]
-template <int NS, bool APPROX>
-__device__ __forceinline__ void forward_tile(const EmbedNetFragH<ns_wparts(NS)> *__restrict__ net, int lane,
-                                             float s0, float s1, float (&y1c)[4][4], float (&t2c)[HNT2][4],
-                                             float (&t3c)[HNT3][4]) {
+template <int NS, bool APPROX, int W>
+__device__ __forceinline__ void forward_tile(const EmbedNetFragH<ns_wparts(NS), W> *__restrict__ net, int lane,
+                                             float s0, float s1, float (&y1c)[4][4], float (&t2c)[HW<W>::HNT2][4],
+                                             float (&t3c)[HW<W>::HNT3][4]) {
+    constexpr int M2E = HW<W>::M2E, HNT2 = HW<W>::HNT2, HNT3 = HW<W>::HNT3;
+    constexpr bool ODD2 = (HNT2 & 1) != 0;      // the K of HNT2 tiles ends with a k8 step
+    (void)M2E; (void)ODD2;
     constexpr int NSW = ns_wparts(NS);
     const int r = lane & 3;
 #pragma unroll
@@ -105,7 +108,7 @@ __device__ __forceinline__ void forward_tile(const EmbedNetFragH<ns_wparts(NS)> 
                             v[h][2 * row + j] = y1c[nt >> 1][2 * row + (nt & 1)] + t2c[nt][2 * row + j];
                 }
             }
-            if (s < 3) {
+            if (s < 3 || !ODD2) {
                 make_afrag<NS>(a, v[0][0], v[0][1], v[0][2], v[0][3], v[1][0], v[1][1], v[1][2], v[1][3]);
 #pragma unroll
                 for (int t = 0; t < HNT3 / 2; ++t) {
@@ -133,8 +136,8 @@ __device__ __forceinline__ void forward_tile(const EmbedNetFragH<ns_wparts(NS)> 
 // G value of layer-3 tile nt3, element k = 2*row + j3
 #define GVAL(nt3, k) ((y1c[(nt3) >> 2][((k) & 2) + (((nt3) >> 1) & 1)] + t2c[(nt3) >> 1][((k) & 2) + ((nt3) & 1)]) + t3c[nt3][k])
 
-template <int NSW>
-__device__ __forceinline__ void copy_net_to_smem(EmbedNetFragH<NSW> *dst, const EmbedNetFragH<NSW> *__restrict__ src,
+template <int NSW, int W>
+__device__ __forceinline__ void copy_net_to_smem(EmbedNetFragH<NSW, W> *dst, const EmbedNetFragH<NSW, W> *__restrict__ src,
                                                  int nwords) {
     const uint32_t *s = reinterpret_cast<const uint32_t *>(src);
     uint32_t *d = reinterpret_cast<uint32_t *>(dst);
@@ -149,21 +152,25 @@ constexpr int MIX_WARP_BUF_FLOATS = MIX_ROWCHUNK * 5;    // rbuf[64][4] + sbuf[6
 //   [p][0..14)[lane]     dG  MMA (k8) B fragment of tile nt3:  (r < 2) ? half2(gA[2r][f], gA[2r+1][f]) : 0, f = f3(nt3, g/2, g%2)
 //   [p][14 + 2s + h][lane] dR^ MMA (k16 step s) B registers h = 0,1: (g < 4) ? half2(gA[g][f3(2s+h, r, 0)], gA[g][f3(2s+h, r, 1)]) : 0
 // all scaled by gscale[i] (a power of two that brings max|gA| near 1); results are multiplied by 1/(Nm*gscale).
-template <int NS, int NSC, bool APPROX, int NSB>
+template <int NS, int NSC, bool APPROX, int NSB, int W>
 __global__ void __launch_bounds__(DP_WARPS_PER_CTA * 32, 1)
-k_embed_bwd_mix(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, EnvParams ep, const EmbedNetFragH<ns_wparts(NS)> *__restrict__ nets,
+k_embed_bwd_mix(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, EnvParams ep, const EmbedNetFragH<ns_wparts(NS), W> *__restrict__ nets,
                 const double *__restrict__ avg, const double *__restrict__ stdv, const int *__restrict__ bin_start,
                 const double *__restrict__ xs, const int *__restrict__ nlist, const int *__restrict__ nreal,
                 const uint32_t *__restrict__ gAf, const float *__restrict__ gscale, double *__restrict__ fsorted,
                 double *__restrict__ virial, unsigned long long *__restrict__ row_counter) {
+    constexpr int M2E = HW<W>::M2E, HNT2 = HW<W>::HNT2, HNT3 = HW<W>::HNT3;
+    constexpr bool ODD2 = (HNT2 & 1) != 0;      // the K of HNT2 tiles ends with a k8 step
+    (void)M2E; (void)ODD2;
     constexpr int NSW = ns_wparts(NS);
+    constexpr int GP = 2 * HNT3;              // gA fragment words per weight part and lane: HNT3 dG tiles + HNT3 dR^ registers
     extern __shared__ __align__(16) uint32_t smem_u[];
-    EmbedNetFragH<NSW> *net = reinterpret_cast<EmbedNetFragH<NSW> *>(smem_u);
+    EmbedNetFragH<NSW, W> *net = reinterpret_cast<EmbedNetFragH<NSW, W> *>(smem_u);
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    float *rbuf = reinterpret_cast<float *>(smem_u) + sizeof(EmbedNetFragH<NSW>) / 4 + wid * MIX_WARP_BUF_FLOATS;
+    float *rbuf = reinterpret_cast<float *>(smem_u) + sizeof(EmbedNetFragH<NSW, W>) / 4 + wid * MIX_WARP_BUF_FLOATS;
     float *sbuf = rbuf + MIX_ROWCHUNK * 4;
     const int *sel = tt.sel;
-    const int gw = blockIdx.x * DP_WARPS_PER_CTA + wid, W = gridDim.x * DP_WARPS_PER_CTA;
+    const int gw = blockIdx.x * DP_WARPS_PER_CTA + wid, NWARP = gridDim.x * DP_WARPS_PER_CTA;
     const int r = lane & 3, g = lane >> 2;
     const double hx = 0.5 * ep.L[0], hy = 0.5 * ep.L[1], hz = 0.5 * ep.L[2];
     unsigned long long my_rows = 0;
@@ -181,12 +188,12 @@ k_embed_bwd_mix(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, En
         int off = 0;
         for (int b = 0; b < T; ++b) {
             __syncthreads();
-            copy_net_to_smem<NSW>(net, nets + (a * T + b), (int)(sizeof(EmbedNetFragH<NSW>) / 4));
+            copy_net_to_smem<NSW, W>(net, nets + (a * T + b), (int)(sizeof(EmbedNetFragH<NSW, W>) / 4));
             __syncthreads();
-            for (int i = ts0 + gw; i < ts1; i += W) {
+            for (int i = ts0 + gw; i < ts1; i += NWARP) {
                 const int nr = nreal[i * T + b];
                 const double xi = xs[3 * (long)i], yi = xs[3 * (long)i + 1], zi = xs[3 * (long)i + 2];
-                const uint32_t *gf = gAf + (long)i * (2 * 28 * 32);
+                const uint32_t *gf = gAf + (long)i * (2 * GP * 32);
                 const float oscale = 1.0f / ((float)Nm * gscale[i]);
                 double fi[3] = {0.0, 0.0, 0.0};
                 for (int r0 = 0; r0 < nr; r0 += MIX_ROWCHUNK) {
@@ -209,7 +216,7 @@ k_embed_bwd_mix(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, En
                     __syncwarp();
                     for (int t = 0; t < ntile; ++t) {
                         float y1c[4][4], t2c[HNT2][4], t3c[HNT3][4];
-                        forward_tile<NS, APPROX>(net, lane, sbuf[t * HROWS + g], sbuf[t * HROWS + g + 8], y1c, t2c, t3c);
+                        forward_tile<NS, APPROX, W>(net, lane, sbuf[t * HROWS + g], sbuf[t * HROWS + g + 8], y1c, t2c, t3c);
                         // dR^[row][c] = sum_m G[row][m] gA[c][m]     (C: c0,c1 row g c=2r,2r+1 ; c2,c3 row g+8)
                         float dR[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
@@ -219,8 +226,8 @@ k_embed_bwd_mix(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, En
                             make_afrag<NSC>(a_, GVAL(ta, 0), GVAL(ta, 1), GVAL(ta, 2), GVAL(ta, 3), GVAL(tb, 0), GVAL(tb, 1),
                                            GVAL(tb, 2), GVAL(tb, 3));
                             uint32_t bh[2], bl[2];
-                            bh[0] = gf[(14 + 2 * s) * 32 + lane]; bh[1] = gf[(15 + 2 * s) * 32 + lane];
-                            if (NSC == 3) { bl[0] = gf[(28 + 14 + 2 * s) * 32 + lane]; bl[1] = gf[(28 + 15 + 2 * s) * 32 + lane]; }
+                            bh[0] = gf[(HNT3 + 2 * s) * 32 + lane]; bh[1] = gf[(HNT3 + 1 + 2 * s) * 32 + lane];
+                            if (NSC == 3) { bl[0] = gf[(GP + HNT3 + 2 * s) * 32 + lane]; bl[1] = gf[(GP + HNT3 + 1 + 2 * s) * 32 + lane]; }
                             else { bl[0] = bl[1] = 0; }
                             mma_k16<NSC>(dR, a_, bh, bl);
                         }
@@ -237,7 +244,7 @@ k_embed_bwd_mix(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, En
                                 float d[4] = {0.f, 0.f, 0.f, 0.f};
                                 uint32_t bh[1], bl[1];
                                 bh[0] = gf[nt3 * 32 + lane];
-                                bl[0] = NSC == 3 ? gf[(28 + nt3) * 32 + lane] : 0u;
+                                bl[0] = NSC == 3 ? gf[(GP + nt3) * 32 + lane] : 0u;
                                 mma_k8<NSC>(d, ar, bh, bl);
 #pragma unroll
                                 for (int k = 0; k < 4; ++k) d[k] *= oscale;
@@ -272,14 +279,16 @@ k_embed_bwd_mix(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, En
 #pragma unroll
                         for (int s = 0; s < 4; ++s) {
                             AFrag<NSB> a_;
-                            if (s < 3) {
-                                make_afrag<NSB>(a_, dy2[2 * s][0], dy2[2 * s][1], dy2[2 * s][2], dy2[2 * s][3], dy2[2 * s + 1][0],
-                                               dy2[2 * s + 1][1], dy2[2 * s + 1][2], dy2[2 * s + 1][3]);
+                            if (s < 3 || !ODD2) {
+                                constexpr int LAST = HNT2 - 1;
+                                const int ta_ = 2 * s, tb_ = 2 * s + 1 <= LAST ? 2 * s + 1 : LAST;
+                                make_afrag<NSB>(a_, dy2[ta_][0], dy2[ta_][1], dy2[ta_][2], dy2[ta_][3], dy2[tb_][0],
+                                               dy2[tb_][1], dy2[tb_][2], dy2[tb_][3]);
 #pragma unroll
                                 for (int t1 = 0; t1 < 4; ++t1)
                                     mma_k16<NSB>(dy1[t1], a_, net->W2Tf[0][s][t1][lane], net->W2Tf[NSW - 1][s][t1][lane]);
                             } else {
-                                make_afrag8<NSB>(a_, dy2[6][0], dy2[6][1], dy2[6][2], dy2[6][3]);
+                                make_afrag8<NSB>(a_, dy2[HNT2 - 1][0], dy2[HNT2 - 1][1], dy2[HNT2 - 1][2], dy2[HNT2 - 1][3]);
 #pragma unroll
                                 for (int t1 = 0; t1 < 4; ++t1)
                                     mma_k8<NSB>(dy1[t1], a_, net->W2Tf[0][s][t1][lane], net->W2Tf[NSW - 1][s][t1][lane]);
@@ -365,9 +374,9 @@ EnvParams make_env(const dp_model *m, const Grid3 &g) {
     return ep;
 }
 
-template <int NS>
+template <int NS, int W>
 int smem_bytes() {
-    return (int)sizeof(EmbedNetFragH<ns_wparts(NS)>) + DP_WARPS_PER_CTA * MIX_WARP_BUF_FLOATS * 4;
+    return (int)sizeof(EmbedNetFragH<ns_wparts(NS), W>) + DP_WARPS_PER_CTA * MIX_WARP_BUF_FLOATS * 4;
 }
 
 int embed_grid(const dp_model *m, long N) {
@@ -375,12 +384,12 @@ int embed_grid(const dp_model *m, long N) {
     return (int)(grid > m->num_sms ? m->num_sms : grid);
 }
 
-template <int NS, int NSC, bool APPROX, int NSB>
+template <int NS, int NSC, bool APPROX, int NSB, int W>
 cudaError_t launch_bwd(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    DP_SMEM_OPTIN((k_embed_bwd_mix<NS, NSC, APPROX, NSB>), smem_bytes<NS>());
+    DP_SMEM_OPTIN((k_embed_bwd_mix<NS, NSC, APPROX, NSB, W>), (smem_bytes<NS, W>()));
     const TypeTab tt = make_typetab(m);
-    k_embed_bwd_mix<NS, NSC, APPROX, NSB><<<embed_grid(m, N), DP_WARPS_PER_CTA * 32, smem_bytes<NS>(), st>>>(
-        m->T, g.ncell, m->Nm, tt, make_env(m, g), (const EmbedNetFragH<ns_wparts(NS)> *)m->embed_frag_dev, m->avg_dev,
+    k_embed_bwd_mix<NS, NSC, APPROX, NSB, W><<<embed_grid(m, N), DP_WARPS_PER_CTA * 32, smem_bytes<NS, W>(), st>>>(
+        m->T, g.ncell, m->Nm, tt, make_env(m, g), (const EmbedNetFragH<ns_wparts(NS), W> *)m->embed_frag_dev, m->avg_dev,
         m->std_dev, (int *)(ws + L.bin_start), (double *)(ws + L.xs), (int *)(ws + L.nlist), (int *)(ws + L.nreal),
         (const uint32_t *)(ws + L.gAf), (const float *)(ws + L.gscale), (double *)(ws + L.fsorted),
         (double *)(ws + L.virial), (unsigned long long *)(ws + L.status + 16));
@@ -391,5 +400,5 @@ cudaError_t launch_bwd(const dp_model *m, long N, const Grid3 &g, char *ws, cons
 
 // MIX-32 ("all the arithmetic operations ... in single precision"): every operand split hi + lo, exact tanhf
 cudaError_t launch_embed_bwd_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    return launch_bwd<3, 3, false, 3>(m, N, g, ws, L, st);
+    return m->m0 == 32 ? launch_bwd<3, 3, false, 3, 32>(m, N, g, ws, L, st) : launch_bwd<3, 3, false, 3, 25>(m, N, g, ws, L, st);
 }

@@ -18,25 +18,32 @@
 #include "dp_internal.h"
 
 constexpr int HQ1 = 8;        // layer-1 slots per thread per row
-constexpr int HNT2 = 7;       // layer-2 8-wide tiles
-constexpr int HNT3 = 14;      // layer-3 8-wide tiles
 constexpr int HROWS = 16;     // rows per MMA tile
 
+// widths (W, 2 W, 4 W): W = 25 (BASELINE) or 32 (the paper's networks)
+template <int W>
+struct HW {
+    static constexpr int M0 = W, M1 = 2 * W, M2E = 4 * W;
+    static constexpr int HNT2 = (W + 3) / 4;     // layer-2 8-wide tiles (7 / 8)
+    static constexpr int HNT3 = 2 * HNT2;        // layer-3 8-wide tiles (14 / 16)
+};
+
 __host__ __device__ inline int h_e1(int q, int r) { return 8 * (q >> 1) + 2 * r + (q & 1); }
-__host__ __device__ inline int h_f2(int nt, int r, int j) { int e = h_e1(nt, r); return e < M0 ? e + M0 * j : -1; }
-__host__ __device__ inline int h_f3(int nt3, int r, int j3) { int f = h_f2(nt3 >> 1, r, nt3 & 1); return f < 0 ? -1 : f + M1 * j3; }
+template <int W> __host__ __device__ inline int h_f2(int nt, int r, int j) { int e = h_e1(nt, r); return e < W ? e + W * j : -1; }
+template <int W> __host__ __device__ inline int h_f3(int nt3, int r, int j3) { int f = h_f2<W>(nt3 >> 1, r, nt3 & 1); return f < 0 ? -1 : f + 2 * W * j3; }
 
 // Fragment-ordered embedding net for the fp16 tensor path.  NSW = 1 (hi only) or 2 (hi, lo) weight parts.
 // k-steps: a K of n tiles is consumed as n/2 k16 steps plus one k8 step if n is odd.
-template <int NSW>
+template <int NSW, int W = 25>
 struct EmbedNetFragH {
+    static constexpr int HNT2 = HW<W>::HNT2, HNT3 = HW<W>::HNT3;
     float w1[32], b1[32];                    // natural order e (zero padded)
     float b2[HNT2 * 8];                      // by position nt*8 + 2r + j
     float b3[HNT3 * 8];
     uint32_t W2f[NSW][2][HNT2][32][2];       // K = 32 (y1 slots, natural order e): 2 k16 steps
-    uint32_t W3f[NSW][4][HNT3][32][2];       // K = 56 positions: 3 k16 + 1 k8
-    uint32_t W3Tf[NSW][7][HNT2][32][2];      // K = 112 positions: 7 k16
-    uint32_t W2Tf[NSW][4][4][32][2];         // K = 56 positions: 3 k16 + 1 k8 ; N = 32 y1 slots (4 tiles)
+    uint32_t W3f[NSW][4][HNT3][32][2];       // K = HNT2 tiles: 3 k16 + 1 k8 (W = 25) / 4 k16 (W = 32)
+    uint32_t W3Tf[NSW][HNT3 / 2][HNT2][32][2];   // K = HNT3 tiles: HNT3 / 2 k16 steps
+    uint32_t W2Tf[NSW][4][4][32][2];         // K = HNT2 tiles: 3 k16 + 1 k8 / 4 k16 ; N = 32 y1 slots (4 tiles)
 };
 
 #ifdef __CUDACC__

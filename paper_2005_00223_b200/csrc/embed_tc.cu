@@ -208,12 +208,13 @@ k_env_rows(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTab tt,
     }
 }
 
-template <int NS, bool APPROX>
+template <int NS, bool APPROX, int W>
 __global__ void __launch_bounds__(256, (NS == 2 ? 2 : 1))
 k_embed_fwd_tc(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, const EmbedNetTC<(NS == 3 ? 2 : 1)> *__restrict__ nets,
                const int *__restrict__ bin_start, const int *__restrict__ rowstart, const float4 *__restrict__ rows_rh,
                const int2 *__restrict__ rows_id, float *__restrict__ Aout, unsigned long long *__restrict__ row_counter) {
     constexpr int NSW = NS == 3 ? 2 : 1;
+    constexpr int M2E = 4 * W;
     using SL = SmemLayout<NSW>;
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ uint32_t tmem_base_s;
@@ -291,7 +292,7 @@ k_embed_fwd_tc(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTab
 #pragma unroll
                     for (int t = 0; t < 16; ++t) {
                         const int p1 = 16 * h + t;
-                        y1[t] = t < tc_ce(h) ? act_tanh<APPROX>(fmaf(s, sw1[p1], sb1[p1])) : 0.f;
+                        y1[t] = t < tc_ce<W>(h) ? act_tanh<APPROX>(fmaf(s, sw1[p1], sb1[p1])) : 0.f;
                     }
                     store_chunk(smem + SL::A1H, smem + SL::A1L, 2 * h, row, y1);
                     store_chunk(smem + SL::A1H, smem + SL::A1L, 2 * h + 1, row, y1 + 8);
@@ -328,7 +329,7 @@ k_embed_fwd_tc(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTab
 #pragma unroll
                     for (int t = 0; t < 16; ++t) {
                         const int n = 32 * h + 16 * j + t;
-                        y2[16 * j + t] = t < tc_ce(h) ? y1[t] + act_tanh<APPROX>(z[t] + sb2[n]) : 0.f;
+                        y2[16 * j + t] = t < tc_ce<W>(h) ? y1[t] + act_tanh<APPROX>(z[t] + sb2[n]) : 0.f;
                     }
                     store_chunk(smem + SL::A2H, smem + SL::A2L, 4 * h + 2 * j, row, y2 + 16 * j);
                     store_chunk(smem + SL::A2H, smem + SL::A2L, 4 * h + 2 * j + 1, row, y2 + 16 * j + 8);
@@ -365,7 +366,7 @@ k_embed_fwd_tc(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTab
                     for (int t = 0; t < 16; ++t) {
                         const int c3 = 64 * h + 16 * q + t;
                         const int u = 16 * (q & 1) + t;
-                        gv[t] = t < tc_ce(h) ? y2[u] + act_tanh<APPROX>(z[t] + sb3[c3]) : 0.f;
+                        gv[t] = t < tc_ce<W>(h) ? y2[u] + act_tanh<APPROX>(z[t] + sb3[c3]) : 0.f;
                     }
                     store_chunk(smem + SL::GH, smem + SL::GL, 8 * h + 2 * q, row, gv);
                     store_chunk(smem + SL::GH, smem + SL::GL, 8 * h + 2 * q + 1, row, gv + 8);
@@ -401,7 +402,7 @@ k_embed_fwd_tc(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTab
                     // ---- E4: read-out: lane = layer-3 column c3, columns = 8*slot + c; h selects slots 3h..3h+2 ----
                     mbar_wait(&bars[2], ph2); ph2 ^= 1;
                     tc_fence_after();
-                    const int m = tc_m_of_c3(row);
+                    const int m = tc_m_of_c3<W>(row);
 #pragma unroll
                     for (int sl = 0; sl < TC_NSLOT / 2; ++sl) {
                         float v[8];
@@ -447,16 +448,17 @@ cudaError_t launch_env_rows(const dp_model *m, long N, const Grid3 &g, char *ws,
 
 namespace {
 
-template <int NS, bool APPROX>
+template <int NS, bool APPROX, int W>
 cudaError_t launch_fwd(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    constexpr int M2E = 4 * W;
     constexpr int NSW = NS == 3 ? 2 : 1;
     const int smem = SmemLayout<NSW>::TOTAL;
-    DP_SMEM_OPTIN((k_embed_fwd_tc<NS, APPROX>), smem);
+    DP_SMEM_OPTIN((k_embed_fwd_tc<NS, APPROX, W>), smem);
     const TypeTab tt = make_typetab(m);
     launch_env_rows(m, N, g, ws, L, st);
     cudaMemsetAsync(ws + L.A, 0, sizeof(float) * (size_t)N * 4 * M2E, st);
     const int grid = m->num_sms * (NS == 2 ? 2 : 1);
-    k_embed_fwd_tc<NS, APPROX><<<grid, 256, smem, st>>>(
+    k_embed_fwd_tc<NS, APPROX, W><<<grid, 256, smem, st>>>(
         N, m->T, g.ncell, m->Nm, tt, (const EmbedNetTC<NSW> *)m->embed_tc_dev, (int *)(ws + L.bin_start),
         (int *)(ws + L.rowstart), (const float4 *)(ws + L.rows_rh), (const int2 *)(ws + L.rows_id), (float *)(ws + L.A),
         (unsigned long long *)(ws + L.status + 8));
@@ -469,6 +471,6 @@ cudaError_t launch_fwd(const dp_model *m, long N, const Grid3 &g, char *ws, cons
 // MIX-16 models with a short neighbour row (Nm < 128, dp_model::fwd_split): activations as hi + lo pairs, fp16 weights,
 // tanh.approx; the single-fp16 activations of embed_tc2.cu average over too few rows there.
 cudaError_t launch_embed_fwd_tc(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    if (m->prec == DP_MIX32) return launch_fwd<3, false>(m, N, g, ws, L, st);
-    return launch_fwd<2, true>(m, N, g, ws, L, st);
+    if (m->prec == DP_MIX32) return m->m0 == 32 ? launch_fwd<3, false, 32>(m, N, g, ws, L, st) : launch_fwd<3, false, 25>(m, N, g, ws, L, st);
+    return launch_fwd<2, true, 25>(m, N, g, ws, L, st);
 }

@@ -17,17 +17,18 @@ constexpr int TC_ROWS = 128;
 constexpr int TC_K1 = 32, TC_N2 = 64, TC_N3 = 128;
 constexpr int TC_NSLOT = 6;       // atoms (contraction slots) per contraction pass: N = 8 * TC_NSLOT = 48
 
-__host__ __device__ inline int tc_e0(int h) { return h ? 13 : 0; }
-__host__ __device__ inline int tc_ce(int h) { return h ? 12 : 13; }
-__host__ __device__ inline int tc_e_of_p1(int p1) { int h = p1 >> 4, t = p1 & 15; return t < tc_ce(h) ? tc_e0(h) + t : -1; }
-__host__ __device__ inline int tc_f_of_n(int n) {
+// widths (W, 2 W, 4 W), W = 25 or 32: e0 = {0, 13} / {0, 16}, ce = {13, 12} / {16, 16}
+template <int W> __host__ __device__ inline int tc_e0(int h) { return h ? (W + 1) / 2 : 0; }
+template <int W> __host__ __device__ inline int tc_ce(int h) { return h ? W / 2 : (W + 1) / 2; }
+template <int W> __host__ __device__ inline int tc_e_of_p1(int p1) { int h = p1 >> 4, t = p1 & 15; return t < tc_ce<W>(h) ? tc_e0<W>(h) + t : -1; }
+template <int W> __host__ __device__ inline int tc_f_of_n(int n) {
     int h = n >> 5, j = (n >> 4) & 1, t = n & 15;
-    return t < tc_ce(h) ? tc_e0(h) + t + M0 * j : -1;
+    return t < tc_ce<W>(h) ? tc_e0<W>(h) + t + W * j : -1;
 }
-__host__ __device__ inline int tc_m_of_c3(int c3) {
+template <int W> __host__ __device__ inline int tc_m_of_c3(int c3) {
     int h = c3 >> 6, j3 = (c3 >> 5) & 1, u = c3 & 31;
-    int f = tc_f_of_n(32 * h + u);
-    return f < 0 ? -1 : f + M1 * j3;
+    int f = tc_f_of_n<W>(32 * h + u);
+    return f < 0 ? -1 : f + 2 * W * j3;
 }
 
 // One (centre type, neighbour type) embedding net as tcgen05 operand images.  NSW weight parts (hi [, lo]).

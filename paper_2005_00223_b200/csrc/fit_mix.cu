@@ -66,12 +66,14 @@ __global__ void __launch_bounds__(256) k_fitm_gemm(FitArgsF p) {
         if (!BT) {
             for (int c = tid; c < BK * (BN / 4); c += 256) {
                 const int k = c / (BN / 4), cc = c % (BN / 4);
-                cp_async16(Bs + k * BS_STRIDE + 4 * cc, Bw + (long)(k0 + k) * p.ldb + n0 + 4 * cc, true);
+                const bool okn = n0 + 4 * cc < p.N;
+                cp_async16(Bs + k * BS_STRIDE + 4 * cc, Bw + (long)(k0 + k) * p.ldb + (okn ? n0 + 4 * cc : 0), okn);
             }
         } else {
             for (int c = tid; c < BN * (BK / 4); c += 256) {
                 const int n = c / (BK / 4), c4 = c % (BK / 4);
-                cp_async16(Bs + n * BT_STRIDE + 4 * c4, Bw + (long)(n0 + n) * p.ldb + k0 + 4 * c4, true);
+                const bool okn = n0 + n < p.N;
+                cp_async16(Bs + n * BT_STRIDE + 4 * c4, Bw + (long)(okn ? n0 + n : 0) * p.ldb + k0 + 4 * c4, okn);
             }
         }
         cp_async_commit();
@@ -141,6 +143,7 @@ __global__ void __launch_bounds__(256) k_fitm_gemm(FitArgsF p) {
 #pragma unroll
             for (int nt = 0; nt < 5; ++nt) {
                 const int col = n0 + wn * 40 + nt * 8 + 2 * r;
+                if (col >= p.N) continue;          // N = 16 m2 need not be a multiple of the tile width
                 const long o = (long)row * p.ldo + col;
                 const float v0 = acc[mt][nt][2 * hrow], v1 = acc[mt][nt][2 * hrow + 1];
                 if (MODE == 0) {
@@ -177,7 +180,9 @@ __global__ void __launch_bounds__(256) k_fitm_gemm(FitArgsF p) {
         }
 }
 
+template <int W>
 __global__ void __launch_bounds__(256) k_descr_f(long N, const float *__restrict__ Amat, float *__restrict__ D) {
+    constexpr int M2E = HW<W>::M2E;
     __shared__ float sA[8][4 * M2E];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const long i = blockIdx.x * 8L + wid;
@@ -216,9 +221,10 @@ __global__ void __launch_bounds__(256) k_energy_f(long N, int T, int ncell, cons
 }
 
 // gA (fp32) -> scaled fp16 MMA fragments for the embedding backward (layout in embed_mix.cu)
-template <int NSW>
+template <int NSW, int W>
 __global__ void __launch_bounds__(128) k_gA_f(long N, const float *__restrict__ Amat, const float *__restrict__ gD,
                                               uint32_t *__restrict__ gAf, float *__restrict__ gscale) {
+    constexpr int M2E = HW<W>::M2E, HNT3 = HW<W>::HNT3, GP = 2 * HNT3;
     extern __shared__ float smg[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const long i = blockIdx.x * 4L + wid;
@@ -248,25 +254,25 @@ __global__ void __launch_bounds__(128) k_gA_f(long N, const float *__restrict__ 
     const float sc = ldexpf(1.f, -ex);
     if (lane == 0) gscale[i] = sc;
     __syncwarp();
-    uint32_t *out = gAf + i * (2 * 28 * 32);
+    uint32_t *out = gAf + i * (2 * GP * 32);
     const int g = lane >> 2, r = lane & 3;
     for (int nt3 = 0; nt3 < HNT3; ++nt3) {
-        const int f = h_f3(nt3, g >> 1, g & 1);
+        const int f = h_f3<W>(nt3, g >> 1, g & 1);
         float x = 0.f, y = 0.f;
         if (f >= 0 && r < 2) { x = sO[(2 * r) * M2E + f] * sc; y = sO[(2 * r + 1) * M2E + f] * sc; }
         uint32_t hi, lo;
         split_h2(x, y, hi, lo);
         out[nt3 * 32 + lane] = hi;
-        if (NSW == 2) out[(28 + nt3) * 32 + lane] = lo;
+        if (NSW == 2) out[(GP + nt3) * 32 + lane] = lo;
     }
     for (int t = 0; t < HNT3; ++t) {
-        const int f0 = h_f3(t, r, 0), f1 = h_f3(t, r, 1);
+        const int f0 = h_f3<W>(t, r, 0), f1 = h_f3<W>(t, r, 1);
         float x = 0.f, y = 0.f;
         if (f0 >= 0 && g < 4) { x = sO[g * M2E + f0] * sc; y = sO[g * M2E + f1] * sc; }
         uint32_t hi, lo;
         split_h2(x, y, hi, lo);
-        out[(14 + t) * 32 + lane] = hi;
-        if (NSW == 2) out[(28 + 14 + t) * 32 + lane] = lo;
+        out[(HNT3 + t) * 32 + lane] = hi;
+        if (NSW == 2) out[(GP + HNT3 + t) * 32 + lane] = lo;
     }
 }
 
@@ -280,7 +286,9 @@ cudaError_t launch_gemm(const FitArgsF &p, dim3 grid, cudaStream_t st) {
 
 }  // namespace
 
-cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+template <int W>
+static cudaError_t launch_fit_mix_w(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    constexpr int M2E = HW<W>::M2E;
     const int F = 240, ND = M2E * 16;
     const int T = m->T;
     float *Amat = (float *)(ws + L.A);
@@ -298,12 +306,12 @@ cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, 
     cudaError_t e = cudaSuccess;
     auto ok = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
 
-    k_descr_f<<<nb8, 256, 0, st>>>(N, Amat, D);
+    k_descr_f<W><<<nb8, 256, 0, st>>>(N, Amat, D);
     FitArgsF p{};
     p.ncell = g.ncell; p.bin_start = bin_start; p.v4 = v4; p.v4_type_stride = F; p.bias_type_stride = F;
     p.K = ND; p.N = F; p.A = D; p.lda = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.ldb = F; p.bias = c1;
     p.out0 = h1; p.ldo = F;
-    const dim3 g240(F / BN, gy, T), g1600(ND / BN, gy, T);
+    const dim3 g240(F / BN, gy, T), g1600((ND + BN - 1) / BN, gy, T);
     ok(launch_gemm<0>(p, g240, st));
     p.K = F; p.A = h1; p.lda = F; p.B = V2; p.b_type_stride = (long)F * F; p.bias = c2; p.aux0 = h1; p.out0 = t2; p.out1 = h2;
     ok(launch_gemm<1>(p, g240, st));
@@ -317,8 +325,12 @@ cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, 
     p.A = gz1; p.N = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.out0 = D; p.ldo = ND;
     ok(launch_gemm<5>(p, g1600, st));
     const int smem = 4 * (4 * M2E + M2E * 16 + 4 * M2E) * 4;
-    DP_SMEM_OPTIN(k_gA_f<2>, smem);
-    k_gA_f<2><<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, Amat, D, (uint32_t *)(ws + L.gAf), (float *)(ws + L.gscale));
+    DP_SMEM_OPTIN((k_gA_f<2, W>), smem);
+    k_gA_f<2, W><<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, Amat, D, (uint32_t *)(ws + L.gAf), (float *)(ws + L.gscale));
     ok(cudaGetLastError());
     return e;
+}
+
+cudaError_t launch_fit_mix(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    return m->m0 == 32 ? launch_fit_mix_w<32>(m, N, g, ws, L, st) : launch_fit_mix_w<25>(m, N, g, ws, L, st);
 }
