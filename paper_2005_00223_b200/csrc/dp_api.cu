@@ -51,7 +51,10 @@ WsLayout ws_layout(const dp_model *m, long N, long NE) {
         L.rowstart = take(sizeof(int) * ((size_t)N + 1) * m->T);
         L.rows_rh = take(sizeof(float) * 4 * (size_t)N * m->Nm);     // block b starts at row offset N*off[b]
         L.rows_id = take(sizeof(int) * 2 * (size_t)N * m->Nm);
-        if (m->prec == DP_MIX16) L.rows_g = take(sizeof(float) * 4 * (size_t)N * m->Nm);
+        if (m->prec == DP_MIX16) {
+            L.rows_g = take(sizeof(float) * 4 * (size_t)N * m->Nm);
+            L.multi_cnt = take(sizeof(int) * DP_MAX_TYPES * DP_MAX_TYPES);
+        }
     }
     const size_t esz = m->prec == DP_FP64 ? sizeof(double) : sizeof(float);
     const int nt3 = 2 * ((m->m0 + 3) / 4);          // EmbW<W>::NT3
@@ -544,7 +547,7 @@ int dp_launches_per_compute(const dp_model *m) {
     } else {
         n += 3 * m->T;                               // row prefix sums, one 3-launch scan per neighbour type
         n += 2;                                      // environment rows + tcgen05 forward
-        if (m->prec == DP_MIX16) n += 3 + 3;         // first layer, fused 240 x 240 chain, last product; gA fold, backward, force + virial
+        if (m->prec == DP_MIX16) n += 3 + 5;         // first layer, fused 240 x 240 chain, last product; gA fold, tile classes, backward (two launches), force + virial
         else n += 9 + 1;                             // descriptor, 6 GEMMs, energy, gA fragments; backward (with S8, S9)
     }
     return n + 1;                                    // finalize

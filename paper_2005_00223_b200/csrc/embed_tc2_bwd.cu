@@ -172,13 +172,34 @@ __device__ __forceinline__ void gradh16(const uint32_t (&g)[16], const uint32_t 
 
 constexpr int WGT = 128;       // threads per warpgroup: thread = row; every stage walks its two column halves h = 0, 1
 
-template <int W>
+// flag[a * T + b] = 1 if some 128-row tile of the (centre type a, neighbour type b) block spans more than T2_NSLOT atoms
+__global__ void __launch_bounds__(256) k_bwd_classify(long N, int T, int ncell, const __grid_constant__ TypeTab tt,
+                                                      const int *__restrict__ bin_start, const int *__restrict__ rowstart,
+                                                      const int2 *__restrict__ rows_id, int *__restrict__ flag) {
+    const int a = blockIdx.y / T, b = blockIdx.y % T;
+    const int ts0 = bin_start[a * ncell], ts1 = bin_start[(a + 1) * ncell];
+    if (ts0 == ts1) return;
+    const int rs = rowstart[(long)b * (N + 1) + ts0], re = rowstart[(long)b * (N + 1) + ts1];
+    const long rbase = N * (long)tt.off[b];
+    const long tile = blockIdx.x * 256L + threadIdx.x;
+    const long r0 = rs + tile * T2_ROWS;
+    if (r0 >= re) return;
+    const long rl = r0 + T2_ROWS - 1 < re ? r0 + T2_ROWS - 1 : re - 1;
+    if ((__ldg(&rows_id[rbase + rl]).x - __ldg(&rows_id[rbase + r0]).x) / T2_NSLOT > 0) flag[blockIdx.y] = 1;
+}
+
+// The products with the per-atom gradient images take T2_NSLOT atoms per pass.  MULTI = false serves the (centre, neighbour)
+// type blocks in which no 128-row tile spans more atoms than that (copper: >= 128 rows per atom): one pass, straight-line code.
+// MULTI = true serves the other blocks (short neighbour blocks: water) with pass loops.  k_bwd_classify sets the per-block
+// flag; each launch skips the blocks of the other kind.  Two kernels, not one with both paths: with both in one kernel
+// the single-pass path loses 3.4 % at config 4 (register allocation), and a per-tile branch in its loop head 1.3 %.
+template <int W, bool MULTI>
 __global__ void __launch_bounds__(NWG * WGT, 1)
 k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, const EmbedNetTC2<W> *__restrict__ nets,
                 const double *__restrict__ stdv, const int *__restrict__ bin_start, const int *__restrict__ rowstart,
                 const float4 *__restrict__ rows_rh, const int2 *__restrict__ rows_id, const uint8_t *__restrict__ gimg,
                 const float *__restrict__ gscale, float4 *__restrict__ rows_g, unsigned long long *__restrict__ row_counter,
-                long long *__restrict__ tdbg) {
+                const int *__restrict__ multi_flag, long long *__restrict__ tdbg) {
     using SL = BwdSmem<W>;
     using LY = T2<W>;
     constexpr int M0 = LY::M0, K3 = LY::K3, COLS = LY::COLS, GA_IMG_BYTES = COLS * 16, TM_DR = SL::TM_DR, QC = SL::QCOPIES;
@@ -255,6 +276,7 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
             const long rbase = N * (long)off[b];
             const int rs = rowstart[(long)b * (N + 1) + ts0], re = rowstart[(long)b * (N + 1) + ts1];
             const int ntiles = (re - rs + T2_ROWS - 1) / T2_ROWS;
+            if (ntiles == 0 || (multi_flag[a * T + b] != 0) != MULTI) continue;      // CTA-uniform
             __syncthreads();
             {   // stage the (a, b) net
                 const EmbedNetTC2<W> *net = nets + (a * T + b);
@@ -298,24 +320,24 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
                 if (tile + 1 < tile1) prefetch_rows(r0 + T2_ROWS, (tile + 1) & 1);
                 const int atom = id.x;
                 DP_TICK(17);
-                // T2_NSLOT atoms per pass; a tile that spans more atoms (short neighbour blocks) is recomputed per pass
-                for (int p0 = atom0; p0 <= atomL; p0 += T2_NSLOT) {
+                // A tile that spans more than T2_NSLOT atoms runs several passes over the SAME recomputed tile: a row is masked
+                // out of the passes of other atoms (its R image rows are zero), so the direct products dT = R^ g~ ACCUMULATE
+                // over the passes, and dR^ = T g~ is read out per pass by the rows of that pass.
+                const int npass = MULTI ? (atomL - atom0) / T2_NSLOT + 1 : 1;
+                const int slot = atom & (T2_NSLOT - 1);
+                                // operand images of one pass: R (A of the direct products) and the per-atom gradient images (async copies)
+                auto setup_images = [&](int p0) {
                     const bool in = atom >= p0 && atom - p0 < T2_NSLOT;
-                    const int slot = atom & (T2_NSLOT - 1);
-                    // operand images of this pass: R (A of the direct products) and the per-atom gradient images (async copies)
-                    {
-                        uint32_t rh01, rl01, rh23, rl23;
-                        tc::split_h2(rh.x, rh.y, rh01, rl01);
-                        tc::split_h2(rh.z, rh.w, rh23, rl23);
-                        const uint4 c0 = make_uint4(rh01, rh23, rh01, rh23), c1 = make_uint4(rl01, rl23, 0u, 0u), z4 = make_uint4(0u, 0u, 0u, 0u);
+                    uint32_t rh01, rl01, rh23, rl23;
+                    tc::split_h2(rh.x, rh.y, rh01, rl01);
+                    tc::split_h2(rh.z, rh.w, rh23, rl23);
+                    const uint4 c0 = make_uint4(rh01, rh23, rh01, rh23), c1 = make_uint4(rl01, rl23, 0u, 0u), z4 = make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll
-                        for (int s_ = 0; s_ < T2_NSLOT; ++s_) {
-                            const bool mine = in && slot == s_;
-                            *reinterpret_cast<uint4 *>(wgs + SL::RIMG + (2 * s_) * 2048 + t * 16) = mine ? c0 : z4;
-                            *reinterpret_cast<uint4 *>(wgs + SL::RIMG + (2 * s_ + 1) * 2048 + t * 16) = mine ? c1 : z4;
-                        }
+                    for (int s_ = 0; s_ < T2_NSLOT; ++s_) {
+                        const bool mine = in && slot == s_;
+                        *reinterpret_cast<uint4 *>(wgs + SL::RIMG + (2 * s_) * 2048 + t * 16) = mine ? c0 : z4;
+                        *reinterpret_cast<uint4 *>(wgs + SL::RIMG + (2 * s_ + 1) * 2048 + t * 16) = mine ? c1 : z4;
                     }
-                    DP_TICK(18);
                     for (int q = p0; q < p0 + T2_NSLOT && q <= atomL; ++q) {
                         const int s_ = q & (T2_NSLOT - 1);
                         const uint4 *C = reinterpret_cast<const uint4 *>(gimg + (long)q * GA_IMG_BYTES);
@@ -324,6 +346,10 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
                             if (QC == 2) cp_async16(s_qimg + (2 * s_ + 1) * (COLS * 16) + k * 16, C + k);
                         }
                     }
+                };
+                {
+                    setup_images(atom0);          // first pass: the copies land under the recomputed forward
+                    DP_TICK(18);
                     uint32_t d1p[2][8], d2p[2][16], d3p[2][HW3 / 2 + 2];   // 1 - t^2 per column half (fp16 pairs; only layer 3's are read back)
                     float d2f[2][32], d1f[2][16];     // layers 1-2 keep 1 - t^2 in fp32: fp16 here costs 2x in force error
                     DP_TICK(0);
@@ -433,34 +459,51 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
                     }
                     tc::wait_st();
                     // ---- backward ----
-                    cp_async_wait_all();
-                    DP_TICK(7);
-                    sync_issue();
-                    if (issuer_warp && tc::elect_one()) {
-                        tc::fence_after();
-                        constexpr uint32_t idr = tc::idesc(128, 8 * T2_NSLOT, false, true);
-#pragma unroll
-                        for (int ks = 0; ks < COLS / 16; ++ks) {
-                            const uint64_t db = tc::desc_at(d_qmn, ks * 256);
-                            tc::mma_ts(tmem + TM_DR, tmem + TM_T + 8 * ks, db, idr, ks > 0);
-                            tc::mma_ss(tmem + TM_DR, tc::desc_at(d_tlo, ks * 2 * 2048), db, idr, true);
-                        }
-                        constexpr uint32_t idg = tc::idesc(128, K3, false, false);
-#pragma unroll
-                        for (int ks = 0; ks < T2_NSLOT; ++ks)
-                            tc::mma_ss(tmem + TM_Z, tc::desc_at(d_rimg, ks * 2 * 2048), tc::desc_at(d_qk, T2_O3 * 16 + ks * QC * (COLS * 16)), idg, ks > 0);
-                        tc::commit(bar);
-                    }
+                    {
+                    const int NP = MULTI ? npass : 1;
                     float gsc = 1.f;
-                    if (in) gsc = __ldg(&gscale[atom]);
-                    DP_TICK(8);
-                    wait_mma();
+                    float dR[4] = {0.f, 0.f, 0.f, 0.f};
+                    for (int pi = 0; pi < NP; ++pi) {
+                        const int p0 = atom0 + pi * T2_NSLOT;
+                        const bool in = atom >= p0 && atom - p0 < T2_NSLOT;
+                        if (pi > 0) setup_images(p0);        // the products of the previous pass are complete (wait_mma below)
+                        cp_async_wait_all();
+                        DP_TICK(7);
+                        sync_issue();
+                        if (issuer_warp && tc::elect_one()) {
+                            tc::fence_after();
+                            constexpr uint32_t idr = tc::idesc(128, 8 * T2_NSLOT, false, true);
+#pragma unroll
+                            for (int ks = 0; ks < COLS / 16; ++ks) {
+                                const uint64_t db = tc::desc_at(d_qmn, ks * 256);
+                                tc::mma_ts(tmem + TM_DR, tmem + TM_T + 8 * ks, db, idr, ks > 0);
+                                tc::mma_ss(tmem + TM_DR, tc::desc_at(d_tlo, ks * 2 * 2048), db, idr, true);
+                            }
+                            constexpr uint32_t idg = tc::idesc(128, K3, false, false);
+#pragma unroll
+                            for (int ks = 0; ks < T2_NSLOT; ++ks)      // dT3 accumulates over the passes
+                                tc::mma_ss(tmem + TM_Z, tc::desc_at(d_rimg, ks * 2 * 2048), tc::desc_at(d_qk, T2_O3 * 16 + ks * QC * (COLS * 16)), idg, pi > 0 || ks > 0);
+                            tc::commit(bar);
+                        }
+                        if (in) gsc = __ldg(&gscale[atom]);
+                        DP_TICK(8);
+                        wait_mma();
+                        if (MULTI) {      // dR^ of the rows of this pass (a single pass reads it under E4 below)
+                            uint32_t v[16];
+                            tc::ld16(tm_lane + TM_DR, v);
+                            tc::wait_ld();
+                            if (in) {
+#pragma unroll
+                                for (int c = 0; c < 4; ++c)
+                                    dR[c] = slot ? __uint_as_float(v[8 + c]) + __uint_as_float(v[12 + c]) : __uint_as_float(v[c]) + __uint_as_float(v[4 + c]);
+                            }
+                        }
+                    }
                     DP_TICK(9);
                     // ---- E4: dR^ of this row; dz3 = dT3 (1 - t3^2) -> TMEM, over the hi parts of t3 ----
-                    float dR[4];
                     {
                         uint32_t v[16];                      // both slots: tcgen05.ld takes one warp-uniform address
-                        tc::ld16(tm_lane + TM_DR, v);
+                        if (!MULTI) tc::ld16(tm_lane + TM_DR, v);
 #pragma unroll
                         for (int h = 0; h < 2; ++h) {
 #pragma unroll
@@ -479,35 +522,51 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
                                         tc::pack_h2(__uint_as_float(g3[2]) * db.x, __uint_as_float(g3[3]) * db.y), 0u, 0u);
                             }
                         }
+                        if (!MULTI) {
 #pragma unroll
-                        for (int c = 0; c < 4; ++c)
-                            dR[c] = slot ? __uint_as_float(v[8 + c]) + __uint_as_float(v[12 + c]) : __uint_as_float(v[c]) + __uint_as_float(v[4 + c]);
+                            for (int c = 0; c < 4; ++c)
+                                dR[c] = slot ? __uint_as_float(v[8 + c]) + __uint_as_float(v[12 + c]) : __uint_as_float(v[c]) + __uint_as_float(v[4 + c]);
+                        }
                         tc::wait_st();
                     }
                     DP_TICK(10);
-                    sync_issue();
-                    if (issuer_warp && tc::elect_one()) {
-                        tc::fence_after();
-                        // dy2 first (the next stage needs it) ...
-                        constexpr uint32_t idy2 = tc::idesc(128, 64, false, false);
+                    // direct parts dT2, dT1 of the other passes first (their images are reloaded; the last pass's are still
+                    // resident and go last, together with the products of dz3)
+                    for (int pi = 0; pi < NP; ++pi) {
+                        const bool last = pi == NP - 1;
+                        if (!last) { setup_images(atom0 + pi * T2_NSLOT); cp_async_wait_all(); }
+                        else if (MULTI) { setup_images(atom0 + pi * T2_NSLOT); cp_async_wait_all(); }
+                        sync_issue();
+                        if (issuer_warp && tc::elect_one()) {
+                            tc::fence_after();
+                            constexpr uint32_t idy2 = tc::idesc(128, 64, false, false);
+                            constexpr uint32_t idy1 = tc::idesc(128, 32, false, false);
 #pragma unroll
-                        for (int ks = 0; ks < T2_NSLOT; ++ks)      // direct part dT2 -> accumulator columns [32,96)
-                            tc::mma_ss(tmem + TM_Z + 32, tc::desc_at(d_rimg, ks * 2 * 2048), tc::desc_at(d_qk, T2_O2 * 16 + ks * QC * (COLS * 16)), idy2, ks > 0);
+                            for (int ks = 0; ks < T2_NSLOT; ++ks)      // direct part dT2 -> accumulator columns [32,96)
+                                tc::mma_ss(tmem + TM_Z + 32, tc::desc_at(d_rimg, ks * 2 * 2048), tc::desc_at(d_qk, T2_O2 * 16 + ks * QC * (COLS * 16)), idy2, pi > 0 || ks > 0);
+                            if (!last) {
 #pragma unroll
-                        for (int ks = 0; ks < K3 / 16; ++ks)
-                            tc::mma_ts(tmem + TM_Z + 32, tmem + TM_T + 48 + 8 * ks, tc::desc_at(d_w3t, 32 * 16 + ks * 2 * (96 * 16)), idy2, true);
-                        tc::commit(bar);
-                        // ... then the part of dy1 that does not depend on dz2 (waited for with the last stage)
-                        constexpr uint32_t idy1 = tc::idesc(128, 32, false, false);
+                                for (int ks = 0; ks < T2_NSLOT; ++ks)  // direct part dT1 -> accumulator columns [0,32)
+                                    tc::mma_ss(tmem + TM_Z, tc::desc_at(d_rimg, ks * 2 * 2048), tc::desc_at(d_qk, ks * QC * (COLS * 16)), idy1, pi > 0 || ks > 0);
+                                tc::commit(bar);
+                            } else {
+                                // dy2 first (the next stage needs it) ...
 #pragma unroll
-                        for (int ks = 0; ks < T2_NSLOT; ++ks)      // direct part dT1 -> accumulator columns [0,32)
-                            tc::mma_ss(tmem + TM_Z, tc::desc_at(d_rimg, ks * 2 * 2048), tc::desc_at(d_qk, ks * QC * (COLS * 16)), idy1, ks > 0);
+                                for (int ks = 0; ks < K3 / 16; ++ks)
+                                    tc::mma_ts(tmem + TM_Z + 32, tmem + TM_T + 48 + 8 * ks, tc::desc_at(d_w3t, 32 * 16 + ks * 2 * (96 * 16)), idy2, true);
+                                tc::commit(bar);
+                                // ... then the part of dy1 that does not depend on dz2 (waited for with the last stage)
 #pragma unroll
-                        for (int ks = 0; ks < K3 / 16; ++ks)
-                            tc::mma_ts(tmem + TM_Z, tmem + TM_T + 48 + 8 * ks, tc::desc_at(d_w3t, ks * 2 * (96 * 16)), idy1, true);
+                                for (int ks = 0; ks < T2_NSLOT; ++ks)
+                                    tc::mma_ss(tmem + TM_Z, tc::desc_at(d_rimg, ks * 2 * 2048), tc::desc_at(d_qk, ks * QC * (COLS * 16)), idy1, pi > 0 || ks > 0);
+#pragma unroll
+                                for (int ks = 0; ks < K3 / 16; ++ks)
+                                    tc::mma_ts(tmem + TM_Z, tmem + TM_T + 48 + 8 * ks, tc::desc_at(d_w3t, ks * 2 * (96 * 16)), idy1, true);
+                            }
+                        }
+                        DP_TICK(11);
+                        wait_mma();
                     }
-                    DP_TICK(11);
-                    wait_mma();
                     DP_TICK(12);
                     // ---- E5: dz2 = dy2 (1 - t2^2) -> TMEM, over the hi parts of t2 ----
 #pragma unroll
@@ -560,14 +619,15 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
                             }
                         }
                         // gradient of E with respect to this row of the environment matrix R~ (S8 + S9 run in k_prod_force_virial)
-                        if (in) {
+                        if (atom >= 0) {
                             const float osc = 1.0f / ((float)Nm * gsc);
                             rows_g[rbase + r0 + t] = make_float4((dR[0] + ds) * osc * isd[0], dR[1] * osc * isd[1], dR[2] * osc * isd[2],
                                                                  dR[3] * osc * isd[3]);
                         }
                     }
+                    }
                     DP_TICK(16);
-                }   // passes
+                }
                 if (tw == 0) my_rows += (unsigned long long)nrows;
             }
         }
@@ -678,7 +738,8 @@ k_prod_force_virial(long N, int T, const __grid_constant__ TypeTab tt, EnvParams
 
 template <int W>
 static cudaError_t launch_bwd_w(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    DP_SMEM_OPTIN(k_embed_bwd_tc2<W>, BwdSmem<W>::TOTAL);
+    DP_SMEM_OPTIN((k_embed_bwd_tc2<W, false>), BwdSmem<W>::TOTAL);
+    DP_SMEM_OPTIN((k_embed_bwd_tc2<W, true>), BwdSmem<W>::TOTAL);
     const TypeTab tt = make_typetab(m);
     EnvParams ep;
     ep.rc = m->rc; ep.rc_smth = m->rc_smth; ep.inv_range = 1.0 / (m->rc - m->rc_smth);
@@ -692,11 +753,26 @@ static cudaError_t launch_bwd_w(const dp_model *m, long N, const Grid3 &g, char 
     tdbg = tbuf;
 #endif
     if (m->profile) cudaEventRecord(m->ev[6], st);
-    k_embed_bwd_tc2<W><<<m->num_sms, NWG * WGT, BwdSmem<W>::TOTAL, st>>>(
+    int *multi_flag = (int *)(ws + L.multi_cnt);
+    cudaMemsetAsync(multi_flag, 0, sizeof(int) * DP_MAX_TYPES * DP_MAX_TYPES, st);
+    {
+        int maxsel = 0;
+        for (int b = 0; b < m->T; ++b) maxsel = m->sel[b] > maxsel ? m->sel[b] : maxsel;
+        const long maxtiles = (N * (long)maxsel + T2_ROWS - 1) / T2_ROWS + 1;
+        k_bwd_classify<<<dim3((unsigned)((maxtiles + 255) / 256), (unsigned)(m->T * m->T)), 256, 0, st>>>(
+            N, m->T, g.ncell, tt, (int *)(ws + L.bin_start), (int *)(ws + L.rowstart), (const int2 *)(ws + L.rows_id), multi_flag);
+    }
+    k_embed_bwd_tc2<W, false><<<m->num_sms, NWG * WGT, BwdSmem<W>::TOTAL, st>>>(
         N, m->T, g.ncell, m->Nm, tt, (const EmbedNetTC2<W> *)m->embed_tc2_dev, m->std_dev, (int *)(ws + L.bin_start),
         (int *)(ws + L.rowstart), (const float4 *)(ws + L.rows_rh), (const int2 *)(ws + L.rows_id),
         (const uint8_t *)(ws + L.gAf), (const float *)(ws + L.gscale), (float4 *)(ws + L.rows_g),
-        (unsigned long long *)(ws + L.status + 16), tdbg);
+        (unsigned long long *)(ws + L.status + 16), multi_flag, tdbg);
+    // the blocks with tiles that span more than T2_NSLOT atoms (none for copper: the launch finds no block of its kind)
+    k_embed_bwd_tc2<W, true><<<m->num_sms, NWG * WGT, BwdSmem<W>::TOTAL, st>>>(
+        N, m->T, g.ncell, m->Nm, tt, (const EmbedNetTC2<W> *)m->embed_tc2_dev, m->std_dev, (int *)(ws + L.bin_start),
+        (int *)(ws + L.rowstart), (const float4 *)(ws + L.rows_rh), (const int2 *)(ws + L.rows_id),
+        (const uint8_t *)(ws + L.gAf), (const float *)(ws + L.gscale), (float4 *)(ws + L.rows_g),
+        (unsigned long long *)(ws + L.status + 16), multi_flag, nullptr);
     if (m->profile) cudaEventRecord(m->ev[7], st);
     k_prod_force_virial<<<m->num_sms * 8, 256, 0, st>>>(N, m->T, tt, ep, (int *)(ws + L.rowstart),
                                                         (const int2 *)(ws + L.rows_id), (const float4 *)(ws + L.rows_g),
