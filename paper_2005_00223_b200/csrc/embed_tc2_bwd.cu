@@ -473,10 +473,14 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
                         if (issuer_warp && tc::elect_one()) {
                             tc::fence_after();
                             constexpr uint32_t idr = tc::idesc(128, 8 * T2_NSLOT, false, true);
+                            // dR^ = T g~.  Single pass: only the t3 columns of T must be read before E4 overwrites them with dz3;
+                            // the t1 / t2 part (12 small MMAs) is issued behind the commit, off the E3 -> E4 critical path, and is
+                            // covered by the next commit (E5 is the first stage that overwrites t2); dR^ is read in E6
+                            constexpr int KS_A = MULTI ? 0 : T2_O3 / 16;
 #pragma unroll
-                            for (int ks = 0; ks < COLS / 16; ++ks) {
+                            for (int ks = KS_A; ks < COLS / 16; ++ks) {
                                 const uint64_t db = tc::desc_at(d_qmn, ks * 256);
-                                tc::mma_ts(tmem + TM_DR, tmem + TM_T + 8 * ks, db, idr, ks > 0);
+                                tc::mma_ts(tmem + TM_DR, tmem + TM_T + 8 * ks, db, idr, ks > KS_A);
                                 tc::mma_ss(tmem + TM_DR, tc::desc_at(d_tlo, ks * 2 * 2048), db, idr, true);
                             }
                             constexpr uint32_t idg = tc::idesc(128, K3, false, false);
@@ -484,11 +488,17 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
                             for (int ks = 0; ks < T2_NSLOT; ++ks)      // dT3 accumulates over the passes
                                 tc::mma_ss(tmem + TM_Z, tc::desc_at(d_rimg, ks * 2 * 2048), tc::desc_at(d_qk, T2_O3 * 16 + ks * QC * (COLS * 16)), idg, pi > 0 || ks > 0);
                             tc::commit(bar);
+#pragma unroll
+                            for (int ks = 0; ks < KS_A; ++ks) {
+                                const uint64_t db = tc::desc_at(d_qmn, ks * 256);
+                                tc::mma_ts(tmem + TM_DR, tmem + TM_T + 8 * ks, db, idr, true);
+                                tc::mma_ss(tmem + TM_DR, tc::desc_at(d_tlo, ks * 2 * 2048), db, idr, true);
+                            }
                         }
                         if (in) gsc = __ldg(&gscale[atom]);
                         DP_TICK(8);
                         wait_mma();
-                        if (MULTI) {      // dR^ of the rows of this pass (a single pass reads it under E4 below)
+                        if (MULTI) {      // dR^ of the rows of this pass (a single pass reads it in E6)
                             uint32_t v[16];
                             tc::ld16(tm_lane + TM_DR, v);
                             tc::wait_ld();
@@ -500,10 +510,8 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
                         }
                     }
                     DP_TICK(9);
-                    // ---- E4: dR^ of this row; dz3 = dT3 (1 - t3^2) -> TMEM, over the hi parts of t3 ----
+                    // ---- E4: dz3 = dT3 (1 - t3^2) -> TMEM, over the hi parts of t3 ----
                     {
-                        uint32_t v[16];                      // both slots: tcgen05.ld takes one warp-uniform address
-                        if (!MULTI) tc::ld16(tm_lane + TM_DR, v);
 #pragma unroll
                         for (int h = 0; h < 2; ++h) {
 #pragma unroll
@@ -521,11 +529,6 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
                                 tc::st4(tm_lane + TM_T + 96, tc::pack_h2(__uint_as_float(g3[0]) * da.x, __uint_as_float(g3[1]) * da.y),
                                         tc::pack_h2(__uint_as_float(g3[2]) * db.x, __uint_as_float(g3[3]) * db.y), 0u, 0u);
                             }
-                        }
-                        if (!MULTI) {
-#pragma unroll
-                            for (int c = 0; c < 4; ++c)
-                                dR[c] = slot ? __uint_as_float(v[8 + c]) + __uint_as_float(v[12 + c]) : __uint_as_float(v[c]) + __uint_as_float(v[4 + c]);
                         }
                         tc::wait_st();
                     }
@@ -606,6 +609,14 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
                     // ---- E6: ds^ = sum_e dy1 (1 - t1^2) w1; gradient of the environment row; S8 + S9 in fp64 ----
                     {
                         float ds = 0.f;
+                        if (!MULTI) {      // dR^ is complete only now (its t1 / t2 part was issued behind the dT3 commit)
+                            uint32_t v[16];
+                            tc::ld16(tm_lane + TM_DR, v);
+                            tc::wait_ld();
+#pragma unroll
+                            for (int c = 0; c < 4; ++c)
+                                dR[c] = slot ? __uint_as_float(v[8 + c]) + __uint_as_float(v[12 + c]) : __uint_as_float(v[c]) + __uint_as_float(v[4 + c]);
+                        }
 #pragma unroll
                         for (int h = 0; h < 2; ++h) {
                             uint32_t g0[16];
