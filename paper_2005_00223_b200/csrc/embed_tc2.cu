@@ -273,13 +273,15 @@ k_embed_fwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
                 // ---- E3 ----
                 {
                     uint8_t *img = timg_row + (T2_O3 / 8) * 2048;
+                    {   // the first 96 columns in six groups of 16, each TMEM load one group ahead of its tanh work
+                        uint32_t zb[2][16];
+                        tc::ld16(tm_lane + TM_Z, zb[0]);
 #pragma unroll
-                    for (int h = 0; h < 2; ++h) {
-                        uint32_t z0[16], z1[16], z2[16];
-                        tc::ld16(tm_lane + TM_Z + 48 * h, z0); tc::ld16(tm_lane + TM_Z + 48 * h + 16, z1);
-                        tc::ld16(tm_lane + TM_Z + 48 * h + 32, z2);
-                        tc::wait_ld();
-                        tanh16_store(z0, img, 6 * h); tanh16_store(z1, img, 6 * h + 2); tanh16_store(z2, img, 6 * h + 4);
+                        for (int u = 0; u < 6; ++u) {
+                            tc::wait_ld();
+                            if (u + 1 < 6) tc::ld16(tm_lane + TM_Z + 16 * (u + 1), zb[(u + 1) & 1]);
+                            tanh16_store(zb[u & 1], img, 2 * u);
+                        }
                     }
                     if (W == 25) {
                         uint32_t z3[4];
