@@ -211,6 +211,33 @@ def kernels_of(s, r, ms_step):
             "step_tflops": (rr * (FLOP_ROW_FWD + FLOP_ROW_BWD) + N * FLOP_ATOM_FIT) / (ms_step * 1e-3) / 1e12}
 
 
+def sweep_leg(args, binding, torch, synth, dev, flush, pk):
+    """Network-size study (Fig. 7): copper, embedding nets (W, 2 W, 4 W), last layer 2 W x 4 W from the
+    paper's 64 x 128 to 1024 x 2048, MIX-16.  Algorithmic flops of the whole evaluation / CUDA-event time of the evaluation."""
+    rows = []
+    for W in [int(x) for x in args.sweep_widths.split(",")]:
+        ncell = args.sweep_ncell
+        s = (synth.paper_copper(ncell, synth.SEED0 + 20, shuffle=True, precision="mix16") if W == 32
+             else synth.wide_copper(ncell, W, synth.SEED0 + 20, shuffle=True))
+        r = time_config(binding, torch, s, dev, args.steps, args.warmup, flush)
+        ms = r["t_ms"] / args.steps
+        ff, fb, fa, _ = flops_of(s.model)
+        ph, rr = r["phases"], r["real_rows"]
+        emb = rr * (ff + fb)
+        rows.append({"W": W, "last_layer": f"{2 * W}x{4 * W}", "natoms": s.natoms, "real_neighbour_rows": rr, "ms_per_step": ms,
+                     "atom_steps_per_s": s.natoms / (ms * 1e-3),
+                     "step_tflops": (emb + s.natoms * fa) / (ms * 1e-3) / 1e12,
+                     "embed_fwd_ms": ph[1], "fit_ms": ph[2], "embed_bwd_ms": ph[3], "nlist_ms": ph[0],
+                     "embed_fwd_bwd_tflops": emb / ((ph[1] + ph[3]) * 1e-3) / 1e12,
+                     "bwd_gemm_ms": ph[5] if W != 32 else None,
+                     "bwd_gemm_tflops": (rr * 2 * (W * 2 * W + 2 * W * 4 * W) / (ph[5] * 1e-3) / 1e12) if W != 32 else None,
+                     "frac_of_bf16_sustained": (emb + s.natoms * fa) / (ms * 1e-3) / 1e12 / pk["bf16_sus"]})
+        r["model"].close()
+        del r
+        torch.cuda.empty_cache()
+    return rows
+
+
 def max_over_ranks(times_ms, world, device):
     """Replicas only: every rank times the same number of steps of its own replica; the job time is the
     MAX over ranks (one all-reduce of the timings, no data-path collective)."""
@@ -277,12 +304,15 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="4",
                     help="BASELINE.json configs index 0..4 (default: 4 = copper 1,048,576 atoms MIX-16, the largest single-GPU "
-                         "config), or paper_cu / paper_water: the paper's network shape (32, 64, 128), capacity 512 / 144 (PAPER.md:151)")
+                         "config), or paper_cu / paper_water: the paper's network shape (32, 64, 128), capacity 512 / 144 (PAPER.md:151), "
+                         "or sweep: the network-size study of PAPER.md:273-279 (copper, last embedding layer 64 x 128 ... 1024 x 2048, MIX-16)")
     ap.add_argument("--no-summary", action="store_true", help="skip the configs_summary leg (the other four configs)")
     ap.add_argument("--precision", default=None, choices=["fp64", "mix32", "mix16"],
                     help="override the config's precision (profiling aid; the default is the precision BASELINE.json names)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep-widths", default="32,64,128,256,512", help="--config sweep: first embedding widths W (nets W, 2 W, 4 W)")
+    ap.add_argument("--sweep-ncell", type=int, default=16, help="--config sweep: FCC cells per edge (atoms = 4 n^3)")
     ap.add_argument("--md-steps", type=int, default=100,
                     help="also time an MD loop of this many velocity-Verlet steps (dp_md_run; 0 = skip; N = 1 only)")
     args = ap.parse_args()
@@ -318,11 +348,26 @@ def main():
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=dev)
 
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > L2 (126 MB)
+    if args.config == "sweep":
+        if rank == 0:
+            pk = peaks()
+            sampler = ClockSampler(local_rank)
+            sampler.start()
+            rows = sweep_leg(args, binding, torch, synth, dev, flush, pk)
+            clocks = sampler.stop()
+            print(json.dumps({"metric": "network_size_sweep_step_tflops", "value": max(x["step_tflops"] for x in rows),
+                              "unit": "TFLOP/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "higher_is_better": True,
+                              "dtype": "f16", "data": "synthetic", "vs_baseline": None,
+                              "config": {"workload": "sweep_cu (PAPER.md:273-279, Fig. 7)", "precision": "mix16",
+                                         "l2": "256 MB flush between timed steps"},
+                              "peak": {"bf16_sustained_tflops": pk["bf16_sus"], "source": pk["src"]},
+                              "sweep": rows, "clocks": clocks}))
+        return
     s = workload()
     if args.precision:
         s.precision = args.precision
     N = s.natoms
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > L2 (126 MB)
     st = torch.cuda.current_stream(dev)
     coords_h = torch.from_numpy(s.coords).pin_memory()
     types_h = torch.from_numpy(s.types).pin_memory()

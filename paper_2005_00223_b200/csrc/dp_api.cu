@@ -59,7 +59,8 @@ WsLayout ws_layout(const dp_model *m, long N, long NE) {
     const size_t esz = m->prec == DP_FP64 ? sizeof(double) : sizeof(float);
     const int nt3 = 2 * ((m->m0 + 3) / 4);          // EmbW<W>::NT3
     L.A = take(esz * (size_t)N * 4 * m->m2);
-    if (m->prec == DP_FP64) L.gAf = take(sizeof(double) * (size_t)N * 3 * nt3 * 32);
+    if (m->wide) L.gAf = take(0);                   // the wide path reads gA itself
+    else if (m->prec == DP_FP64) L.gAf = take(sizeof(double) * (size_t)N * 3 * nt3 * 32);
     else L.gAf = take(sizeof(uint32_t) * (size_t)N * 2 * (2 * nt3) * 32);     // MIX-32 fragments / MIX-16 operand image (smaller)
     L.gscale = take(sizeof(float) * (size_t)N);
     // (MIX-16: buffers 2..6 also hold the gz1 operand images, one per 128-row tile and at least one per type: the pad
@@ -69,6 +70,14 @@ WsLayout ws_layout(const dp_model *m, long N, long NE) {
     L.eatom = take(sizeof(double) * (size_t)N);
     L.fsorted = take(sizeof(double) * 3 * (size_t)NE);
     L.virial = take(sizeof(double) * 16);
+    if (m->wide) {      // activation images of the wide-network path: 128 rows x 9 W fp16 per tile (wide.cu)
+        const size_t tiles = (size_t)wide_tiles_cap(m, N), chunk = 2048;
+        L.wide_tab = take(sizeof(int) * 4 * ((size_t)m->T * m->T + 1));
+        L.wide_t1 = take(tiles * (m->m0 / 8) * chunk);
+        L.wide_y2 = take(tiles * (m->m1 / 8) * chunk);
+        L.wide_t2 = take(tiles * (m->m1 / 8) * chunk);
+        L.wide_t3 = take(tiles * (m->m2 / 8) * chunk);
+    }
     L.total = o;
     return L;
 }
@@ -407,11 +416,14 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
     if (T < 1 || T > DP_MAX_TYPES) return DP_EINVAL;
     if (!(rc > 0) || !(rc_smth >= 0) || !(rc_smth < rc) || !(rc * rc < 128.0)) return DP_EINVAL;
     // embedding widths (W, 2 W, 4 W) with W = 25 (BASELINE configs) or W = 32 (the paper's own networks)
+    // or, MIX-16 only, the wide nets of the network-size study W = 64, 128, 256, 512 (wide.cu)
     const int W0 = w->embed_widths[0];
-    if ((W0 != 25 && W0 != 32) || w->embed_widths[1] != 2 * W0 || w->embed_widths[2] != 4 * W0 || w->axis != 16 ||
+    const bool wide = W0 == 64 || W0 == 128 || W0 == 256 || W0 == 512;
+    if ((W0 != 25 && W0 != 32 && !wide) || w->embed_widths[1] != 2 * W0 || w->embed_widths[2] != 4 * W0 || w->axis != 16 ||
         w->fit_widths[0] != 240 || w->fit_widths[1] != 240 || w->fit_widths[2] != 240)
         return DP_EUNSUPPORTED;
     if (W0 == 32 && !paper_shape_supported(prec)) return DP_EUNSUPPORTED;
+    if (wide && prec != DP_MIX16) return DP_EUNSUPPORTED;
     if (prec != DP_FP64 && prec != DP_MIX32 && prec != DP_MIX16) return DP_EINVAL;
     int maxsel = 0, Nm = 0;
     for (int b = 0; b < T; ++b) { if (sel[b] <= 0) return DP_EINVAL; Nm += sel[b]; if (sel[b] > maxsel) maxsel = sel[b]; }
@@ -426,6 +438,7 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
     m->device = dev;
     m->T = T; m->Nm = Nm; m->axis = 16; m->F = 240; m->rc = rc; m->rc_smth = rc_smth; m->prec = prec;
     m->m0 = W0; m->m1 = 2 * W0; m->m2 = 4 * W0;
+    m->wide = wide ? 1 : 0;
     m->n_type_map = n_type_map;
     for (int b = 0; b < T; ++b) { m->sel[b] = sel[b]; m->off[b + 1] = m->off[b] + sel[b]; }
     int cap = 256;
@@ -464,6 +477,13 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
             for (int ab = 0; ab < T * T; ++ab) build_embed_tc<2, 25>(w->embed + ab * ensz, &nets[ab]);
         }
         ok(upload(nets, &m->embed_tc_dev));
+    } else if (wide) {                  // MIX-16, wide nets: one tcgen05 GEMM per layer (wide.cu)
+        const size_t ie = wide_net_img_elems(W0);
+        std::vector<float> vec((size_t)T * T * 8 * W0);
+        std::vector<__half> img((size_t)T * T * ie);
+        for (int ab = 0; ab < T * T; ++ab) wide_build_net(W0, w->embed + ab * ensz, &vec[(size_t)ab * 8 * W0], &img[(size_t)ab * ie]);
+        ok(upload(vec, &m->wide_vec_dev));
+        ok(upload(img, &m->wide_img_dev));
     } else {                            // MIX-16: warpgroup-per-tile tcgen05 kernels (embed_tc2*.cu)
         if (W0 == 32) {
             std::vector<EmbedNetTC2<32>> nets((size_t)T * T);
@@ -524,7 +544,7 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
 
 void dp_destroy(dp_model *m) {
     if (!m) return;
-    void *ptrs[] = {m->type_map_dev, m->embed_frag_dev, m->embed_tc_dev, m->embed_tc2_dev, m->fit_tc_img_dev, m->avg_dev, m->std_dev, m->ebias_dev, m->fitV1_dev, m->fitV2_dev,
+    void *ptrs[] = {m->wide_vec_dev, m->wide_img_dev, m->type_map_dev, m->embed_frag_dev, m->embed_tc_dev, m->embed_tc2_dev, m->fit_tc_img_dev, m->avg_dev, m->std_dev, m->ebias_dev, m->fitV1_dev, m->fitV2_dev,
                     m->fitV3_dev, m->fitc1_dev, m->fitc2_dev, m->fitc3_dev, m->fitv4_dev, m->fitc4_dev};
     for (void *p : ptrs) if (p) cudaFree(p);
     if (m->ev[0]) for (int k = 0; k < DP_NEVENTS; ++k) cudaEventDestroy(m->ev[k]);
@@ -547,7 +567,8 @@ int dp_launches_per_compute(const dp_model *m) {
     } else {
         n += 3 * m->T;                               // row prefix sums, one 3-launch scan per neighbour type
         n += 2;                                      // environment rows + tcgen05 forward
-        if (m->prec == DP_MIX16) n += 3 + 5;         // first layer, fused 240 x 240 chain, last product; gA fold, tile classes, backward (two launches), force + virial
+        if (m->wide) n += 4 + 3 + 5;                 // tile table, layer 1, two GEMMs, contraction; fitting (3); scale, head, two GEMMs, force + virial
+        else if (m->prec == DP_MIX16) n += 3 + 5;    // first layer, fused 240 x 240 chain, last product; gA fold, tile classes, backward (two launches), force + virial
         else n += 9 + 1;                             // descriptor, 6 GEMMs, energy, gA fragments; backward (with S8, S9)
     }
     return n + 1;                                    // finalize
@@ -593,11 +614,13 @@ int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *ty
     const bool f64 = m->prec == DP_FP64;
     const bool m16 = m->prec == DP_MIX16;
     ok(f64 ? launch_embed_fwd_f64(m, natoms, g, ws, L, st)
+           : m->wide ? launch_embed_fwd_wide(m, natoms, g, ws, L, st)
            : (m16 && !m->fwd_split ? launch_embed_fwd_tc2(m, natoms, g, ws, L, st) : launch_embed_fwd_tc(m, natoms, g, ws, L, st)));
     mark(2);
     ok(f64 ? launch_fit_f64(m, natoms, g, ws, L, st) : (m16 ? launch_fit_tc(m, natoms, g, ws, L, st) : launch_fit_mix(m, natoms, g, ws, L, st)));
     mark(3);
     ok(f64 ? launch_embed_bwd_f64(m, natoms, g, ws, L, st)
+           : m->wide ? launch_embed_bwd_wide(m, natoms, g, ws, L, st)
            : (m16 ? launch_embed_bwd_tc2(m, natoms, g, ws, L, st) : launch_embed_bwd_mix(m, natoms, g, ws, L, st)));
     if (g.ghost) ok(launch_fold_ghost(m, natoms, g, ws, L, st));
     mark(4);

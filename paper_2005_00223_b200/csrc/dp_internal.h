@@ -68,7 +68,10 @@ struct dp_model {
     int sel[DP_MAX_TYPES];
     int off[DP_MAX_TYPES + 1];
     int Nm;
-    int m0, m1, m2;                 // embedding widths (W, 2 W, 4 W): (25, 50, 100) or (32, 64, 128)
+    int m0, m1, m2;                 // embedding widths (W, 2 W, 4 W): (25, 50, 100), (32, 64, 128), or wide: W = 64 ... 512
+    int wide;                       // MIX-16 with W >= 64: layer-by-layer GEMM path with activations in HBM (wide.cu)
+    void *wide_vec_dev;             // wide: [T*T][8 W] floats w1, b1, b2, b3
+    void *wide_img_dev;             // wide: [T*T][20 W^2] fp16 weight images W2, W3, W3^T, W2^T
     int axis;                       // 16
     int F;                          // fitting width 240
     double rc, rc_smth;
@@ -143,6 +146,9 @@ struct WsLayout {
     size_t ext_scode;   // int[cap_ext] packed image shift of sorted item e
     size_t gcnt;        // int[N] ghosts per atom
     size_t gstart;      // int[N+1]
+    // wide networks (wide.cu): tile table and the activation images, per 128-row tile [columns / 8][128][8] fp16
+    size_t wide_tab;    // int4[T*T + 1]
+    size_t wide_t1, wide_y2, wide_t2, wide_t3;      // W, 2 W, 2 W, 4 W columns
 };
 
 // neighbour capacities per type and their prefix sums, passed to kernels by value (a __grid_constant__ parameter: indexed
@@ -197,6 +203,13 @@ cudaError_t launch_embed_fwd_tc(const dp_model *m, long N, const Grid3 &g, char 
 cudaError_t launch_embed_fwd_tc2(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_embed_bwd_tc2(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_fit_tc(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+cudaError_t launch_prod_force_virial(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+// wide networks (wide.cu)
+cudaError_t launch_embed_fwd_wide(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+cudaError_t launch_embed_bwd_wide(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+size_t wide_net_img_elems(int W);
+void wide_build_net(int W, const double *net, float *vec, struct __half *img);
+long wide_tiles_cap(const dp_model *m, long N);
 size_t fit_tc_type_elems(int nd);
 void fit_tc_build_type(int nd, const double *V1, const double *V2, const double *V3, struct __half *out);
 cudaError_t launch_env_rows(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);

@@ -819,6 +819,18 @@ static cudaError_t launch_bwd_w(const dp_model *m, long N, const Grid3 &g, char 
     return cudaGetLastError();
 }
 
+// S8 + S9 from the per-row gradients in rows_g (also the tail of the wide-network backward, wide.cu)
+cudaError_t launch_prod_force_virial(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    const TypeTab tt = make_typetab(m);
+    EnvParams ep;
+    ep.rc = m->rc; ep.rc_smth = m->rc_smth; ep.inv_range = 1.0 / (m->rc - m->rc_smth);
+    ep.L[0] = g.L[0]; ep.L[1] = g.L[1]; ep.L[2] = g.L[2];
+    k_prod_force_virial<<<m->num_sms * 8, 256, 0, st>>>(N, m->T, tt, ep, (int *)(ws + L.rowstart),
+                                                        (const int2 *)(ws + L.rows_id), (const float4 *)(ws + L.rows_g),
+                                                        (double *)(ws + L.xs), (double *)(ws + L.fsorted), (double *)(ws + L.virial));
+    return cudaGetLastError();
+}
+
 cudaError_t launch_embed_bwd_tc2(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
     return m->m0 == 32 ? launch_bwd_w<32>(m, N, g, ws, L, st) : launch_bwd_w<25>(m, N, g, ws, L, st);
 }

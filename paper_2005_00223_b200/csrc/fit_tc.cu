@@ -757,5 +757,12 @@ static cudaError_t launch_fit_tc_nd(const dp_model *m, long N, const Grid3 &g, c
 }
 
 cudaError_t launch_fit_tc(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    return m->m2 == 128 ? launch_fit_tc_nd<2048>(m, N, g, ws, L, st) : launch_fit_tc_nd<1600>(m, N, g, ws, L, st);
+    switch (m->m2) {
+        case 128: return launch_fit_tc_nd<2048>(m, N, g, ws, L, st);
+        case 256: return launch_fit_tc_nd<4096>(m, N, g, ws, L, st);       // wide nets (wide.cu)
+        case 512: return launch_fit_tc_nd<8192>(m, N, g, ws, L, st);
+        case 1024: return launch_fit_tc_nd<16384>(m, N, g, ws, L, st);
+        case 2048: return launch_fit_tc_nd<32768>(m, N, g, ws, L, st);
+        default: return launch_fit_tc_nd<1600>(m, N, g, ws, L, st);
+    }
 }

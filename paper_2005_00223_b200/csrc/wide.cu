@@ -1,0 +1,640 @@
+// S4 + S5 + S7 for WIDE embedding nets (W, 2 W, 4 W), W = 64 ... 512: the network-size study of PAPER.md:273-279 (Fig. 7,
+// last layer 128 x 256 ... 1024 x 2048), MIX-16.
+//
+// At these widths the layer products are GEMM-bound (tanh per flop falls as 1 / W), the weights no longer fit beside two
+// tiles in one SM, and keeping a tile's activations on chip is impossible (128 rows x 7 W fp16 = 448 KB at W = 256).  So the
+// path is the paper's own: one GEMM per layer with the bias / tanh / skip / tanh' work fused into its
+// epilogue, activations kept in HBM between the layers (fp16) and reused by the backward pass.  What is B200-specific:
+//   * activations live in HBM as ready-made tcgen05 operand images: per 128-row tile and per 8 columns one 2 KB block
+//     [128 rows][8 fp16], so a K = 64 slice of the A operand is ONE contiguous 16 KB cp.async.bulk, and an epilogue thread
+//     (= row) writes 16 bytes per 8 columns, a warp 512 contiguous bytes;
+//   * k_wide_gemm: persistent, warp-specialised: warp 0 streams A and B stages (mbarrier transactions), warp 1 issues
+//     tcgen05.mma 128 x BN x 16 (BN <= 256) into one of two TMEM accumulators, eight epilogue warps drain the other one;
+//   * the backward overwrites in place: dz3 over t3, dz2 over t2, (gG_lo + gG_hi) and then dy2 over y2.
+// Forward:  k_wide_l1 (t1)  ->  gemm<0> (t2, y2 = (t1,t1) + t2)  ->  gemm<1> (t3)  ->  k_wide_contract (A_i = R^T G / Nm)
+// Backward: k_wide_gscale  ->  k_wide_bwd_elem (gG = R^ gA, dz3, dR^ = G gA^T)  ->  gemm<2> (dy2, dz2)  ->  gemm<3> (dy1,
+//           dz1, ds^, gradient of the environment row)  ->  k_prod_force_virial (embed_tc2_bwd.cu).
+#include <cstdio>
+#include <vector>
+#include <cuda_fp16.h>
+#include "dp_internal.h"
+#include "tc_common.cuh"
+
+namespace {
+
+constexpr int WR = 128;                        // rows per tile
+constexpr int WKC = 64;                        // K per pipeline stage: 8 chunks of 8 columns
+constexpr int WNST = 4;                        // pipeline stages
+constexpr int W_A_STAGE = WR * WKC * 2;        // 16 KB
+constexpr int W_B_STAGE = 256 * WKC * 2;       // 32 KB (BN <= 256)
+constexpr int W_OFF_A = 0;
+constexpr int W_OFF_B = WNST * W_A_STAGE;
+constexpr int W_OFF_BAR = W_OFF_B + WNST * W_B_STAGE;
+constexpr int W_OFF_RED = W_OFF_BAR + 256;     // float [2][2][128]: ds^ partial sums of the two column halves (double buffered)
+constexpr int W_TOTAL = W_OFF_RED + 2 * 2 * 128 * 4;
+constexpr int W_THREADS = 64 + 256;
+static_assert(W_TOTAL + 1024 <= 227 * 1024, "shared memory budget");
+
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(tc::smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(tc::smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t sdst, const void *gsrc, uint32_t bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(sdst), "l"(gsrc), "r"(bytes), "r"(tc::smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void unpack8(const uint4 &u, float (&x)[8]) {
+    const __half2 *h = reinterpret_cast<const __half2 *>(&u);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) { const float2 f = __half22float2(h[q]); x[2 * q] = f.x; x[2 * q + 1] = f.y; }
+}
+__device__ __forceinline__ uint4 pack8(const float (&x)[8]) {
+    return make_uint4(tc::pack_h2(x[0], x[1]), tc::pack_h2(x[2], x[3]), tc::pack_h2(x[4], x[5]), tc::pack_h2(x[6], x[7]));
+}
+
+// Tile table: entry k = a T + b = {first tile, first row, end row} of the (centre type a, neighbour type b) row block;
+// entry T T = {number of tiles}.  Rows of a block are contiguous (sorted atoms of one type are contiguous).
+__global__ void k_wide_tiles(long N, int T, int ncell, const int *__restrict__ bin_start, const int *__restrict__ rowstart,
+                             int4 *__restrict__ tab) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    int base = 0;
+    for (int a = 0; a < T; ++a) {
+        const int ts0 = bin_start[a * ncell], ts1 = bin_start[(a + 1) * ncell];
+        for (int b = 0; b < T; ++b) {
+            const int rs = rowstart[(long)b * (N + 1) + ts0], re = rowstart[(long)b * (N + 1) + ts1];
+            tab[a * T + b] = make_int4(base, rs, re, 0);
+            base += (re - rs + WR - 1) / WR;
+        }
+    }
+    tab[T * T] = make_int4(base, 0, 0, 0);
+}
+// the block of a tile; k = the block of an earlier tile of the same walk (tiles are visited in increasing order)
+__device__ __forceinline__ int wide_block(const int4 *tab, int nblk, int tile, int k) {
+    while (k + 1 < nblk && tile >= tab[k + 1].x) ++k;
+    return k;
+}
+
+// Layer 1 (K = 1, ALUs): t1 = tanh(s^ w1 + b1) -> T1 image.  Rows past the end of a block are zero.
+__global__ void __launch_bounds__(WR)
+k_wide_l1(long N, int T, int W, const __grid_constant__ TypeTab tt, const int4 *__restrict__ tab, const float *__restrict__ vec,
+          const float4 *__restrict__ rows_rh, uint8_t *__restrict__ T1) {
+    const int nblk = T * T, ntiles = tab[nblk].x, r = threadIdx.x;
+    int k = 0;
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        k = wide_block(tab, nblk, tile, k);
+        const int4 e = tab[k];
+        const long rbase = N * (long)tt.off[k % T];
+        const int row = e.y + (tile - e.x) * WR + r;
+        const bool ok = row < e.z;
+        const float s = ok ? __ldg(&rows_rh[rbase + row]).x : 0.f;
+        const float *w1 = vec + (size_t)k * 8 * W, *b1 = w1 + W;
+        uint4 *dst = reinterpret_cast<uint4 *>(T1 + (size_t)tile * (W / 8) * 2048) + r;
+        for (int c = 0; c < W / 8; ++c) {
+            float y[8];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) y[q] = ok ? tc::tanh_approx(fmaf(s, __ldg(w1 + 8 * c + q), __ldg(b1 + 8 * c + q))) : 0.f;
+            dst[c * WR] = pack8(y);
+        }
+    }
+}
+
+struct WideArgs {
+    long N;
+    int T, W, Nm;
+    int K, NTOT, BN;                      // product shape: [rows x K] . [K x NTOT], N tile BN
+    int G;                                // CTAs that share a row tile, each taking every G-th N tile (the A tile then comes
+                                          // from HBM once and from L2 for the others: the working set is grid / G tiles)
+    const int4 *tab;
+    const uint8_t *Aimg;                  // A operand images: K / 8 chunks per tile
+    const __half *Bimg;                   // B image of this product inside the first net's block, [NTOT / BN][K / 8][BN][8]
+    long b_net_stride;                    // elements per net
+    const float *vec;                     // [T T][8 W]: w1, b1, b2, b3
+    uint8_t *T1, *Y2, *T2, *T3;           // activation images (W, 2 W, 2 W, 4 W columns)
+    const int2 *rows_id;
+    float4 *rows_g;
+    const float *gscale;
+    const double *stdv;
+    TypeTab tt;
+};
+
+// MODE 0: layer 2 forward   A = t1 (K = W),    N = 2 W:  t2 = tanh(acc + b2) -> T2;  y2 = (t1,t1) + t2 -> Y2
+// MODE 1: layer 3 forward   A = y2 (K = 2 W),  N = 4 W:  t3 = tanh(acc + b3) -> T3   (G = (y2,y2) + t3 is formed by its readers)
+// MODE 2: layer 3 backward  A = dz3 (K = 4 W), N = 2 W:  dy2 = acc + (gG[f] + gG[f + 2 W], in Y2) -> Y2;  dz2 = dy2 (1 - t2^2) -> T2
+// MODE 3: layer 2 backward  A = dz2 (K = 2 W), N = W:    dy1 = acc + dy2[e] + dy2[e + W];  dz1 = dy1 (1 - t1^2);  ds^ = dz1 . w1;
+//                           rows_g = dE/dR~ of the row (dR^ from k_wide_bwd_elem + ds^ on component 0, unscaled, / std)
+template <int MODE>
+__global__ void __launch_bounds__(W_THREADS, 1) k_wide_gemm(const __grid_constant__ WideArgs p) {
+    extern __shared__ __align__(1024) uint8_t smem[];
+    __shared__ uint32_t tmem_base_s;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + W_OFF_BAR);
+    uint64_t *full = bars, *empty = bars + WNST, *acc_full = bars + 2 * WNST, *acc_empty = acc_full + 2;
+    if (tid == 0) {
+        for (int k = 0; k < WNST; ++k) { tc::mbar_init(&full[k], 1); tc::mbar_init(&empty[k], 1); }
+        for (int k = 0; k < 2; ++k) { tc::mbar_init(&acc_full[k], 1); tc::mbar_init(&acc_empty[k], 8); }
+        asm volatile("fence.mbarrier_init.release.cluster;");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tc::smem_u32(&tmem_base_s)), "n"(512));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    tc::fence_before();
+    __syncthreads();
+    tc::fence_after();
+    const uint32_t tmem = __shfl_sync(0xffffffffu, tmem_base_s, 0);
+    const uint32_t sbase = tc::smem_u32(smem);
+    const int nblk = p.T * p.T, ntiles = p.tab[nblk].x;
+    const int W = p.W, BN = p.BN, NT = p.NTOT / BN, NKC = p.K / WKC;
+    const uint32_t b_stage_bytes = (uint32_t)BN * WKC * 2;
+    const int G = p.G, tile0 = blockIdx.x / G, tstep = gridDim.x / G, nt0 = blockIdx.x % G;
+
+    if (warp == 0) {
+        // ---------------------------------------------------------------- loader: one A and one B bulk copy per stage
+        if (lane == 0) {
+            uint32_t step = 0;
+            int k = 0;
+            for (int tile = tile0; tile < ntiles; tile += tstep) {
+                k = wide_block(p.tab, nblk, tile, k);
+                const __half *Bw = p.Bimg + (size_t)k * p.b_net_stride;
+                const uint8_t *At = p.Aimg + (size_t)tile * (p.K / 8) * 2048;
+                for (int nt = nt0; nt < NT; nt += G)
+                    for (int kc = 0; kc < NKC; ++kc, ++step) {
+                        const int st = step % WNST;
+                        tc::mbar_wait(&empty[st], ((step / WNST) & 1) ^ 1);
+                        mbar_expect_tx(&full[st], W_A_STAGE + b_stage_bytes);
+                        bulk_g2s(sbase + W_OFF_A + st * W_A_STAGE, At + (size_t)kc * W_A_STAGE, W_A_STAGE, &full[st]);
+                        bulk_g2s(sbase + W_OFF_B + st * W_B_STAGE, Bw + ((size_t)nt * NKC + kc) * (WKC * BN), b_stage_bytes, &full[st]);
+                    }
+            }
+        }
+    } else if (warp == 1) {
+        // ---------------------------------------------------------------- MMA issuer
+        const uint32_t idesc = tc::idesc(128, BN, false, false);
+        uint32_t step = 0, accn = 0;
+        for (int tile = tile0; tile < ntiles; tile += tstep)
+            for (int nt = nt0; nt < NT; nt += G, ++accn) {
+                const int buf = accn & 1;
+                tc::mbar_wait(&acc_empty[buf], ((accn >> 1) & 1) ^ 1);
+                tc::fence_after();
+                for (int kc = 0; kc < NKC; ++kc, ++step) {
+                    const int st = step % WNST;
+                    tc::mbar_wait(&full[st], (step / WNST) & 1);
+                    tc::fence_after();
+                    const uint64_t da = tc::desc(sbase + W_OFF_A + st * W_A_STAGE, 2048, 128);
+                    const uint64_t db = tc::desc(sbase + W_OFF_B + st * W_B_STAGE, BN * 16, 128);
+                    if (tc::elect_one()) {
+#pragma unroll
+                        for (int ks = 0; ks < WKC / 16; ++ks)
+                            tc::mma_ss(tmem + buf * 256, tc::desc_at(da, ks * 2 * 2048), tc::desc_at(db, ks * 2 * (BN * 16)), idesc, (kc | ks) != 0);
+                        tc::commit(&empty[st]);
+                    }
+                    __syncwarp();
+                }
+                if (tc::elect_one()) tc::commit(&acc_full[buf]);
+                __syncwarp();
+            }
+    } else {
+        // ---------------------------------------------------------------- epilogue: thread = (row, every other 16 columns)
+        const int q4 = warp & 3, r = q4 * 32 + lane, hc = ((warp - 2) >> 2) & 1;
+        const uint32_t tm_lane = tmem + ((uint32_t)(q4 * 32) << 16);
+        float *red = reinterpret_cast<float *>(smem + W_OFF_RED);
+        uint32_t accn = 0, it = 0;
+        int k = 0;
+        for (int tile = tile0; tile < ntiles; tile += tstep, ++it) {
+            k = wide_block(p.tab, nblk, tile, k);
+            const float *vec = p.vec + (size_t)k * 8 * W;
+            // this row's 16-byte slot of chunk 0 of each image of the tile
+            uint8_t *t1r = p.T1 + (size_t)tile * (W / 8) * 2048 + r * 16;
+            uint8_t *y2r = p.Y2 + (size_t)tile * (2 * W / 8) * 2048 + r * 16;
+            uint8_t *t2r = p.T2 + (size_t)tile * (2 * W / 8) * 2048 + r * 16;
+            uint8_t *t3r = p.T3 + (size_t)tile * (4 * W / 8) * 2048 + r * 16;
+            (void)t1r; (void)y2r; (void)t2r; (void)t3r;
+            float ds = 0.f;
+            // global operands of a group of 16 columns (two chunks), loaded one group ahead of their use
+            struct Pre { uint4 a[2], b[2], c[2]; };
+            const int ngrp = BN / 32;                       // groups of this thread per N tile (2, 4 or 8)
+            auto fetch = [&](int nt, int g, Pre &P) {
+                const int ch0 = (nt * BN + 16 * hc + 32 * g) / 8;
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const size_t ch = ch0 + h;
+                    if (MODE == 0) P.a[h] = *reinterpret_cast<const uint4 *>(t1r + (ch % (W / 8)) * 2048);
+                    if (MODE == 2) {
+                        P.a[h] = *reinterpret_cast<const uint4 *>(y2r + ch * 2048);
+                        P.b[h] = *reinterpret_cast<const uint4 *>(t2r + ch * 2048);
+                    }
+                    if (MODE == 3) {
+                        P.a[h] = *reinterpret_cast<const uint4 *>(y2r + ch * 2048);
+                        P.b[h] = *reinterpret_cast<const uint4 *>(y2r + (ch + W / 8) * 2048);
+                        P.c[h] = *reinterpret_cast<const uint4 *>(t1r + ch * 2048);
+                    }
+                }
+            };
+            auto process = [&](int nt, int g, int buf, const Pre &P) {
+                const int c0 = 16 * hc + 32 * g, n = nt * BN + c0;      // n: first of these 16 output columns
+                uint32_t v[16];
+                tc::ld16(tm_lane + buf * 256 + c0, v);
+                tc::wait_ld();
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const size_t ch = n / 8 + h;
+                    float x[8];
+                    if (MODE == 0) {
+                        const float4 b0 = __ldg(reinterpret_cast<const float4 *>(vec + 2 * W + n + 8 * h)), b1 = __ldg(reinterpret_cast<const float4 *>(vec + 2 * W + n + 8 * h + 4));
+                        const float bb[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+                        float t1[8];
+                        unpack8(P.a[h], t1);
+#pragma unroll
+                        for (int q = 0; q < 8; ++q) x[q] = tc::tanh_approx(__uint_as_float(v[8 * h + q]) + bb[q]);
+                        *reinterpret_cast<uint4 *>(t2r + ch * 2048) = pack8(x);
+#pragma unroll
+                        for (int q = 0; q < 8; ++q) x[q] += t1[q];
+                        *reinterpret_cast<uint4 *>(y2r + ch * 2048) = pack8(x);
+                    } else if (MODE == 1) {
+                        const float4 b0 = __ldg(reinterpret_cast<const float4 *>(vec + 4 * W + n + 8 * h)), b1 = __ldg(reinterpret_cast<const float4 *>(vec + 4 * W + n + 8 * h + 4));
+                        const float bb[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+#pragma unroll
+                        for (int q = 0; q < 8; ++q) x[q] = tc::tanh_approx(__uint_as_float(v[8 * h + q]) + bb[q]);
+                        *reinterpret_cast<uint4 *>(t3r + ch * 2048) = pack8(x);
+                    } else if (MODE == 2) {
+                        float gs[8], t2[8];
+                        unpack8(P.a[h], gs);
+                        unpack8(P.b[h], t2);
+#pragma unroll
+                        for (int q = 0; q < 8; ++q) x[q] = __uint_as_float(v[8 * h + q]) + gs[q];
+                        *reinterpret_cast<uint4 *>(y2r + ch * 2048) = pack8(x);
+#pragma unroll
+                        for (int q = 0; q < 8; ++q) x[q] *= fmaf(-t2[q], t2[q], 1.f);
+                        *reinterpret_cast<uint4 *>(t2r + ch * 2048) = pack8(x);
+                    } else {
+                        float da[8], db[8], t1[8];
+                        unpack8(P.a[h], da);
+                        unpack8(P.b[h], db);
+                        unpack8(P.c[h], t1);
+                        const float4 w0 = __ldg(reinterpret_cast<const float4 *>(vec + n + 8 * h)), w1 = __ldg(reinterpret_cast<const float4 *>(vec + n + 8 * h + 4));
+                        const float ww[8] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
+#pragma unroll
+                        for (int q = 0; q < 8; ++q) {
+                            const float dy1 = __uint_as_float(v[8 * h + q]) + da[q] + db[q];
+                            ds = fmaf(dy1 * fmaf(-t1[q], t1[q], 1.f), ww[q], ds);
+                        }
+                    }
+                }
+            };
+            Pre P0, P1;
+            fetch(nt0, 0, P0);
+            for (int nt = nt0; nt < NT; nt += G, ++accn) {
+                const int buf = accn & 1;
+                tc::mbar_wait(&acc_full[buf], (accn >> 1) & 1);
+                tc::fence_after();
+                for (int g = 0; g < ngrp; g += 2) {
+                    fetch(nt, g + 1, P1);
+                    process(nt, g, buf, P0);
+                    if (g + 2 < ngrp) fetch(nt, g + 2, P0);
+                    else if (nt + G < NT) fetch(nt + G, 0, P0);
+                    process(nt, g + 1, buf, P1);
+                }
+                tc::fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&acc_empty[buf]);
+            }
+            if (MODE == 3) {
+                float *rd = red + (it & 1) * 256;
+                rd[hc * 128 + r] = ds;
+                tc::bar_sync(1, 256);
+                const int4 e = p.tab[k];
+                const int row = e.y + (tile - e.x) * WR + r;
+                if (hc == 0 && row < e.z) {
+                    const long rbase = p.N * (long)p.tt.off[k % p.T];
+                    const int2 id = __ldg(&p.rows_id[rbase + row]);
+                    if (id.y >= 0) {
+                        const int a = k / p.T;
+                        const float4 g = p.rows_g[rbase + row];          // gscale * dR^ (k_wide_bwd_elem)
+                        const float osc = 1.0f / ((float)p.Nm * __ldg(&p.gscale[id.x]));
+                        const float dsum = rd[r] + rd[128 + r];
+                        p.rows_g[rbase + row] = make_float4((g.x + dsum) * osc / (float)p.stdv[4 * a], g.y * osc / (float)p.stdv[4 * a + 1],
+                                                            g.z * osc / (float)p.stdv[4 * a + 2], g.w * osc / (float)p.stdv[4 * a + 3]);
+                    }
+                }
+            }
+        }
+    }
+    tc::fence_before();
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(512));
+}
+
+// S5: A_i[c][m] = (1 / Nm) sum_rows w R^[row][c] G[row][m],  G = (y2, y2) + t3.
+// One CTA per atom; warp = one group of 8 columns at a time, lane = row; the 32 partial sums (4 components x 8 columns)
+// of a warp are reduced by a transposing butterfly (31 shuffles) and added to the CTA's copy of A_i in shared memory:
+// no atomics, a fixed summation order, A_i written once.
+constexpr int WC_BATCH = 512;                   // rows staged per pass
+__global__ void __launch_bounds__(256)
+k_wide_contract(long N, int T, int ncell, int W, int Nm, const __grid_constant__ TypeTab tt, const int4 *__restrict__ tab,
+                const int *__restrict__ bin_start, const int *__restrict__ rowstart, const float4 *__restrict__ rows_rh,
+                const int2 *__restrict__ rows_id, const uint8_t *__restrict__ Y2, const uint8_t *__restrict__ T3,
+                float *__restrict__ Aout) {
+    extern __shared__ __align__(16) uint8_t csm[];
+    float *sA = reinterpret_cast<float *>(csm);                       // [4][4 W]
+    float4 *srw = reinterpret_cast<float4 *>(csm + 16 * W * 4);       // [WC_BATCH] weighted rows
+    const long i = blockIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int cg = lane >> 2, rs = lane & 3;              // lane = (one of 8 column groups, one of 4 row phases)
+    int a = 0;
+    for (int t = 1; t < T; ++t) a += i >= bin_start[t * ncell];
+    for (int k = tid; k < 16 * W; k += 256) sA[k] = 0.f;
+    const int nch = 4 * W / 8, ych = 2 * W / 8;
+    for (int b = 0; b < T; ++b) {
+        const int4 e = tab[a * T + b];
+        const long rbase = N * (long)tt.off[b];
+        const int r0 = rowstart[(long)b * (N + 1) + i], r1 = rowstart[(long)b * (N + 1) + i + 1];
+        for (int rb = r0; rb < r1; rb += WC_BATCH) {
+            const int nb = min(WC_BATCH, r1 - rb);
+            __syncthreads();
+            for (int j = tid; j < nb; j += 256) {
+                float4 rh = __ldg(&rows_rh[rbase + rb + j]);
+                const int2 id = __ldg(&rows_id[rbase + rb + j]);
+                if (id.y < 0) { const float w = (float)(-id.y); rh.x *= w; rh.y *= w; rh.z *= w; rh.w *= w; }
+                srw[j] = rh;
+            }
+            __syncthreads();
+            for (int ch = 8 * wid + cg; ch < nch; ch += 64) {
+                const int cy = ch % ych;
+                float v[32];
+#pragma unroll
+                for (int q = 0; q < 32; ++q) v[q] = 0.f;
+                for (int j = rs; j < nb; j += 16) {       // four rows per trip: eight independent loads in flight
+                    uint4 u[4], y[4];
+                    float4 w[4];
+#pragma unroll
+                    for (int x = 0; x < 4; ++x) {
+                        const int jj = j + 4 * x;
+                        u[x] = make_uint4(0u, 0u, 0u, 0u); y[x] = u[x]; w[x] = make_float4(0.f, 0.f, 0.f, 0.f);
+                        if (jj < nb) {
+                            const int rel = rb + jj - e.y;
+                            const size_t tl = (size_t)e.x + rel / WR;
+                            const int o = (rel % WR) * 16;
+                            u[x] = __ldg(reinterpret_cast<const uint4 *>(T3 + (tl * nch + ch) * 2048 + o));
+                            y[x] = __ldg(reinterpret_cast<const uint4 *>(Y2 + (tl * ych + cy) * 2048 + o));
+                            w[x] = srw[jj];
+                        }
+                    }
+#pragma unroll
+                    for (int x = 0; x < 4; ++x) {
+                        float g[8], h[8];
+                        unpack8(u[x], g);
+                        unpack8(y[x], h);
+#pragma unroll
+                        for (int q = 0; q < 8; ++q) {
+                            const float G = g[q] + h[q];
+                            v[q] = fmaf(w[x].x, G, v[q]);
+                            v[8 + q] = fmaf(w[x].y, G, v[8 + q]);
+                            v[16 + q] = fmaf(w[x].z, G, v[16 + q]);
+                            v[24 + q] = fmaf(w[x].w, G, v[24 + q]);
+                        }
+                    }
+                }
+                // transposing butterfly over the four row phases: afterwards lane rs holds component c = rs, 8 columns
+#pragma unroll
+                for (int o = 2; o >= 1; o >>= 1) {
+                    const bool up = (lane & o) != 0;
+#pragma unroll
+                    for (int q = 0; q < 8 * o; ++q) {
+                        const float send = up ? v[q] : v[q + 8 * o];
+                        const float keep = up ? v[q + 8 * o] : v[q];
+                        v[q] = keep + __shfl_xor_sync(0xffffffffu, send, o);
+                    }
+                }
+                float *dst = sA + rs * 4 * W + 8 * ch;
+#pragma unroll
+                for (int q = 0; q < 8; ++q) dst[q] += v[q];
+            }
+        }
+    }
+    __syncthreads();
+    const float inv_nm = 1.0f / (float)Nm;
+    for (int k = tid; k < 16 * W; k += 256) Aout[i * 16L * W + k] = sA[k] * inv_nm;
+}
+
+// per-atom power-of-two scale of the gradient images: max |gA_i| in [0.5, 1) (fp16 range; undone in gemm<3>)
+__global__ void __launch_bounds__(256) k_wide_gscale(long N, int n, const float *__restrict__ gA, float *__restrict__ gscale) {
+    const int lane = threadIdx.x & 31;
+    const long i = blockIdx.x * 8L + (threadIdx.x >> 5);
+    if (i >= N) return;
+    const float4 *g = reinterpret_cast<const float4 *>(gA + i * (long)n);
+    float mx = 0.f;
+    for (int k = lane; k < n / 4; k += 32) {
+        const float4 v = __ldg(g + k);
+        mx = fmaxf(fmaxf(mx, fmaxf(fabsf(v.x), fabsf(v.y))), fmaxf(fabsf(v.z), fabsf(v.w)));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    int ex = 0;
+    if (mx > 0.f) frexpf(mx, &ex);
+    if (lane == 0) gscale[i] = ldexpf(1.f, -ex);
+}
+
+// Head of the backward pass, thread = row, per pair of column groups (f, f + 2 W):
+//   gG[m] = sc sum_c R^[c] gA[c][m]          (gradient of E with respect to G, scaled by the atom's sc, without 1 / Nm)
+//   dz3   = gG (1 - t3^2)                     -> over t3 (A operand of gemm<2>)
+//   gG[f] + gG[f + 2 W]                       -> over y2 (the skip connection's share of dy2, added in the epilogue of gemm<2>)
+//   dR^[c] = sc sum_m G[m] gA[c][m]           -> rows_g (finished by gemm<3>)
+// Padded-row representatives carry no gradient (R~ = 0 there is a constant): skipped.
+__global__ void __launch_bounds__(2 * WR, 2)
+k_wide_bwd_elem(long N, int T, int W, const __grid_constant__ TypeTab tt, const int4 *__restrict__ tab,
+                const float4 *__restrict__ rows_rh, const int2 *__restrict__ rows_id, const float *__restrict__ gA,
+                const float *__restrict__ gscale, uint8_t *__restrict__ Y2, uint8_t *__restrict__ T3, float4 *__restrict__ rows_g) {
+    __shared__ float4 sdr[WR];
+    const int nblk = T * T, ntiles = tab[nblk].x, r = threadIdx.x & (WR - 1), hf = threadIdx.x >> 7;
+    const int ych = 2 * W / 8, M2 = 4 * W;
+    int k = 0;
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        k = wide_block(tab, nblk, tile, k);
+        const int4 e = tab[k];
+        const long rbase = N * (long)tt.off[k % T];
+        const int row = e.y + (tile - e.x) * WR + r;
+        int2 id = make_int2(-1, -1);
+        if (row < e.z) id = __ldg(&rows_id[rbase + row]);
+        const bool real = id.y >= 0;
+        float dR[4] = {0.f, 0.f, 0.f, 0.f};
+        float sc = 0.f;
+        if (real) {
+            const float4 rh = __ldg(&rows_rh[rbase + row]);
+            sc = __ldg(&gscale[id.x]);
+            const float R[4] = {rh.x * sc, rh.y * sc, rh.z * sc, rh.w * sc};
+            const float *g = gA + (long)id.x * 4 * M2;
+            uint8_t *y2r = Y2 + (size_t)tile * ych * 2048 + r * 16;
+            uint8_t *t3r = T3 + (size_t)tile * (2 * ych) * 2048 + r * 16;
+            const int f0 = hf * (ych / 2), f1 = f0 + ych / 2;       // this thread's half of the column groups
+            uint4 ny = *reinterpret_cast<const uint4 *>(y2r + (size_t)f0 * 2048);
+            uint4 na = *reinterpret_cast<const uint4 *>(t3r + (size_t)f0 * 2048);
+            uint4 nb = *reinterpret_cast<const uint4 *>(t3r + (size_t)(f0 + ych) * 2048);
+            for (int f = f0; f < f1; ++f) {
+                float y2[8], ta[8], tb[8], oa[8], ob[8], os[8];
+                unpack8(ny, y2);
+                unpack8(na, ta);
+                unpack8(nb, tb);
+                if (f + 1 < f1) {         // the three activation chunks of the next step, in flight under this step's arithmetic
+                    ny = *reinterpret_cast<const uint4 *>(y2r + (size_t)(f + 1) * 2048);
+                    na = *reinterpret_cast<const uint4 *>(t3r + (size_t)(f + 1) * 2048);
+                    nb = *reinterpret_cast<const uint4 *>(t3r + (size_t)(f + 1 + ych) * 2048);
+                }
+#pragma unroll
+                for (int q = 0; q < 8; ++q) { oa[q] = 0.f; ob[q] = 0.f; }
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const float4 a0 = __ldg(reinterpret_cast<const float4 *>(g + c * M2 + 8 * f)), a1 = __ldg(reinterpret_cast<const float4 *>(g + c * M2 + 8 * f + 4));
+                    const float4 b0 = __ldg(reinterpret_cast<const float4 *>(g + c * M2 + 2 * W + 8 * f)), b1 = __ldg(reinterpret_cast<const float4 *>(g + c * M2 + 2 * W + 8 * f + 4));
+                    const float ga[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
+                    const float gb[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+                    float acc = 0.f;
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) {
+                        oa[q] = fmaf(R[c], ga[q], oa[q]);
+                        ob[q] = fmaf(R[c], gb[q], ob[q]);
+                        acc = fmaf(ta[q] + y2[q], ga[q], acc);
+                        acc = fmaf(tb[q] + y2[q], gb[q], acc);
+                    }
+                    dR[c] += acc;
+                }
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    os[q] = oa[q] + ob[q];
+                    oa[q] *= fmaf(-ta[q], ta[q], 1.f);
+                    ob[q] *= fmaf(-tb[q], tb[q], 1.f);
+                }
+                *reinterpret_cast<uint4 *>(y2r + (size_t)f * 2048) = pack8(os);
+                *reinterpret_cast<uint4 *>(t3r + (size_t)f * 2048) = pack8(oa);
+                *reinterpret_cast<uint4 *>(t3r + (size_t)(f + ych) * 2048) = pack8(ob);
+            }
+        }
+        if (hf == 1) sdr[r] = make_float4(dR[0], dR[1], dR[2], dR[3]);
+        __syncthreads();
+        if (hf == 0 && real) {
+            const float4 o = sdr[r];
+            rows_g[rbase + row] = make_float4((dR[0] + o.x) * sc, (dR[1] + o.y) * sc, (dR[2] + o.z) * sc, (dR[3] + o.w) * sc);
+        }
+        __syncthreads();
+    }
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------------------------------
+// Host side.  Weight images of one net, in this order: W2 (K = W, N = 2 W), W3 (K = 2 W, N = 4 W), W3^T (K = 4 W, N = 2 W),
+// W2^T (K = 2 W, N = W); each [N / BN][K / 8][BN][8] fp16 with BN = min(N, 256): a (N tile, K = 64) stage is contiguous.
+static int wide_bn(int n) { return n < 256 ? n : 256; }
+static size_t wide_img_off(int W, int g) {
+    const size_t w2 = (size_t)W * W;
+    const size_t off[5] = {0, 2 * w2, 10 * w2, 18 * w2, 20 * w2};
+    return off[g];
+}
+size_t wide_net_img_elems(int W) { return wide_img_off(W, 4); }
+
+static void wide_image(const double *Wt, int ldw, bool transpose, int K, int Nn, __half *out) {
+    const int BN = wide_bn(Nn), nk8 = K / 8;
+    for (int nt = 0; nt < Nn / BN; ++nt)
+        for (int k8 = 0; k8 < nk8; ++k8)
+            for (int n = 0; n < BN; ++n)
+                for (int kk = 0; kk < 8; ++kk) {
+                    const int k = k8 * 8 + kk, nn = nt * BN + n;
+                    const double v = transpose ? Wt[(size_t)nn * ldw + k] : Wt[(size_t)k * ldw + nn];
+                    out[(((size_t)nt * nk8 + k8) * BN + n) * 8 + kk] = __float2half_rn((float)v);
+                }
+}
+
+// net: w1[W], b1[W], W2[W][2 W], b2[2 W], W3[2 W][4 W], b3[4 W] (dp.h weight order); vec: w1, b1, b2, b3
+void wide_build_net(int W, const double *net, float *vec, __half *img) {
+    const double *w1 = net, *b1 = w1 + W, *W2 = b1 + W, *b2 = W2 + (size_t)W * 2 * W, *W3 = b2 + 2 * W, *b3 = W3 + (size_t)2 * W * 4 * W;
+    for (int e = 0; e < W; ++e) { vec[e] = (float)w1[e]; vec[W + e] = (float)b1[e]; }
+    for (int f = 0; f < 2 * W; ++f) vec[2 * W + f] = (float)b2[f];
+    for (int m = 0; m < 4 * W; ++m) vec[4 * W + m] = (float)b3[m];
+    wide_image(W2, 2 * W, false, W, 2 * W, img + wide_img_off(W, 0));
+    wide_image(W3, 4 * W, false, 2 * W, 4 * W, img + wide_img_off(W, 1));
+    wide_image(W3, 4 * W, true, 4 * W, 2 * W, img + wide_img_off(W, 2));      // B[k = m][n = f] = W3[f][m]
+    wide_image(W2, 2 * W, true, 2 * W, W, img + wide_img_off(W, 3));          // B[k = f][n = e] = W2[e][f]
+}
+
+// capacity of the tile table: every (type, type) block may end in a partial tile
+long wide_tiles_cap(const dp_model *m, long N) {
+    long t = (long)m->T * m->T + 1;
+    for (int b = 0; b < m->T; ++b) t += (N * (long)m->sel[b] + WR - 1) / WR;
+    return t;
+}
+
+static WideArgs wide_args(const dp_model *m, long N, char *ws, const WsLayout &L) {
+    WideArgs p{};
+    p.N = N; p.T = m->T; p.W = m->m0; p.Nm = m->Nm;
+    p.tab = (const int4 *)(ws + L.wide_tab);
+    p.b_net_stride = (long)wide_net_img_elems(m->m0);
+    p.vec = (const float *)m->wide_vec_dev;
+    p.T1 = (uint8_t *)(ws + L.wide_t1); p.Y2 = (uint8_t *)(ws + L.wide_y2);
+    p.T2 = (uint8_t *)(ws + L.wide_t2); p.T3 = (uint8_t *)(ws + L.wide_t3);
+    p.rows_id = (const int2 *)(ws + L.rows_id);
+    p.rows_g = (float4 *)(ws + L.rows_g);
+    p.gscale = (const float *)(ws + L.gscale);
+    p.stdv = m->std_dev;
+    p.tt = make_typetab(m);
+    return p;
+}
+
+template <int MODE>
+static cudaError_t wide_gemm(const dp_model *m, WideArgs p, int K, int Nn, const uint8_t *Aimg, int img, cudaStream_t st) {
+    DP_SMEM_OPTIN(k_wide_gemm<MODE>, W_TOTAL);
+    p.K = K; p.NTOT = Nn; p.BN = wide_bn(Nn);
+    p.Aimg = Aimg;
+    p.Bimg = (const __half *)m->wide_img_dev + wide_img_off(m->m0, img);
+    // MODE 3 sums ds^ over all the N tiles of a row in one thread: no sharing there
+    const int nt = Nn / p.BN;
+    // (worth it when the A tiles of all CTAs, grid x 128 x K fp16, overflow the L2: K = 2048, the layer-3 backward at W = 512)
+    p.G = (MODE != 3 && K >= 2048 && nt >= 4) ? 4 : 1;
+    k_wide_gemm<MODE><<<m->num_sms - m->num_sms % p.G, W_THREADS, W_TOTAL, st>>>(p);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_env_rows(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+
+cudaError_t launch_embed_fwd_wide(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    const int W = m->m0;
+    const TypeTab tt = make_typetab(m);
+    cudaError_t e = launch_env_rows(m, N, g, ws, L, st);
+    auto ok = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
+    int4 *tab = (int4 *)(ws + L.wide_tab);
+    k_wide_tiles<<<1, 32, 0, st>>>(N, m->T, g.ncell, (const int *)(ws + L.bin_start), (const int *)(ws + L.rowstart), tab);
+    k_wide_l1<<<m->num_sms * 8, WR, 0, st>>>(N, m->T, W, tt, tab, (const float *)m->wide_vec_dev, (const float4 *)(ws + L.rows_rh),
+                                           (uint8_t *)(ws + L.wide_t1));
+    ok(cudaGetLastError());
+    const WideArgs p = wide_args(m, N, ws, L);
+    ok(wide_gemm<0>(m, p, W, 2 * W, p.T1, 0, st));
+    ok(wide_gemm<1>(m, p, 2 * W, 4 * W, p.Y2, 1, st));
+    const int csm = 16 * W * 4 + WC_BATCH * 16;
+    DP_SMEM_OPTIN(k_wide_contract, 16 * 512 * 4 + WC_BATCH * 16);
+    k_wide_contract<<<(unsigned)N, 256, csm, st>>>(N, m->T, g.ncell, W, m->Nm, tt, tab, (const int *)(ws + L.bin_start),
+                                                   (const int *)(ws + L.rowstart), (const float4 *)(ws + L.rows_rh),
+                                                   (const int2 *)(ws + L.rows_id), p.Y2, p.T3, (float *)(ws + L.A));
+    ok(cudaGetLastError());
+    return e;
+}
+
+cudaError_t launch_embed_bwd_wide(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    const int W = m->m0;
+    const TypeTab tt = make_typetab(m);
+    cudaError_t e = cudaSuccess;
+    auto ok = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
+    const WideArgs p = wide_args(m, N, ws, L);
+    // the last fitting GEMM left gA itself in the gD buffer (fit_tc.cu MODE 6)
+    const float *gA = (const float *)(ws + L.gD);
+    k_wide_gscale<<<(unsigned)((N + 7) / 8), 256, 0, st>>>(N, 16 * W, gA, (float *)(ws + L.gscale));
+    k_wide_bwd_elem<<<m->num_sms * 4, 2 * WR, 0, st>>>(N, m->T, W, tt, p.tab, (const float4 *)(ws + L.rows_rh), p.rows_id, gA, p.gscale,
+                                                 p.Y2, p.T3, p.rows_g);
+    ok(cudaGetLastError());
+    if (m->profile) cudaEventRecord(m->ev[6], st);      // ev[6] .. ev[7]: the two backward GEMMs
+    ok(wide_gemm<2>(m, p, 4 * W, 2 * W, p.T3, 2, st));
+    ok(wide_gemm<3>(m, p, 2 * W, W, p.T2, 3, st));
+    if (m->profile) cudaEventRecord(m->ev[7], st);
+    ok(launch_prod_force_virial(m, N, g, ws, L, st));
+    return e;
+}

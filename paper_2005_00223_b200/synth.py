@@ -286,6 +286,23 @@ def paper_config(name: str, precision="fp64") -> System:
     raise ValueError(name)
 
 
+# ----------------------------------------------------------------------------- network-size study (Fig. 7)
+SWEEP_WIDTHS = (64, 128, 256, 512)      # first embedding width W: last layer 2 W x 4 W = 128 x 256 ... 1024 x 2048
+
+
+def wide_copper(ncell: int, W: int, seed: int, sigma: float = 0.05, shuffle: bool = False, sel=(512,), precision="mix16",
+                name=None) -> System:
+    """Copper (the system of Fig. 7) with embedding nets (W, 2 W, 4 W); capacity and statistics as paper_copper."""
+    return copper(ncell, sigma, seed, shuffle=shuffle, sel=sel, precision=precision, name=name or f"wide{W}_cu{4 * ncell ** 3}",
+                  embed_widths=(W, 2 * W, 4 * W), avg=PAPER_CU_AVG, std=PAPER_CU_STD)
+
+
+def wide_water(nmol: int, L: float, W: int, seed: int, precision="mix16", name=None) -> System:
+    """Two-type system with embedding nets (W, 2 W, 4 W): exercises the (centre, neighbour) type blocks of the wide path."""
+    return water(nmol, L, seed, sel=(48, 96), precision=precision, name=name or f"wide{W}_water{3 * nmol}",
+                 embed_widths=(W, 2 * W, 4 * W), avg=PAPER_WATER_AVG, std=PAPER_WATER_STD)
+
+
 # ----------------------------------------------------------------------------- tiny systems for self-tests
 def cluster(n: int, seed: int, ntypes: int = 1, L: float = 40.0, spread: float = 3.0,
             rc: float = 6.0, rc_smth: float = 1.0, sel=None, dmin: float = 1.2) -> System:
