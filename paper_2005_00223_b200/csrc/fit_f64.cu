@@ -6,6 +6,7 @@
 // centre type and run on the FP64 tensor pipe (DMMA m8n8k4); bias, tanh, skip and tanh' live in the epilogue
 // (PAPER.md:133-134 merged them into cuBLAS GEMM calls; here they never reach memory as separate passes).
 #include "dp_internal.h"
+#include "tanh64.cuh"
 
 namespace {
 
@@ -128,18 +129,18 @@ __global__ void __launch_bounds__(256) k_fit_gemm(FitArgs p) {
             double v0 = acc[mt][nt][0], v1 = acc[mt][nt][1];
             if (MODE == 0) {
                 const double *b = p.bias + a * p.bias_type_stride + col;
-                *reinterpret_cast<double2 *>(p.out0 + o) = make_double2(tanh(v0 + b[0]), tanh(v1 + b[1]));
+                *reinterpret_cast<double2 *>(p.out0 + o) = make_double2(dp_tanh64(v0 + b[0]), dp_tanh64(v1 + b[1]));
             } else if (MODE == 1) {
                 const double *b = p.bias + a * p.bias_type_stride + col;
                 const double2 h = *reinterpret_cast<const double2 *>(p.aux0 + o);
-                const double t0 = tanh(v0 + b[0]), t1 = tanh(v1 + b[1]);
+                const double t0 = dp_tanh64(v0 + b[0]), t1 = dp_tanh64(v1 + b[1]);
                 *reinterpret_cast<double2 *>(p.out0 + o) = make_double2(t0, t1);
                 *reinterpret_cast<double2 *>(p.out1 + o) = make_double2(h.x + t0, h.y + t1);
             } else if (MODE == 2) {
                 const double *b = p.bias + a * p.bias_type_stride + col;
                 const double *v4 = p.v4 + a * p.v4_type_stride + col;
                 const double2 h = *reinterpret_cast<const double2 *>(p.aux0 + o);
-                const double t0 = tanh(v0 + b[0]), t1 = tanh(v1 + b[1]);
+                const double t0 = dp_tanh64(v0 + b[0]), t1 = dp_tanh64(v1 + b[1]);
                 *reinterpret_cast<double2 *>(p.out0 + o) = make_double2(v4[0] * (1.0 - t0 * t0), v4[1] * (1.0 - t1 * t1));
                 *reinterpret_cast<double2 *>(p.out1 + o) = make_double2(h.x + t0, h.y + t1);
             } else if (MODE == 3) {
