@@ -338,14 +338,17 @@ k_wide_contract(long N, int T, int ncell, int W, int Nm, const __grid_constant__
                 const int2 *__restrict__ rows_id, const uint8_t *__restrict__ Y2, const uint8_t *__restrict__ T3,
                 float *__restrict__ Aout) {
     extern __shared__ __align__(16) uint8_t csm[];
-    float *sA = reinterpret_cast<float *>(csm);                       // [4][4 W]
-    float4 *srw = reinterpret_cast<float4 *>(csm + 16 * W * 4);       // [WC_BATCH] weighted rows
+    // S3 = R^T t3 [4][4 W] followed by S2 = R^T y2 [4][2 W]: G = (y2, y2) + t3, so A_i[c][m] = S3[c][m] + S2[c][m mod 2 W] and
+    // every activation is read from HBM once
+    float *sA = reinterpret_cast<float *>(csm);
+    float *sA2 = sA + 16 * W;
+    float4 *srw = reinterpret_cast<float4 *>(csm + 24 * W * 4);       // [WC_BATCH] weighted rows
     const long i = blockIdx.x;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int cg = lane >> 2, rs = lane & 3;              // lane = (one of 8 column groups, one of 4 row phases)
     int a = 0;
     for (int t = 1; t < T; ++t) a += i >= bin_start[t * ncell];
-    for (int k = tid; k < 16 * W; k += 256) sA[k] = 0.f;
+    for (int k = tid; k < 24 * W; k += 256) sA[k] = 0.f;
     const int nch = 4 * W / 8, ych = 2 * W / 8;
     for (int b = 0; b < T; ++b) {
         const int4 e = tab[a * T + b];
@@ -361,39 +364,36 @@ k_wide_contract(long N, int T, int ncell, int W, int Nm, const __grid_constant__
                 srw[j] = rh;
             }
             __syncthreads();
-            for (int ch = 8 * wid + cg; ch < nch; ch += 64) {
-                const int cy = ch % ych;
+            for (int vc = 8 * wid + cg; vc < nch + ych; vc += 64) {      // groups of 8 chunks: all of t3 or all of y2 (warp-uniform)
+                const bool isy = vc >= nch;
+                const uint8_t *img = isy ? Y2 : T3;
+                const int cpt = isy ? ych : nch, ch = isy ? vc - nch : vc;
                 float v[32];
 #pragma unroll
                 for (int q = 0; q < 32; ++q) v[q] = 0.f;
-                for (int j = rs; j < nb; j += 16) {       // four rows per trip: eight independent loads in flight
-                    uint4 u[4], y[4];
-                    float4 w[4];
+                for (int j = rs; j < nb; j += 32) {       // eight rows per trip: eight independent loads in flight
+                    uint4 u[8];
+                    float4 w[8];
 #pragma unroll
-                    for (int x = 0; x < 4; ++x) {
+                    for (int x = 0; x < 8; ++x) {
                         const int jj = j + 4 * x;
-                        u[x] = make_uint4(0u, 0u, 0u, 0u); y[x] = u[x]; w[x] = make_float4(0.f, 0.f, 0.f, 0.f);
+                        u[x] = make_uint4(0u, 0u, 0u, 0u); w[x] = make_float4(0.f, 0.f, 0.f, 0.f);
                         if (jj < nb) {
                             const int rel = rb + jj - e.y;
-                            const size_t tl = (size_t)e.x + rel / WR;
-                            const int o = (rel % WR) * 16;
-                            u[x] = __ldg(reinterpret_cast<const uint4 *>(T3 + (tl * nch + ch) * 2048 + o));
-                            y[x] = __ldg(reinterpret_cast<const uint4 *>(Y2 + (tl * ych + cy) * 2048 + o));
+                            u[x] = __ldg(reinterpret_cast<const uint4 *>(img + (((size_t)e.x + rel / WR) * cpt + ch) * 2048 + (rel % WR) * 16));
                             w[x] = srw[jj];
                         }
                     }
 #pragma unroll
-                    for (int x = 0; x < 4; ++x) {
-                        float g[8], h[8];
+                    for (int x = 0; x < 8; ++x) {
+                        float g[8];
                         unpack8(u[x], g);
-                        unpack8(y[x], h);
 #pragma unroll
                         for (int q = 0; q < 8; ++q) {
-                            const float G = g[q] + h[q];
-                            v[q] = fmaf(w[x].x, G, v[q]);
-                            v[8 + q] = fmaf(w[x].y, G, v[8 + q]);
-                            v[16 + q] = fmaf(w[x].z, G, v[16 + q]);
-                            v[24 + q] = fmaf(w[x].w, G, v[24 + q]);
+                            v[q] = fmaf(w[x].x, g[q], v[q]);
+                            v[8 + q] = fmaf(w[x].y, g[q], v[8 + q]);
+                            v[16 + q] = fmaf(w[x].z, g[q], v[16 + q]);
+                            v[24 + q] = fmaf(w[x].w, g[q], v[24 + q]);
                         }
                     }
                 }
@@ -408,7 +408,7 @@ k_wide_contract(long N, int T, int ncell, int W, int Nm, const __grid_constant__
                         v[q] = keep + __shfl_xor_sync(0xffffffffu, send, o);
                     }
                 }
-                float *dst = sA + rs * 4 * W + 8 * ch;
+                float *dst = (isy ? sA2 + rs * 2 * W : sA + rs * 4 * W) + 8 * ch;
 #pragma unroll
                 for (int q = 0; q < 8; ++q) dst[q] += v[q];
             }
@@ -416,7 +416,10 @@ k_wide_contract(long N, int T, int ncell, int W, int Nm, const __grid_constant__
     }
     __syncthreads();
     const float inv_nm = 1.0f / (float)Nm;
-    for (int k = tid; k < 16 * W; k += 256) Aout[i * 16L * W + k] = sA[k] * inv_nm;
+    for (int k = tid; k < 16 * W; k += 256) {
+        const int c = k / (4 * W), m = k % (4 * W);
+        Aout[i * 16L * W + k] = (sA[k] + sA2[c * 2 * W + m % (2 * W)]) * inv_nm;
+    }
 }
 
 // per-atom power-of-two scale of the gradient images: max |gA_i| in [0.5, 1) (fp16 range; undone in gemm<3>)
@@ -610,8 +613,8 @@ cudaError_t launch_embed_fwd_wide(const dp_model *m, long N, const Grid3 &g, cha
     const WideArgs p = wide_args(m, N, ws, L);
     ok(wide_gemm<0>(m, p, W, 2 * W, p.T1, 0, st));
     ok(wide_gemm<1>(m, p, 2 * W, 4 * W, p.Y2, 1, st));
-    const int csm = 16 * W * 4 + WC_BATCH * 16;
-    DP_SMEM_OPTIN(k_wide_contract, 16 * 512 * 4 + WC_BATCH * 16);
+    const int csm = 24 * W * 4 + WC_BATCH * 16;
+    DP_SMEM_OPTIN(k_wide_contract, 24 * 512 * 4 + WC_BATCH * 16);
     k_wide_contract<<<(unsigned)N, 256, csm, st>>>(N, m->T, g.ncell, W, m->Nm, tt, tab, (const int *)(ws + L.bin_start),
                                                    (const int *)(ws + L.rowstart), (const float4 *)(ws + L.rows_rh),
                                                    (const int2 *)(ws + L.rows_id), p.Y2, p.T3, (float *)(ws + L.A));
