@@ -4,8 +4,8 @@
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..4] [--impl ours|reference]
 
 The default run times config 4 (headline), then configs 0-3 (`configs_summary`, each with its own roofline and oracle
-timing), measures the arithmetic-pipe peaks it quotes (`peaks`, dp_measure_peaks) and runs the paper's MD protocol
-(`md`, PAPER.md:151-153).
+timing), measures the arithmetic-pipe peaks it quotes (`peaks`, dp_measure_peaks), runs the paper's MD protocol
+(`md`) and the network-size study of PAPER.md:273-279 (`network_size_sweep`; alone: --config sweep).
 
 One "step" = one dp_compute (all of SURVEY.md section 8(a): cell list, formatted neighbour list, environment
 matrix, embedding net + contraction, fitting net forward/backward, embedding backward, ProdForce, ProdViral)
@@ -478,6 +478,19 @@ def main():
                                            "sample": f"{n2} evenly spaced centre atoms of {s2.name}, one evaluation ({dt2:.1f} s)"}
                 summ[s2.name] = rec
             line["configs_summary"] = summ
+            # network-size study (Fig. 7): copper, embedding nets up to 512-1024-2048, MIX-16.
+            # The widest net keeps 77 GB of activations in its workspace: everything above is released first, and a failure
+            # of this leg is recorded instead of losing the line.
+            try:
+                torch.cuda.empty_cache()
+                args.steps_saved, args.steps = args.steps, 3
+                rows = sweep_leg(args, binding, torch, synth, dev, flush, pk)
+                args.steps = args.steps_saved
+                line["network_size_sweep"] = {"workload": f"copper {4 * args.sweep_ncell ** 3} atoms, capacity 512, MIX-16, list build included",
+                                              "unit": "TFLOP/s (algorithmic flops of the whole evaluation / CUDA-event time)",
+                                              "peak_bf16_sustained_tflops": pk["bf16_sus"], "rows": rows}
+            except (Exception, SystemExit) as e:      # noqa: BLE001
+                line["network_size_sweep"] = {"error": repr(e)[:300]}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
