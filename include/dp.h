@@ -163,6 +163,25 @@ int dp_measure_peaks(double *out_host, int n_out, void *cuda_stream);
  * in *step (may be NULL), the ordinal of that call inside dp_compute.  The string is static. */
 const char *dp_last_cuda_error(const dp_model *m, int *step);
 
+/* ---- Exclusive prefix sum of the neighbour-list build (bin and row offsets), callable alone.
+ * start_dev[0 .. n] = exclusive prefix sums of cnt_dev[0 .. n) (n + 1 outputs; start_dev[n] = the total), 32-bit integers,
+ * exact.  Three launches on cuda_stream; returns without synchronising.  DP_EINVAL: n <= 0 or a null pointer; DP_ECUDA.
+ *
+ * dp_scan_exclusive: the path dp_compute runs.  scratch_dev: caller-owned device scratch of at least
+ * dp_scan_scratch_bytes(n) bytes (DP_ENOMEM if scratch_bytes is smaller).
+ *
+ * dp_scan_exclusive_static: the same result from an entry point that ALLOCATES NOTHING and needs no scratch from the caller,
+ * for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it).  Its
+ * scratch is a static device array inside the library (32,784 bytes, held by every GPU that loads the library until exit),
+ * which limits n to DP_SCAN_STATIC_MAX (more: DP_ENOMEM, nothing is launched).  The first call on a device looks the array up
+ * (no allocation; make that call before starting a graph capture).  All calls share the array, which keeps the last call's
+ * contents (the kernels write every word they read, so no clearing is needed): calls that OVERLAP on the GPU (different
+ * streams) race and give wrong sums; calls on one stream are ordered and safe.  It calls no cudaMalloc / cudaFree. */
+#define DP_SCAN_STATIC_MAX 16777216
+size_t dp_scan_scratch_bytes(int n);
+int dp_scan_exclusive(int n, const int *cnt_dev, int *start_dev, void *scratch_dev, size_t scratch_bytes, void *cuda_stream);
+int dp_scan_exclusive_static(int n, const int *cnt_dev, int *start_dev, void *cuda_stream);
+
 void dp_destroy(dp_model *m);
 const char *dp_strerror(int code);
 

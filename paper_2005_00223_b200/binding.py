@@ -18,7 +18,9 @@ DP_FP64, DP_MIX32, DP_MIX16 = 0, 1, 2
 PRECISIONS = {"fp64": DP_FP64, "mix32": DP_MIX32, "mix16": DP_MIX16}
 EXPORTS = ["dp_create", "dp_workspace_bytes", "dp_compute", "dp_get_nlist", "dp_status",
            "dp_launches_per_compute", "dp_last_row_counts", "dp_profile_enable", "dp_profile_read", "dp_md_run",
-           "dp_md_workspace_bytes", "dp_measure_peaks", "dp_last_cuda_error", "dp_destroy", "dp_strerror"]
+           "dp_md_workspace_bytes", "dp_measure_peaks", "dp_last_cuda_error", "dp_destroy", "dp_strerror",
+           "dp_scan_scratch_bytes", "dp_scan_exclusive", "dp_scan_exclusive_static"]
+SCAN_STATIC_MAX = 16777216          # DP_SCAN_STATIC_MAX (include/dp.h)
 
 
 class DPError(RuntimeError):
@@ -75,6 +77,12 @@ def lib():
         L.dp_last_cuda_error.argtypes = [vp, C.POINTER(C.c_int)]
         L.dp_destroy.restype = None
         L.dp_destroy.argtypes = [vp]
+        L.dp_scan_scratch_bytes.restype = C.c_size_t
+        L.dp_scan_scratch_bytes.argtypes = [C.c_int]
+        L.dp_scan_exclusive.restype = C.c_int
+        L.dp_scan_exclusive.argtypes = [C.c_int, vp, vp, vp, C.c_size_t, vp]
+        L.dp_scan_exclusive_static.restype = C.c_int
+        L.dp_scan_exclusive_static.argtypes = [C.c_int, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -248,6 +256,26 @@ def measure_peaks(stream=None) -> dict:
         raise DPError(rc, "dp_measure_peaks")
     return dict(dfma_tflops=out[0], dmma_tflops=out[1], ffma_tflops=out[2], tanh_tera_per_s=out[3],
                 hmma_sync_tflops=out[4], sms=int(out[5]))
+
+
+def scan_exclusive(cnt, out, scratch, stream=None) -> None:
+    """dp_scan_exclusive: out[0..n] = exclusive prefix sums of cnt[0..n) (int32 CUDA tensors), caller-owned scratch tensor."""
+    import torch
+    st = stream if stream is not None else torch.cuda.current_stream()
+    rc = lib().dp_scan_exclusive(int(cnt.numel()), cnt.data_ptr(), out.data_ptr(), scratch.data_ptr(),
+                                 scratch.numel() * scratch.element_size(), st.cuda_stream)
+    if rc != 0:
+        raise DPError(rc, "dp_scan_exclusive")
+
+
+def scan_exclusive_static(cnt, out, stream=None) -> None:
+    """dp_scan_exclusive_static: the same result with the scratch in a static device array of the library: no allocation,
+    n <= SCAN_STATIC_MAX; calls that overlap on the GPU race on that array (include/dp.h)."""
+    import torch
+    st = stream if stream is not None else torch.cuda.current_stream()
+    rc = lib().dp_scan_exclusive_static(int(cnt.numel()), cnt.data_ptr(), out.data_ptr(), st.cuda_stream)
+    if rc != 0:
+        raise DPError(rc, "dp_scan_exclusive_static")
 
 
 def compute_host(model_handle: DPModel, coords_np, types_np, box, device="cuda:0"):
