@@ -53,6 +53,7 @@ WsLayout ws_layout(const dp_model *m, long N, long NE) {
         L.rows_id = take(sizeof(int) * 2 * (size_t)N * m->Nm);
         if (m->prec == DP_MIX16) {
             L.rows_g = take(sizeof(float) * 4 * (size_t)N * m->Nm);
+            L.fj32 = take(sizeof(float) * 4 * (size_t)NE);
             L.multi_cnt = take(sizeof(int) * DP_MAX_TYPES * DP_MAX_TYPES);
         }
     }
@@ -567,8 +568,8 @@ int dp_launches_per_compute(const dp_model *m) {
     } else {
         n += 3 * m->T;                               // row prefix sums, one 3-launch scan per neighbour type
         n += 2;                                      // environment rows + tcgen05 forward
-        if (m->wide) n += 4 + 3 + 5;                 // tile table, layer 1, two GEMMs, contraction; fitting (3); scale, head, two GEMMs, force + virial
-        else if (m->prec == DP_MIX16) n += 3 + 5;    // first layer, fused 240 x 240 chain, last product; gA fold, tile classes, backward (two launches), force + virial
+        if (m->wide) n += 4 + 3 + 6;                 // tile table, layer 1, two GEMMs, contraction; fitting (3); scale, head, two GEMMs, force + virial, fp32 shares
+        else if (m->prec == DP_MIX16) n += 3 + 6;    // first layer, fused 240 x 240 chain, last product; gA fold, tile classes, backward (two launches), force + virial, fp32 shares
         else n += 9 + 1;                             // descriptor, 6 GEMMs, energy, gA fragments; backward (with S8, S9)
     }
     return n + 1;                                    // finalize

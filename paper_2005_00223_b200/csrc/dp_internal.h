@@ -130,6 +130,7 @@ struct WsLayout {
     size_t rows_rh;     // float4[T][N*sel_b...] compact env rows R^ (mixed modes, tcgen05 path)
     size_t rows_id;     // int2 {atom, neighbour j} ; {atom, -npad} for the padded-row representative
     size_t rows_g;      // float4 dE/dR~ per compact row (MIX-16 tcgen05 backward -> ProdForce / ProdViral)
+    size_t fj32;        // float4[NE] MIX-16: the neighbours' force shares, accumulated by 16-byte fp32 vector reductions
     size_t multi_cnt;   // int[16][16] MIX-16 backward: 1 if a tile of the (centre, neighbour) type block spans more than two atoms
     size_t A;           // double[N][4][100]   (float for mixed modes)
     size_t gAf;         // gA fragments [N][42][32] doubles (fp64) / [N][NSW][28][32] words (mixed)

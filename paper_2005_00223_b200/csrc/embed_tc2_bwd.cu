@@ -674,7 +674,7 @@ k_embed_bwd_tc2(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTa
 __global__ void __launch_bounds__(256)
 k_prod_force_virial(long N, int T, const __grid_constant__ TypeTab tt, EnvParams ep, const int *__restrict__ rowstart,
                     const int2 *__restrict__ rows_id, const float4 *__restrict__ rows_g, const double *__restrict__ xs,
-                    double *__restrict__ fsorted, double *__restrict__ virial) {
+                    double *__restrict__ fsorted, float4 *__restrict__ fj32, double *__restrict__ virial) {
     const int lane = threadIdx.x & 31;
     const int *sel = tt.sel, *off = tt.off;
     const double hx = 0.5 * ep.L[0], hy = 0.5 * ep.L[1], hz = 0.5 * ep.L[2];
@@ -721,7 +721,12 @@ k_prod_force_virial(long N, int T, const __grid_constant__ TypeTab tt, EnvParams
                 gk[1] = c0 * dy + c1 * g2_;
                 gk[2] = c0 * dz + c1 * g3_;
 #pragma unroll
-                for (int bb = 0; bb < 3; ++bb) atomicAdd(&fsorted[3 * (long)j + bb], -gk[bb]);
+                for (int bb = 0; bb < 3 && !fj32; ++bb) atomicAdd(&fsorted[3 * (long)j + bb], -gk[bb]);
+                // the neighbour's share: ONE 16-byte fp32 vector reduction per row instead of three fp64 ones (the L2 reduction
+                // rate bounds this kernel); k_force_add32 adds the fp32 sums to the fp64 forces afterwards
+                if (fj32)
+                    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(fj32 + j), "f"((float)-gk[0]), "f"((float)-gk[1]),
+                                 "f"((float)-gk[2]), "f"(0.f) : "memory");
                 vir[0] -= dx * gk[0]; vir[1] -= dx * gk[1]; vir[2] -= dx * gk[2];
                 vir[3] -= dy * gk[0]; vir[4] -= dy * gk[1]; vir[5] -= dy * gk[2];
                 vir[6] -= dz * gk[0]; vir[7] -= dz * gk[1]; vir[8] -= dz * gk[2];
@@ -761,7 +766,32 @@ k_prod_force_virial(long N, int T, const __grid_constant__ TypeTab tt, EnvParams
     }
 }
 
+// fsorted[k] += fj32[k] (the neighbour shares accumulated in fp32 by k_prod_force_virial)
+__global__ void __launch_bounds__(256) k_force_add32(long n, const float4 *__restrict__ fj32, double *__restrict__ fsorted) {
+    const long k = blockIdx.x * 256L + threadIdx.x;
+    if (k >= n) return;
+    const float4 v = fj32[k];
+    fsorted[3 * k] += (double)v.x;
+    fsorted[3 * k + 1] += (double)v.y;
+    fsorted[3 * k + 2] += (double)v.z;
+}
+
 }  // namespace
+
+// S8 + S9 from the per-row gradients in rows_g (the tail of the MIX-16 backward and of the wide-network backward, wide.cu)
+cudaError_t launch_prod_force_virial(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    const TypeTab tt = make_typetab(m);
+    EnvParams ep;
+    ep.rc = m->rc; ep.rc_smth = m->rc_smth; ep.inv_range = 1.0 / (m->rc - m->rc_smth);
+    ep.L[0] = g.L[0]; ep.L[1] = g.L[1]; ep.L[2] = g.L[2];
+    float4 *fj32 = (float4 *)(ws + L.fj32);
+    cudaMemsetAsync(fj32, 0, sizeof(float4) * (size_t)g.cap_ext, st);
+    k_prod_force_virial<<<m->num_sms * 8, 256, 0, st>>>(N, m->T, tt, ep, (int *)(ws + L.rowstart),
+                                                        (const int2 *)(ws + L.rows_id), (const float4 *)(ws + L.rows_g),
+                                                        (double *)(ws + L.xs), (double *)(ws + L.fsorted), fj32, (double *)(ws + L.virial));
+    k_force_add32<<<(unsigned)((g.cap_ext + 255) / 256), 256, 0, st>>>(g.cap_ext, fj32, (double *)(ws + L.fsorted));
+    return cudaGetLastError();
+}
 
 template <int W>
 static cudaError_t launch_bwd_w(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
@@ -801,9 +831,10 @@ static cudaError_t launch_bwd_w(const dp_model *m, long N, const Grid3 &g, char 
         (const uint8_t *)(ws + L.gAf), (const float *)(ws + L.gscale), (float4 *)(ws + L.rows_g),
         (unsigned long long *)(ws + L.status + 16), multi_flag, nullptr);
     if (m->profile) cudaEventRecord(m->ev[7], st);
-    k_prod_force_virial<<<m->num_sms * 8, 256, 0, st>>>(N, m->T, tt, ep, (int *)(ws + L.rowstart),
-                                                        (const int2 *)(ws + L.rows_id), (const float4 *)(ws + L.rows_g),
-                                                        (double *)(ws + L.xs), (double *)(ws + L.fsorted), (double *)(ws + L.virial));
+    {
+        const cudaError_t e2 = launch_prod_force_virial(m, N, g, ws, L, st);
+        if (e2 != cudaSuccess) return e2;
+    }
 #ifdef DP_BWD_TIMING
     if (tdbg) {
         cudaStreamSynchronize(st);
@@ -816,18 +847,6 @@ static cudaError_t launch_bwd_w(const dp_model *m, long N, const Grid3 &g, char 
         fprintf(stderr, "\n");
     }
 #endif
-    return cudaGetLastError();
-}
-
-// S8 + S9 from the per-row gradients in rows_g (also the tail of the wide-network backward, wide.cu)
-cudaError_t launch_prod_force_virial(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    const TypeTab tt = make_typetab(m);
-    EnvParams ep;
-    ep.rc = m->rc; ep.rc_smth = m->rc_smth; ep.inv_range = 1.0 / (m->rc - m->rc_smth);
-    ep.L[0] = g.L[0]; ep.L[1] = g.L[1]; ep.L[2] = g.L[2];
-    k_prod_force_virial<<<m->num_sms * 8, 256, 0, st>>>(N, m->T, tt, ep, (int *)(ws + L.rowstart),
-                                                        (const int2 *)(ws + L.rows_id), (const float4 *)(ws + L.rows_g),
-                                                        (double *)(ws + L.xs), (double *)(ws + L.fsorted), (double *)(ws + L.virial));
     return cudaGetLastError();
 }
 

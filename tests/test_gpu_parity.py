@@ -328,7 +328,7 @@ def test_profile_slots_and_launch_count():
     ms = m.profile_read()
     assert ms.shape == (6,) and (ms >= 0).all()
     assert 0 < ms[5] <= ms[3]                  # the backward kernel alone is a part of the backward phase
-    assert m.launches_per_compute() == 21      # one type: 18 + 3 T (every scan is three launches)
+    assert m.launches_per_compute() == 22      # one type: 19 + 3 T (every scan is three launches)
     m.close()
 
 
