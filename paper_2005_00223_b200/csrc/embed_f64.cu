@@ -128,8 +128,28 @@ __device__ __forceinline__ int feature3(int nt3, int r, int j3) {
     return e < W ? e + W * (nt3 & 1) + 2 * W * j3 : -1;
 }
 
-__device__ __forceinline__ void copy_to_smem(double *dst, const double *__restrict__ src, int n) {
-    for (int k = threadIdx.x; k < n; k += blockDim.x) dst[k] = src[k];
+// Stage one (centre type, neighbour type) net in shared memory: ONE bulk copy (cp.async.bulk, completion on an mbarrier) issued
+// by thread 0; every thread waits on the barrier.  (A loop of per-thread loads took 20-50 us per net: a third of the forward
+// at 500 atoms.)  Callers bracket it with __syncthreads(); phase = parity of the number of copies this CTA has made.
+__device__ __forceinline__ void stage_net(double *dst, const double *__restrict__ src, int n, uint64_t *bar, uint32_t &phase) {
+    const uint32_t b = (uint32_t)__cvta_generic_to_shared(bar);
+    if (threadIdx.x == 0) {
+        const uint32_t bytes = (uint32_t)n * 8u;
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(b), "r"(bytes) : "memory");
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src), "r"(bytes), "r"(b) : "memory");
+    }
+    asm volatile("{\n.reg .pred p;\nSW_%=:\nmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra SD_%=;\nbra SW_%=;\nSD_%=:\n}"
+                 ::"r"(b), "r"(phase) : "memory");
+    phase ^= 1u;
+}
+__device__ __forceinline__ void stage_init(uint64_t *bar) {
+    if (threadIdx.x == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"((uint32_t)__cvta_generic_to_shared(bar)));
+        asm volatile("fence.mbarrier_init.release.cluster;");
+    }
+    __syncthreads();
 }
 
 template <int W> __host__ __device__ constexpr int fwd_net_doubles() {
@@ -142,14 +162,18 @@ constexpr int WARP_BUF_DOUBLES = ROWCHUNK * 5;   // rbuf[ROWCHUNK][4] + sbuf[ROW
 // ------------------------------------------------------------------------------------------------ forward
 template <int W>
 __global__ void __launch_bounds__(DP_WARPS_PER_CTA * 32, 1)
-k_embed_fwd_f64(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, EnvParams ep, const EmbedNetFrag<double, W> *__restrict__ nets,
+k_embed_fwd_f64(int T, int ncell, int Nm, int CH, const __grid_constant__ TypeTab tt, EnvParams ep, const EmbedNetFrag<double, W> *__restrict__ nets,
                 const double *__restrict__ avg, const double *__restrict__ stdv, const int *__restrict__ bin_start,
                 const double *__restrict__ xs, const int *__restrict__ nlist, const int *__restrict__ nreal,
                 double *__restrict__ Aout, unsigned long long *__restrict__ row_counter) {
     constexpr int M0 = EmbW<W>::M0, M1 = EmbW<W>::M1, M2E = EmbW<W>::M2E, KC1 = EmbW<W>::KC1, NT2 = EmbW<W>::NT2, NT3 = EmbW<W>::NT3, NT1 = EmbW<W>::NT1;
     (void)M0; (void)M1; (void)M2E; (void)KC1; (void)NT2; (void)NT3; (void)NT1;
     constexpr int FWD_NET_DOUBLES = fwd_net_doubles<W>();
+    static_assert(FWD_NET_DOUBLES % 2 == 0 && sizeof(EmbedNetFrag<double, W>) % 16 == 0, "bulk copies move multiples of 16 bytes");
     extern __shared__ __align__(16) double smem[];
+    __shared__ uint64_t stage_bar;
+    uint32_t stage_phase = 0;
+    stage_init(&stage_bar);
     EmbedNetFrag<double, W> *net = reinterpret_cast<EmbedNetFrag<double, W> *>(smem);
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     double *rbuf = smem + FWD_NET_DOUBLES + wid * WARP_BUF_DOUBLES;
@@ -170,18 +194,24 @@ k_embed_fwd_f64(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, En
         int off = 0;
         for (int b = 0; b < T; ++b) {
             __syncthreads();
-            copy_to_smem(smem, reinterpret_cast<const double *>(nets + (a * T + b)), FWD_NET_DOUBLES);
+            stage_net(smem, reinterpret_cast<const double *>(nets + (a * T + b)), FWD_NET_DOUBLES, &stage_bar, stage_phase);
             __syncthreads();
-            for (int i = ts0 + gw; i < ts1; i += NW) {
+            // work item = (atom, row chunk).  CH == ROWCHUNK (large systems): one item per atom walks all its chunks and writes
+            // A_i itself.  CH < ROWCHUNK (systems with fewer atoms than warps): S items per atom, one chunk of CH rows each, so
+            // that every warp has work; their partial sums meet in A_i (zeroed by the launcher) through fp64 atomics.
+            const int S = CH == ROWCHUNK ? 1 : (sel[b] + CH) / CH;
+            for (long it = gw; it < (long)(ts1 - ts0) * S; it += NW) {
+                const int i = ts0 + (int)(it / S), part = (int)(it % S);
                 const int nr = nreal[i * T + b];
                 const int npad = sel[b] - nr;
                 const int rows = nr + (npad > 0 ? 1 : 0);
+                if (part * CH >= rows) continue;
                 const double xi = xs[3 * (long)i], yi = xs[3 * (long)i + 1], zi = xs[3 * (long)i + 2];
                 double accA[NT3][2];
 #pragma unroll
                 for (int t = 0; t < NT3; ++t) accA[t][0] = accA[t][1] = 0.0;
-                for (int r0 = 0; r0 < rows; r0 += ROWCHUNK) {
-                    const int nrow_c = min(ROWCHUNK, rows - r0);
+                for (int r0 = part * CH; r0 < rows; r0 += S * CH) {
+                    const int nrow_c = min(CH, rows - r0);
                     const int ntile = (nrow_c + 7) >> 3;
                     // pre-pass: weighted R^ rows and s^ of this chunk
                     for (int rr = lane; rr < ntile * 8; rr += 32) {
@@ -236,7 +266,8 @@ k_embed_fwd_f64(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, En
                             const int f = feature3<W>(nt3, r, j);
                             if (f >= 0) {
                                 const double v = accA[nt3][j] * inv_nm;
-                                Ai[f] = (b == 0) ? v : Ai[f] + v;
+                                if (S > 1) atomicAdd(&Ai[f], v);
+                                else Ai[f] = (b == 0) ? v : Ai[f] + v;
                             }
                         }
                     }
@@ -254,7 +285,7 @@ k_embed_fwd_f64(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, En
 //   [14..42) : dR^ MMA  B fragment of chunk kc = 2*nt3 + j3: lane -> (lane/4 < 4) ? gA[c = lane/4][feature3(nt3, lane%4, j3)] : 0
 template <int W, bool CALL>
 __global__ void __launch_bounds__(DP_WARPS_PER_CTA * 32, 1)
-k_embed_bwd_f64(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, EnvParams ep, const EmbedNetFrag<double, W> *__restrict__ nets,
+k_embed_bwd_f64(int T, int ncell, int Nm, int CH, const __grid_constant__ TypeTab tt, EnvParams ep, const EmbedNetFrag<double, W> *__restrict__ nets,
                 const double *__restrict__ avg, const double *__restrict__ stdv, const int *__restrict__ bin_start,
                 const double *__restrict__ xs, const int *__restrict__ nlist, const int *__restrict__ nreal,
                 const double *__restrict__ gAf, double *__restrict__ fsorted, double *__restrict__ virial,
@@ -263,6 +294,9 @@ k_embed_bwd_f64(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, En
     (void)M0; (void)M1; (void)M2E; (void)KC1; (void)NT2; (void)NT3; (void)NT1;
     constexpr int BWD_NET_DOUBLES = bwd_net_doubles<W>();
     extern __shared__ __align__(16) double smem[];
+    __shared__ uint64_t stage_bar;
+    uint32_t stage_phase = 0;
+    stage_init(&stage_bar);
     EmbedNetFrag<double, W> *net = reinterpret_cast<EmbedNetFrag<double, W> *>(smem);
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     double *rbuf = smem + BWD_NET_DOUBLES + wid * WARP_BUF_DOUBLES;
@@ -285,15 +319,18 @@ k_embed_bwd_f64(int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, En
         int off = 0;
         for (int b = 0; b < T; ++b) {
             __syncthreads();
-            copy_to_smem(smem, reinterpret_cast<const double *>(nets + (a * T + b)), BWD_NET_DOUBLES);
+            stage_net(smem, reinterpret_cast<const double *>(nets + (a * T + b)), BWD_NET_DOUBLES, &stage_bar, stage_phase);
             __syncthreads();
-            for (int i = ts0 + gw; i < ts1; i += NW) {
+            const int S = CH == ROWCHUNK ? 1 : (sel[b] + CH) / CH;       // work items per atom (see the forward kernel)
+            for (long it = gw; it < (long)(ts1 - ts0) * S; it += NW) {
+                const int i = ts0 + (int)(it / S), part = (int)(it % S);
                 const int nr = nreal[i * T + b];
+                if (part * CH >= nr) continue;
                 const double xi = xs[3 * (long)i], yi = xs[3 * (long)i + 1], zi = xs[3 * (long)i + 2];
                 const double *gf = gAf + (long)i * (3 * NT3 * 32);
                 double fi[3] = {0.0, 0.0, 0.0};
-                for (int r0 = 0; r0 < nr; r0 += ROWCHUNK) {
-                    const int nrow_c = min(ROWCHUNK, nr - r0);
+                for (int r0 = part * CH; r0 < nr; r0 += S * CH) {
+                    const int nrow_c = min(CH, nr - r0);
                     const int ntile = (nrow_c + 7) >> 3;
                     for (int rr = lane; rr < ntile * 8; rr += 32) {
                         const int row = r0 + rr;
@@ -428,8 +465,15 @@ EnvParams make_env(const dp_model *m, const Grid3 &g) {
 template <int W> constexpr int smem_fwd() { return (fwd_net_doubles<W>() + DP_WARPS_PER_CTA * WARP_BUF_DOUBLES) * 8; }
 template <int W> constexpr int smem_bwd() { return (bwd_net_doubles<W>() + DP_WARPS_PER_CTA * WARP_BUF_DOUBLES) * 8; }
 
+// rows per work item: a whole atom in chunks of ROWCHUNK when there are several atoms' worth of chunks per warp, else chunks of
+// 16 rows (two 8-row tiles) as items of their own (config 0: 500 atoms for 1,184 warps, 18 tiles per atom)
+static int embed_chunk(const dp_model *m, long N) {
+    return N * (long)m->Nm / ROWCHUNK >= 4L * m->num_sms * DP_WARPS_PER_CTA ? ROWCHUNK : 16;
+}
 static int embed_grid(const dp_model *m, long N) {
-    long grid = (N + DP_WARPS_PER_CTA - 1) / DP_WARPS_PER_CTA;
+    const int CH = embed_chunk(m, N);
+    long items = CH == ROWCHUNK ? N : N * ((m->Nm + CH) / CH);
+    long grid = (items + DP_WARPS_PER_CTA - 1) / DP_WARPS_PER_CTA;
     return (int)(grid > m->num_sms ? m->num_sms : grid);
 }
 
@@ -437,8 +481,10 @@ template <int W>
 static cudaError_t launch_fwd_w(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
     DP_SMEM_OPTIN(k_embed_fwd_f64<W>, smem_fwd<W>());
     const TypeTab tt = make_typetab(m);
+    const int CH = embed_chunk(m, N);
+    if (CH != ROWCHUNK) cudaMemsetAsync(ws + L.A, 0, sizeof(double) * (size_t)N * 4 * m->m2, st);      // partial sums meet by atomics
     k_embed_fwd_f64<W><<<embed_grid(m, N), DP_WARPS_PER_CTA * 32, smem_fwd<W>(), st>>>(
-        m->T, g.ncell, m->Nm, tt, make_env(m, g), (const EmbedNetFrag<double, W> *)m->embed_frag_dev, m->avg_dev,
+        m->T, g.ncell, m->Nm, CH, tt, make_env(m, g), (const EmbedNetFrag<double, W> *)m->embed_frag_dev, m->avg_dev,
         m->std_dev, (int *)(ws + L.bin_start), (double *)(ws + L.xs), (int *)(ws + L.nlist), (int *)(ws + L.nreal),
         (double *)(ws + L.A), (unsigned long long *)(ws + L.status + 8));
     return cudaGetLastError();
@@ -449,7 +495,7 @@ static cudaError_t launch_bwd_w(const dp_model *m, long N, const Grid3 &g, char 
     DP_SMEM_OPTIN((k_embed_bwd_f64<W, CALL>), smem_bwd<W>());
     const TypeTab tt = make_typetab(m);
     k_embed_bwd_f64<W, CALL><<<embed_grid(m, N), DP_WARPS_PER_CTA * 32, smem_bwd<W>(), st>>>(
-        m->T, g.ncell, m->Nm, tt, make_env(m, g), (const EmbedNetFrag<double, W> *)m->embed_frag_dev, m->avg_dev,
+        m->T, g.ncell, m->Nm, embed_chunk(m, N), tt, make_env(m, g), (const EmbedNetFrag<double, W> *)m->embed_frag_dev, m->avg_dev,
         m->std_dev, (int *)(ws + L.bin_start), (double *)(ws + L.xs), (int *)(ws + L.nlist), (int *)(ws + L.nreal),
         (double *)(ws + L.gAf), (double *)(ws + L.fsorted), (double *)(ws + L.virial),
         (unsigned long long *)(ws + L.status + 16));
