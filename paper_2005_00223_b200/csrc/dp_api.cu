@@ -565,6 +565,7 @@ int dp_launches_per_compute(const dp_model *m) {
     int n = 6 + 1;                                   // wrap, 3-launch bin scan, scatter, bin sort; list
     if (m->prec == DP_FP64) {
         n += 1 + 9 + 1;                              // forward; descriptor, 6 GEMMs, energy, gA; backward (with S8, S9)
+        if (m->last_natoms > 0 && fit_f64_splitk(m, m->last_natoms)) n += 1;     // small systems: split-K first layer + bias / tanh
     } else {
         n += 3 * m->T;                               // row prefix sums, one 3-launch scan per neighbour type
         n += 2;                                      // environment rows + tcgen05 forward

@@ -152,6 +152,12 @@ struct WsLayout {
     size_t wide_t1, wide_y2, wide_t2, wide_t3;      // W, 2 W, 2 W, 4 W columns
 };
 
+// FP64 fitting net, first layer (K = 16 m2): split K over four CTAs per output tile when the row tiles (64 rows x 80 columns)
+// are too few to fill the GPU (fit_f64.cu; one more launch per evaluation: dp_launches_per_compute)
+inline bool fit_f64_splitk(const dp_model *m, long N) {
+    return ((N + 63) / 64) * 3 * 2 <= m->num_sms && (m->m2 * 16 / 16) % 4 == 0;
+}
+
 // neighbour capacities per type and their prefix sums, passed to kernels by value (a __grid_constant__ parameter: indexed
 // dynamically straight from constant memory)
 struct TypeTab {

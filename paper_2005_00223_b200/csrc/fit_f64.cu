@@ -36,6 +36,8 @@ struct FitArgs {
     int ncell;
     const int *bin_start;
     int K, N;                 // GEMM inner and output widths
+    int ksplit;               // MODE 0 on small systems: K is split over ksplit CTAs per output tile (0 / 1: no split); the partial
+                              // sums meet in out0 (zeroed by the launcher) through fp64 atomics and k_bias_tanh finishes the layer
     const double *A; int lda;             // [rows][K]
     const double *B; long b_type_stride; int ldb;   // weights of type a at B + a*b_type_stride
     const double *bias; int bias_type_stride;       // epilogue vector (c1/c2/c3 or v4)
@@ -53,7 +55,9 @@ __global__ void __launch_bounds__(256) k_fit_gemm(FitArgs p) {
     const int ts0 = p.bin_start[a * p.ncell], ts1 = p.bin_start[(a + 1) * p.ncell];
     const int row0 = ts0 + blockIdx.x * BM;
     if (row0 >= ts1) return;
-    const int n0 = blockIdx.y * BN;
+    const int ntn = (p.N + BN - 1) / BN;
+    const int n0 = (blockIdx.y % ntn) * BN, kpart = blockIdx.y / ntn;
+    const bool split = MODE == 0 && p.ksplit > 1;
     const double *Bw = p.B + a * p.b_type_stride;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int wm = wid >> 1, wn = wid & 1;         // 4 x 2 warps, warp tile 16 x 40
@@ -91,10 +95,11 @@ __global__ void __launch_bounds__(256) k_fit_gemm(FitArgs p) {
 #pragma unroll
         for (int nt = 0; nt < 5; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
 
-    const int nk = p.K / BK;
-    load_tiles(0, 0);
+    const int nk_all = p.K / BK;
+    const int nk = split ? nk_all / p.ksplit : nk_all, kb = split ? kpart * nk : 0;      // k-steps of this CTA: [kb, kb + nk)
+    load_tiles(0, kb * BK);
     for (int ks = 0; ks < nk; ++ks) {
-        if (ks + 1 < nk) { load_tiles((ks + 1) & 1, (ks + 1) * BK); cp_async_wait<1>(); }
+        if (ks + 1 < nk) { load_tiles((ks + 1) & 1, (kb + ks + 1) * BK); cp_async_wait<1>(); }
         else cp_async_wait<0>();
         __syncthreads();
         const double *As = sm + (ks & 1) * (AS_TILE + B_TILE);
@@ -127,7 +132,10 @@ __global__ void __launch_bounds__(256) k_fit_gemm(FitArgs p) {
             if (col >= p.N) continue;          // N = 16 m2 need not be a multiple of the tile width
             const long o = (long)row * p.ldo + col;
             double v0 = acc[mt][nt][0], v1 = acc[mt][nt][1];
-            if (MODE == 0) {
+            if (MODE == 0 && split) {
+                atomicAdd(p.out0 + o, v0);
+                atomicAdd(p.out0 + o + 1, v1);
+            } else if (MODE == 0) {
                 const double *b = p.bias + a * p.bias_type_stride + col;
                 *reinterpret_cast<double2 *>(p.out0 + o) = make_double2(dp_tanh64(v0 + b[0]), dp_tanh64(v1 + b[1]));
             } else if (MODE == 1) {
@@ -159,6 +167,18 @@ __global__ void __launch_bounds__(256) k_fit_gemm(FitArgs p) {
             }
         }
     }
+}
+
+// second half of the split-K first layer: h1 = tanh(h1 + c1[type]) in place
+__global__ void __launch_bounds__(256) k_bias_tanh(long N, int T, int ncell, int F, const int *__restrict__ bin_start,
+                                                   const double *__restrict__ bias, double *__restrict__ h) {
+    const long k = blockIdx.x * 256L + threadIdx.x;
+    if (k >= N * F) return;
+    const long i = k / F;
+    const int col = (int)(k % F);
+    int a = 0;
+    for (int t = 1; t < T; ++t) a += i >= bin_start[t * ncell];
+    h[k] = dp_tanh64(h[k] + bias[a * F + col]);
 }
 
 // D[i][m*16 + a] = sum_c A[i][c][m] A[i][c][a]    (N6, Q6, Q7); one warp per atom
@@ -273,7 +293,16 @@ static cudaError_t launch_fit_w(const dp_model *m, long N, const Grid3 &g, char 
     // layer 1 forward: h1 = tanh(D V1 + c1)
     p.K = ND; p.N = F; p.A = D; p.lda = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.ldb = F; p.bias = c1;
     p.out0 = h1; p.ldo = F;
-    k_fit_gemm<0><<<dim3(gx, F / BN, T), 256, 0, st>>>(p);
+    // few row tiles (configs 0, 1: 24 / 72 CTAs walking K = 1,600): split K four ways so that the GPU fills
+    p.ksplit = fit_f64_splitk(m, N) ? 4 : 1;
+    if (p.ksplit > 1) {
+        cudaMemsetAsync(h1, 0, sizeof(double) * S, st);
+        k_fit_gemm<0><<<dim3(gx, (F / BN) * p.ksplit, T), 256, 0, st>>>(p);
+        k_bias_tanh<<<(unsigned)((S + 255) / 256), 256, 0, st>>>(N, T, g.ncell, F, bin_start, c1, h1);
+    } else {
+        k_fit_gemm<0><<<dim3(gx, F / BN, T), 256, 0, st>>>(p);
+    }
+    p.ksplit = 1;
     // layer 2 forward: t2 = tanh(h1 V2 + c2), h2 = h1 + t2
     p.K = F; p.A = h1; p.lda = F; p.B = V2; p.b_type_stride = (long)F * F; p.bias = c2; p.aux0 = h1; p.out0 = t2; p.out1 = h2;
     k_fit_gemm<1><<<dim3(gx, F / BN, T), 256, 0, st>>>(p);
