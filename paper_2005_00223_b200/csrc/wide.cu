@@ -446,13 +446,51 @@ __global__ void __launch_bounds__(256) k_wide_gscale(long N, int n, const float 
 //   gG[f] + gG[f + 2 W]                       -> over y2 (the skip connection's share of dy2, added in the epilogue of gemm<2>)
 //   dR^[c] = sc sum_m G[m] gA[c][m]           -> rows_g (finished by gemm<3>)
 // Padded-row representatives carry no gradient (R~ = 0 there is a constant): skipped.
-__global__ void __launch_bounds__(2 * WR, 2)
+// The three 2 KB activation chunks of a step (per column half) are staged in shared memory by a producer warp with bulk copies, four
+// steps (48 KB per CTA, 96 KB per SM) ahead of the arithmetic: with per-thread loads one step ahead the kernel reached 4.5 TB/s.
+constexpr int BE_STAGES = 4;
+constexpr int BE_STAGE_BYTES = 2 * 3 * 2048;          // [column half][y2, t3 lower, t3 upper][128 rows x 16 B]
+constexpr int BE_THREADS = 2 * WR + 32;               // 256 consumers (row, column half) + the producer warp
+__global__ void __launch_bounds__(BE_THREADS, 2)
 k_wide_bwd_elem(long N, int T, int W, const __grid_constant__ TypeTab tt, const int4 *__restrict__ tab,
                 const float4 *__restrict__ rows_rh, const int2 *__restrict__ rows_id, const float *__restrict__ gA,
                 const float *__restrict__ gscale, uint8_t *__restrict__ Y2, uint8_t *__restrict__ T3, float4 *__restrict__ rows_g) {
+    extern __shared__ __align__(128) uint8_t bsm[];
     __shared__ float4 sdr[WR];
-    const int nblk = T * T, ntiles = tab[nblk].x, r = threadIdx.x & (WR - 1), hf = threadIdx.x >> 7;
-    const int ych = 2 * W / 8, M2 = 4 * W;
+    __shared__ uint64_t full[BE_STAGES], empty[BE_STAGES];
+    const int nblk = T * T, ntiles = tab[nblk].x;
+    const int ych = 2 * W / 8, M2 = 4 * W, nstep = ych / 2;
+    if (threadIdx.x == 0) {
+        for (int k = 0; k < BE_STAGES; ++k) { tc::mbar_init(&full[k], 1); tc::mbar_init(&empty[k], 8); }
+        asm volatile("fence.mbarrier_init.release.cluster;");
+    }
+    __syncthreads();
+    if (threadIdx.x >= 2 * WR) {
+        // ---------------------------------------------------------------- producer warp
+        if (threadIdx.x == 2 * WR) {
+            uint32_t step = 0;
+            for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+                const uint8_t *y2t = Y2 + (size_t)tile * ych * 2048, *t3t = T3 + (size_t)tile * (2 * ych) * 2048;
+                for (int sidx = 0; sidx < nstep; ++sidx, ++step) {
+                    const int st = step % BE_STAGES;
+                    tc::mbar_wait(&empty[st], ((step / BE_STAGES) & 1) ^ 1);
+                    mbar_expect_tx(&full[st], BE_STAGE_BYTES);
+                    const uint32_t dst = tc::smem_u32(bsm + st * BE_STAGE_BYTES);
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const size_t f = (size_t)sidx + h * nstep;
+                        bulk_g2s(dst + h * 6144, y2t + f * 2048, 2048, &full[st]);
+                        bulk_g2s(dst + h * 6144 + 2048, t3t + f * 2048, 2048, &full[st]);
+                        bulk_g2s(dst + h * 6144 + 4096, t3t + (f + ych) * 2048, 2048, &full[st]);
+                    }
+                }
+            }
+        }
+        return;
+    }
+    // -------------------------------------------------------------------- consumers: thread = (row, column half)
+    const int r = threadIdx.x & (WR - 1), hf = threadIdx.x >> 7, lane = threadIdx.x & 31;
+    uint32_t step = 0;
     int k = 0;
     for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
         k = wide_block(tab, nblk, tile, k);
@@ -464,27 +502,26 @@ k_wide_bwd_elem(long N, int T, int W, const __grid_constant__ TypeTab tt, const 
         const bool real = id.y >= 0;
         float dR[4] = {0.f, 0.f, 0.f, 0.f};
         float sc = 0.f;
+        float R[4] = {0.f, 0.f, 0.f, 0.f};
+        const float *g = gA;
         if (real) {
             const float4 rh = __ldg(&rows_rh[rbase + row]);
             sc = __ldg(&gscale[id.x]);
-            const float R[4] = {rh.x * sc, rh.y * sc, rh.z * sc, rh.w * sc};
-            const float *g = gA + (long)id.x * 4 * M2;
-            uint8_t *y2r = Y2 + (size_t)tile * ych * 2048 + r * 16;
-            uint8_t *t3r = T3 + (size_t)tile * (2 * ych) * 2048 + r * 16;
-            const int f0 = hf * (ych / 2), f1 = f0 + ych / 2;       // this thread's half of the column groups
-            uint4 ny = *reinterpret_cast<const uint4 *>(y2r + (size_t)f0 * 2048);
-            uint4 na = *reinterpret_cast<const uint4 *>(t3r + (size_t)f0 * 2048);
-            uint4 nb = *reinterpret_cast<const uint4 *>(t3r + (size_t)(f0 + ych) * 2048);
-            for (int f = f0; f < f1; ++f) {
+            R[0] = rh.x * sc; R[1] = rh.y * sc; R[2] = rh.z * sc; R[3] = rh.w * sc;
+            g = gA + (long)id.x * 4 * M2;
+        }
+        uint8_t *y2r = Y2 + (size_t)tile * ych * 2048 + r * 16;
+        uint8_t *t3r = T3 + (size_t)tile * (2 * ych) * 2048 + r * 16;
+        for (int sidx = 0; sidx < nstep; ++sidx, ++step) {
+            const int st = step % BE_STAGES;
+            const int f = sidx + hf * nstep;
+            tc::mbar_wait(&full[st], (step / BE_STAGES) & 1);
+            if (real) {
+                const uint8_t *src = bsm + st * BE_STAGE_BYTES + hf * 6144 + r * 16;
                 float y2[8], ta[8], tb[8], oa[8], ob[8], os[8];
-                unpack8(ny, y2);
-                unpack8(na, ta);
-                unpack8(nb, tb);
-                if (f + 1 < f1) {         // the three activation chunks of the next step, in flight under this step's arithmetic
-                    ny = *reinterpret_cast<const uint4 *>(y2r + (size_t)(f + 1) * 2048);
-                    na = *reinterpret_cast<const uint4 *>(t3r + (size_t)(f + 1) * 2048);
-                    nb = *reinterpret_cast<const uint4 *>(t3r + (size_t)(f + 1 + ych) * 2048);
-                }
+                unpack8(*reinterpret_cast<const uint4 *>(src), y2);
+                unpack8(*reinterpret_cast<const uint4 *>(src + 2048), ta);
+                unpack8(*reinterpret_cast<const uint4 *>(src + 4096), tb);
 #pragma unroll
                 for (int q = 0; q < 8; ++q) { oa[q] = 0.f; ob[q] = 0.f; }
 #pragma unroll
@@ -513,14 +550,16 @@ k_wide_bwd_elem(long N, int T, int W, const __grid_constant__ TypeTab tt, const 
                 *reinterpret_cast<uint4 *>(t3r + (size_t)f * 2048) = pack8(oa);
                 *reinterpret_cast<uint4 *>(t3r + (size_t)(f + ych) * 2048) = pack8(ob);
             }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[st]);
         }
         if (hf == 1) sdr[r] = make_float4(dR[0], dR[1], dR[2], dR[3]);
-        __syncthreads();
+        tc::bar_sync(1, 2 * WR);
         if (hf == 0 && real) {
             const float4 o = sdr[r];
             rows_g[rbase + row] = make_float4((dR[0] + o.x) * sc, (dR[1] + o.y) * sc, (dR[2] + o.z) * sc, (dR[3] + o.w) * sc);
         }
-        __syncthreads();
+        tc::bar_sync(1, 2 * WR);
     }
 }
 
@@ -631,7 +670,8 @@ cudaError_t launch_embed_bwd_wide(const dp_model *m, long N, const Grid3 &g, cha
     // the last fitting GEMM left gA itself in the gD buffer (fit_tc.cu MODE 6)
     const float *gA = (const float *)(ws + L.gD);
     k_wide_gscale<<<(unsigned)((N + 7) / 8), 256, 0, st>>>(N, 16 * W, gA, (float *)(ws + L.gscale));
-    k_wide_bwd_elem<<<m->num_sms * 4, 2 * WR, 0, st>>>(N, m->T, W, tt, p.tab, (const float4 *)(ws + L.rows_rh), p.rows_id, gA, p.gscale,
+    DP_SMEM_OPTIN(k_wide_bwd_elem, BE_STAGES * BE_STAGE_BYTES);
+    k_wide_bwd_elem<<<m->num_sms * 2, BE_THREADS, BE_STAGES * BE_STAGE_BYTES, st>>>(N, m->T, W, tt, p.tab, (const float4 *)(ws + L.rows_rh), p.rows_id, gA, p.gscale,
                                                  p.Y2, p.T3, p.rows_g);
     ok(cudaGetLastError());
     if (m->profile) cudaEventRecord(m->ev[6], st);      // ev[6] .. ev[7]: the two backward GEMMs
