@@ -328,97 +328,143 @@ __global__ void __launch_bounds__(W_THREADS, 1) k_wide_gemm(const __grid_constan
 }
 
 // S5: A_i[c][m] = (1 / Nm) sum_rows w R^[row][c] G[row][m],  G = (y2, y2) + t3.
-// One CTA per atom; warp = one group of 8 columns at a time, lane = row; the 32 partial sums (4 components x 8 columns)
-// of a warp are reduced by a transposing butterfly (31 shuffles) and added to the CTA's copy of A_i in shared memory:
-// no atomics, a fixed summation order, A_i written once.
-constexpr int WC_BATCH = 512;                   // rows staged per pass
+// One CTA per atom, and per batch of up to 192 of its rows: S3 = R^T t3 [4][4 W] and S2 = R^T y2 [4][2 W] are accumulated
+// separately (A_i[c][m] = S3[c][m] + S2[c][m mod 2 W]), so every activation is read from HBM once.  A group of 8 columns is
+// one product [8 x rows] . [rows x 8] on the tensor cores (mma.sync m16n8k16, fp32 accumulate): M = the four components of the
+// weighted row as fp16 hi parts (rows 0-3) and lo parts (rows 4-7), K = rows, N = the 8 columns; the B fragments come straight
+// from the stored [row][8 fp16] blocks through ldmatrix.trans.  Every warp owns every 8th column group and stages it itself:
+// bulk copies of the atom's rows of that group (contiguous inside a tile), three groups ahead, completion on its own mbarriers.
+// With scalar fp32 FMAs (32 per 16 bytes loaded) the kernel was issue-bound at 4.3 TB/s.  No atomics, fixed summation order.
+constexpr int WC_BATCH = 192;                   // rows per pass: 12 k-steps of 16
+constexpr int WC_DEPTH = 3;                     // column groups in flight per warp
+constexpr int WC_SLOT = WC_BATCH * 16;          // bytes of one staged column group
 __global__ void __launch_bounds__(256)
-k_wide_contract(long N, int T, int ncell, int W, int Nm, const __grid_constant__ TypeTab tt, const int4 *__restrict__ tab,
+k_wide_contract(long N, int T, int ncell, int W, int P, int Nm, const __grid_constant__ TypeTab tt, const int4 *__restrict__ tab,
                 const int *__restrict__ bin_start, const int *__restrict__ rowstart, const float4 *__restrict__ rows_rh,
                 const int2 *__restrict__ rows_id, const uint8_t *__restrict__ Y2, const uint8_t *__restrict__ T3,
                 float *__restrict__ Aout) {
-    extern __shared__ __align__(16) uint8_t csm[];
-    // S3 = R^T t3 [4][4 W] followed by S2 = R^T y2 [4][2 W]: G = (y2, y2) + t3, so A_i[c][m] = S3[c][m] + S2[c][m mod 2 W] and
-    // every activation is read from HBM once
-    float *sA = reinterpret_cast<float *>(csm);
-    float *sA2 = sA + 16 * W;
-    float4 *srw = reinterpret_cast<float4 *>(csm + 24 * W * 4);       // [WC_BATCH] weighted rows
-    const long i = blockIdx.x;
+    extern __shared__ __align__(128) uint8_t csm[];
+    __shared__ uint64_t cbar[8][WC_DEPTH];
+    uint8_t *slots = csm;                                                    // [8 warps][WC_DEPTH][WC_SLOT]
+    float4 *srw = reinterpret_cast<float4 *>(csm + 8 * WC_DEPTH * WC_SLOT);   // [WC_BATCH] weighted rows
+    // P CTAs per atom (W = 512: two, so that two CTAs fit an SM): part h takes the y2 chunks [h ych / P, (h + 1) ych / P) and the
+    // t3 chunks of the same columns f and of f + 2 W
+    const int nch = 4 * W / 8, ych = 2 * W / 8, ychp = ych / P, WP = 8 * ychp;      // WP: y2 columns of one part
+    float *sA = reinterpret_cast<float *>(srw + WC_BATCH);                   // S3 [2 (f, f + 2 W)][4][WP]
+    float *sA2 = sA + 8 * WP;                                                // S2 [4][WP]
+    const long i = blockIdx.x / P;
+    const int part = blockIdx.x % P;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    const int cg = lane >> 2, rs = lane & 3;              // lane = (one of 8 column groups, one of 4 row phases)
+    const int g8 = lane >> 2, t4 = lane & 3;
     int a = 0;
     for (int t = 1; t < T; ++t) a += i >= bin_start[t * ncell];
-    for (int k = tid; k < 24 * W; k += 256) sA[k] = 0.f;
-    const int nch = 4 * W / 8, ych = 2 * W / 8;
+    for (int k = tid; k < 12 * WP; k += 256) sA[k] = 0.f;
+    // staged rows beyond a batch's count keep older (finite) activations: they meet zero rows of R.  Start from zeros.
+    for (int k = tid; k < 8 * WC_DEPTH * WC_SLOT / 16; k += 256) reinterpret_cast<uint4 *>(slots)[k] = make_uint4(0u, 0u, 0u, 0u);
+    if (lane == 0)
+        for (int d = 0; d < WC_DEPTH; ++d) tc::mbar_init(&cbar[wid][d], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;");
+    const int ngroups = 3 * ychp;               // group q: q < 2 ychp: t3 chunk (lower then upper columns), else y2 chunk
+    uint32_t issued = 0, consumed = 0;          // per warp: column groups handed to / taken from the staging ring (all batches)
+    uint8_t *myslots = slots + wid * WC_DEPTH * WC_SLOT;
     for (int b = 0; b < T; ++b) {
         const int4 e = tab[a * T + b];
         const long rbase = N * (long)tt.off[b];
         const int r0 = rowstart[(long)b * (N + 1) + i], r1 = rowstart[(long)b * (N + 1) + i + 1];
         for (int rb = r0; rb < r1; rb += WC_BATCH) {
-            const int nb = min(WC_BATCH, r1 - rb);
+            const int nb = min(WC_BATCH, r1 - rb), nks = (nb + 15) / 16;
             __syncthreads();
-            for (int j = tid; j < nb; j += 256) {
-                float4 rh = __ldg(&rows_rh[rbase + rb + j]);
-                const int2 id = __ldg(&rows_id[rbase + rb + j]);
-                if (id.y < 0) { const float w = (float)(-id.y); rh.x *= w; rh.y *= w; rh.z *= w; rh.w *= w; }
+            for (int j = tid; j < WC_BATCH; j += 256) {
+                float4 rh = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (j < nb) {
+                    rh = __ldg(&rows_rh[rbase + rb + j]);
+                    const int2 id = __ldg(&rows_id[rbase + rb + j]);
+                    if (id.y < 0) { const float w = (float)(-id.y); rh.x *= w; rh.y *= w; rh.z *= w; rh.w *= w; }
+                }
                 srw[j] = rh;
             }
             __syncthreads();
-            for (int vc = 8 * wid + cg; vc < nch + ych; vc += 64) {      // groups of 8 chunks: all of t3 or all of y2 (warp-uniform)
-                const bool isy = vc >= nch;
-                const uint8_t *img = isy ? Y2 : T3;
-                const int cpt = isy ? ych : nch, ch = isy ? vc - nch : vc;
-                float v[32];
+            // A fragments of all k-steps: lane (g8, t4) holds rows 2 t4, 2 t4 + 1 (a0) and 2 t4 + 8, 2 t4 + 9 (a2) of the step, M row g8:
+            // component g8 & 3, hi part for g8 < 4, lo part otherwise
+            uint32_t afr[WC_BATCH / 16][2];
+            {
+                const float *sr = reinterpret_cast<const float *>(srw);
+                const int c = g8 & 3;
 #pragma unroll
-                for (int q = 0; q < 32; ++q) v[q] = 0.f;
-                for (int j = rs; j < nb; j += 32) {       // eight rows per trip: eight independent loads in flight
-                    uint4 u[8];
-                    float4 w[8];
-#pragma unroll
-                    for (int x = 0; x < 8; ++x) {
-                        const int jj = j + 4 * x;
-                        u[x] = make_uint4(0u, 0u, 0u, 0u); w[x] = make_float4(0.f, 0.f, 0.f, 0.f);
-                        if (jj < nb) {
-                            const int rel = rb + jj - e.y;
-                            u[x] = __ldg(reinterpret_cast<const uint4 *>(img + (((size_t)e.x + rel / WR) * cpt + ch) * 2048 + (rel % WR) * 16));
-                            w[x] = srw[jj];
-                        }
-                    }
-#pragma unroll
-                    for (int x = 0; x < 8; ++x) {
-                        float g[8];
-                        unpack8(u[x], g);
-#pragma unroll
-                        for (int q = 0; q < 8; ++q) {
-                            v[q] = fmaf(w[x].x, g[q], v[q]);
-                            v[8 + q] = fmaf(w[x].y, g[q], v[8 + q]);
-                            v[16 + q] = fmaf(w[x].z, g[q], v[16 + q]);
-                            v[24 + q] = fmaf(w[x].w, g[q], v[24 + q]);
-                        }
+                for (int ks = 0; ks < WC_BATCH / 16; ++ks) {
+                    const int rr = 16 * ks + 2 * t4;
+                    uint32_t h0, l0, h1, l1;
+                    tc::split_h2(sr[rr * 4 + c], sr[(rr + 1) * 4 + c], h0, l0);
+                    tc::split_h2(sr[(rr + 8) * 4 + c], sr[(rr + 9) * 4 + c], h1, l1);
+                    afr[ks][0] = g8 < 4 ? h0 : l0;
+                    afr[ks][1] = g8 < 4 ? h1 : l1;
+                }
+            }
+            // this warp's column groups of the batch: vc = wid, wid + 8, ...
+            const int rel0 = rb - e.y;
+            auto issue = [&](int vc) {
+                if (lane == 0) {
+                    const bool isy = vc >= 2 * ychp;
+                    const uint8_t *img = isy ? Y2 : T3;
+                    const int cpt = isy ? ych : nch;
+                    const int ch = isy ? part * ychp + (vc - 2 * ychp) : (vc < ychp ? part * ychp + vc : ych + part * ychp + (vc - ychp));
+                    uint64_t *bar = &cbar[wid][issued % WC_DEPTH];
+                    uint8_t *dst = myslots + (issued % WC_DEPTH) * WC_SLOT;
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    mbar_expect_tx(bar, (uint32_t)nb * 16u);
+                    for (int done = 0; done < nb;) {          // the rows are contiguous inside a tile: one copy per tile touched
+                        const int rel = rel0 + done, tl = rel / WR, rr = rel % WR;
+                        const int cnt = min(nb - done, WR - rr);
+                        bulk_g2s(tc::smem_u32(dst + done * 16), img + (((size_t)e.x + tl) * cpt + ch) * 2048 + rr * 16, (uint32_t)cnt * 16u, bar);
+                        done += cnt;
                     }
                 }
-                // transposing butterfly over the four row phases: afterwards lane rs holds component c = rs, 8 columns
+                ++issued;
+            };
+            const int nmine = (ngroups - wid + 7) / 8;
+            __syncwarp();
+            for (int q = 0; q < WC_DEPTH && q < nmine; ++q) issue(wid + 8 * q);
+            for (int q = 0; q < nmine; ++q) {
+                const int vc = wid + 8 * q;
+                const uint32_t sl = consumed % WC_DEPTH;
+                tc::mbar_wait(&cbar[wid][sl], (consumed / WC_DEPTH) & 1);
+                ++consumed;
+                const uint32_t sbase = tc::smem_u32(myslots + sl * WC_SLOT) + lane * 16;
+                float c0 = 0.f, c1 = 0.f, c2 = 0.f, c3 = 0.f;
 #pragma unroll
-                for (int o = 2; o >= 1; o >>= 1) {
-                    const bool up = (lane & o) != 0;
-#pragma unroll
-                    for (int q = 0; q < 8 * o; ++q) {
-                        const float send = up ? v[q] : v[q + 8 * o];
-                        const float keep = up ? v[q + 8 * o] : v[q];
-                        v[q] = keep + __shfl_xor_sync(0xffffffffu, send, o);
+                for (int kp = 0; kp < WC_BATCH / 32; ++kp) {
+                    if (2 * kp < nks) {
+                        uint32_t b0, b1, b2, b3;
+                        asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0, %1, %2, %3}, [%4];"
+                                     : "=r"(b0), "=r"(b1), "=r"(b2), "=r"(b3) : "r"(sbase + kp * 512));
+                        asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, {%0, %1, %2, %3};"
+                                     : "+f"(c0), "+f"(c1), "+f"(c2), "+f"(c3) : "r"(afr[2 * kp][0]), "r"(0u), "r"(afr[2 * kp][1]), "r"(0u), "r"(b0), "r"(b1));
+                        if (2 * kp + 1 < nks)
+                            asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, {%0, %1, %2, %3};"
+                                         : "+f"(c0), "+f"(c1), "+f"(c2), "+f"(c3) : "r"(afr[2 * kp + 1][0]), "r"(0u), "r"(afr[2 * kp + 1][1]), "r"(0u), "r"(b2), "r"(b3));
                     }
                 }
-                float *dst = (isy ? sA2 + rs * 2 * W : sA + rs * 4 * W) + 8 * ch;
-#pragma unroll
-                for (int q = 0; q < 8; ++q) dst[q] += v[q];
+                (void)c2; (void)c3;
+                __syncwarp();                                   // every lane has read the slot: it may be refilled
+                if (q + WC_DEPTH < nmine) issue(vc + 8 * WC_DEPTH);
+                // hi rows (g8 < 4) + lo rows (g8 >= 4): lanes 16 apart
+                c0 += __shfl_xor_sync(0xffffffffu, c0, 16);
+                c1 += __shfl_xor_sync(0xffffffffu, c1, 16);
+                if (g8 < 4) {
+                    // vc < ychp: S3 lower columns, < 2 ychp: S3 upper columns, else S2; each [4][WP]
+                    const int sec = vc >= 2 * ychp ? 2 : (vc >= ychp ? 1 : 0);
+                    float *dst = sA + sec * 4 * WP + g8 * WP + 8 * (vc - sec * ychp);
+                    dst[2 * t4] += c0;
+                    dst[2 * t4 + 1] += c1;
+                }
             }
         }
     }
     __syncthreads();
     const float inv_nm = 1.0f / (float)Nm;
-    for (int k = tid; k < 16 * W; k += 256) {
-        const int c = k / (4 * W), m = k % (4 * W);
-        Aout[i * 16L * W + k] = (sA[k] + sA2[c * 2 * W + m % (2 * W)]) * inv_nm;
+    for (int k = tid; k < 8 * WP; k += 256) {           // (upper / lower, component, column of the part)
+        const int u = k / (4 * WP), c = (k / WP) & 3, f = k % WP;
+        Aout[i * 16L * W + c * 4 * W + u * 2 * W + part * WP + f] = (sA[k] + sA2[c * WP + f]) * inv_nm;
     }
 }
 
@@ -652,9 +698,10 @@ cudaError_t launch_embed_fwd_wide(const dp_model *m, long N, const Grid3 &g, cha
     const WideArgs p = wide_args(m, N, ws, L);
     ok(wide_gemm<0>(m, p, W, 2 * W, p.T1, 0, st));
     ok(wide_gemm<1>(m, p, 2 * W, 4 * W, p.Y2, 1, st));
-    const int csm = 24 * W * 4 + WC_BATCH * 16;
-    DP_SMEM_OPTIN(k_wide_contract, 24 * 512 * 4 + WC_BATCH * 16);
-    k_wide_contract<<<(unsigned)N, 256, csm, st>>>(N, m->T, g.ncell, W, m->Nm, tt, tab, (const int *)(ws + L.bin_start),
+    const int P = W >= 512 ? 2 : 1;             // CTAs per atom: two CTAs (100 KB each) must fit an SM
+    const int csm = 8 * WC_DEPTH * WC_SLOT + WC_BATCH * 16 + 24 * W * 4 / P;
+    DP_SMEM_OPTIN(k_wide_contract, 8 * WC_DEPTH * WC_SLOT + WC_BATCH * 16 + 24 * 256 * 4);
+    k_wide_contract<<<(unsigned)(N * P), 256, csm, st>>>(N, m->T, g.ncell, W, P, m->Nm, tt, tab, (const int *)(ws + L.bin_start),
                                                    (const int *)(ws + L.rowstart), (const float4 *)(ws + L.rows_rh),
                                                    (const int2 *)(ws + L.rows_id), p.Y2, p.T3, (float *)(ws + L.A));
     ok(cudaGetLastError());
