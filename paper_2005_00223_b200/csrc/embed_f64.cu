@@ -23,13 +23,9 @@ __device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b)
         : "d"(a), "d"(b));
 }
 
-// tanh64.cuh: branch-free, 24 fp64-pipe operations, |error| <= 2.3e-16.  CALL = true keeps ONE copy of it in the kernel
-// (a call per value) instead of 49 inlined copies per tile: the backward kernel's unrolled body then shrinks from 7,700 to
-// 4,200 instructions and stops missing the instruction cache (measured at config 2: 6.9 -> 6.1 ms; on systems of a few
-// hundred atoms the calls cost more than the misses, so the launcher picks by size; the forward is always inlined).
-__device__ __noinline__ double dp_tanh_call(double x) { return dp_tanh64(x); }
-template <bool CALL>
-__device__ __forceinline__ double dp_tanh(double x) { return CALL ? dp_tanh_call(x) : dp_tanh64(x); }
+// tanh64.cuh: branch-free, 24 fp64-pipe operations, |error| <= 2.3e-16 (inlined: the lockstep tile loops below keep the
+// instruction cache fed; a called copy was faster only before them)
+__device__ __forceinline__ double dp_tanh(double x) { return dp_tanh64(x); }
 
 __device__ __forceinline__ double min_image(double t, double L, double halfL) {
     double s = t > halfL ? -1.0 : (t < -halfL ? 1.0 : 0.0);
@@ -68,14 +64,14 @@ __device__ __forceinline__ void env_row(const EnvParams &p, double dx, double dy
 //   y1[kc]  layer-1 output, slot (kc, r=lane%4)
 //   t2[p]   tanh of layer-2 pre-activation at position p = 2*nt2 + j2 ;  y2[p] = y1[p>>1] + t2[p]
 //   t3[q]   tanh of layer-3 pre-activation at position q = 2*nt3 + j3 ;  G[q]  = y2[q>>1] + t3[q]
-template <int W, bool CALL>
+template <int W>
 __device__ __forceinline__ void embed_forward_tile(const EmbedNetFrag<double, W> *__restrict__ net, int lane, double s,
                                                    double (&y1)[EmbW<W>::KC1], double (&t2)[2 * EmbW<W>::NT2], double (&t3)[2 * EmbW<W>::NT3]) {
     constexpr int M0 = EmbW<W>::M0, M1 = EmbW<W>::M1, M2E = EmbW<W>::M2E, KC1 = EmbW<W>::KC1, NT2 = EmbW<W>::NT2, NT3 = EmbW<W>::NT3, NT1 = EmbW<W>::NT1;
     (void)M0; (void)M1; (void)M2E; (void)KC1; (void)NT2; (void)NT3; (void)NT1;
     const int r = lane & 3;
 #pragma unroll
-    for (int kc = 0; kc < KC1; ++kc) y1[kc] = dp_tanh<CALL>(fma(s, net->w1[4 * kc + r], net->b1[4 * kc + r]));
+    for (int kc = 0; kc < KC1; ++kc) y1[kc] = dp_tanh(fma(s, net->w1[4 * kc + r], net->b1[4 * kc + r]));
     {
         double acc[NT2][2];
 #pragma unroll
@@ -90,8 +86,8 @@ __device__ __forceinline__ void embed_forward_tile(const EmbedNetFrag<double, W>
         }
 #pragma unroll
         for (int nt = 0; nt < NT2; ++nt) {
-            t2[2 * nt] = dp_tanh<CALL>(acc[nt][0]);
-            t2[2 * nt + 1] = dp_tanh<CALL>(acc[nt][1]);
+            t2[2 * nt] = dp_tanh(acc[nt][0]);
+            t2[2 * nt + 1] = dp_tanh(acc[nt][1]);
         }
     }
 #pragma unroll
@@ -115,8 +111,8 @@ __device__ __forceinline__ void embed_forward_tile(const EmbedNetFrag<double, W>
 #pragma unroll
         for (int t = 0; t < NT3 / 2; ++t) {
             const int nt3 = half * (NT3 / 2) + t;
-            t3[2 * nt3] = dp_tanh<CALL>(acc[t][0]);
-            t3[2 * nt3 + 1] = dp_tanh<CALL>(acc[t][1]);
+            t3[2 * nt3] = dp_tanh(acc[t][0]);
+            t3[2 * nt3 + 1] = dp_tanh(acc[t][1]);
         }
     }
 }
@@ -179,7 +175,7 @@ k_embed_fwd_f64(int T, int ncell, int Nm, int CH, const __grid_constant__ TypeTa
     double *rbuf = smem + FWD_NET_DOUBLES + wid * WARP_BUF_DOUBLES;
     double *sbuf = rbuf + ROWCHUNK * 4;
     const int *sel = tt.sel;
-    const int gw = blockIdx.x * DP_WARPS_PER_CTA + wid, NW = gridDim.x * DP_WARPS_PER_CTA;
+    const int NW = gridDim.x * DP_WARPS_PER_CTA;
     const int r = lane & 3, q4 = lane >> 2;
     const double inv_nm = 1.0 / (double)Nm;
     const double hx = 0.5 * ep.L[0], hy = 0.5 * ep.L[1], hz = 0.5 * ep.L[2];
@@ -199,20 +195,31 @@ k_embed_fwd_f64(int T, int ncell, int Nm, int CH, const __grid_constant__ TypeTa
             // work item = (atom, row chunk).  CH == ROWCHUNK (large systems): one item per atom walks all its chunks and writes
             // A_i itself.  CH < ROWCHUNK (systems with fewer atoms than warps): S items per atom, one chunk of CH rows each, so
             // that every warp has work; their partial sums meet in A_i (zeroed by the launcher) through fp64 atomics.
+            // The items are walked in LOCKSTEP: the eight warps of a CTA meet at a barrier before every 8-row tile, so that the
+            // unrolled tile body (90 KB of code) streams through the instruction cache once per tile for all of them instead of
+            // once per warp (ncu: 2.2 no_instruction stalls per issue without it).  All loop bounds are CTA-uniform: sel[b] + 1
+            // bounds the rows.
+            // (Split items, S > 1, run free: measured slower in lockstep, their empty items would idle at the barriers.)
             const int S = CH == ROWCHUNK ? 1 : (sel[b] + CH) / CH;
-            for (long it = gw; it < (long)(ts1 - ts0) * S; it += NW) {
-                const int i = ts0 + (int)(it / S), part = (int)(it % S);
-                const int nr = nreal[i * T + b];
+            const bool LS = S == 1;
+            const long nitems = (long)(ts1 - ts0) * S;
+            for (long itb = LS ? (long)blockIdx.x * DP_WARPS_PER_CTA : (long)blockIdx.x * DP_WARPS_PER_CTA + wid; itb < nitems; itb += NW) {
+                const long it = LS ? itb + wid : itb;
+                const bool active = it < nitems;
+                const int i = active ? ts0 + (int)(it / S) : ts0, part = active ? (int)(it % S) : 0;
+                const int nr = active ? nreal[i * T + b] : 0;
                 const int npad = sel[b] - nr;
-                const int rows = nr + (npad > 0 ? 1 : 0);
-                if (part * CH >= rows) continue;
+                const int rows = active ? nr + (npad > 0 ? 1 : 0) : 0;
+                if (!LS && part * CH >= rows) continue;
+                const int rows_u = LS ? sel[b] + 1 : rows;          // bound of the chunk loop (CTA-uniform in lockstep)
                 const double xi = xs[3 * (long)i], yi = xs[3 * (long)i + 1], zi = xs[3 * (long)i + 2];
                 double accA[NT3][2];
 #pragma unroll
                 for (int t = 0; t < NT3; ++t) accA[t][0] = accA[t][1] = 0.0;
-                for (int r0 = part * CH; r0 < rows; r0 += S * CH) {
-                    const int nrow_c = min(CH, rows - r0);
+                for (int r0 = part * CH; r0 < rows_u; r0 += S * CH) {
+                    const int nrow_c = max(0, min(CH, rows - r0));
                     const int ntile = (nrow_c + 7) >> 3;
+                    const int ntile_u = LS ? (min(CH, rows_u - r0) + 7) >> 3 : ntile;
                     // pre-pass: weighted R^ rows and s^ of this chunk
                     for (int rr = lane; rr < ntile * 8; rr += 32) {
                         const int row = r0 + rr;
@@ -235,9 +242,11 @@ k_embed_fwd_f64(int T, int ncell, int Nm, int CH, const __grid_constant__ TypeTa
                         for (int c = 1; c < 4; ++c) rbuf[rr * 4 + c] = wgt * ((Rt[c] - av[c]) / sd[c]);
                     }
                     __syncwarp();
-                    for (int t = 0; t < ntile; ++t) {
+                    for (int t = 0; t < ntile_u; ++t) {
+                        if (LS) __syncthreads();
+                        if (t >= ntile) continue;
                         double y1[KC1], t2[2 * NT2], t3[2 * NT3];
-                        embed_forward_tile<W, false>(net, lane, sbuf[t * 8 + q4], y1, t2, t3);
+                        embed_forward_tile<W>(net, lane, sbuf[t * 8 + q4], y1, t2, t3);
                         // G in C-fragment layout -> B fragments of the contraction A^T[c][m] += R^[k][c] G[k][m]
 #pragma unroll
                         for (int g = 0; g < 2; ++g) {
@@ -257,7 +266,7 @@ k_embed_fwd_f64(int T, int ncell, int Nm, int CH, const __grid_constant__ TypeTa
                     __syncwarp();
                 }
                 // accA: (c = lane/4, feature of (nt3, r, j)); lanes with c >= 4 hold zeros
-                if (q4 < 4) {
+                if (q4 < 4 && active) {
                     double *Ai = Aout + ((long)i * 4 + q4) * M2E;
 #pragma unroll
                     for (int nt3 = 0; nt3 < NT3; ++nt3) {
@@ -283,7 +292,7 @@ k_embed_fwd_f64(int T, int ncell, int Nm, int CH, const __grid_constant__ TypeTa
 // gAf: per atom 42 fragments of 32 doubles, already scaled by 1/Nm (written by the fitting backward):
 //   [0..14)  : dG MMA   B fragment of tile nt3: lane -> gA[c = lane%4][feature3(nt3, (lane/4)/2, (lane/4)%2)]
 //   [14..42) : dR^ MMA  B fragment of chunk kc = 2*nt3 + j3: lane -> (lane/4 < 4) ? gA[c = lane/4][feature3(nt3, lane%4, j3)] : 0
-template <int W, bool CALL>
+template <int W>
 __global__ void __launch_bounds__(DP_WARPS_PER_CTA * 32, 1)
 k_embed_bwd_f64(int T, int ncell, int Nm, int CH, const __grid_constant__ TypeTab tt, EnvParams ep, const EmbedNetFrag<double, W> *__restrict__ nets,
                 const double *__restrict__ avg, const double *__restrict__ stdv, const int *__restrict__ bin_start,
@@ -302,7 +311,7 @@ k_embed_bwd_f64(int T, int ncell, int Nm, int CH, const __grid_constant__ TypeTa
     double *rbuf = smem + BWD_NET_DOUBLES + wid * WARP_BUF_DOUBLES;
     double *sbuf = rbuf + ROWCHUNK * 4;
     const int *sel = tt.sel;
-    const int gw = blockIdx.x * DP_WARPS_PER_CTA + wid, NW = gridDim.x * DP_WARPS_PER_CTA;
+    const int NW = gridDim.x * DP_WARPS_PER_CTA;
     const int r = lane & 3, q4 = lane >> 2;
     const double hx = 0.5 * ep.L[0], hy = 0.5 * ep.L[1], hz = 0.5 * ep.L[2];
     unsigned long long my_rows = 0;
@@ -321,17 +330,23 @@ k_embed_bwd_f64(int T, int ncell, int Nm, int CH, const __grid_constant__ TypeTa
             __syncthreads();
             stage_net(smem, reinterpret_cast<const double *>(nets + (a * T + b)), BWD_NET_DOUBLES, &stage_bar, stage_phase);
             __syncthreads();
-            const int S = CH == ROWCHUNK ? 1 : (sel[b] + CH) / CH;       // work items per atom (see the forward kernel)
-            for (long it = gw; it < (long)(ts1 - ts0) * S; it += NW) {
-                const int i = ts0 + (int)(it / S), part = (int)(it % S);
-                const int nr = nreal[i * T + b];
-                if (part * CH >= nr) continue;
+            const int S = CH == ROWCHUNK ? 1 : (sel[b] + CH) / CH;       // work items per atom; lockstep when S == 1 (see the forward kernel)
+            const bool LS = S == 1;
+            const long nitems = (long)(ts1 - ts0) * S;
+            for (long itb = LS ? (long)blockIdx.x * DP_WARPS_PER_CTA : (long)blockIdx.x * DP_WARPS_PER_CTA + wid; itb < nitems; itb += NW) {
+                const long it = LS ? itb + wid : itb;
+                const bool active = it < nitems;
+                const int i = active ? ts0 + (int)(it / S) : ts0, part = active ? (int)(it % S) : 0;
+                const int nr = active ? nreal[i * T + b] : 0;
+                if (!LS && part * CH >= nr) continue;
+                const int rows_u = LS ? sel[b] : nr;
                 const double xi = xs[3 * (long)i], yi = xs[3 * (long)i + 1], zi = xs[3 * (long)i + 2];
                 const double *gf = gAf + (long)i * (3 * NT3 * 32);
                 double fi[3] = {0.0, 0.0, 0.0};
-                for (int r0 = part * CH; r0 < nr; r0 += S * CH) {
-                    const int nrow_c = min(CH, nr - r0);
+                for (int r0 = part * CH; r0 < rows_u; r0 += S * CH) {
+                    const int nrow_c = max(0, min(CH, nr - r0));
                     const int ntile = (nrow_c + 7) >> 3;
+                    const int ntile_u = LS ? (min(CH, rows_u - r0) + 7) >> 3 : ntile;
                     for (int rr = lane; rr < ntile * 8; rr += 32) {
                         const int row = r0 + rr;
                         double Rt[4] = {0.0, 0.0, 0.0, 0.0};
@@ -347,9 +362,11 @@ k_embed_bwd_f64(int T, int ncell, int Nm, int CH, const __grid_constant__ TypeTa
                         sbuf[rr] = rbuf[rr * 4];
                     }
                     __syncwarp();
-                    for (int t = 0; t < ntile; ++t) {
+                    for (int t = 0; t < ntile_u; ++t) {
+                        if (LS) __syncthreads();
+                        if (t >= ntile) continue;
                         double y1[KC1], t2[2 * NT2], t3[2 * NT3];
-                        embed_forward_tile<W, CALL>(net, lane, sbuf[t * 8 + q4], y1, t2, t3);
+                        embed_forward_tile<W>(net, lane, sbuf[t * 8 + q4], y1, t2, t3);
                         const double rfrag = rbuf[(t * 8 + q4) * 4 + r];
                         // dR^[row][c] = sum_m gA[c][m] G[row][m]      (C frag: c = 2r + {0,1}, valid for r < 2)
                         double dR0 = 0.0, dR1 = 0.0;
@@ -490,11 +507,11 @@ static cudaError_t launch_fwd_w(const dp_model *m, long N, const Grid3 &g, char 
     return cudaGetLastError();
 }
 
-template <int W, bool CALL>
+template <int W>
 static cudaError_t launch_bwd_w(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    DP_SMEM_OPTIN((k_embed_bwd_f64<W, CALL>), smem_bwd<W>());
+    DP_SMEM_OPTIN(k_embed_bwd_f64<W>, smem_bwd<W>());
     const TypeTab tt = make_typetab(m);
-    k_embed_bwd_f64<W, CALL><<<embed_grid(m, N), DP_WARPS_PER_CTA * 32, smem_bwd<W>(), st>>>(
+    k_embed_bwd_f64<W><<<embed_grid(m, N), DP_WARPS_PER_CTA * 32, smem_bwd<W>(), st>>>(
         m->T, g.ncell, m->Nm, embed_chunk(m, N), tt, make_env(m, g), (const EmbedNetFrag<double, W> *)m->embed_frag_dev, m->avg_dev,
         m->std_dev, (int *)(ws + L.bin_start), (double *)(ws + L.xs), (int *)(ws + L.nlist), (int *)(ws + L.nreal),
         (double *)(ws + L.gAf), (double *)(ws + L.fsorted), (double *)(ws + L.virial),
@@ -507,8 +524,5 @@ cudaError_t launch_embed_fwd_f64(const dp_model *m, long N, const Grid3 &g, char
 }
 
 cudaError_t launch_embed_bwd_f64(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    // tanh by call (one copy in the instruction cache) once every warp walks many 8-row tiles, inlined below that
-    const bool call = N * (long)m->Nm >= 1L << 20;
-    if (m->m0 == 32) return call ? launch_bwd_w<32, true>(m, N, g, ws, L, st) : launch_bwd_w<32, false>(m, N, g, ws, L, st);
-    return call ? launch_bwd_w<25, true>(m, N, g, ws, L, st) : launch_bwd_w<25, false>(m, N, g, ws, L, st);
+    return m->m0 == 32 ? launch_bwd_w<32>(m, N, g, ws, L, st) : launch_bwd_w<25>(m, N, g, ws, L, st);
 }
