@@ -238,19 +238,19 @@ __global__ void __launch_bounds__(128) k_gA(long N, double inv_nm, const double 
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const long i = blockIdx.x * 4L + wid;
     if (i >= N) return;
-    double *sA = smg + wid * (4 * M2E + M2E * 16 + 4 * M2E);
+    double *sA = smg + wid * (4 * M2E + M2E * 17 + 4 * M2E);
     double *sG = sA + 4 * M2E;
-    double *sO = sG + M2E * 16;
+    double *sO = sG + M2E * 17;      // rows of gD padded to 17: lanes walk consecutive rows m (stride 16 was a 16-way bank conflict)
     for (int k = lane; k < 4 * M2E; k += 32) sA[k] = Amat[i * 4 * M2E + k];
-    for (int k = lane; k < M2E * 16; k += 32) sG[k] = gD[i * (M2E * 16) + k];
+    for (int k = lane; k < M2E * 16; k += 32) sG[(k >> 4) * 17 + (k & 15)] = gD[i * (M2E * 16) + k];
     __syncwarp();
     for (int idx = lane; idx < 4 * M2E; idx += 32) {
         const int c = idx / M2E, m = idx % M2E;
         double acc = 0.0;
 #pragma unroll
-        for (int ax = 0; ax < 16; ++ax) acc += sG[m * 16 + ax] * sA[c * M2E + ax];
+        for (int ax = 0; ax < 16; ++ax) acc += sG[m * 17 + ax] * sA[c * M2E + ax];
         if (m < 16)
-            for (int mp = 0; mp < M2E; ++mp) acc += sG[mp * 16 + m] * sA[c * M2E + mp];
+            for (int mp = 0; mp < M2E; ++mp) acc += sG[mp * 17 + m] * sA[c * M2E + mp];
         sO[idx] = acc * inv_nm;
     }
     __syncwarp();
@@ -320,7 +320,7 @@ static cudaError_t launch_fit_w(const dp_model *m, long N, const Grid3 &g, char 
     p.A = gz1; p.N = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.out0 = D; p.ldo = ND;
     k_fit_gemm<5><<<dim3(gx, (ND + BN - 1) / BN, T), 256, 0, st>>>(p);
     // gD, A -> gA fragments for the embedding backward
-    const int smem = 4 * (4 * M2E + M2E * 16 + 4 * M2E) * 8;
+    const int smem = 4 * (4 * M2E + M2E * 17 + 4 * M2E) * 8;
     DP_SMEM_OPTIN(k_gA<W>, smem);
     k_gA<W><<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, 1.0 / (double)m->Nm, Amat, D, (double *)(ws + L.gAf));
     return cudaGetLastError();

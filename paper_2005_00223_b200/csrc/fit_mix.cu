@@ -229,20 +229,20 @@ __global__ void __launch_bounds__(128) k_gA_f(long N, const float *__restrict__ 
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const long i = blockIdx.x * 4L + wid;
     if (i >= N) return;
-    float *sA = smg + wid * (4 * M2E + M2E * 16 + 4 * M2E);
+    float *sA = smg + wid * (4 * M2E + M2E * 17 + 4 * M2E);
     float *sG = sA + 4 * M2E;
-    float *sO = sG + M2E * 16;
+    float *sO = sG + M2E * 17;      // rows of gD padded to 17: lanes walk consecutive rows m (stride 16 was a 16-way bank conflict)
     for (int k = lane; k < 4 * M2E; k += 32) sA[k] = Amat[i * 4 * M2E + k];
-    for (int k = lane; k < M2E * 16; k += 32) sG[k] = gD[i * (M2E * 16) + k];
+    for (int k = lane; k < M2E * 16; k += 32) sG[(k >> 4) * 17 + (k & 15)] = gD[i * (M2E * 16) + k];
     __syncwarp();
     float mx = 0.f;
     for (int idx = lane; idx < 4 * M2E; idx += 32) {
         const int c = idx / M2E, m = idx % M2E;
         float acc = 0.f;
 #pragma unroll
-        for (int ax = 0; ax < 16; ++ax) acc = fmaf(sG[m * 16 + ax], sA[c * M2E + ax], acc);
+        for (int ax = 0; ax < 16; ++ax) acc = fmaf(sG[m * 17 + ax], sA[c * M2E + ax], acc);
         if (m < 16)
-            for (int mp = 0; mp < M2E; ++mp) acc = fmaf(sG[mp * 16 + m], sA[c * M2E + mp], acc);
+            for (int mp = 0; mp < M2E; ++mp) acc = fmaf(sG[mp * 17 + m], sA[c * M2E + mp], acc);
         sO[idx] = acc;
         mx = fmaxf(mx, fabsf(acc));
     }
@@ -324,7 +324,7 @@ static cudaError_t launch_fit_mix_w(const dp_model *m, long N, const Grid3 &g, c
     ok(launch_gemm<4>(p, g240, st));
     p.A = gz1; p.N = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.out0 = D; p.ldo = ND;
     ok(launch_gemm<5>(p, g1600, st));
-    const int smem = 4 * (4 * M2E + M2E * 16 + 4 * M2E) * 4;
+    const int smem = 4 * (4 * M2E + M2E * 17 + 4 * M2E) * 4;
     DP_SMEM_OPTIN((k_gA_f<2, W>), smem);
     k_gA_f<2, W><<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, Amat, D, (uint32_t *)(ws + L.gAf), (float *)(ws + L.gscale));
     ok(cudaGetLastError());
