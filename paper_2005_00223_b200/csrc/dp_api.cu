@@ -536,6 +536,12 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
             fit_tc_build_type(ND, &V1[(size_t)a * ND * F], &V2[(size_t)a * F * F], &V3[(size_t)a * F * F], &img[(size_t)a * fit_tc_type_elems(ND)]);
         ok(upload(img, &m->fit_tc_img_dev));
     }
+    // MIX-32: the two large fitting products run on the tcgen05 kernels with hi + lo weight images (fit_tc.cu)
+    if (prec == DP_MIX32) {
+        std::vector<__half> img((size_t)T * fit_tc32_type_elems(ND));
+        for (int a = 0; a < T; ++a) fit_tc32_build_type(ND, &V1[(size_t)a * ND * F], &img[(size_t)a * fit_tc32_type_elems(ND)]);
+        ok(upload(img, &m->fit_tc_img_dev));
+    }
     std::vector<double> avg(w->avg, w->avg + 4 * T), sd(w->std, w->std + 4 * T), eb(w->ebias, w->ebias + T);
     ok(upload(avg, (void **)&m->avg_dev)); ok(upload(sd, (void **)&m->std_dev)); ok(upload(eb, (void **)&m->ebias_dev));
     if (e != cudaSuccess) { dp_destroy(m); return DP_ECUDA; }
@@ -571,7 +577,7 @@ int dp_launches_per_compute(const dp_model *m) {
         n += 2;                                      // environment rows + tcgen05 forward
         if (m->wide) n += 4 + 3 + 6;                 // tile table, layer 1, two GEMMs, contraction; fitting (3); scale, head, two GEMMs, force + virial, fp32 shares
         else if (m->prec == DP_MIX16) n += 3 + 6;    // first layer, fused 240 x 240 chain, last product; gA fold, tile classes, backward (two launches), force + virial, fp32 shares
-        else n += 9 + 1;                             // descriptor, 6 GEMMs, energy, gA fragments; backward (with S8, S9)
+        else n += 8 + 1;                             // first layer (tcgen05), 4 GEMMs, energy, last product (tcgen05), gA fragments; backward (with S8, S9)
     }
     return n + 1;                                    // finalize
 }

@@ -217,6 +217,10 @@ cudaError_t launch_embed_bwd_wide(const dp_model *m, long N, const Grid3 &g, cha
 size_t wide_net_img_elems(int W);
 void wide_build_net(int W, const double *net, float *vec, struct __half *img);
 long wide_tiles_cap(const dp_model *m, long N);
+size_t fit_tc32_type_elems(int nd);
+void fit_tc32_build_type(int nd, const double *V1, struct __half *out);
+cudaError_t launch_fit_tc32_first(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+cudaError_t launch_fit_tc32_last(const dp_model *m, long N, const float *gz1, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 size_t fit_tc_type_elems(int nd);
 void fit_tc_build_type(int nd, const double *V1, const double *V2, const double *V3, struct __half *out);
 cudaError_t launch_env_rows(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);

@@ -1,4 +1,6 @@
-// S5 (descriptor) + S6 (fitting net forward and backward) in MIX-32 (MIX-16 runs fit_tc.cu).
+// S6 (fitting net forward and backward) in MIX-32 (MIX-16 runs fit_tc.cu): the four 240 x 240 products, the
+// energy and the gA fragments; the two large products (first layer with the descriptor S5 formed in its operand producer, and
+// the last backward product) run on the tcgen05 kernels of fit_tc.cu with hi + lo weight images.
 // GEMMs batched over the atoms of one centre type on fp16 tensor-core MMAs (m16n8k16) with fp32 accumulation; every
 // operand is split hi + lo (NS = 3: hi hi + hi lo + lo hi), i.e. single-precision products on the tensor pipe, exact
 // tanhf, activations stored in fp32 ("all the arithmetic operations ... performed in single precision").
@@ -180,23 +182,6 @@ __global__ void __launch_bounds__(256) k_fitm_gemm(FitArgsF p) {
         }
 }
 
-template <int W>
-__global__ void __launch_bounds__(256) k_descr_f(long N, const float *__restrict__ Amat, float *__restrict__ D) {
-    constexpr int M2E = HW<W>::M2E;
-    __shared__ float sA[8][4 * M2E];
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const long i = blockIdx.x * 8L + wid;
-    if (i >= N) return;
-    for (int k = lane; k < 4 * M2E; k += 32) sA[wid][k] = Amat[i * 4 * M2E + k];
-    __syncwarp();
-    for (int idx = lane; idx < M2E * 16; idx += 32) {
-        const int m = idx >> 4, ax = idx & 15;
-        float acc = 0.f;
-#pragma unroll
-        for (int c = 0; c < 4; ++c) acc = fmaf(sA[wid][c * M2E + m], sA[wid][c * M2E + ax], acc);
-        D[i * (M2E * 16) + idx] = acc;
-    }
-}
 
 __device__ __forceinline__ int type_of_sorted(int i, int T, int ncell, const int *bin_start) {
     int a = 0;
@@ -220,38 +205,29 @@ __global__ void __launch_bounds__(256) k_energy_f(long N, int T, int ncell, cons
     if (lane == 0) eatom[i] = (double)(acc + c4[a]) + ebias[a];
 }
 
-// gA (fp32) -> scaled fp16 MMA fragments for the embedding backward (layout in embed_mix.cu)
+
+// gA (fp32 [N][4][m2], written by the epilogue of the tcgen05 last product, fit_tc.cu) -> scaled fp16 MMA fragments
+// for the embedding backward (layout in embed_mix.cu)
 template <int NSW, int W>
-__global__ void __launch_bounds__(128) k_gA_f(long N, const float *__restrict__ Amat, const float *__restrict__ gD,
-                                              uint32_t *__restrict__ gAf, float *__restrict__ gscale) {
+__global__ void __launch_bounds__(128) k_gA_frag(long N, const float *__restrict__ gA, uint32_t *__restrict__ gAf,
+                                                 float *__restrict__ gscale) {
     constexpr int M2E = HW<W>::M2E, HNT3 = HW<W>::HNT3, GP = 2 * HNT3;
-    extern __shared__ float smg[];
+    __shared__ float sO_all[4][4 * M2E];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const long i = blockIdx.x * 4L + wid;
     if (i >= N) return;
-    float *sA = smg + wid * (4 * M2E + M2E * 17 + 4 * M2E);
-    float *sG = sA + 4 * M2E;
-    float *sO = sG + M2E * 17;      // rows of gD padded to 17: lanes walk consecutive rows m (stride 16 was a 16-way bank conflict)
-    for (int k = lane; k < 4 * M2E; k += 32) sA[k] = Amat[i * 4 * M2E + k];
-    for (int k = lane; k < M2E * 16; k += 32) sG[(k >> 4) * 17 + (k & 15)] = gD[i * (M2E * 16) + k];
-    __syncwarp();
+    float *sO = sO_all[wid];
     float mx = 0.f;
-    for (int idx = lane; idx < 4 * M2E; idx += 32) {
-        const int c = idx / M2E, m = idx % M2E;
-        float acc = 0.f;
-#pragma unroll
-        for (int ax = 0; ax < 16; ++ax) acc = fmaf(sG[m * 17 + ax], sA[c * M2E + ax], acc);
-        if (m < 16)
-            for (int mp = 0; mp < M2E; ++mp) acc = fmaf(sG[mp * 17 + m], sA[c * M2E + mp], acc);
-        sO[idx] = acc;
-        mx = fmaxf(mx, fabsf(acc));
+    for (int k = lane; k < 4 * M2E; k += 32) {
+        const float v = gA[i * 4 * M2E + k];
+        sO[k] = v;
+        mx = fmaxf(mx, fabsf(v));
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-    // power-of-two scale bringing max|gA| into [0.5, 1)
     int ex = 0;
     if (mx > 0.f) frexpf(mx, &ex);
-    const float sc = ldexpf(1.f, -ex);
+    const float sc = ldexpf(1.f, -ex);          // power-of-two scale bringing max|gA| into [0.5, 1)
     if (lane == 0) gscale[i] = sc;
     __syncwarp();
     uint32_t *out = gAf + i * (2 * GP * 32);
@@ -288,31 +264,28 @@ cudaError_t launch_gemm(const FitArgsF &p, dim3 grid, cudaStream_t st) {
 
 template <int W>
 static cudaError_t launch_fit_mix_w(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    constexpr int M2E = HW<W>::M2E;
-    const int F = 240, ND = M2E * 16;
+    const int F = 240;
     const int T = m->T;
-    float *Amat = (float *)(ws + L.A);
     float *D = (float *)(ws + L.gD);
     float *act = (float *)(ws + L.fit_act);
     const size_t S = (size_t)N * F;
     float *h1 = act, *t2 = act + S, *h2 = act + 2 * S, *gz3 = act + 3 * S, *h3 = act + 4 * S, *g2 = act + 5 * S,
           *gz2 = act + 6 * S, *gz1 = h2;
     const int *bin_start = (const int *)(ws + L.bin_start);
-    const float *V1 = (const float *)m->fitV1_dev, *V2 = (const float *)m->fitV2_dev, *V3 = (const float *)m->fitV3_dev;
-    const float *c1 = (const float *)m->fitc1_dev, *c2 = (const float *)m->fitc2_dev, *c3 = (const float *)m->fitc3_dev;
+    const float *V2 = (const float *)m->fitV2_dev, *V3 = (const float *)m->fitV3_dev;
+    const float *c2 = (const float *)m->fitc2_dev, *c3 = (const float *)m->fitc3_dev;
     const float *v4 = (const float *)m->fitv4_dev, *c4 = (const float *)m->fitc4_dev;
     const unsigned gy = (unsigned)((N + BM - 1) / BM);
     const unsigned nb8 = (unsigned)((N + 7) / 8);
     cudaError_t e = cudaSuccess;
     auto ok = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
 
-    k_descr_f<W><<<nb8, 256, 0, st>>>(N, Amat, D);
+    // first layer (K = 16 m2) on the tcgen05 kernel with hi + lo weights: h1 = tanh(D V1 + c1), D formed in its operand producer
+    ok(launch_fit_tc32_first(m, N, g, ws, L, st));
     FitArgsF p{};
     p.ncell = g.ncell; p.bin_start = bin_start; p.v4 = v4; p.v4_type_stride = F; p.bias_type_stride = F;
-    p.K = ND; p.N = F; p.A = D; p.lda = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.ldb = F; p.bias = c1;
-    p.out0 = h1; p.ldo = F;
-    const dim3 g240(F / BN, gy, T), g1600((ND + BN - 1) / BN, gy, T);
-    ok(launch_gemm<0>(p, g240, st));
+    p.N = F; p.ldb = F; p.ldo = F;
+    const dim3 g240(F / BN, gy, T);
     p.K = F; p.A = h1; p.lda = F; p.B = V2; p.b_type_stride = (long)F * F; p.bias = c2; p.aux0 = h1; p.out0 = t2; p.out1 = h2;
     ok(launch_gemm<1>(p, g240, st));
     p.A = h2; p.B = V3; p.bias = c3; p.aux0 = h2; p.out0 = gz3; p.out1 = h3;
@@ -322,11 +295,9 @@ static cudaError_t launch_fit_mix_w(const dp_model *m, long N, const Grid3 &g, c
     ok(launch_gemm<3>(p, g240, st));
     p.A = gz2; p.B = V2; p.aux0 = g2; p.aux1 = h1; p.out0 = gz1; p.out1 = nullptr;
     ok(launch_gemm<4>(p, g240, st));
-    p.A = gz1; p.N = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.out0 = D; p.ldo = ND;
-    ok(launch_gemm<5>(p, g1600, st));
-    const int smem = 4 * (4 * M2E + M2E * 17 + 4 * M2E) * 4;
-    DP_SMEM_OPTIN((k_gA_f<2, W>), smem);
-    k_gA_f<2, W><<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, Amat, D, (uint32_t *)(ws + L.gAf), (float *)(ws + L.gscale));
+    // last product (N = 16 m2) on the tcgen05 kernel: gD is consumed in its epilogue, gA [N][4][m2] lands in the gD buffer
+    ok(launch_fit_tc32_last(m, N, gz1, g, ws, L, st));
+    k_gA_frag<2, W><<<(unsigned)((N + 3) / 4), 128, 0, st>>>(N, D, (uint32_t *)(ws + L.gAf), (float *)(ws + L.gscale));
     ok(cudaGetLastError());
     return e;
 }

@@ -31,7 +31,9 @@ __host__ __device__ constexpr int nprod(int mode) { return mode == 6 ? 32 : 256;
 __host__ __device__ constexpr int nepi(int mode) { return mode == 6 ? 512 : 256; }
 __host__ __device__ constexpr int nthreads(int mode) { return 64 + nprod(mode) + nepi(mode); }
 
-template <int KTOT, int NTOT>
+// WS (MIX-32: weights as hi + lo fp16 parts, "single precision"): a B stage holds the hi image followed by the lo
+// image and every k-step issues three products (A hi B hi, A lo B hi, A hi B lo; lo lo is below fp32 rounding)
+template <int KTOT, int NTOT, bool WS = false>
 struct Cfg {
     static constexpr bool RESIDENT = KTOT == 240;            // the A tile stays in shared memory for all N tiles
     // K chunk.  K = 1600 (the descriptor producer): 64 = 4 values of m, so that A_i[c][4 kc .. 4 kc + 3] is one aligned float4
@@ -48,8 +50,9 @@ struct Cfg {
     static constexpr int NTILES = NTOT / BN;
     static constexpr int NKC = KTOT / KCH;
     static constexpr int NA = RESIDENT ? NKC : 3;            // A buffers
-    static constexpr int B_STAGE = KCH * BN * 2;
-    static constexpr int NSTAGE = GA_N ? 4 : (DESCR_K ? 3 : 2);   // B pipeline depth (short stages need more copies in flight)
+    static constexpr int B_PART = KCH * BN * 2;                       // one weight image (hi or lo) of a stage
+    static constexpr int B_STAGE = (WS ? 2 : 1) * B_PART;
+    static constexpr int NSTAGE = WS ? 2 : (GA_N ? 4 : (DESCR_K ? 3 : 2));   // B pipeline depth (short stages need more copies in flight)
     static constexpr int A_BUF = 2 * A_PARTC;                // hi + lo
     static constexpr int OFF_A = 0;
     static constexpr int OFF_B = ((NA * A_BUF + 1023) / 1024) * 1024;
@@ -57,7 +60,7 @@ struct Cfg {
     static constexpr int TOTAL = OFF_BAR + 256;
     static constexpr int TM_BUF = 256;                       // TMEM columns per accumulator buffer
     static_assert(KTOT % KCH == 0 && NTOT % BN == 0 && BN % 16 == 0, "tile shapes");
-    static_assert(TOTAL <= 227 * 1024, "shared memory budget");
+    static_assert(TOTAL + 1024 + 64 <= 227 * 1024, "shared memory budget (1 KB: alignment of the dynamic array behind the static word)");
 };
 
 struct FitTcArgs {
@@ -103,11 +106,11 @@ __device__ long long fit_dbg[8];
 #else
 #define FT(i) do { } while (0)
 #endif
-template <int MODE, int KTOT, int NTOT>
+template <int MODE, int KTOT, int NTOT, bool WS>
 __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
     static_assert(MODE == 0 || MODE == 6, "the 240 x 240 products run in k_fit_chain");
     constexpr int NEPI = nepi(MODE), NPROD = nprod(MODE);
-    using C = Cfg<KTOT, NTOT>;
+    using C = Cfg<KTOT, NTOT, WS>;
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ uint32_t tmem_base_s;
     const int tid = threadIdx.x, lane = tid & 31;
@@ -146,7 +149,7 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                         const int st = step % C::NSTAGE;
                         tc::mbar_wait(&b_empty[st], ((step / C::NSTAGE) & 1) ^ 1);
                         mbar_expect_tx(&b_full[st], C::B_STAGE);
-                        bulk_g2s(sbase + C::OFF_B + st * C::B_STAGE, Bw + ((long)nt * C::NKC + kc) * (C::KCH * C::BN), C::B_STAGE, &b_full[st]);
+                        bulk_g2s(sbase + C::OFF_B + st * C::B_STAGE, Bw + ((long)nt * C::NKC + kc) * (C::B_STAGE / 2), C::B_STAGE, &b_full[st]);
                     }
             }
         }
@@ -183,6 +186,12 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                                 for (int ks = 0; ks < C::KCH / 16; ++ks)
                                     tc::mma_ss(tmem + buf * C::TM_BUF, tc::desc_at(da, part * C::A_PARTC + ks * 2 * C::ASS),
                                                tc::desc_at(db, ks * 2 * (C::BN * 16)), idesc, (kc | part | ks) != 0);
+                            if (WS) {       // A hi . B lo
+#pragma unroll
+                                for (int ks = 0; ks < C::KCH / 16; ++ks)
+                                    tc::mma_ss(tmem + buf * C::TM_BUF, tc::desc_at(da, ks * 2 * C::ASS),
+                                               tc::desc_at(db, C::B_PART + ks * 2 * (C::BN * 16)), idesc, true);
+                            }
                             tc::commit(&b_empty[st]);
                             if (!C::RESIDENT || nt == C::NTILES - 1) tc::commit(&a_empty[ab]);
                         }
@@ -399,7 +408,10 @@ __global__ void __launch_bounds__(nthreads(MODE), 1) k_fit_tc(FitTcArgs p) {
                             const float bb[4] = {b.x, b.y, b.z, b.w};
                             float r0[4];
 #pragma unroll
-                            for (int k = 0; k < 4; ++k) r0[k] = tc::tanh_approx(__uint_as_float(v[4 * g4 + k]) + bb[k]);
+                            for (int k = 0; k < 4; ++k) {
+                                const float z = __uint_as_float(v[4 * g4 + k]) + bb[k];
+                                r0[k] = WS ? tanhf(z) : tc::tanh_approx(z);        // MIX-32: exact single-precision tanh
+                            }
                             *reinterpret_cast<float4 *>(p.out0 + o + c) = make_float4(r0[0], r0[1], r0[2], r0[3]);
                         }
                     }
@@ -668,11 +680,11 @@ __global__ void __launch_bounds__(CH_THREADS, 1) k_fit_chain(FitChainArgs p) {
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(512));
 }
 
-template <int MODE, int KTOT, int NTOT>
+template <int MODE, int KTOT, int NTOT, bool WS = false>
 cudaError_t launch(const FitTcArgs &p, int grid, cudaStream_t st) {
-    using C = Cfg<KTOT, NTOT>;
-    DP_SMEM_OPTIN((k_fit_tc<MODE, KTOT, NTOT>), C::TOTAL);
-    k_fit_tc<MODE, KTOT, NTOT><<<grid, nthreads(MODE), C::TOTAL, st>>>(p);
+    using C = Cfg<KTOT, NTOT, WS>;
+    DP_SMEM_OPTIN((k_fit_tc<MODE, KTOT, NTOT, WS>), C::TOTAL);
+    k_fit_tc<MODE, KTOT, NTOT, WS><<<grid, nthreads(MODE), C::TOTAL, st>>>(p);
 #ifdef DP_FIT_TIMING
     {
         cudaStreamSynchronize(st);
@@ -754,6 +766,62 @@ static cudaError_t launch_fit_tc_nd(const dp_model *m, long N, const Grid3 &g, c
     q.aux0 = Amat; q.out0 = (float *)(ws + L.gD); q.ldo = ND;
     ok(launch<6, 240, ND>(q, grid, st));
     return e;
+}
+
+// ---- MIX-32: the two large products of the fitting net (first layer forward, K = 16 m2; last product backward, N = 16 m2)
+// on the same kernels with the weights as hi + lo fp16 parts (WS) and the exact tanhf; the four 240 x 240 products stay in
+// fit_mix.cu.  Images of one type: V1 for MODE 0 (K chunks of 64), then V1^T for MODE 6 (K chunks of 80); per stage (N tile, K
+// chunk) the hi image [KCH / 8][BN][8] followed by the lo image.
+static void fit_tc32_build_image(const double *W, int ldw, bool transpose, int K, int Nn, int KCH, __half *out) {
+    const int BN = Nn == 240 ? 240 : (Nn == 1600 ? 160 : 128);
+    const int ntl = Nn / BN, nkc = K / KCH, sub = KCH / 8;
+    for (int nt = 0; nt < ntl; ++nt)
+        for (int kc = 0; kc < nkc; ++kc)
+            for (int k8 = 0; k8 < sub; ++k8)
+                for (int n = 0; n < BN; ++n)
+                    for (int kk = 0; kk < 8; ++kk) {
+                        const int k = kc * KCH + k8 * 8 + kk, nn = nt * BN + n;
+                        const double v = transpose ? W[(size_t)nn * ldw + k] : W[(size_t)k * ldw + nn];
+                        const float vf = (float)v;                  // "cast to single", then hi + lo fp16 parts
+                        const __half hi = __float2half_rn(vf);
+                        const __half lo = __float2half_rn(vf - __half2float(hi));
+                        const size_t stage = ((size_t)nt * nkc + kc) * 2 * ((size_t)KCH * BN);
+                        const size_t e = ((size_t)k8 * BN + n) * 8 + kk;
+                        out[stage + e] = hi;
+                        out[stage + (size_t)KCH * BN + e] = lo;
+                    }
+}
+size_t fit_tc32_type_elems(int nd) { return 4 * (size_t)nd * 240; }
+void fit_tc32_build_type(int nd, const double *V1, __half *out) {
+    fit_tc32_build_image(V1, 240, false, nd, 240, 64, out);
+    fit_tc32_build_image(V1, 240, true, 240, nd, 80, out + 2 * (size_t)nd * 240);
+}
+
+template <int ND>
+static cudaError_t launch_fit_tc32_first_nd(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    constexpr int M2E = ND / 16;
+    FitTcArgs p{};
+    p.T = m->T; p.ncell = g.ncell; p.bin_start = (const int *)(ws + L.bin_start); p.b_type_stride = (long)fit_tc32_type_elems(ND);
+    p.A = (const float *)(ws + L.A); p.lda = 4 * M2E; p.Bimg = (const __half *)m->fit_tc_img_dev;
+    p.bias = (const float *)m->fitc1_dev; p.out0 = (float *)(ws + L.fit_act); p.ldo = 240;
+    return launch<0, ND, 240, true>(p, m->num_sms, st);
+}
+template <int ND>
+static cudaError_t launch_fit_tc32_last_nd(const dp_model *m, long N, const float *gz1, const Grid3 &g, char *ws, const WsLayout &L,
+                                           cudaStream_t st) {
+    FitTcArgs q{};
+    q.T = m->T; q.ncell = g.ncell; q.bin_start = (const int *)(ws + L.bin_start); q.b_type_stride = (long)fit_tc32_type_elems(ND);
+    q.A = gz1; q.lda = 240; q.Aimg = nullptr; q.Bimg = (const __half *)m->fit_tc_img_dev + 2 * (size_t)ND * 240;
+    q.aux0 = (const float *)(ws + L.A); q.out0 = (float *)(ws + L.gD); q.ldo = ND;
+    return launch<6, 240, ND, true>(q, m->num_sms, st);
+}
+// h1 [N][240] (first activation buffer) = tanh(D V1 + c1), the descriptor D formed in the operand producer from A_i
+cudaError_t launch_fit_tc32_first(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    return m->m2 == 128 ? launch_fit_tc32_first_nd<2048>(m, N, g, ws, L, st) : launch_fit_tc32_first_nd<1600>(m, N, g, ws, L, st);
+}
+// gA [N][4][m2] (in the gD buffer) from gz1 [N][240]: the last backward product with gD consumed in its epilogue
+cudaError_t launch_fit_tc32_last(const dp_model *m, long N, const float *gz1, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    return m->m2 == 128 ? launch_fit_tc32_last_nd<2048>(m, N, gz1, g, ws, L, st) : launch_fit_tc32_last_nd<1600>(m, N, gz1, g, ws, L, st);
 }
 
 cudaError_t launch_fit_tc(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
