@@ -211,14 +211,21 @@ def kernels_of(s, r, ms_step):
             "step_tflops": (rr * (FLOP_ROW_FWD + FLOP_ROW_BWD) + N * FLOP_ATOM_FIT) / (ms_step * 1e-3) / 1e12}
 
 
-def sweep_leg(args, binding, torch, synth, dev, flush, pk):
+def sweep_leg(args, binding, torch, synth, dev, flush, pk, precision="mix16", ncell=None, mp=None):
     """Network-size study (Fig. 7): copper, embedding nets (W, 2 W, 4 W), last layer 2 W x 4 W from the
-    paper's 64 x 128 to 1024 x 2048, MIX-16.  Algorithmic flops of the whole evaluation / CUDA-event time of the evaluation."""
+    paper's 64 x 128 to 1024 x 2048, in one precision.  Algorithmic flops of the whole evaluation / CUDA-event time of the
+    evaluation, against the peak of the precision's arithmetic: MIX-16 the sustained dense bf16 rate (MEASURED_PEAKS.json), FP64
+    the DMMA rate and MIX-32 the fp32 FFMA rate that dp_measure_peaks measures in this run (MIX-32 executes three TF32 tensor
+    products per algorithmic product, so its fraction of the fp32 rate can exceed 1)."""
     rows = []
+    ncell = ncell or args.sweep_ncell
+    peak, peak_name = pk["bf16_sus"], "bf16_sustained"
+    if precision != "mix16":
+        mp = mp or binding.measure_peaks()
+        peak, peak_name = (mp["dmma_tflops"], "dmma") if precision == "fp64" else (mp["ffma_tflops"], "ffma_fp32")
     for W in [int(x) for x in args.sweep_widths.split(",")]:
-        ncell = args.sweep_ncell
-        s = (synth.paper_copper(ncell, synth.SEED0 + 20, shuffle=True, precision="mix16") if W == 32
-             else synth.wide_copper(ncell, W, synth.SEED0 + 20, shuffle=True))
+        s = (synth.paper_copper(ncell, synth.SEED0 + 20, shuffle=True, precision=precision) if W == 32
+             else synth.wide_copper(ncell, W, synth.SEED0 + 20, shuffle=True, precision=precision))
         r = time_config(binding, torch, s, dev, args.steps, args.warmup, flush)
         ms = r["t_ms"] / args.steps
         ff, fb, fa, _ = flops_of(s.model)
@@ -231,7 +238,8 @@ def sweep_leg(args, binding, torch, synth, dev, flush, pk):
                      "embed_fwd_bwd_tflops": emb / ((ph[1] + ph[3]) * 1e-3) / 1e12,
                      "bwd_gemm_ms": ph[5] if W != 32 else None,
                      "bwd_gemm_tflops": (rr * 2 * (W * 2 * W + 2 * W * 4 * W) / (ph[5] * 1e-3) / 1e12) if W != 32 else None,
-                     "frac_of_bf16_sustained": (emb + s.natoms * fa) / (ms * 1e-3) / 1e12 / pk["bf16_sus"]})
+                     "precision": precision, "peak": peak_name, "peak_tflops": peak,
+                     ("frac_of_bf16_sustained" if precision == "mix16" else "frac_of_" + peak_name): (emb + s.natoms * fa) / (ms * 1e-3) / 1e12 / peak})
         r["model"].close()
         del r
         torch.cuda.empty_cache()
@@ -354,12 +362,13 @@ def main():
             pk = peaks()
             sampler = ClockSampler(local_rank)
             sampler.start()
-            rows = sweep_leg(args, binding, torch, synth, dev, flush, pk)
+            prec = args.precision or "mix16"
+            rows = sweep_leg(args, binding, torch, synth, dev, flush, pk, precision=prec)
             clocks = sampler.stop()
             print(json.dumps({"metric": "network_size_sweep_step_tflops", "value": max(x["step_tflops"] for x in rows),
                               "unit": "TFLOP/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "higher_is_better": True,
-                              "dtype": "f16", "data": "synthetic", "vs_baseline": None,
-                              "config": {"workload": "sweep_cu (PAPER.md:273-279, Fig. 7)", "precision": "mix16",
+                              "dtype": {"fp64": "f64", "mix32": "f32", "mix16": "f16"}[prec], "data": "synthetic", "vs_baseline": None,
+                              "config": {"workload": "sweep_cu (PAPER.md:273-279, Fig. 7)", "precision": prec,
                                          "l2": "256 MB flush between timed steps"},
                               "peak": {"bf16_sustained_tflops": pk["bf16_sus"], "source": pk["src"]},
                               "sweep": rows, "clocks": clocks}))

@@ -46,10 +46,10 @@ WsLayout ws_layout(const dp_model *m, long N, long NE) {
     }
     L.nlist = take(sizeof(int) * (size_t)N * m->Nm);
     L.nreal = take(sizeof(int) * (size_t)N * m->T);
-    if (m->prec != DP_FP64) {
+    if (dp_uses_rows(m)) {
         L.rowcnt = take(sizeof(int) * (size_t)N * m->T);
         L.rowstart = take(sizeof(int) * ((size_t)N + 1) * m->T);
-        L.rows_rh = take(sizeof(float) * 4 * (size_t)N * m->Nm);     // block b starts at row offset N*off[b]
+        L.rows_rh = take(m->wide_gen ? 0 : sizeof(float) * 4 * (size_t)N * m->Nm);     // block b starts at row offset N*off[b]
         L.rows_id = take(sizeof(int) * 2 * (size_t)N * m->Nm);
         if (m->prec == DP_MIX16) {
             L.rows_g = take(sizeof(float) * 4 * (size_t)N * m->Nm);
@@ -60,7 +60,7 @@ WsLayout ws_layout(const dp_model *m, long N, long NE) {
     const size_t esz = m->prec == DP_FP64 ? sizeof(double) : sizeof(float);
     const int nt3 = 2 * ((m->m0 + 3) / 4);          // EmbW<W>::NT3
     L.A = take(esz * (size_t)N * 4 * m->m2);
-    if (m->wide) L.gAf = take(0);                   // the wide path reads gA itself
+    if (m->wide) L.gAf = take(m->prec == DP_FP64 ? sizeof(double) * (size_t)N * 4 * m->m2 : 0);      // the wide paths read gA itself
     else if (m->prec == DP_FP64) L.gAf = take(sizeof(double) * (size_t)N * 3 * nt3 * 32);
     else L.gAf = take(sizeof(uint32_t) * (size_t)N * 2 * (2 * nt3) * 32);     // MIX-32 fragments / MIX-16 operand image (smaller)
     L.gscale = take(sizeof(float) * (size_t)N);
@@ -71,7 +71,16 @@ WsLayout ws_layout(const dp_model *m, long N, long NE) {
     L.eatom = take(sizeof(double) * (size_t)N);
     L.fsorted = take(sizeof(double) * 3 * (size_t)NE);
     L.virial = take(sizeof(double) * 16);
-    if (m->wide) {      // activation images of the wide-network path: 128 rows x 9 W fp16 per tile (wide.cu)
+    if (m->wide_gen) {  // FP64 / MIX-32 wide nets (wide_gen.cu): row-major activations and per-row vectors over the compact rows
+        const size_t rows = (size_t)N * m->Nm;
+        L.wide_tab = take(sizeof(int) * 4 * ((size_t)m->T * m->T + 1));
+        L.wide_rh = take(esz * 4 * rows);
+        L.wide_gr = take(esz * 4 * rows);
+        L.wide_t1 = take(esz * rows * m->m0);
+        L.wide_y2 = take(esz * rows * m->m1);
+        L.wide_t2 = take(esz * rows * m->m1);
+        L.wide_t3 = take(esz * rows * m->m2);
+    } else if (m->wide) {      // activation images of the wide-network path: 128 rows x 9 W fp16 per tile (wide.cu)
         const size_t tiles = (size_t)wide_tiles_cap(m, N), chunk = 2048;
         L.wide_tab = take(sizeof(int) * 4 * ((size_t)m->T * m->T + 1));
         L.wide_t1 = take(tiles * (m->m0 / 8) * chunk);
@@ -417,14 +426,13 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
     if (T < 1 || T > DP_MAX_TYPES) return DP_EINVAL;
     if (!(rc > 0) || !(rc_smth >= 0) || !(rc_smth < rc) || !(rc * rc < 128.0)) return DP_EINVAL;
     // embedding widths (W, 2 W, 4 W) with W = 25 (BASELINE configs) or W = 32 (the paper's own networks)
-    // or, MIX-16 only, the wide nets of the network-size study W = 64, 128, 256, 512 (wide.cu)
+    // or the wide nets of the network-size study W = 64, 128, 256, 512 (MIX-16: wide.cu, FP64 / MIX-32: wide_gen.cu)
     const int W0 = w->embed_widths[0];
     const bool wide = W0 == 64 || W0 == 128 || W0 == 256 || W0 == 512;
     if ((W0 != 25 && W0 != 32 && !wide) || w->embed_widths[1] != 2 * W0 || w->embed_widths[2] != 4 * W0 || w->axis != 16 ||
         w->fit_widths[0] != 240 || w->fit_widths[1] != 240 || w->fit_widths[2] != 240)
         return DP_EUNSUPPORTED;
     if (W0 == 32 && !paper_shape_supported(prec)) return DP_EUNSUPPORTED;
-    if (wide && prec != DP_MIX16) return DP_EUNSUPPORTED;
     if (prec != DP_FP64 && prec != DP_MIX32 && prec != DP_MIX16) return DP_EINVAL;
     int maxsel = 0, Nm = 0;
     for (int b = 0; b < T; ++b) { if (sel[b] <= 0) return DP_EINVAL; Nm += sel[b]; if (sel[b] > maxsel) maxsel = sel[b]; }
@@ -440,6 +448,7 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
     m->T = T; m->Nm = Nm; m->axis = 16; m->F = 240; m->rc = rc; m->rc_smth = rc_smth; m->prec = prec;
     m->m0 = W0; m->m1 = 2 * W0; m->m2 = 4 * W0;
     m->wide = wide ? 1 : 0;
+    m->wide_gen = (wide && prec != DP_MIX16) ? 1 : 0;
     m->n_type_map = n_type_map;
     for (int b = 0; b < T; ++b) { m->sel[b] = sel[b]; m->off[b + 1] = m->off[b] + sel[b]; }
     int cap = 256;
@@ -456,7 +465,12 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
     std::vector<int> tm(type_map, type_map + n_type_map);
     ok(upload(tm, (void **)&m->type_map_dev));
     const size_t ensz = (size_t)W0 + W0 + (size_t)W0 * 2 * W0 + 2 * W0 + (size_t)2 * W0 * 4 * W0 + 4 * W0;
-    if (prec == DP_FP64 && W0 == 32) {
+    if (wide && prec != DP_MIX16) {     // wide nets in FP64 / MIX-32: row-major weights and their transposes (wide_gen.cu)
+        const size_t ne = wide_gen_net_elems(W0), esz = prec == DP_FP64 ? 8 : 4;
+        std::vector<char> blk((size_t)T * T * ne * esz);
+        for (int ab = 0; ab < T * T; ++ab) wide_gen_build_net(W0, prec == DP_FP64, w->embed + ab * ensz, &blk[(size_t)ab * ne * esz]);
+        ok(upload(blk, &m->wide_vec_dev));
+    } else if (prec == DP_FP64 && W0 == 32) {
         std::vector<EmbedNetFrag<double, 32>> frags((size_t)T * T);
         for (int ab = 0; ab < T * T; ++ab) build_embed_frag<double, 32>(w->embed + ab * ensz, &frags[ab]);
         ok(upload(frags, &m->embed_frag_dev));
@@ -569,7 +583,13 @@ size_t dp_workspace_bytes(const dp_model *m, long natoms, const double *box_host
 int dp_launches_per_compute(const dp_model *m) {
     if (!m) return 0;
     int n = 6 + 1;                                   // wrap, 3-launch bin scan, scatter, bin sort; list
-    if (m->prec == DP_FP64) {
+    if (m->wide_gen) {                               // wide_gen.cu
+        n += 3 * m->T;                               // row prefix sums
+        n += 6;                                      // environment rows, tile table, layer 1, two GEMMs, contraction
+        n += m->prec == DP_FP64 ? 9 : 7;             // FP64: descriptor, 6 GEMMs, energy, gA; MIX-32: first (tcgen05), 4 GEMMs, energy, last (tcgen05)
+        if (m->prec == DP_FP64 && m->last_natoms > 0 && fit_f64_splitk(m, m->last_natoms)) n += 1;
+        n += 4 + m->T;                               // backward head, two GEMMs, layer 1 + normalisation, force + virial per neighbour type
+    } else if (m->prec == DP_FP64) {
         n += 1 + 9 + 1;                              // forward; descriptor, 6 GEMMs, energy, gA; backward (with S8, S9)
         if (m->last_natoms > 0 && fit_f64_splitk(m, m->last_natoms)) n += 1;     // small systems: split-K first layer + bias / tanh
     } else {
@@ -621,13 +641,15 @@ int dp_compute(dp_model *m, long natoms, const double *coords_dev, const int *ty
     mark(1);
     const bool f64 = m->prec == DP_FP64;
     const bool m16 = m->prec == DP_MIX16;
-    ok(f64 ? launch_embed_fwd_f64(m, natoms, g, ws, L, st)
+    ok(m->wide_gen ? launch_embed_fwd_wide_gen(m, natoms, g, ws, L, st)
+           : f64 ? launch_embed_fwd_f64(m, natoms, g, ws, L, st)
            : m->wide ? launch_embed_fwd_wide(m, natoms, g, ws, L, st)
            : (m16 && !m->fwd_split ? launch_embed_fwd_tc2(m, natoms, g, ws, L, st) : launch_embed_fwd_tc(m, natoms, g, ws, L, st)));
     mark(2);
     ok(f64 ? launch_fit_f64(m, natoms, g, ws, L, st) : (m16 ? launch_fit_tc(m, natoms, g, ws, L, st) : launch_fit_mix(m, natoms, g, ws, L, st)));
     mark(3);
-    ok(f64 ? launch_embed_bwd_f64(m, natoms, g, ws, L, st)
+    ok(m->wide_gen ? launch_embed_bwd_wide_gen(m, natoms, g, ws, L, st)
+           : f64 ? launch_embed_bwd_f64(m, natoms, g, ws, L, st)
            : m->wide ? launch_embed_bwd_wide(m, natoms, g, ws, L, st)
            : (m16 ? launch_embed_bwd_tc2(m, natoms, g, ws, L, st) : launch_embed_bwd_mix(m, natoms, g, ws, L, st)));
     if (g.ghost) ok(launch_fold_ghost(m, natoms, g, ws, L, st));

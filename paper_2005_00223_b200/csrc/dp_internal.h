@@ -69,8 +69,9 @@ struct dp_model {
     int off[DP_MAX_TYPES + 1];
     int Nm;
     int m0, m1, m2;                 // embedding widths (W, 2 W, 4 W): (25, 50, 100), (32, 64, 128), or wide: W = 64 ... 512
-    int wide;                       // MIX-16 with W >= 64: layer-by-layer GEMM path with activations in HBM (wide.cu)
-    void *wide_vec_dev;             // wide: [T*T][8 W] floats w1, b1, b2, b3
+    int wide;                       // W >= 64: layer-by-layer GEMM path with activations in HBM (MIX-16: wide.cu; else wide_gen.cu)
+    int wide_gen;                   // wide and FP64 / MIX-32: DMMA / 3xTF32 GEMMs on row-major activations (wide_gen.cu)
+    void *wide_vec_dev;             // wide: [T*T][8 W] floats w1, b1, b2, b3; wide_gen: [T*T] parameter blocks (8 W + 20 W^2 elements)
     void *wide_img_dev;             // wide: [T*T][20 W^2] fp16 weight images W2, W3, W3^T, W2^T
     int axis;                       // 16
     int F;                          // fitting width 240
@@ -149,8 +150,12 @@ struct WsLayout {
     size_t gstart;      // int[N+1]
     // wide networks (wide.cu): tile table and the activation images, per 128-row tile [columns / 8][128][8] fp16
     size_t wide_tab;    // int4[T*T + 1]
-    size_t wide_t1, wide_y2, wide_t2, wide_t3;      // W, 2 W, 2 W, 4 W columns
+    size_t wide_t1, wide_y2, wide_t2, wide_t3;      // W, 2 W, 2 W, 4 W columns (wide_gen.cu: row-major [N Nm][columns], fp64 / fp32)
+    size_t wide_rh, wide_gr;                        // wide_gen.cu: R^ and dE/dR~ per compact row, [N Nm][4]
 };
+
+// the compact rows (rowcnt, rowstart, rows_id) exist in the mixed modes and on every wide path
+inline bool dp_uses_rows(const dp_model *m) { return m->prec != DP_FP64 || m->wide; }
 
 // FP64 fitting net, first layer (K = 16 m2): split K over four CTAs per output tile when the row tiles (64 rows x 80 columns)
 // are too few to fill the GPU (fit_f64.cu; one more launch per evaluation: dp_launches_per_compute)
@@ -217,6 +222,12 @@ cudaError_t launch_embed_bwd_wide(const dp_model *m, long N, const Grid3 &g, cha
 size_t wide_net_img_elems(int W);
 void wide_build_net(int W, const double *net, float *vec, struct __half *img);
 long wide_tiles_cap(const dp_model *m, long N);
+cudaError_t launch_wide_tiles(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+// wide networks in FP64 and MIX-32 (wide_gen.cu)
+cudaError_t launch_embed_fwd_wide_gen(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+cudaError_t launch_embed_bwd_wide_gen(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
+size_t wide_gen_net_elems(int W);
+void wide_gen_build_net(int W, bool f64, const double *net, void *out);
 size_t fit_tc32_type_elems(int nd);
 void fit_tc32_build_type(int nd, const double *V1, struct __half *out);
 cudaError_t launch_fit_tc32_first(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);

@@ -266,11 +266,49 @@ __global__ void __launch_bounds__(128) k_gA(long N, double inv_nm, const double 
     }
 }
 
+// Wide nets (wide_gen.cu; m2 = 4 W up to 2,048, a run-time value).  The descriptor: one thread per entry.
+__global__ void __launch_bounds__(256) k_descr_wide(int M2, const double *__restrict__ Amat, double *__restrict__ D) {
+    const long i = blockIdx.x;
+    const int idx = blockIdx.y * 256 + threadIdx.x;           // M2 * 16 is a multiple of 256
+    const int mm = idx >> 4, ax = idx & 15;
+    const double *A = Amat + i * 4L * M2;
+    double acc = 0.0;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) acc += A[c * M2 + mm] * A[c * M2 + ax];
+    D[i * (M2 * 16L) + idx] = acc;
+}
+// gA[c][m] = sum_a gD[m][a] A[c][a] + [m < 16] sum_m' gD[m'][m] A[c][m']   (N8), row-major [N][4][M2], without the 1 / Nm that
+// the backward head applies.  One CTA per atom: a thread per (c, m) for the first sum, a warp per eight (c, m < 16) for the second.
+__global__ void __launch_bounds__(256) k_gA_wide(int M2, const double *__restrict__ Amat, const double *__restrict__ gD,
+                                                 double *__restrict__ gA) {
+    __shared__ double s2[64];
+    const long i = blockIdx.x;
+    const double *A = Amat + i * 4L * M2, *G = gD + i * (M2 * 16L);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int o = warp * 8; o < warp * 8 + 8; ++o) {
+        const int c = o >> 4, mm = o & 15;
+        double acc = 0.0;
+        for (int mp = lane; mp < M2; mp += 32) acc += G[mp * 16 + mm] * A[c * M2 + mp];
+#pragma unroll
+        for (int sh = 16; sh > 0; sh >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, sh);
+        if (lane == 0) s2[o] = acc;
+    }
+    __syncthreads();
+    for (int idx = threadIdx.x; idx < 4 * M2; idx += 256) {
+        const int c = idx / M2, mm = idx % M2;
+        double acc = mm < 16 ? s2[c * 16 + mm] : 0.0;
+#pragma unroll
+        for (int ax = 0; ax < 16; ++ax) acc += G[mm * 16 + ax] * A[c * M2 + ax];
+        gA[i * 4L * M2 + idx] = acc;
+    }
+}
+
 }  // namespace
 
+// W = 0: a wide net (m2 taken from the model; descriptor and gA by the run-time kernels above)
 template <int W>
 static cudaError_t launch_fit_w(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    constexpr int M2E = EmbW<W>::M2E;
+    const int M2E = W ? EmbW<(W ? W : 25)>::M2E : m->m2;
     const int F = 240, ND = M2E * 16;
     const int T = m->T;
     double *Amat = (double *)(ws + L.A);
@@ -286,7 +324,8 @@ static cudaError_t launch_fit_w(const dp_model *m, long N, const Grid3 &g, char 
     const unsigned gx = (unsigned)((N + BM - 1) / BM);
     const unsigned nb8 = (unsigned)((N + 7) / 8);
 
-    k_descr<W><<<nb8, 256, 0, st>>>(N, Amat, D);
+    if constexpr (W == 0) k_descr_wide<<<dim3((unsigned)N, (unsigned)(ND / 256)), 256, 0, st>>>(M2E, Amat, D);
+    else k_descr<W><<<nb8, 256, 0, st>>>(N, Amat, D);
 
     FitArgs p{};
     p.ncell = g.ncell; p.bin_start = bin_start; p.v4 = v4; p.v4_type_stride = F; p.bias_type_stride = F;
@@ -320,12 +359,17 @@ static cudaError_t launch_fit_w(const dp_model *m, long N, const Grid3 &g, char 
     p.A = gz1; p.N = ND; p.B = V1; p.b_type_stride = (long)ND * F; p.out0 = D; p.ldo = ND;
     k_fit_gemm<5><<<dim3(gx, (ND + BN - 1) / BN, T), 256, 0, st>>>(p);
     // gD, A -> gA fragments for the embedding backward
-    const int smem = 4 * (4 * M2E + M2E * 17 + 4 * M2E) * 8;
-    DP_SMEM_OPTIN(k_gA<W>, smem);
-    k_gA<W><<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, 1.0 / (double)m->Nm, Amat, D, (double *)(ws + L.gAf));
+    if constexpr (W == 0) {
+        k_gA_wide<<<(unsigned)N, 256, 0, st>>>(M2E, Amat, D, (double *)(ws + L.gAf));
+    } else {
+        const int smem = 4 * (4 * M2E + M2E * 17 + 4 * M2E) * 8;
+        DP_SMEM_OPTIN(k_gA<W>, smem);
+        k_gA<W><<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, 1.0 / (double)m->Nm, Amat, D, (double *)(ws + L.gAf));
+    }
     return cudaGetLastError();
 }
 
 cudaError_t launch_fit_f64(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    if (m->wide) return launch_fit_w<0>(m, N, g, ws, L, st);
     return m->m0 == 32 ? launch_fit_w<32>(m, N, g, ws, L, st) : launch_fit_w<25>(m, N, g, ws, L, st);
 }

@@ -297,8 +297,10 @@ static cudaError_t launch_fit_mix_w(const dp_model *m, long N, const Grid3 &g, c
     ok(launch_gemm<4>(p, g240, st));
     // last product (N = 16 m2) on the tcgen05 kernel: gD is consumed in its epilogue, gA [N][4][m2] lands in the gD buffer
     ok(launch_fit_tc32_last(m, N, gz1, g, ws, L, st));
-    k_gA_frag<2, W><<<(unsigned)((N + 3) / 4), 128, 0, st>>>(N, D, (uint32_t *)(ws + L.gAf), (float *)(ws + L.gscale));
-    ok(cudaGetLastError());
+    if (!m->wide) {     // (the wide path of wide_gen.cu reads gA itself)
+        k_gA_frag<2, W><<<(unsigned)((N + 3) / 4), 128, 0, st>>>(N, D, (uint32_t *)(ws + L.gAf), (float *)(ws + L.gscale));
+        ok(cudaGetLastError());
+    }
     return e;
 }
 

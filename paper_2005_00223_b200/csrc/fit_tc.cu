@@ -817,11 +817,25 @@ static cudaError_t launch_fit_tc32_last_nd(const dp_model *m, long N, const floa
 }
 // h1 [N][240] (first activation buffer) = tanh(D V1 + c1), the descriptor D formed in the operand producer from A_i
 cudaError_t launch_fit_tc32_first(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    return m->m2 == 128 ? launch_fit_tc32_first_nd<2048>(m, N, g, ws, L, st) : launch_fit_tc32_first_nd<1600>(m, N, g, ws, L, st);
+    switch (m->m2) {
+        case 128: return launch_fit_tc32_first_nd<2048>(m, N, g, ws, L, st);
+        case 256: return launch_fit_tc32_first_nd<4096>(m, N, g, ws, L, st);       // wide nets (wide_gen.cu)
+        case 512: return launch_fit_tc32_first_nd<8192>(m, N, g, ws, L, st);
+        case 1024: return launch_fit_tc32_first_nd<16384>(m, N, g, ws, L, st);
+        case 2048: return launch_fit_tc32_first_nd<32768>(m, N, g, ws, L, st);
+        default: return launch_fit_tc32_first_nd<1600>(m, N, g, ws, L, st);
+    }
 }
 // gA [N][4][m2] (in the gD buffer) from gz1 [N][240]: the last backward product with gD consumed in its epilogue
 cudaError_t launch_fit_tc32_last(const dp_model *m, long N, const float *gz1, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
-    return m->m2 == 128 ? launch_fit_tc32_last_nd<2048>(m, N, gz1, g, ws, L, st) : launch_fit_tc32_last_nd<1600>(m, N, gz1, g, ws, L, st);
+    switch (m->m2) {
+        case 128: return launch_fit_tc32_last_nd<2048>(m, N, gz1, g, ws, L, st);
+        case 256: return launch_fit_tc32_last_nd<4096>(m, N, gz1, g, ws, L, st);
+        case 512: return launch_fit_tc32_last_nd<8192>(m, N, gz1, g, ws, L, st);
+        case 1024: return launch_fit_tc32_last_nd<16384>(m, N, gz1, g, ws, L, st);
+        case 2048: return launch_fit_tc32_last_nd<32768>(m, N, gz1, g, ws, L, st);
+        default: return launch_fit_tc32_last_nd<1600>(m, N, gz1, g, ws, L, st);
+    }
 }
 
 cudaError_t launch_fit_tc(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {

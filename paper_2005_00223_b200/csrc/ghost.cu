@@ -315,9 +315,9 @@ cudaError_t launch_nlist_ghost(const dp_model *m, long N, const Grid3 &g, char *
     k_nlist_ghost<<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, m->T, g, m->rc * m->rc, cap, (int *)(ws + L.bin_start),
                                                             (double *)(ws + L.xs), (int *)(ws + L.perm), (int *)(ws + L.ext_base),
                                                             (int *)(ws + L.ext_scode), m->Nm, tt, (int *)(ws + L.nlist),
-                                                            (int *)(ws + L.nreal), m->prec == DP_FP64 ? nullptr : (int *)(ws + L.rowcnt),
+                                                            (int *)(ws + L.nreal), !dp_uses_rows(m) ? nullptr : (int *)(ws + L.rowcnt),
                                                             (int *)(ws + L.status));
-    if (m->prec != DP_FP64)
+    if (dp_uses_rows(m))
         for (int b = 0; b < m->T; ++b)
             dp_launch_scan((int)N, (int *)(ws + L.rowcnt) + (long)b * N, (int *)(ws + L.rowstart) + (long)b * (N + 1), (int *)(ws + L.scan_tmp), st);
     return cudaGetLastError();

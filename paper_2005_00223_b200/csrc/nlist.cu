@@ -589,9 +589,9 @@ cudaError_t launch_nlist(const dp_model *m, long N, const Grid3 &g, char *ws, co
     kern<<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, m->T, g, m->rc * m->rc, gf, cap, (int *)(ws + L.bin_start),
                                                     (double *)(ws + L.xs), (const float4 *)(ws + L.xsf), (int *)(ws + L.perm),
                                                     (int *)(ws + L.inv), m->Nm, tt, (int *)(ws + L.nlist),
-                                                    (int *)(ws + L.nreal), m->prec == DP_FP64 ? nullptr : (int *)(ws + L.rowcnt),
+                                                    (int *)(ws + L.nreal), !dp_uses_rows(m) ? nullptr : (int *)(ws + L.rowcnt),
                                                     (int *)(ws + L.status), m->md_cand, m->md_candcnt);
-    if (m->prec != DP_FP64)
+    if (dp_uses_rows(m))
         for (int b = 0; b < m->T; ++b)
             launch_scan((int)N, (int *)(ws + L.rowcnt) + (long)b * N, (int *)(ws + L.rowstart) + (long)b * (N + 1), (int *)(ws + L.scan_tmp), st);
     return cudaGetLastError();

@@ -685,6 +685,12 @@ static cudaError_t wide_gemm(const dp_model *m, WideArgs p, int K, int Nn, const
 
 cudaError_t launch_env_rows(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 
+// the tile table alone (the FP64 / MIX-32 wide path of wide_gen.cu walks the same 128-row tiles)
+cudaError_t launch_wide_tiles(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    k_wide_tiles<<<1, 32, 0, st>>>(N, m->T, g.ncell, (const int *)(ws + L.bin_start), (const int *)(ws + L.rowstart), (int4 *)(ws + L.wide_tab));
+    return cudaGetLastError();
+}
+
 cudaError_t launch_embed_fwd_wide(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
     const int W = m->m0;
     const TypeTab tt = make_typetab(m);

@@ -1,0 +1,610 @@
+// S3 + S4 + S5 + S7 + S8 + S9 for WIDE embedding nets (W, 2 W, 4 W), W = 64 ... 512, in FP64 and MIX-32: the double and
+// MIX-32 curves of the network-size study (Fig. 7: "the FLOPS curves of both double and MIX-32 versions
+// flatten after the matrix size reaching 256 x 512"); the MIX-16 curve is wide.cu.
+//
+// The structure is the paper's own: one GEMM per layer with the bias / tanh / skip / tanh' work in its
+// epilogue, the activations kept in HBM between the layers (row-major, in the precision of the nets) and reused by the
+// backward pass, which overwrites them in place (dz3 over t3, dz2 over t2, dy2 over y2, dz1 over t1).  Rows are the compact
+// rows of the mixed modes (the real rows of a (centre type, neighbour type) block, contiguous, plus one
+// representative per atom and block for its padded slots, weighted by their number) and the row tiles are those of the
+// tile table of wide.cu, so a tile never straddles two nets.
+//   FP64   ("double"): GEMMs on the FP64 tensor pipe (DMMA m8n8k4), 128 x 128 x 16 tiles staged with cp.async;
+//   MIX-32 (nets in single precision): the same tiles on mma.sync m16n8k8 TF32, every operand split into a
+//          TF32 value and its TF32 remainder and three products per step ("3xTF32": the product keeps 21+ mantissa bits;
+//          the accumulators are fp32), exact tanhf.  Coordinates, environment rows, geometry derivative, force and virial
+//          accumulation stay fp64 in both modes.
+// Forward:  k_wg_env -> k_wg_l1 (t1) -> gemm<0> (t2, y2 = (t1,t1) + t2) -> gemm<1> (t3) -> k_wg_contract (A_i = R^T G / Nm)
+// Backward: k_wg_bwd_head (gG = R^ gA / Nm, dz3, skip share of dy2, dR^ = G gA^T / Nm) -> gemm<2> (dy2, dz2) -> gemm<3> (dz1)
+//           -> k_wg_ds (ds^ = dz1 . w1, dE/dR~ = (dR^ + ds^ e0) / std) -> k_wg_force (N9 geometry derivative, ProdForce,
+//           ProdViral).
+#include <type_traits>
+#include <vector>
+#include "dp_internal.h"
+#include "tanh64.cuh"
+
+namespace {
+
+constexpr int GR = 128;                     // rows per tile (= the tile table's, wide.cu)
+constexpr int GBN = 128, GBK = 16;          // N tile, K step
+constexpr int GA_STRIDE = GBK + 4;          // A tile [128][20]: fragment loads hit distinct banks (fp64: per half warp)
+template <typename R> struct GemmCfg {
+    static constexpr int BS = sizeof(R) == 8 ? GBN + 4 : GBN + 8;       // B tile [16][BS]
+    static constexpr int A_TILE = GR * GA_STRIDE, B_TILE = GBK * BS;
+    static constexpr int SMEM = 2 * (A_TILE + B_TILE) * (int)sizeof(R);
+    static constexpr int EPV = 16 / (int)sizeof(R);                     // elements per 16-byte cp.async
+};
+
+__device__ __forceinline__ double wg_tanh(double x) { return dp_tanh64(x); }
+__device__ __forceinline__ float wg_tanh(float x) { return tanhf(x); }
+
+__device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b) {
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+__device__ __forceinline__ void mma_tf32(float *c, const uint32_t (&a)[4], const uint32_t (&b)[2]) {
+    asm("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+        : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+        : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
+}
+// x = big + small, both TF32 (10 explicit mantissa bits each): big = rna(x), small = rna(x - big)
+__device__ __forceinline__ void split_tf32(float x, uint32_t &big, uint32_t &small) {
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(big) : "f"(x));
+    const float rem = x - __uint_as_float(big);
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(small) : "f"(rem));
+}
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc, bool valid) {
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+    const int sz = valid ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(s), "l"(gsrc), "r"(sz));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N)); }
+
+__device__ __forceinline__ double min_image(double t, double L, double halfL) {
+    const double s = t > halfL ? -1.0 : (t < -halfL ? 1.0 : 0.0);
+    return __dadd_rn(t, __dmul_rn(s, L));
+}
+struct EnvParams {
+    double rc, rc_smth, inv_range;
+    double L[3];
+};
+EnvParams make_env(const dp_model *m, const Grid3 &g) {
+    EnvParams ep;
+    ep.rc = m->rc; ep.rc_smth = m->rc_smth; ep.inv_range = 1.0 / (m->rc - m->rc_smth);
+    ep.L[0] = g.L[0]; ep.L[1] = g.L[1]; ep.L[2] = g.L[2];
+    return ep;
+}
+// N4 (+ N9 when sp_out): R~ = s (1, d / r), s = w(r) / r; sp = ds/dr
+__device__ __forceinline__ void env_row(const EnvParams &p, double dx, double dy, double dz, double Rt[4], double *sp_out, double *r_out) {
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    const double r = sqrt(r2);
+    double w = 1.0, dw = 0.0;
+    if (r >= p.rc_smth) {
+        if (r < p.rc) {
+            const double u = (r - p.rc_smth) * p.inv_range;
+            w = u * u * u * (-6.0 * u * u + 15.0 * u - 10.0) + 1.0;
+            dw = -30.0 * u * u * (u - 1.0) * (u - 1.0) * p.inv_range;
+        } else {
+            w = 0.0;
+        }
+    }
+    const double s = w / r;
+    Rt[0] = s; Rt[1] = s * dx / r; Rt[2] = s * dy / r; Rt[3] = s * dz / r;
+    if (sp_out) { *sp_out = dw / r - w / r2; *r_out = r; }
+}
+
+// the block k = a T + b of a tile of the tile table (entry k = {first tile, first row, end row}; entry T T = {tiles})
+__device__ __forceinline__ int wg_block(const int4 *tab, int nblk, int tile) {
+    int k = 0;
+    while (k + 1 < nblk && tile >= tab[k + 1].x) ++k;
+    return k;
+}
+
+// per-net parameter block (elements of R): w1 | b1 | b2 | b3 | W2 [W][2W] | W3 [2W][4W] | W3^T [4W][2W] | W2^T [2W][W]
+__host__ __device__ inline long wg_off_b2(int W) { return 2L * W; }
+__host__ __device__ inline long wg_off_b3(int W) { return 4L * W; }
+__host__ __device__ inline long wg_off_W2(int W) { return 8L * W; }
+__host__ __device__ inline long wg_off_W3(int W) { return 8L * W + 2L * W * W; }
+__host__ __device__ inline long wg_off_W3T(int W) { return 8L * W + 10L * W * W; }
+__host__ __device__ inline long wg_off_W2T(int W) { return 8L * W + 18L * W * W; }
+
+// S3: compact environment rows in the precision of the nets (computed in fp64), and their ids
+template <typename R>
+__global__ void __launch_bounds__(256)
+k_wg_env(long N, int T, int ncell, int Nm, const __grid_constant__ TypeTab tt, EnvParams ep, const double *__restrict__ avg,
+         const double *__restrict__ stdv, const int *__restrict__ bin_start, const double *__restrict__ xs,
+         const int *__restrict__ nlist, const int *__restrict__ nreal, const int *__restrict__ rowstart, R *__restrict__ rh,
+         int2 *__restrict__ rows_id) {
+    const int lane = threadIdx.x & 31;
+    const long i = blockIdx.x * 8L + (threadIdx.x >> 5);
+    if (i >= N) return;
+    int a = 0;
+    for (int t = 1; t < T; ++t) a += i >= bin_start[t * ncell];
+    double av[4], sd[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) { av[c] = avg[4 * a + c]; sd[c] = stdv[4 * a + c]; }
+    const double xi = xs[3 * i], yi = xs[3 * i + 1], zi = xs[3 * i + 2];
+    const double hx = 0.5 * ep.L[0], hy = 0.5 * ep.L[1], hz = 0.5 * ep.L[2];
+    for (int b = 0; b < T; ++b) {
+        const int nr = nreal[i * T + b];
+        const int tot = nr + (nr < tt.sel[b] ? 1 : 0);
+        const long base = N * (long)tt.off[b] + rowstart[(long)b * (N + 1) + i];
+        const int *nl = nlist + i * Nm + tt.off[b];
+        for (int k = lane; k < tot; k += 32) {
+            double Rt[4] = {0.0, 0.0, 0.0, 0.0};
+            int j = -(tt.sel[b] - nr);
+            if (k < nr) {
+                j = nl[k];
+                const double dx = min_image(xs[3 * (long)j] - xi, ep.L[0], hx);
+                const double dy = min_image(xs[3 * (long)j + 1] - yi, ep.L[1], hy);
+                const double dz = min_image(xs[3 * (long)j + 2] - zi, ep.L[2], hz);
+                env_row(ep, dx, dy, dz, Rt, nullptr, nullptr);
+            }
+#pragma unroll
+            for (int c = 0; c < 4; ++c) rh[4 * (base + k) + c] = (R)((Rt[c] - av[c]) / sd[c]);
+            rows_id[base + k] = make_int2((int)i, j);
+        }
+    }
+}
+
+// Layer 1 (K = 1): t1 = tanh(s^ w1 + b1); one CTA per tile
+template <typename R>
+__global__ void __launch_bounds__(256)
+k_wg_l1(long N, int T, int W, const __grid_constant__ TypeTab tt, const int4 *__restrict__ tab, const R *__restrict__ nets,
+        long net_stride, const R *__restrict__ rh, R *__restrict__ T1) {
+    const int nblk = T * T;
+    const int tile = blockIdx.x;
+    if (tile >= tab[nblk].x) return;
+    const int k = wg_block(tab, nblk, tile);
+    const int4 e = tab[k];
+    const long rbase = N * (long)tt.off[k % T];
+    const int row0 = e.y + (tile - e.x) * GR;
+    const int nrows = min(GR, e.z - row0);
+    const R *w1 = nets + k * net_stride, *b1 = w1 + W;
+    for (long idx = threadIdx.x; idx < (long)nrows * W; idx += 256) {
+        const int rr = (int)(idx / W), c = (int)(idx % W);
+        const long Rg = rbase + row0 + rr;
+        T1[Rg * W + c] = wg_tanh(rh[4 * Rg] * w1[c] + b1[c]);
+    }
+}
+
+template <typename R>
+struct GenArgs {
+    long N;
+    int T, W;
+    int K, NTOT;                          // product shape: [rows x K] . [K x NTOT]
+    const int4 *tab;
+    const R *A;                           // [rows][K] row-major (one of the activation buffers)
+    const R *nets;                        // parameter blocks, net k at nets + k * net_stride
+    long net_stride, b_off;               // B [K][NTOT] row-major at offset b_off of the block
+    R *T1, *Y2, *T2, *T3;                 // activations [rows][W | 2 W | 2 W | 4 W]
+    TypeTab tt;
+};
+
+// MODE 0: layer 2 forward   A = t1,  B = W2:    t2 = tanh(acc + b2) -> T2;  y2 = (t1,t1) + t2 -> Y2
+// MODE 1: layer 3 forward   A = y2,  B = W3:    t3 = tanh(acc + b3) -> T3   (G = (y2,y2) + t3 is formed by its readers)
+// MODE 2: layer 3 backward  A = dz3, B = W3^T:  dy2 = acc + (gG[f] + gG[f + 2 W], in Y2) -> Y2;  dz2 = dy2 (1 - t2^2) -> T2
+// MODE 3: layer 2 backward  A = dz2, B = W2^T:  dy1 = acc + dy2[e] + dy2[e + W];  dz1 = dy1 (1 - t1^2) -> T1
+template <typename R, int MODE>
+__device__ __forceinline__ void wg_epilogue(const GenArgs<R> &p, const R *__restrict__ net, long Rg, int col, R v0, R v1) {
+    using R2 = typename std::conditional<sizeof(R) == 8, double2, float2>::type;
+    const int W = p.W;
+    if (MODE == 0) {
+        const R *b2 = net + wg_off_b2(W);
+        const R t0 = wg_tanh(v0 + b2[col]), t1 = wg_tanh(v1 + b2[col + 1]);
+        const R2 y = *reinterpret_cast<const R2 *>(p.T1 + Rg * W + (col % W));
+        R2 o; o.x = t0; o.y = t1;
+        *reinterpret_cast<R2 *>(p.T2 + Rg * 2 * W + col) = o;
+        o.x += y.x; o.y += y.y;
+        *reinterpret_cast<R2 *>(p.Y2 + Rg * 2 * W + col) = o;
+    } else if (MODE == 1) {
+        const R *b3 = net + wg_off_b3(W);
+        R2 o; o.x = wg_tanh(v0 + b3[col]); o.y = wg_tanh(v1 + b3[col + 1]);
+        *reinterpret_cast<R2 *>(p.T3 + Rg * 4 * W + col) = o;
+    } else if (MODE == 2) {
+        R2 *y = reinterpret_cast<R2 *>(p.Y2 + Rg * 2 * W + col), *t = reinterpret_cast<R2 *>(p.T2 + Rg * 2 * W + col);
+        R2 d = *y;
+        const R2 t2 = *t;
+        d.x += v0; d.y += v1;
+        *y = d;
+        d.x *= (R)1 - t2.x * t2.x; d.y *= (R)1 - t2.y * t2.y;
+        *t = d;
+    } else {
+        const R2 ya = *reinterpret_cast<const R2 *>(p.Y2 + Rg * 2 * W + col), yb = *reinterpret_cast<const R2 *>(p.Y2 + Rg * 2 * W + W + col);
+        R2 *t = reinterpret_cast<R2 *>(p.T1 + Rg * W + col);
+        const R2 t1 = *t;
+        R2 d;
+        d.x = (v0 + ya.x + yb.x) * ((R)1 - t1.x * t1.x);
+        d.y = (v1 + ya.y + yb.y) * ((R)1 - t1.y * t1.y);
+        *t = d;
+    }
+}
+
+// One 128 x 128 output tile per CTA, eight warps as 4 (rows) x 2 (columns): warp tile 32 x 64.  A and B stages of K = 16 arrive
+// by cp.async (two buffers); rows past the end of the tile's block and columns past NTOT are zero-filled and never stored.
+template <typename R, int MODE>
+__global__ void __launch_bounds__(256, 1) k_wg_gemm(const __grid_constant__ GenArgs<R> p) {
+    using C = GemmCfg<R>;
+    constexpr bool F64 = sizeof(R) == 8;
+    extern __shared__ __align__(16) unsigned char wg_smem[];
+    R *sm = reinterpret_cast<R *>(wg_smem);
+    const int nblk = p.T * p.T;
+    const int ntn = (p.NTOT + GBN - 1) / GBN;
+    const int tile = blockIdx.x / ntn, n0 = (blockIdx.x % ntn) * GBN;
+    if (tile >= p.tab[nblk].x) return;
+    const int k = wg_block(p.tab, nblk, tile);
+    const int4 e = p.tab[k];
+    const long rbase = p.N * (long)p.tt.off[k % p.T];
+    const int row0 = e.y + (tile - e.x) * GR;
+    const int nrows = min(GR, e.z - row0);
+    const R *net = p.nets + k * p.net_stride;
+    const R *Ag = p.A + (rbase + row0) * (long)p.K;
+    const R *Bg = net + p.b_off + n0;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wm = warp >> 1, wn = warp & 1, g = lane >> 2, t = lane & 3;
+
+    auto load_stage = [&](int buf, int k0) {
+        R *As = sm + buf * (C::A_TILE + C::B_TILE), *Bs = As + C::A_TILE;
+        constexpr int AV = GBK / C::EPV, BV = GBN / C::EPV;       // 16-byte vectors per A row / per B row
+#pragma unroll
+        for (int q = 0; q < GR * AV / 256; ++q) {
+            const int idx = tid + q * 256, r = idx / AV, kv = (idx % AV) * C::EPV;
+            const bool ok = r < nrows;
+            cp_async16(As + r * GA_STRIDE + kv, Ag + (ok ? (long)r * p.K + k0 + kv : 0), ok);
+        }
+#pragma unroll
+        for (int q = 0; q < GBK * BV / 256; ++q) {
+            const int idx = tid + q * 256, kk = idx / BV, nv = (idx % BV) * C::EPV;
+            const bool ok = n0 + nv < p.NTOT;
+            cp_async16(Bs + kk * C::BS + nv, Bg + (ok ? (long)(k0 + kk) * p.NTOT + nv : 0), ok);
+        }
+        cp_async_commit();
+    };
+
+    constexpr int NACC = 64;                     // fp64: 4 x 8 fragments of 2; fp32: 2 x 8 fragments of 4
+    R acc[NACC];
+#pragma unroll
+    for (int q = 0; q < NACC; ++q) acc[q] = (R)0;
+
+    const int nk = p.K / GBK;
+    load_stage(0, 0);
+    for (int ks = 0; ks < nk; ++ks) {
+        if (ks + 1 < nk) { load_stage((ks + 1) & 1, (ks + 1) * GBK); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
+        __syncthreads();
+        const R *As = sm + (ks & 1) * (C::A_TILE + C::B_TILE), *Bs = As + C::A_TILE;
+        if constexpr (F64) {
+#pragma unroll
+            for (int kk = 0; kk < GBK / 4; ++kk) {
+                double a[4], b[8];
+#pragma unroll
+                for (int mi = 0; mi < 4; ++mi) a[mi] = As[(32 * wm + 8 * mi + g) * GA_STRIDE + 4 * kk + t];
+#pragma unroll
+                for (int ni = 0; ni < 8; ++ni) b[ni] = Bs[(4 * kk + t) * C::BS + 64 * wn + 8 * ni + g];
+#pragma unroll
+                for (int mi = 0; mi < 4; ++mi)
+#pragma unroll
+                    for (int ni = 0; ni < 8; ++ni) dmma(acc[2 * (mi * 8 + ni)], acc[2 * (mi * 8 + ni) + 1], a[mi], b[ni]);
+            }
+        } else {
+#pragma unroll
+            for (int kk = 0; kk < GBK / 8; ++kk) {
+                uint32_t ab[2][4], as[2][4], bb[8][2], bs[8][2];
+#pragma unroll
+                for (int mi = 0; mi < 2; ++mi) {
+                    const float *ap = As + (32 * wm + 16 * mi + g) * GA_STRIDE + 8 * kk + t;
+                    split_tf32(ap[0], ab[mi][0], as[mi][0]);
+                    split_tf32(ap[8 * GA_STRIDE], ab[mi][1], as[mi][1]);
+                    split_tf32(ap[4], ab[mi][2], as[mi][2]);
+                    split_tf32(ap[8 * GA_STRIDE + 4], ab[mi][3], as[mi][3]);
+                }
+#pragma unroll
+                for (int ni = 0; ni < 8; ++ni) {
+                    const float *bp = Bs + (8 * kk + t) * C::BS + 64 * wn + 8 * ni + g;
+                    split_tf32(bp[0], bb[ni][0], bs[ni][0]);
+                    split_tf32(bp[4 * C::BS], bb[ni][1], bs[ni][1]);
+                }
+#pragma unroll
+                for (int mi = 0; mi < 2; ++mi)
+#pragma unroll
+                    for (int ni = 0; ni < 8; ++ni) {
+                        float *c = &acc[4 * (mi * 8 + ni)];
+                        mma_tf32(c, as[mi], bb[ni]);          // small terms first
+                        mma_tf32(c, ab[mi], bs[ni]);
+                        mma_tf32(c, ab[mi], bb[ni]);
+                    }
+            }
+        }
+        __syncthreads();
+    }
+
+    // epilogue: pairs of adjacent columns
+    if constexpr (F64) {
+#pragma unroll
+        for (int mi = 0; mi < 4; ++mi) {
+            const int r = 32 * wm + 8 * mi + g;
+            if (r >= nrows) continue;
+#pragma unroll
+            for (int ni = 0; ni < 8; ++ni) {
+                const int col = n0 + 64 * wn + 8 * ni + 2 * t;
+                if (col < p.NTOT) wg_epilogue<R, MODE>(p, net, rbase + row0 + r, col, acc[2 * (mi * 8 + ni)], acc[2 * (mi * 8 + ni) + 1]);
+            }
+        }
+    } else {
+#pragma unroll
+        for (int mi = 0; mi < 2; ++mi)
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int r = 32 * wm + 16 * mi + 8 * h + g;
+                if (r >= nrows) continue;
+#pragma unroll
+                for (int ni = 0; ni < 8; ++ni) {
+                    const int col = n0 + 64 * wn + 8 * ni + 2 * t;
+                    if (col < p.NTOT) wg_epilogue<R, MODE>(p, net, rbase + row0 + r, col, acc[4 * (mi * 8 + ni) + 2 * h], acc[4 * (mi * 8 + ni) + 2 * h + 1]);
+                }
+            }
+    }
+}
+
+// S5: A_i[c][m] = (1 / Nm) sum over the atom's rows of wt R^[c] G[m], G[m] = y2[m mod 2 W] + t3[m]; wt = the number of padded
+// slots a representative row stands for, 1 for a real row.  One thread per column m.
+template <typename R>
+__global__ void __launch_bounds__(256)
+k_wg_contract(long N, int T, int W, R inv_nm, const __grid_constant__ TypeTab tt, const int *__restrict__ rowstart,
+              const R *__restrict__ rh, const int2 *__restrict__ rows_id, const R *__restrict__ Y2, const R *__restrict__ T3,
+              R *__restrict__ Aout) {
+    const long i = blockIdx.x;
+    const int m = blockIdx.y * 256 + threadIdx.x, f = m % (2 * W), M2 = 4 * W;
+    R acc[4] = {(R)0, (R)0, (R)0, (R)0};
+    for (int b = 0; b < T; ++b) {
+        const int r0 = rowstart[(long)b * (N + 1) + i], r1 = rowstart[(long)b * (N + 1) + i + 1];
+        const long base = N * (long)tt.off[b];
+#pragma unroll 4
+        for (int row = r0; row < r1; ++row) {
+            const long Rg = base + row;
+            const int jj = rows_id[Rg].y;
+            const R wt = jj < 0 ? (R)(-jj) : (R)1;
+            const R G = (Y2[Rg * 2 * W + f] + T3[Rg * M2 + m]) * wt;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) acc[c] += rh[4 * Rg + c] * G;
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < 4; ++c) Aout[(i * 4 + c) * M2 + m] = acc[c] * inv_nm;
+}
+
+// Head of the backward pass; one CTA per atom, one warp per row, a lane per pair of columns (f, f + 2 W):
+//   gG[m]  = (1 / Nm) sum_c R^[c] gA[c][m]       gradient of E with respect to G of a real row
+//   dz3    = gG (1 - t3^2)                       -> over t3 (A operand of gemm<2>)
+//   gG[f] + gG[f + 2 W]                          -> over y2 (the skip connection's share of dy2, added in the epilogue of gemm<2>)
+//   dR^[c] = (1 / Nm) sum_m G[m] gA[c][m]        -> dR
+// The representative of the padded slots carries no gradient (R~ = 0 there is a constant): its rows are zeroed.
+template <typename R>
+__global__ void __launch_bounds__(256)
+k_wg_bwd_head(long N, int T, int W, R inv_nm, const __grid_constant__ TypeTab tt, const int *__restrict__ rowstart,
+              const R *__restrict__ rh, const int2 *__restrict__ rows_id, const R *__restrict__ gA, R *__restrict__ Y2,
+              R *__restrict__ T3, R *__restrict__ dR) {
+    const long i = blockIdx.x;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, M2 = 4 * W;
+    const R *ga = gA + i * 4L * M2;
+    for (int b = 0; b < T; ++b) {
+        const int r0 = rowstart[(long)b * (N + 1) + i], r1 = rowstart[(long)b * (N + 1) + i + 1];
+        const long base = N * (long)tt.off[b];
+        for (int row = r0 + warp; row < r1; row += 8) {
+            const long Rg = base + row;
+            R *y2 = Y2 + Rg * 2 * W, *t3 = T3 + Rg * M2;
+            if (rows_id[Rg].y < 0) {
+                for (int f = lane; f < 2 * W; f += 32) { y2[f] = (R)0; t3[f] = (R)0; t3[f + 2 * W] = (R)0; }
+                if (lane < 4) dR[4 * Rg + lane] = (R)0;
+                continue;
+            }
+            R r[4], acc[4] = {(R)0, (R)0, (R)0, (R)0};
+#pragma unroll
+            for (int c = 0; c < 4; ++c) r[c] = rh[4 * Rg + c] * inv_nm;
+            for (int f = lane; f < 2 * W; f += 32) {
+                const R y = y2[f], ta = t3[f], tb = t3[f + 2 * W];
+                const R Ga = y + ta, Gb = y + tb;
+                R gGa = (R)0, gGb = (R)0;
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const R a = ga[c * M2 + f], bq = ga[c * M2 + 2 * W + f];
+                    gGa += r[c] * a; gGb += r[c] * bq;
+                    acc[c] += Ga * a + Gb * bq;
+                }
+                t3[f] = gGa * ((R)1 - ta * ta);
+                t3[f + 2 * W] = gGb * ((R)1 - tb * tb);
+                y2[f] = gGa + gGb;
+            }
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], o);
+            }
+            if (lane == 0) {
+#pragma unroll
+                for (int c = 0; c < 4; ++c) dR[4 * Rg + c] = acc[c] * inv_nm;
+            }
+        }
+    }
+}
+
+// Layer 1 backward and the normalisation: ds^ = dz1 . w1 (dz1 in T1 after gemm<3>); dE/dR~[c] = (dR^[c] + [c = 0] ds^) / std[c],
+// written over dR.  One CTA per tile, one warp per row.
+template <typename R>
+__global__ void __launch_bounds__(256)
+k_wg_ds(long N, int T, int W, const __grid_constant__ TypeTab tt, const int4 *__restrict__ tab, const R *__restrict__ nets,
+        long net_stride, const double *__restrict__ stdv, const R *__restrict__ T1, R *__restrict__ dR) {
+    const int nblk = T * T;
+    const int tile = blockIdx.x;
+    if (tile >= tab[nblk].x) return;
+    const int k = wg_block(tab, nblk, tile);
+    const int4 e = tab[k];
+    const long rbase = N * (long)tt.off[k % T];
+    const int row0 = e.y + (tile - e.x) * GR;
+    const int nrows = min(GR, e.z - row0);
+    const R *w1 = nets + k * net_stride;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, a = k / T;
+    for (int rr = warp; rr < nrows; rr += 8) {
+        const long Rg = rbase + row0 + rr;
+        R ds = (R)0;
+        for (int c = lane; c < W; c += 32) ds += T1[Rg * W + c] * w1[c];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) ds += __shfl_xor_sync(0xffffffffu, ds, o);
+        if (lane < 4) dR[4 * Rg + lane] = (R)(((double)dR[4 * Rg + lane] + (lane == 0 ? (double)ds : 0.0)) / stdv[4 * a + lane]);
+    }
+}
+
+// S8 + S9: per real row, the geometry derivative N9 in fp64, F_i += g, F_j -= g, Xi_ab -= d_a g_b (Q18)
+template <typename R>
+__global__ void __launch_bounds__(256)
+k_wg_force(long N, int b, long row_off, EnvParams ep, const int *__restrict__ rowstart, const int2 *__restrict__ rows_id,
+           const R *__restrict__ gR, const double *__restrict__ xs, double *__restrict__ fsorted, double *__restrict__ virial) {
+    const long row = blockIdx.x * 256L + threadIdx.x;
+    const int nrow = rowstart[(long)b * (N + 1) + N];
+    double vir[9];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) vir[k] = 0.0;
+    if (row < nrow) {
+        const long Rg = row_off + row;
+        const int2 id = rows_id[Rg];
+        if (id.y >= 0) {
+            const long i = id.x, j = id.y;
+            const double dx = min_image(xs[3 * j] - xs[3 * i], ep.L[0], 0.5 * ep.L[0]);
+            const double dy = min_image(xs[3 * j + 1] - xs[3 * i + 1], ep.L[1], 0.5 * ep.L[1]);
+            const double dz = min_image(xs[3 * j + 2] - xs[3 * i + 2], ep.L[2], 0.5 * ep.L[2]);
+            double Rt[4], sp, rl;
+            env_row(ep, dx, dy, dz, Rt, &sp, &rl);
+            const double s = Rt[0];
+            const double g0 = (double)gR[4 * Rg], g1 = (double)gR[4 * Rg + 1], g2 = (double)gR[4 * Rg + 2], g3 = (double)gR[4 * Rg + 3];
+            const double d[3] = {dx, dy, dz};
+            const double gd = g1 * dx + g2 * dy + g3 * dz;
+            const double coef = (sp / rl - s / (rl * rl)) / rl;
+#pragma unroll
+            for (int bb = 0; bb < 3; ++bb) {
+                const double gk = g0 * sp * d[bb] / rl + coef * d[bb] * gd + (s / rl) * (bb == 0 ? g1 : (bb == 1 ? g2 : g3));
+                atomicAdd(&fsorted[3 * i + bb], gk);
+                atomicAdd(&fsorted[3 * j + bb], -gk);
+#pragma unroll
+                for (int aa = 0; aa < 3; ++aa) vir[3 * aa + bb] -= d[aa] * gk;
+            }
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < 9; ++k) {
+        double v = vir[k];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if ((threadIdx.x & 31) == 0 && v != 0.0) atomicAdd(&virial[k], v);
+    }
+}
+
+}  // namespace
+
+// ---- host side -------------------------------------------------------------------------------------------------------------
+
+size_t wide_gen_net_elems(int W) { return 8 * (size_t)W + 20 * (size_t)W * W; }
+
+// net: w1[W] b1[W] W2[W][2W] b2[2W] W3[2W][4W] b3[4W] (dp_weights order) -> the parameter block of the kernels above
+template <typename R>
+static void build_net(int W, const double *net, R *out) {
+    const double *w1 = net, *b1 = w1 + W, *W2 = b1 + W, *b2 = W2 + (size_t)W * 2 * W, *W3 = b2 + 2 * W, *b3 = W3 + (size_t)2 * W * 4 * W;
+    for (int e = 0; e < W; ++e) { out[e] = (R)w1[e]; out[W + e] = (R)b1[e]; }
+    for (int f = 0; f < 2 * W; ++f) out[wg_off_b2(W) + f] = (R)b2[f];
+    for (int m = 0; m < 4 * W; ++m) out[wg_off_b3(W) + m] = (R)b3[m];
+    for (int e = 0; e < W; ++e)
+        for (int f = 0; f < 2 * W; ++f) {
+            out[wg_off_W2(W) + (size_t)e * 2 * W + f] = (R)W2[(size_t)e * 2 * W + f];
+            out[wg_off_W2T(W) + (size_t)f * W + e] = (R)W2[(size_t)e * 2 * W + f];
+        }
+    for (int f = 0; f < 2 * W; ++f)
+        for (int m = 0; m < 4 * W; ++m) {
+            out[wg_off_W3(W) + (size_t)f * 4 * W + m] = (R)W3[(size_t)f * 4 * W + m];
+            out[wg_off_W3T(W) + (size_t)m * 2 * W + f] = (R)W3[(size_t)f * 4 * W + m];
+        }
+}
+void wide_gen_build_net(int W, bool f64, const double *net, void *out) {
+    if (f64) build_net<double>(W, net, (double *)out); else build_net<float>(W, net, (float *)out);
+}
+
+template <typename R>
+static GenArgs<R> gen_args(const dp_model *m, long N, char *ws, const WsLayout &L) {
+    GenArgs<R> p{};
+    p.N = N; p.T = m->T; p.W = m->m0;
+    p.tab = (const int4 *)(ws + L.wide_tab);
+    p.nets = (const R *)m->wide_vec_dev; p.net_stride = (long)wide_gen_net_elems(m->m0);
+    p.T1 = (R *)(ws + L.wide_t1); p.Y2 = (R *)(ws + L.wide_y2); p.T2 = (R *)(ws + L.wide_t2); p.T3 = (R *)(ws + L.wide_t3);
+    p.tt = make_typetab(m);
+    return p;
+}
+
+template <typename R, int MODE>
+static cudaError_t gen_gemm(const dp_model *m, long N, GenArgs<R> p, int K, int Nn, const R *A, long b_off, cudaStream_t st) {
+    DP_SMEM_OPTIN((k_wg_gemm<R, MODE>), GemmCfg<R>::SMEM);
+    p.K = K; p.NTOT = Nn; p.A = A; p.b_off = b_off;
+    const long tiles = wide_tiles_cap(m, N), ntn = (Nn + GBN - 1) / GBN;
+    k_wg_gemm<R, MODE><<<(unsigned)(tiles * ntn), 256, GemmCfg<R>::SMEM, st>>>(p);
+    return cudaGetLastError();
+}
+
+template <typename R>
+static cudaError_t fwd_gen(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    const int W = m->m0, T = m->T;
+    const TypeTab tt = make_typetab(m);
+    cudaError_t e = cudaSuccess;
+    auto ok = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
+    const GenArgs<R> p = gen_args<R>(m, N, ws, L);
+    R *rh = (R *)(ws + L.wide_rh);
+    int2 *rows_id = (int2 *)(ws + L.rows_id);
+    const int *rowstart = (const int *)(ws + L.rowstart);
+    k_wg_env<R><<<(unsigned)((N + 7) / 8), 256, 0, st>>>(N, T, g.ncell, m->Nm, tt, make_env(m, g), m->avg_dev, m->std_dev,
+                                                         (const int *)(ws + L.bin_start), (const double *)(ws + L.xs),
+                                                         (const int *)(ws + L.nlist), (const int *)(ws + L.nreal), rowstart, rh, rows_id);
+    ok(cudaGetLastError());
+    ok(launch_wide_tiles(m, N, g, ws, L, st));
+    const unsigned tiles = (unsigned)wide_tiles_cap(m, N);
+    k_wg_l1<R><<<tiles, 256, 0, st>>>(N, T, W, tt, p.tab, p.nets, p.net_stride, rh, p.T1);
+    ok(cudaGetLastError());
+    ok((gen_gemm<R, 0>(m, N, p, W, 2 * W, p.T1, wg_off_W2(W), st)));
+    ok((gen_gemm<R, 1>(m, N, p, 2 * W, 4 * W, p.Y2, wg_off_W3(W), st)));
+    k_wg_contract<R><<<dim3((unsigned)N, (unsigned)(4 * W / 256)), 256, 0, st>>>(N, T, W, (R)(1.0 / (double)m->Nm), tt, rowstart, rh, rows_id,
+                                                                              p.Y2, p.T3, (R *)(ws + L.A));
+    ok(cudaGetLastError());
+    return e;
+}
+
+template <typename R>
+static cudaError_t bwd_gen(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    const int W = m->m0, T = m->T;
+    const TypeTab tt = make_typetab(m);
+    cudaError_t e = cudaSuccess;
+    auto ok = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
+    const GenArgs<R> p = gen_args<R>(m, N, ws, L);
+    const R *rh = (const R *)(ws + L.wide_rh);
+    R *dR = (R *)(ws + L.wide_gr);
+    const int2 *rows_id = (const int2 *)(ws + L.rows_id);
+    const int *rowstart = (const int *)(ws + L.rowstart);
+    // gA [N][4][m2]: FP64 from k_gA_wide (fit_f64.cu), MIX-32 left in the gD buffer by the last fitting product (fit_tc.cu MODE 6)
+    const R *gA = sizeof(R) == 8 ? (const R *)(ws + L.gAf) : (const R *)(ws + L.gD);
+    k_wg_bwd_head<R><<<(unsigned)N, 256, 0, st>>>(N, T, W, (R)(1.0 / (double)m->Nm), tt, rowstart, rh, rows_id, gA, p.Y2, p.T3, dR);
+    ok(cudaGetLastError());
+    if (m->profile) cudaEventRecord(m->ev[6], st);      // ev[6] .. ev[7]: the two backward GEMMs
+    ok((gen_gemm<R, 2>(m, N, p, 4 * W, 2 * W, p.T3, wg_off_W3T(W), st)));
+    ok((gen_gemm<R, 3>(m, N, p, 2 * W, W, p.T2, wg_off_W2T(W), st)));
+    if (m->profile) cudaEventRecord(m->ev[7], st);
+    const unsigned tiles = (unsigned)wide_tiles_cap(m, N);
+    k_wg_ds<R><<<tiles, 256, 0, st>>>(N, T, W, tt, p.tab, p.nets, p.net_stride, m->std_dev, p.T1, dR);
+    ok(cudaGetLastError());
+    for (int b = 0; b < T; ++b) {
+        const long cap = N * (long)m->sel[b];
+        k_wg_force<R><<<(unsigned)((cap + 255) / 256), 256, 0, st>>>(N, b, N * (long)m->off[b], make_env(m, g), rowstart, rows_id, dR,
+                                                                    (const double *)(ws + L.xs), (double *)(ws + L.fsorted),
+                                                                    (double *)(ws + L.virial));
+        ok(cudaGetLastError());
+    }
+    return e;
+}
+
+cudaError_t launch_embed_fwd_wide_gen(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    return m->prec == DP_FP64 ? fwd_gen<double>(m, N, g, ws, L, st) : fwd_gen<float>(m, N, g, ws, L, st);
+}
+cudaError_t launch_embed_bwd_wide_gen(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st) {
+    return m->prec == DP_FP64 ? bwd_gen<double>(m, N, g, ws, L, st) : bwd_gen<float>(m, N, g, ws, L, st);
+}
