@@ -466,7 +466,7 @@ int dp_create(dp_model **out, const dp_weights *w, const int *type_map, int n_ty
     ok(upload(tm, (void **)&m->type_map_dev));
     const size_t ensz = (size_t)W0 + W0 + (size_t)W0 * 2 * W0 + 2 * W0 + (size_t)2 * W0 * 4 * W0 + 4 * W0;
     if (wide && prec != DP_MIX16) {     // wide nets in FP64 / MIX-32: row-major weights and their transposes (wide_gen.cu)
-        const size_t ne = wide_gen_net_elems(W0), esz = prec == DP_FP64 ? 8 : 4;
+        const size_t ne = wide_gen_net_elems(W0, prec == DP_FP64), esz = prec == DP_FP64 ? 8 : 4;
         std::vector<char> blk((size_t)T * T * ne * esz);
         for (int ab = 0; ab < T * T; ++ab) wide_gen_build_net(W0, prec == DP_FP64, w->embed + ab * ensz, &blk[(size_t)ab * ne * esz]);
         ok(upload(blk, &m->wide_vec_dev));
@@ -685,7 +685,7 @@ int dp_profile_read(dp_model *m, double *ms_host) {
         ms_host[k] = ms;
     }
     ms_host[5] = ms_host[3];
-    if (m->prec == DP_MIX16) {
+    if (m->prec == DP_MIX16 || m->wide_gen) {
         float ms = 0.f;
         if (cudaEventElapsedTime(&ms, m->ev[6], m->ev[7]) != cudaSuccess) return DP_ECUDA;
         ms_host[5] = ms;

@@ -226,7 +226,7 @@ cudaError_t launch_wide_tiles(const dp_model *m, long N, const Grid3 &g, char *w
 // wide networks in FP64 and MIX-32 (wide_gen.cu)
 cudaError_t launch_embed_fwd_wide_gen(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
 cudaError_t launch_embed_bwd_wide_gen(const dp_model *m, long N, const Grid3 &g, char *ws, const WsLayout &L, cudaStream_t st);
-size_t wide_gen_net_elems(int W);
+size_t wide_gen_net_elems(int W, bool f64);
 void wide_gen_build_net(int W, bool f64, const double *net, void *out);
 size_t fit_tc32_type_elems(int nd);
 void fit_tc32_build_type(int nd, const double *V1, struct __half *out);

@@ -17,6 +17,7 @@
 // Backward: k_wg_bwd_head (gG = R^ gA / Nm, dz3, skip share of dy2, dR^ = G gA^T / Nm) -> gemm<2> (dy2, dz2) -> gemm<3> (dz1)
 //           -> k_wg_ds (ds^ = dz1 . w1, dE/dR~ = (dR^ + ds^ e0) / std) -> k_wg_force (N9 geometry derivative, ProdForce,
 //           ProdViral).
+#include <cstring>
 #include <type_traits>
 #include <vector>
 #include "dp_internal.h"
@@ -25,11 +26,12 @@
 namespace {
 
 constexpr int GR = 128;                     // rows per tile (= the tile table's, wide.cu)
-constexpr int GBN = 128, GBK = 16;          // N tile, K step
-constexpr int GA_STRIDE = GBK + 4;          // A tile [128][20]: fragment loads hit distinct banks (fp64: per half warp)
+constexpr int GBN = 128, GBK = 32;          // N tile, K step
+constexpr int GA_STRIDE = GBK + 4;          // A tile [128][36]: fragment loads hit distinct banks (fp64: per half warp)
 template <typename R> struct GemmCfg {
-    static constexpr int BS = sizeof(R) == 8 ? GBN + 4 : GBN + 8;       // B tile [16][BS]
-    static constexpr int A_TILE = GR * GA_STRIDE, B_TILE = GBK * BS;
+    static constexpr int BS = sizeof(R) == 8 ? GBN + 4 : GBN + 8;       // B tile [32][BS]; fp32: two of them (TF32 value, remainder)
+    static constexpr int NB = sizeof(R) == 8 ? 1 : 2;
+    static constexpr int A_TILE = GR * GA_STRIDE, B_TILE = NB * GBK * BS;
     static constexpr int SMEM = 2 * (A_TILE + B_TILE) * (int)sizeof(R);
     static constexpr int EPV = 16 / (int)sizeof(R);                     // elements per 16-byte cp.async
 };
@@ -176,6 +178,7 @@ struct GenArgs {
     const R *A;                           // [rows][K] row-major (one of the activation buffers)
     const R *nets;                        // parameter blocks, net k at nets + k * net_stride
     long net_stride, b_off;               // B [K][NTOT] row-major at offset b_off of the block
+    long b_small;                         // fp32: distance from a weight matrix to the matrix of its TF32 remainders
     R *T1, *Y2, *T2, *T3;                 // activations [rows][W | 2 W | 2 W | 4 W]
     TypeTab tt;
 };
@@ -184,45 +187,60 @@ struct GenArgs {
 // MODE 1: layer 3 forward   A = y2,  B = W3:    t3 = tanh(acc + b3) -> T3   (G = (y2,y2) + t3 is formed by its readers)
 // MODE 2: layer 3 backward  A = dz3, B = W3^T:  dy2 = acc + (gG[f] + gG[f + 2 W], in Y2) -> Y2;  dz2 = dy2 (1 - t2^2) -> T2
 // MODE 3: layer 2 backward  A = dz2, B = W2^T:  dy1 = acc + dy2[e] + dy2[e + W];  dz1 = dy1 (1 - t1^2) -> T1
+// The epilogue of one pair of adjacent columns, in two steps so that the kernel can issue the loads of several pairs before the
+// first store (the activation pointers may alias as far as the compiler knows: interleaved, every load would wait for the store
+// before it).
+template <typename R> struct EpiAux { typename std::conditional<sizeof(R) == 8, double2, float2>::type a, b, c; };
+
 template <typename R, int MODE>
-__device__ __forceinline__ void wg_epilogue(const GenArgs<R> &p, const R *__restrict__ net, long Rg, int col, R v0, R v1) {
+__device__ __forceinline__ EpiAux<R> wg_epi_load(const GenArgs<R> &p, const R *__restrict__ net, long Rg, int col) {
     using R2 = typename std::conditional<sizeof(R) == 8, double2, float2>::type;
     const int W = p.W;
+    EpiAux<R> x;
     if (MODE == 0) {
-        const R *b2 = net + wg_off_b2(W);
-        const R t0 = wg_tanh(v0 + b2[col]), t1 = wg_tanh(v1 + b2[col + 1]);
-        const R2 y = *reinterpret_cast<const R2 *>(p.T1 + Rg * W + (col % W));
-        R2 o; o.x = t0; o.y = t1;
+        x.a = *reinterpret_cast<const R2 *>(net + wg_off_b2(W) + col);
+        x.b = *reinterpret_cast<const R2 *>(p.T1 + Rg * W + (col % W));
+    } else if (MODE == 1) {
+        x.a = *reinterpret_cast<const R2 *>(net + wg_off_b3(W) + col);
+    } else if (MODE == 2) {
+        x.a = *reinterpret_cast<const R2 *>(p.Y2 + Rg * 2 * W + col);
+        x.b = *reinterpret_cast<const R2 *>(p.T2 + Rg * 2 * W + col);
+    } else {
+        x.a = *reinterpret_cast<const R2 *>(p.Y2 + Rg * 2 * W + col);
+        x.b = *reinterpret_cast<const R2 *>(p.Y2 + Rg * 2 * W + W + col);
+        x.c = *reinterpret_cast<const R2 *>(p.T1 + Rg * W + col);
+    }
+    return x;
+}
+template <typename R, int MODE>
+__device__ __forceinline__ void wg_epi_store(const GenArgs<R> &p, long Rg, int col, R v0, R v1, const EpiAux<R> &x) {
+    using R2 = typename std::conditional<sizeof(R) == 8, double2, float2>::type;
+    const int W = p.W;
+    R2 o;
+    if (MODE == 0) {
+        o.x = wg_tanh(v0 + x.a.x); o.y = wg_tanh(v1 + x.a.y);
         *reinterpret_cast<R2 *>(p.T2 + Rg * 2 * W + col) = o;
-        o.x += y.x; o.y += y.y;
+        o.x += x.b.x; o.y += x.b.y;
         *reinterpret_cast<R2 *>(p.Y2 + Rg * 2 * W + col) = o;
     } else if (MODE == 1) {
-        const R *b3 = net + wg_off_b3(W);
-        R2 o; o.x = wg_tanh(v0 + b3[col]); o.y = wg_tanh(v1 + b3[col + 1]);
+        o.x = wg_tanh(v0 + x.a.x); o.y = wg_tanh(v1 + x.a.y);
         *reinterpret_cast<R2 *>(p.T3 + Rg * 4 * W + col) = o;
     } else if (MODE == 2) {
-        R2 *y = reinterpret_cast<R2 *>(p.Y2 + Rg * 2 * W + col), *t = reinterpret_cast<R2 *>(p.T2 + Rg * 2 * W + col);
-        R2 d = *y;
-        const R2 t2 = *t;
-        d.x += v0; d.y += v1;
-        *y = d;
-        d.x *= (R)1 - t2.x * t2.x; d.y *= (R)1 - t2.y * t2.y;
-        *t = d;
+        o.x = x.a.x + v0; o.y = x.a.y + v1;
+        *reinterpret_cast<R2 *>(p.Y2 + Rg * 2 * W + col) = o;
+        o.x *= (R)1 - x.b.x * x.b.x; o.y *= (R)1 - x.b.y * x.b.y;
+        *reinterpret_cast<R2 *>(p.T2 + Rg * 2 * W + col) = o;
     } else {
-        const R2 ya = *reinterpret_cast<const R2 *>(p.Y2 + Rg * 2 * W + col), yb = *reinterpret_cast<const R2 *>(p.Y2 + Rg * 2 * W + W + col);
-        R2 *t = reinterpret_cast<R2 *>(p.T1 + Rg * W + col);
-        const R2 t1 = *t;
-        R2 d;
-        d.x = (v0 + ya.x + yb.x) * ((R)1 - t1.x * t1.x);
-        d.y = (v1 + ya.y + yb.y) * ((R)1 - t1.y * t1.y);
-        *t = d;
+        o.x = (v0 + x.a.x + x.b.x) * ((R)1 - x.c.x * x.c.x);
+        o.y = (v1 + x.a.y + x.b.y) * ((R)1 - x.c.y * x.c.y);
+        *reinterpret_cast<R2 *>(p.T1 + Rg * W + col) = o;
     }
 }
 
 // One 128 x 128 output tile per CTA, eight warps as 4 (rows) x 2 (columns): warp tile 32 x 64.  A and B stages of K = 16 arrive
 // by cp.async (two buffers); rows past the end of the tile's block and columns past NTOT are zero-filled and never stored.
 template <typename R, int MODE>
-__global__ void __launch_bounds__(256, 1) k_wg_gemm(const __grid_constant__ GenArgs<R> p) {
+__global__ void __launch_bounds__(256, sizeof(R) == 8 ? 1 : 2) k_wg_gemm(const __grid_constant__ GenArgs<R> p) {
     using C = GemmCfg<R>;
     constexpr bool F64 = sizeof(R) == 8;
     extern __shared__ __align__(16) unsigned char wg_smem[];
@@ -256,6 +274,8 @@ __global__ void __launch_bounds__(256, 1) k_wg_gemm(const __grid_constant__ GenA
             const int idx = tid + q * 256, kk = idx / BV, nv = (idx % BV) * C::EPV;
             const bool ok = n0 + nv < p.NTOT;
             cp_async16(Bs + kk * C::BS + nv, Bg + (ok ? (long)(k0 + kk) * p.NTOT + nv : 0), ok);
+            if constexpr (!F64)     // the remainders of the weights (split once, by dp_create)
+                cp_async16(Bs + GBK * C::BS + kk * C::BS + nv, Bg + p.b_small + (ok ? (long)(k0 + kk) * p.NTOT + nv : 0), ok);
         }
         cp_async_commit();
     };
@@ -287,7 +307,7 @@ __global__ void __launch_bounds__(256, 1) k_wg_gemm(const __grid_constant__ GenA
         } else {
 #pragma unroll
             for (int kk = 0; kk < GBK / 8; ++kk) {
-                uint32_t ab[2][4], as[2][4], bb[8][2], bs[8][2];
+                uint32_t ab[2][4], as[2][4];
 #pragma unroll
                 for (int mi = 0; mi < 2; ++mi) {
                     const float *ap = As + (32 * wm + 16 * mi + g) * GA_STRIDE + 8 * kk + t;
@@ -298,49 +318,41 @@ __global__ void __launch_bounds__(256, 1) k_wg_gemm(const __grid_constant__ GenA
                 }
 #pragma unroll
                 for (int ni = 0; ni < 8; ++ni) {
-                    const float *bp = Bs + (8 * kk + t) * C::BS + 64 * wn + 8 * ni + g;
-                    split_tf32(bp[0], bb[ni][0], bs[ni][0]);
-                    split_tf32(bp[4 * C::BS], bb[ni][1], bs[ni][1]);
+                    const uint32_t *bp = reinterpret_cast<const uint32_t *>(Bs) + (8 * kk + t) * C::BS + 64 * wn + 8 * ni + g;
+                    const uint32_t bb[2] = {bp[0], bp[4 * C::BS]}, bs[2] = {bp[GBK * C::BS], bp[GBK * C::BS + 4 * C::BS]};
+                    // small terms first
+                    mma_tf32(&acc[4 * ni], as[0], bb);
+                    mma_tf32(&acc[4 * (8 + ni)], as[1], bb);
+                    mma_tf32(&acc[4 * ni], ab[0], bs);
+                    mma_tf32(&acc[4 * (8 + ni)], ab[1], bs);
+                    mma_tf32(&acc[4 * ni], ab[0], bb);
+                    mma_tf32(&acc[4 * (8 + ni)], ab[1], bb);
                 }
-#pragma unroll
-                for (int mi = 0; mi < 2; ++mi)
-#pragma unroll
-                    for (int ni = 0; ni < 8; ++ni) {
-                        float *c = &acc[4 * (mi * 8 + ni)];
-                        mma_tf32(c, as[mi], bb[ni]);          // small terms first
-                        mma_tf32(c, ab[mi], bs[ni]);
-                        mma_tf32(c, ab[mi], bb[ni]);
-                    }
             }
         }
         __syncthreads();
     }
 
-    // epilogue: pairs of adjacent columns
-    if constexpr (F64) {
+    // epilogue: pairs of adjacent columns, eight pairs of one row at a time (loads first)
+    constexpr int NROWSETS = 4;
 #pragma unroll
-        for (int mi = 0; mi < 4; ++mi) {
-            const int r = 32 * wm + 8 * mi + g;
-            if (r >= nrows) continue;
+    for (int rs = 0; rs < NROWSETS; ++rs) {
+        // fp64: fragment row set mi = rs (rows 8 mi + g); fp32: mi = rs / 2, half h = rs % 2 (rows 16 mi + 8 h + g)
+        const int r = F64 ? 32 * wm + 8 * rs + g : 32 * wm + 16 * (rs >> 1) + 8 * (rs & 1) + g;
+        if (r >= nrows) continue;
+        const long Rg = rbase + row0 + r;
+        EpiAux<R> aux[8];
 #pragma unroll
-            for (int ni = 0; ni < 8; ++ni) {
-                const int col = n0 + 64 * wn + 8 * ni + 2 * t;
-                if (col < p.NTOT) wg_epilogue<R, MODE>(p, net, rbase + row0 + r, col, acc[2 * (mi * 8 + ni)], acc[2 * (mi * 8 + ni) + 1]);
-            }
+        for (int ni = 0; ni < 8; ++ni) {
+            const int col = n0 + 64 * wn + 8 * ni + 2 * t;
+            if (col < p.NTOT) aux[ni] = wg_epi_load<R, MODE>(p, net, Rg, col);
         }
-    } else {
 #pragma unroll
-        for (int mi = 0; mi < 2; ++mi)
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int r = 32 * wm + 16 * mi + 8 * h + g;
-                if (r >= nrows) continue;
-#pragma unroll
-                for (int ni = 0; ni < 8; ++ni) {
-                    const int col = n0 + 64 * wn + 8 * ni + 2 * t;
-                    if (col < p.NTOT) wg_epilogue<R, MODE>(p, net, rbase + row0 + r, col, acc[4 * (mi * 8 + ni) + 2 * h], acc[4 * (mi * 8 + ni) + 2 * h + 1]);
-                }
-            }
+        for (int ni = 0; ni < 8; ++ni) {
+            const int col = n0 + 64 * wn + 8 * ni + 2 * t;
+            const int q = F64 ? 2 * (rs * 8 + ni) : 4 * ((rs >> 1) * 8 + ni) + 2 * (rs & 1);
+            if (col < p.NTOT) wg_epi_store<R, MODE>(p, Rg, col, acc[q], acc[q + 1], aux[ni]);
+        }
     }
 }
 
@@ -500,7 +512,16 @@ k_wg_force(long N, int b, long row_off, EnvParams ep, const int *__restrict__ ro
 
 // ---- host side -------------------------------------------------------------------------------------------------------------
 
-size_t wide_gen_net_elems(int W) { return 8 * (size_t)W + 20 * (size_t)W * W; }
+// fp32 blocks carry the weight matrices twice: rounded to TF32, and the TF32 remainders (the 3xTF32 products of k_wg_gemm)
+size_t wide_gen_net_elems(int W, bool f64) { return 8 * (size_t)W + (f64 ? 20 : 40) * (size_t)W * W; }
+
+static float tf32_rna(float x) {          // cvt.rna.tf32.f32: nearest, ties away from zero, 13 low mantissa bits cleared
+    uint32_t u;
+    std::memcpy(&u, &x, 4);
+    u = (u + 0x1000u) & 0xffffe000u;
+    std::memcpy(&x, &u, 4);
+    return x;
+}
 
 // net: w1[W] b1[W] W2[W][2W] b2[2W] W3[2W][4W] b3[4W] (dp_weights order) -> the parameter block of the kernels above
 template <typename R>
@@ -521,7 +542,15 @@ static void build_net(int W, const double *net, R *out) {
         }
 }
 void wide_gen_build_net(int W, bool f64, const double *net, void *out) {
-    if (f64) build_net<double>(W, net, (double *)out); else build_net<float>(W, net, (float *)out);
+    if (f64) { build_net<double>(W, net, (double *)out); return; }
+    float *o = (float *)out;
+    build_net<float>(W, net, o);
+    const size_t m0 = 8 * (size_t)W, nm = 20 * (size_t)W * W;
+    for (size_t k = 0; k < nm; ++k) {
+        const float x = o[m0 + k], big = tf32_rna(x);
+        o[m0 + k] = big;
+        o[m0 + nm + k] = tf32_rna(x - big);
+    }
 }
 
 template <typename R>
@@ -529,7 +558,8 @@ static GenArgs<R> gen_args(const dp_model *m, long N, char *ws, const WsLayout &
     GenArgs<R> p{};
     p.N = N; p.T = m->T; p.W = m->m0;
     p.tab = (const int4 *)(ws + L.wide_tab);
-    p.nets = (const R *)m->wide_vec_dev; p.net_stride = (long)wide_gen_net_elems(m->m0);
+    p.nets = (const R *)m->wide_vec_dev; p.net_stride = (long)wide_gen_net_elems(m->m0, sizeof(R) == 8);
+    p.b_small = 20L * m->m0 * m->m0;
     p.T1 = (R *)(ws + L.wide_t1); p.Y2 = (R *)(ws + L.wide_y2); p.T2 = (R *)(ws + L.wide_t2); p.T3 = (R *)(ws + L.wide_t3);
     p.tt = make_typetab(m);
     return p;
