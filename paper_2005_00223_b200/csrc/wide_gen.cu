@@ -18,10 +18,12 @@
 //           -> k_wg_ds (ds^ = dz1 . w1, dE/dR~ = (dR^ + ds^ e0) / std) -> k_wg_force (N9 geometry derivative, ProdForce,
 //           ProdViral).
 #include <cstring>
+#include <cuda.h>          // CUtensorMap (types only: the encoder is looked up through the runtime, no libcuda link)
 #include <type_traits>
 #include <vector>
 #include "dp_internal.h"
 #include "tanh64.cuh"
+#include "tc_common.cuh"
 
 namespace {
 
@@ -356,6 +358,241 @@ __global__ void __launch_bounds__(256, sizeof(R) == 8 ? 1 : 2) k_wg_gemm(const _
     }
 }
 
+// ---- MIX-32 on the 5th-generation tensor cores: tcgen05.mma kind::tf32, three products per K step ("3xTF32") -------------------
+// C = A B with A = the fp32 activations [rows][K] and B^T = a weight matrix [NTOT][K] (both K-major operands: dp_create keeps every
+// matrix and its transpose).  Persistent, one CTA per SM, warp-specialised:
+//   warp 13    loader (one thread): per K = 16 stage ONE TMA tensor copy of A (the row-major activations seen as a
+//              (4, rows, K / 4) tensor, box {4, 128, 4}: it lands as the un-swizzled K-major operand image, per 16 bytes of K a
+//              column [128 rows][16 B]) and ONE bulk copy of the weights' operand images (TF32 values and TF32 remainders, laid
+//              out by dp_create), both counted by the stage's "landed" barrier;
+//   warps 0-7  splitters: a_big = a with the 13 low mantissa bits cleared (what the tensor core would read), in place,
+//              a_small = a - a_big (exact) into a second image; fence.proxy.async; arrive on the stage's "full" barrier;
+//   warp 12    MMA issuer: per K = 8 step a_small b_big, a_big b_small, a_big b_big into one of two 128 x BN fp32 accumulators
+//              in TMEM; tcgen05.commit frees the stage, the last one of a tile hands the accumulator over;
+//   warps 8-11 epilogue: thread = row = TMEM lane, tcgen05.ld of 16 columns at a time, the layer's bias / tanh / skip / tanh'
+//              work on the row-major fp32 activations.
+constexpr int TQ_KC = 16;                          // K per stage: 4 pieces of 16 bytes
+constexpr int TQ_NST = 4;
+constexpr int TQ_A_PIECE = 128 * 16;               // distance between the piece columns of an image (the descriptors' LBO)
+constexpr int TQ_A_IMG = 4 * TQ_A_PIECE;           // 8 KB: [4 pieces][128 rows][16 B], written by one TMA tensor copy
+constexpr int TQ_B_IMG = 256 * TQ_KC * 4;          // 16 KB (BN <= 256), un-padded: written by dp_create, one bulk copy per stage
+constexpr int TQ_STAGE = 2 * TQ_A_IMG + 2 * TQ_B_IMG;      // a_big | a_small | b_big | b_small
+constexpr int TQ_OFF_BAR = TQ_NST * TQ_STAGE;
+constexpr int TQ_TOTAL = TQ_OFF_BAR + 256;
+constexpr int TQ_THREADS = 448;                  // 8 splitter, 4 epilogue warps, the MMA warp, the loader warp
+static_assert(TQ_TOTAL + 1024 <= 227 * 1024, "shared memory budget");
+
+__device__ __forceinline__ void mma_tf32_ss(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t id, bool accumulate) {
+    asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}"
+                 ::"r"(tmem_d), "l"(da), "l"(db), "r"(id), "r"((uint32_t)accumulate) : "memory");
+}
+// kind::tf32 instruction descriptor: tf32 x tf32 -> fp32, M x N, both operands K-major
+__host__ __device__ constexpr uint32_t idesc_tf32(int M, int N) {
+    return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+__device__ __forceinline__ void mbar_expect_tx_cta(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(tc::smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s_cta(uint32_t sdst, const void *gsrc, uint32_t bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(sdst), "l"(gsrc), "r"(bytes), "r"(tc::smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_cta(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(tc::smem_u32(bar)) : "memory");
+}
+
+// box {4 elements, 128 rows, 4 pieces} of the activation tensor viewed as (4, rows, K / 4) -> the [4][128][16 B] operand image
+__device__ __forceinline__ void tma_load_3d(uint32_t sdst, const CUtensorMap *tm, int c0, int c1, int c2, uint64_t *bar) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"(sdst), "l"((uint64_t)tm), "r"(c0), "r"(c1), "r"(c2), "r"(tc::smem_u32(bar)) : "memory");
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(TQ_THREADS, 1) k_wg_gemm_tf32(const __grid_constant__ GenArgs<float> p, const __grid_constant__ CUtensorMap tmA) {
+    extern __shared__ __align__(1024) unsigned char tq_smem[];
+    __shared__ uint32_t tmem_base_s;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(tq_smem + TQ_OFF_BAR);
+    uint64_t *full = bars, *empty = bars + TQ_NST, *acc_full = bars + 2 * TQ_NST, *acc_empty = acc_full + 2, *landed = acc_empty + 2;
+    if (tid == 0) {
+        for (int k = 0; k < TQ_NST; ++k) { tc::mbar_init(&full[k], 256); tc::mbar_init(&empty[k], 1); tc::mbar_init(&landed[k], 1); }
+        for (int k = 0; k < 2; ++k) { tc::mbar_init(&acc_full[k], 1); tc::mbar_init(&acc_empty[k], 4); }
+        asm volatile("fence.mbarrier_init.release.cluster;");
+    }
+    if (warp == 12) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tc::smem_u32(&tmem_base_s)), "n"(512));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    tc::fence_before();
+    __syncthreads();
+    tc::fence_after();
+    const uint32_t tmem = tmem_base_s;
+    const uint32_t sbase = tc::smem_u32(tq_smem);
+    const int nblk = p.T * p.T, ntiles = p.tab[nblk].x;
+    const int W = p.W, K = p.K, BN = p.NTOT < 256 ? p.NTOT : 256, NT = p.NTOT / BN, NKC = K / TQ_KC;
+    const long nwork = (long)ntiles * NT;          // work item = (row tile, N tile), the N tiles of a row tile adjacent
+
+    if (warp == 13) {
+        // ------------------------------------------------------------------------------------------------ loader
+        if (lane == 0) {
+            const uint32_t b_stage_bytes = 2u * BN * TQ_KC * 4;                 // TF32 values and remainders of one stage
+            uint32_t step = 0;
+            for (long w = blockIdx.x; w < nwork; w += gridDim.x) {
+                const int tile = (int)(w / NT), nt = (int)(w % NT);
+                const int k = wg_block(p.tab, nblk, tile);
+                const int4 e = p.tab[k];
+                const long row = p.N * (long)p.tt.off[k % p.T] + e.y + (long)(tile - e.x) * GR;       // first row of the tile
+                const float *Bg = p.nets + k * p.net_stride + p.b_off + (long)nt * NKC * (2 * BN * TQ_KC);
+                for (int kc = 0; kc < NKC; ++kc, ++step) {
+                    const int st = step % TQ_NST;
+                    tc::mbar_wait(&empty[st], ((step / TQ_NST) & 1) ^ 1);
+                    mbar_expect_tx_cta(&landed[st], TQ_A_IMG + b_stage_bytes);
+                    tma_load_3d(sbase + st * TQ_STAGE, &tmA, 0, (int)row, kc * 4, &landed[st]);
+                    bulk_g2s_cta(sbase + st * TQ_STAGE + 2 * TQ_A_IMG, Bg + (long)kc * (2 * BN * TQ_KC), b_stage_bytes, &landed[st]);
+                }
+            }
+        }
+    } else if (warp < 8) {
+        // ------------------------------------------------------------------------------------------------ splitters
+        // every thread splits two 16-byte pieces of the landed A image in place: a_big, and a_small into the second image
+        const uint32_t a_off = ((tid >> 3) & 3) * TQ_A_PIECE + (8 * (tid >> 5) + (tid & 7)) * 16;      // + 64 rows for the second piece
+        const long nstage = nwork > (long)blockIdx.x ? ((nwork - blockIdx.x + gridDim.x - 1) / gridDim.x) * NKC : 0;
+        for (long it = 0; it < nstage; ++it) {
+            const int st = (int)(it % TQ_NST);
+            tc::mbar_wait(&landed[st], (uint32_t)((it / TQ_NST) & 1));
+            unsigned char *stage = tq_smem + st * TQ_STAGE;
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+                uint4 *pb = reinterpret_cast<uint4 *>(stage + a_off + q * (64 * 16));
+                uint4 *ps = reinterpret_cast<uint4 *>(stage + TQ_A_IMG + a_off + q * (64 * 16));
+                const uint4 x = *pb;
+                uint4 b, sm;
+                b.x = x.x & 0xffffe000u; b.y = x.y & 0xffffe000u; b.z = x.z & 0xffffe000u; b.w = x.w & 0xffffe000u;
+                sm.x = __float_as_uint(__uint_as_float(x.x) - __uint_as_float(b.x));
+                sm.y = __float_as_uint(__uint_as_float(x.y) - __uint_as_float(b.y));
+                sm.z = __float_as_uint(__uint_as_float(x.z) - __uint_as_float(b.z));
+                sm.w = __float_as_uint(__uint_as_float(x.w) - __uint_as_float(b.w));
+                *pb = b;
+                *ps = sm;
+            }
+            tc::proxy_fence();
+            mbar_arrive_cta(&full[st]);
+        }
+    } else if (warp == 12) {
+        // ------------------------------------------------------------------------------------------------ MMA issuer
+        const uint32_t idesc = idesc_tf32(128, BN);
+        uint32_t step = 0, accn = 0;
+        for (long w = blockIdx.x; w < nwork; w += gridDim.x, ++accn) {
+            const int buf = accn & 1;
+            tc::mbar_wait(&acc_empty[buf], ((accn >> 1) & 1) ^ 1);
+            tc::fence_after();
+            for (int kc = 0; kc < NKC; ++kc, ++step) {
+                const int st = step % TQ_NST;
+                tc::mbar_wait(&full[st], (step / TQ_NST) & 1);
+                tc::fence_after();
+                const uint32_t sa = sbase + st * TQ_STAGE;
+                const uint32_t B_PIECE = BN * 16;
+                const uint64_t dab = tc::desc(sa, TQ_A_PIECE, 128), das = tc::desc(sa + TQ_A_IMG, TQ_A_PIECE, 128);
+                const uint64_t dbb = tc::desc(sa + 2 * TQ_A_IMG, B_PIECE, 128), dbs = tc::desc(sa + 2 * TQ_A_IMG + BN * TQ_KC * 4, B_PIECE, 128);
+                if (tc::elect_one()) {
+#pragma unroll
+                    for (int ks = 0; ks < TQ_KC / 8; ++ks) {
+                        const uint32_t oa = ks * 2 * TQ_A_PIECE, ob = ks * 2 * B_PIECE;
+                        mma_tf32_ss(tmem + buf * 256, tc::desc_at(das, oa), tc::desc_at(dbb, ob), idesc, (kc | ks) != 0);     // small terms first
+                        mma_tf32_ss(tmem + buf * 256, tc::desc_at(dab, oa), tc::desc_at(dbs, ob), idesc, true);
+                        mma_tf32_ss(tmem + buf * 256, tc::desc_at(dab, oa), tc::desc_at(dbb, ob), idesc, true);
+                    }
+                    tc::commit(&empty[st]);
+                }
+                __syncwarp();
+            }
+            if (tc::elect_one()) tc::commit(&acc_full[buf]);
+            __syncwarp();
+        }
+    } else {
+        // ------------------------------------------------------------------------------------------------ epilogue
+        const int q4 = warp & 3, r = q4 * 32 + lane;
+        const uint32_t tm_lane = tmem + ((uint32_t)(q4 * 32) << 16);
+        uint32_t accn = 0;
+        for (long w = blockIdx.x; w < nwork; w += gridDim.x, ++accn) {
+            const int tile = (int)(w / NT), nt = (int)(w % NT);
+            const int k = wg_block(p.tab, nblk, tile);
+            const int4 e = p.tab[k];
+            const long rbase = p.N * (long)p.tt.off[k % p.T];
+            const int row0 = e.y + (tile - e.x) * GR, nrows = min(GR, e.z - row0);
+            const float *net = p.nets + k * p.net_stride;
+            const long Rg = rbase + row0 + r;
+            const bool ok = r < nrows;
+            const int buf = accn & 1;
+            tc::mbar_wait(&acc_full[buf], (accn >> 1) & 1);
+            tc::fence_after();
+            // 32 columns per step; the step's global loads are all issued before its first store (the activation pointers may
+            // alias as far as the compiler knows: interleaved, every load would wait a full memory round trip behind a store)
+            for (int c0 = 0; c0 < BN; c0 += 32) {
+                const int col = nt * BN + c0;
+                float4 xa[8], xb[8], xc[8];
+                if (ok) {
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) {
+                        const int cq = col + 4 * q;
+                        if (MODE == 0) {
+                            xa[q] = *reinterpret_cast<const float4 *>(net + wg_off_b2(W) + cq);
+                            xb[q] = *reinterpret_cast<const float4 *>(p.T1 + Rg * W + (cq % W));
+                        } else if (MODE == 1) {
+                            xa[q] = *reinterpret_cast<const float4 *>(net + wg_off_b3(W) + cq);
+                        } else if (MODE == 2) {
+                            xa[q] = *reinterpret_cast<const float4 *>(p.Y2 + Rg * 2 * W + cq);
+                            xb[q] = *reinterpret_cast<const float4 *>(p.T2 + Rg * 2 * W + cq);
+                        } else {
+                            xa[q] = *reinterpret_cast<const float4 *>(p.Y2 + Rg * 2 * W + cq);
+                            xb[q] = *reinterpret_cast<const float4 *>(p.Y2 + Rg * 2 * W + W + cq);
+                            xc[q] = *reinterpret_cast<const float4 *>(p.T1 + Rg * W + cq);
+                        }
+                    }
+                }
+                uint32_t z[32];
+                tc::ld16(tm_lane + buf * 256 + c0, *reinterpret_cast<uint32_t(*)[16]>(&z[0]));
+                tc::ld16(tm_lane + buf * 256 + c0 + 16, *reinterpret_cast<uint32_t(*)[16]>(&z[16]));
+                tc::wait_ld();
+                if (!ok) continue;
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    const int cq = col + 4 * q;
+                    float4 v = make_float4(__uint_as_float(z[4 * q]), __uint_as_float(z[4 * q + 1]), __uint_as_float(z[4 * q + 2]), __uint_as_float(z[4 * q + 3]));
+                    if (MODE == 0) {
+                        v.x = tanhf(v.x + xa[q].x); v.y = tanhf(v.y + xa[q].y); v.z = tanhf(v.z + xa[q].z); v.w = tanhf(v.w + xa[q].w);
+                        *reinterpret_cast<float4 *>(p.T2 + Rg * 2 * W + cq) = v;
+                        v.x += xb[q].x; v.y += xb[q].y; v.z += xb[q].z; v.w += xb[q].w;
+                        *reinterpret_cast<float4 *>(p.Y2 + Rg * 2 * W + cq) = v;
+                    } else if (MODE == 1) {
+                        v.x = tanhf(v.x + xa[q].x); v.y = tanhf(v.y + xa[q].y); v.z = tanhf(v.z + xa[q].z); v.w = tanhf(v.w + xa[q].w);
+                        *reinterpret_cast<float4 *>(p.T3 + Rg * 4 * W + cq) = v;
+                    } else if (MODE == 2) {
+                        const float4 t = xb[q];
+                        v.x += xa[q].x; v.y += xa[q].y; v.z += xa[q].z; v.w += xa[q].w;
+                        *reinterpret_cast<float4 *>(p.Y2 + Rg * 2 * W + cq) = v;
+                        v.x *= 1.f - t.x * t.x; v.y *= 1.f - t.y * t.y; v.z *= 1.f - t.z * t.z; v.w *= 1.f - t.w * t.w;
+                        *reinterpret_cast<float4 *>(p.T2 + Rg * 2 * W + cq) = v;
+                    } else {
+                        const float4 t = xc[q];
+                        v.x = (v.x + xa[q].x + xb[q].x) * (1.f - t.x * t.x); v.y = (v.y + xa[q].y + xb[q].y) * (1.f - t.y * t.y);
+                        v.z = (v.z + xa[q].z + xb[q].z) * (1.f - t.z * t.z); v.w = (v.w + xa[q].w + xb[q].w) * (1.f - t.w * t.w);
+                        *reinterpret_cast<float4 *>(p.T1 + Rg * W + cq) = v;
+                    }
+                }
+            }
+            tc::fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cta(&acc_empty[buf]);
+        }
+    }
+    tc::fence_before();
+    __syncthreads();
+    tc::fence_after();
+    if (warp == 12) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(512));
+}
+
 // S5: A_i[c][m] = (1 / Nm) sum over the atom's rows of wt R^[c] G[m], G[m] = y2[m mod 2 W] + t3[m]; wt = the number of padded
 // slots a representative row stands for, 1 for a real row.  One thread per column m.
 template <typename R>
@@ -541,16 +778,38 @@ static void build_net(int W, const double *net, R *out) {
             out[wg_off_W3T(W) + (size_t)m * 2 * W + f] = (R)W3[(size_t)f * 4 * W + m];
         }
 }
+// MIX-32: the operand images of B^T [NTOT][K] of one product: per N tile (BN = min(256, NTOT) rows) and per K = 16 stage the
+// TF32 values [4 pieces][BN][4] followed by the TF32 remainders in the same order (one contiguous bulk copy per stage)
+static void tf32_image(const std::vector<float> &Bt, int NTOT, int K, float *out) {
+    const int BN = NTOT < 256 ? NTOT : 256, NKC = K / TQ_KC;
+    for (int n = 0; n < NTOT; ++n)
+        for (int k = 0; k < K; ++k) {
+            const float x = Bt[(size_t)n * K + k], big = tf32_rna(x), small = tf32_rna(x - big);
+            const size_t stage = ((size_t)(n / BN) * NKC + k / TQ_KC) * (2 * (size_t)BN * TQ_KC);
+            const size_t in = (size_t)((k % TQ_KC) / 4) * (BN * 4) + (size_t)(n % BN) * 4 + (k % 4);
+            out[stage + in] = big;
+            out[stage + (size_t)BN * TQ_KC + in] = small;
+        }
+}
+__host__ __device__ inline long wg_off_img(int W, int mode) {      // MODE 0: W2^T, 1: W3^T, 2: W3, 3: W2 as B^T [NTOT][K]
+    return 8L * W + (mode == 0 ? 0L : mode == 1 ? 4L : mode == 2 ? 20L : 36L) * W * W;
+}
 void wide_gen_build_net(int W, bool f64, const double *net, void *out) {
     if (f64) { build_net<double>(W, net, (double *)out); return; }
     float *o = (float *)out;
-    build_net<float>(W, net, o);
-    const size_t m0 = 8 * (size_t)W, nm = 20 * (size_t)W * W;
-    for (size_t k = 0; k < nm; ++k) {
-        const float x = o[m0 + k], big = tf32_rna(x);
-        o[m0 + k] = big;
-        o[m0 + nm + k] = tf32_rna(x - big);
-    }
+    const double *w1 = net, *b1 = w1 + W, *W2 = b1 + W, *b2 = W2 + (size_t)W * 2 * W, *W3 = b2 + 2 * W, *b3 = W3 + (size_t)2 * W * 4 * W;
+    for (int e = 0; e < W; ++e) { o[e] = (float)w1[e]; o[W + e] = (float)b1[e]; }
+    for (int f = 0; f < 2 * W; ++f) o[wg_off_b2(W) + f] = (float)b2[f];
+    for (int m = 0; m < 4 * W; ++m) o[wg_off_b3(W) + m] = (float)b3[m];
+    std::vector<float> w2((size_t)W * 2 * W), w2t(w2.size()), w3((size_t)2 * W * 4 * W), w3t(w3.size());
+    for (int e = 0; e < W; ++e)
+        for (int f = 0; f < 2 * W; ++f) { w2[(size_t)e * 2 * W + f] = (float)W2[(size_t)e * 2 * W + f]; w2t[(size_t)f * W + e] = w2[(size_t)e * 2 * W + f]; }
+    for (int f = 0; f < 2 * W; ++f)
+        for (int m = 0; m < 4 * W; ++m) { w3[(size_t)f * 4 * W + m] = (float)W3[(size_t)f * 4 * W + m]; w3t[(size_t)m * 2 * W + f] = w3[(size_t)f * 4 * W + m]; }
+    tf32_image(w2t, 2 * W, W, o + wg_off_img(W, 0));        // t1 . W2:     B^T[f][e]
+    tf32_image(w3t, 4 * W, 2 * W, o + wg_off_img(W, 1));    // y2 . W3:     B^T[m][f]
+    tf32_image(w3, 2 * W, 4 * W, o + wg_off_img(W, 2));     // dz3 . W3^T:  B^T[f][m]
+    tf32_image(w2, W, 2 * W, o + wg_off_img(W, 3));         // dz2 . W2^T:  B^T[e][f]
 }
 
 template <typename R>
@@ -565,13 +824,50 @@ static GenArgs<R> gen_args(const dp_model *m, long N, char *ws, const WsLayout &
     return p;
 }
 
+typedef CUresult (*tmap_encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                   const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static tmap_encode_fn tmap_encoder() {
+    static const tmap_encode_fn fn = [] {
+        void *q = nullptr;
+        cudaDriverEntryPointQueryResult res;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &q, cudaEnableDefault, &res) != cudaSuccess || res != cudaDriverEntryPointSuccess)
+            q = nullptr;
+        return (tmap_encode_fn)q;
+    }();
+    return fn;
+}
+
+// MIX-32: the tcgen05 kernel; bt_off = offset of the product's B^T [Nn][K] (the transposed copy of the weight matrix)
+template <int MODE>
+static cudaError_t gen_gemm_tf32(const dp_model *m, GenArgs<float> p, int K, int Nn, const float *A, long bt_off, cudaStream_t st) {
+    DP_SMEM_OPTIN((k_wg_gemm_tf32<MODE>), TQ_TOTAL);
+    p.K = K; p.NTOT = Nn; p.A = A; p.b_off = bt_off;
+    // the activations [rows][K] as a (4, rows, K / 4) tensor: strides K * 4 bytes (rows) and 16 bytes (pieces of a row)
+    const tmap_encode_fn enc = tmap_encoder();
+    if (!enc) return cudaErrorNotSupported;
+    CUtensorMap tm;
+    const cuuint64_t gdim[3] = {4, (cuuint64_t)p.N * (cuuint64_t)m->Nm, (cuuint64_t)(K / 4)};
+    const cuuint64_t gstr[2] = {(cuuint64_t)K * 4, 16};
+    const cuuint32_t box[3] = {4, 128, 4}, estr[3] = {1, 1, 1};
+    if (enc(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)A, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return cudaErrorInvalidValue;
+    k_wg_gemm_tf32<MODE><<<m->num_sms, TQ_THREADS, TQ_TOTAL, st>>>(p, tm);
+    return cudaGetLastError();
+}
+
 template <typename R, int MODE>
 static cudaError_t gen_gemm(const dp_model *m, long N, GenArgs<R> p, int K, int Nn, const R *A, long b_off, cudaStream_t st) {
+    if constexpr (sizeof(R) == 4) {
+        return gen_gemm_tf32<MODE>(m, p, K, Nn, A, wg_off_img(m->m0, MODE), st);
+    } else {
     DP_SMEM_OPTIN((k_wg_gemm<R, MODE>), GemmCfg<R>::SMEM);
     p.K = K; p.NTOT = Nn; p.A = A; p.b_off = b_off;
     const long tiles = wide_tiles_cap(m, N), ntn = (Nn + GBN - 1) / GBN;
     k_wg_gemm<R, MODE><<<(unsigned)(tiles * ntn), 256, GemmCfg<R>::SMEM, st>>>(p);
     return cudaGetLastError();
+    }
 }
 
 template <typename R>
