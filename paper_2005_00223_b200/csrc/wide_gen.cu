@@ -8,11 +8,12 @@
 // rows of the mixed modes (the real rows of a (centre type, neighbour type) block, contiguous, plus one
 // representative per atom and block for its padded slots, weighted by their number) and the row tiles are those of the
 // tile table of wide.cu, so a tile never straddles two nets.
-//   FP64   ("double"): GEMMs on the FP64 tensor pipe (DMMA m8n8k4), 128 x 128 x 16 tiles staged with cp.async;
-//   MIX-32 (nets in single precision): the same tiles on mma.sync m16n8k8 TF32, every operand split into a
-//          TF32 value and its TF32 remainder and three products per step ("3xTF32": the product keeps 21+ mantissa bits;
-//          the accumulators are fp32), exact tanhf.  Coordinates, environment rows, geometry derivative, force and virial
-//          accumulation stay fp64 in both modes.
+//   FP64   ("double"): k_wg_gemm_f64, the FP64 tensor pipe (DMMA m8n8k4), 128 x 128 x 32 tiles staged with cp.async;
+//   MIX-32 (nets in single precision): k_wg_gemm_tf32, tcgen05.mma kind::tf32 with TMEM accumulators; every operand
+//          is split into a TF32 value and its TF32 remainder and each K step takes three products ("3xTF32": the product keeps
+//          21+ mantissa bits; the accumulators are fp32); the activations arrive by TMA tensor copies, the weights' operand
+//          images by bulk copies; exact tanhf.
+//   Coordinates, environment rows, geometry derivative, force and virial accumulation stay fp64 in both modes.
 // Forward:  k_wg_env -> k_wg_l1 (t1) -> gemm<0> (t2, y2 = (t1,t1) + t2) -> gemm<1> (t3) -> k_wg_contract (A_i = R^T G / Nm)
 // Backward: k_wg_bwd_head (gG = R^ gA / Nm, dz3, skip share of dy2, dR^ = G gA^T / Nm) -> gemm<2> (dy2, dz2) -> gemm<3> (dz1)
 //           -> k_wg_ds (ds^ = dz1 . w1, dE/dR~ = (dR^ + ds^ e0) / std) -> k_wg_force (N9 geometry derivative, ProdForce,
@@ -29,13 +30,12 @@ namespace {
 
 constexpr int GR = 128;                     // rows per tile (= the tile table's, wide.cu)
 constexpr int GBN = 128, GBK = 32;          // N tile, K step
-constexpr int GA_STRIDE = GBK + 4;          // A tile [128][36]: fragment loads hit distinct banks (fp64: per half warp)
-template <typename R> struct GemmCfg {
-    static constexpr int BS = sizeof(R) == 8 ? GBN + 4 : GBN + 8;       // B tile [32][BS]; fp32: two of them (TF32 value, remainder)
-    static constexpr int NB = sizeof(R) == 8 ? 1 : 2;
-    static constexpr int A_TILE = GR * GA_STRIDE, B_TILE = NB * GBK * BS;
-    static constexpr int SMEM = 2 * (A_TILE + B_TILE) * (int)sizeof(R);
-    static constexpr int EPV = 16 / (int)sizeof(R);                     // elements per 16-byte cp.async
+constexpr int GA_STRIDE = GBK + 4;          // A tile [128][36]: fragment loads hit distinct banks (per half warp)
+struct GemmCfg {                             // the FP64 kernel's tiles
+    static constexpr int BS = GBN + 4;                                  // B tile [32][BS]
+    static constexpr int A_TILE = GR * GA_STRIDE, B_TILE = GBK * BS;
+    static constexpr int SMEM = 2 * (A_TILE + B_TILE) * 8;
+    static constexpr int EPV = 2;                                       // doubles per 16-byte cp.async
 };
 
 __device__ __forceinline__ double wg_tanh(double x) { return dp_tanh64(x); }
@@ -43,17 +43,6 @@ __device__ __forceinline__ float wg_tanh(float x) { return tanhf(x); }
 
 __device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b) {
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
-}
-__device__ __forceinline__ void mma_tf32(float *c, const uint32_t (&a)[4], const uint32_t (&b)[2]) {
-    asm("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
-        : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
-        : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
-}
-// x = big + small, both TF32 (10 explicit mantissa bits each): big = rna(x), small = rna(x - big)
-__device__ __forceinline__ void split_tf32(float x, uint32_t &big, uint32_t &small) {
-    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(big) : "f"(x));
-    const float rem = x - __uint_as_float(big);
-    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(small) : "f"(rem));
 }
 __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc, bool valid) {
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
@@ -179,8 +168,7 @@ struct GenArgs {
     const int4 *tab;
     const R *A;                           // [rows][K] row-major (one of the activation buffers)
     const R *nets;                        // parameter blocks, net k at nets + k * net_stride
-    long net_stride, b_off;               // B [K][NTOT] row-major at offset b_off of the block
-    long b_small;                         // fp32: distance from a weight matrix to the matrix of its TF32 remainders
+    long net_stride, b_off;               // FP64: B [K][NTOT] row-major at offset b_off of the block; MIX-32: the operand images of B^T
     R *T1, *Y2, *T2, *T3;                 // activations [rows][W | 2 W | 2 W | 4 W]
     TypeTab tt;
 };
@@ -189,64 +177,62 @@ struct GenArgs {
 // MODE 1: layer 3 forward   A = y2,  B = W3:    t3 = tanh(acc + b3) -> T3   (G = (y2,y2) + t3 is formed by its readers)
 // MODE 2: layer 3 backward  A = dz3, B = W3^T:  dy2 = acc + (gG[f] + gG[f + 2 W], in Y2) -> Y2;  dz2 = dy2 (1 - t2^2) -> T2
 // MODE 3: layer 2 backward  A = dz2, B = W2^T:  dy1 = acc + dy2[e] + dy2[e + W];  dz1 = dy1 (1 - t1^2) -> T1
-// The epilogue of one pair of adjacent columns, in two steps so that the kernel can issue the loads of several pairs before the
-// first store (the activation pointers may alias as far as the compiler knows: interleaved, every load would wait for the store
-// before it).
-template <typename R> struct EpiAux { typename std::conditional<sizeof(R) == 8, double2, float2>::type a, b, c; };
+// The FP64 epilogue of one pair of adjacent columns, in two steps so that the kernel can issue the loads of several pairs before
+// the first store (the activation pointers may alias as far as the compiler knows: interleaved, every load would wait for the
+// store before it).
+struct EpiAux { double2 a, b, c; };
 
-template <typename R, int MODE>
-__device__ __forceinline__ EpiAux<R> wg_epi_load(const GenArgs<R> &p, const R *__restrict__ net, long Rg, int col) {
-    using R2 = typename std::conditional<sizeof(R) == 8, double2, float2>::type;
+template <int MODE>
+__device__ __forceinline__ EpiAux wg_epi_load(const GenArgs<double> &p, const double *__restrict__ net, long Rg, int col) {
     const int W = p.W;
-    EpiAux<R> x;
+    EpiAux x;
     if (MODE == 0) {
-        x.a = *reinterpret_cast<const R2 *>(net + wg_off_b2(W) + col);
-        x.b = *reinterpret_cast<const R2 *>(p.T1 + Rg * W + (col % W));
+        x.a = *reinterpret_cast<const double2 *>(net + wg_off_b2(W) + col);
+        x.b = *reinterpret_cast<const double2 *>(p.T1 + Rg * W + (col % W));
     } else if (MODE == 1) {
-        x.a = *reinterpret_cast<const R2 *>(net + wg_off_b3(W) + col);
+        x.a = *reinterpret_cast<const double2 *>(net + wg_off_b3(W) + col);
     } else if (MODE == 2) {
-        x.a = *reinterpret_cast<const R2 *>(p.Y2 + Rg * 2 * W + col);
-        x.b = *reinterpret_cast<const R2 *>(p.T2 + Rg * 2 * W + col);
+        x.a = *reinterpret_cast<const double2 *>(p.Y2 + Rg * 2 * W + col);
+        x.b = *reinterpret_cast<const double2 *>(p.T2 + Rg * 2 * W + col);
     } else {
-        x.a = *reinterpret_cast<const R2 *>(p.Y2 + Rg * 2 * W + col);
-        x.b = *reinterpret_cast<const R2 *>(p.Y2 + Rg * 2 * W + W + col);
-        x.c = *reinterpret_cast<const R2 *>(p.T1 + Rg * W + col);
+        x.a = *reinterpret_cast<const double2 *>(p.Y2 + Rg * 2 * W + col);
+        x.b = *reinterpret_cast<const double2 *>(p.Y2 + Rg * 2 * W + W + col);
+        x.c = *reinterpret_cast<const double2 *>(p.T1 + Rg * W + col);
     }
     return x;
 }
-template <typename R, int MODE>
-__device__ __forceinline__ void wg_epi_store(const GenArgs<R> &p, long Rg, int col, R v0, R v1, const EpiAux<R> &x) {
-    using R2 = typename std::conditional<sizeof(R) == 8, double2, float2>::type;
+template <int MODE>
+__device__ __forceinline__ void wg_epi_store(const GenArgs<double> &p, long Rg, int col, double v0, double v1, const EpiAux &x) {
     const int W = p.W;
-    R2 o;
+    double2 o;
     if (MODE == 0) {
-        o.x = wg_tanh(v0 + x.a.x); o.y = wg_tanh(v1 + x.a.y);
-        *reinterpret_cast<R2 *>(p.T2 + Rg * 2 * W + col) = o;
+        o.x = dp_tanh64(v0 + x.a.x); o.y = dp_tanh64(v1 + x.a.y);
+        *reinterpret_cast<double2 *>(p.T2 + Rg * 2 * W + col) = o;
         o.x += x.b.x; o.y += x.b.y;
-        *reinterpret_cast<R2 *>(p.Y2 + Rg * 2 * W + col) = o;
+        *reinterpret_cast<double2 *>(p.Y2 + Rg * 2 * W + col) = o;
     } else if (MODE == 1) {
-        o.x = wg_tanh(v0 + x.a.x); o.y = wg_tanh(v1 + x.a.y);
-        *reinterpret_cast<R2 *>(p.T3 + Rg * 4 * W + col) = o;
+        o.x = dp_tanh64(v0 + x.a.x); o.y = dp_tanh64(v1 + x.a.y);
+        *reinterpret_cast<double2 *>(p.T3 + Rg * 4 * W + col) = o;
     } else if (MODE == 2) {
         o.x = x.a.x + v0; o.y = x.a.y + v1;
-        *reinterpret_cast<R2 *>(p.Y2 + Rg * 2 * W + col) = o;
-        o.x *= (R)1 - x.b.x * x.b.x; o.y *= (R)1 - x.b.y * x.b.y;
-        *reinterpret_cast<R2 *>(p.T2 + Rg * 2 * W + col) = o;
+        *reinterpret_cast<double2 *>(p.Y2 + Rg * 2 * W + col) = o;
+        o.x *= 1.0 - x.b.x * x.b.x; o.y *= 1.0 - x.b.y * x.b.y;
+        *reinterpret_cast<double2 *>(p.T2 + Rg * 2 * W + col) = o;
     } else {
-        o.x = (v0 + x.a.x + x.b.x) * ((R)1 - x.c.x * x.c.x);
-        o.y = (v1 + x.a.y + x.b.y) * ((R)1 - x.c.y * x.c.y);
-        *reinterpret_cast<R2 *>(p.T1 + Rg * W + col) = o;
+        o.x = (v0 + x.a.x + x.b.x) * (1.0 - x.c.x * x.c.x);
+        o.y = (v1 + x.a.y + x.b.y) * (1.0 - x.c.y * x.c.y);
+        *reinterpret_cast<double2 *>(p.T1 + Rg * W + col) = o;
     }
 }
 
-// One 128 x 128 output tile per CTA, eight warps as 4 (rows) x 2 (columns): warp tile 32 x 64.  A and B stages of K = 16 arrive
-// by cp.async (two buffers); rows past the end of the tile's block and columns past NTOT are zero-filled and never stored.
-template <typename R, int MODE>
-__global__ void __launch_bounds__(256, sizeof(R) == 8 ? 1 : 2) k_wg_gemm(const __grid_constant__ GenArgs<R> p) {
-    using C = GemmCfg<R>;
-    constexpr bool F64 = sizeof(R) == 8;
+// FP64: one 128 x 128 output tile per CTA, eight warps as 4 (rows) x 2 (columns): warp tile 32 x 64 = 4 x 8 DMMA m8n8k4 fragments.
+// A and B stages of K = 32 arrive by cp.async (two buffers); rows past the end of the tile's block and columns past NTOT are
+// zero-filled and never stored.
+template <int MODE>
+__global__ void __launch_bounds__(256, 1) k_wg_gemm_f64(const __grid_constant__ GenArgs<double> p) {
+    using C = GemmCfg;
     extern __shared__ __align__(16) unsigned char wg_smem[];
-    R *sm = reinterpret_cast<R *>(wg_smem);
+    double *sm = reinterpret_cast<double *>(wg_smem);
     const int nblk = p.T * p.T;
     const int ntn = (p.NTOT + GBN - 1) / GBN;
     const int tile = blockIdx.x / ntn, n0 = (blockIdx.x % ntn) * GBN;
@@ -256,14 +242,14 @@ __global__ void __launch_bounds__(256, sizeof(R) == 8 ? 1 : 2) k_wg_gemm(const _
     const long rbase = p.N * (long)p.tt.off[k % p.T];
     const int row0 = e.y + (tile - e.x) * GR;
     const int nrows = min(GR, e.z - row0);
-    const R *net = p.nets + k * p.net_stride;
-    const R *Ag = p.A + (rbase + row0) * (long)p.K;
-    const R *Bg = net + p.b_off + n0;
+    const double *net = p.nets + k * p.net_stride;
+    const double *Ag = p.A + (rbase + row0) * (long)p.K;
+    const double *Bg = net + p.b_off + n0;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wm = warp >> 1, wn = warp & 1, g = lane >> 2, t = lane & 3;
 
     auto load_stage = [&](int buf, int k0) {
-        R *As = sm + buf * (C::A_TILE + C::B_TILE), *Bs = As + C::A_TILE;
+        double *As = sm + buf * (C::A_TILE + C::B_TILE), *Bs = As + C::A_TILE;
         constexpr int AV = GBK / C::EPV, BV = GBN / C::EPV;       // 16-byte vectors per A row / per B row
 #pragma unroll
         for (int q = 0; q < GR * AV / 256; ++q) {
@@ -276,84 +262,51 @@ __global__ void __launch_bounds__(256, sizeof(R) == 8 ? 1 : 2) k_wg_gemm(const _
             const int idx = tid + q * 256, kk = idx / BV, nv = (idx % BV) * C::EPV;
             const bool ok = n0 + nv < p.NTOT;
             cp_async16(Bs + kk * C::BS + nv, Bg + (ok ? (long)(k0 + kk) * p.NTOT + nv : 0), ok);
-            if constexpr (!F64)     // the remainders of the weights (split once, by dp_create)
-                cp_async16(Bs + GBK * C::BS + kk * C::BS + nv, Bg + p.b_small + (ok ? (long)(k0 + kk) * p.NTOT + nv : 0), ok);
         }
         cp_async_commit();
     };
 
-    constexpr int NACC = 64;                     // fp64: 4 x 8 fragments of 2; fp32: 2 x 8 fragments of 4
-    R acc[NACC];
+    double acc[64];                              // 4 x 8 fragments of 2
 #pragma unroll
-    for (int q = 0; q < NACC; ++q) acc[q] = (R)0;
+    for (int q = 0; q < 64; ++q) acc[q] = 0.0;
 
     const int nk = p.K / GBK;
     load_stage(0, 0);
     for (int ks = 0; ks < nk; ++ks) {
         if (ks + 1 < nk) { load_stage((ks + 1) & 1, (ks + 1) * GBK); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
         __syncthreads();
-        const R *As = sm + (ks & 1) * (C::A_TILE + C::B_TILE), *Bs = As + C::A_TILE;
-        if constexpr (F64) {
+        const double *As = sm + (ks & 1) * (C::A_TILE + C::B_TILE), *Bs = As + C::A_TILE;
 #pragma unroll
-            for (int kk = 0; kk < GBK / 4; ++kk) {
-                double a[4], b[8];
+        for (int kk = 0; kk < GBK / 4; ++kk) {
+            double a[4], b[8];
 #pragma unroll
-                for (int mi = 0; mi < 4; ++mi) a[mi] = As[(32 * wm + 8 * mi + g) * GA_STRIDE + 4 * kk + t];
+            for (int mi = 0; mi < 4; ++mi) a[mi] = As[(32 * wm + 8 * mi + g) * GA_STRIDE + 4 * kk + t];
 #pragma unroll
-                for (int ni = 0; ni < 8; ++ni) b[ni] = Bs[(4 * kk + t) * C::BS + 64 * wn + 8 * ni + g];
+            for (int ni = 0; ni < 8; ++ni) b[ni] = Bs[(4 * kk + t) * C::BS + 64 * wn + 8 * ni + g];
 #pragma unroll
-                for (int mi = 0; mi < 4; ++mi)
+            for (int mi = 0; mi < 4; ++mi)
 #pragma unroll
-                    for (int ni = 0; ni < 8; ++ni) dmma(acc[2 * (mi * 8 + ni)], acc[2 * (mi * 8 + ni) + 1], a[mi], b[ni]);
-            }
-        } else {
-#pragma unroll
-            for (int kk = 0; kk < GBK / 8; ++kk) {
-                uint32_t ab[2][4], as[2][4];
-#pragma unroll
-                for (int mi = 0; mi < 2; ++mi) {
-                    const float *ap = As + (32 * wm + 16 * mi + g) * GA_STRIDE + 8 * kk + t;
-                    split_tf32(ap[0], ab[mi][0], as[mi][0]);
-                    split_tf32(ap[8 * GA_STRIDE], ab[mi][1], as[mi][1]);
-                    split_tf32(ap[4], ab[mi][2], as[mi][2]);
-                    split_tf32(ap[8 * GA_STRIDE + 4], ab[mi][3], as[mi][3]);
-                }
-#pragma unroll
-                for (int ni = 0; ni < 8; ++ni) {
-                    const uint32_t *bp = reinterpret_cast<const uint32_t *>(Bs) + (8 * kk + t) * C::BS + 64 * wn + 8 * ni + g;
-                    const uint32_t bb[2] = {bp[0], bp[4 * C::BS]}, bs[2] = {bp[GBK * C::BS], bp[GBK * C::BS + 4 * C::BS]};
-                    // small terms first
-                    mma_tf32(&acc[4 * ni], as[0], bb);
-                    mma_tf32(&acc[4 * (8 + ni)], as[1], bb);
-                    mma_tf32(&acc[4 * ni], ab[0], bs);
-                    mma_tf32(&acc[4 * (8 + ni)], ab[1], bs);
-                    mma_tf32(&acc[4 * ni], ab[0], bb);
-                    mma_tf32(&acc[4 * (8 + ni)], ab[1], bb);
-                }
-            }
+                for (int ni = 0; ni < 8; ++ni) dmma(acc[2 * (mi * 8 + ni)], acc[2 * (mi * 8 + ni) + 1], a[mi], b[ni]);
         }
         __syncthreads();
     }
 
-    // epilogue: pairs of adjacent columns, eight pairs of one row at a time (loads first)
-    constexpr int NROWSETS = 4;
+    // epilogue: pairs of adjacent columns, the eight pairs of one fragment row at a time (loads first)
 #pragma unroll
-    for (int rs = 0; rs < NROWSETS; ++rs) {
-        // fp64: fragment row set mi = rs (rows 8 mi + g); fp32: mi = rs / 2, half h = rs % 2 (rows 16 mi + 8 h + g)
-        const int r = F64 ? 32 * wm + 8 * rs + g : 32 * wm + 16 * (rs >> 1) + 8 * (rs & 1) + g;
+    for (int mi = 0; mi < 4; ++mi) {
+        const int r = 32 * wm + 8 * mi + g;
         if (r >= nrows) continue;
         const long Rg = rbase + row0 + r;
-        EpiAux<R> aux[8];
+        EpiAux aux[8];
 #pragma unroll
         for (int ni = 0; ni < 8; ++ni) {
             const int col = n0 + 64 * wn + 8 * ni + 2 * t;
-            if (col < p.NTOT) aux[ni] = wg_epi_load<R, MODE>(p, net, Rg, col);
+            if (col < p.NTOT) aux[ni] = wg_epi_load<MODE>(p, net, Rg, col);
         }
 #pragma unroll
         for (int ni = 0; ni < 8; ++ni) {
             const int col = n0 + 64 * wn + 8 * ni + 2 * t;
-            const int q = F64 ? 2 * (rs * 8 + ni) : 4 * ((rs >> 1) * 8 + ni) + 2 * (rs & 1);
-            if (col < p.NTOT) wg_epi_store<R, MODE>(p, Rg, col, acc[q], acc[q + 1], aux[ni]);
+            if (col < p.NTOT) wg_epi_store<MODE>(p, Rg, col, acc[2 * (mi * 8 + ni)], acc[2 * (mi * 8 + ni) + 1], aux[ni]);
         }
     }
 }
@@ -818,7 +771,6 @@ static GenArgs<R> gen_args(const dp_model *m, long N, char *ws, const WsLayout &
     p.N = N; p.T = m->T; p.W = m->m0;
     p.tab = (const int4 *)(ws + L.wide_tab);
     p.nets = (const R *)m->wide_vec_dev; p.net_stride = (long)wide_gen_net_elems(m->m0, sizeof(R) == 8);
-    p.b_small = 20L * m->m0 * m->m0;
     p.T1 = (R *)(ws + L.wide_t1); p.Y2 = (R *)(ws + L.wide_y2); p.T2 = (R *)(ws + L.wide_t2); p.T3 = (R *)(ws + L.wide_t3);
     p.tt = make_typetab(m);
     return p;
@@ -857,16 +809,17 @@ static cudaError_t gen_gemm_tf32(const dp_model *m, GenArgs<float> p, int K, int
     return cudaGetLastError();
 }
 
+// b_off: offset of the product's weight matrix in the FP64 parameter block (MIX-32: the product's images, by MODE)
 template <typename R, int MODE>
 static cudaError_t gen_gemm(const dp_model *m, long N, GenArgs<R> p, int K, int Nn, const R *A, long b_off, cudaStream_t st) {
     if constexpr (sizeof(R) == 4) {
         return gen_gemm_tf32<MODE>(m, p, K, Nn, A, wg_off_img(m->m0, MODE), st);
     } else {
-    DP_SMEM_OPTIN((k_wg_gemm<R, MODE>), GemmCfg<R>::SMEM);
-    p.K = K; p.NTOT = Nn; p.A = A; p.b_off = b_off;
-    const long tiles = wide_tiles_cap(m, N), ntn = (Nn + GBN - 1) / GBN;
-    k_wg_gemm<R, MODE><<<(unsigned)(tiles * ntn), 256, GemmCfg<R>::SMEM, st>>>(p);
-    return cudaGetLastError();
+        DP_SMEM_OPTIN((k_wg_gemm_f64<MODE>), GemmCfg::SMEM);
+        p.K = K; p.NTOT = Nn; p.A = A; p.b_off = b_off;
+        const long tiles = wide_tiles_cap(m, N), ntn = (Nn + GBN - 1) / GBN;
+        k_wg_gemm_f64<MODE><<<(unsigned)(tiles * ntn), 256, GemmCfg::SMEM, st>>>(p);
+        return cudaGetLastError();
     }
 }
 
