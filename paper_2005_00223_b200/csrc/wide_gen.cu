@@ -41,6 +41,14 @@ struct GemmCfg {                             // the FP64 kernel's tiles
 __device__ __forceinline__ double wg_tanh(double x) { return dp_tanh64(x); }
 __device__ __forceinline__ float wg_tanh(float x) { return tanhf(x); }
 
+// 16 bytes of a row: 2 doubles / 4 floats (the element-wise kernels move whole vectors)
+template <typename R> struct alignas(16) Vec {
+    static constexpr int V = 16 / (int)sizeof(R);
+    R v[V];
+};
+template <typename R> __device__ __forceinline__ Vec<R> vld(const R *p) { return *reinterpret_cast<const Vec<R> *>(p); }
+template <typename R> __device__ __forceinline__ void vst(R *p, const Vec<R> &x) { *reinterpret_cast<Vec<R> *>(p) = x; }
+
 __device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b) {
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
@@ -153,10 +161,17 @@ k_wg_l1(long N, int T, int W, const __grid_constant__ TypeTab tt, const int4 *__
     const int row0 = e.y + (tile - e.x) * GR;
     const int nrows = min(GR, e.z - row0);
     const R *w1 = nets + k * net_stride, *b1 = w1 + W;
-    for (long idx = threadIdx.x; idx < (long)nrows * W; idx += 256) {
-        const int rr = (int)(idx / W), c = (int)(idx % W);
+    constexpr int V = Vec<R>::V;
+    const int vpr = W / V;                                   // vectors per row
+    for (int idx = threadIdx.x; idx < nrows * vpr; idx += 256) {
+        const int rr = idx / vpr, c = (idx % vpr) * V;
         const long Rg = rbase + row0 + rr;
-        T1[Rg * W + c] = wg_tanh(rh[4 * Rg] * w1[c] + b1[c]);
+        const R s = rh[4 * Rg];
+        const Vec<R> w = vld(w1 + c), b = vld(b1 + c);
+        Vec<R> o;
+#pragma unroll
+        for (int q = 0; q < V; ++q) o.v[q] = wg_tanh(s * w.v[q] + b.v[q]);
+        vst(T1 + Rg * W + c, o);
     }
 }
 
@@ -547,15 +562,20 @@ __global__ void __launch_bounds__(TQ_THREADS, 1) k_wg_gemm_tf32(const __grid_con
 }
 
 // S5: A_i[c][m] = (1 / Nm) sum over the atom's rows of wt R^[c] G[m], G[m] = y2[m mod 2 W] + t3[m]; wt = the number of padded
-// slots a representative row stands for, 1 for a real row.  One thread per column m.
+// slots a representative row stands for, 1 for a real row.  One thread per 16 bytes of columns.
 template <typename R>
 __global__ void __launch_bounds__(256)
 k_wg_contract(long N, int T, int W, R inv_nm, const __grid_constant__ TypeTab tt, const int *__restrict__ rowstart,
               const R *__restrict__ rh, const int2 *__restrict__ rows_id, const R *__restrict__ Y2, const R *__restrict__ T3,
               R *__restrict__ Aout) {
+    constexpr int V = Vec<R>::V;
     const long i = blockIdx.x;
-    const int m = blockIdx.y * 256 + threadIdx.x, f = m % (2 * W), M2 = 4 * W;
-    R acc[4] = {(R)0, (R)0, (R)0, (R)0};
+    const int m = (blockIdx.y * blockDim.x + threadIdx.x) * V, f = m % (2 * W), M2 = 4 * W;
+    R acc[4][V];
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+#pragma unroll
+        for (int q = 0; q < V; ++q) acc[c][q] = (R)0;
     for (int b = 0; b < T; ++b) {
         const int r0 = rowstart[(long)b * (N + 1) + i], r1 = rowstart[(long)b * (N + 1) + i + 1];
         const long base = N * (long)tt.off[b];
@@ -564,13 +584,25 @@ k_wg_contract(long N, int T, int W, R inv_nm, const __grid_constant__ TypeTab tt
             const long Rg = base + row;
             const int jj = rows_id[Rg].y;
             const R wt = jj < 0 ? (R)(-jj) : (R)1;
-            const R G = (Y2[Rg * 2 * W + f] + T3[Rg * M2 + m]) * wt;
+            const Vec<R> y = vld(Y2 + Rg * 2 * W + f), t = vld(T3 + Rg * M2 + m);
+            R r[4];
 #pragma unroll
-            for (int c = 0; c < 4; ++c) acc[c] += rh[4 * Rg + c] * G;
+            for (int c = 0; c < 4; ++c) r[c] = rh[4 * Rg + c] * wt;
+#pragma unroll
+            for (int q = 0; q < V; ++q) {
+                const R G = y.v[q] + t.v[q];
+#pragma unroll
+                for (int c = 0; c < 4; ++c) acc[c][q] += r[c] * G;
+            }
         }
     }
 #pragma unroll
-    for (int c = 0; c < 4; ++c) Aout[(i * 4 + c) * M2 + m] = acc[c] * inv_nm;
+    for (int c = 0; c < 4; ++c) {
+        Vec<R> o;
+#pragma unroll
+        for (int q = 0; q < V; ++q) o.v[q] = acc[c][q] * inv_nm;
+        vst(Aout + (i * 4 + c) * M2 + m, o);
+    }
 }
 
 // Head of the backward pass; one CTA per atom, one warp per row, a lane per pair of columns (f, f + 2 W):
@@ -586,34 +618,46 @@ k_wg_bwd_head(long N, int T, int W, R inv_nm, const __grid_constant__ TypeTab tt
               R *__restrict__ T3, R *__restrict__ dR) {
     const long i = blockIdx.x;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, M2 = 4 * W;
-    const R *ga = gA + i * 4L * M2;
+    const R *__restrict__ ga = gA + i * 4L * M2;
     for (int b = 0; b < T; ++b) {
         const int r0 = rowstart[(long)b * (N + 1) + i], r1 = rowstart[(long)b * (N + 1) + i + 1];
         const long base = N * (long)tt.off[b];
         for (int row = r0 + warp; row < r1; row += 8) {
             const long Rg = base + row;
-            R *y2 = Y2 + Rg * 2 * W, *t3 = T3 + Rg * M2;
+            R *__restrict__ y2 = Y2 + Rg * 2 * W;
+            R *__restrict__ t3 = T3 + Rg * M2;
+            constexpr int V = Vec<R>::V;
             if (rows_id[Rg].y < 0) {
-                for (int f = lane; f < 2 * W; f += 32) { y2[f] = (R)0; t3[f] = (R)0; t3[f + 2 * W] = (R)0; }
+                Vec<R> zero;
+#pragma unroll
+                for (int q = 0; q < V; ++q) zero.v[q] = (R)0;
+                for (int f = lane * V; f < 2 * W; f += 32 * V) { vst(y2 + f, zero); vst(t3 + f, zero); vst(t3 + f + 2 * W, zero); }
                 if (lane < 4) dR[4 * Rg + lane] = (R)0;
                 continue;
             }
             R r[4], acc[4] = {(R)0, (R)0, (R)0, (R)0};
 #pragma unroll
             for (int c = 0; c < 4; ++c) r[c] = rh[4 * Rg + c] * inv_nm;
-            for (int f = lane; f < 2 * W; f += 32) {
-                const R y = y2[f], ta = t3[f], tb = t3[f + 2 * W];
-                const R Ga = y + ta, Gb = y + tb;
-                R gGa = (R)0, gGb = (R)0;
+#pragma unroll 2
+            for (int f = lane * V; f < 2 * W; f += 32 * V) {
+                const Vec<R> y = vld(y2 + f), ta = vld(t3 + f), tb = vld(t3 + f + 2 * W);
+                Vec<R> a[4], bq[4], oa, ob, oy;
 #pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    const R a = ga[c * M2 + f], bq = ga[c * M2 + 2 * W + f];
-                    gGa += r[c] * a; gGb += r[c] * bq;
-                    acc[c] += Ga * a + Gb * bq;
+                for (int c = 0; c < 4; ++c) { a[c] = vld(ga + c * M2 + f); bq[c] = vld(ga + c * M2 + 2 * W + f); }
+#pragma unroll
+                for (int q = 0; q < V; ++q) {
+                    const R Ga = y.v[q] + ta.v[q], Gb = y.v[q] + tb.v[q];
+                    R gGa = (R)0, gGb = (R)0;
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        gGa += r[c] * a[c].v[q]; gGb += r[c] * bq[c].v[q];
+                        acc[c] += Ga * a[c].v[q] + Gb * bq[c].v[q];
+                    }
+                    oa.v[q] = gGa * ((R)1 - ta.v[q] * ta.v[q]);
+                    ob.v[q] = gGb * ((R)1 - tb.v[q] * tb.v[q]);
+                    oy.v[q] = gGa + gGb;
                 }
-                t3[f] = gGa * ((R)1 - ta * ta);
-                t3[f + 2 * W] = gGb * ((R)1 - tb * tb);
-                y2[f] = gGa + gGb;
+                vst(t3 + f, oa); vst(t3 + f + 2 * W, ob); vst(y2 + f, oy);
             }
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
@@ -843,7 +887,8 @@ static cudaError_t fwd_gen(const dp_model *m, long N, const Grid3 &g, char *ws, 
     ok(cudaGetLastError());
     ok((gen_gemm<R, 0>(m, N, p, W, 2 * W, p.T1, wg_off_W2(W), st)));
     ok((gen_gemm<R, 1>(m, N, p, 2 * W, 4 * W, p.Y2, wg_off_W3(W), st)));
-    k_wg_contract<R><<<dim3((unsigned)N, (unsigned)(4 * W / 256)), 256, 0, st>>>(N, T, W, (R)(1.0 / (double)m->Nm), tt, rowstart, rh, rows_id,
+    const int cthreads = 4 * W / Vec<R>::V < 256 ? 4 * W / Vec<R>::V : 256;       // one thread per 16 bytes of the 4 W columns
+    k_wg_contract<R><<<dim3((unsigned)N, (unsigned)(4 * W / Vec<R>::V / cthreads)), cthreads, 0, st>>>(N, T, W, (R)(1.0 / (double)m->Nm), tt, rowstart, rh, rows_id,
                                                                               p.Y2, p.T3, (R *)(ws + L.A));
     ok(cudaGetLastError());
     return e;
