@@ -313,7 +313,7 @@ def main():
     ap.add_argument("--config", default="4",
                     help="BASELINE.json configs index 0..4 (default: 4 = copper 1,048,576 atoms MIX-16, the largest single-GPU "
                          "config), or paper_cu / paper_water: the paper's network shape (32, 64, 128), capacity 512 / 144 (PAPER.md:151), "
-                         "or sweep: the network-size study of PAPER.md:273-279 (copper, last embedding layer 64 x 128 ... 1024 x 2048, MIX-16)")
+                         "or sweep: the network-size study of PAPER.md:273-279 (copper, last embedding layer 64 x 128 ... 1024 x 2048; MIX-16, or --precision)")
     ap.add_argument("--no-summary", action="store_true", help="skip the configs_summary leg (the other four configs)")
     ap.add_argument("--precision", default=None, choices=["fp64", "mix32", "mix16"],
                     help="override the config's precision (profiling aid; the default is the precision BASELINE.json names)")
@@ -500,6 +500,20 @@ def main():
                                               "peak_bf16_sustained_tflops": pk["bf16_sus"], "rows": rows}
             except (Exception, SystemExit) as e:      # noqa: BLE001
                 line["network_size_sweep"] = {"error": repr(e)[:300]}
+            # the double and MIX-32 curves of the same figure (csrc/wide_gen.cu): 4,000 atoms (the fp64 activations of the widest
+            # net take 76 GB there), each against the peak of its own arithmetic
+            for prec in ("fp64", "mix32"):
+                try:
+                    torch.cuda.empty_cache()
+                    args.steps_saved, args.steps = args.steps, 2
+                    rows = sweep_leg(args, binding, torch, synth, dev, flush, pk, precision=prec, ncell=10, mp=mp)
+                    args.steps = args.steps_saved
+                    line["network_size_sweep_" + prec] = {
+                        "workload": "copper 4000 atoms, capacity 512, " + prec + ", list build included",
+                        "unit": "TFLOP/s (algorithmic flops of the whole evaluation / CUDA-event time)", "rows": rows}
+                except (Exception, SystemExit) as e:      # noqa: BLE001
+                    args.steps = getattr(args, "steps_saved", args.steps)
+                    line["network_size_sweep_" + prec] = {"error": repr(e)[:300]}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -57,9 +57,9 @@ typedef enum {
 typedef struct {
     int ntypes;              /* T, 1..16 (the type field of the sort key has 4 bits)          */
     int embed_widths[3];     /* (m0, m1, m2) = (W, 2 W, 4 W): (25, 50, 100), or the paper's (32, 64, 128);
-                                DP_MIX16 only: W = 64, 128, 256, 512, the network-size study of PAPER.md:273-279 (Fig. 7),
-                                other precisions -> DP_EUNSUPPORTED.  The wide nets keep their activations in the
-                                workspace: dp_workspace_bytes grows by 18 W bytes per neighbour-list slot             */
+                                or W = 64, 128, 256, 512, the network-size study of PAPER.md:273-279 (Fig. 7), in every
+                                precision.  The wide nets keep their activations in the workspace: dp_workspace_bytes
+                                grows by 18 W (DP_MIX16), 36 W (DP_MIX32) or 72 W (DP_FP64) bytes per neighbour-list slot   */
     int axis;                /* M2 (16): D = A^T A[:, :M2]                                                   */
     int fit_widths[3];       /* (240, 240, 240)                                                             */
     const double *embed;     /* T*T nets, index a*T+b (a centre type, b neighbour type):
