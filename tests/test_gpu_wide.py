@@ -155,3 +155,28 @@ def test_wide_mix32_two_types():
     assert err <= 1e-4 * rms, err / rms
     assert abs(g["energy"][0] - o["energy"]) / s.natoms <= 2e-5
     assert np.abs(g["virial"] - o["virial"]).max() / s.natoms <= 2e-5
+
+
+def test_wide_fp64_md_with_buffered_list():
+    """dp_md_run on a wide FP64 model (PAPER.md:151-153 loop, 2 A buffered list searched every 2 evaluations): the compact rows of
+    the wide path are rebuilt from the stored candidates on the reuse steps"""
+    import torch
+    from oracle import md_oracle
+    from paper_2005_00223_b200 import binding
+    s = synth.wide_copper(5, 64, 777, sigma=0.1, precision="fp64")
+    masses = synth.MASS_AMU["cu"]
+    v = synth.boltzmann_velocities(s.types, masses, 330.0, 4343)
+    o = md_oracle.run(s.coords, v, s.types, masses, s.box, s.model, 1.0, 3)
+    m = binding.DPModel(s.model, "fp64")
+    c = torch.from_numpy(s.coords.copy()).cuda()
+    vel = torch.from_numpy(v.copy()).cuda()
+    out = m.md_run(c, vel, torch.from_numpy(s.types).cuda(), masses, s.box, 1.0, 3, skin=2.0, rebuild_every=2)
+    rc, _ = m.status()
+    assert rc == 0
+    torch.cuda.synchronize()
+    assert np.abs(c.cpu().numpy() - o["coords"]).max() <= 1e-11
+    fr = np.sqrt((o["forces"] ** 2).mean())
+    assert np.abs(out["forces"].cpu().numpy() - o["forces"]).max() <= 1e-9 * fr
+    th = out["thermo"].cpu().numpy()
+    assert np.abs(th[:, 0] - o["thermo"][:, 0]).max() <= 1e-12 * abs(o["thermo"][0, 0])
+    m.close()
