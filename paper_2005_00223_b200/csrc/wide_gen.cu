@@ -333,8 +333,8 @@ __global__ void __launch_bounds__(256, 1) k_wg_gemm_f64(const __grid_constant__ 
 //              (4, rows, K / 4) tensor, box {4, 128, 4}: it lands as the un-swizzled K-major operand image, per 16 bytes of K a
 //              column [128 rows][16 B]) and ONE bulk copy of the weights' operand images (TF32 values and TF32 remainders, laid
 //              out by dp_create), both counted by the stage's "landed" barrier;
-//   warps 0-7  splitters: a_big = a with the 13 low mantissa bits cleared (what the tensor core would read), in place,
-//              a_small = a - a_big (exact) into a second image; fence.proxy.async; arrive on the stage's "full" barrier;
+//   warps 0-7  splitters: a_small = a - a_big (exact) into a second image, a_big = a with the 13 low mantissa bits cleared = what
+//              the tensor core reads from the landed image itself; fence.proxy.async; arrive on the stage's "full" barrier;
 //   warp 12    MMA issuer: per K = 8 step a_small b_big, a_big b_small, a_big b_big into one of two 128 x BN fp32 accumulators
 //              in TMEM; tcgen05.commit frees the stage, the last one of a tile hands the accumulator over;
 //   warps 8-11 epilogue: thread = row = TMEM lane, tcgen05.ld of 16 columns at a time, the layer's bias / tanh / skip / tanh'
@@ -423,7 +423,7 @@ __global__ void __launch_bounds__(TQ_THREADS, 1) k_wg_gemm_tf32(const __grid_con
         }
     } else if (warp < 8) {
         // ------------------------------------------------------------------------------------------------ splitters
-        // every thread splits two 16-byte pieces of the landed A image in place: a_big, and a_small into the second image
+        // every thread splits two 16-byte pieces of the landed A image: a_small into the second image
         const uint32_t a_off = ((tid >> 3) & 3) * TQ_A_PIECE + (8 * (tid >> 5) + (tid & 7)) * 16;      // + 64 rows for the second piece
         const long nstage = nwork > (long)blockIdx.x ? ((nwork - blockIdx.x + gridDim.x - 1) / gridDim.x) * NKC : 0;
         for (long it = 0; it < nstage; ++it) {
@@ -432,8 +432,10 @@ __global__ void __launch_bounds__(TQ_THREADS, 1) k_wg_gemm_tf32(const __grid_con
             unsigned char *stage = tq_smem + st * TQ_STAGE;
 #pragma unroll
             for (int q = 0; q < 2; ++q) {
-                uint4 *pb = reinterpret_cast<uint4 *>(stage + a_off + q * (64 * 16));
+                const uint4 *pb = reinterpret_cast<const uint4 *>(stage + a_off + q * (64 * 16));
                 uint4 *ps = reinterpret_cast<uint4 *>(stage + TQ_A_IMG + a_off + q * (64 * 16));
+                // (the landed image itself is a_big: the tensor core reads the top 19 bits of each fp32 word and ignores the 13
+                // low mantissa bits; storing the masked words back changes no result bit and was measured, so it is not done)
                 const uint4 x = *pb;
                 uint4 b, sm;
                 b.x = x.x & 0xffffe000u; b.y = x.y & 0xffffe000u; b.z = x.z & 0xffffe000u; b.w = x.w & 0xffffe000u;
@@ -441,7 +443,6 @@ __global__ void __launch_bounds__(TQ_THREADS, 1) k_wg_gemm_tf32(const __grid_con
                 sm.y = __float_as_uint(__uint_as_float(x.y) - __uint_as_float(b.y));
                 sm.z = __float_as_uint(__uint_as_float(x.z) - __uint_as_float(b.z));
                 sm.w = __float_as_uint(__uint_as_float(x.w) - __uint_as_float(b.w));
-                *pb = b;
                 *ps = sm;
             }
             tc::proxy_fence();

@@ -180,3 +180,14 @@ def test_wide_fp64_md_with_buffered_list():
     th = out["thermo"].cpu().numpy()
     assert np.abs(th[:, 0] - o["thermo"][:, 0]).max() <= 1e-12 * abs(o["thermo"][0, 0])
     m.close()
+
+
+def test_unsupported_widths_are_refused():
+    """embedding widths outside (25 | 32 | 64 | 128 | 256 | 512) x (1, 2, 4): DP_EUNSUPPORTED (include/dp.h), in every precision"""
+    from paper_2005_00223_b200 import binding
+    for W in (48, 96):
+        s = synth.wide_copper(5, W, 777)
+        for prec in ("fp64", "mix32", "mix16"):
+            with pytest.raises(binding.DPError) as ei:
+                binding.DPModel(s.model, prec)
+            assert ei.value.code == -7
