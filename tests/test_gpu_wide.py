@@ -191,3 +191,26 @@ def test_unsupported_widths_are_refused():
             with pytest.raises(binding.DPError) as ei:
                 binding.DPModel(s.model, prec)
             assert ei.value.code == -7
+
+
+@pytest.mark.parametrize("prec", ["fp64", "mix32", "mix16"])
+def test_wide_empty_type_blocks(prec):
+    """A two-type model on a system whose atoms are all of type 0: the (1, .) blocks have no rows and no tiles, the (0, 1) block
+    consists of padded-slot representatives only (one weighted row per atom, no gradient)"""
+    s = synth.wide_water(64, 14.0, 64, 781, precision=prec)
+    types = np.zeros_like(s.types)
+    o = oracle.evaluate(s.coords, types, s.box, s.model)
+    import torch
+    from paper_2005_00223_b200 import binding
+    m = binding.DPModel(s.model, prec)
+    out = m.compute(torch.from_numpy(s.coords).cuda(), torch.from_numpy(types).cuda(), s.box)
+    rc, ntr = m.status()
+    assert rc == 0 and ntr == o["n_truncated"]
+    nl = m.get_nlist().cpu().numpy()
+    g = {k: v.cpu().numpy() for k, v in out.items()}
+    m.close()
+    assert np.array_equal(nl, o["nlist"])
+    rms = np.sqrt((o["forces"] ** 2).mean())
+    err = np.abs(g["forces"] - o["forces"]).max() / rms
+    assert err <= {"fp64": 1e-10, "mix32": 1e-4, "mix16": 5e-3}[prec], err
+    assert abs(g["energy"][0] - o["energy"]) / len(types) <= {"fp64": 1e-12, "mix32": 2e-5, "mix16": 1e-3}[prec]
