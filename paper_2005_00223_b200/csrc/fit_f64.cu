@@ -278,28 +278,54 @@ __global__ void __launch_bounds__(256) k_descr_wide(int M2, const double *__rest
     D[i * (M2 * 16L) + idx] = acc;
 }
 // gA[c][m] = sum_a gD[m][a] A[c][a] + [m < 16] sum_m' gD[m'][m] A[c][m']   (N8), row-major [N][4][M2], without the 1 / Nm that
-// the backward head applies.  One CTA per atom: a thread per (c, m) for the first sum, a warp per eight (c, m < 16) for the second.
+// the backward head applies.  One CTA per atom.  Second sum (a 4 x M2 by M2 x 16 product): thread (m', quarter q of the 16
+// columns) reads 32 contiguous bytes of gD[m'] and keeps 4 x 4 partial sums; lanes of equal q meet by shuffles, warps in
+// shared memory.  First sum: a thread per (c, m) reads the 128 contiguous bytes of gD[m].
 __global__ void __launch_bounds__(256) k_gA_wide(int M2, const double *__restrict__ Amat, const double *__restrict__ gD,
                                                  double *__restrict__ gA) {
+    __shared__ double part[8][64];
     __shared__ double s2[64];
     const long i = blockIdx.x;
     const double *A = Amat + i * 4L * M2, *G = gD + i * (M2 * 16L);
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int o = warp * 8; o < warp * 8 + 8; ++o) {
-        const int c = o >> 4, mm = o & 15;
-        double acc = 0.0;
-        for (int mp = lane; mp < M2; mp += 32) acc += G[mp * 16 + mm] * A[c * M2 + mp];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, q = threadIdx.x & 3;
+    double acc[4][4];
 #pragma unroll
-        for (int sh = 16; sh > 0; sh >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, sh);
-        if (lane == 0) s2[o] = acc;
+    for (int c = 0; c < 4; ++c)
+#pragma unroll
+        for (int k = 0; k < 4; ++k) acc[c][k] = 0.0;
+    for (int mp = threadIdx.x >> 2; mp < M2; mp += 64) {
+        const double2 g0 = *reinterpret_cast<const double2 *>(G + mp * 16 + 4 * q), g1 = *reinterpret_cast<const double2 *>(G + mp * 16 + 4 * q + 2);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const double a = A[c * M2 + mp];
+            acc[c][0] += g0.x * a; acc[c][1] += g0.y * a; acc[c][2] += g1.x * a; acc[c][3] += g1.y * a;
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            double v = acc[c][k];
+            v += __shfl_xor_sync(0xffffffffu, v, 4);
+            v += __shfl_xor_sync(0xffffffffu, v, 8);
+            v += __shfl_xor_sync(0xffffffffu, v, 16);
+            if (lane < 4) part[warp][c * 16 + 4 * q + k] = v;
+        }
+    __syncthreads();
+    if (threadIdx.x < 64) {
+        double v = 0.0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) v += part[w][threadIdx.x];
+        s2[threadIdx.x] = v;
     }
     __syncthreads();
     for (int idx = threadIdx.x; idx < 4 * M2; idx += 256) {
         const int c = idx / M2, mm = idx % M2;
-        double acc = mm < 16 ? s2[c * 16 + mm] : 0.0;
+        double acc1 = mm < 16 ? s2[c * 16 + mm] : 0.0;
+        const double2 *g = reinterpret_cast<const double2 *>(G + mm * 16);
 #pragma unroll
-        for (int ax = 0; ax < 16; ++ax) acc += G[mm * 16 + ax] * A[c * M2 + ax];
-        gA[i * 4L * M2 + idx] = acc;
+        for (int ax = 0; ax < 8; ++ax) { const double2 v = g[ax]; acc1 += v.x * A[c * M2 + 2 * ax] + v.y * A[c * M2 + 2 * ax + 1]; }
+        gA[i * 4L * M2 + idx] = acc1;
     }
 }
 
