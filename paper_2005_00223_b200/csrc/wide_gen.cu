@@ -328,35 +328,44 @@ __global__ void __launch_bounds__(256, 1) k_wg_gemm_f64(const __grid_constant__ 
 
 // ---- MIX-32 on the 5th-generation tensor cores: tcgen05.mma kind::tf32, three products per K step ("3xTF32") -------------------
 // C = A B with A = the fp32 activations [rows][K] and B^T = a weight matrix [NTOT][K] (both K-major operands: dp_create keeps every
-// matrix and its transpose).  Persistent, one CTA per SM, warp-specialised:
+// matrix and its transpose).  Persistent, one CTA PAIR per two SMs (cluster of 2, tcgen05 cta_group::2): the pair computes
+// two 128-row tiles of one net against one N tile; each CTA stages its own rows of A and HALF of the B tile, and the MMA of the
+// leader (M = 256) reads both halves, so a CTA moves and reads half the weight bytes of a single-CTA tile.  Per CTA:
 //   warp 13    loader (one thread): per K = 16 stage ONE TMA tensor copy of A (the row-major activations seen as a
 //              (4, rows, K / 4) tensor, box {4, 128, 4}: it lands as the un-swizzled K-major operand image, per 16 bytes of K a
-//              column [128 rows][16 B]) and ONE bulk copy of the weights' operand images (TF32 values and TF32 remainders, laid
-//              out by dp_create), both counted by the stage's "landed" barrier;
+//              column [128 rows][16 B]) and ONE bulk copy of this CTA's half of the weights' operand images (TF32 values and TF32
+//              remainders, laid out by dp_create), both counted by the stage's "landed" barrier;
 //   warps 0-7  splitters: a_small = a - a_big (exact) into a second image, a_big = a with the 13 low mantissa bits cleared = what
-//              the tensor core reads from the landed image itself; fence.proxy.async; arrive on the stage's "full" barrier;
-//   warp 12    MMA issuer: per K = 8 step a_small b_big, a_big b_small, a_big b_big into one of two 128 x BN fp32 accumulators
-//              in TMEM; tcgen05.commit frees the stage, the last one of a tile hands the accumulator over;
-//   warps 8-11 epilogue: thread = row = TMEM lane, tcgen05.ld of 16 columns at a time, the layer's bias / tanh / skip / tanh'
-//              work on the row-major fp32 activations.
+//              the tensor core reads from the landed image itself; fence.proxy.async; arrive on the LEADER's "full" barrier
+//              (the peer's threads through its cluster address);
+//   warp 12    MMA issuer (leader only): per K = 8 step a_small b_big, a_big b_small, a_big b_big into one of two 256 x BN fp32
+//              accumulators (128 TMEM lanes in each CTA); tcgen05.commit multicasts "stage free" and "accumulator ready" to both CTAs;
+//   warps 8-11 epilogue: thread = row = TMEM lane, 32 columns per step, the layer's bias / tanh / skip / tanh' work on the
+//              row-major fp32 activations; "accumulator drained" goes to the leader.
 constexpr int TQ_KC = 16;                          // K per stage: 4 pieces of 16 bytes
-constexpr int TQ_NST = 4;
+constexpr int TQ_NST = 6;
 constexpr int TQ_A_PIECE = 128 * 16;               // distance between the piece columns of an image (the descriptors' LBO)
 constexpr int TQ_A_IMG = 4 * TQ_A_PIECE;           // 8 KB: [4 pieces][128 rows][16 B], written by one TMA tensor copy
-constexpr int TQ_B_IMG = 256 * TQ_KC * 4;          // 16 KB (BN <= 256), un-padded: written by dp_create, one bulk copy per stage
+constexpr int TQ_B_IMG = 128 * TQ_KC * 4;          // 8 KB: this CTA's half (<= 128 rows of B^T) of one weight image
 constexpr int TQ_STAGE = 2 * TQ_A_IMG + 2 * TQ_B_IMG;      // a_big | a_small | b_big | b_small
 constexpr int TQ_OFF_BAR = TQ_NST * TQ_STAGE;
 constexpr int TQ_TOTAL = TQ_OFF_BAR + 256;
 constexpr int TQ_THREADS = 448;                  // 8 splitter, 4 epilogue warps, the MMA warp, the loader warp
 static_assert(TQ_TOTAL + 1024 <= 227 * 1024, "shared memory budget");
+static_assert((3 * TQ_NST + 4) * 8 <= 256, "barriers");
 
-__device__ __forceinline__ void mma_tf32_ss(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t id, bool accumulate) {
-    asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}"
+__device__ __forceinline__ void mma_tf32_ss2(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t id, bool accumulate) {
+    asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::2.kind::tf32 [%0], %1, %2, %3, p;\n}"
                  ::"r"(tmem_d), "l"(da), "l"(db), "r"(id), "r"((uint32_t)accumulate) : "memory");
 }
 // kind::tf32 instruction descriptor: tf32 x tf32 -> fp32, M x N, both operands K-major
 __host__ __device__ constexpr uint32_t idesc_tf32(int M, int N) {
     return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+// the MMAs issued so far by this thread arrive on the barrier at this shared-memory offset in BOTH CTAs of the pair
+__device__ __forceinline__ void commit_pair(uint64_t *bar) {
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+                 ::"r"(tc::smem_u32(bar)), "h"((uint16_t)3) : "memory");
 }
 __device__ __forceinline__ void mbar_expect_tx_cta(uint64_t *bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(tc::smem_u32(bar)), "r"(bytes) : "memory");
@@ -365,59 +374,100 @@ __device__ __forceinline__ void bulk_g2s_cta(uint32_t sdst, const void *gsrc, ui
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(sdst), "l"(gsrc), "r"(bytes), "r"(tc::smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void mbar_arrive_cta(uint64_t *bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(tc::smem_u32(bar)) : "memory");
+// arrive on the barrier at this shared-memory offset in the leader CTA (rank 0 of the pair), from either CTA.  Release at CTA
+// scope (the default), as cluster barriers are commonly signalled: what the arrival publishes is shared memory of the arriving
+// CTA that its own fence.proxy.async has handed to the asynchronous proxy.  A .release.cluster here compiles to a memory
+// barrier per arrival and made the pairs 1.4x SLOWER than single CTAs (ncu: 9.9 membar stall cycles per issued instruction).
+__device__ __forceinline__ void mbar_arrive_leader(uint64_t *bar) {
+    asm volatile("{\n.reg .b32 ra;\nmapa.shared::cluster.u32 ra, %0, 0;\nmbarrier.arrive.shared::cluster.b64 _, [ra];\n}"
+                 ::"r"(tc::smem_u32(bar)) : "memory");
 }
-
+// wait for a phase that CTAs of the cluster complete (acquire at cluster scope)
+__device__ __forceinline__ void mbar_wait_cluster(uint64_t *bar, uint32_t parity) {
+    asm volatile("{\n.reg .pred p;\nWAITC_%=:\nmbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n@p bra DONEC_%=;\nbra WAITC_%=;\nDONEC_%=:\n}"
+                 ::"r"(tc::smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
 // box {4 elements, 128 rows, 4 pieces} of the activation tensor viewed as (4, rows, K / 4) -> the [4][128][16 B] operand image
 __device__ __forceinline__ void tma_load_3d(uint32_t sdst, const CUtensorMap *tm, int c0, int c1, int c2, uint64_t *bar) {
     asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
                  ::"r"(sdst), "l"((uint64_t)tm), "r"(c0), "r"(c1), "r"(c2), "r"(tc::smem_u32(bar)) : "memory");
 }
 
+// Work item w of the pairs: (pair of consecutive tiles of one block, N tile).  Returns the block; row0 / nrows of this CTA's tile
+// (nrows <= 0: the block has an odd number of tiles and this CTA of its last pair has none: it stages operands, stores nothing).
+__device__ __forceinline__ int pair_item(const GenArgs<float> &p, int nblk, int NT, long w, int rank, int &nt, long &row0, int &nrows) {
+    const int pt = (int)(w / NT);
+    nt = (int)(w % NT);
+    int k = 0, base = 0;
+    for (;; ++k) {
+        const int ntk = k + 1 < nblk + 1 ? p.tab[k + 1].x - p.tab[k].x : 0;        // tiles of block k (entry nblk = {tiles})
+        const int np = (ntk + 1) >> 1;
+        if (pt < base + np || k == nblk - 1) break;
+        base += np;
+    }
+    const int4 e = p.tab[k];
+    const int t = 2 * (pt - base) + rank;
+    const int r0 = e.y + t * GR;
+    nrows = min(GR, e.z - r0);
+    row0 = p.N * (long)p.tt.off[k % p.T] + r0;
+    return k;
+}
+__device__ __forceinline__ long pair_count(const GenArgs<float> &p, int nblk) {
+    long n = 0;
+    for (int k = 0; k < nblk; ++k) n += (p.tab[k + 1].x - p.tab[k].x + 1) >> 1;
+    return n;
+}
+
 template <int MODE>
-__global__ void __launch_bounds__(TQ_THREADS, 1) k_wg_gemm_tf32(const __grid_constant__ GenArgs<float> p, const __grid_constant__ CUtensorMap tmA) {
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(TQ_THREADS, 1)
+k_wg_gemm_tf32(const __grid_constant__ GenArgs<float> p, const __grid_constant__ CUtensorMap tmA) {
     extern __shared__ __align__(1024) unsigned char tq_smem[];
     __shared__ uint32_t tmem_base_s;
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
+    uint32_t rank;
+    asm("mov.u32 %0, %%cluster_ctarank;" : "=r"(rank));
     uint64_t *bars = reinterpret_cast<uint64_t *>(tq_smem + TQ_OFF_BAR);
-    uint64_t *full = bars, *empty = bars + TQ_NST, *acc_full = bars + 2 * TQ_NST, *acc_empty = acc_full + 2, *landed = acc_empty + 2;
+    uint64_t *full = bars, *empty = bars + TQ_NST, *landed = bars + 2 * TQ_NST, *acc_full = bars + 3 * TQ_NST, *acc_empty = acc_full + 2;
     if (tid == 0) {
-        for (int k = 0; k < TQ_NST; ++k) { tc::mbar_init(&full[k], 256); tc::mbar_init(&empty[k], 1); tc::mbar_init(&landed[k], 1); }
-        for (int k = 0; k < 2; ++k) { tc::mbar_init(&acc_full[k], 1); tc::mbar_init(&acc_empty[k], 4); }
+        for (int k = 0; k < TQ_NST; ++k) { tc::mbar_init(&full[k], 16); tc::mbar_init(&empty[k], 1); tc::mbar_init(&landed[k], 1); }
+        for (int k = 0; k < 2; ++k) { tc::mbar_init(&acc_full[k], 1); tc::mbar_init(&acc_empty[k], 8); }
         asm volatile("fence.mbarrier_init.release.cluster;");
     }
-    if (warp == 12) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tc::smem_u32(&tmem_base_s)), "n"(512));
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    if (warp == 12) {      // the same warp of both CTAs, the same shared-memory word
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tc::smem_u32(&tmem_base_s)), "n"(512));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;");
     }
     tc::fence_before();
-    __syncthreads();
+    cluster_sync_all();
     tc::fence_after();
     const uint32_t tmem = tmem_base_s;
     const uint32_t sbase = tc::smem_u32(tq_smem);
-    const int nblk = p.T * p.T, ntiles = p.tab[nblk].x;
-    const int W = p.W, K = p.K, BN = p.NTOT < 256 ? p.NTOT : 256, NT = p.NTOT / BN, NKC = K / TQ_KC;
-    const long nwork = (long)ntiles * NT;          // work item = (row tile, N tile), the N tiles of a row tile adjacent
+    const int nblk = p.T * p.T;
+    const int W = p.W, K = p.K, BN = p.NTOT < 256 ? p.NTOT : 256, HB = BN / 2, NT = p.NTOT / BN, NKC = K / TQ_KC;
+    const long nwork = pair_count(p, nblk) * NT;   // work item = (pair of row tiles, N tile), the N tiles of a pair adjacent
+    const long pair0 = blockIdx.x >> 1, npair = gridDim.x >> 1;
 
     if (warp == 13) {
         // ------------------------------------------------------------------------------------------------ loader
         if (lane == 0) {
-            const uint32_t b_stage_bytes = 2u * BN * TQ_KC * 4;                 // TF32 values and remainders of one stage
+            const uint32_t b_half_bytes = 2u * HB * TQ_KC * 4;                  // TF32 values and remainders of HB rows of B^T
             uint32_t step = 0;
-            for (long w = blockIdx.x; w < nwork; w += gridDim.x) {
-                const int tile = (int)(w / NT), nt = (int)(w % NT);
-                const int k = wg_block(p.tab, nblk, tile);
-                const int4 e = p.tab[k];
-                const long row = p.N * (long)p.tt.off[k % p.T] + e.y + (long)(tile - e.x) * GR;       // first row of the tile
-                const float *Bg = p.nets + k * p.net_stride + p.b_off + (long)nt * NKC * (2 * BN * TQ_KC);
+            for (long w = pair0; w < nwork; w += npair) {
+                int nt, nrows;
+                long row0;
+                const int k = pair_item(p, nblk, NT, w, (int)rank, nt, row0, nrows);
+                if (nrows <= 0) row0 -= GR;                                     // no tile of its own: any valid rows will do
+                const float *Bg = p.nets + k * p.net_stride + p.b_off + ((long)nt * NKC * 2 + rank) * (2 * HB * TQ_KC);
                 for (int kc = 0; kc < NKC; ++kc, ++step) {
                     const int st = step % TQ_NST;
                     tc::mbar_wait(&empty[st], ((step / TQ_NST) & 1) ^ 1);
-                    mbar_expect_tx_cta(&landed[st], TQ_A_IMG + b_stage_bytes);
-                    tma_load_3d(sbase + st * TQ_STAGE, &tmA, 0, (int)row, kc * 4, &landed[st]);
-                    bulk_g2s_cta(sbase + st * TQ_STAGE + 2 * TQ_A_IMG, Bg + (long)kc * (2 * BN * TQ_KC), b_stage_bytes, &landed[st]);
+                    mbar_expect_tx_cta(&landed[st], TQ_A_IMG + b_half_bytes);
+                    tma_load_3d(sbase + st * TQ_STAGE, &tmA, 0, (int)row0, kc * 4, &landed[st]);
+                    bulk_g2s_cta(sbase + st * TQ_STAGE + 2 * TQ_A_IMG, Bg + (long)kc * 2 * (2 * HB * TQ_KC), b_half_bytes, &landed[st]);
                 }
             }
         }
@@ -425,17 +475,17 @@ __global__ void __launch_bounds__(TQ_THREADS, 1) k_wg_gemm_tf32(const __grid_con
         // ------------------------------------------------------------------------------------------------ splitters
         // every thread splits two 16-byte pieces of the landed A image: a_small into the second image
         const uint32_t a_off = ((tid >> 3) & 3) * TQ_A_PIECE + (8 * (tid >> 5) + (tid & 7)) * 16;      // + 64 rows for the second piece
-        const long nstage = nwork > (long)blockIdx.x ? ((nwork - blockIdx.x + gridDim.x - 1) / gridDim.x) * NKC : 0;
+        const long nstage = nwork > pair0 ? ((nwork - pair0 + npair - 1) / npair) * NKC : 0;
         for (long it = 0; it < nstage; ++it) {
             const int st = (int)(it % TQ_NST);
             tc::mbar_wait(&landed[st], (uint32_t)((it / TQ_NST) & 1));
             unsigned char *stage = tq_smem + st * TQ_STAGE;
 #pragma unroll
             for (int q = 0; q < 2; ++q) {
-                const uint4 *pb = reinterpret_cast<const uint4 *>(stage + a_off + q * (64 * 16));
-                uint4 *ps = reinterpret_cast<uint4 *>(stage + TQ_A_IMG + a_off + q * (64 * 16));
                 // (the landed image itself is a_big: the tensor core reads the top 19 bits of each fp32 word and ignores the 13
                 // low mantissa bits; storing the masked words back changes no result bit and was measured, so it is not done)
+                const uint4 *pb = reinterpret_cast<const uint4 *>(stage + a_off + q * (64 * 16));
+                uint4 *ps = reinterpret_cast<uint4 *>(stage + TQ_A_IMG + a_off + q * (64 * 16));
                 const uint4 x = *pb;
                 uint4 b, sm;
                 b.x = x.x & 0xffffe000u; b.y = x.y & 0xffffe000u; b.z = x.z & 0xffffe000u; b.w = x.w & 0xffffe000u;
@@ -446,52 +496,53 @@ __global__ void __launch_bounds__(TQ_THREADS, 1) k_wg_gemm_tf32(const __grid_con
                 *ps = sm;
             }
             tc::proxy_fence();
-            mbar_arrive_cta(&full[st]);
+            __syncwarp();
+            if (lane == 0) mbar_arrive_leader(&full[st]);         // one arrival per warp: 8 local + 8 from the peer
         }
     } else if (warp == 12) {
-        // ------------------------------------------------------------------------------------------------ MMA issuer
-        const uint32_t idesc = idesc_tf32(128, BN);
-        uint32_t step = 0, accn = 0;
-        for (long w = blockIdx.x; w < nwork; w += gridDim.x, ++accn) {
-            const int buf = accn & 1;
-            tc::mbar_wait(&acc_empty[buf], ((accn >> 1) & 1) ^ 1);
-            tc::fence_after();
-            for (int kc = 0; kc < NKC; ++kc, ++step) {
-                const int st = step % TQ_NST;
-                tc::mbar_wait(&full[st], (step / TQ_NST) & 1);
+        // ------------------------------------------------------------------------------------------------ MMA issuer (leader)
+        if (rank == 0) {
+            const uint32_t idesc = idesc_tf32(256, BN);
+            const uint32_t B_PIECE = HB * 16;
+            uint32_t step = 0, accn = 0;
+            for (long w = pair0; w < nwork; w += npair, ++accn) {
+                const int buf = accn & 1;
+                mbar_wait_cluster(&acc_empty[buf], ((accn >> 1) & 1) ^ 1);
                 tc::fence_after();
-                const uint32_t sa = sbase + st * TQ_STAGE;
-                const uint32_t B_PIECE = BN * 16;
-                const uint64_t dab = tc::desc(sa, TQ_A_PIECE, 128), das = tc::desc(sa + TQ_A_IMG, TQ_A_PIECE, 128);
-                const uint64_t dbb = tc::desc(sa + 2 * TQ_A_IMG, B_PIECE, 128), dbs = tc::desc(sa + 2 * TQ_A_IMG + BN * TQ_KC * 4, B_PIECE, 128);
-                if (tc::elect_one()) {
+                for (int kc = 0; kc < NKC; ++kc, ++step) {
+                    const int st = step % TQ_NST;
+                    mbar_wait_cluster(&full[st], (step / TQ_NST) & 1);
+                    tc::fence_after();
+                    const uint32_t sa = sbase + st * TQ_STAGE;
+                    const uint64_t dab = tc::desc(sa, TQ_A_PIECE, 128), das = tc::desc(sa + TQ_A_IMG, TQ_A_PIECE, 128);
+                    const uint64_t dbb = tc::desc(sa + 2 * TQ_A_IMG, B_PIECE, 128), dbs = tc::desc(sa + 2 * TQ_A_IMG + HB * TQ_KC * 4, B_PIECE, 128);
+                    if (tc::elect_one()) {
 #pragma unroll
-                    for (int ks = 0; ks < TQ_KC / 8; ++ks) {
-                        const uint32_t oa = ks * 2 * TQ_A_PIECE, ob = ks * 2 * B_PIECE;
-                        mma_tf32_ss(tmem + buf * 256, tc::desc_at(das, oa), tc::desc_at(dbb, ob), idesc, (kc | ks) != 0);     // small terms first
-                        mma_tf32_ss(tmem + buf * 256, tc::desc_at(dab, oa), tc::desc_at(dbs, ob), idesc, true);
-                        mma_tf32_ss(tmem + buf * 256, tc::desc_at(dab, oa), tc::desc_at(dbb, ob), idesc, true);
+                        for (int ks = 0; ks < TQ_KC / 8; ++ks) {
+                            const uint32_t oa = ks * 2 * TQ_A_PIECE, ob = ks * 2 * B_PIECE;
+                            mma_tf32_ss2(tmem + buf * 256, tc::desc_at(das, oa), tc::desc_at(dbb, ob), idesc, (kc | ks) != 0);     // small terms first
+                            mma_tf32_ss2(tmem + buf * 256, tc::desc_at(dab, oa), tc::desc_at(dbs, ob), idesc, true);
+                            mma_tf32_ss2(tmem + buf * 256, tc::desc_at(dab, oa), tc::desc_at(dbb, ob), idesc, true);
+                        }
+                        commit_pair(&empty[st]);
                     }
-                    tc::commit(&empty[st]);
+                    __syncwarp();
                 }
+                if (tc::elect_one()) commit_pair(&acc_full[buf]);
                 __syncwarp();
             }
-            if (tc::elect_one()) tc::commit(&acc_full[buf]);
-            __syncwarp();
         }
     } else {
         // ------------------------------------------------------------------------------------------------ epilogue
         const int q4 = warp & 3, r = q4 * 32 + lane;
         const uint32_t tm_lane = tmem + ((uint32_t)(q4 * 32) << 16);
         uint32_t accn = 0;
-        for (long w = blockIdx.x; w < nwork; w += gridDim.x, ++accn) {
-            const int tile = (int)(w / NT), nt = (int)(w % NT);
-            const int k = wg_block(p.tab, nblk, tile);
-            const int4 e = p.tab[k];
-            const long rbase = p.N * (long)p.tt.off[k % p.T];
-            const int row0 = e.y + (tile - e.x) * GR, nrows = min(GR, e.z - row0);
+        for (long w = pair0; w < nwork; w += npair, ++accn) {
+            int nt, nrows;
+            long row0;
+            const int k = pair_item(p, nblk, NT, w, (int)rank, nt, row0, nrows);
             const float *net = p.nets + k * p.net_stride;
-            const long Rg = rbase + row0 + r;
+            const long Rg = row0 + r;
             const bool ok = r < nrows;
             const int buf = accn & 1;
             tc::mbar_wait(&acc_full[buf], (accn >> 1) & 1);
@@ -553,13 +604,13 @@ __global__ void __launch_bounds__(TQ_THREADS, 1) k_wg_gemm_tf32(const __grid_con
             }
             tc::fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cta(&acc_empty[buf]);
+            if (lane == 0) mbar_arrive_leader(&acc_empty[buf]);
         }
     }
     tc::fence_before();
-    __syncthreads();
+    cluster_sync_all();
     tc::fence_after();
-    if (warp == 12) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(512));
+    if (warp == 12) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(512));
 }
 
 // S5: A_i[c][m] = (1 / Nm) sum over the atom's rows of wt R^[c] G[m], G[m] = y2[m mod 2 W] + t3[m]; wt = the number of padded
@@ -776,17 +827,18 @@ static void build_net(int W, const double *net, R *out) {
             out[wg_off_W3T(W) + (size_t)m * 2 * W + f] = (R)W3[(size_t)f * 4 * W + m];
         }
 }
-// MIX-32: the operand images of B^T [NTOT][K] of one product: per N tile (BN = min(256, NTOT) rows) and per K = 16 stage the
-// TF32 values [4 pieces][BN][4] followed by the TF32 remainders in the same order (one contiguous bulk copy per stage)
+// MIX-32: the operand images of B^T [NTOT][K] of one product: per N tile (BN = min(256, NTOT) rows), per K = 16 stage and per half
+// of the tile's rows (one half per CTA of a pair) the TF32 values [4 pieces][BN / 2][4] followed by the TF32 remainders in the
+// same order (one contiguous bulk copy per stage and CTA)
 static void tf32_image(const std::vector<float> &Bt, int NTOT, int K, float *out) {
-    const int BN = NTOT < 256 ? NTOT : 256, NKC = K / TQ_KC;
+    const int BN = NTOT < 256 ? NTOT : 256, HB = BN / 2, NKC = K / TQ_KC;
     for (int n = 0; n < NTOT; ++n)
         for (int k = 0; k < K; ++k) {
             const float x = Bt[(size_t)n * K + k], big = tf32_rna(x), small = tf32_rna(x - big);
-            const size_t stage = ((size_t)(n / BN) * NKC + k / TQ_KC) * (2 * (size_t)BN * TQ_KC);
-            const size_t in = (size_t)((k % TQ_KC) / 4) * (BN * 4) + (size_t)(n % BN) * 4 + (k % 4);
-            out[stage + in] = big;
-            out[stage + (size_t)BN * TQ_KC + in] = small;
+            const size_t half = ((size_t)((n / BN) * NKC + k / TQ_KC) * 2 + (n % BN) / HB) * (2 * (size_t)HB * TQ_KC);
+            const size_t in = (size_t)((k % TQ_KC) / 4) * (HB * 4) + (size_t)(n % HB) * 4 + (k % 4);
+            out[half + in] = big;
+            out[half + (size_t)HB * TQ_KC + in] = small;
         }
 }
 __host__ __device__ inline long wg_off_img(int W, int mode) {      // MODE 0: W2^T, 1: W3^T, 2: W3, 3: W2 as B^T [NTOT][K]
@@ -850,7 +902,7 @@ static cudaError_t gen_gemm_tf32(const dp_model *m, GenArgs<float> p, int K, int
     if (enc(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)A, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
         return cudaErrorInvalidValue;
-    k_wg_gemm_tf32<MODE><<<m->num_sms, TQ_THREADS, TQ_TOTAL, st>>>(p, tm);
+    k_wg_gemm_tf32<MODE><<<m->num_sms & ~1, TQ_THREADS, TQ_TOTAL, st>>>(p, tm);      // CTA pairs (__cluster_dims__(2, 1, 1))
     return cudaGetLastError();
 }
 
