@@ -8,8 +8,10 @@
 //   * activations live in HBM as ready-made tcgen05 operand images: per 128-row tile and per 8 columns one 2 KB block
 //     [128 rows][8 fp16], so a K = 64 slice of the A operand is ONE contiguous 16 KB cp.async.bulk, and an epilogue thread
 //     (= row) writes 16 bytes per 8 columns, a warp 512 contiguous bytes;
-//   * k_wide_gemm: persistent, warp-specialised: warp 0 streams A and B stages (mbarrier transactions), warp 1 issues
-//     tcgen05.mma 128 x BN x 16 (BN <= 256) into one of two TMEM accumulators, eight epilogue warps drain the other one;
+//   * k_wide_gemm: persistent, warp-specialised, CTA pairs (cluster of 2, tcgen05 cta_group::2: a pair takes two consecutive row
+//     tiles of one net against one N tile, each CTA staging its own A tile and half of the B tile): warp 0 streams A and B
+//     stages (mbarrier transactions), warp 1 of the leader issues tcgen05.mma 256 x BN x 16 (BN <= 256) into one of two TMEM
+//     accumulators (warp 1 of the peer relays "stage landed"), eight epilogue warps drain the other one;
 //   * the backward overwrites in place: dz3 over t3, dz2 over t2, (gG_lo + gG_hi) and then dy2 over y2.
 // Forward:  k_wide_l1 (t1)  ->  gemm<0> (t2, y2 = (t1,t1) + t2)  ->  gemm<1> (t3)  ->  k_wide_contract (A_i = R^T G / Nm)
 // Backward: k_wide_gscale  ->  k_wide_bwd_elem (gG = R^ gA, dz3, dR^ = G gA^T)  ->  gemm<2> (dy2, dz2)  ->  gemm<3> (dy1,
@@ -24,9 +26,9 @@ namespace {
 
 constexpr int WR = 128;                        // rows per tile
 constexpr int WKC = 64;                        // K per pipeline stage: 8 chunks of 8 columns
-constexpr int WNST = 4;                        // pipeline stages
+constexpr int WNST = 6;                        // pipeline stages
 constexpr int W_A_STAGE = WR * WKC * 2;        // 16 KB
-constexpr int W_B_STAGE = 256 * WKC * 2;       // 32 KB (BN <= 256)
+constexpr int W_B_STAGE = 128 * WKC * 2;       // 16 KB: this CTA's half (<= 128 rows) of the B tile (BN <= 256)
 constexpr int W_OFF_A = 0;
 constexpr int W_OFF_B = WNST * W_A_STAGE;
 constexpr int W_OFF_BAR = W_OFF_B + WNST * W_B_STAGE;
@@ -40,6 +42,47 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
 }
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(tc::smem_u32(bar)) : "memory");
+}
+// ---- CTA pairs (cluster of 2, tcgen05 cta_group::2): the leader (rank 0) issues M = 256 MMAs over both CTAs' operands
+__device__ __forceinline__ void mma_ss2(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t id, bool accumulate) {
+    asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n}"
+                 ::"r"(tmem_d), "l"(da), "l"(db), "r"(id), "r"((uint32_t)accumulate) : "memory");
+}
+// the MMAs issued so far by this thread arrive on the barrier at this shared-memory offset in BOTH CTAs of the pair
+__device__ __forceinline__ void commit_pair(uint64_t *bar) {
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+                 ::"r"(tc::smem_u32(bar)), "h"((uint16_t)3) : "memory");
+}
+// arrive on the barrier at this shared-memory offset in the leader CTA, from either CTA (release at CTA scope, the default: a
+// .release.cluster compiles to a memory barrier per arrival and made pairs slower than single CTAs)
+__device__ __forceinline__ void mbar_arrive_leader(uint64_t *bar) {
+    asm volatile("{\n.reg .b32 ra;\nmapa.shared::cluster.u32 ra, %0, 0;\nmbarrier.arrive.shared::cluster.b64 _, [ra];\n}"
+                 ::"r"(tc::smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_cluster(uint64_t *bar, uint32_t parity) {
+    asm volatile("{\n.reg .pred p;\nWAITC_%=:\nmbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n@p bra DONEC_%=;\nbra WAITC_%=;\nDONEC_%=:\n}"
+                 ::"r"(tc::smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// Pair pw of the tile table: two consecutive tiles of one block (one net).  Returns the block; tile = this CTA's tile, valid =
+// false for the second CTA of the last pair of a block with an odd number of tiles (it stages operands and stores nothing).
+__device__ __forceinline__ int wide_pair(const int4 *tab, int nblk, int pw, int rank, int &tile, bool &valid) {
+    int k = 0, base = 0;
+    for (;; ++k) {
+        const int np = (tab[k + 1].x - tab[k].x + 1) >> 1;
+        if (pw < base + np || k == nblk - 1) break;
+        base += np;
+    }
+    tile = tab[k].x + 2 * (pw - base) + rank;
+    valid = tile < tab[k + 1].x;
+    return k;
+}
+__device__ __forceinline__ int wide_pair_count(const int4 *tab, int nblk) {
+    int n = 0;
+    for (int k = 0; k < nblk; ++k) n += (tab[k + 1].x - tab[k].x + 1) >> 1;
+    return n;
 }
 __device__ __forceinline__ void bulk_g2s(uint32_t sdst, const void *gsrc, uint32_t bytes, uint64_t *bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -125,86 +168,116 @@ struct WideArgs {
 // MODE 3: layer 2 backward  A = dz2 (K = 2 W), N = W:    dy1 = acc + dy2[e] + dy2[e + W];  dz1 = dy1 (1 - t1^2);  ds^ = dz1 . w1;
 //                           rows_g = dE/dR~ of the row (dR^ from k_wide_bwd_elem + ds^ on component 0, unscaled, / std)
 template <int MODE>
-__global__ void __launch_bounds__(W_THREADS, 1) k_wide_gemm(const __grid_constant__ WideArgs p) {
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(W_THREADS, 1) k_wide_gemm(const __grid_constant__ WideArgs p) {
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ uint32_t tmem_base_s;
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem + W_OFF_BAR);
-    uint64_t *full = bars, *empty = bars + WNST, *acc_full = bars + 2 * WNST, *acc_empty = acc_full + 2;
+    uint64_t *full = bars, *empty = bars + WNST, *pfull = bars + 2 * WNST, *acc_full = bars + 3 * WNST, *acc_empty = acc_full + 2;
+    uint32_t rank;
+    asm("mov.u32 %0, %%cluster_ctarank;" : "=r"(rank));
     if (tid == 0) {
-        for (int k = 0; k < WNST; ++k) { tc::mbar_init(&full[k], 1); tc::mbar_init(&empty[k], 1); }
-        for (int k = 0; k < 2; ++k) { tc::mbar_init(&acc_full[k], 1); tc::mbar_init(&acc_empty[k], 8); }
+        for (int k = 0; k < WNST; ++k) { tc::mbar_init(&full[k], 1); tc::mbar_init(&empty[k], 1); tc::mbar_init(&pfull[k], 1); }
+        for (int k = 0; k < 2; ++k) { tc::mbar_init(&acc_full[k], 1); tc::mbar_init(&acc_empty[k], 16); }
         asm volatile("fence.mbarrier_init.release.cluster;");
     }
-    if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tc::smem_u32(&tmem_base_s)), "n"(512));
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    if (warp == 0) {       // the same warp of both CTAs, the same shared-memory word
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tc::smem_u32(&tmem_base_s)), "n"(512));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;");
     }
     tc::fence_before();
-    __syncthreads();
+    cluster_sync_all();
     tc::fence_after();
     const uint32_t tmem = __shfl_sync(0xffffffffu, tmem_base_s, 0);
     const uint32_t sbase = tc::smem_u32(smem);
-    const int nblk = p.T * p.T, ntiles = p.tab[nblk].x;
-    const int W = p.W, BN = p.BN, NT = p.NTOT / BN, NKC = p.K / WKC;
-    const uint32_t b_stage_bytes = (uint32_t)BN * WKC * 2;
-    const int G = p.G, tile0 = blockIdx.x / G, tstep = gridDim.x / G, nt0 = blockIdx.x % G;
+    const int nblk = p.T * p.T;
+    const int W = p.W, BN = p.BN, HB = BN / 2, NT = p.NTOT / BN, NKC = p.K / WKC;
+    const uint32_t b_half_bytes = (uint32_t)HB * WKC * 2;
+    // pairs of CTAs walk pairs of tiles; G pairs share one pair of tiles, each taking every G-th N tile
+    const int G = p.G, npairs = wide_pair_count(p.tab, nblk);
+    const int pw0 = (blockIdx.x >> 1) / G, pwstep = (gridDim.x >> 1) / G, nt0 = (blockIdx.x >> 1) % G;
 
     if (warp == 0) {
-        // ---------------------------------------------------------------- loader: one A and one B bulk copy per stage
+        // ---------------------------------------------------------------- loader: one A and one B (half) bulk copy per stage
         if (lane == 0) {
             uint32_t step = 0;
-            int k = 0;
-            for (int tile = tile0; tile < ntiles; tile += tstep) {
-                k = wide_block(p.tab, nblk, tile, k);
+            for (int pw = pw0; pw < npairs; pw += pwstep) {
+                int tile;
+                bool valid;
+                const int k = wide_pair(p.tab, nblk, pw, (int)rank, tile, valid);
                 const __half *Bw = p.Bimg + (size_t)k * p.b_net_stride;
-                const uint8_t *At = p.Aimg + (size_t)tile * (p.K / 8) * 2048;
+                const uint8_t *At = p.Aimg + (size_t)(valid ? tile : tile - 1) * (p.K / 8) * 2048;      // (no tile of its own: any tile will do)
                 for (int nt = nt0; nt < NT; nt += G)
                     for (int kc = 0; kc < NKC; ++kc, ++step) {
                         const int st = step % WNST;
                         tc::mbar_wait(&empty[st], ((step / WNST) & 1) ^ 1);
-                        mbar_expect_tx(&full[st], W_A_STAGE + b_stage_bytes);
+                        mbar_expect_tx(&full[st], W_A_STAGE + b_half_bytes);
                         bulk_g2s(sbase + W_OFF_A + st * W_A_STAGE, At + (size_t)kc * W_A_STAGE, W_A_STAGE, &full[st]);
-                        bulk_g2s(sbase + W_OFF_B + st * W_B_STAGE, Bw + ((size_t)nt * NKC + kc) * (WKC * BN), b_stage_bytes, &full[st]);
+                        bulk_g2s(sbase + W_OFF_B + st * W_B_STAGE, Bw + (((size_t)nt * NKC + kc) * 2 + rank) * (WKC * HB), b_half_bytes, &full[st]);
                     }
             }
         }
     } else if (warp == 1) {
-        // ---------------------------------------------------------------- MMA issuer
-        const uint32_t idesc = tc::idesc(128, BN, false, false);
-        uint32_t step = 0, accn = 0;
-        for (int tile = tile0; tile < ntiles; tile += tstep)
-            for (int nt = nt0; nt < NT; nt += G, ++accn) {
-                const int buf = accn & 1;
-                tc::mbar_wait(&acc_empty[buf], ((accn >> 1) & 1) ^ 1);
-                tc::fence_after();
-                for (int kc = 0; kc < NKC; ++kc, ++step) {
-                    const int st = step % WNST;
-                    tc::mbar_wait(&full[st], (step / WNST) & 1);
+        if (rank == 0) {
+            // ------------------------------------------------------------ MMA issuer (leader): M = 256 over both CTAs
+            const uint32_t idesc = tc::idesc(256, BN, false, false);
+            uint32_t step = 0, accn = 0;
+            for (int pw = pw0; pw < npairs; pw += pwstep)
+                for (int nt = nt0; nt < NT; nt += G, ++accn) {
+                    const int buf = accn & 1;
+                    mbar_wait_cluster(&acc_empty[buf], ((accn >> 1) & 1) ^ 1);
                     tc::fence_after();
-                    const uint64_t da = tc::desc(sbase + W_OFF_A + st * W_A_STAGE, 2048, 128);
-                    const uint64_t db = tc::desc(sbase + W_OFF_B + st * W_B_STAGE, BN * 16, 128);
-                    if (tc::elect_one()) {
+                    for (int kc = 0; kc < NKC; ++kc, ++step) {
+                        const int st = step % WNST;
+                        tc::mbar_wait(&full[st], (step / WNST) & 1);
+                        mbar_wait_cluster(&pfull[st], (step / WNST) & 1);
+                        tc::fence_after();
+                        const uint64_t da = tc::desc(sbase + W_OFF_A + st * W_A_STAGE, 2048, 128);
+                        const uint64_t db = tc::desc(sbase + W_OFF_B + st * W_B_STAGE, HB * 16, 128);
+                        if (tc::elect_one()) {
 #pragma unroll
-                        for (int ks = 0; ks < WKC / 16; ++ks)
-                            tc::mma_ss(tmem + buf * 256, tc::desc_at(da, ks * 2 * 2048), tc::desc_at(db, ks * 2 * (BN * 16)), idesc, (kc | ks) != 0);
-                        tc::commit(&empty[st]);
+                            for (int ks = 0; ks < WKC / 16; ++ks)
+                                mma_ss2(tmem + buf * 256, tc::desc_at(da, ks * 2 * 2048), tc::desc_at(db, ks * 2 * (HB * 16)), idesc, (kc | ks) != 0);
+                            commit_pair(&empty[st]);
+                        }
+                        __syncwarp();
                     }
+                    if (tc::elect_one()) commit_pair(&acc_full[buf]);
                     __syncwarp();
                 }
-                if (tc::elect_one()) tc::commit(&acc_full[buf]);
-                __syncwarp();
-            }
+        } else {
+            // ------------------------------------------------------------ relay (peer): "my stage has landed" to the leader
+            uint32_t step = 0;
+            for (int pw = pw0; pw < npairs; pw += pwstep)
+                for (int nt = nt0; nt < NT; nt += G)
+                    for (int kc = 0; kc < NKC; ++kc, ++step) {
+                        const int st = step % WNST;
+                        tc::mbar_wait(&full[st], (step / WNST) & 1);
+                        if (lane == 0) mbar_arrive_leader(&pfull[st]);
+                        __syncwarp();
+                    }
+        }
     } else {
         // ---------------------------------------------------------------- epilogue: thread = (row, every other 16 columns)
         const int q4 = warp & 3, r = q4 * 32 + lane, hc = ((warp - 2) >> 2) & 1;
         const uint32_t tm_lane = tmem + ((uint32_t)(q4 * 32) << 16);
         float *red = reinterpret_cast<float *>(smem + W_OFF_RED);
         uint32_t accn = 0, it = 0;
-        int k = 0;
-        for (int tile = tile0; tile < ntiles; tile += tstep, ++it) {
-            k = wide_block(p.tab, nblk, tile, k);
+        for (int pw = pw0; pw < npairs; pw += pwstep, ++it) {
+            int tile;
+            bool valid;
+            const int k = wide_pair(p.tab, nblk, pw, (int)rank, tile, valid);
+            if (!valid) {          // no tile of its own: keep the accumulator hand-shake of the pair going, store nothing
+                for (int nt = nt0; nt < NT; nt += G, ++accn) {
+                    const int buf = accn & 1;
+                    tc::mbar_wait(&acc_full[buf], (accn >> 1) & 1);
+                    tc::fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive_leader(&acc_empty[buf]);
+                }
+                continue;
+            }
             const float *vec = p.vec + (size_t)k * 8 * W;
             // this row's 16-byte slot of chunk 0 of each image of the tile
             uint8_t *t1r = p.T1 + (size_t)tile * (W / 8) * 2048 + r * 16;
@@ -299,7 +372,7 @@ __global__ void __launch_bounds__(W_THREADS, 1) k_wide_gemm(const __grid_constan
                 }
                 tc::fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&acc_empty[buf]);
+                if (lane == 0) mbar_arrive_leader(&acc_empty[buf]);
             }
             if (MODE == 3) {
                 float *rd = red + (it & 1) * 256;
@@ -323,8 +396,9 @@ __global__ void __launch_bounds__(W_THREADS, 1) k_wide_gemm(const __grid_constan
         }
     }
     tc::fence_before();
-    __syncthreads();
-    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(512));
+    cluster_sync_all();
+    tc::fence_after();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(512));
 }
 
 // S5: A_i[c][m] = (1 / Nm) sum_rows w R^[row][c] G[row][m],  G = (y2, y2) + t3.
@@ -622,16 +696,16 @@ static size_t wide_img_off(int W, int g) {
 }
 size_t wide_net_img_elems(int W) { return wide_img_off(W, 4); }
 
+// B image of one product: per N tile (BN columns), per K = 64 stage and per half of the tile's columns (one half per CTA of a
+// pair) the block [8 chunks][BN / 2][8 fp16]: one contiguous bulk copy per stage and CTA
 static void wide_image(const double *Wt, int ldw, bool transpose, int K, int Nn, __half *out) {
-    const int BN = wide_bn(Nn), nk8 = K / 8;
-    for (int nt = 0; nt < Nn / BN; ++nt)
-        for (int k8 = 0; k8 < nk8; ++k8)
-            for (int n = 0; n < BN; ++n)
-                for (int kk = 0; kk < 8; ++kk) {
-                    const int k = k8 * 8 + kk, nn = nt * BN + n;
-                    const double v = transpose ? Wt[(size_t)nn * ldw + k] : Wt[(size_t)k * ldw + nn];
-                    out[(((size_t)nt * nk8 + k8) * BN + n) * 8 + kk] = __float2half_rn((float)v);
-                }
+    const int BN = wide_bn(Nn), HB = BN / 2, nkc = K / WKC;
+    for (int nn = 0; nn < Nn; ++nn)
+        for (int k = 0; k < K; ++k) {
+            const double v = transpose ? Wt[(size_t)nn * ldw + k] : Wt[(size_t)k * ldw + nn];
+            const int nt = nn / BN, n = nn % BN, kc = k / WKC, k8 = (k % WKC) / 8, kk = k % 8;
+            out[((((size_t)nt * nkc + kc) * 2 + n / HB) * 8 + k8) * ((size_t)HB * 8) + (size_t)(n % HB) * 8 + kk] = __float2half_rn((float)v);
+        }
 }
 
 // net: w1[W], b1[W], W2[W][2 W], b2[2 W], W3[2 W][4 W], b3[4 W] (dp.h weight order); vec: w1, b1, b2, b3
@@ -679,7 +753,7 @@ static cudaError_t wide_gemm(const dp_model *m, WideArgs p, int K, int Nn, const
     const int nt = Nn / p.BN;
     // (worth it when the A tiles of all CTAs, grid x 128 x K fp16, overflow the L2: K = 2048, the layer-3 backward at W = 512)
     p.G = (MODE != 3 && K >= 2048 && nt >= 4) ? 4 : 1;
-    k_wide_gemm<MODE><<<m->num_sms - m->num_sms % p.G, W_THREADS, W_TOTAL, st>>>(p);
+    k_wide_gemm<MODE><<<m->num_sms - m->num_sms % (2 * p.G), W_THREADS, W_TOTAL, st>>>(p);      // CTA pairs
     return cudaGetLastError();
 }
 
