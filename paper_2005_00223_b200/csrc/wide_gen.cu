@@ -331,8 +331,8 @@ __global__ void __launch_bounds__(256, 1) k_wg_gemm_f64(const __grid_constant__ 
 // matrix and its transpose).  Persistent, one CTA PAIR per two SMs (cluster of 2, tcgen05 cta_group::2): the pair computes
 // two 128-row tiles of one net against one N tile; each CTA stages its own rows of A and HALF of the B tile, and the MMA of the
 // leader (M = 256) reads both halves, so a CTA moves and reads half the weight bytes of a single-CTA tile.  Per CTA:
-//   warp 13    loader (one thread): per K = 16 stage ONE TMA tensor copy of A (the row-major activations seen as a
-//              (4, rows, K / 4) tensor, box {4, 128, 4}: it lands as the un-swizzled K-major operand image, per 16 bytes of K a
+//   warp 13    loader (one thread): per K = 32 stage ONE TMA tensor copy of A (the row-major activations seen as a
+//              (4, rows, K / 4) tensor, box {4, 128, 8}: it lands as the un-swizzled K-major operand image, per 16 bytes of K a
 //              column [128 rows][16 B]) and ONE bulk copy of this CTA's half of the weights' operand images (TF32 values and TF32
 //              remainders, laid out by dp_create), both counted by the stage's "landed" barrier;
 //   warps 0-7  splitters: a_small = a - a_big (exact) into a second image, a_big = a with the 13 low mantissa bits cleared = what
@@ -342,11 +342,11 @@ __global__ void __launch_bounds__(256, 1) k_wg_gemm_f64(const __grid_constant__ 
 //              accumulators (128 TMEM lanes in each CTA); tcgen05.commit multicasts "stage free" and "accumulator ready" to both CTAs;
 //   warps 8-11 epilogue: thread = row = TMEM lane, 32 columns per step, the layer's bias / tanh / skip / tanh' work on the
 //              row-major fp32 activations; "accumulator drained" goes to the leader.
-constexpr int TQ_KC = 16;                          // K per stage: 4 pieces of 16 bytes
-constexpr int TQ_NST = 6;
+constexpr int TQ_KC = 32;                          // K per stage: 8 pieces of 16 bytes
+constexpr int TQ_NST = 3;
 constexpr int TQ_A_PIECE = 128 * 16;               // distance between the piece columns of an image (the descriptors' LBO)
-constexpr int TQ_A_IMG = 4 * TQ_A_PIECE;           // 8 KB: [4 pieces][128 rows][16 B], written by one TMA tensor copy
-constexpr int TQ_B_IMG = 128 * TQ_KC * 4;          // 8 KB: this CTA's half (<= 128 rows of B^T) of one weight image
+constexpr int TQ_A_IMG = (TQ_KC / 4) * TQ_A_PIECE;   // 16 KB: [8 pieces][128 rows][16 B], written by one TMA tensor copy
+constexpr int TQ_B_IMG = 128 * TQ_KC * 4;          // 16 KB: this CTA's half (<= 128 rows of B^T) of one weight image
 constexpr int TQ_STAGE = 2 * TQ_A_IMG + 2 * TQ_B_IMG;      // a_big | a_small | b_big | b_small
 constexpr int TQ_OFF_BAR = TQ_NST * TQ_STAGE;
 constexpr int TQ_TOTAL = TQ_OFF_BAR + 256;
@@ -390,7 +390,7 @@ __device__ __forceinline__ void mbar_wait_cluster(uint64_t *bar, uint32_t parity
 __device__ __forceinline__ void cluster_sync_all() {
     asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
-// box {4 elements, 128 rows, 4 pieces} of the activation tensor viewed as (4, rows, K / 4) -> the [4][128][16 B] operand image
+// box {4 elements, 128 rows, 8 pieces} of the activation tensor viewed as (4, rows, K / 4) -> the [8][128][16 B] operand image
 __device__ __forceinline__ void tma_load_3d(uint32_t sdst, const CUtensorMap *tm, int c0, int c1, int c2, uint64_t *bar) {
     asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
                  ::"r"(sdst), "l"((uint64_t)tm), "r"(c0), "r"(c1), "r"(c2), "r"(tc::smem_u32(bar)) : "memory");
@@ -466,14 +466,14 @@ k_wg_gemm_tf32(const __grid_constant__ GenArgs<float> p, const __grid_constant__
                     const int st = step % TQ_NST;
                     tc::mbar_wait(&empty[st], ((step / TQ_NST) & 1) ^ 1);
                     mbar_expect_tx_cta(&landed[st], TQ_A_IMG + b_half_bytes);
-                    tma_load_3d(sbase + st * TQ_STAGE, &tmA, 0, (int)row0, kc * 4, &landed[st]);
+                    tma_load_3d(sbase + st * TQ_STAGE, &tmA, 0, (int)row0, kc * (TQ_KC / 4), &landed[st]);
                     bulk_g2s_cta(sbase + st * TQ_STAGE + 2 * TQ_A_IMG, Bg + (long)kc * 2 * (2 * HB * TQ_KC), b_half_bytes, &landed[st]);
                 }
             }
         }
     } else if (warp < 8) {
         // ------------------------------------------------------------------------------------------------ splitters
-        // every thread splits two 16-byte pieces of the landed A image: a_small into the second image
+        // every thread splits four 16-byte pieces of the landed A image: a_small into the second image
         const uint32_t a_off = ((tid >> 3) & 3) * TQ_A_PIECE + (8 * (tid >> 5) + (tid & 7)) * 16;      // + 64 rows for the second piece
         const long nstage = nwork > pair0 ? ((nwork - pair0 + npair - 1) / npair) * NKC : 0;
         for (long it = 0; it < nstage; ++it) {
@@ -481,11 +481,11 @@ k_wg_gemm_tf32(const __grid_constant__ GenArgs<float> p, const __grid_constant__
             tc::mbar_wait(&landed[st], (uint32_t)((it / TQ_NST) & 1));
             unsigned char *stage = tq_smem + st * TQ_STAGE;
 #pragma unroll
-            for (int q = 0; q < 2; ++q) {
+            for (int q = 0; q < TQ_KC / 8; ++q) {          // q & 1: + 64 rows; q >> 1: + 4 piece columns
                 // (the landed image itself is a_big: the tensor core reads the top 19 bits of each fp32 word and ignores the 13
                 // low mantissa bits; storing the masked words back changes no result bit and was measured, so it is not done)
-                const uint4 *pb = reinterpret_cast<const uint4 *>(stage + a_off + q * (64 * 16));
-                uint4 *ps = reinterpret_cast<uint4 *>(stage + TQ_A_IMG + a_off + q * (64 * 16));
+                const uint4 *pb = reinterpret_cast<const uint4 *>(stage + a_off + (q & 1) * (64 * 16) + (q >> 1) * 4 * TQ_A_PIECE);
+                uint4 *ps = reinterpret_cast<uint4 *>(stage + TQ_A_IMG + a_off + (q & 1) * (64 * 16) + (q >> 1) * 4 * TQ_A_PIECE);
                 const uint4 x = *pb;
                 uint4 b, sm;
                 b.x = x.x & 0xffffe000u; b.y = x.y & 0xffffe000u; b.z = x.z & 0xffffe000u; b.w = x.w & 0xffffe000u;
@@ -827,9 +827,9 @@ static void build_net(int W, const double *net, R *out) {
             out[wg_off_W3T(W) + (size_t)m * 2 * W + f] = (R)W3[(size_t)f * 4 * W + m];
         }
 }
-// MIX-32: the operand images of B^T [NTOT][K] of one product: per N tile (BN = min(256, NTOT) rows), per K = 16 stage and per half
+// MIX-32: the operand images of B^T [NTOT][K] of one product: per N tile (BN = min(256, NTOT) rows), per K = 32 stage and per half
 // of the tile's rows (one half per CTA of a pair) the TF32 values [4 pieces][BN / 2][4] followed by the TF32 remainders in the
-// same order (one contiguous bulk copy per stage and CTA)
+// same order, pieces of 16 bytes of K outermost (one contiguous bulk copy per stage and CTA)
 static void tf32_image(const std::vector<float> &Bt, int NTOT, int K, float *out) {
     const int BN = NTOT < 256 ? NTOT : 256, HB = BN / 2, NKC = K / TQ_KC;
     for (int n = 0; n < NTOT; ++n)
@@ -898,7 +898,7 @@ static cudaError_t gen_gemm_tf32(const dp_model *m, GenArgs<float> p, int K, int
     CUtensorMap tm;
     const cuuint64_t gdim[3] = {4, (cuuint64_t)p.N * (cuuint64_t)m->Nm, (cuuint64_t)(K / 4)};
     const cuuint64_t gstr[2] = {(cuuint64_t)K * 4, 16};
-    const cuuint32_t box[3] = {4, 128, 4}, estr[3] = {1, 1, 1};
+    const cuuint32_t box[3] = {4, 128, TQ_KC / 4}, estr[3] = {1, 1, 1};
     if (enc(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)A, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
         return cudaErrorInvalidValue;
