@@ -214,3 +214,34 @@ def test_wide_empty_type_blocks(prec):
     err = np.abs(g["forces"] - o["forces"]).max() / rms
     assert err <= {"fp64": 1e-10, "mix32": 1e-4, "mix16": 5e-3}[prec], err
     assert abs(g["energy"][0] - o["energy"]) / len(types) <= {"fp64": 1e-12, "mix32": 2e-5, "mix16": 1e-3}[prec]
+
+
+@pytest.mark.parametrize("prec,tol,tolEi", [("fp64", 1e-10, 1e-11), ("mix32", 1e-4, 2e-5), ("mix16", 5e-3, 1e-3)])
+def test_wide_bench_size_sampled(prec, tol, tolEi):
+    """The bench workload of the FP64 / MIX-32 sweeps (4,000 Cu atoms, capacity 512, shuffled order: 5,500 tiles, every CTA pair
+    walks dozens of them) at W = 128 against the sampled oracle (tests/sampling.py: complete forces of 4 sample atoms, E_i and
+    list rows of the ~680 centres around them), at the north_star tolerance of each precision, and the properties that hold at
+    any size"""
+    import os
+    import sys
+    import torch
+    sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+    from sampling import sampled_oracle
+    from paper_2005_00223_b200 import binding
+    s = synth.wide_copper(10, 128, 790, sigma=0.3, shuffle=True, precision=prec)
+    so = sampled_oracle(s, nsample=4, seed=5)
+    m = binding.DPModel(s.model, prec)
+    out = m.compute(torch.from_numpy(s.coords).cuda(), torch.from_numpy(s.types).cuda(), s.box)
+    rc, _ = m.status()
+    assert rc == 0
+    nl = m.get_nlist()[torch.from_numpy(so["centers"]).cuda()].cpu().numpy()
+    F = out["forces"].cpu().numpy()
+    ea = out["atom_energy"].cpu().numpy()
+    E = float(out["energy"].item())
+    m.close()
+    assert np.array_equal(nl, so["nlist"])
+    assert np.abs(ea[so["centers"]] - so["atom_energy"]).max() <= tolEi
+    err = np.abs(F[so["sample"]] - so["forces"]).max()
+    assert err <= tol * so["rms_f"], (err / so["rms_f"], tol)
+    assert abs(E - ea.sum()) <= 1e-9 * abs(E)
+    assert np.abs(F.sum(0)).max() <= 1e-6 * np.abs(F).sum(0).max()
