@@ -325,7 +325,7 @@ def cluster(n: int, seed: int, ntypes: int = 1, L: float = 40.0, spread: float =
 
 
 def small_fcc(ncell: int, seed: int, sigma: float = 0.05, a: float = 3.634, rc: float = 5.0,
-              rc_smth: float = 1.5, sel=(64,), ntypes: int = 1) -> System:
+              rc_smth: float = 1.5, sel=(64,), ntypes: int = 1, embed_widths=EMBED_WIDTHS) -> System:
     """Jittered FCC with a reduced cutoff (periodic, box may be < 2 rc: oracle-only)."""
     rng = np.random.default_rng(seed)
     x = fcc_positions(ncell, a)
@@ -336,7 +336,7 @@ def small_fcc(ncell: int, seed: int, sigma: float = 0.05, a: float = 3.634, rc: 
     sel = tuple(sel) if len(sel) == ntypes else tuple([sel[0]] * ntypes)
     avg = [[0.12, 0, 0, 0]] * ntypes
     std = [[0.15, 0.1, 0.1, 0.1]] * ntypes
-    model = make_model(ntypes, rc, rc_smth, sel, seed + 1000, avg, std)
+    model = make_model(ntypes, rc, rc_smth, sel, seed + 1000, avg, std, embed_widths=embed_widths)
     box = np.diag([L, L, L]).reshape(9).astype(np.float64)
     return System(f"fcc{n}", np.ascontiguousarray(x), types, box, model, "fp64")
 

@@ -245,3 +245,26 @@ def test_wide_bench_size_sampled(prec, tol, tolEi):
     assert err <= tol * so["rms_f"], (err / so["rms_f"], tol)
     assert abs(E - ea.sum()) <= 1e-9 * abs(E)
     assert np.abs(F.sum(0)).max() <= 1e-6 * np.abs(F).sum(0).max()
+
+
+@pytest.mark.parametrize("prec,tol,tolE", [("fp64", 1e-10, 1e-12), ("mix32", 1e-4, 2e-5), ("mix16", 5e-3, 1e-3)])
+def test_wide_three_types(prec, tol, tolE):
+    """Three atom types: nine (centre, neighbour) nets and row blocks, most of them a few tiles long, with wide
+    nets (W = 64) in the three precisions at their north_star tolerances"""
+    import torch
+    from paper_2005_00223_b200 import binding
+    s = synth.small_fcc(4, 53, sigma=0.08, rc=5.0, rc_smth=1.5, sel=(24,), ntypes=3, embed_widths=(64, 128, 256))
+    o = oracle.evaluate(s.coords, s.types, s.box, s.model)
+    m = binding.DPModel(s.model, prec)
+    out = m.compute(torch.from_numpy(s.coords).cuda(), torch.from_numpy(s.types).cuda(), s.box)
+    rc, ntr = m.status()
+    assert rc == 0 and ntr == o["n_truncated"]
+    nl = m.get_nlist().cpu().numpy()
+    g = {k: v.cpu().numpy() for k, v in out.items()}
+    m.close()
+    assert np.array_equal(nl, o["nlist"])
+    rms = np.sqrt((o["forces"] ** 2).mean())
+    err = np.abs(g["forces"] - o["forces"]).max()
+    assert err <= tol * rms, err / rms
+    assert abs(g["energy"][0] - o["energy"]) / s.natoms <= tolE * (abs(o["energy"]) / s.natoms if prec == "fp64" else 1.0)
+    assert np.abs(g["virial"] - o["virial"]).max() / s.natoms <= (1e-12 if prec == "fp64" else tolE)
