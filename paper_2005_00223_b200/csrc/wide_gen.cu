@@ -8,7 +8,7 @@
 // rows of the mixed modes (the real rows of a (centre type, neighbour type) block, contiguous, plus one
 // representative per atom and block for its padded slots, weighted by their number) and the row tiles are those of the
 // tile table of wide.cu, so a tile never straddles two nets.
-//   FP64   ("double"): k_wg_gemm_f64, the FP64 tensor pipe (DMMA m8n8k4), 128 x 128 x 32 tiles staged with cp.async;
+//   FP64   ("double"): k_wg_gemm_f64, the FP64 tensor pipe (DMMA m8n8k4), 64 x 128 x 32 tiles staged with cp.async, two CTAs per SM;
 //   MIX-32 (nets in single precision): k_wg_gemm_tf32, tcgen05.mma kind::tf32 with TMEM accumulators; every operand
 //          is split into a TF32 value and its TF32 remainder and each K step takes three products ("3xTF32": the product keeps
 //          21+ mantissa bits; the accumulators are fp32); the activations arrive by TMA tensor copies, the weights' operand
@@ -29,11 +29,12 @@
 namespace {
 
 constexpr int GR = 128;                     // rows per tile (= the tile table's, wide.cu)
-constexpr int GBN = 128, GBK = 32;          // N tile, K step
-constexpr int GA_STRIDE = GBK + 4;          // A tile [128][36]: fragment loads hit distinct banks (per half warp)
+constexpr int GBM = 64, GBN = 128, GBK = 32; // FP64 kernel: rows (half a tile of the table), columns, K step per CTA
+constexpr int GTHREADS = 128;               // four warps as 2 (rows) x 2 (columns)
+constexpr int GA_STRIDE = GBK + 4;          // A tile [64][36]: fragment loads hit distinct banks (per half warp)
 struct GemmCfg {                             // the FP64 kernel's tiles
     static constexpr int BS = GBN + 4;                                  // B tile [32][BS]
-    static constexpr int A_TILE = GR * GA_STRIDE, B_TILE = GBK * BS;
+    static constexpr int A_TILE = GBM * GA_STRIDE, B_TILE = GBK * BS;
     static constexpr int SMEM = 2 * (A_TILE + B_TILE) * 8;
     static constexpr int EPV = 2;                                       // doubles per 16-byte cp.async
 };
@@ -240,23 +241,26 @@ __device__ __forceinline__ void wg_epi_store(const GenArgs<double> &p, long Rg, 
     }
 }
 
-// FP64: one 128 x 128 output tile per CTA, eight warps as 4 (rows) x 2 (columns): warp tile 32 x 64 = 4 x 8 DMMA m8n8k4 fragments.
-// A and B stages of K = 32 arrive by cp.async (two buffers); rows past the end of the tile's block and columns past NTOT are
-// zero-filled and never stored.
+// FP64: one 64 x 128 output tile per CTA (half a tile of the table), four warps as 2 (rows) x 2 (columns): warp tile 32 x 64 =
+// 4 x 8 DMMA m8n8k4 fragments; TWO CTAs per SM (241 registers x 128 threads, 104 KB of shared memory each), so that one CTA's
+// barriers, prologue and epilogue run under the other's DMMAs.  A and B stages of K = 32 arrive by cp.async (two buffers); rows
+// past the end of the tile's block and columns past NTOT are zero-filled and never stored.
 template <int MODE>
-__global__ void __launch_bounds__(256, 1) k_wg_gemm_f64(const __grid_constant__ GenArgs<double> p) {
+__global__ void __launch_bounds__(GTHREADS, 2) k_wg_gemm_f64(const __grid_constant__ GenArgs<double> p) {
     using C = GemmCfg;
     extern __shared__ __align__(16) unsigned char wg_smem[];
     double *sm = reinterpret_cast<double *>(wg_smem);
     const int nblk = p.T * p.T;
     const int ntn = (p.NTOT + GBN - 1) / GBN;
-    const int tile = blockIdx.x / ntn, n0 = (blockIdx.x % ntn) * GBN;
+    constexpr int SUB = GR / GBM;                 // CTAs per tile of the table
+    const int tile = blockIdx.x / (ntn * SUB), sub = (blockIdx.x / ntn) % SUB, n0 = (blockIdx.x % ntn) * GBN;
     if (tile >= p.tab[nblk].x) return;
     const int k = wg_block(p.tab, nblk, tile);
     const int4 e = p.tab[k];
     const long rbase = p.N * (long)p.tt.off[k % p.T];
-    const int row0 = e.y + (tile - e.x) * GR;
-    const int nrows = min(GR, e.z - row0);
+    const int row0 = e.y + (tile - e.x) * GR + sub * GBM;
+    const int nrows = min(GBM, e.z - row0);
+    if (nrows <= 0) return;
     const double *net = p.nets + k * p.net_stride;
     const double *Ag = p.A + (rbase + row0) * (long)p.K;
     const double *Bg = net + p.b_off + n0;
@@ -267,14 +271,14 @@ __global__ void __launch_bounds__(256, 1) k_wg_gemm_f64(const __grid_constant__ 
         double *As = sm + buf * (C::A_TILE + C::B_TILE), *Bs = As + C::A_TILE;
         constexpr int AV = GBK / C::EPV, BV = GBN / C::EPV;       // 16-byte vectors per A row / per B row
 #pragma unroll
-        for (int q = 0; q < GR * AV / 256; ++q) {
-            const int idx = tid + q * 256, r = idx / AV, kv = (idx % AV) * C::EPV;
+        for (int q = 0; q < GBM * AV / GTHREADS; ++q) {
+            const int idx = tid + q * GTHREADS, r = idx / AV, kv = (idx % AV) * C::EPV;
             const bool ok = r < nrows;
             cp_async16(As + r * GA_STRIDE + kv, Ag + (ok ? (long)r * p.K + k0 + kv : 0), ok);
         }
 #pragma unroll
-        for (int q = 0; q < GBK * BV / 256; ++q) {
-            const int idx = tid + q * 256, kk = idx / BV, nv = (idx % BV) * C::EPV;
+        for (int q = 0; q < GBK * BV / GTHREADS; ++q) {
+            const int idx = tid + q * GTHREADS, kk = idx / BV, nv = (idx % BV) * C::EPV;
             const bool ok = n0 + nv < p.NTOT;
             cp_async16(Bs + kk * C::BS + nv, Bg + (ok ? (long)(k0 + kk) * p.NTOT + nv : 0), ok);
         }
@@ -914,8 +918,8 @@ static cudaError_t gen_gemm(const dp_model *m, long N, GenArgs<R> p, int K, int 
     } else {
         DP_SMEM_OPTIN((k_wg_gemm_f64<MODE>), GemmCfg::SMEM);
         p.K = K; p.NTOT = Nn; p.A = A; p.b_off = b_off;
-        const long tiles = wide_tiles_cap(m, N), ntn = (Nn + GBN - 1) / GBN;
-        k_wg_gemm_f64<MODE><<<(unsigned)(tiles * ntn), 256, GemmCfg::SMEM, st>>>(p);
+        const long tiles = wide_tiles_cap(m, N) * (GR / GBM), ntn = (Nn + GBN - 1) / GBN;
+        k_wg_gemm_f64<MODE><<<(unsigned)(tiles * ntn), GTHREADS, GemmCfg::SMEM, st>>>(p);
         return cudaGetLastError();
     }
 }
