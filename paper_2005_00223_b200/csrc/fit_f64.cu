@@ -229,40 +229,42 @@ __device__ __forceinline__ int feature3(int nt3, int r, int j3) {
 }
 
 // gA[c][m] = sum_a gD[m][a] A[c][a] + [m < 16] sum_m' gD[m'][m] A[c][m']   (N8), written as the MMA fragments the
-// embedding backward consumes (layout in embed_f64.cu), pre-scaled by 1/Nm.  One warp per atom.
+// embedding backward consumes (layout in embed_f64.cu), pre-scaled by 1/Nm.  One CTA of four warps works on one atom at a time
+// (20 KB of shared memory per CTA: eleven CTAs per SM; one warp per atom with its own 20 KB left eight warps per SM).
 template <int W>
 __global__ void __launch_bounds__(128) k_gA(long N, double inv_nm, const double *__restrict__ Amat,
                                             const double *__restrict__ gD, double *__restrict__ gAf) {
     constexpr int M2E = EmbW<W>::M2E, NT3 = EmbW<W>::NT3;
     extern __shared__ double smg[];
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const long i = blockIdx.x * 4L + wid;
-    if (i >= N) return;
-    double *sA = smg + wid * (4 * M2E + M2E * 17 + 4 * M2E);
-    double *sG = sA + 4 * M2E;
-    double *sO = sG + M2E * 17;      // rows of gD padded to 17: lanes walk consecutive rows m (stride 16 was a 16-way bank conflict)
-    for (int k = lane; k < 4 * M2E; k += 32) sA[k] = Amat[i * 4 * M2E + k];
-    for (int k = lane; k < M2E * 16; k += 32) sG[(k >> 4) * 17 + (k & 15)] = gD[i * (M2E * 16) + k];
-    __syncwarp();
-    for (int idx = lane; idx < 4 * M2E; idx += 32) {
-        const int c = idx / M2E, m = idx % M2E;
-        double acc = 0.0;
+    double *sA = smg;                       // [4][M2E]
+    double *sG = sA + 4 * M2E;              // [M2E][17]: rows of gD padded (lanes walk consecutive rows m: stride 16 was a 16-way bank conflict)
+    double *sO = sG + M2E * 17;             // [4][M2E]
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    for (long i = blockIdx.x; i < N; i += gridDim.x) {
+        __syncthreads();
+        for (int k = tid; k < 4 * M2E; k += 128) sA[k] = Amat[i * 4 * M2E + k];
+        for (int k = tid; k < M2E * 16; k += 128) sG[(k >> 4) * 17 + (k & 15)] = gD[i * (M2E * 16) + k];
+        __syncthreads();
+        for (int idx = tid; idx < 4 * M2E; idx += 128) {
+            const int c = idx / M2E, m = idx % M2E;
+            double acc = 0.0;
 #pragma unroll
-        for (int ax = 0; ax < 16; ++ax) acc += sG[m * 17 + ax] * sA[c * M2E + ax];
-        if (m < 16)
-            for (int mp = 0; mp < M2E; ++mp) acc += sG[mp * 17 + m] * sA[c * M2E + mp];
-        sO[idx] = acc * inv_nm;
-    }
-    __syncwarp();
-    double *out = gAf + i * (3 * NT3 * 32);
-    const int q4 = lane >> 2, r = lane & 3;
-    for (int nt3 = 0; nt3 < NT3; ++nt3) {
-        const int f = feature3<W>(nt3, q4 >> 1, q4 & 1);
-        out[nt3 * 32 + lane] = f >= 0 ? sO[r * M2E + f] : 0.0;
-    }
-    for (int kc = 0; kc < 2 * NT3; ++kc) {
-        const int f = feature3<W>(kc >> 1, r, kc & 1);
-        out[(NT3 + kc) * 32 + lane] = (f >= 0 && q4 < 4) ? sO[q4 * M2E + f] : 0.0;
+            for (int ax = 0; ax < 16; ++ax) acc += sG[m * 17 + ax] * sA[c * M2E + ax];
+            if (m < 16)
+                for (int mp = 0; mp < M2E; ++mp) acc += sG[mp * 17 + m] * sA[c * M2E + mp];
+            sO[idx] = acc * inv_nm;
+        }
+        __syncthreads();
+        double *out = gAf + i * (3 * NT3 * 32);
+        const int q4 = lane >> 2, r = lane & 3;
+        for (int nt3 = wid; nt3 < NT3; nt3 += 4) {
+            const int f = feature3<W>(nt3, q4 >> 1, q4 & 1);
+            out[nt3 * 32 + lane] = f >= 0 ? sO[r * M2E + f] : 0.0;
+        }
+        for (int kc = wid; kc < 2 * NT3; kc += 4) {
+            const int f = feature3<W>(kc >> 1, r, kc & 1);
+            out[(NT3 + kc) * 32 + lane] = (f >= 0 && q4 < 4) ? sO[q4 * M2E + f] : 0.0;
+        }
     }
 }
 
@@ -388,9 +390,9 @@ static cudaError_t launch_fit_w(const dp_model *m, long N, const Grid3 &g, char 
     if constexpr (W == 0) {
         k_gA_wide<<<(unsigned)N, 256, 0, st>>>(M2E, Amat, D, (double *)(ws + L.gAf));
     } else {
-        const int smem = 4 * (4 * M2E + M2E * 17 + 4 * M2E) * 8;
-        DP_SMEM_OPTIN(k_gA<W>, smem);
-        k_gA<W><<<(unsigned)((N + 3) / 4), 128, smem, st>>>(N, 1.0 / (double)m->Nm, Amat, D, (double *)(ws + L.gAf));
+        const int smem = (4 * M2E + M2E * 17 + 4 * M2E) * 8;
+        const long gmax = (long)m->num_sms * 11;
+        k_gA<W><<<(unsigned)(N < gmax ? N : gmax), 128, smem, st>>>(N, 1.0 / (double)m->Nm, Amat, D, (double *)(ws + L.gAf));
     }
     return cudaGetLastError();
 }
