@@ -8,7 +8,7 @@
 // rows of the mixed modes (the real rows of a (centre type, neighbour type) block, contiguous, plus one
 // representative per atom and block for its padded slots, weighted by their number) and the row tiles are those of the
 // tile table of wide.cu, so a tile never straddles two nets.
-//   FP64   ("double"): k_wg_gemm_f64, the FP64 tensor pipe (DMMA m8n8k4), 64 x 128 x 32 tiles staged with cp.async, two CTAs per SM;
+//   FP64   ("double"): k_wg_gemm_f64, the FP64 tensor pipe (DMMA m8n8k4), 64 x 64 x 32 tiles staged with cp.async, three CTAs per SM;
 //   MIX-32 (nets in single precision): k_wg_gemm_tf32, tcgen05.mma kind::tf32 with TMEM accumulators; every operand
 //          is split into a TF32 value and its TF32 remainder and each K step takes three products ("3xTF32": the product keeps
 //          21+ mantissa bits; the accumulators are fp32); the activations arrive by TMA tensor copies, the weights' operand
@@ -29,9 +29,10 @@
 namespace {
 
 constexpr int GR = 128;                     // rows per tile (= the tile table's, wide.cu)
-constexpr int GBM = 64, GBN = 128, GBK = 32; // FP64 kernel: rows (half a tile of the table), columns, K step per CTA
+constexpr int GBM = 64, GBN = 64, GBK = 32;  // FP64 kernel: rows (half a tile of the table), columns, K step per CTA
+constexpr int GNI = GBN / 16, GCTAS = 3;     // 8-column fragments per warp; CTAs per SM
 constexpr int GTHREADS = 128;               // four warps as 2 (rows) x 2 (columns)
-constexpr int GA_STRIDE = GBK + 4;          // A tile [64][36]: fragment loads hit distinct banks (per half warp)
+constexpr int GA_STRIDE = GBK + 4;          // A tile [64][36], B tile [32][68]: fragment loads hit distinct banks (per half warp)
 struct GemmCfg {                             // the FP64 kernel's tiles
     static constexpr int BS = GBN + 4;                                  // B tile [32][BS]
     static constexpr int A_TILE = GBM * GA_STRIDE, B_TILE = GBK * BS;
@@ -241,12 +242,12 @@ __device__ __forceinline__ void wg_epi_store(const GenArgs<double> &p, long Rg, 
     }
 }
 
-// FP64: one 64 x 128 output tile per CTA (half a tile of the table), four warps as 2 (rows) x 2 (columns): warp tile 32 x 64 =
-// 4 x 8 DMMA m8n8k4 fragments; TWO CTAs per SM (241 registers x 128 threads, 104 KB of shared memory each), so that one CTA's
-// barriers, prologue and epilogue run under the other's DMMAs.  A and B stages of K = 32 arrive by cp.async (two buffers); rows
+// FP64: one 64 x 64 output tile per CTA (half a tile of the table), four warps as 2 (rows) x 2 (columns): warp tile 32 x 32 =
+// 4 x 4 DMMA m8n8k4 fragments; THREE CTAs per SM (168 registers x 128 threads, 72 KB of shared memory each), so that one CTA's
+// barriers, prologue and epilogue run under the others' DMMAs.  A and B stages of K = 32 arrive by cp.async (two buffers); rows
 // past the end of the tile's block and columns past NTOT are zero-filled and never stored.
 template <int MODE>
-__global__ void __launch_bounds__(GTHREADS, 2) k_wg_gemm_f64(const __grid_constant__ GenArgs<double> p) {
+__global__ void __launch_bounds__(GTHREADS, GCTAS) k_wg_gemm_f64(const __grid_constant__ GenArgs<double> p) {
     using C = GemmCfg;
     extern __shared__ __align__(16) unsigned char wg_smem[];
     double *sm = reinterpret_cast<double *>(wg_smem);
@@ -285,9 +286,9 @@ __global__ void __launch_bounds__(GTHREADS, 2) k_wg_gemm_f64(const __grid_consta
         cp_async_commit();
     };
 
-    double acc[64];                              // 4 x 8 fragments of 2
+    double acc[8 * GNI];                         // 4 x GNI fragments of 2
 #pragma unroll
-    for (int q = 0; q < 64; ++q) acc[q] = 0.0;
+    for (int q = 0; q < 8 * GNI; ++q) acc[q] = 0.0;
 
     const int nk = p.K / GBK;
     load_stage(0, 0);
@@ -297,15 +298,15 @@ __global__ void __launch_bounds__(GTHREADS, 2) k_wg_gemm_f64(const __grid_consta
         const double *As = sm + (ks & 1) * (C::A_TILE + C::B_TILE), *Bs = As + C::A_TILE;
 #pragma unroll
         for (int kk = 0; kk < GBK / 4; ++kk) {
-            double a[4], b[8];
+            double a[4], b[GNI];
 #pragma unroll
             for (int mi = 0; mi < 4; ++mi) a[mi] = As[(32 * wm + 8 * mi + g) * GA_STRIDE + 4 * kk + t];
 #pragma unroll
-            for (int ni = 0; ni < 8; ++ni) b[ni] = Bs[(4 * kk + t) * C::BS + 64 * wn + 8 * ni + g];
+            for (int ni = 0; ni < GNI; ++ni) b[ni] = Bs[(4 * kk + t) * C::BS + 8 * GNI * wn + 8 * ni + g];
 #pragma unroll
             for (int mi = 0; mi < 4; ++mi)
 #pragma unroll
-                for (int ni = 0; ni < 8; ++ni) dmma(acc[2 * (mi * 8 + ni)], acc[2 * (mi * 8 + ni) + 1], a[mi], b[ni]);
+                for (int ni = 0; ni < GNI; ++ni) dmma(acc[2 * (mi * GNI + ni)], acc[2 * (mi * GNI + ni) + 1], a[mi], b[ni]);
         }
         __syncthreads();
     }
@@ -316,16 +317,16 @@ __global__ void __launch_bounds__(GTHREADS, 2) k_wg_gemm_f64(const __grid_consta
         const int r = 32 * wm + 8 * mi + g;
         if (r >= nrows) continue;
         const long Rg = rbase + row0 + r;
-        EpiAux aux[8];
+        EpiAux aux[GNI];
 #pragma unroll
-        for (int ni = 0; ni < 8; ++ni) {
-            const int col = n0 + 64 * wn + 8 * ni + 2 * t;
+        for (int ni = 0; ni < GNI; ++ni) {
+            const int col = n0 + 8 * GNI * wn + 8 * ni + 2 * t;
             if (col < p.NTOT) aux[ni] = wg_epi_load<MODE>(p, net, Rg, col);
         }
 #pragma unroll
-        for (int ni = 0; ni < 8; ++ni) {
-            const int col = n0 + 64 * wn + 8 * ni + 2 * t;
-            if (col < p.NTOT) wg_epi_store<MODE>(p, Rg, col, acc[2 * (mi * 8 + ni)], acc[2 * (mi * 8 + ni) + 1], aux[ni]);
+        for (int ni = 0; ni < GNI; ++ni) {
+            const int col = n0 + 8 * GNI * wn + 8 * ni + 2 * t;
+            if (col < p.NTOT) wg_epi_store<MODE>(p, Rg, col, acc[2 * (mi * GNI + ni)], acc[2 * (mi * GNI + ni) + 1], aux[ni]);
         }
     }
 }
