@@ -8,7 +8,7 @@
 // rows of the mixed modes (the real rows of a (centre type, neighbour type) block, contiguous, plus one
 // representative per atom and block for its padded slots, weighted by their number) and the row tiles are those of the
 // tile table of wide.cu, so a tile never straddles two nets.
-//   FP64   ("double"): k_wg_gemm_f64, the FP64 tensor pipe (DMMA m8n8k4), 64 x 64 x 32 tiles staged with cp.async, three CTAs per SM;
+//   FP64   ("double"): k_wg_gemm_f64, the FP64 tensor pipe (DMMA m8n8k4), 64 x 64 x 16 tiles staged with cp.async, four CTAs per SM;
 //   MIX-32 (nets in single precision): k_wg_gemm_tf32, tcgen05.mma kind::tf32 with TMEM accumulators; every operand
 //          is split into a TF32 value and its TF32 remainder and each K step takes three products ("3xTF32": the product keeps
 //          21+ mantissa bits; the accumulators are fp32); the activations arrive by TMA tensor copies, the weights' operand
@@ -29,10 +29,10 @@
 namespace {
 
 constexpr int GR = 128;                     // rows per tile (= the tile table's, wide.cu)
-constexpr int GBM = 64, GBN = 64, GBK = 32;  // FP64 kernel: rows (half a tile of the table), columns, K step per CTA
-constexpr int GNI = GBN / 16, GCTAS = 3;     // 8-column fragments per warp; CTAs per SM
+constexpr int GBM = 64, GBN = 64, GBK = 16;  // FP64 kernel: rows (half a tile of the table), columns, K step per CTA
+constexpr int GNI = GBN / 16, GCTAS = 4;     // 8-column fragments per warp; CTAs per SM
 constexpr int GTHREADS = 128;               // four warps as 2 (rows) x 2 (columns)
-constexpr int GA_STRIDE = GBK + 4;          // A tile [64][36], B tile [32][68]: fragment loads hit distinct banks (per half warp)
+constexpr int GA_STRIDE = GBK + 4;          // A tile [64][20], B tile [16][68]: fragment loads hit distinct banks (per half warp)
 struct GemmCfg {                             // the FP64 kernel's tiles
     static constexpr int BS = GBN + 4;                                  // B tile [32][BS]
     static constexpr int A_TILE = GBM * GA_STRIDE, B_TILE = GBK * BS;
@@ -243,8 +243,8 @@ __device__ __forceinline__ void wg_epi_store(const GenArgs<double> &p, long Rg, 
 }
 
 // FP64: one 64 x 64 output tile per CTA (half a tile of the table), four warps as 2 (rows) x 2 (columns): warp tile 32 x 32 =
-// 4 x 4 DMMA m8n8k4 fragments; THREE CTAs per SM (168 registers x 128 threads, 72 KB of shared memory each), so that one CTA's
-// barriers, prologue and epilogue run under the others' DMMAs.  A and B stages of K = 32 arrive by cp.async (two buffers); rows
+// 4 x 4 DMMA m8n8k4 fragments; FOUR CTAs per SM (128 registers x 128 threads, 37 KB of shared memory each), so that one CTA's
+// barriers, prologue and epilogue run under the others' DMMAs.  A and B stages of K = 16 arrive by cp.async (two buffers); rows
 // past the end of the tile's block and columns past NTOT are zero-filled and never stored.
 template <int MODE>
 __global__ void __launch_bounds__(GTHREADS, GCTAS) k_wg_gemm_f64(const __grid_constant__ GenArgs<double> p) {
